@@ -1,0 +1,624 @@
+"""Pins for the fp64 oracle: closed forms, invariants,
+hand-derived Lagrangian dynamics and brute force, none of which call back into
+the oracle's own formulas.  CPU only."""
+from __future__ import annotations
+
+import dataclasses
+import math
+import os
+
+import numpy as np
+import pytest
+import scipy.linalg
+from scipy.spatial.transform import Rotation
+
+from helpers import GOLDEN, chain_spec, quat_axis, strip_apples
+from oracle import OracleWorld, philox4x32_10
+from workloads import Params, binary_tree_config1, config1_loads, config_params, stochastic_world
+
+G = float(np.float32(9.81))      # the fp32 value both implementations receive
+
+
+def _level_of(parent):
+    lv = np.zeros(len(parent), dtype=int)
+    for i in range(1, len(parent)):
+        lv[i] = lv[parent[i]] + 1
+    return lv
+
+
+# ---------------------------------------------------------------- P12 Philox
+def test_philox_known_answers():
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "philox4x32_10_kat.txt")) if l.strip() and l[0] != "#"]
+    assert len(rows) == 3
+    for r in rows:
+        v = [int(x, 16) for x in r]
+        out = philox4x32_10(v[0:4], v[4:6])
+        assert [int(x) for x in out] == v[6:10]
+
+
+def test_philox_bijection_and_uniformity():
+    # a counter-based generator is a bijection of the counter for a fixed key
+    key = [0x1234, 0x5678]
+    outs = {tuple(int(x) for x in philox4x32_10([i, 0, 0, 0], key)) for i in range(2000)}
+    assert len(outs) == 2000
+    u = np.array([philox4x32_10([i, 3, 1, 0], key)[0] >> 8 for i in range(4000)], dtype=np.float64) / 2 ** 24
+    assert abs(u.mean() - 0.5) < 0.02 and abs(u.var() - 1 / 12) < 0.01
+
+
+def test_randomize_draws_follow_reading_A23():
+    spec = binary_tree_config1()
+    P = config_params(2)
+    w = OracleWorld(spec, P, world_index=7)
+    seed = 0x0123456789ABCDEF
+    w.randomize(seed)
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    o = philox4x32_10([7, 0, 0, 0], key)
+
+    def uni(x, lo, hi):
+        u = np.float32(int(x) >> 8) * np.float32(2.0 ** -24)
+        # fmaf in fp32: a double product/sum of fp32 operands is exact before the single rounding
+        return np.float32(np.float64(u) * np.float64(np.float32(hi) - np.float32(lo)) + np.float64(np.float32(lo)))
+    mat = w.material()
+    assert mat["E"] == uni(o[0], *P.range_E)
+    assert mat["MOR"] == uni(o[1], *P.range_MOR)
+    assert mat["density"] == uni(o[2], *P.range_density)
+    for a in range(spec.n_apples):
+        oa = philox4x32_10([7, a, 1, 0], key)
+        assert np.float32(mat["detach"][a]) == uni(oa[0], *P.range_detach)
+        assert np.float32(mat["mass"][a]) == uni(oa[1], *P.range_apple_mass)
+    assert P.range_E[0] <= mat["E"] <= P.range_E[1]
+    # degenerate ranges keep the spec
+    w2 = OracleWorld(spec, config_params(1), world_index=7)
+    w2.randomize(seed)
+    m2 = w2.material()
+    assert m2["E"] == np.float32(8e9) and m2["MOR"] == np.float32(60e6) and m2["density"] == np.float32(800.0)
+    assert np.allclose(m2["detach"], 20.0) and np.allclose(m2["mass"], 0.2)
+
+
+# ---------------------------------------------------------------- P1 constants
+def test_config1_closed_form_constants():
+    spec = binary_tree_config1()
+    w = OracleWorld(spec, config_params(1))
+    d = w.derived()
+    lv = _level_of(spec.parent)
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "config1_closed_forms.txt")) if l.strip() and l[0] != "#"]
+    for r in rows:
+        level, K, Mmax, m = int(r[0]), float(r[1]), float(r[2]), float(r[3])
+        idx = np.nonzero(lv == level)[0]
+        assert idx.size == 2 ** level
+        # fp32 inputs (d, L) carry ~1e-7 relative error; the printed values carry 4-6 digits
+        assert np.all(np.abs(d["K"][idx] - K) <= 0.5 + 1e-5 * K)
+        assert np.all(np.abs(d["Mmax"][idx] - Mmax) <= 0.5)
+        assert np.all(np.abs(d["m"][idx] - m) <= 0.0005)
+    # r-form of Eq. 4 / Eq. 5 (the oracle uses the d-form, reading A31)
+    r = spec.diameter.astype(np.float64) / 2
+    L = spec.length.astype(np.float64)
+    assert np.allclose(d["K"], math.pi / 4 * 8e9 * r ** 4 / L, rtol=1e-12)
+    assert np.allclose(d["Mmax"], 60e6 * math.pi * r ** 3 / 4, rtol=1e-12)
+    # cylinder inertia about its centre (textbook)
+    assert np.allclose(d["Ixx"], d["m"] * (3 * r * r + L * L) / 12, rtol=1e-12)
+    assert np.allclose(d["Izz"], d["m"] * r * r / 2, rtol=1e-12)
+
+
+# ---------------------------------------------------------------- FK vs scipy
+def _numpy_fk(spec, q):
+    N = spec.n_links
+    R = [None] * N
+    p = np.zeros((N, 3))
+    for i in range(N):
+        qr = spec.rest_quat[i].astype(np.float64)
+        Q = Rotation.from_quat([qr[1], qr[2], qr[3], qr[0]])
+        rel = Q * Rotation.from_euler("XY", [q[2 * i], q[2 * i + 1]])  # intrinsic x then y
+        pa = spec.parent[i]
+        if pa < 0:
+            R[i] = rel
+        else:
+            R[i] = R[pa] * rel
+            p[i] = p[pa] + R[pa].apply([0, 0, float(spec.length[pa])])
+    return np.stack([r.as_matrix() for r in R]), p
+
+
+def test_fk_matches_scipy_rotations():
+    rng = np.random.default_rng(5)
+    spec = stochastic_world(rng, 40, 60, 4, depth_choices=(4,))
+    w = OracleWorld(spec, Params())
+    q = rng.uniform(-0.6, 0.6, size=2 * spec.n_links)
+    w.set_state(q=q)
+    R, p, a1, a2 = w.fk()
+    R2, p2 = _numpy_fk(spec, q)
+    assert np.abs(R - R2).max() < 1e-12
+    assert np.abs(p - p2).max() < 1e-12
+    # rest pose reproduces the skeleton: Eq. 3 -> tips chain up
+    w.set_state(q=np.zeros_like(q))
+    R0, p0, _, _ = w.fk()
+    for i in range(1, spec.n_links):
+        pa = spec.parent[i]
+        assert np.allclose(p0[i], p0[pa] + R0[pa] @ [0, 0, spec.length[pa]], atol=1e-13)
+
+
+# ---------------------------------------------------------------- P2 mass matrix
+def test_mass_matrix_single_link_closed_form():
+    L, d, rho = 1.0, 0.05, 800.0
+    spec = chain_spec(1, L, d, density=rho)
+    w = OracleWorld(spec, Params())
+    L, d = float(spec.length[0]), float(spec.diameter[0])          # the fp32 inputs both sides receive
+    m = rho * math.pi * (d / 2) ** 2 * L
+    J = m * L * L / 3 + m * (d / 2) ** 2 / 4
+    Izz = m * (d / 2) ** 2 / 2
+    assert abs(m - 1.5708) < 1e-4 and abs(J - 0.5238) < 1e-4   # SURVEY.md Appendix A values
+    for th1, th2 in [(0.0, 0.0), (0.3, 0.0), (0.0, 0.7), (-0.4, 1.1)]:
+        w.set_state(q=[th1, th2])
+        M = w.mass_matrix()
+        c, s = math.cos(th2), math.sin(th2)
+        assert np.allclose(M, np.diag([J * c * c + Izz * s * s, J]), rtol=1e-12, atol=1e-15)
+
+
+def test_mass_matrix_planar_double_pendulum():
+    # two rods hinged about parallel x axes: textbook double pendulum (distributed mass)
+    L, d, rho = 1.0, 0.04, 700.0
+    spec = chain_spec(2, L, d, density=rho)
+    w = OracleWorld(spec, Params())
+    l = float(spec.length[0])
+    r = float(spec.diameter[0]) / 2
+    m = rho * math.pi * r * r * l
+    Ij = m * l * l / 3 + m * r * r / 4       # rod about its own joint
+    lc = l / 2
+    for phi2 in (0.0, 0.5, -1.2):
+        w.set_state(q=[0.2, 0.0, phi2, 0.0])
+        M = w.mass_matrix()
+        M11 = Ij + Ij + m * l * l + 2 * m * l * lc * math.cos(phi2)
+        M12 = Ij + m * l * lc * math.cos(phi2)
+        assert abs(M[0, 0] - M11) < 1e-12 and abs(M[0, 2] - M12) < 1e-12 and abs(M[2, 2] - Ij) < 1e-12
+
+
+def test_mass_matrix_equals_kinetic_energy_from_fk_differences():
+    """1/2 qd^T M qd = sum 1/2 m |v_cm|^2 + 1/2 w^T I w with v_cm and w obtained by central
+    differences of the (separately pinned) FK output: ties RNEA columns to sum J^T I J."""
+    rng = np.random.default_rng(11)
+    spec = stochastic_world(rng, 20, 30, 2, depth_choices=(3, 4))
+    w = OracleWorld(spec, Params())
+    N = spec.n_links
+    q = rng.uniform(-0.5, 0.5, size=2 * N)
+    w.set_state(q=q)
+    M = w.mass_matrix()
+    assert np.abs(M - M.T).max() < 1e-12 * np.abs(M).max()
+    assert np.linalg.eigvalsh(M).min() > 0
+    dv = w.derived()
+    L = spec.length.astype(np.float64)
+    for trial in range(3):
+        qd = rng.normal(size=2 * N)
+        eps = 1e-6
+        Rp, pp = _numpy_fk(spec, q + eps * qd)
+        Rm, pm = _numpy_fk(spec, q - eps * qd)
+        R0, _ = _numpy_fk(spec, q)
+        T = 0.0
+        for i in range(N):
+            cp = pp[i] + Rp[i] @ [0, 0, L[i] / 2]
+            cm_ = pm[i] + Rm[i] @ [0, 0, L[i] / 2]
+            v = (cp - cm_) / (2 * eps)
+            Wm = (Rp[i] - Rm[i]) / (2 * eps) @ R0[i].T          # [w]x
+            wv = np.array([Wm[2, 1], Wm[0, 2], Wm[1, 0]])
+            wl = R0[i].T @ wv
+            T += 0.5 * dv["m"][i] * v @ v + 0.5 * (dv["Ixx"][i] * (wl[0] ** 2 + wl[1] ** 2) + dv["Izz"][i] * wl[2] ** 2)
+        assert abs(0.5 * qd @ M @ qd - T) < 1e-7 * T
+
+
+# ---------------------------------------------------------------- P3 gravity
+def test_gravity_torque_horizontal_rod():
+    L, d, rho = 1.0, 0.05, 800.0
+    spec = chain_spec(1, L, d, root_quat=quat_axis("x", -90.0), density=rho)   # +z of the link -> world +y
+    w = OracleWorld(spec, Params())
+    L, d = float(spec.length[0]), float(spec.diameter[0])
+    m = rho * math.pi * (d / 2) ** 2 * L
+    tau = w.rnea()
+    assert abs(abs(tau[0]) - m * G * L / 2) < 1e-12 * m * G * L and abs(tau[1]) < 1e-12
+    assert abs(m * G * L / 2 - 7.7048) < 1e-4
+
+
+# ---------------------------------------------------------------- P4 cantilever
+@pytest.mark.parametrize("n", [1, 2, 4, 8, 16, 32])
+def test_cantilever_tip_deflection(n):
+    """n-link horizontal cantilever, tip load P, no gravity, small load:
+    delta_n = (P L^3 / EI) (n+1)(2n+1)/(6 n^2)  ->  P L^3/(3EI) as n grows (north_star)."""
+    L, d, E, Pload = 1.0, 0.05, 8e9, 0.1
+    spec = chain_spec(n, L, d, root_quat=quat_axis("x", -90.0), E=E)
+    par = Params(h=50.0, gravity=(0.0, 0.0, 0.0), c_d=0.0, qd_max=0.0)
+    w = OracleWorld(spec, par)
+    w.apply_wrench(n - 1, (0, 0, float(spec.length[-1])), (0, 0, -Pload))
+    _, p0, _, _ = w.fk()
+    R0, _, _, _ = w.fk()
+    tip0 = p0[-1] + R0[-1] @ [0, 0, float(spec.length[-1])]
+    w.step(6)          # huge h: each step is a Newton step of the static problem
+    R, p, _, _ = w.fk()
+    tip = p[-1] + R[-1] @ [0, 0, float(spec.length[-1])]
+    EI = E * math.pi * float(spec.diameter[0]) ** 4 / 64
+    Ltot = float(spec.length.astype(np.float64).sum())
+    delta = Pload * Ltot ** 3 / EI * (n + 1) * (2 * n + 1) / (6 * n * n)
+    got = -(tip - tip0)[2]
+    assert abs(got / delta - 1) < 2e-6
+    ratio = got / (Pload * Ltot ** 3 / (3 * EI))
+    assert abs(ratio - (1 + 1.5 / n + 0.5 / n ** 2)) < 1e-5
+
+
+# ---------------------------------------------------------------- P5 linear dynamics
+def test_single_dof_step_map_closed_form():
+    L, d, rho, E = 0.6, 0.02, 800.0, 1e8
+    spec = chain_spec(1, L, d, density=rho, E=E)
+    h, c_d = 2e-3, 0.05
+    par = Params(h=h, gravity=(0, 0, 0), c_d=c_d, qd_max=0.0)
+    w = OracleWorld(spec, par)
+    hh, cd = float(np.float32(h)), float(np.float32(c_d))
+    r = float(spec.diameter[0]) / 2
+    Lf = float(spec.length[0])
+    m = rho * math.pi * r * r * Lf
+    J = m * Lf * Lf / 3 + m * r * r / 4
+    K = E * math.pi * (2 * r) ** 4 / (64 * Lf)
+    D = cd * K
+    q, v = 0.01, -0.3
+    w.set_state(q=[0.0, q], qd=[0.0, v])
+    for _ in range(50):
+        v = (J * v - hh * K * q) / (J + hh * D + hh * hh * K)
+        q = q + hh * v
+        w.step(1)
+        s = w.get_state()
+        assert abs(s["q"][1] - q) < 1e-13 and abs(s["qd"][1] - v) < 1e-11
+        assert s["q"][0] == 0.0 and s["qd"][0] == 0.0
+
+
+def test_small_oscillation_frequencies_match_generalized_eigenvalues():
+    """log-eigenvalues of the linearised step map / h -> sqrt(eig(K, M)) for D = 0, h -> 0 (north_star)."""
+    rng = np.random.default_rng(3)
+    spec = stochastic_world(rng, 6, 8, 0, depth_choices=(2,))
+    spec = dataclasses.replace(spec, E=2e6)
+    h = 1e-4
+    par = Params(h=h, gravity=(0, 0, 0), c_d=0.0, qd_max=0.0)
+    w = OracleWorld(spec, par)
+    n = 2 * spec.n_links
+    M = w.mass_matrix()
+    Kd = np.repeat(w.derived()["K"], 2)
+    lam = scipy.linalg.eigh(np.diag(Kd), M, eigvals_only=True)
+    omega_ref = np.sqrt(lam)
+    # linearise the step map by central differences about rest
+    eps = 1e-7
+    S = np.zeros((2 * n, 2 * n))
+    for j in range(2 * n):
+        cols = []
+        for sgn in (+1, -1):
+            x = np.zeros(2 * n)
+            x[j] = sgn * eps
+            w.set_state(q=x[:n], qd=x[n:])
+            w.step(1)
+            s = w.get_state()
+            cols.append(np.concatenate([s["q"], s["qd"]]))
+        S[:, j] = (cols[0] - cols[1]) / (2 * eps)
+    ev = np.linalg.eigvals(S)
+    assert np.abs(ev).max() < 1.0 + 1e-9          # never unstable
+    omega = np.sort(np.abs(np.log(ev).imag) / float(np.float32(h)))
+    omega = omega[::2]                             # conjugate pairs
+    assert np.allclose(omega, np.sort(omega_ref), rtol=2e-3)
+
+
+# ---------------------------------------------------------------- P16 Lagrangian brute force
+def test_single_link_two_dof_against_hand_derived_lagrangian():
+    """Universal joint + symmetric rod: T = 1/2 (J c2^2 + Izz s2^2) th1'^2 + 1/2 J th2'^2,
+    V = -m (L/2) g . R e_z with R e_z = (s2, -s1 c2, c1 c2); same linearly implicit scheme."""
+    L, d, rho, E = 0.8, 0.03, 800.0, 3e5
+    spec = chain_spec(1, L, d, density=rho, E=E, root_quat=quat_axis("y", 40.0))
+    h, c_d = 1e-3, 0.02
+    gvec = (0.3, -0.2, -9.81)
+    par = Params(h=h, gravity=gvec, c_d=c_d, qd_max=0.0)
+    w = OracleWorld(spec, par)
+    hh, cd = float(np.float32(h)), float(np.float32(c_d))
+    r = float(spec.diameter[0]) / 2
+    Lf = float(spec.length[0])
+    m = rho * math.pi * r * r * Lf
+    J = m * Lf * Lf / 3 + m * r * r / 4
+    Izz = m * r * r / 2
+    K = E * math.pi * (2 * r) ** 4 / (64 * Lf)
+    D = cd * K
+    qr = spec.rest_quat[0].astype(np.float64)
+    Q = Rotation.from_quat([qr[1], qr[2], qr[3], qr[0]]).as_matrix()
+    gl = Q.T @ np.array([float(np.float32(x)) for x in gvec])      # gravity in the joint's rest frame
+    q = np.array([0.3, -0.5])
+    v = np.array([1.0, 2.0])
+    w.set_state(q=q, qd=v)
+    for _ in range(300):
+        s1, c1, s2, c2 = math.sin(q[0]), math.cos(q[0]), math.sin(q[1]), math.cos(q[1])
+        M11 = J * c2 * c2 + Izz * s2 * s2
+        dM11 = 2 * (Izz - J) * s2 * c2
+        cor = np.array([dM11 * v[0] * v[1], -0.5 * dM11 * v[0] ** 2])
+        dV = -m * Lf / 2 * np.array([gl @ [0, -c1 * c2, -s1 * c2], gl @ [c2, s1 * s2, -c1 * s2]])
+        A = np.diag([M11, J]) + np.eye(2) * (hh * D + hh * hh * K)
+        b = hh * (-cor - dV - K * q - (D + hh * K) * v)
+        v = v + np.linalg.solve(A, b)
+        q = q + hh * v
+        w.step(1)
+    s = w.get_state()
+    assert np.abs(s["q"] - q).max() < 1e-10 and np.abs(s["qd"] - v).max() < 1e-9
+
+
+# ---------------------------------------------------------------- P6 / P7 energy, order
+def _soft_tree():
+    rng = np.random.default_rng(21)
+    spec = stochastic_world(rng, 14, 18, 0, depth_choices=(3,))
+    return dataclasses.replace(spec, E=3e6)
+
+
+def _energy_run(h, t_end=0.5):
+    spec = _soft_tree()
+    w = OracleWorld(spec, Params(h=h, c_d=0.0, qd_max=0.0))
+    T0, V0 = w.energy()
+    Es = [T0 + V0]
+    Tmax = 0.0
+    for _ in range(int(round(t_end / h))):
+        w.step(1)
+        T, V = w.energy()
+        Es.append(T + V)
+        Tmax = max(Tmax, T)
+    return np.array(Es), Tmax, w.get_state()
+
+
+def test_energy_drift_is_first_order_and_never_grows():
+    drift = []
+    for h in (1e-3, 5e-4, 2.5e-4):
+        Es, Tmax, _ = _energy_run(h)
+        assert Tmax > 0
+        rel = (Es - Es[0]) / Tmax
+        assert rel.max() < 1e-9             # never gains energy (implicit spring, D = 0)
+        drift.append(rel[-1])
+    assert drift[0] < 0 and abs(drift[0]) < 0.05          # small
+    assert 1.6 < drift[0] / drift[1] < 2.4 and 1.6 < drift[1] / drift[2] < 2.4
+
+
+def test_first_order_convergence_in_h():
+    _, _, ref = _energy_run(2.5e-5, t_end=0.1)
+    errs = []
+    for h in (4e-4, 2e-4, 1e-4):
+        _, _, s = _energy_run(h, t_end=0.1)
+        errs.append(np.linalg.norm(s["q"] - ref["q"]))
+    assert 1.6 < errs[0] / errs[1] < 2.5 and 1.6 < errs[1] / errs[2] < 2.7
+
+
+# ---------------------------------------------------------------- P8 rupture
+def test_rupture_fires_exactly_at_the_closed_form_moment():
+    L, d = 0.5, 0.02
+    big = np.full((1, 2), 1e9, dtype=np.float32)       # armature pins the joint in place
+    spec = chain_spec(1, L, d, armature=big)
+    Mmax = 60e6 * math.pi * float(spec.diameter[0]) ** 3 / 32
+    K = 8e9 * math.pi * float(spec.diameter[0]) ** 4 / (64 * float(spec.length[0]))
+    for nr in (1, 3, 5):
+        for factor, fires in ((1 + 1e-3, True), (1 - 1e-3, False)):
+            w = OracleWorld(spec, Params(gravity=(0, 0, 0), rupture_frames=nr))
+            th = factor * Mmax / K
+            w.set_state(q=[0.6 * th, 0.8 * th])
+            w.step(nr - 1) if nr > 1 else None
+            assert w.events() == []
+            w.step(4)
+            ev = w.events()
+            if fires:
+                assert len(ev) == 1 and ev[0][1] == nr - 1 and ev[0][2] == 0 and ev[0][3] == 0
+                assert abs(ev[0][4] / (factor * Mmax) - 1) < 1e-6 and abs(ev[0][5] / Mmax - 1) < 1e-12
+                assert w.get_state()["ruptured"][0] == 1
+            else:
+                assert ev == [] and w.get_state()["ruptured"][0] == 0
+
+
+def test_rupture_under_quasi_static_ramp():
+    """One horizontal link, N_r = 1, slow tip-load ramp: at the first event P L cos(theta) is within the
+    damper lag (c_d dP/dt L) of M_max = MOR pi d^3/32."""
+    L, d, E, MOR = 0.4, 0.01, 8e9, 60e6
+    spec = chain_spec(1, L, d, root_quat=quat_axis("x", -90.0), E=E, MOR=MOR)
+    h, c_d, nsteps = 2e-3, 0.05, 4000
+    Mmax = MOR * math.pi * float(spec.diameter[0]) ** 3 / 32
+    Lf = float(spec.length[0])
+    Pmax = 1.5 * Mmax / Lf
+    w = OracleWorld(spec, Params(h=h, c_d=c_d, gravity=(0, 0, 0), rupture_frames=1, qd_max=0.0))
+    ev = []
+    for s in range(nsteps):
+        w.apply_wrench(0, (0, 0, Lf), (0, 0, -Pmax * (s + 1) / nsteps))
+        w.step(1)
+        ev = w.events()
+        if ev:
+            break
+    assert ev and ev[0][2] == 0
+    s = ev[0][1]
+    th = np.linalg.norm(w.get_state()["q"])
+    P = Pmax * (s + 1) / nsteps
+    lag = c_d * (Pmax / (nsteps * h)) * Lf
+    assert abs(P * Lf * math.cos(th) - Mmax) < lag + 2 * Pmax / nsteps * Lf + 1e-3 * Mmax
+    assert ev[0][4] > ev[0][5] and ev[0][4] / ev[0][5] < 1.001
+
+
+def test_ruptured_joint_is_a_free_hinge():
+    L, d, rho = 0.5, 0.02, 800.0
+    spec = chain_spec(1, L, d, root_quat=quat_axis("x", -90.0), density=rho)
+    h = 1e-3
+    w = OracleWorld(spec, Params(h=h, qd_max=0.0))
+    w.set_state(ruptured=[1])
+    w.step(1)
+    r = float(spec.diameter[0]) / 2
+    Lf = float(spec.length[0])
+    m = rho * math.pi * r * r * Lf
+    J = m * Lf * Lf / 3 + m * r * r / 4
+    qd = w.get_state()["qd"]
+    assert abs(abs(qd[0]) - float(np.float32(h)) * (m * G * Lf / 2) / J) < 1e-12 and abs(qd[1]) < 1e-14
+
+
+# ---------------------------------------------------------------- P9 / P10 / P11 apples
+def test_config1_events_as_written_and_1b():
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "config1_events.txt")) if l.strip() and l[0] != "#"]
+    spec = binary_tree_config1()
+    for variant, fmax in (("1", 400.0), ("1b", 5000.0)):
+        for implicit in (1, 0):                                   # P11: explicit and implicit tether agree
+            P = dataclasses.replace(config_params(1), tether_implicit=implicit)
+            w = OracleWorld(spec, P)
+            for s in range(500):
+                for (_, body, pt, f) in config1_loads(spec, s, 500, 30.0, fmax):
+                    w.apply_wrench(body, pt, f)
+                w.step(1)
+            ev = w.events()
+            exp = [r for r in rows if r[0] == variant]
+            assert len(ev) == len(exp), (variant, implicit, ev)
+            for e, r in zip(ev, exp):
+                step, kind, index, value, thr = int(r[1]), int(r[2]), int(r[3]), float(r[4]), float(r[5])
+                assert e[2] == kind and e[3] == index
+                if kind == 1:
+                    assert e[1] == step and abs(e[4] - value) < 1e-5 and abs(e[5] - thr) < 1e-6
+                else:
+                    assert abs(e[1] - step) <= 2 and 1.0 < e[4] / e[5] < 1.01 and abs(e[5] - thr) < 0.1
+            assert w.get_state()["status"] == 0
+
+
+def test_detach_by_stem_tension_path():
+    """Slow vertical pull on a hanging apple: |f_s| = P + m g quasi-statically, path B fires when it has
+    exceeded kappa f_detach for N_B steps (reading A14)."""
+    mA, k, fdet = 0.2, 2e3, 20.0
+    spec = chain_spec(1, 0.5, 0.08, apples=[(0, (0, 0, 0.5), mA, k, fdet)])
+    P = Params(detach_frames_pull=10 ** 6, detach_frames_tension=10, zeta_s=1.0)
+    w = OracleWorld(spec, P)
+    nsteps = 6000
+    Pmax = 30.0
+    fired = None
+    for s in range(nsteps):
+        w.apply_wrench(1, (0, 0, 0), (0, 0, -Pmax * (s + 1) / nsteps))
+        w.step(1)
+        ev = w.events()
+        if ev:
+            fired = ev[0]
+            break
+    assert fired is not None and fired[2] == 1 and fired[3] == 0
+    thr = float(np.float32(1.1)) * fdet
+    assert abs(fired[5] - thr) < 1e-9
+    s10 = fired[1] - 9                                    # first step of the 10-step window
+    Pq = Pmax * (s10 + 1) / nsteps
+    # quasi-static balance on the apple: f_s = P + m g - c_s |v|, with v = (dP/dt)/k_s the ramp-following speed
+    c_s = 2.0 * 1.0 * math.sqrt(k * mA)
+    lag = c_s * (Pmax / (nsteps * 2e-3)) / k
+    assert abs((Pq + mA * G - lag) - thr) < 2 * Pmax / nsteps
+
+
+def test_apple_rest_sag_zero_reaction_and_identical_tree():
+    spec = binary_tree_config1()
+    P = config_params(1)
+    w = OracleWorld(spec, P)
+    s0 = w.get_state()
+    R, p, _, _ = w.fk()
+    for a in range(spec.n_apples):
+        b = spec.apple_link[a]
+        xh = p[b] + R[b] @ spec.apple_offset[a].astype(np.float64)
+        sag = xh - s0["apple_x"][a]
+        assert np.allclose(sag, [0, 0, float(spec.apple_mass[a]) * G / float(spec.apple_k[a])], atol=1e-9)
+    w0 = OracleWorld(strip_apples(spec), P)
+    A1, b1 = w.system()
+    A0, b0 = w0.system()
+    assert np.abs(b1 - b0).max() < 1e-9 * np.abs(b0).max()      # zero reaction at rest
+    w.step(100)
+    w0.step(100)
+    assert np.abs(w.get_state()["q"] - w0.get_state()["q"]).max() < 5e-6
+    assert w.events() == []
+
+
+def test_virtual_mass_identity():
+    """h^2 k_s J^T J (A15) equals the mass-matrix increment of a point mass h^2 k_s at the attach point:
+    checked with a heavy, short, thin extra link standing in for the point mass."""
+    spec = binary_tree_config1()
+    P = config_params(1)
+    w = OracleWorld(spec, P)
+    rng = np.random.default_rng(2)
+    q = rng.uniform(-0.2, 0.2, size=2 * spec.n_links)
+    w.set_state(q=q)
+    A1, _ = w.system()
+    w0 = OracleWorld(strip_apples(spec), P)
+    w0.set_state(q=q)
+    A0, _ = w0.system()
+    dA = A1 - A0
+    R, p, a1, a2 = w.fk()
+    hh = float(np.float32(P.h))
+    ref = np.zeros_like(dA)
+    for a in range(spec.n_apples):
+        b = int(spec.apple_link[a])
+        xh = p[b] + R[b] @ spec.apple_offset[a].astype(np.float64)
+        J = np.zeros((3, 2 * spec.n_links))
+        j = b
+        while j >= 0:
+            J[:, 2 * j] = np.cross(a1[j], xh - p[j])
+            J[:, 2 * j + 1] = np.cross(a2[j], xh - p[j])
+            j = int(spec.parent[j])
+        ref += hh * hh * float(spec.apple_k[a]) * J.T @ J
+    assert np.abs(dA - ref).max() < 1e-12 * np.abs(ref).max()
+    # and J is the true Jacobian of the hang point (finite differences of FK)
+    eps = 1e-6
+    b = int(spec.apple_link[0])
+    o = spec.apple_offset[0].astype(np.float64)
+    for j in (0, 1, 2 * b, 2 * b + 1):
+        dq = np.zeros_like(q)
+        dq[j] = eps
+        Rp, pp = _numpy_fk(spec, q + dq)
+        Rm, pm = _numpy_fk(spec, q - dq)
+        col = ((pp[b] + Rp[b] @ o) - (pm[b] + Rm[b] @ o)) / (2 * eps)
+        jj = b
+        Jc = np.zeros(3)
+        xh = p[b] + R[b] @ o
+        while jj >= 0:
+            if 2 * jj == j:
+                Jc = np.cross(a1[jj], xh - p[jj])
+            if 2 * jj + 1 == j:
+                Jc = np.cross(a2[jj], xh - p[jj])
+            jj = int(spec.parent[jj])
+        assert np.abs(col - Jc).max() < 1e-8
+
+
+# ---------------------------------------------------------------- P13 PCG vs Cholesky
+def test_fp64_pcg_equals_cholesky():
+    rng = np.random.default_rng(8)
+    spec = stochastic_world(rng, 60, 80, 6, depth_choices=(4, 5))
+    P = config_params(2)
+    a = OracleWorld(spec, P, solver=0)
+    b = OracleWorld(spec, P, solver=1)
+    b.set_solver(1, 1e-13, 5000)
+    for w in (a, b):
+        w.randomize(99)
+        w.apply_wrench(10, (0, 0, 0.01), (3.0, -2.0, 1.0))
+    a.step(20)
+    b.step(20)
+    sa, sb = a.get_state(), b.get_state()
+    assert np.abs(sa["q"] - sb["q"]).max() < 1e-10 and np.abs(sa["qd"] - sb["qd"]).max() < 1e-8
+    assert 0 < sb["last_iters"] < 200
+
+
+# ---------------------------------------------------------------- P14 symmetry
+def test_config1_c2_symmetry_under_gravity():
+    spec = binary_tree_config1()
+    w = OracleWorld(spec, config_params(1))
+    w.step(100)
+    q = w.get_state()["q"].reshape(-1, 2)
+    nrm = np.linalg.norm(q, axis=1)
+    for i, j in [(1, 2), (3, 5), (4, 6), (7, 11), (15, 23), (16, 24), (19, 27)]:
+        assert nrm[i] > 0 and abs(nrm[i] - nrm[j]) < 1e-9 * nrm[i]
+
+
+# ---------------------------------------------------------------- P15 restart after rupture
+def test_state_round_trip_reproduces_the_run_after_a_rupture():
+    spec = binary_tree_config1()
+    P = config_params(1)
+    a = OracleWorld(spec, P)
+    for s in range(460):
+        for (_, body, pt, f) in config1_loads(spec, s, 500, 30.0, 5000.0):
+            a.apply_wrench(body, pt, f)
+        a.step(1)
+    st = a.get_state()
+    assert st["ruptured"][4] == 1 and st["attached"][0] == 0
+    b = OracleWorld(spec, P)
+    b.set_state(st["q"], st["qd"], st["apple_x"], st["apple_v"], st["ruptured"], st["attached"])
+    for w in (a, b):
+        for (_, body, pt, f) in config1_loads(spec, 460, 500, 30.0, 5000.0):
+            w.apply_wrench(body, pt, f)
+        w.step(20)
+    sa, sb = a.get_state(), b.get_state()
+    assert np.abs(sa["q"] - sb["q"]).max() < 1e-12 and np.abs(sa["apple_x"] - sb["apple_x"]).max() < 1e-12
+    # forces on a snapped sub-tree are disabled (reading A10): the load on link 4 no longer matters
+    c = OracleWorld(spec, P)
+    c.set_state(st["q"], st["qd"], st["apple_x"], st["apple_v"], st["ruptured"], st["attached"])
+    c.apply_wrench(spec.n_links + 0, (0, 0, 0), config1_loads(spec, 460, 500, 30.0, 5000.0)[0][3])
+    c.step(20)
+    assert np.abs(c.get_state()["q"] - sb["q"]).max() < 1e-12
