@@ -1,0 +1,766 @@
+// ob_host.cu -- host runtime behind the C ABI of include/orchard.h: validation, level-order layout,
+// workspace carving, wrench staging, launches, state / event copy-out.  No physics here: every step of the
+// path runs in the kernels of ob_kernels.cu.
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "ob_internal.h"
+
+using namespace ob;
+
+namespace {
+
+constexpr size_t kAlign = 256;
+constexpr int kBlock = 256;
+constexpr int kMaxSmem = 227 * 1024 - 2048;   // per-CTA limit minus the kernel's static shared memory
+const char *kNullCtx = "null context";
+
+struct Pool {
+  size_t off = 0, bytes = 0;
+};
+
+struct HostWorld {
+  std::vector<int32_t> ext2int_link, int2ext_link, ext2int_apple, int2ext_apple;
+  std::vector<double> anchor;   // [3*A] caller order, filled after k_rest_pose
+};
+
+}  // namespace
+
+struct ob_ctx {
+  std::string err;
+  int n_worlds = 0;
+  cudaStream_t stream = nullptr;
+  DevCtx dev{};
+  std::vector<WorldDesc> desc;
+  std::vector<HostWorld> hw;
+  std::vector<WrenchSlots> wrench;       // host mirror (internal body indices)
+  int dirty_lo = 0, dirty_hi = -1;
+  WrenchSlots *staging[2] = {nullptr, nullptr};
+  cudaEvent_t staging_ev[2] = {nullptr, nullptr};
+  int staging_next = 0;
+  unsigned char *dev_base = nullptr;
+  int grid = 0, block = kBlock, smem = 0, launches = 0;
+  int max_Np = 0, max_Ap = 0;
+  size_t ev_cap = 0;
+  bool anchors_ready = false;
+};
+
+namespace {
+
+int fail(ob_ctx *c, int code, const char *fmt, ...) {
+  if (c) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof(buf), fmt, ap);
+    va_end(ap);
+    c->err = buf;
+  }
+  return code;
+}
+
+thread_local std::string g_err;   // errors raised before a context exists
+
+int fail0(int code, const char *msg) {
+  g_err = msg;
+  return code;
+}
+
+int validate(const ob_world_spec *specs, int n_worlds, const ob_params *P, std::string &why) {
+  char b[256];
+  if (!specs || !P || n_worlds < 1) { why = "null specs/params or n_worlds < 1"; return OB_E_ARG; }
+  if (!(P->h > 0.f) || !(P->cg_tol > 0.f) || P->cg_max_iter < 1 || P->rupture_frames < 1 || P->rupture_frames > 255 ||
+      P->detach_frames_pull < 1 || P->detach_frames_pull > 255 || P->detach_frames_tension < 1 ||
+      P->detach_frames_tension > 255 || !(P->react_max >= 0.f) || !(P->c_d >= 0.f) || P->precond < 0 || P->precond > 1 || P->cg_norm < 0 || P->cg_norm > 1) {
+    why = "ob_params out of range";
+    return OB_E_ARG;
+  }
+  for (int w = 0; w < n_worlds; w++) {
+    const ob_world_spec &s = specs[w];
+    if (s.n_links < 1 || s.n_links > 32767 || !s.parent || !s.length || !s.diameter || !s.rest_quat) {
+      snprintf(b, sizeof(b), "world %d: n_links out of range or null link arrays", w); why = b; return OB_E_ARG;
+    }
+    if (s.n_apples < 0 || s.n_apples > 1024 ||
+        (s.n_apples > 0 && (!s.apple_link || !s.apple_offset || !s.apple_mass || !s.apple_k || !s.apple_detach))) {
+      snprintf(b, sizeof(b), "world %d: n_apples out of range or null apple arrays", w); why = b; return OB_E_ARG;
+    }
+    if (!(s.density > 0.f) || !(s.E > 0.f) || !(s.MOR > 0.f)) {
+      snprintf(b, sizeof(b), "world %d: density/E/MOR must be positive", w); why = b; return OB_E_ARG;
+    }
+    for (int i = 0; i < s.n_links; i++) {
+      if ((i == 0 && s.parent[0] != -1) || (i > 0 && (s.parent[i] < 0 || s.parent[i] >= i))) {
+        snprintf(b, sizeof(b), "world %d: parent[%d] = %d is not topological", w, i, s.parent[i]); why = b; return OB_E_ARG;
+      }
+      if (!(s.length[i] > 0.f) || !(s.diameter[i] > 0.f) || !std::isfinite(s.length[i]) || !std::isfinite(s.diameter[i])) {
+        snprintf(b, sizeof(b), "world %d: link %d has non-positive length or diameter", w, i); why = b; return OB_E_ARG;
+      }
+      const float *q = s.rest_quat + 4 * i;
+      double n = std::sqrt((double)q[0] * q[0] + (double)q[1] * q[1] + (double)q[2] * q[2] + (double)q[3] * q[3]);
+      if (!(std::fabs(n - 1.0) <= 1e-3)) {
+        snprintf(b, sizeof(b), "world %d: rest_quat[%d] is not a unit quaternion", w, i); why = b; return OB_E_ARG;
+      }
+      if (s.armature && (!(s.armature[2 * i] >= 0.f) || !(s.armature[2 * i + 1] >= 0.f))) {
+        snprintf(b, sizeof(b), "world %d: negative armature on link %d", w, i); why = b; return OB_E_ARG;
+      }
+    }
+    for (int a = 0; a < s.n_apples; a++) {
+      if (s.apple_link[a] < 0 || s.apple_link[a] >= s.n_links || !(s.apple_mass[a] > 0.f) || !(s.apple_k[a] > 0.f) ||
+          !(s.apple_detach[a] >= 0.f) || (s.apple_c && !(s.apple_c[a] >= 0.f))) {
+        snprintf(b, sizeof(b), "world %d: apple %d has a bad link, mass, stiffness, damping or detach force", w, a);
+        why = b; return OB_E_ARG;
+      }
+    }
+  }
+  return OB_OK;
+}
+
+// level (BFS) order: parents before children, links of one level contiguous, children of one parent contiguous
+void bfs_order(const ob_world_spec &s, std::vector<int32_t> &int2ext, std::vector<int32_t> &level_off) {
+  const int N = s.n_links;
+  std::vector<std::vector<int32_t>> kids(N);
+  for (int i = 1; i < N; i++) kids[s.parent[i]].push_back(i);
+  int2ext.clear();
+  int2ext.reserve(N);
+  level_off.clear();
+  level_off.push_back(0);
+  int2ext.push_back(0);
+  size_t begin = 0;
+  while (begin < int2ext.size()) {
+    size_t end = int2ext.size();
+    level_off.push_back((int32_t)end);
+    for (size_t k = begin; k < end; k++)
+      for (int32_t ch : kids[int2ext[k]]) int2ext.push_back(ch);
+    begin = end;
+  }
+}
+
+struct Layout {
+  size_t total = 0;
+  Pool desc, order, link_blk, apple_blk, topo, quat, R0, Mmax, Lown, diam, arm, link_ext, apple_ext, apple_nom,
+      apple_c, anchor, level_off, info, wrench, events, ev_count, queue, pose7;
+  size_t sumNp = 0, sumAp = 0, sumLev = 0, ev_cap = 0;
+  int max_Np = 0, max_Ap = 0, max_smem = 0;
+  bool any_arm = false;
+};
+
+void take(Layout &L, Pool &p, size_t bytes) {
+  L.total = (L.total + kAlign - 1) / kAlign * kAlign;
+  p.off = L.total;
+  p.bytes = bytes;
+  L.total += bytes;
+}
+
+int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) {
+  size_t ev = 0;
+  for (int w = 0; w < n_worlds; w++) {
+    const ob_world_spec &s = specs[w];
+    std::vector<int32_t> i2e, lev;
+    bfs_order(s, i2e, lev);
+    const int Np = pad16(s.n_links), Ap = pad16(s.n_apples), nlev = (int)lev.size() - 1;
+    L.sumNp += Np; L.sumAp += Ap; L.sumLev += nlev + 1;
+    L.max_Np = std::max(L.max_Np, Np); L.max_Ap = std::max(L.max_Ap, Ap);
+    const int sm = step_smem_bytes(Np, Ap, nlev);
+    if (sm > kMaxSmem) {
+      char b[200];
+      snprintf(b, sizeof(b), "world %d (%d links, %d apples) needs %d B of shared memory, limit %d", w, s.n_links,
+               s.n_apples, sm, kMaxSmem);
+      why = b;
+      return OB_E_CAPACITY;
+    }
+    L.max_smem = std::max(L.max_smem, sm);
+    if (s.armature) L.any_arm = true;
+    ev += (size_t)s.n_links + s.n_apples;
+  }
+  L.ev_cap = std::max<size_t>(ev, 64);
+  take(L, L.desc, sizeof(WorldDesc) * n_worlds);
+  take(L, L.order, sizeof(int32_t) * n_worlds);
+  take(L, L.link_blk, (size_t)link_block_bytes(1) * L.sumNp);
+  take(L, L.apple_blk, (size_t)apple_block_bytes(1) * std::max<size_t>(L.sumAp, 16));
+  take(L, L.topo, sizeof(int4) * L.sumNp);
+  take(L, L.quat, sizeof(float4) * L.sumNp);
+  take(L, L.R0, sizeof(float) * 9 * L.sumNp);
+  take(L, L.Mmax, sizeof(float) * L.sumNp);
+  take(L, L.Lown, sizeof(float) * L.sumNp);
+  take(L, L.diam, sizeof(float) * L.sumNp);
+  take(L, L.arm, L.any_arm ? sizeof(float) * 2 * L.sumNp : 0);
+  take(L, L.link_ext, sizeof(int32_t) * L.sumNp);
+  take(L, L.apple_ext, sizeof(int32_t) * std::max<size_t>(L.sumAp, 16));
+  take(L, L.apple_nom, sizeof(float) * 2 * std::max<size_t>(L.sumAp, 16));
+  take(L, L.apple_c, sizeof(float) * std::max<size_t>(L.sumAp, 16));
+  take(L, L.anchor, sizeof(double) * 3 * std::max<size_t>(L.sumAp, 16));
+  take(L, L.level_off, sizeof(int32_t) * L.sumLev);
+  take(L, L.info, sizeof(WorldInfo) * n_worlds);
+  take(L, L.wrench, sizeof(WrenchSlots) * n_worlds);
+  take(L, L.events, sizeof(ob_event) * L.ev_cap);
+  take(L, L.ev_count, sizeof(int32_t) * 4);
+  take(L, L.queue, sizeof(int32_t) * 4);
+  take(L, L.pose7, sizeof(float) * 7 * L.max_Np);
+  L.total = (L.total + kAlign - 1) / kAlign * kAlign;
+  return OB_OK;
+}
+
+#define CU(call)                                                                                  \
+  do {                                                                                            \
+    cudaError_t e_ = (call);                                                                      \
+    if (e_ != cudaSuccess) return fail(ctx, OB_E_CUDA, "%s: %s", #call, cudaGetErrorString(e_));  \
+  } while (0)
+
+int flush_wrenches(ob_ctx *ctx) {
+  if (ctx->dirty_hi < ctx->dirty_lo) return OB_OK;
+  const int lo = ctx->dirty_lo, n = ctx->dirty_hi - ctx->dirty_lo + 1;
+  const int sidx = ctx->staging_next;
+  ctx->staging_next ^= 1;
+  CU(cudaEventSynchronize(ctx->staging_ev[sidx]));
+  std::memcpy(ctx->staging[sidx] + lo, ctx->wrench.data() + lo, sizeof(WrenchSlots) * n);
+  CU(cudaMemcpyAsync(const_cast<WrenchSlots *>(ctx->dev.wrench) + lo, ctx->staging[sidx] + lo, sizeof(WrenchSlots) * n,
+                     cudaMemcpyHostToDevice, ctx->stream));
+  CU(cudaEventRecord(ctx->staging_ev[sidx], ctx->stream));
+  ctx->dirty_lo = 0;
+  ctx->dirty_hi = -1;
+  return OB_OK;
+}
+
+int check_world(ob_ctx *ctx, int world) {
+  if (!ctx) return OB_E_ARG;
+  if (world < 0 || world >= ctx->n_worlds) return fail(ctx, OB_E_ARG, "world %d out of range", world);
+  return OB_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ob_default_params(ob_params *p) {
+  if (!p) return OB_E_ARG;
+  std::memset(p, 0, sizeof(*p));
+  p->h = 2e-3f;
+  p->gravity[0] = 0.f; p->gravity[1] = 0.f; p->gravity[2] = -9.81f;
+  p->c_d = 0.05f;
+  p->cg_tol = 1e-6f;
+  p->cg_max_iter = 200;
+  p->precond = 1;
+  p->rupture_frames = 3;
+  p->detach_frames_pull = 3;
+  p->detach_kappa = 1.1f;
+  p->detach_frames_tension = 10;
+  p->react_max = 40.f;
+  p->tether_implicit = 1;
+  p->qd_max = 50.f;
+  p->zeta_s = 0.1f;
+  p->forces_off_on_snapped = 1;
+  return OB_OK;
+}
+
+int ob_workspace_bytes(const ob_world_spec *specs, int n_worlds, const ob_params *params, size_t *out) {
+  std::string why;
+  if (!out) return fail0(OB_E_ARG, "out is null");
+  int rc = validate(specs, n_worlds, params, why);
+  if (rc != OB_OK) return fail0(rc, why.c_str());
+  Layout L;
+  rc = plan(specs, n_worlds, L, why);
+  if (rc != OB_OK) return fail0(rc, why.c_str());
+  *out = L.total;
+  return OB_OK;
+}
+
+int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params, void *dev_workspace,
+              size_t workspace_bytes, void *cuda_stream, ob_ctx **out) {
+  std::string why;
+  if (!out) return fail0(OB_E_ARG, "out is null");
+  *out = nullptr;
+  int rc = validate(specs, n_worlds, params, why);
+  if (rc != OB_OK) return fail0(rc, why.c_str());
+  Layout L;
+  rc = plan(specs, n_worlds, L, why);
+  if (rc != OB_OK) return fail0(rc, why.c_str());
+  if (!dev_workspace || workspace_bytes < L.total || ((uintptr_t)dev_workspace % kAlign) != 0)
+    return fail0(OB_E_WORKSPACE, "workspace null, misaligned (256 B) or smaller than ob_workspace_bytes");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail0(OB_E_CUDA, "no CUDA device: there is no CPU fallback");
+
+  ob_ctx *ctx = new ob_ctx();
+  ctx->n_worlds = n_worlds;
+  ctx->stream = (cudaStream_t)cuda_stream;
+  ctx->dev_base = (unsigned char *)dev_workspace;
+  ctx->max_Np = L.max_Np; ctx->max_Ap = L.max_Ap;
+  ctx->ev_cap = L.ev_cap;
+  ctx->desc.resize(n_worlds);
+  ctx->hw.resize(n_worlds);
+  ctx->wrench.assign(n_worlds, WrenchSlots{});
+  unsigned char *base = ctx->dev_base;
+
+  // ---- host images of every pool ----
+  std::vector<unsigned char> h_link(L.link_blk.bytes, 0), h_apple(L.apple_blk.bytes, 0);
+  std::vector<int4> h_topo(L.sumNp, make_int4(-1, 0, 0, 0));
+  std::vector<float4> h_quat(L.sumNp, make_float4(1.f, 0.f, 0.f, 0.f));
+  std::vector<float> h_Lown(L.sumNp, 1.f), h_diam(L.sumNp, 1.f), h_arm(L.any_arm ? 2 * L.sumNp : 0, 0.f);
+  std::vector<int32_t> h_link_ext(L.sumNp, 0), h_apple_ext(std::max<size_t>(L.sumAp, 16), 0), h_lev(L.sumLev, 0);
+  std::vector<float> h_nom(2 * std::max<size_t>(L.sumAp, 16), 0.f), h_c(std::max<size_t>(L.sumAp, 16), 0.f);
+  std::vector<int32_t> h_order(n_worlds);
+  size_t link_base = 0, apple_base = 0, lev_base = 0, link_off = 0, apple_off = 0;
+  for (int w = 0; w < n_worlds; w++) {
+    const ob_world_spec &s = specs[w];
+    HostWorld &H = ctx->hw[w];
+    std::vector<int32_t> lev;
+    bfs_order(s, H.int2ext_link, lev);
+    const int N = s.n_links, A = s.n_apples, Np = pad16(N), Ap = pad16(A), nlev = (int)lev.size() - 1;
+    H.ext2int_link.assign(N, 0);
+    for (int i = 0; i < N; i++) H.ext2int_link[H.int2ext_link[i]] = i;
+    // apples sorted by internal link (stable), so each link's apples are contiguous
+    H.int2ext_apple.resize(A);
+    for (int a = 0; a < A; a++) H.int2ext_apple[a] = a;
+    std::stable_sort(H.int2ext_apple.begin(), H.int2ext_apple.end(), [&](int32_t x, int32_t y) {
+      return H.ext2int_link[s.apple_link[x]] < H.ext2int_link[s.apple_link[y]];
+    });
+    H.ext2int_apple.assign(A, 0);
+    for (int a = 0; a < A; a++) H.ext2int_apple[H.int2ext_apple[a]] = a;
+
+    WorldDesc &d = ctx->desc[w];
+    d.N = N; d.A = A; d.Np = Np; d.Ap = Ap; d.n_levels = nlev;
+    d.link_base = (int32_t)link_base; d.apple_base = (int32_t)apple_base; d.level_base = (int32_t)lev_base;
+    d.link_blk_off = (int64_t)link_off; d.apple_blk_off = (int64_t)apple_off;
+    d.density = s.density; d.E = s.E; d.MOR = s.MOR;
+    d.has_apple_c = s.apple_c ? 1 : 0;
+
+    std::vector<int32_t> first_child(N, 0), n_child(N, 0), first_apple(N, 0), n_apple(N, 0);
+    for (int i = 1; i < N; i++) {
+      const int p = H.ext2int_link[s.parent[H.int2ext_link[i]]];
+      if (n_child[p] == 0) first_child[p] = i;
+      n_child[p]++;
+    }
+    for (int a = 0; a < A; a++) {
+      const int l = H.ext2int_link[s.apple_link[H.int2ext_apple[a]]];
+      if (n_apple[l] == 0) first_apple[l] = a;
+      n_apple[l]++;
+    }
+    float *lconst = reinterpret_cast<float *>(h_link.data() + link_off + link_state_bytes(Np));
+    for (int i = 0; i < N; i++) {
+      const int e = H.int2ext_link[i];
+      const int p = e == 0 ? -1 : H.ext2int_link[s.parent[e]];
+      h_topo[link_base + i] = make_int4(p, first_child[i], n_child[i] | (n_apple[i] << 16), first_apple[i]);
+      const float *q = s.rest_quat + 4 * e;
+      const double n = std::sqrt((double)q[0] * q[0] + (double)q[1] * q[1] + (double)q[2] * q[2] + (double)q[3] * q[3]);
+      h_quat[link_base + i] = make_float4((float)(q[0] / n), (float)(q[1] / n), (float)(q[2] / n), (float)(q[3] / n));
+      h_Lown[link_base + i] = s.length[e];
+      h_diam[link_base + i] = s.diameter[e];
+      h_link_ext[link_base + i] = e;
+      if (L.any_arm && s.armature) {
+        h_arm[2 * link_base + i] = s.armature[2 * e];
+        h_arm[2 * link_base + Np + i] = s.armature[2 * e + 1];
+      }
+      (void)lconst;
+    }
+    for (int l = 0; l <= nlev; l++) h_lev[lev_base + l] = lev[l];
+    unsigned char *ab = h_apple.data() + apple_off;
+    float *aconst = reinterpret_cast<float *>(ab + apple_state_bytes(Ap));
+    int32_t *alink = reinterpret_cast<int32_t *>(ab + apple_state_bytes(Ap) + 7 * 4 * Ap);
+    for (int a = 0; a < A; a++) {
+      const int e = H.int2ext_apple[a];
+      for (int k = 0; k < 3; k++) aconst[k * Ap + a] = s.apple_offset[3 * e + k];
+      aconst[3 * Ap + a] = s.apple_k[e];
+      aconst[4 * Ap + a] = s.apple_mass[e];
+      aconst[6 * Ap + a] = s.apple_detach[e];
+      alink[a] = H.ext2int_link[s.apple_link[e]];
+      h_apple_ext[apple_base + a] = e;
+      h_nom[2 * apple_base + a] = s.apple_mass[e];
+      h_nom[2 * apple_base + Ap + a] = s.apple_detach[e];
+      h_c[apple_base + a] = s.apple_c ? s.apple_c[e] : 0.f;
+    }
+    for (int a = A; a < Ap; a++) { aconst[3 * Ap + a] = 1.f; aconst[4 * Ap + a] = 1.f; alink[a] = 0; }
+    link_base += Np; apple_base += Ap; lev_base += nlev + 1;
+    link_off += link_block_bytes(Np); apple_off += apple_block_bytes(Ap);
+    h_order[w] = w;
+  }
+  // work-queue order: largest worlds first (longest-processing-time rule for heterogeneous batches)
+  std::stable_sort(h_order.begin(), h_order.end(), [&](int a, int b) { return ctx->desc[a].N > ctx->desc[b].N; });
+
+  DevCtx &D = ctx->dev;
+  D.n_worlds = n_worlds;
+  D.desc = reinterpret_cast<WorldDesc *>(base + L.desc.off);
+  D.order = reinterpret_cast<int32_t *>(base + L.order.off);
+  D.link_blk = base + L.link_blk.off;
+  D.apple_blk = base + L.apple_blk.off;
+  D.topo = reinterpret_cast<int4 *>(base + L.topo.off);
+  D.quat = reinterpret_cast<float4 *>(base + L.quat.off);
+  D.R0 = reinterpret_cast<float *>(base + L.R0.off);
+  D.Mmax = reinterpret_cast<float *>(base + L.Mmax.off);
+  D.Lown = reinterpret_cast<float *>(base + L.Lown.off);
+  D.diam = reinterpret_cast<float *>(base + L.diam.off);
+  D.arm = L.any_arm ? reinterpret_cast<float *>(base + L.arm.off) : nullptr;
+  D.link_ext = reinterpret_cast<int32_t *>(base + L.link_ext.off);
+  D.apple_ext = reinterpret_cast<int32_t *>(base + L.apple_ext.off);
+  D.apple_nominal = reinterpret_cast<float *>(base + L.apple_nom.off);
+  D.apple_c_in = reinterpret_cast<float *>(base + L.apple_c.off);
+  D.anchor = reinterpret_cast<double *>(base + L.anchor.off);
+  D.level_off = reinterpret_cast<int32_t *>(base + L.level_off.off);
+  D.info = reinterpret_cast<WorldInfo *>(base + L.info.off);
+  D.wrench = reinterpret_cast<WrenchSlots *>(base + L.wrench.off);
+  D.events = reinterpret_cast<ob_event *>(base + L.events.off);
+  D.ev_cap = (int32_t)std::min<size_t>(L.ev_cap, 0x7fffffff);
+  D.ev_count = reinterpret_cast<int32_t *>(base + L.ev_count.off);
+  D.queue = reinterpret_cast<int32_t *>(base + L.queue.off);
+  D.pose7 = reinterpret_cast<float *>(base + L.pose7.off);
+  D.P = *params;
+
+#define UP(pool, vec)                                                                                        \
+  do {                                                                                                       \
+    if ((pool).bytes && !(vec).empty()) {                                                                    \
+      cudaError_t e_ = cudaMemcpyAsync(base + (pool).off, (vec).data(),                                      \
+                                       std::min((pool).bytes, (vec).size() * sizeof((vec)[0])),              \
+                                       cudaMemcpyHostToDevice, ctx->stream);                                 \
+      if (e_ != cudaSuccess) { g_err = cudaGetErrorString(e_); delete ctx; return OB_E_CUDA; }               \
+    }                                                                                                        \
+  } while (0)
+  cudaError_t e = cudaMemsetAsync(base, 0, L.total, ctx->stream);
+  if (e != cudaSuccess) { g_err = cudaGetErrorString(e); delete ctx; return OB_E_CUDA; }
+  UP(L.desc, ctx->desc); UP(L.order, h_order); UP(L.link_blk, h_link); UP(L.apple_blk, h_apple); UP(L.topo, h_topo);
+  UP(L.quat, h_quat); UP(L.Lown, h_Lown); UP(L.diam, h_diam); UP(L.arm, h_arm); UP(L.link_ext, h_link_ext);
+  UP(L.apple_ext, h_apple_ext); UP(L.apple_nom, h_nom); UP(L.apple_c, h_c); UP(L.level_off, h_lev);
+#undef UP
+  e = cudaStreamSynchronize(ctx->stream);   // the host images die at the end of this call
+  if (e == cudaSuccess) e = launch_rest_pose(D, 0, 0, ctx->stream);
+  if (e == cudaSuccess) e = launch_randomize(D, 0ull, 0, ctx->stream);
+  // launch geometry of k_step
+  ctx->smem = L.max_smem;
+  int per_sm = 0, n_sm = 0, dev = 0;
+  if (e == cudaSuccess) e = step_kernel_setup(ctx->smem, ctx->block, &per_sm);
+  if (e == cudaSuccess) e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  if (e == cudaSuccess && per_sm < 1) e = cudaErrorInvalidConfiguration;
+  ctx->grid = std::max(1, std::min(n_worlds, n_sm * std::max(per_sm, 1)));
+  for (int k = 0; k < 2 && e == cudaSuccess; k++) {
+    e = cudaHostAlloc((void **)&ctx->staging[k], sizeof(WrenchSlots) * n_worlds, cudaHostAllocDefault);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->staging_ev[k], cudaEventDisableTiming);
+  }
+  // anchors come back once (rest geometry never changes)
+  std::vector<double> h_anchor(3 * std::max<size_t>(L.sumAp, 16));
+  if (e == cudaSuccess)
+    e = cudaMemcpyAsync(h_anchor.data(), D.anchor, sizeof(double) * h_anchor.size(), cudaMemcpyDeviceToHost, ctx->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+  if (e != cudaSuccess) {
+    g_err = std::string("ob_create: ") + cudaGetErrorString(e);
+    ob_destroy(ctx);
+    return OB_E_CUDA;
+  }
+  for (int w = 0; w < n_worlds; w++) {
+    const WorldDesc &d = ctx->desc[w];
+    HostWorld &H = ctx->hw[w];
+    H.anchor.resize(3 * (size_t)d.A);
+    for (int a = 0; a < d.A; a++)
+      for (int k = 0; k < 3; k++)
+        H.anchor[3 * H.int2ext_apple[a] + k] = h_anchor[3 * (size_t)d.apple_base + (size_t)k * d.Ap + a];
+  }
+  *out = ctx;
+  return OB_OK;
+}
+
+int ob_randomize(ob_ctx *ctx, uint64_t seed) {
+  if (!ctx) return OB_E_ARG;
+  for (auto &wv : ctx->wrench) wv = WrenchSlots{};
+  ctx->dirty_lo = 0;
+  ctx->dirty_hi = ctx->n_worlds - 1;
+  int rc = flush_wrenches(ctx);
+  if (rc != OB_OK) return rc;
+  CU(launch_randomize(ctx->dev, (unsigned long long)seed, 1, ctx->stream));
+  return OB_OK;
+}
+
+int ob_apply_wrench(ob_ctx *ctx, int world, int body, const float point[3], const float force[3]) {
+  int rc = check_world(ctx, world);
+  if (rc != OB_OK) return rc;
+  if (!force) return fail(ctx, OB_E_ARG, "force is null");
+  const WorldDesc &d = ctx->desc[world];
+  if (body < 0 || body >= d.N + d.A) return fail(ctx, OB_E_ARG, "world %d: body %d out of range", world, body);
+  const HostWorld &H = ctx->hw[world];
+  const int ib = body < d.N ? H.ext2int_link[body] : d.N + H.ext2int_apple[body - d.N];
+  WrenchSlots &W = ctx->wrench[world];
+  int slot = -1;
+  for (int k = 0; k < W.n; k++)
+    if (W.body[k] == ib) slot = k;
+  const bool zero = force[0] == 0.f && force[1] == 0.f && force[2] == 0.f;
+  if (zero) {
+    if (slot < 0) return OB_OK;
+    const int last = W.n - 1;    // keep the active slots dense
+    W.body[slot] = W.body[last];
+    for (int k = 0; k < 3; k++) { W.point[slot][k] = W.point[last][k]; W.force[slot][k] = W.force[last][k]; }
+    W.n = last;
+  } else {
+    if (slot < 0) {
+      if (W.n >= OB_MAX_WRENCH) return fail(ctx, OB_E_CAPACITY, "world %d: all %d wrench slots in use", world, OB_MAX_WRENCH);
+      slot = W.n++;
+    }
+    W.body[slot] = ib;
+    for (int k = 0; k < 3; k++) { W.point[slot][k] = point ? point[k] : 0.f; W.force[slot][k] = force[k]; }
+  }
+  if (ctx->dirty_hi < ctx->dirty_lo) { ctx->dirty_lo = world; ctx->dirty_hi = world; }
+  else { ctx->dirty_lo = std::min(ctx->dirty_lo, world); ctx->dirty_hi = std::max(ctx->dirty_hi, world); }
+  return OB_OK;
+}
+
+int ob_apply_wrench_batch(ob_ctx *ctx, int n, const int32_t *world, const int32_t *body, const float *point3,
+                          const float *force3) {
+  if (!ctx) return OB_E_ARG;
+  if (n < 0 || (n > 0 && (!world || !body || !force3))) return fail(ctx, OB_E_ARG, "null batch arrays");
+  for (int k = 0; k < n; k++) {
+    int rc = ob_apply_wrench(ctx, world[k], body[k], point3 ? point3 + 3 * k : nullptr, force3 + 3 * k);
+    if (rc != OB_OK) return rc;
+  }
+  return OB_OK;
+}
+
+int ob_step(ob_ctx *ctx, int n) {
+  if (!ctx) return OB_E_ARG;
+  if (n < 0) return fail(ctx, OB_E_ARG, "n < 0");
+  if (n == 0) return OB_OK;
+  int rc = flush_wrenches(ctx);
+  if (rc != OB_OK) return rc;
+  CU(cudaMemsetAsync(ctx->dev.queue, 0, sizeof(int32_t), ctx->stream));
+  CU(launch_step(ctx->dev, n, ctx->grid, ctx->block, ctx->smem, ctx->stream));
+  ctx->launches = 1;
+  return OB_OK;
+}
+
+int ob_get_state(ob_ctx *ctx, int world, float *q, float *qd, float *apple_x, float *apple_v, uint8_t *ruptured,
+                 uint8_t *attached, float *link_pose7, int32_t *info) {
+  int rc = check_world(ctx, world);
+  if (rc != OB_OK) return rc;
+  const WorldDesc &d = ctx->desc[world];
+  const HostWorld &H = ctx->hw[world];
+  std::vector<unsigned char> lb(link_state_bytes(d.Np)), ab(std::max(apple_state_bytes(d.Ap), 1));
+  std::vector<float> pose(link_pose7 ? 7 * (size_t)d.N : 0);
+  WorldInfo wi;
+  if (link_pose7) CU(launch_pose(ctx->dev, world, ctx->stream));
+  CU(cudaMemcpyAsync(lb.data(), ctx->dev.link_blk + d.link_blk_off, lb.size(), cudaMemcpyDeviceToHost, ctx->stream));
+  if (d.Ap)
+    CU(cudaMemcpyAsync(ab.data(), ctx->dev.apple_blk + d.apple_blk_off, apple_state_bytes(d.Ap), cudaMemcpyDeviceToHost,
+                       ctx->stream));
+  if (link_pose7)
+    CU(cudaMemcpyAsync(pose.data(), ctx->dev.pose7, sizeof(float) * pose.size(), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaMemcpyAsync(&wi, ctx->dev.info + world, sizeof(wi), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  const float *st = reinterpret_cast<const float *>(lb.data());
+  const unsigned char *fl = lb.data() + kLinkStateFloats * 4 * d.Np;
+  for (int i = 0; i < d.N; i++) {
+    const int e = H.int2ext_link[i];
+    if (q) { q[2 * e] = st[i]; q[2 * e + 1] = st[d.Np + i]; }
+    if (qd) { qd[2 * e] = st[2 * d.Np + i]; qd[2 * e + 1] = st[3 * d.Np + i]; }
+    if (ruptured) ruptured[e] = fl[i];
+    if (link_pose7) std::memcpy(link_pose7 + 7 * e, pose.data() + 7 * i, 7 * sizeof(float));
+  }
+  const float *as = reinterpret_cast<const float *>(ab.data());
+  const unsigned char *af = ab.data() + 6 * 4 * d.Ap;
+  for (int a = 0; a < d.A; a++) {
+    const int e = H.int2ext_apple[a];
+    for (int k = 0; k < 3; k++) {
+      if (apple_x) apple_x[3 * e + k] = (float)(H.anchor[3 * e + k] + (double)as[k * d.Ap + a]);
+      if (apple_v) apple_v[3 * e + k] = as[(3 + k) * d.Ap + a];
+    }
+    if (attached) attached[e] = af[a];
+  }
+  if (info) { info[0] = wi.step; info[1] = wi.last_iters; info[2] = wi.status; }
+  return OB_OK;
+}
+
+int ob_set_state(ob_ctx *ctx, int world, const float *q, const float *qd, const float *apple_x, const float *apple_v,
+                 const uint8_t *ruptured, const uint8_t *attached) {
+  int rc = check_world(ctx, world);
+  if (rc != OB_OK) return rc;
+  const WorldDesc &d = ctx->desc[world];
+  const HostWorld &H = ctx->hw[world];
+  std::vector<unsigned char> lb(link_state_bytes(d.Np)), ab(std::max(apple_state_bytes(d.Ap), 1));
+  WorldInfo wi;
+  CU(cudaMemcpyAsync(lb.data(), ctx->dev.link_blk + d.link_blk_off, lb.size(), cudaMemcpyDeviceToHost, ctx->stream));
+  if (d.Ap)
+    CU(cudaMemcpyAsync(ab.data(), ctx->dev.apple_blk + d.apple_blk_off, apple_state_bytes(d.Ap), cudaMemcpyDeviceToHost,
+                       ctx->stream));
+  CU(cudaMemcpyAsync(&wi, ctx->dev.info + world, sizeof(wi), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  float *st = reinterpret_cast<float *>(lb.data());
+  unsigned char *fl = lb.data() + kLinkStateFloats * 4 * d.Np;
+  for (int i = 0; i < d.N; i++) {
+    const int e = H.int2ext_link[i];
+    if (q) { st[i] = q[2 * e]; st[d.Np + i] = q[2 * e + 1]; }
+    if (qd) { st[2 * d.Np + i] = qd[2 * e]; st[3 * d.Np + i] = qd[2 * e + 1]; }
+    st[4 * d.Np + i] = 0.f; st[5 * d.Np + i] = 0.f;          // warm start cleared
+    if (ruptured) { fl[i] = ruptured[e] ? 1 : 0; fl[d.Np + i] = 0; }
+  }
+  float *as = reinterpret_cast<float *>(ab.data());
+  unsigned char *af = ab.data() + 6 * 4 * d.Ap;
+  for (int a = 0; a < d.A; a++) {
+    const int e = H.int2ext_apple[a];
+    for (int k = 0; k < 3; k++) {
+      if (apple_x) as[k * d.Ap + a] = (float)((double)apple_x[3 * e + k] - H.anchor[3 * e + k]);
+      if (apple_v) as[(3 + k) * d.Ap + a] = apple_v[3 * e + k];
+    }
+    if (attached) { af[a] = attached[e] ? 1 : 0; af[d.Ap + a] = 0; af[2 * d.Ap + a] = 0; }
+  }
+  wi.status = 0;
+  CU(cudaMemcpyAsync(ctx->dev.link_blk + d.link_blk_off, lb.data(), lb.size(), cudaMemcpyHostToDevice, ctx->stream));
+  if (d.Ap)
+    CU(cudaMemcpyAsync(ctx->dev.apple_blk + d.apple_blk_off, ab.data(), apple_state_bytes(d.Ap), cudaMemcpyHostToDevice,
+                       ctx->stream));
+  CU(cudaMemcpyAsync(ctx->dev.info + world, &wi, sizeof(wi), cudaMemcpyHostToDevice, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  return OB_OK;
+}
+
+int ob_get_apple_x64(ob_ctx *ctx, int world, double *apple_x) {
+  int rc = check_world(ctx, world);
+  if (rc != OB_OK) return rc;
+  if (!apple_x) return fail(ctx, OB_E_ARG, "apple_x is null");
+  const WorldDesc &d = ctx->desc[world];
+  const HostWorld &H = ctx->hw[world];
+  if (!d.A) return OB_OK;
+  std::vector<float> u(3 * (size_t)d.Ap);
+  CU(cudaMemcpyAsync(u.data(), ctx->dev.apple_blk + d.apple_blk_off, sizeof(float) * u.size(), cudaMemcpyDeviceToHost,
+                     ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  for (int a = 0; a < d.A; a++) {
+    const int e = H.int2ext_apple[a];
+    for (int k = 0; k < 3; k++) apple_x[3 * e + k] = H.anchor[3 * e + k] + (double)u[k * d.Ap + a];
+  }
+  return OB_OK;
+}
+
+int ob_get_counters(ob_ctx *ctx, int world, int32_t *rupture_count, int32_t *pull_count, int32_t *tension_count) {
+  int rc = check_world(ctx, world);
+  if (rc != OB_OK) return rc;
+  const WorldDesc &d = ctx->desc[world];
+  const HostWorld &H = ctx->hw[world];
+  std::vector<unsigned char> lf(2 * d.Np), af(std::max(3 * d.Ap, 1));
+  CU(cudaMemcpyAsync(lf.data(), ctx->dev.link_blk + d.link_blk_off + kLinkStateFloats * 4 * d.Np, lf.size(),
+                     cudaMemcpyDeviceToHost, ctx->stream));
+  if (d.Ap)
+    CU(cudaMemcpyAsync(af.data(), ctx->dev.apple_blk + d.apple_blk_off + 6 * 4 * d.Ap, 3 * d.Ap, cudaMemcpyDeviceToHost,
+                       ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  if (rupture_count)
+    for (int i = 0; i < d.N; i++) rupture_count[H.int2ext_link[i]] = lf[d.Np + i];
+  for (int a = 0; a < d.A; a++) {
+    if (pull_count) pull_count[H.int2ext_apple[a]] = af[d.Ap + a];
+    if (tension_count) tension_count[H.int2ext_apple[a]] = af[2 * d.Ap + a];
+  }
+  return OB_OK;
+}
+
+int ob_set_counters(ob_ctx *ctx, int world, const int32_t *rupture_count, const int32_t *pull_count,
+                    const int32_t *tension_count) {
+  int rc = check_world(ctx, world);
+  if (rc != OB_OK) return rc;
+  const WorldDesc &d = ctx->desc[world];
+  const HostWorld &H = ctx->hw[world];
+  std::vector<unsigned char> lf(2 * d.Np), af(std::max(3 * d.Ap, 1));
+  CU(cudaMemcpyAsync(lf.data(), ctx->dev.link_blk + d.link_blk_off + kLinkStateFloats * 4 * d.Np, lf.size(),
+                     cudaMemcpyDeviceToHost, ctx->stream));
+  if (d.Ap)
+    CU(cudaMemcpyAsync(af.data(), ctx->dev.apple_blk + d.apple_blk_off + 6 * 4 * d.Ap, 3 * d.Ap, cudaMemcpyDeviceToHost,
+                       ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  auto clampc = [](int32_t v) { return (unsigned char)std::min(std::max(v, 0), 255); };
+  if (rupture_count)
+    for (int i = 0; i < d.N; i++) lf[d.Np + i] = clampc(rupture_count[H.int2ext_link[i]]);
+  for (int a = 0; a < d.A; a++) {
+    if (pull_count) af[d.Ap + a] = clampc(pull_count[H.int2ext_apple[a]]);
+    if (tension_count) af[2 * d.Ap + a] = clampc(tension_count[H.int2ext_apple[a]]);
+  }
+  CU(cudaMemcpyAsync(ctx->dev.link_blk + d.link_blk_off + kLinkStateFloats * 4 * d.Np, lf.data(), lf.size(),
+                     cudaMemcpyHostToDevice, ctx->stream));
+  if (d.Ap)
+    CU(cudaMemcpyAsync(ctx->dev.apple_blk + d.apple_blk_off + 6 * 4 * d.Ap, af.data(), 3 * d.Ap, cudaMemcpyHostToDevice,
+                       ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  return OB_OK;
+}
+
+int ob_get_material(ob_ctx *ctx, int world, float *emr, float *apple_detach, float *apple_mass) {
+  int rc = check_world(ctx, world);
+  if (rc != OB_OK) return rc;
+  const WorldDesc &d = ctx->desc[world];
+  const HostWorld &H = ctx->hw[world];
+  WorldInfo wi;
+  std::vector<float> ac(std::max(7 * d.Ap, 1));
+  CU(cudaMemcpyAsync(&wi, ctx->dev.info + world, sizeof(wi), cudaMemcpyDeviceToHost, ctx->stream));
+  if (d.Ap)
+    CU(cudaMemcpyAsync(ac.data(), ctx->dev.apple_blk + d.apple_blk_off + apple_state_bytes(d.Ap), sizeof(float) * 7 * d.Ap,
+                       cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  if (emr) { emr[0] = wi.E; emr[1] = wi.MOR; emr[2] = wi.density; }
+  for (int a = 0; a < d.A; a++) {
+    if (apple_mass) apple_mass[H.int2ext_apple[a]] = ac[4 * d.Ap + a];
+    if (apple_detach) apple_detach[H.int2ext_apple[a]] = ac[6 * d.Ap + a];
+  }
+  return OB_OK;
+}
+
+int ob_events(ob_ctx *ctx, ob_event *buf, int cap, int *n_out) {
+  if (!ctx) return OB_E_ARG;
+  if (!n_out || cap < 0 || (cap > 0 && !buf)) return fail(ctx, OB_E_ARG, "null output");
+  int32_t cnt[2] = {0, 0};
+  CU(cudaMemcpyAsync(cnt, ctx->dev.ev_count, sizeof(cnt), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  const int have = (int)std::min<long long>(cnt[0], (long long)ctx->dev.ev_cap);
+  std::vector<ob_event> ev(have);
+  if (have) {
+    CU(cudaMemcpyAsync(ev.data(), ctx->dev.events, sizeof(ob_event) * have, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+  }
+  std::sort(ev.begin(), ev.end(), [](const ob_event &a, const ob_event &b) {
+    if (a.step != b.step) return a.step < b.step;
+    if (a.world != b.world) return a.world < b.world;
+    if (a.kind != b.kind) return a.kind < b.kind;
+    return a.index < b.index;
+  });
+  const int n = std::min(have, cap);
+  if (n) std::memcpy(buf, ev.data(), sizeof(ob_event) * n);
+  *n_out = n;
+  // keep what did not fit, in sorted order, at the head of the device list
+  const int rest = have - n;
+  if (rest) CU(cudaMemcpyAsync(ctx->dev.events, ev.data() + n, sizeof(ob_event) * rest, cudaMemcpyHostToDevice, ctx->stream));
+  int32_t newcnt[2] = {rest, 0};
+  CU(cudaMemcpyAsync(ctx->dev.ev_count, newcnt, sizeof(newcnt), cudaMemcpyHostToDevice, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  if (cnt[1] || cnt[0] > ctx->dev.ev_cap) return fail(ctx, OB_E_CAPACITY, "device event list overflowed (capacity %d)", ctx->dev.ev_cap);
+  return OB_OK;
+}
+
+int ob_stats(ob_ctx *ctx, uint64_t *cg_iters_total, uint64_t *world_steps_total, int32_t *n_flagged) {
+  if (!ctx) return OB_E_ARG;
+  std::vector<WorldInfo> wi(ctx->n_worlds);
+  CU(cudaMemcpyAsync(wi.data(), ctx->dev.info, sizeof(WorldInfo) * wi.size(), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  uint64_t it = 0, ws = 0;
+  int32_t fl = 0;
+  for (const WorldInfo &x : wi) { it += x.cg_iters; ws += (uint64_t)x.steps_taken; fl += x.status != 0; }
+  if (cg_iters_total) *cg_iters_total = it;
+  if (world_steps_total) *world_steps_total = ws;
+  if (n_flagged) *n_flagged = fl;
+  return OB_OK;
+}
+
+int ob_launch_info(ob_ctx *ctx, int32_t *n_launches, int32_t *grid, int32_t *block, int32_t *smem_bytes) {
+  if (!ctx) return OB_E_ARG;
+  if (n_launches) *n_launches = ctx->launches;
+  if (grid) *grid = ctx->grid;
+  if (block) *block = ctx->block;
+  if (smem_bytes) *smem_bytes = ctx->smem;
+  return OB_OK;
+}
+
+const char *ob_last_error(const ob_ctx *ctx) { return ctx ? ctx->err.c_str() : (g_err.empty() ? kNullCtx : g_err.c_str()); }
+
+void ob_destroy(ob_ctx *ctx) {
+  if (!ctx) return;
+  cudaStreamSynchronize(ctx->stream);
+  for (int k = 0; k < 2; k++) {
+    if (ctx->staging[k]) cudaFreeHost(ctx->staging[k]);
+    if (ctx->staging_ev[k]) cudaEventDestroy(ctx->staging_ev[k]);
+  }
+  delete ctx;
+}
+
+}  // extern "C"

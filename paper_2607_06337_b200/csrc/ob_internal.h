@@ -1,0 +1,113 @@
+// ob_internal.h -- device data layout shared by the host runtime (ob_host.cu) and the kernels
+// (ob_kernels.cu).  Nothing here is visible across the C ABI (include/orchard.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/orchard.h"
+
+namespace ob {
+
+constexpr int kPad = 16;  // links and apples per world are padded to a multiple of 16 (16-byte TMA granules)
+__host__ __device__ inline int pad16(int n) { return (n + kPad - 1) / kPad * kPad; }
+
+// ---- per-world "link block" in global memory: one contiguous chunk, staged to shared memory by one TMA
+//      bulk copy and written back (state part only) by one bulk store.
+//   floats  q0[Np] q1[Np] qd0[Np] qd1[Np] x0[Np] x1[Np]      state (x = previous dqd, the PCG warm start)
+//   bytes   ruptured[Np] rc[Np]                               state
+//   floats  K[Np] m[Np] mc[Np] Io[Np] Iz[Np] rz[Np]           constants (after ob_randomize)
+constexpr int kLinkStateFloats = 6;
+constexpr int kLinkConstFloats = 6;
+__host__ __device__ inline int link_state_bytes(int Np) { return kLinkStateFloats * 4 * Np + 2 * Np; }
+__host__ __device__ inline int link_block_bytes(int Np) { return link_state_bytes(Np) + kLinkConstFloats * 4 * Np; }
+
+// ---- per-world "apple block":
+//   floats  u[3][Ap] v[3][Ap]              state (u = x - anchor, anchor = rest hang point, fp64 on the host side)
+//   bytes   attached[Ap] cA[Ap] cB[Ap]     state
+//   floats  o[3][Ap] k[Ap] m[Ap] c[Ap] fdet[Ap]   constants
+//   int32   link[Ap]                       internal link index
+__host__ __device__ inline int apple_state_bytes(int Ap) { return 6 * 4 * Ap + 3 * Ap; }
+__host__ __device__ inline int apple_block_bytes(int Ap) { return apple_state_bytes(Ap) + 7 * 4 * Ap + 4 * Ap; }
+
+struct WorldDesc {
+  int32_t N, A, Np, Ap;
+  int32_t n_levels;
+  int32_t link_base;    // sum of Np of the worlds before this one
+  int32_t apple_base;   // sum of Ap
+  int32_t level_base;   // offset into the level-offset pool (n_levels + 1 entries)
+  int64_t link_blk_off;   // byte offset of the link block in the link-block pool
+  int64_t apple_blk_off;  // byte offset of the apple block in the apple-block pool
+  float density, E, MOR;  // nominal (spec) values
+  int32_t has_apple_c;
+};
+
+struct WorldInfo {       // mutable per-world scalars
+  int32_t step;
+  int32_t last_iters;
+  int32_t status;
+  int32_t steps_taken;           // world-steps actually advanced (frozen worlds do not count)
+  unsigned long long cg_iters;   // PCG iterations since ob_create
+  float E, MOR, density;         // current material draws
+  int32_t pad_;
+};
+
+struct WrenchSlots {     // device mirror of the persistent wrenches of one world (internal body indices)
+  int32_t n;
+  int32_t body[OB_MAX_WRENCH];
+  float point[OB_MAX_WRENCH][3];
+  float force[OB_MAX_WRENCH][3];
+  int32_t pad_[3];
+};
+static_assert(sizeof(WrenchSlots) % 16 == 0, "WrenchSlots must stay 16-byte sized");
+
+struct DevCtx {
+  int32_t n_worlds;
+  const WorldDesc *desc;
+  const int32_t *order;          // worlds sorted by size, largest first (work queue order)
+  unsigned char *link_blk;       // link-block pool
+  unsigned char *apple_blk;      // apple-block pool
+  // per-link statics, indexed link_base + i (SoA pools use k * Np + i inside the world's slice)
+  const int4 *topo;              // x = parent, y = first child, z = n_children | n_apples << 16, w = first apple
+  const float4 *quat;            // rest quaternion (w,x,y,z)
+  float *R0;                     // [9 * link_base + k * Np + i] rest world rotation, row-major k
+  float *Mmax;                   // rupture moment (after randomize)
+  const float *Lown;             // link length
+  const float *diam;             // link diameter
+  const float *arm;              // [2 * link_base + k * Np + i] armature or nullptr
+  const int32_t *link_ext;       // internal -> caller's link index
+  const int32_t *apple_ext;      // internal -> caller's apple index
+  const float *apple_nominal;    // [2 * apple_base + k * Ap + a]: nominal mass, detach force
+  const float *apple_c_in;       // [apple_base + a] caller's c_s or nullptr-equivalent (see has_apple_c)
+  double *anchor;                // [3 * apple_base + k * Ap + a] rest hang point, world frame, fp64
+  const int32_t *level_off;
+  WorldInfo *info;
+  const WrenchSlots *wrench;
+  ob_event *events;
+  int32_t ev_cap;
+  int32_t *ev_count;             // [0] = appended, [1] = overflow flag
+  int32_t *queue;                // work-queue counter
+  float *pose7;                  // scratch for ob_get_state(link_pose7): 7 * max Np floats
+  ob_params P;
+};
+
+// shared-memory footprint of one world in k_step (bytes); the host uses it to size the launch
+__host__ __device__ inline int step_smem_bytes(int Np, int Ap, int n_levels) {
+  int b = 0;
+  b += link_block_bytes(Np);
+  b += apple_block_bytes(Ap);
+  b += (9 + 2 + 6 + 24) * 4 * Np;   // E, (c2,s2), mailbox, scratch (aliases invd/r/p/Ap + 16)
+  b += Np;                          // snapped
+  b += (3 + 3 + 2) * 4 * Ap;        // f_tether, f_user, |f_s|, |f_user|
+  b += ((n_levels + 1 + 3) / 4 * 4) * 4;
+  b += (int)sizeof(WrenchSlots);
+  return (b + 127) / 128 * 128;
+}
+
+// kernel launchers (ob_kernels.cu)
+cudaError_t launch_rest_pose(const DevCtx &c, int total_links_padded, int total_apples_padded, cudaStream_t s);
+cudaError_t launch_randomize(const DevCtx &c, unsigned long long seed, int redraw, cudaStream_t s);
+cudaError_t launch_step(const DevCtx &c, int n_steps, int grid, int block, int smem, cudaStream_t s);
+cudaError_t launch_pose(const DevCtx &c, int world, cudaStream_t s);
+cudaError_t step_kernel_setup(int smem_bytes, int block, int *max_blocks_per_sm);
+
+}  // namespace ob

@@ -60,6 +60,7 @@ class Params:
     cg_tol: float = 1e-6
     cg_max_iter: int = 200
     precond: int = 1
+    cg_norm: int = 0
     rupture_frames: int = 3
     detach_frames_pull: int = 3
     detach_kappa: float = 1.1
