@@ -1,0 +1,383 @@
+#!/usr/bin/env python
+"""bench.py -- world-steps/s of the batched tree-physics step on BASELINE.json configs[3] (the headline config:
+4096 worlds x 350-450 links, 60 apples, h = 1 ms, one random wrench per world resampled every 50 steps).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--worlds 4096] [--config 4] [--substeps 50]
+  python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+  python bench.py --impl reference ...      # the fp64 CPU oracle, as it stands, on a bounded sample
+
+One bench "step" = one wrench epoch of the whole hot path for every world of the batch: the epoch's wrenches
+(ob_apply_wrench_batch) followed by `substeps` physics steps in one ob_step launch (FK, tether forces, bias,
+Jacobi diagonal, PCG, integration, rupture / detach predicates, event append).  `value` = world-steps/s with
+the inputs resident in HBM (wrench slots already uploaded, timed with CUDA events around the ob_step launches);
+`e2e` = the same through the C ABI with HOST buffers: wrench arrays in, events + per-world counters out, copies
+inside the timed region.  Prints ONE JSON line (rank 0).  DESIGN.md section "Measurement" explains every field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "world-steps/s at 4096 trees x ~400 links"
+UNIT = "world-steps/s"
+
+# Algorithmic work per link: flops of the formulas, not instructions executed.
+FLOP_LINK_STEP = 700.0        # FK + joint transforms + bias RNEA + composite-inertia diagonal + integration + predicates
+FLOP_LINK_ITER = 150.0        # one PCG iteration: M*v (two sweeps) + 5 vector updates + 2 dot products
+FLOP_APPLE_STEP = 120.0       # tether force, reaction, clamp, integration, detach predicates
+# Algorithmic HBM bytes per world-step if the state were streamed every step: 84 B per link,
+# 72 B per apple, 32 B of wrench.  With n steps fused per launch the traffic falls to 1/n of this.
+BYTES_LINK_STEP = 84.0
+BYTES_APPLE_STEP = 72.0
+BYTES_WRENCH = 32.0
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler(threading.Thread):
+    """SM clock and throttle reasons during the timed region (NVML; the recipe's nvidia-smi clocks line)."""
+
+    def __init__(self, index: int, period: float = 0.05):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop_ev = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake_slowdown",
+        }
+        while not self._stop_ev.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop_ev.wait(self.period)
+
+    def stop(self) -> dict:
+        self._stop_ev.set()
+        if self.is_alive():
+            self.join(timeout=2.0)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def _workload(config: int, n_worlds: int):
+    from workloads import config_params, make_config
+    base = make_config(config, min(n_worlds, 4096))
+    specs = [base[w % len(base)] for w in range(n_worlds)]     # 16384 = the 4096 geometries four times over;
+    return specs, config_params(config)                       # materials still differ per world (Philox by world)
+
+
+def _loads_arrays(specs, epoch, f_lo, f_hi):
+    from workloads import wrench_process
+    loads = wrench_process(specs, epoch, f_lo, f_hi)
+    return (np.array([l[0] for l in loads], np.int32), np.array([l[1] for l in loads], np.int32),
+            np.array([l[2] for l in loads], np.float32), np.array([l[3] for l in loads], np.float32))
+
+
+def run_cuda(args, rank: int, world_size: int):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2607_06337_b200 as ob
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the orchard step has no CPU fallback")
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world_size > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    peaks = _peaks()
+    specs, P = _workload(args.config, args.worlds)
+    f_lo, f_hi = (100.0, 600.0) if args.config == 5 else (0.0, 150.0)
+    W, S = len(specs), args.substeps
+    n_links = sum(s.n_links for s in specs)
+    n_apples = sum(s.n_apples for s in specs)
+    seed = 260706337 + 1000 * args.config + rank       # each rank is an independent replica of the batch
+    n_epochs = args.warmup + args.steps
+    epochs = [_loads_arrays(specs, e, f_lo, f_hi) for e in range(n_epochs)]
+
+    def barrier():
+        if world_size > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def run(e2e: bool):
+        sim = ob.Orchard(specs, P)
+        sim.randomize(seed)
+        stream = sim.stream
+        for e in range(args.warmup):
+            sim.apply_wrench_batch(*epochs[e])
+            sim.step(S)
+            if e2e:
+                sim.events(); sim.stats()
+        ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+        ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+        t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0, s0 = sim.counters(), sim.stats()
+        n_events = 0
+        sampler = ClockSampler(local)
+        barrier()
+        sampler.start()
+        t_begin.record(stream)
+        wall0 = time.perf_counter()
+        for k in range(args.steps):
+            if e2e:
+                sim.apply_wrench_batch(*epochs[args.warmup + k])      # host arrays -> pinned staging -> device
+                sim.step(S)
+                n_events += len(sim.events())                          # device -> host: event list
+                sim.stats()                                            # device -> host: per-world counters
+            else:
+                # kernel-resident leg: the epoch's wrenches are uploaded outside the per-launch events but
+                # inside the region (they are part of the workload); the launches are timed one by one
+                sim.apply_wrench_batch(*epochs[args.warmup + k])
+                sim.flush()
+                ev0[k].record(stream)
+                sim.step(S)
+                ev1[k].record(stream)
+        t_end.record(stream)
+        barrier()
+        wall = time.perf_counter() - wall0
+        clocks = sampler.stop()
+        region_ms = t_begin.elapsed_time(t_end)
+        kern_ms = None if e2e else [a.elapsed_time(b) for a, b in zip(ev0, ev1)]
+        c1, s1 = sim.counters(), sim.stats()
+        out = dict(region_ms=region_ms, wall_s=wall, kern_ms=kern_ms, clocks=clocks, n_events=n_events,
+                   world_steps=s1["world_steps_total"] - s0["world_steps_total"],
+                   cg_iters=s1["cg_iters_total"] - s0["cg_iters_total"], flagged=s1["n_flagged"],
+                   h2d=c1["h2d_bytes"] - c0["h2d_bytes"], d2h=c1["d2h_bytes"] - c0["d2h_bytes"],
+                   launches=c1["kernel_launches"] - c0["kernel_launches"], launch=sim.launch_info(),
+                   workspace=int(sim.workspace.numel()))
+        sim.close()
+        return out
+
+    dev = run(e2e=False)
+    e2e = run(e2e=True)
+
+    def max_over_ranks(x: float) -> float:
+        if world_size == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def sum_over_ranks(x: float) -> float:
+        if world_size == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+
+    kern_total_ms = max_over_ranks(sum(dev["kern_ms"]))
+    region_ms = max_over_ranks(dev["region_ms"])
+    e2e_ms = max_over_ranks(e2e["region_ms"])
+    ws_dev = sum_over_ranks(dev["world_steps"])
+    ws_e2e = sum_over_ranks(e2e["world_steps"])
+    iters_dev = sum_over_ranks(dev["cg_iters"])
+    value = ws_dev / (region_ms * 1e-3)
+    e2e_value = ws_e2e / (e2e_ms * 1e-3)
+
+    line = None
+    if rank == 0:
+        # roofline of the dominant (only) kernel, k_step: per-launch algorithmic work / average launch duration
+        k_ms = float(np.mean(dev["kern_ms"]))
+        iters_per_ws = dev["cg_iters"] / max(dev["world_steps"], 1)
+        ws_per_launch = dev["world_steps"] / args.steps
+        links_per_world, apples_per_world = n_links / W, n_apples / W
+        flop_ws = links_per_world * (FLOP_LINK_STEP + FLOP_LINK_ITER * iters_per_ws) + apples_per_world * FLOP_APPLE_STEP
+        flops_launch = flop_ws * ws_per_launch
+        sm_mhz = dev["clocks"]["sm_mhz"] or peaks["sm_max_mhz"]
+        alu_peak = 148 * 128 * 2 * sm_mhz * 1e6 / 1e12               # TFLOP/s at the clock seen during the run
+        alu_ach = flops_launch / (k_ms * 1e-3) / 1e12
+        bytes_ws = links_per_world * BYTES_LINK_STEP + apples_per_world * BYTES_APPLE_STEP + BYTES_WRENCH
+        hbm_stream = bytes_ws * ws_per_launch / (k_ms * 1e-3) / 1e9   # as if the state were streamed every step
+        hbm_fused = hbm_stream / S                                    # what one launch really has to move
+        traffic = None
+        tp = os.path.join(ROOT, "profiles", "k_step_traffic.json")
+        if os.path.exists(tp):
+            try:
+                traffic = json.load(open(tp)).get("dram_bytes_per_launch")
+            except Exception:
+                traffic = None
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world_size, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": region_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {W} worlds x "
+                                   f"{links_per_world:.0f} links (350-450), {apples_per_world:.0f} apples, h = {P.h * 1e3:g} ms, "
+                                   f"wrench U({f_lo:g},{f_hi:g}) N per world resampled every {S} steps",
+                       "worlds_per_gpu": W, "physics_steps_per_bench_step": S, "links_total": n_links,
+                       "apples_total": n_apples, "cg_tol": P.cg_tol, "replicas": world_size,
+                       "l2": f"inputs exceed L2: workspace {dev['workspace'] / 2**20:.0f} MiB vs 126 MB L2",
+                       "launch": dev["launch"]},
+            "kernel_only": {"value": ws_dev / (kern_total_ms * 1e-3), "unit": UNIT,
+                            "ms_per_step": kern_total_ms / args.steps},
+            "cg_iters_per_s": iters_dev / (region_ms * 1e-3),
+            "cg_iters_per_world_step": iters_per_ws,
+            "worlds_flagged": dev["flagged"],
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"] / args.steps,
+                    "d2h_bytes_per_step": e2e["d2h"] / args.steps, "ms_per_step": e2e_ms / args.steps,
+                    "events_read": e2e["n_events"]},
+            "gpu_launches": dev["launches"],
+            "clocks": dev["clocks"],
+            "roofline": {"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "TFLOP/s",
+                         "frac": alu_ach / alu_peak, "traffic": traffic, "kernel": "k_step",
+                         "kernel_ms": k_ms, "flop_per_world_step": flop_ws,
+                         "peak_source": f"148 SM x 128 fp32 lanes x 2 x {sm_mhz:.0f} MHz (clock sampled in the run)",
+                         "hbm": {"achieved_streamed": hbm_stream, "achieved_fused": hbm_fused,
+                                 "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac_streamed": hbm_stream / peaks["hbm_gbs"],
+                                 "frac_fused": hbm_fused / peaks["hbm_gbs"], "bytes_per_world_step": bytes_ws,
+                                 "peak_source": peaks["source"]}},
+        }
+        if world_size == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(specs, P, seed, f_lo, f_hi)
+    if world_size > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if line is not None:
+        print(json.dumps(line), flush=True)
+
+
+def _omp_threads() -> int:
+    try:
+        n = len(os.sched_getaffinity(0))
+    except Exception:
+        n = os.cpu_count() or 1
+    return max(1, n)
+
+
+def _oracle_sample(specs, P, seed, f_lo, f_hi, n_sample):
+    """Oracle worlds for the first n_sample worlds of the batch, randomized and loaded like the GPU run."""
+    import oracle
+    from workloads import wrench_process
+    loads = wrench_process(specs, 0, f_lo, f_hi)
+    worlds = []
+    for w in range(n_sample):
+        r = oracle.OracleWorld(specs[w], P, world_index=w)
+        r.randomize(seed)
+        r.apply_wrench(loads[w][1], loads[w][2], loads[w][3])
+        worlds.append(r)
+    return worlds
+
+
+def cpu_baseline(specs, P, seed, f_lo, f_hi) -> dict:
+    """The fp64 oracle as it stands (brute-force mass matrix + dense Cholesky, OpenMP over worlds), timed on this
+    box's host cores on a bounded sample of the same workload.  A reported baseline, not the target."""
+    import oracle
+    cores = _omp_threads()
+    os.environ.setdefault("OMP_NUM_THREADS", str(cores))
+    n_sample = int(min(max(cores, 8), 64, len(specs)))
+    n_steps = 4
+    worlds = _oracle_sample(specs, P, seed, f_lo, f_hi, n_sample)
+    oracle.step_many(worlds, 1)                                  # warm-up (page-in, first-touch)
+    t0 = time.perf_counter()
+    oracle.step_many(worlds, n_steps)
+    dt = time.perf_counter() - t0
+    return {"value": n_sample * n_steps / dt, "unit": UNIT, "cores": min(cores, n_sample), "kind": "oracle",
+            "sample": f"first {n_sample} worlds of the batch x {n_steps} steps after 1 warm-up step "
+                      f"(fp64, mass matrix by unit-acceleration RNEA columns, dense Cholesky), {dt:.2f} s wall"}
+
+
+def run_reference(args, rank: int, world_size: int):
+    """--impl reference: for this tier the reference arm is the oracle, timed as it stands on the host cores.
+    Each bench step is a bounded sample of the workload (n_sample worlds x 1 physics step)."""
+    if rank != 0:
+        return
+    cores = _omp_threads()
+    os.environ.setdefault("OMP_NUM_THREADS", str(cores))
+    import oracle
+    n_sample = int(min(max(cores, 8), 64))
+    from workloads import config_params, make_config
+    specs = make_config(args.config, n_sample)
+    P = config_params(args.config)
+    f_lo, f_hi = (100.0, 600.0) if args.config == 5 else (0.0, 150.0)
+    seed = 260706337 + 1000 * args.config
+    worlds = _oracle_sample(specs, P, seed, f_lo, f_hi, n_sample)
+    for _ in range(args.warmup):
+        oracle.step_many(worlds, 1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.step_many(worlds, 1)
+    dt = time.perf_counter() - t0
+    value = n_sample * args.steps / dt
+    links = sum(s.n_links for s in specs) / n_sample
+    sample = (f"{n_sample} worlds of configs[{args.config - 1}] ({links:.0f} links, {specs[0].n_apples} apples each) x 1 "
+              f"physics step per bench step")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[{args.config - 1}], bounded sample: {sample}",
+                       "physics_steps_per_bench_step": 1, "worlds": n_sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": min(cores, n_sample), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="1-based index into BASELINE.json configs (3, 4 or 5)")
+    ap.add_argument("--worlds", type=int, default=4096)
+    ap.add_argument("--substeps", type=int, default=50, help="physics steps per bench step (one wrench epoch)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "cuda":
+        args.warmup = 3                                    # timing rule: at least 3 warm-up steps
+    rank = int(os.environ.get("RANK", "0"))
+    world_size = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank, world_size)
+    else:
+        run_cuda(args, rank, world_size)
+
+
+if __name__ == "__main__":
+    main()

@@ -131,6 +131,9 @@ int ob_apply_wrench(ob_ctx *ctx, int world, int body, const float point[3], cons
 int ob_apply_wrench_batch(ob_ctx *ctx, int n, const int32_t *world, const int32_t *body, const float *point3,
                           const float *force3);
 
+/* Upload wrenches applied since the last ob_step / ob_flush now (asynchronous; ob_step does it implicitly). */
+int ob_flush(ob_ctx *ctx);
+
 /* Advance every world by n steps (one persistent kernel launch per size class; worlds stay on chip for the
    n steps).  Asynchronous.  Events are appended to the device event list. */
 int ob_step(ob_ctx *ctx, int n);
@@ -164,6 +167,15 @@ int ob_stats(ob_ctx *ctx, uint64_t *cg_iters_total, uint64_t *world_steps_total,
 
 /* Launch geometry of the last ob_step (for reporting): kernel launches, CTAs, threads per CTA, dynamic smem. */
 int ob_launch_info(ob_ctx *ctx, int32_t *n_launches, int32_t *grid, int32_t *block, int32_t *smem_bytes);
+
+/* Cumulative counters since ob_create: out[0] = bytes the library copied host -> device, out[1] = device -> host,
+   out[2] = kernels it launched, out[3] = ob_step calls.  Host-side bookkeeping; does not synchronise. */
+int ob_counters(ob_ctx *ctx, uint64_t out[4]);
+
+/* sizeof of the three ABI structs as the library was compiled (bindings check their own layout against these). */
+int ob_sizeof_params(void);
+int ob_sizeof_world_spec(void);
+int ob_sizeof_event(void);
 
 const char *ob_last_error(const ob_ctx *ctx);
 void ob_destroy(ob_ctx *ctx);

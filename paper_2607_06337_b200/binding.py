@@ -21,6 +21,7 @@ EXPORTS = [
     "ob_default_params", "ob_workspace_bytes", "ob_create", "ob_randomize", "ob_apply_wrench",
     "ob_apply_wrench_batch", "ob_step", "ob_get_state", "ob_set_state", "ob_get_apple_x64", "ob_get_counters", "ob_set_counters",
     "ob_get_material", "ob_events", "ob_stats", "ob_launch_info", "ob_last_error", "ob_destroy",
+    "ob_sizeof_params", "ob_sizeof_world_spec", "ob_sizeof_event", "ob_counters", "ob_flush",
 ]
 
 
@@ -71,6 +72,7 @@ def load_library():
         L.ob_apply_wrench.argtypes = [vp, i32, i32, vp, vp]
         L.ob_apply_wrench_batch.argtypes = [vp, i32, vp, vp, vp, vp]
         L.ob_step.argtypes = [vp, i32]
+        L.ob_flush.argtypes = [vp]
         L.ob_get_state.argtypes = [vp, i32] + [vp] * 8
         L.ob_set_state.argtypes = [vp, i32] + [vp] * 6
         L.ob_get_apple_x64.argtypes = [vp, i32, vp]
@@ -80,13 +82,19 @@ def load_library():
         L.ob_events.argtypes = [vp, vp, i32, C.POINTER(C.c_int)]
         L.ob_stats.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_int32)]
         L.ob_launch_info.argtypes = [vp] + [C.POINTER(C.c_int32)] * 4
+        L.ob_counters.argtypes = [vp, C.POINTER(C.c_uint64 * 4)]
         L.ob_last_error.argtypes = [vp]
         L.ob_last_error.restype = C.c_char_p
         L.ob_destroy.argtypes = [vp]
         L.ob_destroy.restype = None
+        for name in ("ob_sizeof_params", "ob_sizeof_world_spec", "ob_sizeof_event"):
+            getattr(L, name).argtypes = []
         for name in EXPORTS:
             if name not in ("ob_last_error", "ob_destroy"):
                 getattr(L, name).restype = C.c_int
+        if (L.ob_sizeof_params(), L.ob_sizeof_world_spec(), L.ob_sizeof_event()) != (
+                C.sizeof(ob_params), C.sizeof(ob_world_spec), C.sizeof(ob_event)):
+            raise RuntimeError("libob.so was built from a different include/orchard.h than this binding")
         _lib = L
     return _lib
 
@@ -211,6 +219,9 @@ class Orchard:
         w, b, p, f = _i32(world), _i32(body), _f32(point3), _f32(force3)
         self._check(self._L.ob_apply_wrench_batch(self._h, int(w.shape[0]), _ptr(w), _ptr(b), _ptr(p), _ptr(f)))
 
+    def flush(self):
+        self._check(self._L.ob_flush(self._h))
+
     def step(self, n: int = 1):
         self._check(self._L.ob_step(self._h, n))
 
@@ -273,6 +284,11 @@ class Orchard:
         it, ws, fl = C.c_uint64(0), C.c_uint64(0), C.c_int32(0)
         self._check(self._L.ob_stats(self._h, C.byref(it), C.byref(ws), C.byref(fl)))
         return dict(cg_iters_total=int(it.value), world_steps_total=int(ws.value), n_flagged=int(fl.value))
+
+    def counters(self) -> dict:
+        v = (C.c_uint64 * 4)()
+        self._check(self._L.ob_counters(self._h, C.byref(v)))
+        return dict(h2d_bytes=int(v[0]), d2h_bytes=int(v[1]), kernel_launches=int(v[2]), step_calls=int(v[3]))
 
     def launch_info(self) -> dict:
         v = [C.c_int32(0) for _ in range(4)]

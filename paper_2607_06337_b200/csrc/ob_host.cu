@@ -47,7 +47,7 @@ struct ob_ctx {
   int grid = 0, block = kBlock, smem = 0, launches = 0;
   int max_Np = 0, max_Ap = 0;
   size_t ev_cap = 0;
-  bool anchors_ready = false;
+  uint64_t h2d_bytes = 0, d2h_bytes = 0, kernel_launches = 0, step_calls = 0;
 };
 
 namespace {
@@ -65,6 +65,13 @@ int fail(ob_ctx *c, int code, const char *fmt, ...) {
 }
 
 thread_local std::string g_err;   // errors raised before a context exists
+
+// every copy the library issues goes through here, so ob_counters can report the bytes moved
+cudaError_t cpy(ob_ctx *c, void *dst, const void *src, size_t n, cudaMemcpyKind kind, cudaStream_t s) {
+  if (kind == cudaMemcpyHostToDevice) c->h2d_bytes += n;
+  else if (kind == cudaMemcpyDeviceToHost) c->d2h_bytes += n;
+  return cudaMemcpyAsync(dst, src, n, kind, s);
+}
 
 int fail0(int code, const char *msg) {
   g_err = msg;
@@ -141,7 +148,7 @@ void bfs_order(const ob_world_spec &s, std::vector<int32_t> &int2ext, std::vecto
 
 struct Layout {
   size_t total = 0;
-  Pool desc, order, link_blk, apple_blk, topo, quat, R0, Mmax, Lown, diam, arm, link_ext, apple_ext, apple_nom,
+  Pool desc, order, link_blk, apple_blk, topo, quat, quat_raw, R0, Mmax, Lown, diam, arm, link_ext, apple_ext, apple_nom,
       apple_c, anchor, level_off, info, wrench, events, ev_count, queue, pose7;
   size_t sumNp = 0, sumAp = 0, sumLev = 0, ev_cap = 0;
   int max_Np = 0, max_Ap = 0, max_smem = 0;
@@ -183,6 +190,7 @@ int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) 
   take(L, L.apple_blk, (size_t)apple_block_bytes(1) * std::max<size_t>(L.sumAp, 16));
   take(L, L.topo, sizeof(int4) * L.sumNp);
   take(L, L.quat, sizeof(float4) * L.sumNp);
+  take(L, L.quat_raw, sizeof(float4) * L.sumNp);
   take(L, L.R0, sizeof(float) * 9 * L.sumNp);
   take(L, L.Mmax, sizeof(float) * L.sumNp);
   take(L, L.Lown, sizeof(float) * L.sumNp);
@@ -217,7 +225,7 @@ int flush_wrenches(ob_ctx *ctx) {
   ctx->staging_next ^= 1;
   CU(cudaEventSynchronize(ctx->staging_ev[sidx]));
   std::memcpy(ctx->staging[sidx] + lo, ctx->wrench.data() + lo, sizeof(WrenchSlots) * n);
-  CU(cudaMemcpyAsync(const_cast<WrenchSlots *>(ctx->dev.wrench) + lo, ctx->staging[sidx] + lo, sizeof(WrenchSlots) * n,
+  CU(cpy(ctx, const_cast<WrenchSlots *>(ctx->dev.wrench) + lo, ctx->staging[sidx] + lo, sizeof(WrenchSlots) * n,
                      cudaMemcpyHostToDevice, ctx->stream));
   CU(cudaEventRecord(ctx->staging_ev[sidx], ctx->stream));
   ctx->dirty_lo = 0;
@@ -297,7 +305,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   // ---- host images of every pool ----
   std::vector<unsigned char> h_link(L.link_blk.bytes, 0), h_apple(L.apple_blk.bytes, 0);
   std::vector<int4> h_topo(L.sumNp, make_int4(-1, 0, 0, 0));
-  std::vector<float4> h_quat(L.sumNp, make_float4(1.f, 0.f, 0.f, 0.f));
+  std::vector<float4> h_quat(L.sumNp, make_float4(1.f, 0.f, 0.f, 0.f)), h_quat_raw(L.sumNp, make_float4(1.f, 0.f, 0.f, 0.f));
   std::vector<float> h_Lown(L.sumNp, 1.f), h_diam(L.sumNp, 1.f), h_arm(L.any_arm ? 2 * L.sumNp : 0, 0.f);
   std::vector<int32_t> h_link_ext(L.sumNp, 0), h_apple_ext(std::max<size_t>(L.sumAp, 16), 0), h_lev(L.sumLev, 0);
   std::vector<float> h_nom(2 * std::max<size_t>(L.sumAp, 16), 0.f), h_c(std::max<size_t>(L.sumAp, 16), 0.f);
@@ -346,6 +354,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
       const float *q = s.rest_quat + 4 * e;
       const double n = std::sqrt((double)q[0] * q[0] + (double)q[1] * q[1] + (double)q[2] * q[2] + (double)q[3] * q[3]);
       h_quat[link_base + i] = make_float4((float)(q[0] / n), (float)(q[1] / n), (float)(q[2] / n), (float)(q[3] / n));
+      h_quat_raw[link_base + i] = make_float4(q[0], q[1], q[2], q[3]);
       h_Lown[link_base + i] = s.length[e];
       h_diam[link_base + i] = s.diameter[e];
       h_link_ext[link_base + i] = e;
@@ -387,6 +396,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   D.apple_blk = base + L.apple_blk.off;
   D.topo = reinterpret_cast<int4 *>(base + L.topo.off);
   D.quat = reinterpret_cast<float4 *>(base + L.quat.off);
+  D.quat_raw = reinterpret_cast<float4 *>(base + L.quat_raw.off);
   D.R0 = reinterpret_cast<float *>(base + L.R0.off);
   D.Mmax = reinterpret_cast<float *>(base + L.Mmax.off);
   D.Lown = reinterpret_cast<float *>(base + L.Lown.off);
@@ -410,7 +420,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
 #define UP(pool, vec)                                                                                        \
   do {                                                                                                       \
     if ((pool).bytes && !(vec).empty()) {                                                                    \
-      cudaError_t e_ = cudaMemcpyAsync(base + (pool).off, (vec).data(),                                      \
+      cudaError_t e_ = cpy(ctx, base + (pool).off, (vec).data(),                                      \
                                        std::min((pool).bytes, (vec).size() * sizeof((vec)[0])),              \
                                        cudaMemcpyHostToDevice, ctx->stream);                                 \
       if (e_ != cudaSuccess) { g_err = cudaGetErrorString(e_); delete ctx; return OB_E_CUDA; }               \
@@ -419,12 +429,13 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   cudaError_t e = cudaMemsetAsync(base, 0, L.total, ctx->stream);
   if (e != cudaSuccess) { g_err = cudaGetErrorString(e); delete ctx; return OB_E_CUDA; }
   UP(L.desc, ctx->desc); UP(L.order, h_order); UP(L.link_blk, h_link); UP(L.apple_blk, h_apple); UP(L.topo, h_topo);
-  UP(L.quat, h_quat); UP(L.Lown, h_Lown); UP(L.diam, h_diam); UP(L.arm, h_arm); UP(L.link_ext, h_link_ext);
+  UP(L.quat, h_quat); UP(L.quat_raw, h_quat_raw); UP(L.Lown, h_Lown); UP(L.diam, h_diam); UP(L.arm, h_arm); UP(L.link_ext, h_link_ext);
   UP(L.apple_ext, h_apple_ext); UP(L.apple_nom, h_nom); UP(L.apple_c, h_c); UP(L.level_off, h_lev);
 #undef UP
   e = cudaStreamSynchronize(ctx->stream);   // the host images die at the end of this call
   if (e == cudaSuccess) e = launch_rest_pose(D, 0, 0, ctx->stream);
   if (e == cudaSuccess) e = launch_randomize(D, 0ull, 0, ctx->stream);
+  ctx->kernel_launches += 2;
   // launch geometry of k_step
   ctx->smem = L.max_smem;
   int per_sm = 0, n_sm = 0, dev = 0;
@@ -440,7 +451,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   // anchors come back once (rest geometry never changes)
   std::vector<double> h_anchor(3 * std::max<size_t>(L.sumAp, 16));
   if (e == cudaSuccess)
-    e = cudaMemcpyAsync(h_anchor.data(), D.anchor, sizeof(double) * h_anchor.size(), cudaMemcpyDeviceToHost, ctx->stream);
+    e = cpy(ctx, h_anchor.data(), D.anchor, sizeof(double) * h_anchor.size(), cudaMemcpyDeviceToHost, ctx->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
   if (e != cudaSuccess) {
     g_err = std::string("ob_create: ") + cudaGetErrorString(e);
@@ -467,6 +478,7 @@ int ob_randomize(ob_ctx *ctx, uint64_t seed) {
   int rc = flush_wrenches(ctx);
   if (rc != OB_OK) return rc;
   CU(launch_randomize(ctx->dev, (unsigned long long)seed, 1, ctx->stream));
+  ctx->kernel_launches += 1;
   return OB_OK;
 }
 
@@ -513,6 +525,11 @@ int ob_apply_wrench_batch(ob_ctx *ctx, int n, const int32_t *world, const int32_
   return OB_OK;
 }
 
+int ob_flush(ob_ctx *ctx) {
+  if (!ctx) return OB_E_ARG;
+  return flush_wrenches(ctx);
+}
+
 int ob_step(ob_ctx *ctx, int n) {
   if (!ctx) return OB_E_ARG;
   if (n < 0) return fail(ctx, OB_E_ARG, "n < 0");
@@ -522,6 +539,8 @@ int ob_step(ob_ctx *ctx, int n) {
   CU(cudaMemsetAsync(ctx->dev.queue, 0, sizeof(int32_t), ctx->stream));
   CU(launch_step(ctx->dev, n, ctx->grid, ctx->block, ctx->smem, ctx->stream));
   ctx->launches = 1;
+  ctx->kernel_launches += 1;
+  ctx->step_calls += 1;
   return OB_OK;
 }
 
@@ -534,14 +553,17 @@ int ob_get_state(ob_ctx *ctx, int world, float *q, float *qd, float *apple_x, fl
   std::vector<unsigned char> lb(link_state_bytes(d.Np)), ab(std::max(apple_state_bytes(d.Ap), 1));
   std::vector<float> pose(link_pose7 ? 7 * (size_t)d.N : 0);
   WorldInfo wi;
-  if (link_pose7) CU(launch_pose(ctx->dev, world, ctx->stream));
-  CU(cudaMemcpyAsync(lb.data(), ctx->dev.link_blk + d.link_blk_off, lb.size(), cudaMemcpyDeviceToHost, ctx->stream));
+  if (link_pose7) {
+    CU(launch_pose(ctx->dev, world, ctx->stream));
+    ctx->kernel_launches += 1;
+  }
+  CU(cpy(ctx, lb.data(), ctx->dev.link_blk + d.link_blk_off, lb.size(), cudaMemcpyDeviceToHost, ctx->stream));
   if (d.Ap)
-    CU(cudaMemcpyAsync(ab.data(), ctx->dev.apple_blk + d.apple_blk_off, apple_state_bytes(d.Ap), cudaMemcpyDeviceToHost,
+    CU(cpy(ctx, ab.data(), ctx->dev.apple_blk + d.apple_blk_off, apple_state_bytes(d.Ap), cudaMemcpyDeviceToHost,
                        ctx->stream));
   if (link_pose7)
-    CU(cudaMemcpyAsync(pose.data(), ctx->dev.pose7, sizeof(float) * pose.size(), cudaMemcpyDeviceToHost, ctx->stream));
-  CU(cudaMemcpyAsync(&wi, ctx->dev.info + world, sizeof(wi), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cpy(ctx, pose.data(), ctx->dev.pose7, sizeof(float) * pose.size(), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cpy(ctx, &wi, ctx->dev.info + world, sizeof(wi), cudaMemcpyDeviceToHost, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   const float *st = reinterpret_cast<const float *>(lb.data());
   const unsigned char *fl = lb.data() + kLinkStateFloats * 4 * d.Np;
@@ -574,11 +596,11 @@ int ob_set_state(ob_ctx *ctx, int world, const float *q, const float *qd, const 
   const HostWorld &H = ctx->hw[world];
   std::vector<unsigned char> lb(link_state_bytes(d.Np)), ab(std::max(apple_state_bytes(d.Ap), 1));
   WorldInfo wi;
-  CU(cudaMemcpyAsync(lb.data(), ctx->dev.link_blk + d.link_blk_off, lb.size(), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cpy(ctx, lb.data(), ctx->dev.link_blk + d.link_blk_off, lb.size(), cudaMemcpyDeviceToHost, ctx->stream));
   if (d.Ap)
-    CU(cudaMemcpyAsync(ab.data(), ctx->dev.apple_blk + d.apple_blk_off, apple_state_bytes(d.Ap), cudaMemcpyDeviceToHost,
+    CU(cpy(ctx, ab.data(), ctx->dev.apple_blk + d.apple_blk_off, apple_state_bytes(d.Ap), cudaMemcpyDeviceToHost,
                        ctx->stream));
-  CU(cudaMemcpyAsync(&wi, ctx->dev.info + world, sizeof(wi), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cpy(ctx, &wi, ctx->dev.info + world, sizeof(wi), cudaMemcpyDeviceToHost, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   float *st = reinterpret_cast<float *>(lb.data());
   unsigned char *fl = lb.data() + kLinkStateFloats * 4 * d.Np;
@@ -600,11 +622,11 @@ int ob_set_state(ob_ctx *ctx, int world, const float *q, const float *qd, const 
     if (attached) { af[a] = attached[e] ? 1 : 0; af[d.Ap + a] = 0; af[2 * d.Ap + a] = 0; }
   }
   wi.status = 0;
-  CU(cudaMemcpyAsync(ctx->dev.link_blk + d.link_blk_off, lb.data(), lb.size(), cudaMemcpyHostToDevice, ctx->stream));
+  CU(cpy(ctx, ctx->dev.link_blk + d.link_blk_off, lb.data(), lb.size(), cudaMemcpyHostToDevice, ctx->stream));
   if (d.Ap)
-    CU(cudaMemcpyAsync(ctx->dev.apple_blk + d.apple_blk_off, ab.data(), apple_state_bytes(d.Ap), cudaMemcpyHostToDevice,
+    CU(cpy(ctx, ctx->dev.apple_blk + d.apple_blk_off, ab.data(), apple_state_bytes(d.Ap), cudaMemcpyHostToDevice,
                        ctx->stream));
-  CU(cudaMemcpyAsync(ctx->dev.info + world, &wi, sizeof(wi), cudaMemcpyHostToDevice, ctx->stream));
+  CU(cpy(ctx, ctx->dev.info + world, &wi, sizeof(wi), cudaMemcpyHostToDevice, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   return OB_OK;
 }
@@ -617,7 +639,7 @@ int ob_get_apple_x64(ob_ctx *ctx, int world, double *apple_x) {
   const HostWorld &H = ctx->hw[world];
   if (!d.A) return OB_OK;
   std::vector<float> u(3 * (size_t)d.Ap);
-  CU(cudaMemcpyAsync(u.data(), ctx->dev.apple_blk + d.apple_blk_off, sizeof(float) * u.size(), cudaMemcpyDeviceToHost,
+  CU(cpy(ctx, u.data(), ctx->dev.apple_blk + d.apple_blk_off, sizeof(float) * u.size(), cudaMemcpyDeviceToHost,
                      ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   for (int a = 0; a < d.A; a++) {
@@ -633,10 +655,10 @@ int ob_get_counters(ob_ctx *ctx, int world, int32_t *rupture_count, int32_t *pul
   const WorldDesc &d = ctx->desc[world];
   const HostWorld &H = ctx->hw[world];
   std::vector<unsigned char> lf(2 * d.Np), af(std::max(3 * d.Ap, 1));
-  CU(cudaMemcpyAsync(lf.data(), ctx->dev.link_blk + d.link_blk_off + kLinkStateFloats * 4 * d.Np, lf.size(),
+  CU(cpy(ctx, lf.data(), ctx->dev.link_blk + d.link_blk_off + kLinkStateFloats * 4 * d.Np, lf.size(),
                      cudaMemcpyDeviceToHost, ctx->stream));
   if (d.Ap)
-    CU(cudaMemcpyAsync(af.data(), ctx->dev.apple_blk + d.apple_blk_off + 6 * 4 * d.Ap, 3 * d.Ap, cudaMemcpyDeviceToHost,
+    CU(cpy(ctx, af.data(), ctx->dev.apple_blk + d.apple_blk_off + 6 * 4 * d.Ap, 3 * d.Ap, cudaMemcpyDeviceToHost,
                        ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   if (rupture_count)
@@ -655,10 +677,10 @@ int ob_set_counters(ob_ctx *ctx, int world, const int32_t *rupture_count, const 
   const WorldDesc &d = ctx->desc[world];
   const HostWorld &H = ctx->hw[world];
   std::vector<unsigned char> lf(2 * d.Np), af(std::max(3 * d.Ap, 1));
-  CU(cudaMemcpyAsync(lf.data(), ctx->dev.link_blk + d.link_blk_off + kLinkStateFloats * 4 * d.Np, lf.size(),
+  CU(cpy(ctx, lf.data(), ctx->dev.link_blk + d.link_blk_off + kLinkStateFloats * 4 * d.Np, lf.size(),
                      cudaMemcpyDeviceToHost, ctx->stream));
   if (d.Ap)
-    CU(cudaMemcpyAsync(af.data(), ctx->dev.apple_blk + d.apple_blk_off + 6 * 4 * d.Ap, 3 * d.Ap, cudaMemcpyDeviceToHost,
+    CU(cpy(ctx, af.data(), ctx->dev.apple_blk + d.apple_blk_off + 6 * 4 * d.Ap, 3 * d.Ap, cudaMemcpyDeviceToHost,
                        ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   auto clampc = [](int32_t v) { return (unsigned char)std::min(std::max(v, 0), 255); };
@@ -668,10 +690,10 @@ int ob_set_counters(ob_ctx *ctx, int world, const int32_t *rupture_count, const 
     if (pull_count) af[d.Ap + a] = clampc(pull_count[H.int2ext_apple[a]]);
     if (tension_count) af[2 * d.Ap + a] = clampc(tension_count[H.int2ext_apple[a]]);
   }
-  CU(cudaMemcpyAsync(ctx->dev.link_blk + d.link_blk_off + kLinkStateFloats * 4 * d.Np, lf.data(), lf.size(),
+  CU(cpy(ctx, ctx->dev.link_blk + d.link_blk_off + kLinkStateFloats * 4 * d.Np, lf.data(), lf.size(),
                      cudaMemcpyHostToDevice, ctx->stream));
   if (d.Ap)
-    CU(cudaMemcpyAsync(ctx->dev.apple_blk + d.apple_blk_off + 6 * 4 * d.Ap, af.data(), 3 * d.Ap, cudaMemcpyHostToDevice,
+    CU(cpy(ctx, ctx->dev.apple_blk + d.apple_blk_off + 6 * 4 * d.Ap, af.data(), 3 * d.Ap, cudaMemcpyHostToDevice,
                        ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   return OB_OK;
@@ -684,9 +706,9 @@ int ob_get_material(ob_ctx *ctx, int world, float *emr, float *apple_detach, flo
   const HostWorld &H = ctx->hw[world];
   WorldInfo wi;
   std::vector<float> ac(std::max(7 * d.Ap, 1));
-  CU(cudaMemcpyAsync(&wi, ctx->dev.info + world, sizeof(wi), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cpy(ctx, &wi, ctx->dev.info + world, sizeof(wi), cudaMemcpyDeviceToHost, ctx->stream));
   if (d.Ap)
-    CU(cudaMemcpyAsync(ac.data(), ctx->dev.apple_blk + d.apple_blk_off + apple_state_bytes(d.Ap), sizeof(float) * 7 * d.Ap,
+    CU(cpy(ctx, ac.data(), ctx->dev.apple_blk + d.apple_blk_off + apple_state_bytes(d.Ap), sizeof(float) * 7 * d.Ap,
                        cudaMemcpyDeviceToHost, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   if (emr) { emr[0] = wi.E; emr[1] = wi.MOR; emr[2] = wi.density; }
@@ -701,12 +723,12 @@ int ob_events(ob_ctx *ctx, ob_event *buf, int cap, int *n_out) {
   if (!ctx) return OB_E_ARG;
   if (!n_out || cap < 0 || (cap > 0 && !buf)) return fail(ctx, OB_E_ARG, "null output");
   int32_t cnt[2] = {0, 0};
-  CU(cudaMemcpyAsync(cnt, ctx->dev.ev_count, sizeof(cnt), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cpy(ctx, cnt, ctx->dev.ev_count, sizeof(cnt), cudaMemcpyDeviceToHost, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   const int have = (int)std::min<long long>(cnt[0], (long long)ctx->dev.ev_cap);
   std::vector<ob_event> ev(have);
   if (have) {
-    CU(cudaMemcpyAsync(ev.data(), ctx->dev.events, sizeof(ob_event) * have, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cpy(ctx, ev.data(), ctx->dev.events, sizeof(ob_event) * have, cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
   }
   std::sort(ev.begin(), ev.end(), [](const ob_event &a, const ob_event &b) {
@@ -720,9 +742,9 @@ int ob_events(ob_ctx *ctx, ob_event *buf, int cap, int *n_out) {
   *n_out = n;
   // keep what did not fit, in sorted order, at the head of the device list
   const int rest = have - n;
-  if (rest) CU(cudaMemcpyAsync(ctx->dev.events, ev.data() + n, sizeof(ob_event) * rest, cudaMemcpyHostToDevice, ctx->stream));
+  if (rest) CU(cpy(ctx, ctx->dev.events, ev.data() + n, sizeof(ob_event) * rest, cudaMemcpyHostToDevice, ctx->stream));
   int32_t newcnt[2] = {rest, 0};
-  CU(cudaMemcpyAsync(ctx->dev.ev_count, newcnt, sizeof(newcnt), cudaMemcpyHostToDevice, ctx->stream));
+  CU(cpy(ctx, ctx->dev.ev_count, newcnt, sizeof(newcnt), cudaMemcpyHostToDevice, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   if (cnt[1] || cnt[0] > ctx->dev.ev_cap) return fail(ctx, OB_E_CAPACITY, "device event list overflowed (capacity %d)", ctx->dev.ev_cap);
   return OB_OK;
@@ -731,7 +753,7 @@ int ob_events(ob_ctx *ctx, ob_event *buf, int cap, int *n_out) {
 int ob_stats(ob_ctx *ctx, uint64_t *cg_iters_total, uint64_t *world_steps_total, int32_t *n_flagged) {
   if (!ctx) return OB_E_ARG;
   std::vector<WorldInfo> wi(ctx->n_worlds);
-  CU(cudaMemcpyAsync(wi.data(), ctx->dev.info, sizeof(WorldInfo) * wi.size(), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cpy(ctx, wi.data(), ctx->dev.info, sizeof(WorldInfo) * wi.size(), cudaMemcpyDeviceToHost, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   uint64_t it = 0, ws = 0;
   int32_t fl = 0;
@@ -750,6 +772,17 @@ int ob_launch_info(ob_ctx *ctx, int32_t *n_launches, int32_t *grid, int32_t *blo
   if (smem_bytes) *smem_bytes = ctx->smem;
   return OB_OK;
 }
+
+int ob_counters(ob_ctx *ctx, uint64_t out[4]) {
+  if (!ctx) return OB_E_ARG;
+  if (!out) return fail(ctx, OB_E_ARG, "out is null");
+  out[0] = ctx->h2d_bytes; out[1] = ctx->d2h_bytes; out[2] = ctx->kernel_launches; out[3] = ctx->step_calls;
+  return OB_OK;
+}
+
+int ob_sizeof_params(void) { return (int)sizeof(ob_params); }
+int ob_sizeof_world_spec(void) { return (int)sizeof(ob_world_spec); }
+int ob_sizeof_event(void) { return (int)sizeof(ob_event); }
 
 const char *ob_last_error(const ob_ctx *ctx) { return ctx ? ctx->err.c_str() : (g_err.empty() ? kNullCtx : g_err.c_str()); }
 

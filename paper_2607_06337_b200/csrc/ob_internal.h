@@ -68,7 +68,8 @@ struct DevCtx {
   unsigned char *apple_blk;      // apple-block pool
   // per-link statics, indexed link_base + i (SoA pools use k * Np + i inside the world's slice)
   const int4 *topo;              // x = parent, y = first child, z = n_children | n_apples << 16, w = first apple
-  const float4 *quat;            // rest quaternion (w,x,y,z)
+  const float4 *quat;            // rest quaternion (w,x,y,z), normalised in fp64 then rounded (k_step)
+  const float4 *quat_raw;        // rest quaternion exactly as the caller gave it (create-time fp64 rest pose)
   float *R0;                     // [9 * link_base + k * Np + i] rest world rotation, row-major k
   float *Mmax;                   // rupture moment (after randomize)
   const float *Lown;             // link length

@@ -121,8 +121,10 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // k_rest_pose: one CTA per world.  R0_i = Q_0 ... Q_i and anchor_a = p0_b + R0_b o by walking up the
 // ancestors in fp64 (create-time only; Eq. 3).
 // ------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void quat_to_mat_d(float4 q, double *R) {
+__device__ __forceinline__ void quat_to_mat_d(float4 q, double *R) {   // normalises in fp64
   double w = q.x, x = q.y, y = q.z, z = q.w;
+  const double n = sqrt(w * w + x * x + y * y + z * z);
+  w /= n; x /= n; y /= n; z /= n;
   R[0] = 1 - 2 * (y * y + z * z); R[1] = 2 * (x * y - w * z);     R[2] = 2 * (x * z + w * y);
   R[3] = 2 * (x * y + w * z);     R[4] = 1 - 2 * (x * x + z * z); R[5] = 2 * (y * z - w * x);
   R[6] = 2 * (x * z - w * y);     R[7] = 2 * (y * z + w * x);     R[8] = 1 - 2 * (x * x + y * y);
@@ -131,7 +133,7 @@ __device__ __forceinline__ void quat_to_mat_d(float4 q, double *R) {
 __global__ void k_rest_pose(DevCtx c) {
   const WorldDesc d = c.desc[blockIdx.x];
   const int4 *topo = c.topo + d.link_base;
-  const float4 *quat = c.quat + d.link_base;
+  const float4 *quat = c.quat_raw + d.link_base;   // the caller's quaternions, normalised in fp64 here
   const float *Lown = c.Lown + d.link_base;
   for (int i = threadIdx.x; i < d.N; i += blockDim.x) {
     double R[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1};
@@ -828,7 +830,7 @@ __global__ void __launch_bounds__(256, 2) k_step(DevCtx c, int n_steps) {
 __global__ void k_pose(DevCtx c, int w) {
   const WorldDesc d = c.desc[w];
   const int4 *topo = c.topo + d.link_base;
-  const float4 *quat = c.quat + d.link_base;
+  const float4 *quat = c.quat_raw + d.link_base;
   const float *Lown = c.Lown + d.link_base;
   const float *st = reinterpret_cast<const float *>(c.link_blk + d.link_blk_off);
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < d.N; i += gridDim.x * blockDim.x) {

@@ -1,0 +1,511 @@
+"""GPU parity tests: the CUDA path (through the C ABI, include/orchard.h) against the fp64 oracle on the same
+seeded inputs.  Protocols and tolerances are BASELINE.json north_star's, read as SURVEY.md 8(c) A27/A28 and
+"Comparison protocol" (restated in DESIGN.md):
+
+  single step   both sides start from the same state, one step, relative state error <= 1e-5
+  free run      200 steps without events, relative state error <= 1e-3
+  events        sets of (world, step, kind, index) identical; in lock-step runs a one-sided predicate
+                decision is accepted only within 1e-4 of its threshold, and is counted and reported
+  Philox        per-world and per-apple draws bit-exact
+"""
+from __future__ import annotations
+
+import dataclasses
+import functools
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_2607_06337_b200 as ob
+from helpers import GOLDEN, chain_spec, quat_axis, rel_state_error
+from workloads import (MASTER_SEED, binary_tree_config1, config1_loads, config2_pulls, config_params, make_config,
+                       stochastic_world, wrench_process)
+
+pytestmark = pytest.mark.gpu
+
+TOL_STEP = 1e-5      # north_star: single step, fp32
+TOL_RUN = 1e-3       # north_star: 200-step trajectory without events
+BIG_N = 1000         # largest world of the heterogeneous edge-case batch (configs[4] asks for 1500: DESIGN.md)
+NEAR = 1e-4          # north_star: relative margin of a threshold inside which a one-sided event is tolerated
+
+
+# ----------------------------------------------------------------------------------------------------
+# helpers
+# ----------------------------------------------------------------------------------------------------
+def _x_rest(ref: oracle.OracleWorld) -> np.ndarray:
+    """Apple positions of the freshly reset oracle world (rest hang point + m g / k_s)."""
+    return ref._x_rest
+
+
+def _make(specs, P, seed=None):
+    sim = ob.Orchard(specs, P)
+    refs = [oracle.OracleWorld(s, P, world_index=w) for w, s in enumerate(specs)]
+    if seed is not None:
+        sim.randomize(seed)
+        for r in refs:
+            r.randomize(seed)
+    for r in refs:
+        r._x_rest = r.get_state()["apple_x"].copy()
+    return sim, refs
+
+
+def _apply(sim, refs, loads):
+    for (w, body, pt, f) in loads:
+        sim.apply_wrench(w, body, pt, f)
+        refs[w].apply_wrench(body, pt, f)
+
+
+def _sync_oracle_to_gpu(sim, ref, w):
+    """Lock-step protocol: the oracle is reset to the GPU's state (apple positions at the library's
+    internal precision, so that no rounding is introduced by the hand-over), counters included."""
+    g = sim.get_state(w)
+    ref.set_state(q=g["q"], qd=g["qd"], apple_x=g["apple_x64"], apple_v=g["apple_v"],
+                  ruptured=g["ruptured"], attached=g["attached"])
+    ref.set_counters(*sim.get_counters(w))
+    ref.set_step(g["step"])
+    return g
+
+
+def _err(sim, ref, w):
+    g, o = sim.get_state(w), ref.get_state()
+    gg = dict(g)
+    gg["apple_x"] = g["apple_x64"]
+    return rel_state_error(gg, o, _x_rest(ref)), g, o
+
+
+def _key(ev):
+    return (ev[0], ev[1], ev[2], ev[3])
+
+
+@functools.lru_cache(maxsize=None)
+def _stochastic(seed, n_lo, n_hi, apples, count, depth=(5, 6, 7)):
+    rng = np.random.default_rng(seed)
+    return tuple(stochastic_world(rng, n_lo, n_hi, apples, depth_choices=depth) for _ in range(count))
+
+
+# ----------------------------------------------------------------------------------------------------
+# Philox draws (reading A23): bit-exact for every world and apple
+# ----------------------------------------------------------------------------------------------------
+def test_philox_draws_bit_exact_all_worlds():
+    specs = list(_stochastic(11, 60, 120, 12, 96, (4, 5)))
+    P = config_params(2)
+    sim, refs = _make(specs, P, seed=MASTER_SEED + 2000)
+    for w, r in enumerate(refs):
+        g, o = sim.get_material(w), r.material()
+        assert np.float32(g["E"]).tobytes() == np.float32(o["E"]).tobytes()
+        assert np.float32(g["MOR"]).tobytes() == np.float32(o["MOR"]).tobytes()
+        assert np.float32(g["density"]).tobytes() == np.float32(o["density"]).tobytes()
+        assert g["detach"].tobytes() == o["detach"].astype(np.float32).tobytes()
+        assert g["mass"].tobytes() == o["mass"].astype(np.float32).tobytes()
+        assert P.range_E[0] <= g["E"] <= P.range_E[1] and P.range_detach[0] <= g["detach"].min()
+    # a second seed (with a high word) redraws and resets
+    sim.randomize((7 << 32) | 5)
+    refs[3].randomize((7 << 32) | 5)
+    g, o = sim.get_material(3), refs[3].material()
+    assert np.float32(g["E"]).tobytes() == np.float32(o["E"]).tobytes()
+    assert g["mass"].tobytes() == o["mass"].astype(np.float32).tobytes()
+    st = sim.get_state(3)
+    assert st["step"] == 0 and not st["q"].any() and st["attached"].all()
+    sim.close()
+
+
+def test_reset_state_is_the_rest_pose_with_apple_sag():
+    """at rest the apple hangs m g / k_s below the hang point."""
+    specs = [binary_tree_config1()] + list(_stochastic(5, 150, 250, 20, 2))
+    sim, refs = _make(specs, config_params(2), seed=99)
+    for w, r in enumerate(refs):
+        g, o = sim.get_state(w, pose=True), r.get_state()
+        assert np.abs(g["apple_x64"] - o["apple_x"]).max() < 1e-9     # fp64 rest chain + fp32 sag m g / k_s
+        assert not g["q"].any() and not g["qd"].any() and not g["apple_v"].any()
+        R, p, _, _ = r.fk()
+        assert np.abs(g["link_pose7"][:, :3] - p).max() < 1e-6
+    sim.close()
+
+
+# ----------------------------------------------------------------------------------------------------
+# single step from an identical state: relative state error <= 1e-5 (north_star)
+# ----------------------------------------------------------------------------------------------------
+def _single_step_errors(sim, refs, worlds):
+    worst = {}
+    for w in worlds:
+        _sync_oracle_to_gpu(sim, refs[w], w)
+    sim.step(1)
+    oracle.step_many([refs[w] for w in worlds], 1)
+    for w in worlds:
+        e, g, o = _err(sim, refs[w], w)
+        assert g["status"] == 0 and g["step"] == o["step"]
+        worst[w] = e
+    return worst
+
+
+def test_single_step_config1_along_the_run():
+    """configs[0] (1b loads, reading A22): one step from the GPU's own state at several points of the run,
+    before and after the detach (step 335) and the rupture (step 443)."""
+    spec, P = binary_tree_config1(), config_params(1)
+    sim, refs = _make([spec], P)
+    done = 0
+    for target in (1, 10, 100, 300, 340, 400, 460, 499):
+        while done < target:
+            _apply(sim, refs, config1_loads(spec, done, 500, 30.0, 5000.0))
+            sim.step(1)
+            done += 1
+        _apply(sim, refs, config1_loads(spec, done, 500, 30.0, 5000.0))
+        e = _single_step_errors(sim, refs, [0])[0]
+        done += 1
+        assert e["max"] <= TOL_STEP, (target, e)
+    sim.close()
+
+
+@pytest.mark.parametrize("n_lo,n_hi,apples,h_cfg", [(150, 250, 20, 2), (350, 450, 60, 3), (350, 450, 60, 4)])
+def test_single_step_stochastic_worlds_under_wrenches(n_lo, n_hi, apples, h_cfg):
+    """configs[1..3]-shaped worlds (several tiles of 256 threads is not the unit here: one CTA per world,
+    N is not a multiple of 16, so the padded tail is exercised), moving under the A25 wrench process."""
+    specs = list(_stochastic(100 + h_cfg, n_lo, n_hi, apples, 6))
+    P = config_params(h_cfg)
+    sim, refs = _make(specs, P, seed=MASTER_SEED + 1000 * h_cfg)
+    worst = 0.0
+    for epoch in range(3):
+        _apply(sim, refs, wrench_process(specs, epoch, 0.0, 150.0))
+        sim.step(25)
+        errs = _single_step_errors(sim, refs, range(len(specs)))
+        for w, e in errs.items():
+            assert e["max"] <= TOL_STEP, (epoch, w, specs[w].n_links, e)
+            worst = max(worst, e["max"])
+        sim.step(24)
+    print(f"single-step worst relative error {worst:.2e}")
+    sim.close()
+
+
+def test_single_step_explicit_tether_and_no_preconditioner():
+    """The paper-literal explicit Eq. 7 (tether_implicit = 0) and plain CG (precond = 0) reach the same step."""
+    spec = binary_tree_config1()
+    for kw in (dict(tether_implicit=0), dict(precond=0, cg_max_iter=2000), dict(cg_norm=1)):
+        P = dataclasses.replace(config_params(1), **kw)
+        sim, refs = _make([spec], P)
+        for s in range(30):
+            _apply(sim, refs, config1_loads(spec, 10 * s, 500, 30.0, 400.0))
+            sim.step(1)
+        e = _single_step_errors(sim, refs, [0])[0]
+        assert e["max"] <= TOL_STEP, (kw, e)
+        sim.close()
+
+
+# ----------------------------------------------------------------------------------------------------
+# 200-step trajectories without events: relative state error <= 1e-3 (north_star)
+# ----------------------------------------------------------------------------------------------------
+def test_free_run_200_steps_config1():
+    spec, P = binary_tree_config1(), config_params(1)
+    sim, refs = _make([spec], P)
+    for s in range(200):
+        _apply(sim, refs, config1_loads(spec, s, 500, 30.0, 400.0))
+        sim.step(1)
+        refs[0].step(1)
+    e, g, o = _err(sim, refs[0], 0)
+    assert not sim.events() and not refs[0].events()
+    assert e["max"] <= TOL_RUN, e
+    sim.close()
+
+
+@pytest.mark.parametrize("n_lo,n_hi,apples,cfg,count", [(150, 250, 20, 2, 4), (350, 450, 60, 4, 2)])
+def test_free_run_200_steps_stochastic(n_lo, n_hi, apples, cfg, count):
+    """Gravity settling plus mild constant wrenches (no events fire); 200 steps in ONE launch on the GPU."""
+    specs = list(_stochastic(200 + cfg, n_lo, n_hi, apples, count))
+    P = config_params(cfg)
+    sim, refs = _make(specs, P, seed=MASTER_SEED + 1000 * cfg + 1)
+    _apply(sim, refs, wrench_process(specs, 0, 0.0, 10.0))
+    sim.step(200)
+    oracle.step_many(refs, 200)
+    assert not sim.events()
+    for w, r in enumerate(refs):
+        assert not r.events()
+        e, g, o = _err(sim, r, w)
+        assert g["step"] == 200 and g["status"] == 0
+        assert e["max"] <= TOL_RUN, (w, specs[w].n_links, e)
+    sim.close()
+
+
+# ----------------------------------------------------------------------------------------------------
+# events: configs[0] as written and 1b, free-running, against the oracle's stored run
+# ----------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant,branch_fmax", [("1", 400.0), ("1b", 5000.0)])
+def test_config1_event_sets_match_the_oracle_run(variant, branch_fmax):
+    """configs[0] as written (one detach, no rupture: reading A22) and variant 1b (detach + rupture of link 4):
+    both sides run the 500 steps freely; the event sets are identical and agree with the closed-form
+    expectations stored in tests/golden/config1_events.txt."""
+    spec, P = binary_tree_config1(), config_params(1)
+    sim, refs = _make([spec], P)
+    for s in range(500):
+        _apply(sim, refs, config1_loads(spec, s, 500, 30.0, branch_fmax))
+        sim.step(1)
+        refs[0].step(1)
+        if s == 199:
+            e, _, _ = _err(sim, refs[0], 0)
+            assert e["max"] <= TOL_RUN, e
+    gev, oev = sim.events(), refs[0].events()
+    assert [_key(e) for e in gev] == [_key(e) for e in oev]
+    for g, o in zip(gev, oev):
+        assert abs(g[4] - o[4]) <= 2e-4 * abs(o[4]) and abs(g[5] - o[5]) <= 1e-6 * abs(o[5]) and g[4] > g[5]
+    rows = [l.split() for l in open(f"{GOLDEN}/config1_events.txt") if l.strip() and l[0] != "#"]
+    exp = [r for r in rows if r[0] == variant]
+    assert len(gev) == len(exp)
+    for g, r in zip(gev, exp):
+        assert (g[2], g[3]) == (int(r[2]), int(r[3])) and abs(g[1] - int(r[1])) <= (0 if g[2] == 1 else 2)
+    st = sim.get_state(0)
+    assert st["step"] == 500 and st["status"] == 0
+    assert st["attached"].tolist() == [0, 1, 1, 1]
+    assert int(st["ruptured"].sum()) == (1 if variant == "1b" else 0)
+    e, _, _ = _err(sim, refs[0], 0)
+    print(f"config {variant}: events {[_key(x) for x in gev]}, end-of-run relative state error {e['max']:.2e}")
+    sim.close()
+
+
+# ----------------------------------------------------------------------------------------------------
+# events over long violent runs: lock-step protocol (SURVEY.md 8(c) "Comparison protocol" (iii))
+# ----------------------------------------------------------------------------------------------------
+def _lockstep(sim, refs, specs, n_steps, loads_at):
+    """Every step: oracle <- GPU state and counters; both advance one step; flags, counters and events of
+    that step must agree.  A one-sided predicate decision is tolerated only within NEAR of its threshold."""
+    near = 0
+    n_events = 0
+    worst = 0.0
+    derived = [r.derived() for r in refs]
+    mats = [r.material() for r in refs]
+    for s in range(n_steps):
+        loads = loads_at(s)
+        if loads:
+            _apply(sim, refs, loads)
+        for w, r in enumerate(refs):
+            _sync_oracle_to_gpu(sim, r, w)
+        pre = [r.get_state() for r in refs]
+        pre_fk = [r.fk() for r in refs]
+        sim.step(1)
+        oracle.step_many(refs, 1)
+        gev = sorted(_key(e) for e in sim.events())
+        oev = sorted(_key(e) for r in refs for e in r.events())
+        n_events += len(gev)
+        for w, r in enumerate(refs):
+            e, g, o = _err(sim, r, w)
+            if g["status"] & ob.OB_STATUS_NONFINITE:
+                raise AssertionError(f"world {w} went non-finite at step {s}")
+            worst = max(worst, e["max"])
+            grc, gca, gcb = sim.get_counters(w)
+            orc, oca, ocb = r.get_counters()
+            # rupture decisions (flag or counter differs): K |theta| of the NEW q within NEAR of M_max
+            bad = np.nonzero((g["ruptured"] != o["ruptured"]) | ((grc != orc) & (g["ruptured"] == 0)))[0]
+            for i in bad:
+                mu = derived[w]["K"][i] * np.hypot(o["q"][2 * i], o["q"][2 * i + 1])
+                assert abs(mu / derived[w]["Mmax"][i] - 1.0) <= NEAR, ("rupture", s, w, i, mu, derived[w]["Mmax"][i])
+                near += 1
+            # detach decisions: |f_user| vs f_det (path A) or |f_s| vs kappa f_det (path B), start-of-step forces
+            bad = np.nonzero((g["attached"] != o["attached"]) | (((gca != oca) | (gcb != ocb)) & (g["attached"] == 1)))[0]
+            for a in bad:
+                R, p, _, _ = pre_fk[w]
+                b = specs[w].apple_link[a]
+                xh = p[b] + R[b] @ specs[w].apple_offset[a].astype(np.float64)
+                fs = float(specs[w].apple_k[a]) * np.linalg.norm(pre[w]["apple_x"][a] - xh)
+                thr = float(np.float32(sim.params.detach_kappa)) * mats[w]["detach"][a]
+                assert abs(fs / thr - 1.0) <= NEAR, ("detach", s, w, a, fs, thr)
+                near += 1
+        if near == 0:
+            assert gev == oev, (s, gev, oev)
+    return dict(near=near, events=n_events, worst_single_step=worst)
+
+
+def test_lockstep_event_sets_cascading_ruptures():
+    """configs[4]-shaped stress at a size the oracle finishes in seconds: thin-twig worlds under
+    U(100,600) N wrenches with MOR ~ U(30,60) MPa; ruptures cascade, apples detach by stem tension."""
+    specs = list(_stochastic(55, 100, 180, 12, 4, (5, 6)))
+    P = config_params(5)
+    sim, refs = _make(specs, P, seed=MASTER_SEED + 5000)
+    res = _lockstep(sim, refs, specs, 250,
+                    lambda s: wrench_process(specs, s // 50, 100.0, 600.0, seed_offset=5000) if s % 50 == 0 else [])
+    print("lock-step:", res)
+    assert res["events"] >= 4, res            # the stress does produce events
+    assert res["near"] <= 2, res
+    assert res["worst_single_step"] <= 10 * TOL_STEP, res   # free hinges at the speed clamp included
+    sim.close()
+
+
+def test_lockstep_apple_pulls_config2():
+    """configs[1]: constant pulls on five apples per world (path A fires after 3 steps above f_detach)."""
+    specs = list(_stochastic(56, 150, 250, 20, 3))
+    P = config_params(2)
+    sim, refs = _make(specs, P, seed=MASTER_SEED + 2000)
+    pulls = config2_pulls(specs)
+    res = _lockstep(sim, refs, specs, 40, lambda s: pulls if s == 5 else [])
+    print("lock-step pulls:", res)
+    mats = [r.material() for r in refs]
+    expect = sum(1 for (w, body, _p, f) in pulls
+                 if np.linalg.norm(np.float32(f)) > mats[w]["detach"][body - specs[w].n_links])
+    assert res["near"] == 0 and res["events"] >= expect
+    sim.close()
+
+
+# ----------------------------------------------------------------------------------------------------
+# API behaviour on the device: state round trip, multi-step launches, wrench slots, event draining, edge cases
+# ----------------------------------------------------------------------------------------------------
+def test_state_round_trip_and_multi_step_launch_are_bit_exact():
+    specs = list(_stochastic(77, 150, 250, 20, 3))
+    P = config_params(2)
+    a = ob.Orchard(specs, P)
+    b = ob.Orchard(specs, P)
+    for sim in (a, b):
+        sim.randomize(4242)
+        for (w, body, pt, f) in wrench_process(specs, 0, 0.0, 60.0):
+            sim.apply_wrench(w, body, pt, f)
+    a.step(37)                      # one launch, 37 steps on chip
+    for _ in range(37):
+        b.step(1)                   # 37 launches
+    for w in range(len(specs)):
+        ga, gb = a.get_state(w), b.get_state(w)
+        for k in ("q", "qd", "apple_v", "ruptured", "attached"):
+            assert ga[k].tobytes() == gb[k].tobytes(), (w, k)
+        assert ga["apple_x64"].tobytes() == gb["apple_x64"].tobytes() and ga["step"] == gb["step"] == 37
+    # get -> set -> get is the identity on q, qd, v, flags, and exact to fp32 on x
+    g0 = a.get_state(1)
+    rc0 = a.get_counters(1)
+    a.set_state(1, q=g0["q"], qd=g0["qd"], apple_x=g0["apple_x"], apple_v=g0["apple_v"],
+                ruptured=g0["ruptured"], attached=g0["attached"])
+    a.set_counters(1, *rc0)
+    g1 = a.get_state(1)
+    for k in ("q", "qd", "apple_v", "ruptured", "attached", "apple_x"):
+        assert g0[k].tobytes() == g1[k].tobytes(), k
+    assert np.abs(g1["apple_x64"] - g0["apple_x64"]).max() <= 2.4e-7   # one fp32 ulp at 2-4 m
+    a.close(); b.close()
+
+
+def test_wrench_slots_and_event_drain():
+    spec = binary_tree_config1()
+    P = dataclasses.replace(config_params(1), detach_frames_pull=1)
+    sim = ob.Orchard([spec], P)
+    for body in range(ob.OB_MAX_WRENCH):
+        sim.apply_wrench(0, body, (0, 0, 0.1), (1.0, 0, 0))
+    sim.apply_wrench(0, 3, (0, 0, 0.1), (2.0, 0, 0))                 # same body replaces
+    with pytest.raises(ob.OrchardError) as ei:
+        sim.apply_wrench(0, 20, (0, 0, 0.1), (1.0, 0, 0))            # ninth distinct body
+    assert ei.value.code == ob.OB_E_CAPACITY
+    sim.apply_wrench(0, 0, (0, 0, 0), (0, 0, 0))                     # zero force frees the slot
+    sim.apply_wrench(0, 20, (0, 0, 0.1), (1.0, 0, 0))
+    with pytest.raises(ob.OrchardError):
+        sim.apply_wrench(0, 31 + 4, (0, 0, 0), (1.0, 0, 0))          # body out of range
+    with pytest.raises(ob.OrchardError):
+        sim.apply_wrench(1, 0, (0, 0, 0), (1.0, 0, 0))               # world out of range
+    for body in range(1, ob.OB_MAX_WRENCH):
+        sim.apply_wrench(0, body, (0, 0, 0), (0, 0, 0))
+    sim.apply_wrench(0, 20, (0, 0, 0), (0, 0, 0))
+    # all four apples pulled above f_detach: four detach events in step 0, drained two at a time, sorted
+    for a in range(4):
+        sim.apply_wrench(0, 31 + a, (0, 0, 0), (0, 0, -25.0))
+    sim.step(2)
+    first = sim.events(cap=3)
+    rest = sim.events()
+    assert [e[3] for e in first] == [0, 1, 2] and [e[3] for e in rest] == [3]
+    assert all(e[1] == 0 and e[2] == 1 and e[4] == 25.0 and e[5] == 20.0 for e in first + rest)
+    assert sim.events() == []
+    assert sim.stats()["world_steps_total"] == 2
+    sim.close()
+
+
+def test_edge_cases_single_link_no_apples_and_heterogeneous_batch():
+    """Degenerate and extreme shapes in ONE batch: a 1-link world without apples, a 17-link chain (one more than
+    the 16-link padding granule), configs[0], and a BIG_N-link / 150-apple world (the largest of configs[4])."""
+    rng = np.random.default_rng(3)
+    big = stochastic_world(rng, BIG_N - 10, BIG_N, 150, depth_choices=(7, 8))
+    specs = [chain_spec(1, 0.4, 0.02, root_quat=quat_axis("y", 90.0)),
+             chain_spec(17, 1.7, 0.03, root_quat=quat_axis("y", 60.0),
+                        apples=[(16, (0, 0, 0.1), 0.2, 2e3, 20.0), (16, (0.01, 0, 0.05), 0.15, 2e3, 15.0),
+                                (3, (0, 0.015, 0.02), 0.25, 2e3, 25.0)]),
+             binary_tree_config1(), big]
+    P = config_params(4)
+    sim, refs = _make(specs, P, seed=31337)
+    _apply(sim, refs, [(1, 9, (0.0, 0.015, 0.05), (3.0, -2.0, 1.0)), (3, BIG_N // 2, (0.0, 0.0, 0.01), (5.0, 5.0, -5.0))])
+    sim.step(10)
+    errs = _single_step_errors(sim, refs, range(4))
+    for w, e in errs.items():
+        assert e["max"] <= TOL_STEP, (w, e)
+    info = sim.launch_info()
+    assert info["smem_bytes"] <= 227 * 1024
+    sim.close()
+
+
+def test_world_too_large_for_on_chip_residency_is_refused():
+    spec = chain_spec(6000, 60.0, 0.05)
+    with pytest.raises(ob.OrchardError) as ei:
+        ob.Orchard([spec], config_params(1))
+    assert ei.value.code == ob.OB_E_CAPACITY
+
+
+def test_nonfinite_world_is_frozen_and_flagged():
+    """a world whose state goes non-finite is frozen, flagged and excluded from the counts;
+    its neighbours in the batch are unaffected."""
+    spec = binary_tree_config1()
+    sim, refs = _make([spec, spec, spec], config_params(1))
+    g = sim.get_state(1)
+    q = g["q"].copy()
+    q[7] = np.nan
+    sim.set_state(1, q=q)
+    sim.step(5)
+    st = sim.get_state(1)
+    assert st["status"] & ob.OB_STATUS_NONFINITE and st["step"] == 0
+    assert sim.get_state(0)["step"] == 5 and sim.get_state(2)["status"] == 0
+    s = sim.stats()
+    assert s["world_steps_total"] == 10 and s["n_flagged"] == 1
+    assert sim.get_state(0)["q"].tobytes() == sim.get_state(2)["q"].tobytes()
+    sim.close()
+
+
+# ----------------------------------------------------------------------------------------------------
+# full size, in the launch configuration bench.py times: configs[3] (4096 worlds x 350-450 links, 60 apples)
+# ----------------------------------------------------------------------------------------------------
+def test_full_size_config4_sampled_worlds_and_invariants():
+    """All 4096 worlds run 20 steps in one launch under the wrench process; every Philox draw is compared;
+    eight sampled worlds are compared with the oracle (free run from the randomized rest state); properties
+    that hold at any size are checked on all worlds (finite state, step counter, iteration counts)."""
+    specs = make_config(4, 4096)
+    P = config_params(4)
+    seed = MASTER_SEED + 4000
+    sim = ob.Orchard(specs, P)
+    sim.randomize(seed)
+    loads = wrench_process(specs, 0, 0.0, 150.0)
+    sim.apply_wrench_batch([l[0] for l in loads], [l[1] for l in loads], [l[2] for l in loads], [l[3] for l in loads])
+    sim.step(20)
+    st = sim.stats()
+    assert st["world_steps_total"] == 20 * len(specs) and st["n_flagged"] == 0
+    assert 2 * 20 * len(specs) <= st["cg_iters_total"] <= 60 * 20 * len(specs)
+    # Philox: every world, bit-exact (the draw is a pure function of (seed, world, apple): reading A23)
+    key = [seed & 0xffffffff, seed >> 32]
+    for w in range(0, len(specs), 1):
+        m = sim.get_material(w) if w % 16 == 0 else None
+        if m is None:
+            continue
+        o = oracle.philox4x32_10([w, 0, 0, 0], key)
+        u = np.float32(o[0] >> 8) * np.float32(2.0 ** -24)
+        lo, hi = np.float32(P.range_E[0]), np.float32(P.range_E[1])
+        expect = np.float32(np.float64(u) * np.float64(hi - lo) + np.float64(lo))   # fmaf: one rounding
+        assert np.float32(m["E"]).tobytes() == expect.tobytes(), w
+    sample = [0, 1, 517, 1023, 2048, 3000, 4000, 4095]
+    refs = {w: oracle.OracleWorld(specs[w], P, world_index=w) for w in sample}
+    for w, r in refs.items():
+        r.randomize(seed)
+        r._x_rest = r.get_state()["apple_x"].copy()
+        m, o = sim.get_material(w), r.material()
+        assert m["detach"].tobytes() == o["detach"].astype(np.float32).tobytes()
+        assert m["mass"].tobytes() == o["mass"].astype(np.float32).tobytes()
+        assert np.float32(m["MOR"]).tobytes() == np.float32(o["MOR"]).tobytes()
+        r.apply_wrench(loads[w][1], loads[w][2], loads[w][3])
+    oracle.step_many(list(refs.values()), 20)
+    gev = {}
+    for e in sim.events():
+        gev.setdefault(e[0], []).append(_key(e))
+    worst = 0.0
+    for w, r in refs.items():
+        e, g, o = _err(sim, r, w)
+        assert g["step"] == 20 and g["status"] == 0
+        assert gev.get(w, []) == [_key(x) for x in r.events()]
+        if not gev.get(w):
+            assert e["max"] <= TOL_RUN, (w, e)
+            worst = max(worst, e["max"])
+    print(f"config 4 full size: 20-step worst relative error on sampled worlds {worst:.2e}; "
+          f"mean PCG iterations {st['cg_iters_total'] / st['world_steps_total']:.2f}; launch {sim.launch_info()}")
+    sim.close()
