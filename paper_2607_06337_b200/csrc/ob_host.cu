@@ -233,6 +233,23 @@ int flush_wrenches(ob_ctx *ctx) {
   return OB_OK;
 }
 
+// rest sag m g / k_s of every apple of one world in fp64 (caller order), from the fp32 constants on the device;
+// apple positions cross the ABI as anchor + sag + u (the kernel stores u = x - x_rest in fp32)
+int fetch_sag(ob_ctx *ctx, int world, std::vector<double> &sag) {
+  const WorldDesc &d = ctx->desc[world];
+  const HostWorld &H = ctx->hw[world];
+  sag.assign(3 * (size_t)d.A, 0.0);
+  if (!d.A) return OB_OK;
+  std::vector<float> km(2 * (size_t)d.Ap);
+  CU(cpy(ctx, km.data(), ctx->dev.apple_blk + d.apple_blk_off + apple_state_bytes(d.Ap) + 3 * 4 * d.Ap,
+         sizeof(float) * km.size(), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  for (int a = 0; a < d.A; a++)
+    for (int k = 0; k < 3; k++)
+      sag[3 * H.int2ext_apple[a] + k] = (double)km[d.Ap + a] * (double)ctx->dev.P.gravity[k] / (double)km[a];
+  return OB_OK;
+}
+
 int check_world(ob_ctx *ctx, int world) {
   if (!ctx) return OB_E_ARG;
   if (world < 0 || world >= ctx->n_worlds) return fail(ctx, OB_E_ARG, "world %d out of range", world);
@@ -576,10 +593,12 @@ int ob_get_state(ob_ctx *ctx, int world, float *q, float *qd, float *apple_x, fl
   }
   const float *as = reinterpret_cast<const float *>(ab.data());
   const unsigned char *af = ab.data() + 6 * 4 * d.Ap;
+  std::vector<double> sag;
+  if (apple_x && (rc = fetch_sag(ctx, world, sag)) != OB_OK) return rc;
   for (int a = 0; a < d.A; a++) {
     const int e = H.int2ext_apple[a];
     for (int k = 0; k < 3; k++) {
-      if (apple_x) apple_x[3 * e + k] = (float)(H.anchor[3 * e + k] + (double)as[k * d.Ap + a]);
+      if (apple_x) apple_x[3 * e + k] = (float)(H.anchor[3 * e + k] + sag[3 * e + k] + (double)as[k * d.Ap + a]);
       if (apple_v) apple_v[3 * e + k] = as[(3 + k) * d.Ap + a];
     }
     if (attached) attached[e] = af[a];
@@ -613,10 +632,12 @@ int ob_set_state(ob_ctx *ctx, int world, const float *q, const float *qd, const 
   }
   float *as = reinterpret_cast<float *>(ab.data());
   unsigned char *af = ab.data() + 6 * 4 * d.Ap;
+  std::vector<double> sag;
+  if (apple_x && (rc = fetch_sag(ctx, world, sag)) != OB_OK) return rc;
   for (int a = 0; a < d.A; a++) {
     const int e = H.int2ext_apple[a];
     for (int k = 0; k < 3; k++) {
-      if (apple_x) as[k * d.Ap + a] = (float)((double)apple_x[3 * e + k] - H.anchor[3 * e + k]);
+      if (apple_x) as[k * d.Ap + a] = (float)((double)apple_x[3 * e + k] - H.anchor[3 * e + k] - sag[3 * e + k]);
       if (apple_v) as[(3 + k) * d.Ap + a] = apple_v[3 * e + k];
     }
     if (attached) { af[a] = attached[e] ? 1 : 0; af[d.Ap + a] = 0; af[2 * d.Ap + a] = 0; }
@@ -642,9 +663,11 @@ int ob_get_apple_x64(ob_ctx *ctx, int world, double *apple_x) {
   CU(cpy(ctx, u.data(), ctx->dev.apple_blk + d.apple_blk_off, sizeof(float) * u.size(), cudaMemcpyDeviceToHost,
                      ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
+  std::vector<double> sag;
+  if ((rc = fetch_sag(ctx, world, sag)) != OB_OK) return rc;
   for (int a = 0; a < d.A; a++) {
     const int e = H.int2ext_apple[a];
-    for (int k = 0; k < 3; k++) apple_x[3 * e + k] = H.anchor[3 * e + k] + (double)u[k * d.Ap + a];
+    for (int k = 0; k < 3; k++) apple_x[3 * e + k] = H.anchor[3 * e + k] + sag[3 * e + k] + (double)u[k * d.Ap + a];
   }
   return OB_OK;
 }

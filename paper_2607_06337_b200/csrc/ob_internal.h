@@ -22,7 +22,7 @@ __host__ __device__ inline int link_state_bytes(int Np) { return kLinkStateFloat
 __host__ __device__ inline int link_block_bytes(int Np) { return link_state_bytes(Np) + kLinkConstFloats * 4 * Np; }
 
 // ---- per-world "apple block":
-//   floats  u[3][Ap] v[3][Ap]              state (u = x - anchor, anchor = rest hang point, fp64 on the host side)
+//   floats  u[3][Ap] v[3][Ap]              state (u = x - x_rest, x_rest = anchor + m g / k_s; anchor = rest hang point, fp64, host side)
 //   bytes   attached[Ap] cA[Ap] cB[Ap]     state
 //   floats  o[3][Ap] k[Ap] m[Ap] c[Ap] fdet[Ap]   constants
 //   int32   link[Ap]                       internal link index

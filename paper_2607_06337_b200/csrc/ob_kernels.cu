@@ -234,8 +234,7 @@ __global__ void k_randomize(DevCtx c, unsigned long long seed, int redraw) {
       ac[5 * d.Ap + a] = d.has_apple_c ? c.apple_c_in[d.apple_base + a]
                                         : (float)(2.0 * (double)P.zeta_s * sqrt((double)k * (double)m));
       ac[6 * d.Ap + a] = fd;
-      // rest sag: u = m g / k_s
-      for (int kk = 0; kk < 3; kk++) as[kk * d.Ap + a] = (float)((double)m * (double)P.gravity[kk] / (double)k);
+      // u = x - (anchor + m g / k_s) stays 0: the apple starts at its rest sag
     }
   }
   if (threadIdx.x == 0) {
@@ -412,9 +411,12 @@ __device__ __forceinline__ void link_topdown_bias(const Sm &s, const DevCtx &c, 
     if (!s.att[a]) continue;
     const float3 o = f3(s.ao[a], s.ao[Ap + a], s.ao[2 * Ap + a]);
     const float3 dh = dp + mul(dR, o);                                   // x_hang - anchor
-    const float3 st = f3(s.u[a], s.u[Ap + a], s.u[2 * Ap + a]) - dh;     // x_a - x_hang
-    const float3 vh = mul(R, vl + cross(om, o));                         // world velocity of the hang point
     const float k = s.ak[a], cdamp = s.ac[a], ma = s.am[a];
+    // x_a - x_hang = u + sag - dh with the rest sag m g / k_s (u is stored relative to the rest position)
+    const float gk = ma / k;
+    const float3 st = f3(s.u[a] + (gk * P.gravity[0] - dh.x), s.u[Ap + a] + (gk * P.gravity[1] - dh.y),
+                         s.u[2 * Ap + a] + (gk * P.gravity[2] - dh.z));
+    const float3 vh = mul(R, vl + cross(om, o));                         // world velocity of the hang point
     const float3 fs = (-k) * st;
     const float3 va = f3(s.v[a], s.v[Ap + a], s.v[2 * Ap + a]);
     s.ft[a] = fs.x - cdamp * va.x; s.ft[Ap + a] = fs.y - cdamp * va.y; s.ft[2 * Ap + a] = fs.z - cdamp * va.z;
