@@ -8,8 +8,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libob.so")
-SOURCES = ["ob_host.cu", "ob_kernels.cu"]
-HEADERS = ["ob_internal.h", os.path.join("..", "..", "include", "orchard.h")]
+SOURCES = ["ob_host.cu", "ob_kernels.cu", "ob_step.cu"]
+HEADERS = ["ob_internal.h", "ob_device.h", os.path.join("..", "..", "include", "orchard.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--use_fast_math=false", "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
 

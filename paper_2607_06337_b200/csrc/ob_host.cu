@@ -16,7 +16,6 @@ using namespace ob;
 namespace {
 
 constexpr size_t kAlign = 256;
-constexpr int kBlock = 256;
 constexpr int kMaxSmem = 227 * 1024 - 2048;   // per-CTA limit minus the kernel's static shared memory
 const char *kNullCtx = "null context";
 
@@ -44,7 +43,9 @@ struct ob_ctx {
   cudaEvent_t staging_ev[2] = {nullptr, nullptr};
   int staging_next = 0;
   unsigned char *dev_base = nullptr;
-  int grid = 0, block = kBlock, smem = 0, launches = 0;
+  // k_step launch geometry per size class: worlds [cls_off, cls_off + cls_n) of the order list
+  int cls_off[kNumClasses] = {}, cls_n[kNumClasses] = {}, cls_grid[kNumClasses] = {}, cls_smem[kNumClasses] = {};
+  int main_cls = 0, launches = 0;
   int max_Np = 0, max_Ap = 0;
   size_t ev_cap = 0;
   uint64_t h2d_bytes = 0, d2h_bytes = 0, kernel_launches = 0, step_calls = 0;
@@ -171,11 +172,11 @@ int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) 
     const int Np = pad16(s.n_links), Ap = pad16(s.n_apples), nlev = (int)lev.size() - 1;
     L.sumNp += Np; L.sumAp += Ap; L.sumLev += nlev + 1;
     L.max_Np = std::max(L.max_Np, Np); L.max_Ap = std::max(L.max_Ap, Ap);
-    const int sm = step_smem_bytes(Np, Ap, nlev);
-    if (sm > kMaxSmem) {
+    const int sm = step_smem_bytes(Np, Ap);
+    if (sm > kMaxSmem || step_class_of(Np) < 0) {
       char b[200];
-      snprintf(b, sizeof(b), "world %d (%d links, %d apples) needs %d B of shared memory, limit %d", w, s.n_links,
-               s.n_apples, sm, kMaxSmem);
+      snprintf(b, sizeof(b), "world %d (%d links, %d apples) does not fit on chip: %d B of shared memory (limit %d), "
+               "%d links (limit %d)", w, s.n_links, s.n_apples, sm, kMaxSmem, s.n_links, kMaxLinksOnChip);
       why = b;
       return OB_E_CAPACITY;
     }
@@ -206,7 +207,7 @@ int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) 
   take(L, L.wrench, sizeof(WrenchSlots) * n_worlds);
   take(L, L.events, sizeof(ob_event) * L.ev_cap);
   take(L, L.ev_count, sizeof(int32_t) * 4);
-  take(L, L.queue, sizeof(int32_t) * 4);
+  take(L, L.queue, sizeof(int32_t) * 2 * kNumClasses);
   take(L, L.pose7, sizeof(float) * 7 * L.max_Np);
   L.total = (L.total + kAlign - 1) / kAlign * kAlign;
   return OB_OK;
@@ -347,6 +348,9 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
 
     WorldDesc &d = ctx->desc[w];
     d.N = N; d.A = A; d.Np = Np; d.Ap = Ap; d.n_levels = nlev;
+    d.n_top = 0;
+    while (d.n_top < nlev && lev[d.n_top + 1] <= 32) d.n_top++;
+    d.cls = step_class_of(Np);
     d.link_base = (int32_t)link_base; d.apple_base = (int32_t)apple_base; d.level_base = (int32_t)lev_base;
     d.link_blk_off = (int64_t)link_off; d.apple_blk_off = (int64_t)apple_off;
     d.density = s.density; d.E = s.E; d.MOR = s.MOR;
@@ -363,11 +367,14 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
       if (n_apple[l] == 0) first_apple[l] = a;
       n_apple[l]++;
     }
-    float *lconst = reinterpret_cast<float *>(h_link.data() + link_off + link_state_bytes(Np));
+    std::vector<int32_t> level_of(N, 0);
+    for (int l = 0; l < nlev; l++)
+      for (int i = lev[l]; i < lev[l + 1]; i++) level_of[i] = l;
     for (int i = 0; i < N; i++) {
       const int e = H.int2ext_link[i];
       const int p = e == 0 ? -1 : H.ext2int_link[s.parent[e]];
-      h_topo[link_base + i] = make_int4(p, first_child[i], n_child[i] | (n_apple[i] << 16), first_apple[i]);
+      h_topo[link_base + i] = make_int4(p, first_child[i], n_child[i] | (n_apple[i] << 16),
+                                        first_apple[i] | (level_of[i] << 16));
       const float *q = s.rest_quat + 4 * e;
       const double n = std::sqrt((double)q[0] * q[0] + (double)q[1] * q[1] + (double)q[2] * q[2] + (double)q[3] * q[3]);
       h_quat[link_base + i] = make_float4((float)(q[0] / n), (float)(q[1] / n), (float)(q[2] / n), (float)(q[3] / n));
@@ -379,7 +386,6 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
         h_arm[2 * link_base + i] = s.armature[2 * e];
         h_arm[2 * link_base + Np + i] = s.armature[2 * e + 1];
       }
-      (void)lconst;
     }
     for (int l = 0; l <= nlev; l++) h_lev[lev_base + l] = lev[l];
     unsigned char *ab = h_apple.data() + apple_off;
@@ -402,8 +408,16 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
     link_off += link_block_bytes(Np); apple_off += apple_block_bytes(Ap);
     h_order[w] = w;
   }
-  // work-queue order: largest worlds first (longest-processing-time rule for heterogeneous batches)
-  std::stable_sort(h_order.begin(), h_order.end(), [&](int a, int b) { return ctx->desc[a].N > ctx->desc[b].N; });
+  // work-queue order: grouped by size class, largest worlds first inside a class (longest-processing-time rule)
+  std::stable_sort(h_order.begin(), h_order.end(), [&](int a, int b) {
+    if (ctx->desc[a].cls != ctx->desc[b].cls) return ctx->desc[a].cls < ctx->desc[b].cls;
+    return ctx->desc[a].N > ctx->desc[b].N;
+  });
+  for (int k = 0; k < n_worlds; k++) {
+    const WorldDesc &d = ctx->desc[h_order[k]];
+    if (ctx->cls_n[d.cls]++ == 0) ctx->cls_off[d.cls] = k;
+    ctx->cls_smem[d.cls] = std::max(ctx->cls_smem[d.cls], step_smem_bytes(d.Np, d.Ap));
+  }
 
   DevCtx &D = ctx->dev;
   D.n_worlds = n_worlds;
@@ -454,13 +468,17 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   if (e == cudaSuccess) e = launch_randomize(D, 0ull, 0, ctx->stream);
   ctx->kernel_launches += 2;
   // launch geometry of k_step
-  ctx->smem = L.max_smem;
-  int per_sm = 0, n_sm = 0, dev = 0;
-  if (e == cudaSuccess) e = step_kernel_setup(ctx->smem, ctx->block, &per_sm);
+  int n_sm = 0, dev = 0;
   if (e == cudaSuccess) e = cudaGetDevice(&dev);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-  if (e == cudaSuccess && per_sm < 1) e = cudaErrorInvalidConfiguration;
-  ctx->grid = std::max(1, std::min(n_worlds, n_sm * std::max(per_sm, 1)));
+  for (int k = 0; k < kNumClasses && e == cudaSuccess; k++) {
+    if (!ctx->cls_n[k]) continue;
+    int per_sm = 0;
+    e = step_kernel_setup(k, ctx->cls_smem[k], &per_sm);
+    if (e == cudaSuccess && per_sm < 1) e = cudaErrorInvalidConfiguration;
+    ctx->cls_grid[k] = std::max(1, std::min(ctx->cls_n[k], n_sm * std::max(per_sm, 1)));
+    if (ctx->cls_n[k] > ctx->cls_n[ctx->main_cls]) ctx->main_cls = k;
+  }
   for (int k = 0; k < 2 && e == cudaSuccess; k++) {
     e = cudaHostAlloc((void **)&ctx->staging[k], sizeof(WrenchSlots) * n_worlds, cudaHostAllocDefault);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->staging_ev[k], cudaEventDisableTiming);
@@ -553,10 +571,15 @@ int ob_step(ob_ctx *ctx, int n) {
   if (n == 0) return OB_OK;
   int rc = flush_wrenches(ctx);
   if (rc != OB_OK) return rc;
-  CU(cudaMemsetAsync(ctx->dev.queue, 0, sizeof(int32_t), ctx->stream));
-  CU(launch_step(ctx->dev, n, ctx->grid, ctx->block, ctx->smem, ctx->stream));
-  ctx->launches = 1;
-  ctx->kernel_launches += 1;
+  CU(cudaMemsetAsync(ctx->dev.queue, 0, sizeof(int32_t) * kNumClasses, ctx->stream));
+  ctx->launches = 0;
+  for (int k = kNumClasses - 1; k >= 0; k--) {      // the class of the largest worlds first
+    if (!ctx->cls_n[k]) continue;
+    CU(launch_step(ctx->dev, k, ctx->dev.order + ctx->cls_off[k], ctx->cls_n[k], ctx->dev.queue + k, n,
+                   ctx->cls_grid[k], ctx->cls_smem[k], ctx->stream));
+    ctx->launches += 1;
+    ctx->kernel_launches += 1;
+  }
   ctx->step_calls += 1;
   return OB_OK;
 }
@@ -790,9 +813,9 @@ int ob_stats(ob_ctx *ctx, uint64_t *cg_iters_total, uint64_t *world_steps_total,
 int ob_launch_info(ob_ctx *ctx, int32_t *n_launches, int32_t *grid, int32_t *block, int32_t *smem_bytes) {
   if (!ctx) return OB_E_ARG;
   if (n_launches) *n_launches = ctx->launches;
-  if (grid) *grid = ctx->grid;
-  if (block) *block = ctx->block;
-  if (smem_bytes) *smem_bytes = ctx->smem;
+  if (grid) *grid = ctx->cls_grid[ctx->main_cls];
+  if (block) *block = kStepClasses[ctx->main_cls].nt;
+  if (smem_bytes) *smem_bytes = ctx->cls_smem[ctx->main_cls];
   return OB_OK;
 }
 

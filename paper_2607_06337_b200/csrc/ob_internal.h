@@ -32,6 +32,8 @@ __host__ __device__ inline int apple_block_bytes(int Ap) { return apple_state_by
 struct WorldDesc {
   int32_t N, A, Np, Ap;
   int32_t n_levels;
+  int32_t n_top;        // leading levels whose links all lie in [0, 32): swept by warp 0 with __syncwarp only
+  int32_t cls;          // size class (index into kStepClasses)
   int32_t link_base;    // sum of Np of the worlds before this one
   int32_t apple_base;   // sum of Ap
   int32_t level_base;   // offset into the level-offset pool (n_levels + 1 entries)
@@ -63,11 +65,12 @@ static_assert(sizeof(WrenchSlots) % 16 == 0, "WrenchSlots must stay 16-byte size
 struct DevCtx {
   int32_t n_worlds;
   const WorldDesc *desc;
-  const int32_t *order;          // worlds sorted by size, largest first (work queue order)
+  const int32_t *order;          // worlds grouped by size class, largest first inside a class (work queues)
   unsigned char *link_blk;       // link-block pool
   unsigned char *apple_blk;      // apple-block pool
   // per-link statics, indexed link_base + i (SoA pools use k * Np + i inside the world's slice)
-  const int4 *topo;              // x = parent, y = first child, z = n_children | n_apples << 16, w = first apple
+  const int4 *topo;              // x = parent, y = first child, z = n_children | n_apples << 16,
+                                 // w = first apple | level << 16
   const float4 *quat;            // rest quaternion (w,x,y,z), normalised in fp64 then rounded (k_step)
   const float4 *quat_raw;        // rest quaternion exactly as the caller gave it (create-time fp64 rest pose)
   float *R0;                     // [9 * link_base + k * Np + i] rest world rotation, row-major k
@@ -86,29 +89,43 @@ struct DevCtx {
   ob_event *events;
   int32_t ev_cap;
   int32_t *ev_count;             // [0] = appended, [1] = overflow flag
-  int32_t *queue;                // work-queue counter
+  int32_t *queue;                // work-queue counters, one per size class
   float *pose7;                  // scratch for ob_get_state(link_pose7): 7 * max Np floats
   ob_params P;
 };
 
+// ---- k_step size classes: threads per CTA x links per thread (a thread owns the same links for the whole
+//      launch and keeps their joint transform, inertia, diagonal and PCG vectors in registers)
+struct StepClass { int nt, lpt, min_ctas; };
+constexpr int kNumClasses = 4;
+constexpr StepClass kStepClasses[kNumClasses] = {{256, 1, 3}, {256, 2, 2}, {512, 2, 1}, {512, 3, 1}};
+constexpr int kMaxLinksOnChip = 512 * 3;
+inline int step_class_of(int Np) {   // host only
+  for (int k = 0; k < kNumClasses; k++)
+    if (Np <= kStepClasses[k].nt * kStepClasses[k].lpt) return k;
+  return -1;
+}
+
 // shared-memory footprint of one world in k_step (bytes); the host uses it to size the launch
-__host__ __device__ inline int step_smem_bytes(int Np, int Ap, int n_levels) {
+//   link block | apple block | scratch float4[6][Np] | f_tether, f_user [3][Ap], |f_s|, |f_user| [Ap] |
+//   wrench slots | snapped[Np]
+__host__ __device__ inline int step_smem_bytes(int Np, int Ap) {
   int b = 0;
   b += link_block_bytes(Np);
   b += apple_block_bytes(Ap);
-  b += (9 + 2 + 6 + 24) * 4 * Np;   // E, (c2,s2), mailbox, scratch (aliases invd/r/p/Ap + 16)
-  b += Np;                          // snapped
-  b += (3 + 3 + 2) * 4 * Ap;        // f_tether, f_user, |f_s|, |f_user|
-  b += ((n_levels + 1 + 3) / 4 * 4) * 4;
+  b += 6 * 16 * Np;
+  b += (3 + 3 + 2) * 4 * Ap;
   b += (int)sizeof(WrenchSlots);
+  b += Np;
   return (b + 127) / 128 * 128;
 }
 
 // kernel launchers (ob_kernels.cu)
 cudaError_t launch_rest_pose(const DevCtx &c, int total_links_padded, int total_apples_padded, cudaStream_t s);
 cudaError_t launch_randomize(const DevCtx &c, unsigned long long seed, int redraw, cudaStream_t s);
-cudaError_t launch_step(const DevCtx &c, int n_steps, int grid, int block, int smem, cudaStream_t s);
+cudaError_t launch_step(const DevCtx &c, int cls, const int32_t *order, int n_in_class, int32_t *queue, int n_steps,
+                        int grid, int smem, cudaStream_t s);
 cudaError_t launch_pose(const DevCtx &c, int world, cudaStream_t s);
-cudaError_t step_kernel_setup(int smem_bytes, int block, int *max_blocks_per_sm);
+cudaError_t step_kernel_setup(int cls, int smem_bytes, int *max_blocks_per_sm);
 
 }  // namespace ob
