@@ -112,8 +112,8 @@ def _workload(config: int, n_worlds: int):
 
 
 def _loads_arrays(specs, epoch, f_lo, f_hi):
-    from workloads import wrench_process
-    loads = wrench_process(specs, epoch, f_lo, f_hi)
+    from workloads import wrench_epoch_loads
+    loads = wrench_epoch_loads(specs, epoch, f_lo, f_hi)      # clears of epoch - 1, then the new wrenches
     return (np.array([l[0] for l in loads], np.int32), np.array([l[1] for l in loads], np.int32),
             np.array([l[2] for l in loads], np.float32), np.array([l[3] for l in loads], np.float32))
 

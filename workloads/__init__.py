@@ -21,4 +21,5 @@ from .loads import (  # noqa: F401
     config1_loads,
     config2_pulls,
     wrench_process,
+    wrench_epoch_loads,
 )

@@ -76,3 +76,20 @@ def wrench_process(specs: Sequence[WorldSpec], epoch: int, f_lo: float, f_hi: fl
         out.append((w, link, (float(p[0]), float(p[1]), float(p[2])),
                     (float(f[0]), float(f[1]), float(f[2]))))
     return out
+
+
+def wrench_epoch_loads(specs: Sequence[WorldSpec], epoch: int, f_lo: float, f_hi: float,
+                       seed_offset: int = 3000) -> List[Load]:
+    """The A25 process as a stream of `ob_apply_wrench` calls: "resampled" means
+    the wrench of epoch - 1 is withdrawn (a zero force frees its slot, reading
+    A24) before the wrench of this epoch is applied, so every world carries
+    exactly one external wrench at any time.  Clears come first, world by
+    world, and are skipped where the new wrench lands on the same link (same
+    body replaces)."""
+    new = wrench_process(specs, epoch, f_lo, f_hi, seed_offset)
+    if epoch == 0:
+        return new
+    old = wrench_process(specs, epoch - 1, f_lo, f_hi, seed_offset)
+    zero = (0.0, 0.0, 0.0)
+    clears = [(w, body, zero, zero) for (w, body, _p, _f), (_w, nbody, _np, _nf) in zip(old, new) if body != nbody]
+    return clears + new
