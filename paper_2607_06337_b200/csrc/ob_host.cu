@@ -127,8 +127,10 @@ int validate(const ob_world_spec *specs, int n_worlds, const ob_params *P, std::
   return OB_OK;
 }
 
-// level (BFS) order: parents before children, links of one level contiguous, children of one parent contiguous
-void bfs_order(const ob_world_spec &s, std::vector<int32_t> &int2ext, std::vector<int32_t> &level_off) {
+// level order: parents before children, links of one level contiguous and, inside a level, the links WITH
+// children first (a warp of k_step then holds either inner links or leaves, not a mix).  Returns the number of
+// links with children.
+int level_order(const ob_world_spec &s, std::vector<int32_t> &int2ext, std::vector<int32_t> &level_off) {
   const int N = s.n_links;
   std::vector<std::vector<int32_t>> kids(N);
   for (int i = 1; i < N; i++) kids[s.parent[i]].push_back(i);
@@ -138,18 +140,26 @@ void bfs_order(const ob_world_spec &s, std::vector<int32_t> &int2ext, std::vecto
   level_off.push_back(0);
   int2ext.push_back(0);
   size_t begin = 0;
+  int n_inner = 0;
   while (begin < int2ext.size()) {
     size_t end = int2ext.size();
     level_off.push_back((int32_t)end);
-    for (size_t k = begin; k < end; k++)
-      for (int32_t ch : kids[int2ext[k]]) int2ext.push_back(ch);
+    std::vector<int32_t> next;
+    for (size_t k = begin; k < end; k++) {
+      if (!kids[int2ext[k]].empty()) n_inner++;
+      for (int32_t ch : kids[int2ext[k]]) next.push_back(ch);
+    }
+    std::stable_partition(next.begin(), next.end(), [&](int32_t e) { return !kids[e].empty(); });
+    int2ext.insert(int2ext.end(), next.begin(), next.end());
     begin = end;
   }
+  return n_inner;
 }
+inline int pad8(int n) { return (n + 7) / 8 * 8; }
 
 struct Layout {
   size_t total = 0;
-  Pool desc, order, link_blk, apple_blk, topo, quat, quat_raw, R0, Mmax, Lown, diam, arm, link_ext, apple_ext, apple_nom,
+  Pool desc, order, link_blk, apple_blk, topo, topo2, child_list, quat, quat_raw, R0, Mmax, Lown, diam, arm, link_ext, apple_ext, apple_nom,
       apple_c, anchor, level_off, info, wrench, events, ev_count, queue, pose7;
   size_t sumNp = 0, sumAp = 0, sumLev = 0, ev_cap = 0;
   int max_Np = 0, max_Ap = 0, max_smem = 0;
@@ -168,11 +178,11 @@ int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) 
   for (int w = 0; w < n_worlds; w++) {
     const ob_world_spec &s = specs[w];
     std::vector<int32_t> i2e, lev;
-    bfs_order(s, i2e, lev);
+    const int NIp = pad8(level_order(s, i2e, lev));
     const int Np = pad16(s.n_links), Ap = pad16(s.n_apples), nlev = (int)lev.size() - 1;
     L.sumNp += Np; L.sumAp += Ap; L.sumLev += nlev + 1;
     L.max_Np = std::max(L.max_Np, Np); L.max_Ap = std::max(L.max_Ap, Ap);
-    const int sm = step_smem_bytes(Np, Ap);
+    const int sm = step_smem_bytes(Np, Ap, NIp);
     if (sm > kMaxSmem || step_class_of(Np) < 0) {
       char b[200];
       snprintf(b, sizeof(b), "world %d (%d links, %d apples) does not fit on chip: %d B of shared memory (limit %d), "
@@ -190,6 +200,8 @@ int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) 
   take(L, L.link_blk, (size_t)link_block_bytes(1) * L.sumNp);
   take(L, L.apple_blk, (size_t)apple_block_bytes(1) * std::max<size_t>(L.sumAp, 16));
   take(L, L.topo, sizeof(int4) * L.sumNp);
+  take(L, L.topo2, sizeof(int4) * L.sumNp);
+  take(L, L.child_list, sizeof(int32_t) * L.sumNp);
   take(L, L.quat, sizeof(float4) * L.sumNp);
   take(L, L.quat_raw, sizeof(float4) * L.sumNp);
   take(L, L.R0, sizeof(float) * 9 * L.sumNp);
@@ -322,7 +334,8 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
 
   // ---- host images of every pool ----
   std::vector<unsigned char> h_link(L.link_blk.bytes, 0), h_apple(L.apple_blk.bytes, 0);
-  std::vector<int4> h_topo(L.sumNp, make_int4(-1, 0, 0, 0));
+  std::vector<int4> h_topo(L.sumNp, make_int4(-1, -1, -1, 0xfff)), h_topo2(L.sumNp, make_int4(0, -1, 0, 0));
+  std::vector<int32_t> h_child(L.sumNp, 0);
   std::vector<float4> h_quat(L.sumNp, make_float4(1.f, 0.f, 0.f, 0.f)), h_quat_raw(L.sumNp, make_float4(1.f, 0.f, 0.f, 0.f));
   std::vector<float> h_Lown(L.sumNp, 1.f), h_diam(L.sumNp, 1.f), h_arm(L.any_arm ? 2 * L.sumNp : 0, 0.f);
   std::vector<int32_t> h_link_ext(L.sumNp, 0), h_apple_ext(std::max<size_t>(L.sumAp, 16), 0), h_lev(L.sumLev, 0);
@@ -333,7 +346,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
     const ob_world_spec &s = specs[w];
     HostWorld &H = ctx->hw[w];
     std::vector<int32_t> lev;
-    bfs_order(s, H.int2ext_link, lev);
+    const int n_inner = level_order(s, H.int2ext_link, lev);
     const int N = s.n_links, A = s.n_apples, Np = pad16(N), Ap = pad16(A), nlev = (int)lev.size() - 1;
     H.ext2int_link.assign(N, 0);
     for (int i = 0; i < N; i++) H.ext2int_link[H.int2ext_link[i]] = i;
@@ -347,7 +360,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
     for (int a = 0; a < A; a++) H.ext2int_apple[H.int2ext_apple[a]] = a;
 
     WorldDesc &d = ctx->desc[w];
-    d.N = N; d.A = A; d.Np = Np; d.Ap = Ap; d.n_levels = nlev;
+    d.N = N; d.A = A; d.Np = Np; d.Ap = Ap; d.NIp = pad8(n_inner); d.n_levels = nlev;
     d.n_top = 0;
     while (d.n_top < nlev && lev[d.n_top + 1] <= 32) d.n_top++;
     d.cls = step_class_of(Np);
@@ -356,11 +369,17 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
     d.density = s.density; d.E = s.E; d.MOR = s.MOR;
     d.has_apple_c = s.apple_c ? 1 : 0;
 
-    std::vector<int32_t> first_child(N, 0), n_child(N, 0), first_apple(N, 0), n_apple(N, 0);
+    std::vector<int32_t> n_child(N, 0), first_apple(N, 0), n_apple(N, 0), cl_off(N, 0), islot(N, 0xffff), par(N, -1);
+    std::vector<std::vector<int32_t>> kids(N);
     for (int i = 1; i < N; i++) {
-      const int p = H.ext2int_link[s.parent[H.int2ext_link[i]]];
-      if (n_child[p] == 0) first_child[p] = i;
-      n_child[p]++;
+      par[i] = H.ext2int_link[s.parent[H.int2ext_link[i]]];
+      kids[par[i]].push_back(i);          // ascending internal index: a fixed summation order
+    }
+    for (int i = 0, off = 0, slot = 0; i < N; i++) {
+      n_child[i] = (int32_t)kids[i].size();
+      cl_off[i] = off;
+      for (int32_t ch : kids[i]) h_child[link_base + off++] = ch;
+      if (n_child[i]) islot[i] = slot++;
     }
     for (int a = 0; a < A; a++) {
       const int l = H.ext2int_link[s.apple_link[H.int2ext_apple[a]]];
@@ -372,9 +391,12 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
       for (int i = lev[l]; i < lev[l + 1]; i++) level_of[i] = l;
     for (int i = 0; i < N; i++) {
       const int e = H.int2ext_link[i];
-      const int p = e == 0 ? -1 : H.ext2int_link[s.parent[e]];
-      h_topo[link_base + i] = make_int4(p, first_child[i], n_child[i] | (n_apple[i] << 16),
-                                        first_apple[i] | (level_of[i] << 16));
+      const int p = par[i];
+      auto kid = [&](int c) { return c < n_child[i] ? kids[i][c] : 0xffff; };
+      h_topo[link_base + i] = make_int4(p, kid(0) | (kid(1) << 16), kid(2) | (kid(3) << 16),
+                                        level_of[i] | (std::min(n_child[i], 5) << 12));
+      h_topo2[link_base + i] = make_int4(first_apple[i] | (n_apple[i] << 16),
+                                         islot[i] | ((p >= 0 ? islot[p] : 0xffff) << 16), cl_off[i], n_child[i]);
       const float *q = s.rest_quat + 4 * e;
       const double n = std::sqrt((double)q[0] * q[0] + (double)q[1] * q[1] + (double)q[2] * q[2] + (double)q[3] * q[3]);
       h_quat[link_base + i] = make_float4((float)(q[0] / n), (float)(q[1] / n), (float)(q[2] / n), (float)(q[3] / n));
@@ -416,7 +438,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   for (int k = 0; k < n_worlds; k++) {
     const WorldDesc &d = ctx->desc[h_order[k]];
     if (ctx->cls_n[d.cls]++ == 0) ctx->cls_off[d.cls] = k;
-    ctx->cls_smem[d.cls] = std::max(ctx->cls_smem[d.cls], step_smem_bytes(d.Np, d.Ap));
+    ctx->cls_smem[d.cls] = std::max(ctx->cls_smem[d.cls], step_smem_bytes(d.Np, d.Ap, d.NIp));
   }
 
   DevCtx &D = ctx->dev;
@@ -426,6 +448,8 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   D.link_blk = base + L.link_blk.off;
   D.apple_blk = base + L.apple_blk.off;
   D.topo = reinterpret_cast<int4 *>(base + L.topo.off);
+  D.topo2 = reinterpret_cast<int4 *>(base + L.topo2.off);
+  D.child_list = reinterpret_cast<int32_t *>(base + L.child_list.off);
   D.quat = reinterpret_cast<float4 *>(base + L.quat.off);
   D.quat_raw = reinterpret_cast<float4 *>(base + L.quat_raw.off);
   D.R0 = reinterpret_cast<float *>(base + L.R0.off);
@@ -459,7 +483,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   } while (0)
   cudaError_t e = cudaMemsetAsync(base, 0, L.total, ctx->stream);
   if (e != cudaSuccess) { g_err = cudaGetErrorString(e); delete ctx; return OB_E_CUDA; }
-  UP(L.desc, ctx->desc); UP(L.order, h_order); UP(L.link_blk, h_link); UP(L.apple_blk, h_apple); UP(L.topo, h_topo);
+  UP(L.desc, ctx->desc); UP(L.order, h_order); UP(L.link_blk, h_link); UP(L.apple_blk, h_apple); UP(L.topo, h_topo); UP(L.topo2, h_topo2); UP(L.child_list, h_child);
   UP(L.quat, h_quat); UP(L.quat_raw, h_quat_raw); UP(L.Lown, h_Lown); UP(L.diam, h_diam); UP(L.arm, h_arm); UP(L.link_ext, h_link_ext);
   UP(L.apple_ext, h_apple_ext); UP(L.apple_nom, h_nom); UP(L.apple_c, h_c); UP(L.level_off, h_lev);
 #undef UP
@@ -609,8 +633,8 @@ int ob_get_state(ob_ctx *ctx, int world, float *q, float *qd, float *apple_x, fl
   const unsigned char *fl = lb.data() + kLinkStateFloats * 4 * d.Np;
   for (int i = 0; i < d.N; i++) {
     const int e = H.int2ext_link[i];
-    if (q) { q[2 * e] = st[i]; q[2 * e + 1] = st[d.Np + i]; }
-    if (qd) { qd[2 * e] = st[2 * d.Np + i]; qd[2 * e + 1] = st[3 * d.Np + i]; }
+    if (q) { q[2 * e] = st[2 * i]; q[2 * e + 1] = st[2 * i + 1]; }
+    if (qd) { qd[2 * e] = st[2 * d.Np + 2 * i]; qd[2 * e + 1] = st[2 * d.Np + 2 * i + 1]; }
     if (ruptured) ruptured[e] = fl[i];
     if (link_pose7) std::memcpy(link_pose7 + 7 * e, pose.data() + 7 * i, 7 * sizeof(float));
   }
@@ -648,9 +672,9 @@ int ob_set_state(ob_ctx *ctx, int world, const float *q, const float *qd, const 
   unsigned char *fl = lb.data() + kLinkStateFloats * 4 * d.Np;
   for (int i = 0; i < d.N; i++) {
     const int e = H.int2ext_link[i];
-    if (q) { st[i] = q[2 * e]; st[d.Np + i] = q[2 * e + 1]; }
-    if (qd) { st[2 * d.Np + i] = qd[2 * e]; st[3 * d.Np + i] = qd[2 * e + 1]; }
-    st[4 * d.Np + i] = 0.f; st[5 * d.Np + i] = 0.f;          // warm start cleared
+    if (q) { st[2 * i] = q[2 * e]; st[2 * i + 1] = q[2 * e + 1]; }
+    if (qd) { st[2 * d.Np + 2 * i] = qd[2 * e]; st[2 * d.Np + 2 * i + 1] = qd[2 * e + 1]; }
+    st[4 * d.Np + 2 * i] = 0.f; st[4 * d.Np + 2 * i + 1] = 0.f;          // warm start cleared
     if (ruptured) { fl[i] = ruptured[e] ? 1 : 0; fl[d.Np + i] = 0; }
   }
   float *as = reinterpret_cast<float *>(ab.data());

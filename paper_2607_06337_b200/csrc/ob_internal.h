@@ -11,11 +11,13 @@ namespace ob {
 constexpr int kPad = 16;  // links and apples per world are padded to a multiple of 16 (16-byte TMA granules)
 __host__ __device__ inline int pad16(int n) { return (n + kPad - 1) / kPad * kPad; }
 
-// ---- per-world "link block" in global memory: one contiguous chunk, staged to shared memory by one TMA
-//      bulk copy and written back (state part only) by one bulk store.
-//   floats  q0[Np] q1[Np] qd0[Np] qd1[Np] x0[Np] x1[Np]      state (x = previous dqd, the PCG warm start)
-//   bytes   ruptured[Np] rc[Np]                               state
-//   floats  K[Np] m[Np] mc[Np] Io[Np] Iz[Np] rz[Np]           constants (after ob_randomize)
+// ---- per-world "link block" in global memory: one contiguous chunk; its state part is staged to shared
+//      memory by one TMA bulk copy and written back by one bulk store, its constants are read from L2 once
+//      per step (they are consumed straight into registers).
+//   float2  q[Np] qd[Np] x[Np]          state, the two DoF of a joint interleaved (x = previous dqd, PCG warm start)
+//   bytes   ruptured[Np] rc[Np]         state
+//   float4  c4[Np] = (m, m c, I about the joint, I_zz)   constants (after ob_randomize)
+//   floats  K[Np] rz[Np]                constants (joint stiffness Eq. 4, parent length)
 constexpr int kLinkStateFloats = 6;
 constexpr int kLinkConstFloats = 6;
 __host__ __device__ inline int link_state_bytes(int Np) { return kLinkStateFloats * 4 * Np + 2 * Np; }
@@ -31,6 +33,7 @@ __host__ __device__ inline int apple_block_bytes(int Ap) { return apple_state_by
 
 struct WorldDesc {
   int32_t N, A, Np, Ap;
+  int32_t NIp;          // links with children, padded to a multiple of 8 (phase-A overflow mailbox)
   int32_t n_levels;
   int32_t n_top;        // leading levels whose links all lie in [0, 32): swept by warp 0 with __syncwarp only
   int32_t cls;          // size class (index into kStepClasses)
@@ -41,6 +44,7 @@ struct WorldDesc {
   int64_t apple_blk_off;  // byte offset of the apple block in the apple-block pool
   float density, E, MOR;  // nominal (spec) values
   int32_t has_apple_c;
+  int32_t pad_[3];
 };
 
 struct WorldInfo {       // mutable per-world scalars
@@ -69,8 +73,11 @@ struct DevCtx {
   unsigned char *link_blk;       // link-block pool
   unsigned char *apple_blk;      // apple-block pool
   // per-link statics, indexed link_base + i (SoA pools use k * Np + i inside the world's slice)
-  const int4 *topo;              // x = parent, y = first child, z = n_children | n_apples << 16,
-                                 // w = first apple | level << 16
+  const int4 *topo;              // x = parent (-1 = trunk), y = child0 | child1 << 16, z = child2 | child3 << 16
+                                 // (0xffff = none), w = level | min(n_children, 5) << 12
+  const int4 *topo2;             // x = first apple | n_apples << 16, y = inner slot | parent's inner slot << 16,
+                                 // z = offset of this link's children in child_list, w = n_children
+  const int32_t *child_list;     // [link_base + z + c] children of every link (internal indices), CSR
   const float4 *quat;            // rest quaternion (w,x,y,z), normalised in fp64 then rounded (k_step)
   const float4 *quat_raw;        // rest quaternion exactly as the caller gave it (create-time fp64 rest pose)
   float *R0;                     // [9 * link_base + k * Np + i] rest world rotation, row-major k
@@ -94,11 +101,12 @@ struct DevCtx {
   ob_params P;
 };
 
-// ---- k_step size classes: threads per CTA x links per thread (a thread owns the same links for the whole
-//      launch and keeps their joint transform, inertia, diagonal and PCG vectors in registers)
+// ---- k_step size classes: threads per CTA x links per thread x CTAs per SM the registers are budgeted for.
+//      A thread owns the same links for the whole launch (link i <-> slot i / NT of thread i % NT) and keeps
+//      their joint transform, inertia, diagonal terms and the PCG search direction in registers.
 struct StepClass { int nt, lpt, min_ctas; };
 constexpr int kNumClasses = 4;
-constexpr StepClass kStepClasses[kNumClasses] = {{256, 1, 3}, {256, 2, 2}, {512, 2, 1}, {512, 3, 1}};
+constexpr StepClass kStepClasses[kNumClasses] = {{128, 2, 6}, {128, 4, 4}, {256, 4, 2}, {512, 3, 1}};
 constexpr int kMaxLinksOnChip = 512 * 3;
 inline int step_class_of(int Np) {   // host only
   for (int k = 0; k < kNumClasses; k++)
@@ -107,13 +115,17 @@ inline int step_class_of(int Np) {   // host only
 }
 
 // shared-memory footprint of one world in k_step (bytes); the host uses it to size the launch
-//   link block | apple block | scratch float4[6][Np] | f_tether, f_user [3][Ap], |f_s|, |f_user| [Ap] |
-//   wrench slots | snapped[Np]
-__host__ __device__ inline int step_smem_bytes(int Np, int Ap) {
+//   link state | apple block | scratch: four float4 planes [4][Np + 1] + overflow float4 [2][NIp] |
+//   f_tether, f_user [3][Ap], |f_s|, |f_user| [Ap] | wrench slots | snapped[Np]
+// The scratch planes carry, phase by phase (ob_step.cu): the parent -> child mailbox of the top-down bias pass
+// (24 floats per link WITH children: planes 0-3 + overflow), the child -> parent mailboxes of the bottom-up
+// passes, and the PCG vectors r, 1/diag, A p.
+__host__ __device__ inline int step_scratch_bytes(int Np, int NIp) { return 64 * (Np + 1) + 32 * NIp; }
+__host__ __device__ inline int step_smem_bytes(int Np, int Ap, int NIp) {
   int b = 0;
-  b += link_block_bytes(Np);
+  b += link_state_bytes(Np);
   b += apple_block_bytes(Ap);
-  b += 6 * 16 * Np;
+  b += step_scratch_bytes(Np, NIp);
   b += (3 + 3 + 2) * 4 * Ap;
   b += (int)sizeof(WrenchSlots);
   b += Np;

@@ -114,15 +114,16 @@ __global__ void k_randomize(DevCtx c, unsigned long long seed, int redraw) {
       double m = (double)rho * PI * r * r * L;                      // solid cylinder
       double Ic = m * (3.0 * r * r + L * L) / 12.0, cz = 0.5 * L;
       int pa = topo[i].x;
-      cs[0 * d.Np + i] = (float)K;
-      cs[1 * d.Np + i] = (float)m;
-      cs[2 * d.Np + i] = (float)(m * cz);
-      cs[3 * d.Np + i] = (float)(Ic + m * cz * cz);                  // about the joint
-      cs[4 * d.Np + i] = (float)(0.5 * m * r * r);
+      // c4 = (m, m c, I about the joint, I_zz), then K[Np], rz[Np]  (ob_internal.h)
+      reinterpret_cast<float4 *>(cs)[i] =
+          make_float4((float)m, (float)(m * cz), (float)(Ic + m * cz * cz), (float)(0.5 * m * r * r));
+      cs[4 * d.Np + i] = (float)K;
       cs[5 * d.Np + i] = pa >= 0 ? Lown[pa] : 0.f;
       c.Mmax[d.link_base + i] = (float)Mx;
     } else {
-      for (int k = 0; k < kLinkConstFloats; k++) cs[k * d.Np + i] = 0.f;
+      reinterpret_cast<float4 *>(cs)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+      cs[4 * d.Np + i] = 0.f;
+      cs[5 * d.Np + i] = 0.f;
     }
   }
   unsigned char *ab = c.apple_blk + d.apple_blk_off;
@@ -175,8 +176,8 @@ __global__ void k_pose(DevCtx c, int w) {
       double Q[9], T[9], A[9];
       quat_to_mat_d(quat[j], Q);
       double s1, c1, s2, c2;
-      sincos((double)st[j], &s1, &c1);
-      sincos((double)st[d.Np + j], &s2, &c2);
+      sincos((double)st[2 * j], &s1, &c1);
+      sincos((double)st[2 * j + 1], &s2, &c2);
       const double XY[9] = {c2, 0, s2, s1 * s2, c1, -s1 * c2, -c1 * s2, s1, c1 * c2};
       for (int r = 0; r < 3; r++)
         for (int cc = 0; cc < 3; cc++) A[3 * r + cc] = Q[3 * r] * XY[cc] + Q[3 * r + 1] * XY[3 + cc] + Q[3 * r + 2] * XY[6 + cc];
