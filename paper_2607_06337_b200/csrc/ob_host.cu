@@ -127,9 +127,8 @@ int validate(const ob_world_spec *specs, int n_worlds, const ob_params *P, std::
   return OB_OK;
 }
 
-// level order: parents before children, links of one level contiguous and, inside a level, the links WITH
-// children first (a warp of k_step then holds either inner links or leaves, not a mix).  Returns the number of
-// links with children.
+// level order: plain breadth-first order -- parents before children, the links of one level contiguous and the
+// children of one link contiguous (k_step gathers them as a range).  Returns the number of links with children.
 int level_order(const ob_world_spec &s, std::vector<int32_t> &int2ext, std::vector<int32_t> &level_off) {
   const int N = s.n_links;
   std::vector<std::vector<int32_t>> kids(N);
@@ -149,7 +148,6 @@ int level_order(const ob_world_spec &s, std::vector<int32_t> &int2ext, std::vect
       if (!kids[int2ext[k]].empty()) n_inner++;
       for (int32_t ch : kids[int2ext[k]]) next.push_back(ch);
     }
-    std::stable_partition(next.begin(), next.end(), [&](int32_t e) { return !kids[e].empty(); });
     int2ext.insert(int2ext.end(), next.begin(), next.end());
     begin = end;
   }
@@ -182,7 +180,18 @@ int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) 
     const int Np = pad16(s.n_links), Ap = pad16(s.n_apples), nlev = (int)lev.size() - 1;
     L.sumNp += Np; L.sumAp += Ap; L.sumLev += nlev + 1;
     L.max_Np = std::max(L.max_Np, Np); L.max_Ap = std::max(L.max_Ap, Ap);
-    const int sm = step_smem_bytes(Np, Ap, NIp);
+    const int sm = step_smem_bytes(Np, Ap, NIp, nlev);
+    int max_kids = 0;
+    {
+      std::vector<int> nk(s.n_links, 0);
+      for (int i = 1; i < s.n_links; i++) max_kids = std::max(max_kids, ++nk[s.parent[i]]);
+    }
+    if (max_kids > kMaxChildren) {
+      char b[160];
+      snprintf(b, sizeof(b), "world %d: a link has %d children (limit %d)", w, max_kids, kMaxChildren);
+      why = b;
+      return OB_E_CAPACITY;
+    }
     if (sm > kMaxSmem || step_class_of(Np) < 0) {
       char b[200];
       snprintf(b, sizeof(b), "world %d (%d links, %d apples) does not fit on chip: %d B of shared memory (limit %d), "
@@ -438,7 +447,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   for (int k = 0; k < n_worlds; k++) {
     const WorldDesc &d = ctx->desc[h_order[k]];
     if (ctx->cls_n[d.cls]++ == 0) ctx->cls_off[d.cls] = k;
-    ctx->cls_smem[d.cls] = std::max(ctx->cls_smem[d.cls], step_smem_bytes(d.Np, d.Ap, d.NIp));
+    ctx->cls_smem[d.cls] = std::max(ctx->cls_smem[d.cls], step_smem_bytes(d.Np, d.Ap, d.NIp, d.n_levels));
   }
 
   DevCtx &D = ctx->dev;

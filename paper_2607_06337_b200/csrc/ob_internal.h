@@ -101,34 +101,39 @@ struct DevCtx {
   ob_params P;
 };
 
-// ---- k_step size classes: threads per CTA x links per thread x CTAs per SM the registers are budgeted for.
-//      A thread owns the same links for the whole launch (link i <-> slot i / NT of thread i % NT) and keeps
-//      their joint transform, inertia, diagonal terms and the PCG search direction in registers.
+// ---- k_step size classes: threads per CTA x links per thread (flat ownership: link tid + k * nt) x the CTAs
+//      per SM the registers are budgeted for.  Only the PCG vectors x, r and the Jacobi factors live in
+//      registers; everything the level sweeps touch lives in shared memory, so the sweep code exists once and
+//      runs over any number of links.
 struct StepClass { int nt, lpt, min_ctas; };
 constexpr int kNumClasses = 4;
-constexpr StepClass kStepClasses[kNumClasses] = {{128, 2, 6}, {128, 4, 4}, {256, 4, 2}, {512, 3, 1}};
+constexpr StepClass kStepClasses[kNumClasses] = {{128, 2, 6}, {256, 2, 3}, {512, 2, 1}, {512, 3, 1}};
 constexpr int kMaxLinksOnChip = 512 * 3;
+constexpr int kMaxChildren = 15;     // children per link (4 bits of the packed topology word)
 inline int step_class_of(int Np) {   // host only
   for (int k = 0; k < kNumClasses; k++)
     if (Np <= kStepClasses[k].nt * kStepClasses[k].lpt) return k;
   return -1;
 }
 
-// shared-memory footprint of one world in k_step (bytes); the host uses it to size the launch
-//   link state | apple block | scratch: four float4 planes [4][Np + 1] + overflow float4 [2][NIp] |
-//   f_tether, f_user [3][Ap], |f_s|, |f_user| [Ap] | wrench slots | snapped[Np]
-// The scratch planes carry, phase by phase (ob_step.cu): the parent -> child mailbox of the top-down bias pass
-// (24 floats per link WITH children: planes 0-3 + overflow), the child -> parent mailboxes of the bottom-up
-// passes, and the PCG vectors r, 1/diag, A p.
-__host__ __device__ inline int step_scratch_bytes(int Np, int NIp) { return 64 * (Np + 1) + 32 * NIp; }
-__host__ __device__ inline int step_smem_bytes(int Np, int Ap, int NIp) {
+// shared-memory footprint of one world in k_step (bytes); the host uses it to size the launch.  S = Np + 1
+// columns per plane (column Np stays zero: the trunk's parent).
+//   seven float4 planes [S]: M0, M1 (parent <-> child mailboxes, A p), PD (p, diagonal terms), C0..C2 (joint
+//   transform E, c2, s2, parent length), C3 (effective link inertia) | G float2 [S] (b, then 1/diag) |
+//   T uint32 [S] (packed topology + flags) | overflow float4 [2][NIp] (phase A) | level offsets |
+//   apple block (TMA) | f_tether, f_user [3][Ap], |f_s|, |f_user| [Ap] | wrench slots
+__host__ __device__ inline int r16(int b) { return (b + 15) / 16 * 16; }
+__host__ __device__ inline int step_planes_bytes(int Np) { return 7 * 16 * (Np + 1); }
+__host__ __device__ inline int step_smem_bytes(int Np, int Ap, int NIp, int nlev) {
   int b = 0;
-  b += link_state_bytes(Np);
-  b += apple_block_bytes(Ap);
-  b += step_scratch_bytes(Np, NIp);
+  b += step_planes_bytes(Np);
+  b += r16(8 * (Np + 1));
+  b += r16(4 * (Np + 1));
+  b += 32 * NIp;
+  b += r16(4 * (nlev + 1));
+  b += r16(apple_block_bytes(Ap));
   b += (3 + 3 + 2) * 4 * Ap;
   b += (int)sizeof(WrenchSlots);
-  b += Np;
   return (b + 127) / 128 * 128;
 }
 
