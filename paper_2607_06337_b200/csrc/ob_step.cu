@@ -50,7 +50,7 @@ constexpr uint32_t kHasApples = 1u << 26, kOffax = 1u << 27, kSnapped = 1u << 28
 // ------------------------------------------------------------------------------------------------------
 struct Sm {
   int Np, Ap, NIp, S;
-  float4 *P;                          // planes: P[j * S + i], j = 0 M0, 1 M1, 2 PD, 3..5 C0..C2, 6 C3
+  float4 *P;                          // records: P[7 * i + j], j = 0 M0, 1 M1, 2 PD, 3..5 C0..C2, 6 C3
   float2 *G;
   uint32_t *T;
   float4 *ovf;                        // ovf[j * NIp + inner slot]
@@ -151,18 +151,18 @@ struct Jt {
   M3 E;                // parent -> link rotation
   float c2, s2, rz;
 };
-__device__ __forceinline__ Jt load_jt(const float4 *P, const int S, const int i) {
-  const float4 e0 = P[3 * S + i], e1 = P[4 * S + i], e2 = P[5 * S + i];
+__device__ __forceinline__ Jt load_jt(const float4 *P, const int i) {
+  const float4 e0 = P[7 * i + 3], e1 = P[7 * i + 4], e2 = P[7 * i + 5];
   Jt j;
   j.E.a[0] = e0.x; j.E.a[1] = e0.y; j.E.a[2] = e0.z; j.E.a[3] = e0.w;
   j.E.a[4] = e1.x; j.E.a[5] = e1.y; j.E.a[6] = e1.z; j.E.a[7] = e1.w;
   j.E.a[8] = e2.x; j.c2 = e2.y; j.s2 = e2.z; j.rz = e2.w;
   return j;
 }
-__device__ __forceinline__ void store_jt(float4 *P, const int S, const int i, const Jt &j) {
-  P[3 * S + i] = make_float4(j.E.a[0], j.E.a[1], j.E.a[2], j.E.a[3]);
-  P[4 * S + i] = make_float4(j.E.a[4], j.E.a[5], j.E.a[6], j.E.a[7]);
-  P[5 * S + i] = make_float4(j.E.a[8], j.c2, j.s2, j.rz);
+__device__ __forceinline__ void store_jt(float4 *P, const int i, const Jt &j) {
+  P[7 * i + 3] = make_float4(j.E.a[0], j.E.a[1], j.E.a[2], j.E.a[3]);
+  P[7 * i + 4] = make_float4(j.E.a[4], j.E.a[5], j.E.a[6], j.E.a[7]);
+  P[7 * i + 5] = make_float4(j.E.a[8], j.c2, j.s2, j.rz);
 }
 
 // kinematic quantities of one link that the bias pass hands from its top-down half to its bottom-up half
@@ -253,13 +253,13 @@ __device__ __forceinline__ void finish_bias(const Jt &j, const int i, const uint
     dt0 += __ldg(g.arm + i);
     dt1 += __ldg(g.arm + Np + i);
   }
-  reinterpret_cast<float2 *>(s.P + 2 * S + i)[1] = make_float2(dt0, dt1);    // arm + (h c_d + h^2) K per DoF
+  reinterpret_cast<float2 *>(s.P + 7 * i + 2)[1] = make_float2(dt0, dt1);    // arm + (h c_d + h^2) K per DoF
   if (!(tw & kTrunk)) {
     const float3 fp = mulT(j.E, f);
     float3 np = mulT(j.E, n);
     np.x -= j.rz * fp.y; np.y += j.rz * fp.x;
-    s.P[i] = make_float4(np.x, np.y, np.z, fp.x);
-    *reinterpret_cast<float2 *>(s.P + S + i) = make_float2(fp.y, fp.z);
+    s.P[7 * i] = make_float4(np.x, np.y, np.z, fp.x);
+    *reinterpret_cast<float2 *>(s.P + 7 * i + 1) = make_float2(fp.y, fp.z);
   }
 }
 
@@ -299,7 +299,7 @@ __device__ __forceinline__ void down_bias(const int i, const Sm &s, const Gm &g,
   for (int q = 0; q < 9; q++) dRp.a[q] = 0.f;
   if (!(tw & kTrunk)) {
     const int par = (int)(tw & kParMask), ps = (int)((uint32_t)t2.y >> 16);
-    const float4 t0 = s.P[par], t1 = s.P[S + par], t2v = s.P[2 * S + par], t3 = s.P[6 * S + par],
+    const float4 t0 = s.P[7 * par], t1 = s.P[7 * par + 1], t2v = s.P[7 * par + 2], t3 = s.P[7 * par + 6],
                  t4 = s.ovf[ps], t5 = s.ovf[NIp + ps];
     dRp.a[0] = t0.x; dRp.a[1] = t0.y; dRp.a[2] = t0.z; dRp.a[3] = t0.w;
     dRp.a[4] = t1.x; dRp.a[5] = t1.y; dRp.a[6] = t1.z; dRp.a[7] = t1.w;
@@ -310,7 +310,7 @@ __device__ __forceinline__ void down_bias(const int i, const Sm &s, const Gm &g,
     rz = __ldg(g.rz + i);
   }
   j.rz = rz;
-  store_jt(s.P, S, i, j);
+  store_jt(s.P, i, j);
   // displacement-form FK: R_i = R0_i + dR_i,  dR_i = dR_p Rrel + R0_i (RxRy - I);  dp_i = dp_p + dR_p (0,0,rz)
   Kin k;
   {
@@ -337,10 +337,10 @@ __device__ __forceinline__ void down_bias(const int i, const Sm &s, const Gm &g,
 
   if ((tw >> kNcShift) & kNcMask) {
     const int is = t2.y & 0xffff;
-    s.P[i] = make_float4(k.dR.a[0], k.dR.a[1], k.dR.a[2], k.dR.a[3]);
-    s.P[S + i] = make_float4(k.dR.a[4], k.dR.a[5], k.dR.a[6], k.dR.a[7]);
-    s.P[2 * S + i] = make_float4(k.dR.a[8], k.dp.x, k.dp.y, k.dp.z);
-    s.P[6 * S + i] = make_float4(k.om.x, k.om.y, k.om.z, k.vl.x);
+    s.P[7 * i] = make_float4(k.dR.a[0], k.dR.a[1], k.dR.a[2], k.dR.a[3]);
+    s.P[7 * i + 1] = make_float4(k.dR.a[4], k.dR.a[5], k.dR.a[6], k.dR.a[7]);
+    s.P[7 * i + 2] = make_float4(k.dR.a[8], k.dp.x, k.dp.y, k.dp.z);
+    s.P[7 * i + 6] = make_float4(k.om.x, k.om.y, k.om.z, k.vl.x);
     s.ovf[is] = make_float4(k.vl.y, k.vl.z, k.al.x, k.al.y);
     s.ovf[NIp + is] = make_float4(k.al.z, k.aln.x, k.aln.y, k.aln.z);
   } else {
@@ -357,7 +357,7 @@ __device__ __forceinline__ void up_bias(const int i, const uint32_t tw, const Sm
   const int is = __ldg(g.topo2 + i).y & 0xffff;
   Kin k;
   {
-    const float4 t0 = s.P[i], t1 = s.P[S + i], t2v = s.P[2 * S + i], t3 = s.P[6 * S + i], t4 = s.ovf[is],
+    const float4 t0 = s.P[7 * i], t1 = s.P[7 * i + 1], t2v = s.P[7 * i + 2], t3 = s.P[7 * i + 6], t4 = s.ovf[is],
                  t5 = s.ovf[NIp + is];
     k.dR.a[0] = t0.x; k.dR.a[1] = t0.y; k.dR.a[2] = t0.z; k.dR.a[3] = t0.w;
     k.dR.a[4] = t1.x; k.dR.a[5] = t1.y; k.dR.a[6] = t1.z; k.dR.a[7] = t1.w;
@@ -369,12 +369,12 @@ __device__ __forceinline__ void up_bias(const int i, const uint32_t tw, const Sm
   bias_force(i, k, tw, s, g, c, n, f);
   const int fc = (int)((tw >> kChShift) & kParMask), nc = (int)((tw >> kNcShift) & kNcMask);
   for (int ch = fc; ch < fc + nc; ch++) {
-    const float4 u = s.P[ch];
-    const float2 v = *reinterpret_cast<const float2 *>(s.P + S + ch);
+    const float4 u = s.P[7 * ch];
+    const float2 v = *reinterpret_cast<const float2 *>(s.P + 7 * ch + 1);
     n = n + f3(u.x, u.y, u.z);
     f = f + f3(u.w, v.x, v.y);
   }
-  finish_bias(load_jt(s.P, S, i), i, tw, n, f, s, g, c);
+  finish_bias(load_jt(s.P, i), i, tw, n, f, s, g, c);
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -407,19 +407,19 @@ __device__ __forceinline__ void up_inertia(const int i, const Sm &s, const Gm &g
     }
     s.T[i] = tw;
   }
-  s.P[6 * S + i] = eff;
+  s.P[7 * i + 6] = eff;
   const int fc = (int)((tw >> kChShift) & kParMask), nc = (int)((tw >> kNcShift) & kNcMask);
   for (int ch = fc; ch < fc + nc; ch++) {
-    const float4 u0 = s.P[ch];
-    const float4 u1 = s.P[S + ch];
-    const float2 u2 = *reinterpret_cast<const float2 *>(s.P + 2 * S + ch);
+    const float4 u0 = s.P[7 * ch];
+    const float4 u1 = s.P[7 * ch + 1];
+    const float2 u2 = *reinterpret_cast<const float2 *>(s.P + 7 * ch + 2);
     cm += u0.x;
     ch3 = ch3 + f3(u0.y, u0.z, u0.w);
     Ixx += u1.x; Iyy += u1.y; Izz += u1.z; Ixy += u1.w; Ixz += u2.x; Iyz += u2.y;
   }
-  const Jt j = load_jt(s.P, S, i);
+  const Jt j = load_jt(s.P, i);
   const float c2 = j.c2, s2 = j.s2;
-  const float2 dt = reinterpret_cast<const float2 *>(s.P + 2 * S + i)[1];
+  const float2 dt = reinterpret_cast<const float2 *>(s.P + 7 * i + 2)[1];
   const float d1 = c2 * c2 * Ixx + 2.f * c2 * s2 * Ixz + s2 * s2 * Izz + dt.x;
   const float d2 = Iyy + dt.y;
   float2 id = make_float2(1.f, 1.f);
@@ -438,9 +438,9 @@ __device__ __forceinline__ void up_inertia(const int i, const Sm &s, const Gm &g
       for (int cc = 0; cc < 3; cc++) T.a[3 * r + cc] = E.a[r] * I.a[cc] + E.a[3 + r] * I.a[3 + cc] + E.a[6 + r] * I.a[6 + cc];
     Ip = mul(T, E);
     const float sh = 2.f * rz * hp.z + cm * rz * rz;
-    s.P[i] = make_float4(cm, hp.x, hp.y, hp.z + cm * rz);
-    s.P[S + i] = make_float4(Ip.a[0] + sh, Ip.a[4] + sh, Ip.a[8], Ip.a[1]);
-    *reinterpret_cast<float2 *>(s.P + 2 * S + i) = make_float2(Ip.a[2] - rz * hp.x, Ip.a[5] - rz * hp.y);
+    s.P[7 * i] = make_float4(cm, hp.x, hp.y, hp.z + cm * rz);
+    s.P[7 * i + 1] = make_float4(Ip.a[0] + sh, Ip.a[4] + sh, Ip.a[8], Ip.a[1]);
+    *reinterpret_cast<float2 *>(s.P + 7 * i + 2) = make_float2(Ip.a[2] - rz * hp.x, Ip.a[5] - rz * hp.y);
   }
 }
 
@@ -470,30 +470,29 @@ __device__ __noinline__ Force6 offaxis_tethers(const int4 t2, const float3 al, c
   return r;
 }
 
-__device__ __forceinline__ void mv_down(const Jt &j, const float4 *P, const int S, const uint32_t tw, const float4 pd,
-                                        float3 &al, float3 &a) {
-  const int par = (int)(tw & kParMask);
-  const float4 u = P[par];
-  const float2 v = *reinterpret_cast<const float2 *>(P + S + par);
+__device__ __forceinline__ void mv_down(const Jt &j, const float4 *P, const uint32_t tw, const float4 pd, float3 &al,
+                                        float3 &a) {
+  const float4 *par = P + 7 * (int)(tw & kParMask);
+  const float4 u = par[0], v = par[1];
   const float3 alp = f3(u.x, u.y, u.z), ap = f3(u.w, v.x, v.y);
   al = mul(j.E, alp) + f3(j.c2 * pd.x, pd.y, j.s2 * pd.x);
   a = mul(j.E, f3(ap.x + alp.y * j.rz, ap.y - alp.x * j.rz, ap.z));
 }
 
-__device__ __forceinline__ float mv_up(const Jt &j, float4 *P, const int S, const int i, const uint32_t tw,
-                                       const float4 pd, const float3 al, const float3 a, const Sm &s, const Gm &g,
-                                       const DevCtx &c) {
-  const float4 I = P[6 * S + i];                              // (m, m c, I about the joint, I_zz)
+__device__ __forceinline__ float mv_up(const Jt &j, float4 *P, const int i, const uint32_t tw, const float4 pd,
+                                       const float3 al, const float3 a, const Sm &s, const Gm &g, const DevCtx &c) {
+  float4 *rec = P + 7 * i;
+  const float4 I = rec[6];                                    // (m, m c, I about the joint, I_zz)
   float3 n = f3(I.z * al.x - I.y * a.y, I.z * al.y + I.y * a.x, I.w * al.z);
   float3 f = f3(I.x * a.x + I.y * al.y, I.x * a.y - I.y * al.x, I.x * a.z);
   if (tw & kOffax) {
     const Force6 t = offaxis_tethers(__ldg(g.topo2 + i), al, a, s.att, s.ao, s.ak, s.Ap, c.P.h * c.P.h);
     n = n + t.n; f = f + t.f;
   }
-  const int fc = (int)((tw >> kChShift) & kParMask), nc = (int)((tw >> kNcShift) & kNcMask);
-  for (int ch = fc; ch < fc + nc; ch++) {
-    const float4 u = P[ch];
-    const float2 v = *reinterpret_cast<const float2 *>(P + S + ch);
+  const float4 *ch = P + 7 * (int)((tw >> kChShift) & kParMask);
+#pragma unroll 1
+  for (int nc = (int)((tw >> kNcShift) & kNcMask); nc > 0; nc--, ch += 7) {
+    const float4 u = ch[0], v = ch[1];
     n = n + f3(u.x, u.y, u.z);
     f = f + f3(u.w, v.x, v.y);
   }
@@ -502,8 +501,8 @@ __device__ __forceinline__ float mv_up(const Jt &j, float4 *P, const int S, cons
   const float3 fp = mulT(j.E, f);                             // the trunk publishes into its own column, which nobody reads
   float3 np = mulT(j.E, n);
   np.x -= j.rz * fp.y; np.y += j.rz * fp.x;
-  P[i] = make_float4(np.x, np.y, np.z, fp.x);
-  P[S + i] = make_float4(fp.y, fp.z, t1, t2);
+  rec[0] = make_float4(np.x, np.y, np.z, fp.x);
+  rec[1] = make_float4(fp.y, fp.z, t1, t2);
   return pd.x * t1 + pd.y * t2;
 }
 
@@ -545,6 +544,9 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
     const Sm s = carve(smem, d);
     const int Np = d.Np, S = Np + 1, N = d.N;
     const int nlev = d.n_levels, ntop = d.n_top;
+    // warps other than warp 0 own no link of the n_top leading levels: they enter a top-down sweep at the level
+    // whose fence is the first block barrier and leave a bottom-up sweep after the last one
+    const int l_first_down = tid < 32 ? 0 : ntop - 1, l_last_up = tid < 32 ? 0 : ntop;
     float4 *const PL = s.P;
     Gm g;
     {
@@ -573,7 +575,7 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
       const int32_t *src = reinterpret_cast<const int32_t *>(c.wrench + w);
       int32_t *dst = reinterpret_cast<int32_t *>(s.wr);
       for (int k = tid; k < (int)(sizeof(WrenchSlots) / 4); k += NT) dst[k] = __ldg(src + k);
-      if (tid < 7) PL[tid * S + Np] = make_float4(0.f, 0.f, 0.f, 0.f);            // the zero column
+      if (tid < 7) PL[7 * Np + tid] = make_float4(0.f, 0.f, 0.f, 0.f);            // the zero column
       for (int k = tid; k <= nlev; k += NT) s.lev[k] = __ldg(c.level_off + d.level_base + k);
       for (int i = tid; i < S; i += NT) {
         uint32_t tw = (uint32_t)Np | kTrunk;
@@ -615,7 +617,7 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
     for (int sidx = 0; sidx < n_steps; sidx++) {
       // ---- A (+ B1 for leaves): top-down ----
 #pragma unroll 1
-      for (int l = 0; l < nlev; l++) {
+      for (int l = l_first_down; l < nlev; l++) {
         const int le = s.lev[l + 1];
 #pragma unroll 1
         for (int i = s.lev[l] + tid; i < le; i += NT) down_bias(i, s, g, c);
@@ -623,7 +625,7 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
       }
       // ---- B1: bias forces bottom-up over the inner links -> rhs b ----
 #pragma unroll 1
-      for (int l = nlev - 2; l >= 0; l--) {
+      for (int l = nlev - 2; l >= l_last_up; l--) {
         const int le = s.lev[l + 1];
 #pragma unroll 1
         for (int i = s.lev[l] + tid; i < le; i += NT) {
@@ -644,7 +646,7 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
         if (((s.T[i] >> kNcShift) & kNcMask) == 0u) up_inertia(i, s, g, c);
       __syncthreads();
 #pragma unroll 1
-      for (int l = nlev - 2; l >= 0; l--) {
+      for (int l = nlev - 2; l >= l_last_up; l--) {
         const int le = s.lev[l + 1];
 #pragma unroll 1
         for (int i = s.lev[l] + tid; i < le; i += NT)
@@ -676,46 +678,48 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
 #pragma unroll
         for (int k = 0; k < LPT; k++) {                 // first product: A x, i.e. p = x
           const int i = tid + k * NT;
-          if (i < N) *reinterpret_cast<float2 *>(PL + 2 * S + i) = x[k];
+          if (i < N) *reinterpret_cast<float2 *>(PL + 7 * i + 2) = x[k];
         }
         bool first = true;
         float rz = 0.f, rr = 0.f;
         // stopping rule: |r| <= tol |b| in the 2-norm (cg_norm 0) or in the preconditioned norm (cg_norm 1)
         const float tol2 = P.cg_tol * P.cg_tol * (P.cg_norm ? bz : bb);
         for (;;) {
-          // ---- A p: top-down (the deepest level turns around at once), then bottom-up ----
+          // ---- A p: top-down (the deepest level turns around at once), then bottom-up.  Warps other than warp
+          //      0 have no links in the n_top leading levels and join at the first block barrier ----
           float pAp_part = 0.f;
 #pragma unroll 1
-          for (int l = 0; l < nlev; l++) {
+          for (int l = l_first_down; l < nlev; l++) {
             const int le = s.lev[l + 1];
             const bool deepest = l == nlev - 1;
 #pragma unroll 1
             for (int i = s.lev[l] + tid; i < le; i += NT) {
               const uint32_t tw = s.T[i];
-              const float4 pd = PL[2 * S + i];
-              const Jt j = load_jt(PL, S, i);
+              float4 *rec = PL + 7 * i;
+              const float4 pd = rec[2];
+              const Jt j = load_jt(PL, i);
               float3 al, a;
-              mv_down(j, PL, S, tw, pd, al, a);
+              mv_down(j, PL, tw, pd, al, a);
               if (deepest) {
-                pAp_part += mv_up(j, PL, S, i, tw, pd, al, a, s, g, c);
+                pAp_part += mv_up(j, PL, i, tw, pd, al, a, s, g, c);
               } else {
-                PL[i] = make_float4(al.x, al.y, al.z, a.x);
-                *reinterpret_cast<float2 *>(PL + S + i) = make_float2(a.y, a.z);
+                rec[0] = make_float4(al.x, al.y, al.z, a.x);
+                *reinterpret_cast<float2 *>(rec + 1) = make_float2(a.y, a.z);
               }
             }
             OB_FENCE_DOWN(l)
           }
 #pragma unroll 1
-          for (int l = nlev - 2; l >= 0; l--) {
+          for (int l = nlev - 2; l >= l_last_up; l--) {
             const int le = s.lev[l + 1];
 #pragma unroll 1
             for (int i = s.lev[l] + tid; i < le; i += NT) {
               const uint32_t tw = s.T[i];
-              const float4 pd = PL[2 * S + i];
-              const Jt j = load_jt(PL, S, i);
-              const float4 u = PL[i];
-              const float2 v = *reinterpret_cast<const float2 *>(PL + S + i);
-              pAp_part += mv_up(j, PL, S, i, tw, pd, f3(u.x, u.y, u.z), f3(u.w, v.x, v.y), s, g, c);
+              const float4 *rec = PL + 7 * i;
+              const float4 pd = rec[2];
+              const Jt j = load_jt(PL, i);
+              const float4 u = rec[0], v = rec[1];
+              pAp_part += mv_up(j, PL, i, tw, pd, f3(u.x, u.y, u.z), f3(u.w, v.x, v.y), s, g, c);
             }
             OB_FENCE_UP(l)
           }
@@ -727,10 +731,10 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
             for (int k = 0; k < LPT; k++) {
               const int i = tid + k * NT;
               if (i < N) {
-                const float2 ap = reinterpret_cast<const float2 *>(PL + S + i)[1];
+                const float2 ap = reinterpret_cast<const float2 *>(PL + 7 * i + 1)[1];
                 r[k].x -= ap.x; r[k].y -= ap.y;
                 const float za = r[k].x * idg[k].x, zb = r[k].y * idg[k].y;
-                *reinterpret_cast<float2 *>(PL + 2 * S + i) = make_float2(za, zb);
+                *reinterpret_cast<float2 *>(PL + 7 * i + 2) = make_float2(za, zb);
                 rz_p += r[k].x * za + r[k].y * zb; rr_p += r[k].x * r[k].x + r[k].y * r[k].y;
               }
             }
@@ -745,8 +749,8 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
               const int i = tid + k * NT;
               z[k] = make_float2(0.f, 0.f); pk[k] = make_float2(0.f, 0.f);
               if (i < N) {
-                const float2 ap = reinterpret_cast<const float2 *>(PL + S + i)[1];
-                pk[k] = *reinterpret_cast<const float2 *>(PL + 2 * S + i);
+                const float2 ap = reinterpret_cast<const float2 *>(PL + 7 * i + 1)[1];
+                pk[k] = *reinterpret_cast<const float2 *>(PL + 7 * i + 2);
                 x[k].x += alpha * pk[k].x; x[k].y += alpha * pk[k].y;
                 r[k].x -= alpha * ap.x; r[k].y -= alpha * ap.y;
                 z[k] = make_float2(r[k].x * idg[k].x, r[k].y * idg[k].y);
@@ -760,7 +764,7 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
             for (int k = 0; k < LPT; k++) {
               const int i = tid + k * NT;
               if (i < N)
-                *reinterpret_cast<float2 *>(PL + 2 * S + i) = make_float2(z[k].x + beta * pk[k].x, z[k].y + beta * pk[k].y);
+                *reinterpret_cast<float2 *>(PL + 7 * i + 2) = make_float2(z[k].x + beta * pk[k].x, z[k].y + beta * pk[k].y);
             }
             it++;
           }
