@@ -53,7 +53,7 @@ struct Sm {
   float4 *P;                          // records: P[7 * i + j], j = 0 M0, 1 M1, 2 PD, 3..5 C0..C2, 6 C3
   float2 *G;
   uint32_t *T;
-  float4 *ovf;                        // ovf[j * NIp + inner slot]
+  float4 *ovf;                        // ovf[j * NIp + inner slot], j = 0..2
   int *lev;                           // level offsets [n_levels + 1]
   // apple block (TMA)
   float *u, *v;                       // [3][Ap]
@@ -71,7 +71,7 @@ __device__ __forceinline__ Sm carve(unsigned char *base, const WorldDesc &d) {
   s.P = reinterpret_cast<float4 *>(p); p += step_planes_bytes(Np);
   s.G = reinterpret_cast<float2 *>(p); p += r16(8 * (Np + 1));
   s.T = reinterpret_cast<uint32_t *>(p); p += r16(4 * (Np + 1));
-  s.ovf = reinterpret_cast<float4 *>(p); p += 32 * d.NIp;
+  s.ovf = reinterpret_cast<float4 *>(p); p += 48 * d.NIp;
   s.lev = reinterpret_cast<int *>(p); p += r16(4 * (d.n_levels + 1));
   float *f = reinterpret_cast<float *>(p);
   s.u = f; s.v = f + 3 * Ap;
@@ -168,7 +168,8 @@ __device__ __forceinline__ void store_jt(float4 *P, const int i, const Jt &j) {
 // kinematic quantities of one link that the bias pass hands from its top-down half to its bottom-up half
 struct Kin {
   M3 dR;               // R - R0 (displacement form)
-  float3 dp;           // origin - rest origin
+  double dpx, dpy, dpz; // origin - rest origin; fp64: the tether stretch is the small difference of two sums
+                        // along the chain and k_s times its rounding error is what the thinnest twigs feel
   float3 om, vl;       // spatial velocity
   float3 al, aln;      // bias spatial acceleration (gravity as base acceleration)
 };
@@ -206,12 +207,14 @@ __device__ __forceinline__ void bias_force(const int i, const Kin &k, const uint
   for (int a = ast; a < ast + nap; a++) {
     if (!s.att[a]) continue;
     const float3 o = f3(s.ao[a], s.ao[Ap + a], s.ao[2 * Ap + a]);
-    const float3 dh = k.dp + mul(k.dR, o);                                // x_hang - anchor
+    const float3 dro = mul(k.dR, o);
+    const double dhx = k.dpx + (double)dro.x, dhy = k.dpy + (double)dro.y, dhz = k.dpz + (double)dro.z;   // x_hang - anchor
     const float ks = s.ak[a], cdamp = s.ac[a], ma = s.am[a];
     // x_a - x_hang = u + sag - dh with the rest sag m g / k_s (u is stored relative to the rest position)
     const float gk = ma / ks;
-    const float3 st = f3(s.u[a] + (gk * P.gravity[0] - dh.x), s.u[Ap + a] + (gk * P.gravity[1] - dh.y),
-                         s.u[2 * Ap + a] + (gk * P.gravity[2] - dh.z));
+    const float3 st = f3((float)((double)s.u[a] + ((double)(gk * P.gravity[0]) - dhx)),
+                         (float)((double)s.u[Ap + a] + ((double)(gk * P.gravity[1]) - dhy)),
+                         (float)((double)s.u[2 * Ap + a] + ((double)(gk * P.gravity[2]) - dhz)));
     const float3 vh = mul(R, vl + cross(om, o));                          // world velocity of the hang point
     const float3 fs = (-ks) * st;
     const float3 va = f3(s.v[a], s.v[Ap + a], s.v[2 * Ap + a]);
@@ -291,7 +294,8 @@ __device__ __forceinline__ void down_bias(const int i, const Sm &s, const Gm &g,
 
   // parent quantities (world = parent of the trunk: at rest, spatial acceleration (0; -g))
   M3 dRp;
-  float3 dpp = f3(0, 0, 0), wp = f3(0, 0, 0), vp = f3(0, 0, 0), alp = f3(0, 0, 0);
+  double dppx = 0.0, dppy = 0.0, dppz = 0.0;
+  float3 wp = f3(0, 0, 0), vp = f3(0, 0, 0), alp = f3(0, 0, 0);
   float3 ap = f3(-P.gravity[0], -P.gravity[1], -P.gravity[2]);
   uint32_t snapped_p = 0;
   float rz = 0.f;
@@ -301,11 +305,13 @@ __device__ __forceinline__ void down_bias(const int i, const Sm &s, const Gm &g,
     const int par = (int)(tw & kParMask), ps = (int)((uint32_t)t2.y >> 16);
     const float4 t0 = s.P[7 * par], t1 = s.P[7 * par + 1], t2v = s.P[7 * par + 2], t3 = s.P[7 * par + 6],
                  t4 = s.ovf[ps], t5 = s.ovf[NIp + ps];
+    const double2 d0 = *reinterpret_cast<const double2 *>(s.ovf + 2 * NIp + ps);
     dRp.a[0] = t0.x; dRp.a[1] = t0.y; dRp.a[2] = t0.z; dRp.a[3] = t0.w;
     dRp.a[4] = t1.x; dRp.a[5] = t1.y; dRp.a[6] = t1.z; dRp.a[7] = t1.w;
-    dRp.a[8] = t2v.x; dpp = f3(t2v.y, t2v.z, t2v.w);
-    wp = f3(t3.x, t3.y, t3.z); vp = f3(t3.w, t4.x, t4.y);
-    alp = f3(t4.z, t4.w, t5.x); ap = f3(t5.y, t5.z, t5.w);
+    dRp.a[8] = t2v.x; wp = f3(t2v.y, t2v.z, t2v.w);
+    vp = f3(t3.x, t3.y, t3.z); alp = f3(t3.w, t4.x, t4.y);
+    ap = f3(t4.z, t4.w, t5.x);
+    dppx = (double)t5.y + (double)t5.z; dppy = d0.x; dppz = d0.y;      // x as a float pair, y and z as doubles
     snapped_p = s.T[par] & kSnapped;
     rz = __ldg(g.rz + i);
   }
@@ -322,7 +328,9 @@ __device__ __forceinline__ void down_bias(const int i, const Sm &s, const Gm &g,
 #pragma unroll
     for (int q = 0; q < 9; q++) k.dR.a[q] = t1m.a[q] + t2m.a[q];
   }
-  k.dp = f3(dpp.x + rz * dRp.a[2], dpp.y + rz * dRp.a[5], dpp.z + rz * dRp.a[8]);
+  k.dpx = dppx + (double)rz * (double)dRp.a[2];
+  k.dpy = dppy + (double)rz * (double)dRp.a[5];
+  k.dpz = dppz + (double)rz * (double)dRp.a[8];
 
   // velocity and (bias) spatial acceleration in link coordinates
   const float3 vJ = f3(c2 * w1, w2, s2 * w1);
@@ -339,10 +347,12 @@ __device__ __forceinline__ void down_bias(const int i, const Sm &s, const Gm &g,
     const int is = t2.y & 0xffff;
     s.P[7 * i] = make_float4(k.dR.a[0], k.dR.a[1], k.dR.a[2], k.dR.a[3]);
     s.P[7 * i + 1] = make_float4(k.dR.a[4], k.dR.a[5], k.dR.a[6], k.dR.a[7]);
-    s.P[7 * i + 2] = make_float4(k.dR.a[8], k.dp.x, k.dp.y, k.dp.z);
-    s.P[7 * i + 6] = make_float4(k.om.x, k.om.y, k.om.z, k.vl.x);
-    s.ovf[is] = make_float4(k.vl.y, k.vl.z, k.al.x, k.al.y);
-    s.ovf[NIp + is] = make_float4(k.al.z, k.aln.x, k.aln.y, k.aln.z);
+    s.P[7 * i + 2] = make_float4(k.dR.a[8], k.om.x, k.om.y, k.om.z);
+    s.P[7 * i + 6] = make_float4(k.vl.x, k.vl.y, k.vl.z, k.al.x);
+    s.ovf[is] = make_float4(k.al.y, k.al.z, k.aln.x, k.aln.y);
+    const float dxh = (float)k.dpx;
+    s.ovf[NIp + is] = make_float4(k.aln.z, dxh, (float)(k.dpx - (double)dxh), 0.f);
+    *reinterpret_cast<double2 *>(s.ovf + 2 * NIp + is) = make_double2(k.dpy, k.dpz);
   } else {
     float3 n, f;
     bias_force(i, k, tw, s, g, c, n, f);
@@ -361,9 +371,11 @@ __device__ __forceinline__ void up_bias(const int i, const uint32_t tw, const Sm
                  t5 = s.ovf[NIp + is];
     k.dR.a[0] = t0.x; k.dR.a[1] = t0.y; k.dR.a[2] = t0.z; k.dR.a[3] = t0.w;
     k.dR.a[4] = t1.x; k.dR.a[5] = t1.y; k.dR.a[6] = t1.z; k.dR.a[7] = t1.w;
-    k.dR.a[8] = t2v.x; k.dp = f3(t2v.y, t2v.z, t2v.w);
-    k.om = f3(t3.x, t3.y, t3.z); k.vl = f3(t3.w, t4.x, t4.y);
-    k.al = f3(t4.z, t4.w, t5.x); k.aln = f3(t5.y, t5.z, t5.w);
+    const double2 d0 = *reinterpret_cast<const double2 *>(s.ovf + 2 * NIp + is);
+    k.dR.a[8] = t2v.x; k.om = f3(t2v.y, t2v.z, t2v.w);
+    k.vl = f3(t3.x, t3.y, t3.z); k.al = f3(t3.w, t4.x, t4.y);
+    k.aln = f3(t4.z, t4.w, t5.x);
+    k.dpx = (double)t5.y + (double)t5.z; k.dpy = d0.x; k.dpz = d0.y;
   }
   float3 n, f;
   bias_force(i, k, tw, s, g, c, n, f);
@@ -479,8 +491,9 @@ __device__ __forceinline__ void mv_down(const Jt &j, const float4 *P, const uint
   a = mul(j.E, f3(ap.x + alp.y * j.rz, ap.y - alp.x * j.rz, ap.z));
 }
 
-__device__ __forceinline__ float mv_up(const Jt &j, float4 *P, const int i, const uint32_t tw, const float4 pd,
-                                       const float3 al, const float3 a, const Sm &s, const Gm &g, const DevCtx &c) {
+__device__ __forceinline__ float mv_up(const Jt &j, float4 *P, const float4 *zero_rec, const int i, const uint32_t tw,
+                                       const float4 pd, const float3 al, const float3 a, const Sm &s, const Gm &g,
+                                       const DevCtx &c) {
   float4 *rec = P + 7 * i;
   const float4 I = rec[6];                                    // (m, m c, I about the joint, I_zz)
   float3 n = f3(I.z * al.x - I.y * a.y, I.z * al.y + I.y * a.x, I.w * al.z);
@@ -489,10 +502,25 @@ __device__ __forceinline__ float mv_up(const Jt &j, float4 *P, const int i, cons
     const Force6 t = offaxis_tethers(__ldg(g.topo2 + i), al, a, s.att, s.ao, s.ak, s.Ap, c.P.h * c.P.h);
     n = n + t.n; f = f + t.f;
   }
+  // children: the first four with all loads in flight at once (a missing child reads the zero record)
   const float4 *ch = P + 7 * (int)((tw >> kChShift) & kParMask);
+  const int nc = (int)((tw >> kNcShift) & kNcMask);
+  {
+    float4 cu[4], cv[4];
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+      const float4 *q = k < nc ? ch + 7 * k : zero_rec;
+      cu[k] = q[0]; cv[k] = q[1];
+    }
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+      n = n + f3(cu[k].x, cu[k].y, cu[k].z);
+      f = f + f3(cu[k].w, cv[k].x, cv[k].y);
+    }
+  }
 #pragma unroll 1
-  for (int nc = (int)((tw >> kNcShift) & kNcMask); nc > 0; nc--, ch += 7) {
-    const float4 u = ch[0], v = ch[1];
+  for (int k = 4; k < nc; k++) {
+    const float4 u = ch[7 * k], v = ch[7 * k + 1];
     n = n + f3(u.x, u.y, u.z);
     f = f + f3(u.w, v.x, v.y);
   }
@@ -602,6 +630,16 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
       parity ^= 1;
     }
     __syncthreads();
+    // lanes of warp 0 <-> links of the n_top leading levels: level of the lane's link, widest child list that
+    // stays inside the warp
+    const int ntopN = s.lev[ntop];
+    int top_lvl = -1, top_maxc = 0;
+    if (tid < ntopN) {
+      for (int l = 0; l < ntop; l++)
+        if (tid >= s.lev[l]) top_lvl = l;
+      if (top_lvl < ntop - 1) top_maxc = (int)((s.T[tid] >> kNcShift) & kNcMask);
+    }
+    top_maxc = __reduce_max_sync(0xffffffffu, top_maxc);
     // user forces on apples are constant over the launch
     for (int a = tid; a < d.A; a += NT) {
       float3 fu = f3(0, 0, 0);
@@ -685,11 +723,39 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
         // stopping rule: |r| <= tol |b| in the 2-norm (cg_norm 0) or in the preconditioned norm (cg_norm 1)
         const float tol2 = P.cg_tol * P.cg_tol * (P.cg_norm ? bz : bb);
         for (;;) {
-          // ---- A p: top-down (the deepest level turns around at once), then bottom-up.  Warps other than warp
-          //      0 have no links in the n_top leading levels and join at the first block barrier ----
+          // ---- A p.  The n_top leading levels live in warp 0, lane = link: own record in registers, parents
+          //      and children by shuffle, no barrier.  The other levels are swept by the whole CTA, one block
+          //      barrier per level; the deepest level turns around at once ----
           float pAp_part = 0.f;
+          if (tid < 32) {
+            const int me = tid < ntopN ? tid : Np;               // idle lanes work on the zero record
+            const uint32_t tw = s.T[me];
+            float4 *rec = PL + 7 * me;
+            const float4 pd = rec[2];
+            const Jt j = load_jt(PL, me);
+            const int parl = (tw & kTrunk) ? tid : (int)(tw & kParMask);
+            float3 al = f3(0, 0, 0), a = f3(0, 0, 0);
 #pragma unroll 1
-          for (int l = l_first_down; l < nlev; l++) {
+            for (int l = 0; l < ntop; l++) {
+              float3 alp, ap;
+              alp.x = __shfl_sync(0xffffffffu, al.x, parl); alp.y = __shfl_sync(0xffffffffu, al.y, parl);
+              alp.z = __shfl_sync(0xffffffffu, al.z, parl);
+              ap.x = __shfl_sync(0xffffffffu, a.x, parl); ap.y = __shfl_sync(0xffffffffu, a.y, parl);
+              ap.z = __shfl_sync(0xffffffffu, a.z, parl);
+              if (top_lvl == l) {
+                if (tw & kTrunk) { alp = f3(0, 0, 0); ap = f3(0, 0, 0); }
+                al = mul(j.E, alp) + f3(j.c2 * pd.x, pd.y, j.s2 * pd.x);
+                a = mul(j.E, f3(ap.x + alp.y * j.rz, ap.y - alp.x * j.rz, ap.z));
+              }
+            }
+            if (tid < ntopN) {
+              rec[0] = make_float4(al.x, al.y, al.z, a.x);
+              *reinterpret_cast<float2 *>(rec + 1) = make_float2(a.y, a.z);
+            }
+          }
+          __syncthreads();
+#pragma unroll 1
+          for (int l = ntop; l < nlev; l++) {
             const int le = s.lev[l + 1];
             const bool deepest = l == nlev - 1;
 #pragma unroll 1
@@ -701,16 +767,16 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
               float3 al, a;
               mv_down(j, PL, tw, pd, al, a);
               if (deepest) {
-                pAp_part += mv_up(j, PL, i, tw, pd, al, a, s, g, c);
+                pAp_part += mv_up(j, PL, PL + 7 * Np, i, tw, pd, al, a, s, g, c);
               } else {
                 rec[0] = make_float4(al.x, al.y, al.z, a.x);
                 *reinterpret_cast<float2 *>(rec + 1) = make_float2(a.y, a.z);
               }
             }
-            OB_FENCE_DOWN(l)
+            __syncthreads();
           }
 #pragma unroll 1
-          for (int l = nlev - 2; l >= l_last_up; l--) {
+          for (int l = nlev - 2; l >= ntop; l--) {
             const int le = s.lev[l + 1];
 #pragma unroll 1
             for (int i = s.lev[l] + tid; i < le; i += NT) {
@@ -719,9 +785,63 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
               const float4 pd = rec[2];
               const Jt j = load_jt(PL, i);
               const float4 u = rec[0], v = rec[1];
-              pAp_part += mv_up(j, PL, i, tw, pd, f3(u.x, u.y, u.z), f3(u.w, v.x, v.y), s, g, c);
+              pAp_part += mv_up(j, PL, PL + 7 * Np, i, tw, pd, f3(u.x, u.y, u.z), f3(u.w, v.x, v.y), s, g, c);
             }
-            OB_FENCE_UP(l)
+            __syncthreads();
+          }
+          if (tid < 32) {
+            const int me = tid < ntopN ? tid : Np;
+            const uint32_t tw = s.T[me];
+            float4 *rec = PL + 7 * me;
+            const float4 pd = rec[2], I = rec[6];
+            const Jt j = load_jt(PL, me);
+            const float4 u = rec[0], v = rec[1];
+            const float3 al = f3(u.x, u.y, u.z), a = f3(u.w, v.x, v.y);
+            const int fc = (int)((tw >> kChShift) & kParMask), nc = (int)((tw >> kNcShift) & kNcMask);
+            float3 un = f3(0, 0, 0), uf = f3(0, 0, 0);           // (n, f) of this link in its parent's frame
+            float t1 = 0.f, t2 = 0.f;
+#pragma unroll 1
+            for (int l = ntop - 1; l >= 0; l--) {
+              const bool mine = top_lvl == l;
+              float3 n = f3(I.z * al.x - I.y * a.y, I.z * al.y + I.y * a.x, I.w * al.z);
+              float3 f = f3(I.x * a.x + I.y * al.y, I.x * a.y - I.y * al.x, I.x * a.z);
+              if (mine && (tw & kOffax)) {
+                const Force6 t = offaxis_tethers(__ldg(g.topo2 + me), al, a, s.att, s.ao, s.ak, s.Ap, P.h * P.h);
+                n = n + t.n; f = f + t.f;
+              }
+              if (l == ntop - 1) {                               // children (if any) are in shared memory
+                if (mine) {
+#pragma unroll 1
+                  for (int k = 0; k < nc; k++) {
+                    const float4 cu = PL[7 * (fc + k)], cv = PL[7 * (fc + k) + 1];
+                    n = n + f3(cu.x, cu.y, cu.z);
+                    f = f + f3(cu.w, cv.x, cv.y);
+                  }
+                }
+              } else {                                           // children are lanes fc .. fc + nc - 1
+#pragma unroll 1
+                for (int k = 0; k < top_maxc; k++) {
+                  const int src = min(fc + k, 31);
+                  float3 cn, cf;
+                  cn.x = __shfl_sync(0xffffffffu, un.x, src); cn.y = __shfl_sync(0xffffffffu, un.y, src);
+                  cn.z = __shfl_sync(0xffffffffu, un.z, src);
+                  cf.x = __shfl_sync(0xffffffffu, uf.x, src); cf.y = __shfl_sync(0xffffffffu, uf.y, src);
+                  cf.z = __shfl_sync(0xffffffffu, uf.z, src);
+                  if (k < nc) { n = n + cn; f = f + cf; }
+                }
+              }
+              if (mine) {
+                t1 = j.c2 * n.x + j.s2 * n.z + pd.z * pd.x;
+                t2 = n.y + pd.w * pd.y;
+                uf = mulT(j.E, f);
+                un = mulT(j.E, n);
+                un.x -= j.rz * uf.y; un.y += j.rz * uf.x;
+              }
+            }
+            if (tid < ntopN) {
+              reinterpret_cast<float2 *>(rec + 1)[1] = make_float2(t1, t2);
+              pAp_part += pd.x * t1 + pd.y * t2;
+            }
           }
           float rz_p = 0.f, rr_p = 0.f;
           if (first) {                                 // r = b - A x, z = P^-1 r, p = z
