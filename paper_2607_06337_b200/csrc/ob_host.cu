@@ -45,7 +45,7 @@ struct ob_ctx {
   unsigned char *dev_base = nullptr;
   // k_step launch geometry per size class: worlds [cls_off, cls_off + cls_n) of the order list
   int cls_off[kNumClasses] = {}, cls_n[kNumClasses] = {}, cls_grid[kNumClasses] = {}, cls_smem[kNumClasses] = {};
-  int main_cls = 0, launches = 0;
+  int main_cls = 0, launches = 0, n_sm = 0;
   int max_Np = 0, max_Ap = 0;
   size_t ev_cap = 0;
   uint64_t h2d_bytes = 0, d2h_bytes = 0, kernel_launches = 0, step_calls = 0;
@@ -504,6 +504,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   int n_sm = 0, dev = 0;
   if (e == cudaSuccess) e = cudaGetDevice(&dev);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  ctx->n_sm = n_sm;
   for (int k = 0; k < kNumClasses && e == cudaSuccess; k++) {
     if (!ctx->cls_n[k]) continue;
     int per_sm = 0;
@@ -609,7 +610,7 @@ int ob_step(ob_ctx *ctx, int n) {
   for (int k = kNumClasses - 1; k >= 0; k--) {      // the class of the largest worlds first
     if (!ctx->cls_n[k]) continue;
     CU(launch_step(ctx->dev, k, ctx->dev.order + ctx->cls_off[k], ctx->cls_n[k], ctx->dev.queue + k, n,
-                   ctx->cls_grid[k], ctx->cls_smem[k], ctx->stream));
+                   ctx->cls_grid[k], ctx->cls_smem[k], ctx->n_sm, ctx->stream));
     ctx->launches += 1;
     ctx->kernel_launches += 1;
   }

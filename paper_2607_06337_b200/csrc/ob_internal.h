@@ -107,7 +107,7 @@ struct DevCtx {
 //      runs over any number of links.
 struct StepClass { int nt, lpt, min_ctas; };
 constexpr int kNumClasses = 4;
-constexpr StepClass kStepClasses[kNumClasses] = {{128, 2, 6}, {256, 2, 3}, {512, 2, 1}, {512, 3, 1}};
+constexpr StepClass kStepClasses[kNumClasses] = {{128, 2, 6}, {192, 3, 3}, {512, 2, 1}, {512, 3, 1}};
 constexpr int kMaxLinksOnChip = 512 * 3;
 constexpr int kMaxChildren = 15;     // children per link (4 bits of the packed topology word)
 inline int step_class_of(int Np) {   // host only
@@ -141,7 +141,7 @@ __host__ __device__ inline int step_smem_bytes(int Np, int Ap, int NIp, int nlev
 cudaError_t launch_rest_pose(const DevCtx &c, int total_links_padded, int total_apples_padded, cudaStream_t s);
 cudaError_t launch_randomize(const DevCtx &c, unsigned long long seed, int redraw, cudaStream_t s);
 cudaError_t launch_step(const DevCtx &c, int cls, const int32_t *order, int n_in_class, int32_t *queue, int n_steps,
-                        int grid, int smem, cudaStream_t s);
+                        int grid, int smem, int n_sm, cudaStream_t s);
 cudaError_t launch_pose(const DevCtx &c, int world, cudaStream_t s);
 cudaError_t step_kernel_setup(int cls, int smem_bytes, int *max_blocks_per_sm);
 

@@ -28,7 +28,7 @@
 //   PD       (p, diagonal terms arm + (h c_d + h^2) K); B2 borrows .xy
 //   C0..C2   E (parent -> link rotation, row-major), c2, s2, parent length
 //   C3       effective link inertia (m, m c, I about the joint, I_zz) incl. on-axis virtual tether masses (A15)
-//   G        b after B1, then 1 / diag(A) after B2 (both end up in the owner's registers)
+//   G        b after B1 (it moves into the owner's registers), then 1 / diag(A) after B2
 //   T        packed topology word: parent | first child << 11 | children << 22 | flags
 //
 // Spatial vectors are [angular; linear at the link origin] in link coordinates.  Link frame: origin at the
@@ -165,50 +165,206 @@ __device__ __forceinline__ void store_jt(float4 *P, const int i, const Jt &j) {
   P[7 * i + 5] = make_float4(j.E.a[8], j.c2, j.s2, j.rz);
 }
 
-// kinematic quantities of one link that the bias pass hands from its top-down half to its bottom-up half
-struct Kin {
-  M3 dR;               // R - R0 (displacement form)
-  double dpx, dpy, dpz; // origin - rest origin; fp64: the tether stretch is the small difference of two sums
-                        // along the chain and k_s times its rounding error is what the thinnest twigs feel
-  float3 om, vl;       // spatial velocity
-  float3 al, aln;      // bias spatial acceleration (gravity as base acceleration)
-};
+// ------------------------------------------------------------------------------------------------------
+// phase C: A v for one link.  mv_down: accelerations from the parent (the trunk reads the zero column).
+// mv_up: f = I a + children, project on S (+ diagonal terms) -> A p (M1[i].zw), publish (n, f) in the parent
+// frame; returns p . (A p) of this link.  Mailbox: M0[i] = (x, y, z of the angular part, x of the linear part),
+// M1[i].xy = (y, z of the linear part).
+// ------------------------------------------------------------------------------------------------------
+// virtual tether masses off the link axis (rare: the workloads hang apples on the axis), one by one.  Everything
+// goes in and out by value so that nothing of the caller is forced into local memory.
+struct Force6 { float3 n, f; };
+__device__ __noinline__ Force6 offaxis_tethers(const int4 t2, const float3 al, const float3 a, const unsigned char *att,
+                                               const float *ao, const float *ak, const int Ap, const float hh) {
+  Force6 r;
+  r.n = f3(0, 0, 0); r.f = f3(0, 0, 0);
+  const int ast = t2.x & 0xffff, nap = t2.x >> 16;
+  for (int q = ast; q < ast + nap; q++) {
+    if (!att[q]) continue;
+    const float3 o = f3(ao[q], ao[Ap + q], ao[2 * Ap + q]);
+    if (o.x == 0.f && o.y == 0.f) continue;                 // already inside (m, mc, Io)
+    const float mv = hh * ak[q];
+    const float3 fp = mv * (a + cross(al, o));
+    r.f = r.f + fp;
+    r.n = r.n + cross(o, fp);
+  }
+  return r;
+}
+
+__device__ __forceinline__ void mv_down(const Jt &j, const float4 *P, const uint32_t tw, const float4 pd, float3 &al,
+                                        float3 &a) {
+  const float4 *par = P + 7 * (int)(tw & kParMask);
+  const float4 u = par[0], v = par[1];
+  const float3 alp = f3(u.x, u.y, u.z), ap = f3(u.w, v.x, v.y);
+  al = mul(j.E, alp) + f3(j.c2 * pd.x, pd.y, j.s2 * pd.x);
+  a = mul(j.E, f3(ap.x + alp.y * j.rz, ap.y - alp.x * j.rz, ap.z));
+}
+
+// children of a link out of shared memory, added in ascending order: the first four with all loads in flight
+// at once (a missing child reads the zero record), the rest one by one
+__device__ __forceinline__ void gather_children(const float4 *P, const float4 *zero_rec, const int fc, const int nc,
+                                                float3 &n, float3 &f) {
+  const float4 *ch = P + 7 * fc;
+  float4 cu[4], cv[4];
+#pragma unroll
+  for (int k = 0; k < 4; k++) {
+    const float4 *q = k < nc ? ch + 7 * k : zero_rec;
+    cu[k] = q[0]; cv[k] = q[1];
+  }
+#pragma unroll
+  for (int k = 0; k < 4; k++) {
+    n = n + f3(cu[k].x, cu[k].y, cu[k].z);
+    f = f + f3(cu[k].w, cv[k].x, cv[k].y);
+  }
+#pragma unroll 1
+  for (int k = 4; k < nc; k++) {
+    const float4 u = ch[7 * k], v = ch[7 * k + 1];
+    n = n + f3(u.x, u.y, u.z);
+    f = f + f3(u.w, v.x, v.y);
+  }
+}
+
+template <bool GATHER>
+__device__ __forceinline__ float mv_up(const Jt &j, float4 *P, const float4 *zero_rec, const int i, const uint32_t tw,
+                                       const float4 pd, const float3 al, const float3 a, const Sm &s, const Gm &g,
+                                       const DevCtx &c) {
+  float4 *rec = P + 7 * i;
+  const float4 I = rec[6];                                    // (m, m c, I about the joint, I_zz)
+  float3 n = f3(I.z * al.x - I.y * a.y, I.z * al.y + I.y * a.x, I.w * al.z);
+  float3 f = f3(I.x * a.x + I.y * al.y, I.x * a.y - I.y * al.x, I.x * a.z);
+  if (tw & kOffax) {
+    const Force6 t = offaxis_tethers(__ldg(g.topo2 + i), al, a, s.att, s.ao, s.ak, s.Ap, c.P.h * c.P.h);
+    n = n + t.n; f = f + t.f;
+  }
+  if (GATHER) gather_children(P, zero_rec, (int)((tw >> kChShift) & kParMask), (int)((tw >> kNcShift) & kNcMask), n, f);
+  const float t1 = j.c2 * n.x + j.s2 * n.z + pd.z * pd.x;     // pd = (p0, p1, dt0, dt1)
+  const float t2 = n.y + pd.w * pd.y;
+  const float3 fp = mulT(j.E, f);                             // the trunk publishes into its own column, which nobody reads
+  float3 np = mulT(j.E, n);
+  np.x -= j.rz * fp.y; np.y += j.rz * fp.x;
+  rec[0] = make_float4(np.x, np.y, np.z, fp.x);
+  rec[1] = make_float4(fp.y, fp.z, t1, t2);
+  return pd.x * t1 + pd.y * t2;
+}
 
 // ------------------------------------------------------------------------------------------------------
-// bias force of one link: f = I a + v x* I v - tether reactions - user wrenches (RNEA with qdd = 0)
+// The once-per-step phases, cut into passes that each keep a small working set in registers (a spilled
+// register costs an L2 round trip here: the three CTAs of an SM leave the L1 only ~28 KB):
+//   A0  flat      per link, no dependence on other links: joint transform E (-> C0..C2), R0 (RxRy - I)
+//                 (-> M0, M1, PD.x), spring-damper part of the rhs (-> G), diagonal terms (-> PD.w)
+//   A1  top-down  displacement-form FK: dR, dp of every link (-> M0, M1, PD.xyz, C3), snapped flags
+//   A2  top-down  velocities and bias accelerations (inner links publish 12 floats in the overflow); own bias
+//                 force of every link incl. tethers and wrenches; a leaf finishes at once, an inner link
+//                 parks (n, f) in M0, M1.xy
+//   B1  bottom-up inner links: own (n, f) + children -> rhs b (-> G), (n, f) for the parent
 // ------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void bias_force(const int i, const Kin &k, const uint32_t tw, const Sm &s, const Gm &g,
-                                           const DevCtx &c, float3 &n, float3 &f) {
+
+// a double carried as two floats (hi + lo): 48 bits, plenty for a displacement summed along <= 2000 links
+__device__ __forceinline__ float2 split2(const double v) {
+  const float hi = (float)v;
+  return make_float2(hi, (float)(v - (double)hi));
+}
+__device__ __forceinline__ double join2(const float hi, const float lo) { return (double)hi + (double)lo; }
+
+// ---- A0 ----
+__device__ __forceinline__ void link_prepare(const int i, const Sm &s, const Gm &g, const DevCtx &c) {
+  const ob_params &P = c.P;
+  const int Np = s.Np;
+  const float2 th = g.q2[i], w = g.w2[i];
+  const float4 qt = __ldg(g.quat + i);
+  const float Ki = __ldg(g.K + i);
+  const float rz = (s.T[i] & kTrunk) ? 0.f : __ldg(g.rz + i);
+  M3 R0;
+#pragma unroll
+  for (int q = 0; q < 9; q++) R0.a[q] = __ldg(g.R0 + (size_t)q * Np + i);
+  const float2 sc1 = sincos2(th.x), sc2 = sincos2(th.y);
+  const float s1 = sc1.x, c1 = sc1.y, s2 = sc2.x, c2 = sc2.y;
+  const float vc1 = cos_minus_one(s1, c1), vc2 = cos_minus_one(s2, c2);
+  M3 XY;                                                           // Rx(th1) Ry(th2)
+  XY.a[0] = c2;       XY.a[1] = 0.f; XY.a[2] = s2;
+  XY.a[3] = s1 * s2;  XY.a[4] = c1;  XY.a[5] = -s1 * c2;
+  XY.a[6] = -c1 * s2; XY.a[7] = s1;  XY.a[8] = c1 * c2;
+  {
+    const M3 Rrel = mul(quat_to_mat(qt), XY);
+    Jt j;                                                          // E = Rrel^T
+#pragma unroll
+    for (int r = 0; r < 3; r++)
+#pragma unroll
+      for (int cc = 0; cc < 3; cc++) j.E.a[3 * r + cc] = Rrel.a[3 * cc + r];
+    j.c2 = c2; j.s2 = s2; j.rz = rz;
+    store_jt(s.P, i, j);
+  }
+  // displacement-form FK, own part: R0_i (RxRy - I)
+  XY.a[0] = vc2; XY.a[4] = vc1; XY.a[8] = fmaf(vc1, vc2, vc1 + vc2);
+  const M3 t2m = mul(R0, XY);
+  // spring-damper part of the rhs and of the diagonal (Eq. 4); a ruptured joint has K = D = 0
+  const float Kt = (s.T[i] & kRuptured) ? 0.f : Ki, Dt = P.c_d * Kt;
+  s.G[i] = make_float2(Kt * th.x + (Dt + P.h * Kt) * w.x, Kt * th.y + (Dt + P.h * Kt) * w.y);
+  s.P[7 * i] = make_float4(t2m.a[0], t2m.a[1], t2m.a[2], t2m.a[3]);
+  s.P[7 * i + 1] = make_float4(t2m.a[4], t2m.a[5], t2m.a[6], t2m.a[7]);
+  s.P[7 * i + 2] = make_float4(t2m.a[8], 0.f, 0.f, (P.h * P.c_d + P.h * P.h) * Kt);
+}
+
+// ---- A1 ----  dR_i = dR_p Rrel + R0_i (RxRy - I),  dp_i = dp_p + dR_p (0,0,rz)
+__device__ __forceinline__ void link_fk(const int i, const Sm &s) {
+  float4 *rec = s.P + 7 * i;
+  uint32_t tw = s.T[i];
+  const float4 *par = s.P + 7 * (int)(tw & kParMask);             // the trunk reads the zero record
+  const float4 p0 = par[0], p1 = par[1], p2 = par[2], p3 = par[6];
+  const uint32_t snapped_p = (tw & kTrunk) ? 0u : (s.T[tw & kParMask] & kSnapped);
+  const float4 o0 = rec[0], o1 = rec[1];
+  const float o8 = rec[2].x;
+  const Jt j = load_jt(s.P, i);
+  M3 dRp, Rrel, dR;
+  dRp.a[0] = p0.x; dRp.a[1] = p0.y; dRp.a[2] = p0.z; dRp.a[3] = p0.w;
+  dRp.a[4] = p1.x; dRp.a[5] = p1.y; dRp.a[6] = p1.z; dRp.a[7] = p1.w; dRp.a[8] = p2.x;
+#pragma unroll
+  for (int r = 0; r < 3; r++)
+#pragma unroll
+    for (int cc = 0; cc < 3; cc++) Rrel.a[3 * r + cc] = j.E.a[3 * cc + r];
+  dR = mul(dRp, Rrel);
+  dR.a[0] += o0.x; dR.a[1] += o0.y; dR.a[2] += o0.z; dR.a[3] += o0.w;
+  dR.a[4] += o1.x; dR.a[5] += o1.y; dR.a[6] += o1.z; dR.a[7] += o1.w; dR.a[8] += o8;
+  // fp64: the tether stretch is the small difference of two sums along the chain, and k_s times its rounding
+  // error is what the thinnest twigs feel
+  const double rz = (double)j.rz;
+  const float2 dx = split2(join2(p2.y, p2.z) + rz * (double)dRp.a[2]);
+  const float2 dy = split2(join2(p3.x, p3.y) + rz * (double)dRp.a[5]);
+  const float2 dz = split2(join2(p3.z, p3.w) + rz * (double)dRp.a[8]);
+  const float dt0 = rec[2].w;
+  rec[0] = make_float4(dR.a[0], dR.a[1], dR.a[2], dR.a[3]);
+  rec[1] = make_float4(dR.a[4], dR.a[5], dR.a[6], dR.a[7]);
+  rec[2] = make_float4(dR.a[8], dx.x, dx.y, dt0);
+  rec[6] = make_float4(dy.x, dy.y, dz.x, dz.y);
+  tw = (tw & ~kSnapped) | (((tw & kRuptured) || snapped_p) ? kSnapped : 0u);
+  s.T[i] = tw;
+}
+
+// tether reactions (Eq. 6 / Eq. 7) and user wrenches on one link, subtracted from its bias
+// force (n, f); also leaves the tether force and |f_s| of each apple for phase D.  Only links that carry apples or
+// a wrench come here.
+__device__ __noinline__ Force6 external_forces(const int i, const float3 om, const float3 vl, const uint32_t tw,
+                                               const Sm &s, const Gm &g, const DevCtx &c) {
   const ob_params &P = c.P;
   const int Np = s.Np, Ap = s.Ap;
-  const float4 c4 = __ldg(g.c4 + i);
-  const float m = c4.x, mc = c4.y, Io = c4.z, Iz = c4.w;
-  const float3 om = k.om, vl = k.vl, al = k.al, aln = k.aln;
-  // f = I a + v x* I v  (cylinder: com on +z)
-  n = f3(Io * al.x - mc * aln.y, Io * al.y + mc * aln.x, Iz * al.z);
-  f = f3(m * aln.x + mc * al.y, m * aln.y - mc * al.x, m * aln.z);
-  const float3 hn = f3(Io * om.x - mc * vl.y, Io * om.y + mc * vl.x, Iz * om.z);
-  const float3 hf = f3(m * vl.x + mc * om.y, m * vl.y - mc * om.x, m * vl.z);
-  n = n + cross(om, hn) + cross(vl, hf);
-  f = f + cross(om, hf);
-
-  const int nwr = s.wr->n;
-  bool wr_here = false;
-  for (int q = 0; q < nwr; q++) wr_here |= s.wr->body[q] == i;
-  if (!(tw & kHasApples) && !wr_here) return;
-
-  M3 R;                                                                   // world rotation R0 + dR
+  Force6 out;
+  out.n = f3(0, 0, 0); out.f = f3(0, 0, 0);
+  const float4 *rec = s.P + 7 * i;
+  const float4 r0 = rec[0], r1 = rec[1], r2 = rec[2], r3 = rec[6];
+  M3 dR, R;                                                               // world rotation R0 + dR
+  dR.a[0] = r0.x; dR.a[1] = r0.y; dR.a[2] = r0.z; dR.a[3] = r0.w;
+  dR.a[4] = r1.x; dR.a[5] = r1.y; dR.a[6] = r1.z; dR.a[7] = r1.w; dR.a[8] = r2.x;
+  const double dpx = join2(r2.y, r2.z), dpy = join2(r3.x, r3.y), dpz = join2(r3.z, r3.w);
 #pragma unroll
-  for (int q = 0; q < 9; q++) R.a[q] = __ldg(g.R0 + (size_t)q * Np + i) + k.dR.a[q];
-  // tethers on this link (Eq. 6, Eq. 7): everything about the hang point is at hand here
+  for (int q = 0; q < 9; q++) R.a[q] = __ldg(g.R0 + (size_t)q * Np + i) + dR.a[q];
   const int4 t2 = __ldg(g.topo2 + i);
   const int ast = t2.x & 0xffff, nap = t2.x >> 16;
   const float eta_h = P.tether_implicit ? P.h : 0.f;
   for (int a = ast; a < ast + nap; a++) {
     if (!s.att[a]) continue;
     const float3 o = f3(s.ao[a], s.ao[Ap + a], s.ao[2 * Ap + a]);
-    const float3 dro = mul(k.dR, o);
-    const double dhx = k.dpx + (double)dro.x, dhy = k.dpy + (double)dro.y, dhz = k.dpz + (double)dro.z;   // x_hang - anchor
+    const float3 dro = mul(dR, o);
+    const double dhx = dpx + (double)dro.x, dhy = dpy + (double)dro.y, dhz = dpz + (double)dro.z;   // x_hang - anchor
     const float ks = s.ak[a], cdamp = s.ac[a], ma = s.am[a];
     // x_a - x_hang = u + sag - dh with the rest sag m g / k_s (u is stored relative to the rest position)
     const float gk = ma / ks;
@@ -225,167 +381,105 @@ __device__ __forceinline__ void bias_force(const int i, const Kin &k, const uint
     const float nr = sqrtf(dot(fr, fr));
     if (nr > P.react_max) fr = (P.react_max / nr) * fr;                   // clamp
     const float3 fl = mulT(R, fr);
-    f = f - fl;
-    n = n - cross(o, fl);
+    out.f = out.f - fl;
+    out.n = out.n - cross(o, fl);
   }
   // user wrenches on this link (disabled on snapped sub-trees)
+  const int nwr = s.wr->n;
   for (int q = 0; q < nwr; q++) {
     if (s.wr->body[q] != i) continue;
     if ((tw & kSnapped) && P.forces_off_on_snapped) continue;
     const float3 fl = mulT(R, f3(s.wr->force[q][0], s.wr->force[q][1], s.wr->force[q][2]));
     const float3 pt = f3(s.wr->point[q][0], s.wr->point[q][1], s.wr->point[q][2]);
-    f = f - fl;
-    n = n - cross(pt, fl);
+    out.f = out.f - fl;
+    out.n = out.n - cross(pt, fl);
   }
+  return out;
 }
 
-// project the accumulated bias force on the joint axes -> rhs b (G[i]), the diagonal damping / stiffness terms
-// (PD[i].zw), and publish (n, f) in the parent frame (M0[i], M1[i].xy)
+// project the accumulated bias force on the joint axes -> rhs b (G[i]), the diagonal terms of both DoF (PD[i].zw),
+// and publish (n, f) in the parent frame (M0[i], M1[i].xy)
 __device__ __forceinline__ void finish_bias(const Jt &j, const int i, const uint32_t tw, float3 n, float3 f,
                                             const Sm &s, const Gm &g, const DevCtx &c) {
   const ob_params &P = c.P;
-  const int Np = s.Np, S = s.S;
-  const float tau1 = j.c2 * n.x + j.s2 * n.z, tau2 = n.y;
-  const float Kt = (tw & kRuptured) ? 0.f : __ldg(g.K + i), Dt = P.c_d * Kt;
-  const float2 th = g.q2[i], w = g.w2[i];
-  const float b1 = P.h * (-tau1 - Kt * th.x - (Dt + P.h * Kt) * w.x);
-  const float b2 = P.h * (-tau2 - Kt * th.y - (Dt + P.h * Kt) * w.y);
-  s.G[i] = make_float2(b1, b2);
-  float dt0 = (P.h * P.c_d + P.h * P.h) * Kt, dt1 = dt0;
+  float4 *rec = s.P + 7 * i;
+  const float2 kq = s.G[i];
+  s.G[i] = make_float2(P.h * (-(j.c2 * n.x + j.s2 * n.z) - kq.x), P.h * (-n.y - kq.y));
+  float dt0 = rec[2].w, dt1 = dt0;
   if (g.arm) {
     dt0 += __ldg(g.arm + i);
-    dt1 += __ldg(g.arm + Np + i);
+    dt1 += __ldg(g.arm + s.Np + i);
   }
-  reinterpret_cast<float2 *>(s.P + 7 * i + 2)[1] = make_float2(dt0, dt1);    // arm + (h c_d + h^2) K per DoF
+  reinterpret_cast<float2 *>(rec + 2)[1] = make_float2(dt0, dt1);            // arm + (h c_d + h^2) K per DoF
   if (!(tw & kTrunk)) {
     const float3 fp = mulT(j.E, f);
     float3 np = mulT(j.E, n);
     np.x -= j.rz * fp.y; np.y += j.rz * fp.x;
-    s.P[7 * i] = make_float4(np.x, np.y, np.z, fp.x);
-    *reinterpret_cast<float2 *>(s.P + 7 * i + 1) = make_float2(fp.y, fp.z);
+    rec[0] = make_float4(np.x, np.y, np.z, fp.x);
+    *reinterpret_cast<float2 *>(rec + 1) = make_float2(fp.y, fp.z);
   }
 }
 
-// ------------------------------------------------------------------------------------------------------
-// phase A for one link (top-down); a leaf goes straight on to its phase-B1 half
-// ------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void down_bias(const int i, const Sm &s, const Gm &g, const DevCtx &c) {
-  const int Np = s.Np, NIp = s.NIp, S = s.S;
+// ---- A2 ----  velocity, bias acceleration (gravity as base acceleration), own bias force
+//               f = I a + v x* I v - tether reactions - user wrenches  (RNEA with qdd = 0)
+__device__ __forceinline__ void link_bias(const int i, const Sm &s, const Gm &g, const DevCtx &c) {
   const ob_params &P = c.P;
-  uint32_t tw = s.T[i];
-  const float2 th = g.q2[i], w = g.w2[i];
-  const float th1 = th.x, th2 = th.y, w1 = w.x, w2 = w.y;
-  const float2 sc1 = sincos2(th1), sc2 = sincos2(th2);
-  const float s1 = sc1.x, c1 = sc1.y, s2 = sc2.x, c2 = sc2.y;
-  const float vc1 = cos_minus_one(s1, c1), vc2 = cos_minus_one(s2, c2);
-  const M3 Q = quat_to_mat(__ldg(g.quat + i));
-  M3 XY;                                                           // Rx(th1) Ry(th2)
-  XY.a[0] = c2;       XY.a[1] = 0.f; XY.a[2] = s2;
-  XY.a[3] = s1 * s2;  XY.a[4] = c1;  XY.a[5] = -s1 * c2;
-  XY.a[6] = -c1 * s2; XY.a[7] = s1;  XY.a[8] = c1 * c2;
-  const M3 Rrel = mul(Q, XY);
-  Jt j;                                                            // E = Rrel^T
-#pragma unroll
-  for (int r = 0; r < 3; r++)
-#pragma unroll
-    for (int cc = 0; cc < 3; cc++) j.E.a[3 * r + cc] = Rrel.a[3 * cc + r];
-  j.c2 = c2; j.s2 = s2;
-  const int4 t2 = __ldg(g.topo2 + i);
-
-  // parent quantities (world = parent of the trunk: at rest, spatial acceleration (0; -g))
-  M3 dRp;
-  double dppx = 0.0, dppy = 0.0, dppz = 0.0;
+  const int NIp = s.NIp;
+  const uint32_t tw = s.T[i];
+  const float2 w = g.w2[i];
+  const float4 c4 = __ldg(g.c4 + i);
+  const int ty = __ldg(&g.topo2[i].y);                            // inner slot | parent's inner slot << 16
+  const Jt j = load_jt(s.P, i);
   float3 wp = f3(0, 0, 0), vp = f3(0, 0, 0), alp = f3(0, 0, 0);
-  float3 ap = f3(-P.gravity[0], -P.gravity[1], -P.gravity[2]);
-  uint32_t snapped_p = 0;
-  float rz = 0.f;
-#pragma unroll
-  for (int q = 0; q < 9; q++) dRp.a[q] = 0.f;
+  float3 ap = f3(-P.gravity[0], -P.gravity[1], -P.gravity[2]);   // world = parent of the trunk: at rest, (0; -g)
   if (!(tw & kTrunk)) {
-    const int par = (int)(tw & kParMask), ps = (int)((uint32_t)t2.y >> 16);
-    const float4 t0 = s.P[7 * par], t1 = s.P[7 * par + 1], t2v = s.P[7 * par + 2], t3 = s.P[7 * par + 6],
-                 t4 = s.ovf[ps], t5 = s.ovf[NIp + ps];
-    const double2 d0 = *reinterpret_cast<const double2 *>(s.ovf + 2 * NIp + ps);
-    dRp.a[0] = t0.x; dRp.a[1] = t0.y; dRp.a[2] = t0.z; dRp.a[3] = t0.w;
-    dRp.a[4] = t1.x; dRp.a[5] = t1.y; dRp.a[6] = t1.z; dRp.a[7] = t1.w;
-    dRp.a[8] = t2v.x; wp = f3(t2v.y, t2v.z, t2v.w);
-    vp = f3(t3.x, t3.y, t3.z); alp = f3(t3.w, t4.x, t4.y);
-    ap = f3(t4.z, t4.w, t5.x);
-    dppx = (double)t5.y + (double)t5.z; dppy = d0.x; dppz = d0.y;      // x as a float pair, y and z as doubles
-    snapped_p = s.T[par] & kSnapped;
-    rz = __ldg(g.rz + i);
+    const int ps = (int)((uint32_t)ty >> 16);
+    const float4 t0 = s.ovf[ps], t1 = s.ovf[NIp + ps], t2 = s.ovf[2 * NIp + ps];
+    wp = f3(t0.x, t0.y, t0.z); vp = f3(t0.w, t1.x, t1.y);
+    alp = f3(t1.z, t1.w, t2.x); ap = f3(t2.y, t2.z, t2.w);
   }
-  j.rz = rz;
-  store_jt(s.P, i, j);
-  // displacement-form FK: R_i = R0_i + dR_i,  dR_i = dR_p Rrel + R0_i (RxRy - I);  dp_i = dp_p + dR_p (0,0,rz)
-  Kin k;
-  {
-    M3 R0, G = XY;
-#pragma unroll
-    for (int q = 0; q < 9; q++) R0.a[q] = __ldg(g.R0 + (size_t)q * Np + i);
-    G.a[0] = vc2; G.a[4] = vc1; G.a[8] = fmaf(vc1, vc2, vc1 + vc2);
-    const M3 t1m = mul(dRp, Rrel), t2m = mul(R0, G);
-#pragma unroll
-    for (int q = 0; q < 9; q++) k.dR.a[q] = t1m.a[q] + t2m.a[q];
+  const float rz = j.rz, c2 = j.c2, s2 = j.s2;
+  const float3 vJ = f3(c2 * w.x, w.y, s2 * w.x);
+  const float3 om = mul(j.E, wp) + vJ;
+  const float3 vl = mul(j.E, f3(vp.x + wp.y * rz, vp.y - wp.x * rz, vp.z));
+  const float ww = w.x * w.y;
+  const float3 al = mul(j.E, alp) + f3(-s2 * ww, 0.f, c2 * ww) + cross(om, vJ);
+  const float3 aln = mul(j.E, f3(ap.x + alp.y * rz, ap.y - alp.x * rz, ap.z)) + cross(vl, vJ);
+  const bool inner = ((tw >> kNcShift) & kNcMask) != 0u;
+  if (inner) {
+    const int is = ty & 0xffff;
+    s.ovf[is] = make_float4(om.x, om.y, om.z, vl.x);
+    s.ovf[NIp + is] = make_float4(vl.y, vl.z, al.x, al.y);
+    s.ovf[2 * NIp + is] = make_float4(al.z, aln.x, aln.y, aln.z);
   }
-  k.dpx = dppx + (double)rz * (double)dRp.a[2];
-  k.dpy = dppy + (double)rz * (double)dRp.a[5];
-  k.dpz = dppz + (double)rz * (double)dRp.a[8];
-
-  // velocity and (bias) spatial acceleration in link coordinates
-  const float3 vJ = f3(c2 * w1, w2, s2 * w1);
-  k.om = mul(j.E, wp) + vJ;
-  k.vl = mul(j.E, f3(vp.x + wp.y * rz, vp.y - wp.x * rz, vp.z));
-  const float ww = w1 * w2;
-  k.al = mul(j.E, alp) + f3(-s2 * ww, 0.f, c2 * ww) + cross(k.om, vJ);
-  k.aln = mul(j.E, f3(ap.x + alp.y * rz, ap.y - alp.x * rz, ap.z)) + cross(k.vl, vJ);
-
-  tw = (tw & ~kSnapped) | (((tw & kRuptured) || snapped_p) ? kSnapped : 0u);
-  s.T[i] = tw;
-
-  if ((tw >> kNcShift) & kNcMask) {
-    const int is = t2.y & 0xffff;
-    s.P[7 * i] = make_float4(k.dR.a[0], k.dR.a[1], k.dR.a[2], k.dR.a[3]);
-    s.P[7 * i + 1] = make_float4(k.dR.a[4], k.dR.a[5], k.dR.a[6], k.dR.a[7]);
-    s.P[7 * i + 2] = make_float4(k.dR.a[8], k.om.x, k.om.y, k.om.z);
-    s.P[7 * i + 6] = make_float4(k.vl.x, k.vl.y, k.vl.z, k.al.x);
-    s.ovf[is] = make_float4(k.al.y, k.al.z, k.aln.x, k.aln.y);
-    const float dxh = (float)k.dpx;
-    s.ovf[NIp + is] = make_float4(k.aln.z, dxh, (float)(k.dpx - (double)dxh), 0.f);
-    *reinterpret_cast<double2 *>(s.ovf + 2 * NIp + is) = make_double2(k.dpy, k.dpz);
+  // f = I a + v x* I v  (cylinder: com on +z)
+  const float m = c4.x, mc = c4.y, Io = c4.z, Iz = c4.w;
+  float3 n = f3(Io * al.x - mc * aln.y, Io * al.y + mc * aln.x, Iz * al.z);
+  float3 f = f3(m * aln.x + mc * al.y, m * aln.y - mc * al.x, m * aln.z);
+  const float3 hn = f3(Io * om.x - mc * vl.y, Io * om.y + mc * vl.x, Iz * om.z);
+  const float3 hf = f3(m * vl.x + mc * om.y, m * vl.y - mc * om.x, m * vl.z);
+  n = n + cross(om, hn) + cross(vl, hf);
+  f = f + cross(om, hf);
+  bool ext = (tw & kHasApples) != 0u;
+  for (int q = 0; q < s.wr->n; q++) ext |= s.wr->body[q] == i;
+  if (ext) {
+    const Force6 e = external_forces(i, om, vl, tw, s, g, c);
+    n = n + e.n; f = f + e.f;
+  }
+  if (inner) {                                                    // parked until B1 adds the children
+    s.P[7 * i] = make_float4(n.x, n.y, n.z, f.x);
+    *reinterpret_cast<float2 *>(s.P + 7 * i + 1) = make_float2(f.y, f.z);
   } else {
-    float3 n, f;
-    bias_force(i, k, tw, s, g, c, n, f);
     finish_bias(j, i, tw, n, f, s, g, c);
   }
 }
 
-// phase B1 for one inner link: its own bias force (from the kinematics it published on the way down) plus
-// what its children sent up
-__device__ __forceinline__ void up_bias(const int i, const uint32_t tw, const Sm &s, const Gm &g, const DevCtx &c) {
-  const int NIp = s.NIp, S = s.S;
-  const int is = __ldg(g.topo2 + i).y & 0xffff;
-  Kin k;
-  {
-    const float4 t0 = s.P[7 * i], t1 = s.P[7 * i + 1], t2v = s.P[7 * i + 2], t3 = s.P[7 * i + 6], t4 = s.ovf[is],
-                 t5 = s.ovf[NIp + is];
-    k.dR.a[0] = t0.x; k.dR.a[1] = t0.y; k.dR.a[2] = t0.z; k.dR.a[3] = t0.w;
-    k.dR.a[4] = t1.x; k.dR.a[5] = t1.y; k.dR.a[6] = t1.z; k.dR.a[7] = t1.w;
-    const double2 d0 = *reinterpret_cast<const double2 *>(s.ovf + 2 * NIp + is);
-    k.dR.a[8] = t2v.x; k.om = f3(t2v.y, t2v.z, t2v.w);
-    k.vl = f3(t3.x, t3.y, t3.z); k.al = f3(t3.w, t4.x, t4.y);
-    k.aln = f3(t4.z, t4.w, t5.x);
-    k.dpx = (double)t5.y + (double)t5.z; k.dpy = d0.x; k.dpz = d0.y;
-  }
-  float3 n, f;
-  bias_force(i, k, tw, s, g, c, n, f);
-  const int fc = (int)((tw >> kChShift) & kParMask), nc = (int)((tw >> kNcShift) & kNcMask);
-  for (int ch = fc; ch < fc + nc; ch++) {
-    const float4 u = s.P[7 * ch];
-    const float2 v = *reinterpret_cast<const float2 *>(s.P + 7 * ch + 1);
-    n = n + f3(u.x, u.y, u.z);
-    f = f + f3(u.w, v.x, v.y);
-  }
+// ---- B1 ----  one inner link: its parked bias force plus what its children sent up
+__device__ __forceinline__ void link_bias_up(const int i, const uint32_t tw, const Sm &s, const Gm &g, const DevCtx &c) {
+  const float4 u0 = s.P[7 * i];
+  const float2 v0 = *reinterpret_cast<const float2 *>(s.P + 7 * i + 1);
+  float3 n = f3(u0.x, u0.y, u0.z), f = f3(u0.w, v0.x, v0.y);
+  gather_children(s.P, s.P + 7 * s.Np, (int)((tw >> kChShift) & kParMask), (int)((tw >> kNcShift) & kNcMask), n, f);
   finish_bias(load_jt(s.P, i), i, tw, n, f, s, g, c);
 }
 
@@ -456,99 +550,99 @@ __device__ __forceinline__ void up_inertia(const int i, const Sm &s, const Gm &g
   }
 }
 
-// ------------------------------------------------------------------------------------------------------
-// phase C: A v for one link.  mv_down: accelerations from the parent (the trunk reads the zero column).
-// mv_up: f = I a + children, project on S (+ diagonal terms) -> A p (M1[i].zw), publish (n, f) in the parent
-// frame; returns p . (A p) of this link.  Mailbox: M0[i] = (x, y, z of the angular part, x of the linear part),
-// M1[i].xy = (y, z of the linear part).
-// ------------------------------------------------------------------------------------------------------
-// virtual tether masses off the link axis (rare: the workloads hang apples on the axis), one by one.  Everything
-// goes in and out by value so that nothing of the caller is forced into local memory.
-struct Force6 { float3 n, f; };
-__device__ __noinline__ Force6 offaxis_tethers(const int4 t2, const float3 al, const float3 a, const unsigned char *att,
-                                               const float *ao, const float *ak, const int Ap, const float hh) {
-  Force6 r;
-  r.n = f3(0, 0, 0); r.f = f3(0, 0, 0);
-  const int ast = t2.x & 0xffff, nap = t2.x >> 16;
-  for (int q = ast; q < ast + nap; q++) {
-    if (!att[q]) continue;
-    const float3 o = f3(ao[q], ao[Ap + q], ao[2 * Ap + q]);
-    if (o.x == 0.f && o.y == 0.f) continue;                 // already inside (m, mc, Io)
-    const float mv = hh * ak[q];
-    const float3 fp = mv * (a + cross(al, o));
-    r.f = r.f + fp;
-    r.n = r.n + cross(o, fp);
-  }
-  return r;
-}
-
-__device__ __forceinline__ void mv_down(const Jt &j, const float4 *P, const uint32_t tw, const float4 pd, float3 &al,
-                                        float3 &a) {
-  const float4 *par = P + 7 * (int)(tw & kParMask);
-  const float4 u = par[0], v = par[1];
-  const float3 alp = f3(u.x, u.y, u.z), ap = f3(u.w, v.x, v.y);
-  al = mul(j.E, alp) + f3(j.c2 * pd.x, pd.y, j.s2 * pd.x);
-  a = mul(j.E, f3(ap.x + alp.y * j.rz, ap.y - alp.x * j.rz, ap.z));
-}
-
-__device__ __forceinline__ float mv_up(const Jt &j, float4 *P, const float4 *zero_rec, const int i, const uint32_t tw,
-                                       const float4 pd, const float3 al, const float3 a, const Sm &s, const Gm &g,
-                                       const DevCtx &c) {
-  float4 *rec = P + 7 * i;
-  const float4 I = rec[6];                                    // (m, m c, I about the joint, I_zz)
-  float3 n = f3(I.z * al.x - I.y * a.y, I.z * al.y + I.y * a.x, I.w * al.z);
-  float3 f = f3(I.x * a.x + I.y * al.y, I.x * a.y - I.y * al.x, I.x * a.z);
-  if (tw & kOffax) {
-    const Force6 t = offaxis_tethers(__ldg(g.topo2 + i), al, a, s.att, s.ao, s.ak, s.Ap, c.P.h * c.P.h);
-    n = n + t.n; f = f + t.f;
-  }
-  // children: the first four with all loads in flight at once (a missing child reads the zero record)
-  const float4 *ch = P + 7 * (int)((tw >> kChShift) & kParMask);
-  const int nc = (int)((tw >> kNcShift) & kNcMask);
-  {
-    float4 cu[4], cv[4];
-#pragma unroll
-    for (int k = 0; k < 4; k++) {
-      const float4 *q = k < nc ? ch + 7 * k : zero_rec;
-      cu[k] = q[0]; cv[k] = q[1];
-    }
-#pragma unroll
-    for (int k = 0; k < 4; k++) {
-      n = n + f3(cu[k].x, cu[k].y, cu[k].z);
-      f = f + f3(cu[k].w, cv[k].x, cv[k].y);
-    }
-  }
-#pragma unroll 1
-  for (int k = 4; k < nc; k++) {
-    const float4 u = ch[7 * k], v = ch[7 * k + 1];
-    n = n + f3(u.x, u.y, u.z);
-    f = f + f3(u.w, v.x, v.y);
-  }
-  const float t1 = j.c2 * n.x + j.s2 * n.z + pd.z * pd.x;     // pd = (p0, p1, dt0, dt1)
-  const float t2 = n.y + pd.w * pd.y;
-  const float3 fp = mulT(j.E, f);                             // the trunk publishes into its own column, which nobody reads
-  float3 np = mulT(j.E, n);
-  np.x -= j.rz * fp.y; np.y += j.rz * fp.x;
-  rec[0] = make_float4(np.x, np.y, np.z, fp.x);
-  rec[1] = make_float4(fp.y, fp.z, t1, t2);
-  return pd.x * t1 + pd.y * t2;
-}
-
 // fence after level l of a top-down sweep / after level l of a bottom-up sweep (see "Order" above)
 #define OB_FENCE_DOWN(l) { if ((l) + 1 < ntop) __syncwarp(); else __syncthreads(); }
 #define OB_FENCE_UP(l) { if ((l) < ntop) __syncwarp(); else __syncthreads(); }
+
+// ------------------------------------------------------------------------------------------------------
+// the once-per-step sweeps as functions of their own (not inlined): their register pressure (24 kinematic
+// quantities per link in flight) stays out of the allocation of the PCG loop.  The views of the world live in
+// shared memory (World), the context is the kernel's __grid_constant__ parameter.
+// ------------------------------------------------------------------------------------------------------
+struct World { Sm s; Gm g; int N, nlev, ntop; };
+#ifndef OB_COLD_ATTR
+#define OB_COLD_ATTR __noinline__
+#endif
+
+__device__ OB_COLD_ATTR void sweep_bias(const World *wd, const DevCtx &c, const int nt) {
+  const Sm s = wd->s;
+  const Gm g = wd->g;
+  const int nlev = wd->nlev, ntop = wd->ntop, tid = threadIdx.x;
+  const int l_first_down = tid < 32 ? 0 : ntop - 1, l_last_up = tid < 32 ? 0 : ntop;
+  // ---- A0: per link, flat ----
+#pragma unroll 1
+  for (int i = tid; i < wd->N; i += nt) link_prepare(i, s, g, c);
+  __syncthreads();
+  // ---- A1: displacement-form FK, top-down ----
+#pragma unroll 1
+  for (int l = l_first_down; l < nlev; l++) {
+    const int le = s.lev[l + 1];
+#pragma unroll 1
+    for (int i = s.lev[l] + tid; i < le; i += nt) link_fk(i, s);
+    OB_FENCE_DOWN(l)
+  }
+  // ---- A2 (+ B1 for leaves): velocities, bias accelerations, bias forces, top-down ----
+#pragma unroll 1
+  for (int l = l_first_down; l < nlev; l++) {
+    const int le = s.lev[l + 1];
+#pragma unroll 1
+    for (int i = s.lev[l] + tid; i < le; i += nt) link_bias(i, s, g, c);
+    OB_FENCE_DOWN(l)
+  }
+  // ---- B1: bias forces bottom-up over the inner links -> rhs b ----
+#pragma unroll 1
+  for (int l = nlev - 2; l >= l_last_up; l--) {
+    const int le = s.lev[l + 1];
+#pragma unroll 1
+    for (int i = s.lev[l] + tid; i < le; i += nt) {
+      const uint32_t tw = s.T[i];
+      if ((tw >> kNcShift) & kNcMask) link_bias_up(i, tw, s, g, c);
+    }
+    OB_FENCE_UP(l)
+  }
+  __syncthreads();
+}
+
+__device__ OB_COLD_ATTR void sweep_inertia(const World *wd, const DevCtx &c, const int nt, const int otid) {
+  const Sm s = wd->s;
+  const Gm g = wd->g;
+  const int nlev = wd->nlev, ntop = wd->ntop, N = wd->N, tid = threadIdx.x;
+  const int l_last_up = tid < 32 ? 0 : ntop;
+  // ---- B2: composite inertia bottom-up -> Jacobi factors, effective inertia (all leaves first) ----
+#pragma unroll 1
+  for (int i = otid; i < N; i += nt)                       // flat ownership: G[i] was just read by this thread
+    if (((s.T[i] >> kNcShift) & kNcMask) == 0u) up_inertia(i, s, g, c);
+  __syncthreads();
+#pragma unroll 1
+  for (int l = nlev - 2; l >= l_last_up; l--) {
+    const int le = s.lev[l + 1];
+#pragma unroll 1
+    for (int i = s.lev[l] + tid; i < le; i += nt)
+      if ((s.T[i] >> kNcShift) & kNcMask) up_inertia(i, s, g, c);
+    OB_FENCE_UP(l)
+  }
+  __syncthreads();
+}
 
 // ------------------------------------------------------------------------------------------------------
 // k_step<NT, LPT>
 // ------------------------------------------------------------------------------------------------------
 template <int NT, int LPT, int MINB>
 __global__ void __launch_bounds__(NT, MINB)
-k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *queue, int n_steps) {
+k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *queue, int n_steps,
+       int top_rot) {
   extern __shared__ __align__(128) unsigned char smem[];
   __shared__ __align__(8) uint64_t s_bar;
   __shared__ int s_next;
+  __shared__ World s_world;
   __shared__ __align__(16) float2 s_stage[64];
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, lane = tid & 31;
+  // the warp that sweeps the top levels of the PCG products: rotated over the CTAs that share an SM, so that these
+  // serial stretches do not all land on the same warp scheduler
+  const int topw = (int)((blockIdx.x / (unsigned)top_rot) % (NT / 32));
+  const bool top_warp = (tid >> 5) == topw;
+  // flat ownership: thread otid + k * NT <-> link; the top warp owns links 0..31, i.e. exactly its lanes' links
+  const int otid = (tid - 32 * topw + NT) % NT;
   const ob_params &P = c.P;
   uint32_t parity = 0;
   if (tid == 0) mbar_init(&s_bar, 1);
@@ -572,9 +666,6 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
     const Sm s = carve(smem, d);
     const int Np = d.Np, S = Np + 1, N = d.N;
     const int nlev = d.n_levels, ntop = d.n_top;
-    // warps other than warp 0 own no link of the n_top leading levels: they enter a top-down sweep at the level
-    // whose fence is the first block barrier and leave a bottom-up sweep after the last one
-    const int l_first_down = tid < 32 ? 0 : ntop - 1, l_last_up = tid < 32 ? 0 : ntop;
     float4 *const PL = s.P;
     Gm g;
     {
@@ -591,6 +682,7 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
       g.arm = c.arm ? c.arm + 2 * (size_t)d.link_base : nullptr;
       g.topo2 = c.topo2 + d.link_base;
     }
+    if (tid == 0) { s_world.s = s; s_world.g = g; s_world.N = N; s_world.nlev = nlev; s_world.ntop = ntop; }
 
     // ---- stage the world: the apple block by one TMA bulk copy; topology words, level offsets, wrench slots ----
     if (tid == 0 && d.Ap) {
@@ -617,13 +709,12 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
         s.T[i] = tw;
       }
     }
-    float2 x[LPT], r[LPT], idg[LPT];
+    float2 x[LPT], r[LPT];
 #pragma unroll
     for (int k = 0; k < LPT; k++) {
-      const int i = tid + k * NT;
+      const int i = otid + k * NT;
       x[k] = i < N ? g.x2[i] : make_float2(0.f, 0.f);
       r[k] = make_float2(0.f, 0.f);
-      idg[k] = make_float2(0.f, 0.f);
     }
     if (d.Ap) {
       mbar_wait(&s_bar, parity);
@@ -634,10 +725,10 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
     // stays inside the warp
     const int ntopN = s.lev[ntop];
     int top_lvl = -1, top_maxc = 0;
-    if (tid < ntopN) {
+    if (lane < ntopN) {
       for (int l = 0; l < ntop; l++)
-        if (tid >= s.lev[l]) top_lvl = l;
-      if (top_lvl < ntop - 1) top_maxc = (int)((s.T[tid] >> kNcShift) & kNcMask);
+        if (lane >= s.lev[l]) top_lvl = l;
+      if (top_lvl < ntop - 1) top_maxc = (int)((s.T[lane] >> kNcShift) & kNcMask);
     }
     top_maxc = __reduce_max_sync(0xffffffffu, top_maxc);
     // user forces on apples are constant over the launch
@@ -653,53 +744,21 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
     int step0 = info->step, steps_done = 0, last_iters = 0;
     unsigned long long iters_total = 0;
     for (int sidx = 0; sidx < n_steps; sidx++) {
-      // ---- A (+ B1 for leaves): top-down ----
-#pragma unroll 1
-      for (int l = l_first_down; l < nlev; l++) {
-        const int le = s.lev[l + 1];
-#pragma unroll 1
-        for (int i = s.lev[l] + tid; i < le; i += NT) down_bias(i, s, g, c);
-        OB_FENCE_DOWN(l)
-      }
-      // ---- B1: bias forces bottom-up over the inner links -> rhs b ----
-#pragma unroll 1
-      for (int l = nlev - 2; l >= l_last_up; l--) {
-        const int le = s.lev[l + 1];
-#pragma unroll 1
-        for (int i = s.lev[l] + tid; i < le; i += NT) {
-          const uint32_t tw = s.T[i];
-          if ((tw >> kNcShift) & kNcMask) up_bias(i, tw, s, g, c);
-        }
-        OB_FENCE_UP(l)
-      }
-      __syncthreads();
+      sweep_bias(&s_world, c, NT);                      // A, B1
 #pragma unroll
       for (int k = 0; k < LPT; k++) {
-        const int i = tid + k * NT;
+        const int i = otid + k * NT;
         if (i < N) r[k] = s.G[i];                       // b
       }
-      // ---- B2: composite inertia bottom-up -> Jacobi factors, effective inertia (all leaves first) ----
-#pragma unroll 1
-      for (int i = tid; i < N; i += NT)
-        if (((s.T[i] >> kNcShift) & kNcMask) == 0u) up_inertia(i, s, g, c);
-      __syncthreads();
-#pragma unroll 1
-      for (int l = nlev - 2; l >= l_last_up; l--) {
-        const int le = s.lev[l + 1];
-#pragma unroll 1
-        for (int i = s.lev[l] + tid; i < le; i += NT)
-          if ((s.T[i] >> kNcShift) & kNcMask) up_inertia(i, s, g, c);
-        OB_FENCE_UP(l)
-      }
-      __syncthreads();
+      sweep_inertia(&s_world, c, NT, otid);                   // B2: G[i] is first rewritten by the thread that just read it
       float bb_part = 0.f, bz_part = 0.f;
 #pragma unroll
       for (int k = 0; k < LPT; k++) {
-        const int i = tid + k * NT;
+        const int i = otid + k * NT;
         if (i < N) {
-          idg[k] = s.G[i];
+          const float2 idg = s.G[i];
           bb_part += r[k].x * r[k].x + r[k].y * r[k].y;
-          bz_part += r[k].x * r[k].x * idg[k].x + r[k].y * r[k].y * idg[k].y;
+          bz_part += r[k].x * r[k].x * idg.x + r[k].y * r[k].y * idg.y;
         }
       }
       const float2 bbz = red.sum(bb_part, bz_part);
@@ -715,7 +774,7 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
       } else {
 #pragma unroll
         for (int k = 0; k < LPT; k++) {                 // first product: A x, i.e. p = x
-          const int i = tid + k * NT;
+          const int i = otid + k * NT;
           if (i < N) *reinterpret_cast<float2 *>(PL + 7 * i + 2) = x[k];
         }
         bool first = true;
@@ -727,28 +786,29 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
           //      and children by shuffle, no barrier.  The other levels are swept by the whole CTA, one block
           //      barrier per level; the deepest level turns around at once ----
           float pAp_part = 0.f;
-          if (tid < 32) {
-            const int me = tid < ntopN ? tid : Np;               // idle lanes work on the zero record
+          if (top_warp) {
+            const int me = lane < ntopN ? lane : Np;             // idle lanes work on the zero record
             const uint32_t tw = s.T[me];
             float4 *rec = PL + 7 * me;
             const float4 pd = rec[2];
             const Jt j = load_jt(PL, me);
-            const int parl = (tw & kTrunk) ? tid : (int)(tw & kParMask);
+            const int parl = (tw & kTrunk) ? lane : (int)(tw & kParMask);   // the trunk's "parent" is all zero at level 0
+            const float3 sp = f3(j.c2 * pd.x, pd.y, j.s2 * pd.x);
             float3 al = f3(0, 0, 0), a = f3(0, 0, 0);
 #pragma unroll 1
-            for (int l = 0; l < ntop; l++) {
+            for (int l = 0; l < ntop; l++) {                      // branch-free: every lane computes, level l commits
               float3 alp, ap;
               alp.x = __shfl_sync(0xffffffffu, al.x, parl); alp.y = __shfl_sync(0xffffffffu, al.y, parl);
               alp.z = __shfl_sync(0xffffffffu, al.z, parl);
               ap.x = __shfl_sync(0xffffffffu, a.x, parl); ap.y = __shfl_sync(0xffffffffu, a.y, parl);
               ap.z = __shfl_sync(0xffffffffu, a.z, parl);
-              if (top_lvl == l) {
-                if (tw & kTrunk) { alp = f3(0, 0, 0); ap = f3(0, 0, 0); }
-                al = mul(j.E, alp) + f3(j.c2 * pd.x, pd.y, j.s2 * pd.x);
-                a = mul(j.E, f3(ap.x + alp.y * j.rz, ap.y - alp.x * j.rz, ap.z));
-              }
+              const float3 nal = mul(j.E, alp) + sp;
+              const float3 na = mul(j.E, f3(ap.x + alp.y * j.rz, ap.y - alp.x * j.rz, ap.z));
+              const bool mine = top_lvl == l;
+              al.x = mine ? nal.x : al.x; al.y = mine ? nal.y : al.y; al.z = mine ? nal.z : al.z;
+              a.x = mine ? na.x : a.x; a.y = mine ? na.y : a.y; a.z = mine ? na.z : a.z;
             }
-            if (tid < ntopN) {
+            if (lane < ntopN) {
               rec[0] = make_float4(al.x, al.y, al.z, a.x);
               *reinterpret_cast<float2 *>(rec + 1) = make_float2(a.y, a.z);
             }
@@ -767,7 +827,7 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
               float3 al, a;
               mv_down(j, PL, tw, pd, al, a);
               if (deepest) {
-                pAp_part += mv_up(j, PL, PL + 7 * Np, i, tw, pd, al, a, s, g, c);
+                pAp_part += mv_up<false>(j, PL, PL + 7 * Np, i, tw, pd, al, a, s, g, c);
               } else {
                 rec[0] = make_float4(al.x, al.y, al.z, a.x);
                 *reinterpret_cast<float2 *>(rec + 1) = make_float2(a.y, a.z);
@@ -785,12 +845,12 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
               const float4 pd = rec[2];
               const Jt j = load_jt(PL, i);
               const float4 u = rec[0], v = rec[1];
-              pAp_part += mv_up(j, PL, PL + 7 * Np, i, tw, pd, f3(u.x, u.y, u.z), f3(u.w, v.x, v.y), s, g, c);
+              pAp_part += mv_up<true>(j, PL, PL + 7 * Np, i, tw, pd, f3(u.x, u.y, u.z), f3(u.w, v.x, v.y), s, g, c);
             }
             __syncthreads();
           }
-          if (tid < 32) {
-            const int me = tid < ntopN ? tid : Np;
+          if (top_warp) {
+            const int me = lane < ntopN ? lane : Np;
             const uint32_t tw = s.T[me];
             float4 *rec = PL + 7 * me;
             const float4 pd = rec[2], I = rec[6];
@@ -798,47 +858,53 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
             const float4 u = rec[0], v = rec[1];
             const float3 al = f3(u.x, u.y, u.z), a = f3(u.w, v.x, v.y);
             const int fc = (int)((tw >> kChShift) & kParMask), nc = (int)((tw >> kNcShift) & kNcMask);
+            // own inertia force; the children of the last top level are in shared memory, all others are lanes
+            float3 n0 = f3(I.z * al.x - I.y * a.y, I.z * al.y + I.y * a.x, I.w * al.z);
+            float3 f0 = f3(I.x * a.x + I.y * al.y, I.x * a.y - I.y * al.x, I.x * a.z);
+            if (tw & kOffax) {
+              const Force6 t = offaxis_tethers(__ldg(g.topo2 + me), al, a, s.att, s.ao, s.ak, s.Ap, P.h * P.h);
+              n0 = n0 + t.n; f0 = f0 + t.f;
+            }
+            if (top_lvl == ntop - 1) gather_children(PL, PL + 7 * Np, fc, nc, n0, f0);
+            const int nct = (top_lvl >= 0 && top_lvl < ntop - 1) ? nc : 0;
             float3 un = f3(0, 0, 0), uf = f3(0, 0, 0);           // (n, f) of this link in its parent's frame
             float t1 = 0.f, t2 = 0.f;
 #pragma unroll 1
-            for (int l = ntop - 1; l >= 0; l--) {
-              const bool mine = top_lvl == l;
-              float3 n = f3(I.z * al.x - I.y * a.y, I.z * al.y + I.y * a.x, I.w * al.z);
-              float3 f = f3(I.x * a.x + I.y * al.y, I.x * a.y - I.y * al.x, I.x * a.z);
-              if (mine && (tw & kOffax)) {
-                const Force6 t = offaxis_tethers(__ldg(g.topo2 + me), al, a, s.att, s.ao, s.ak, s.Ap, P.h * P.h);
-                n = n + t.n; f = f + t.f;
+            for (int l = ntop - 1; l >= 0; l--) {                // branch-free: every lane computes, level l commits
+              float3 n = n0, f = f0;
+#pragma unroll
+              for (int k = 0; k < 4; k++) {
+                const int src = min(fc + k, 31);
+                const float c0 = __shfl_sync(0xffffffffu, un.x, src), c1 = __shfl_sync(0xffffffffu, un.y, src),
+                            c2 = __shfl_sync(0xffffffffu, un.z, src), c3 = __shfl_sync(0xffffffffu, uf.x, src),
+                            c4 = __shfl_sync(0xffffffffu, uf.y, src), c5 = __shfl_sync(0xffffffffu, uf.z, src);
+                const bool on = k < nct;
+                n.x += on ? c0 : 0.f; n.y += on ? c1 : 0.f; n.z += on ? c2 : 0.f;
+                f.x += on ? c3 : 0.f; f.y += on ? c4 : 0.f; f.z += on ? c5 : 0.f;
               }
-              if (l == ntop - 1) {                               // children (if any) are in shared memory
-                if (mine) {
+              if (top_maxc > 4) {                                // uniform over the warp; wide fans are rare
 #pragma unroll 1
-                  for (int k = 0; k < nc; k++) {
-                    const float4 cu = PL[7 * (fc + k)], cv = PL[7 * (fc + k) + 1];
-                    n = n + f3(cu.x, cu.y, cu.z);
-                    f = f + f3(cu.w, cv.x, cv.y);
-                  }
-                }
-              } else {                                           // children are lanes fc .. fc + nc - 1
-#pragma unroll 1
-                for (int k = 0; k < top_maxc; k++) {
+                for (int k = 4; k < top_maxc; k++) {
                   const int src = min(fc + k, 31);
-                  float3 cn, cf;
-                  cn.x = __shfl_sync(0xffffffffu, un.x, src); cn.y = __shfl_sync(0xffffffffu, un.y, src);
-                  cn.z = __shfl_sync(0xffffffffu, un.z, src);
-                  cf.x = __shfl_sync(0xffffffffu, uf.x, src); cf.y = __shfl_sync(0xffffffffu, uf.y, src);
-                  cf.z = __shfl_sync(0xffffffffu, uf.z, src);
-                  if (k < nc) { n = n + cn; f = f + cf; }
+                  const float c0 = __shfl_sync(0xffffffffu, un.x, src), c1 = __shfl_sync(0xffffffffu, un.y, src),
+                              c2 = __shfl_sync(0xffffffffu, un.z, src), c3 = __shfl_sync(0xffffffffu, uf.x, src),
+                              c4 = __shfl_sync(0xffffffffu, uf.y, src), c5 = __shfl_sync(0xffffffffu, uf.z, src);
+                  const bool on = k < nct;
+                  n.x += on ? c0 : 0.f; n.y += on ? c1 : 0.f; n.z += on ? c2 : 0.f;
+                  f.x += on ? c3 : 0.f; f.y += on ? c4 : 0.f; f.z += on ? c5 : 0.f;
                 }
               }
-              if (mine) {
-                t1 = j.c2 * n.x + j.s2 * n.z + pd.z * pd.x;
-                t2 = n.y + pd.w * pd.y;
-                uf = mulT(j.E, f);
-                un = mulT(j.E, n);
-                un.x -= j.rz * uf.y; un.y += j.rz * uf.x;
-              }
+              const float nt1 = j.c2 * n.x + j.s2 * n.z + pd.z * pd.x;
+              const float nt2 = n.y + pd.w * pd.y;
+              const float3 nuf = mulT(j.E, f);
+              float3 nun = mulT(j.E, n);
+              nun.x -= j.rz * nuf.y; nun.y += j.rz * nuf.x;
+              const bool mine = top_lvl == l;
+              t1 = mine ? nt1 : t1; t2 = mine ? nt2 : t2;
+              un.x = mine ? nun.x : un.x; un.y = mine ? nun.y : un.y; un.z = mine ? nun.z : un.z;
+              uf.x = mine ? nuf.x : uf.x; uf.y = mine ? nuf.y : uf.y; uf.z = mine ? nuf.z : uf.z;
             }
-            if (tid < ntopN) {
+            if (lane < ntopN) {
               reinterpret_cast<float2 *>(rec + 1)[1] = make_float2(t1, t2);
               pAp_part += pd.x * t1 + pd.y * t2;
             }
@@ -849,11 +915,12 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
             __syncthreads();
 #pragma unroll
             for (int k = 0; k < LPT; k++) {
-              const int i = tid + k * NT;
+              const int i = otid + k * NT;
               if (i < N) {
                 const float2 ap = reinterpret_cast<const float2 *>(PL + 7 * i + 1)[1];
+                const float2 idg = s.G[i];
                 r[k].x -= ap.x; r[k].y -= ap.y;
-                const float za = r[k].x * idg[k].x, zb = r[k].y * idg[k].y;
+                const float za = r[k].x * idg.x, zb = r[k].y * idg.y;
                 *reinterpret_cast<float2 *>(PL + 7 * i + 2) = make_float2(za, zb);
                 rz_p += r[k].x * za + r[k].y * zb; rr_p += r[k].x * r[k].x + r[k].y * r[k].y;
               }
@@ -866,14 +933,15 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
             float2 z[LPT], pk[LPT];
 #pragma unroll
             for (int k = 0; k < LPT; k++) {
-              const int i = tid + k * NT;
+              const int i = otid + k * NT;
               z[k] = make_float2(0.f, 0.f); pk[k] = make_float2(0.f, 0.f);
               if (i < N) {
                 const float2 ap = reinterpret_cast<const float2 *>(PL + 7 * i + 1)[1];
+                const float2 idg = s.G[i];
                 pk[k] = *reinterpret_cast<const float2 *>(PL + 7 * i + 2);
                 x[k].x += alpha * pk[k].x; x[k].y += alpha * pk[k].y;
                 r[k].x -= alpha * ap.x; r[k].y -= alpha * ap.y;
-                z[k] = make_float2(r[k].x * idg[k].x, r[k].y * idg[k].y);
+                z[k] = make_float2(r[k].x * idg.x, r[k].y * idg.y);
                 rz_p += r[k].x * z[k].x + r[k].y * z[k].y; rr_p += r[k].x * r[k].x + r[k].y * r[k].y;
               }
             }
@@ -882,7 +950,7 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
             rz = t.x; rr = P.cg_norm ? t.x : t.y;
 #pragma unroll
             for (int k = 0; k < LPT; k++) {
-              const int i = tid + k * NT;
+              const int i = otid + k * NT;
               if (i < N)
                 *reinterpret_cast<float2 *>(PL + 7 * i + 2) = make_float2(z[k].x + beta * pk[k].x, z[k].y + beta * pk[k].y);
             }
@@ -905,7 +973,7 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
       const int step_now = step0 + sidx;
 #pragma unroll
       for (int k = 0; k < LPT; k++) {
-        const int i = tid + k * NT;
+        const int i = otid + k * NT;
         if (i >= N) continue;
         const float2 w0 = g.w2[i], q0 = g.q2[i];
         float wa = w0.x + x[k].x, wb = w0.y + x[k].y;
@@ -968,7 +1036,7 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
     // ---- write the state back: x from the registers, the apple state by one TMA bulk store ----
 #pragma unroll
     for (int k = 0; k < LPT; k++) {
-      const int i = tid + k * NT;
+      const int i = otid + k * NT;
       if (i < N) g.x2[i] = (status & OB_STATUS_NONFINITE) ? make_float2(0.f, 0.f) : x[k];
     }
     fence_proxy_async();
@@ -994,7 +1062,7 @@ k_step(DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *que
 #define OB_FOR_CLASS(cls, CALL)                         \
   switch (cls) {                                        \
     case 0: { CALL(128, 2, 6); break; }                 \
-    case 1: { CALL(256, 2, 3); break; }                 \
+    case 1: { CALL(192, 3, 3); break; }                 \
     case 2: { CALL(512, 2, 1); break; }                 \
     case 3: { CALL(512, 3, 1); break; }                 \
     default: return cudaErrorInvalidValue;              \
@@ -1012,8 +1080,9 @@ cudaError_t step_kernel_setup(int cls, int smem_bytes, int *max_blocks_per_sm) {
 }
 
 cudaError_t launch_step(const DevCtx &c, int cls, const int32_t *order, int n_in_class, int32_t *queue, int n_steps,
-                        int grid, int smem, cudaStream_t s) {
-#define OB_LAUNCH(NT, LPT, MINB) k_step<NT, LPT, MINB><<<grid, NT, smem, s>>>(c, order, n_in_class, queue, n_steps);
+                        int grid, int smem, int n_sm, cudaStream_t s) {
+#define OB_LAUNCH(NT, LPT, MINB) \
+  k_step<NT, LPT, MINB><<<grid, NT, smem, s>>>(c, order, n_in_class, queue, n_steps, n_sm > 0 ? n_sm : 1);
   OB_FOR_CLASS(cls, OB_LAUNCH)
 #undef OB_LAUNCH
   return cudaGetLastError();
