@@ -107,7 +107,11 @@ struct DevCtx {
 //      runs over any number of links.
 struct StepClass { int nt, lpt, min_ctas; };
 constexpr int kNumClasses = 4;
-constexpr StepClass kStepClasses[kNumClasses] = {{128, 2, 6}, {192, 3, 3}, {512, 2, 1}, {512, 3, 1}};
+#ifndef OB_CLS1_NT
+#define OB_CLS1_NT 192
+#define OB_CLS1_LPT 3
+#endif
+constexpr StepClass kStepClasses[kNumClasses] = {{128, 2, 6}, {OB_CLS1_NT, OB_CLS1_LPT, 3}, {512, 2, 1}, {512, 3, 1}};
 constexpr int kMaxLinksOnChip = 512 * 3;
 constexpr int kMaxChildren = 15;     // children per link (4 bits of the packed topology word)
 inline int step_class_of(int Np) {   // host only
@@ -124,12 +128,14 @@ inline int step_class_of(int Np) {   // host only
 //   apple block (TMA) | f_tether, f_user [3][Ap], |f_s|, |f_user| [Ap] | wrench slots
 __host__ __device__ inline int r16(int b) { return (b + 15) / 16 * 16; }
 __host__ __device__ inline int step_planes_bytes(int Np) { return 7 * 16 * (Np + 1); }
+// phase-A overflow (three float4 per inner link) and the PCG's (x, r) (one float4 per link) share one region
+__host__ __device__ inline int step_ovf_bytes(int Np, int NIp) { return 48 * NIp > 16 * Np ? 48 * NIp : 16 * Np; }
 __host__ __device__ inline int step_smem_bytes(int Np, int Ap, int NIp, int nlev) {
   int b = 0;
   b += step_planes_bytes(Np);
   b += r16(8 * (Np + 1));
   b += r16(4 * (Np + 1));
-  b += 48 * NIp;
+  b += step_ovf_bytes(Np, NIp);
   b += r16(4 * (nlev + 1));
   b += r16(apple_block_bytes(Ap));
   b += (3 + 3 + 2) * 4 * Ap;

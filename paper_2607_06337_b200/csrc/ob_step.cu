@@ -54,6 +54,7 @@ struct Sm {
   float2 *G;
   uint32_t *T;
   float4 *ovf;                        // ovf[j * NIp + inner slot], j = 0..2
+  float4 *XR;                         // [Np] (x, r) of the PCG; same memory as ovf (phase A2 / B1 only)
   int *lev;                           // level offsets [n_levels + 1]
   // apple block (TMA)
   float *u, *v;                       // [3][Ap]
@@ -71,7 +72,7 @@ __device__ __forceinline__ Sm carve(unsigned char *base, const WorldDesc &d) {
   s.P = reinterpret_cast<float4 *>(p); p += step_planes_bytes(Np);
   s.G = reinterpret_cast<float2 *>(p); p += r16(8 * (Np + 1));
   s.T = reinterpret_cast<uint32_t *>(p); p += r16(4 * (Np + 1));
-  s.ovf = reinterpret_cast<float4 *>(p); p += 48 * d.NIp;
+  s.ovf = reinterpret_cast<float4 *>(p); s.XR = s.ovf; p += step_ovf_bytes(Np, d.NIp);
   s.lev = reinterpret_cast<int *>(p); p += r16(4 * (d.n_levels + 1));
   float *f = reinterpret_cast<float *>(p);
   s.u = f; s.v = f + 3 * Ap;
@@ -709,13 +710,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         s.T[i] = tw;
       }
     }
-    float2 x[LPT], r[LPT];
-#pragma unroll
-    for (int k = 0; k < LPT; k++) {
-      const int i = otid + k * NT;
-      x[k] = i < N ? g.x2[i] : make_float2(0.f, 0.f);
-      r[k] = make_float2(0.f, 0.f);
-    }
+    float4 *const XR = s.XR;                           // (x, r) of the PCG per link; aliases the phase-A overflow
     if (d.Ap) {
       mbar_wait(&s_bar, parity);
       parity ^= 1;
@@ -748,7 +743,10 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
 #pragma unroll
       for (int k = 0; k < LPT; k++) {
         const int i = otid + k * NT;
-        if (i < N) r[k] = s.G[i];                       // b
+        if (i < N) {                                    // r = b; x = previous dqd (warm start), kept in global memory
+          const float2 b = s.G[i], x0 = g.x2[i];
+          XR[i] = make_float4(x0.x, x0.y, b.x, b.y);
+        }
       }
       sweep_inertia(&s_world, c, NT, otid);                   // B2: G[i] is first rewritten by the thread that just read it
       float bb_part = 0.f, bz_part = 0.f;
@@ -757,8 +755,9 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         const int i = otid + k * NT;
         if (i < N) {
           const float2 idg = s.G[i];
-          bb_part += r[k].x * r[k].x + r[k].y * r[k].y;
-          bz_part += r[k].x * r[k].x * idg.x + r[k].y * r[k].y * idg.y;
+          const float4 xr = XR[i];
+          bb_part += xr.z * xr.z + xr.w * xr.w;
+          bz_part += xr.z * xr.z * idg.x + xr.w * xr.w * idg.y;
         }
       }
       const float2 bbz = red.sum(bb_part, bz_part);
@@ -768,14 +767,17 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       bool bad = false;
       if (bb == 0.f) {
 #pragma unroll
-        for (int k = 0; k < LPT; k++) x[k] = make_float2(0.f, 0.f);
+        for (int k = 0; k < LPT; k++) {
+          const int i = otid + k * NT;
+          if (i < N) XR[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
       } else if (!(bb < INFINITY)) {
         bad = true;
       } else {
 #pragma unroll
         for (int k = 0; k < LPT; k++) {                 // first product: A x, i.e. p = x
           const int i = otid + k * NT;
-          if (i < N) *reinterpret_cast<float2 *>(PL + 7 * i + 2) = x[k];
+          if (i < N) *reinterpret_cast<float2 *>(PL + 7 * i + 2) = *reinterpret_cast<const float2 *>(XR + i);
         }
         bool first = true;
         float rz = 0.f, rr = 0.f;
@@ -919,10 +921,12 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
               if (i < N) {
                 const float2 ap = reinterpret_cast<const float2 *>(PL + 7 * i + 1)[1];
                 const float2 idg = s.G[i];
-                r[k].x -= ap.x; r[k].y -= ap.y;
-                const float za = r[k].x * idg.x, zb = r[k].y * idg.y;
+                float2 r = reinterpret_cast<const float2 *>(XR + i)[1];
+                r.x -= ap.x; r.y -= ap.y;
+                reinterpret_cast<float2 *>(XR + i)[1] = r;
+                const float za = r.x * idg.x, zb = r.y * idg.y;
                 *reinterpret_cast<float2 *>(PL + 7 * i + 2) = make_float2(za, zb);
-                rz_p += r[k].x * za + r[k].y * zb; rr_p += r[k].x * r[k].x + r[k].y * r[k].y;
+                rz_p += r.x * za + r.y * zb; rr_p += r.x * r.x + r.y * r.y;
               }
             }
             const float2 t = red.sum(rz_p, rr_p);
@@ -939,10 +943,12 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
                 const float2 ap = reinterpret_cast<const float2 *>(PL + 7 * i + 1)[1];
                 const float2 idg = s.G[i];
                 pk[k] = *reinterpret_cast<const float2 *>(PL + 7 * i + 2);
-                x[k].x += alpha * pk[k].x; x[k].y += alpha * pk[k].y;
-                r[k].x -= alpha * ap.x; r[k].y -= alpha * ap.y;
-                z[k] = make_float2(r[k].x * idg.x, r[k].y * idg.y);
-                rz_p += r[k].x * z[k].x + r[k].y * z[k].y; rr_p += r[k].x * r[k].x + r[k].y * r[k].y;
+                float4 xr = XR[i];
+                xr.x += alpha * pk[k].x; xr.y += alpha * pk[k].y;
+                xr.z -= alpha * ap.x; xr.w -= alpha * ap.y;
+                XR[i] = xr;
+                z[k] = make_float2(xr.z * idg.x, xr.w * idg.y);
+                rz_p += xr.z * z[k].x + xr.w * z[k].y; rr_p += xr.z * xr.z + xr.w * xr.w;
               }
             }
             const float2 t = red.sum(rz_p, rr_p);
@@ -966,7 +972,13 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       // a non-finite solve freezes the world at its last finite state
       int nf = 0;
 #pragma unroll
-      for (int k = 0; k < LPT; k++) nf |= !(fabsf(x[k].x) < INFINITY) || !(fabsf(x[k].y) < INFINITY);
+      for (int k = 0; k < LPT; k++) {
+        const int i = otid + k * NT;
+        if (i < N) {
+          const float2 x = *reinterpret_cast<const float2 *>(XR + i);
+          nf |= !(fabsf(x.x) < INFINITY) || !(fabsf(x.y) < INFINITY);
+        }
+      }
       if (__syncthreads_or(nf || bad)) { status |= OB_STATUS_NONFINITE; break; }
 
       // ---- D: integrate, predicates ----
@@ -976,7 +988,9 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         const int i = otid + k * NT;
         if (i >= N) continue;
         const float2 w0 = g.w2[i], q0 = g.q2[i];
-        float wa = w0.x + x[k].x, wb = w0.y + x[k].y;
+        const float2 x = *reinterpret_cast<const float2 *>(XR + i);
+        g.x2[i] = x;
+        float wa = w0.x + x.x, wb = w0.y + x.y;
         if (P.qd_max > 0.f) {
           wa = fminf(fmaxf(wa, -P.qd_max), P.qd_max);
           wb = fminf(fmaxf(wb, -P.qd_max), P.qd_max);
@@ -1033,11 +1047,13 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       __syncthreads();
     }
 
-    // ---- write the state back: x from the registers, the apple state by one TMA bulk store ----
+    // ---- write the state back: the apple state by one TMA bulk store; a frozen world restarts from x = 0 ----
+    if (status & OB_STATUS_NONFINITE) {
 #pragma unroll
-    for (int k = 0; k < LPT; k++) {
-      const int i = otid + k * NT;
-      if (i < N) g.x2[i] = (status & OB_STATUS_NONFINITE) ? make_float2(0.f, 0.f) : x[k];
+      for (int k = 0; k < LPT; k++) {
+        const int i = otid + k * NT;
+        if (i < N) g.x2[i] = make_float2(0.f, 0.f);
+      }
     }
     fence_proxy_async();
     __syncthreads();
@@ -1062,7 +1078,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
 #define OB_FOR_CLASS(cls, CALL)                         \
   switch (cls) {                                        \
     case 0: { CALL(128, 2, 6); break; }                 \
-    case 1: { CALL(192, 3, 3); break; }                 \
+    case 1: { CALL(OB_CLS1_NT, OB_CLS1_LPT, 3); break; }                 \
     case 2: { CALL(512, 2, 1); break; }                 \
     case 3: { CALL(512, 3, 1); break; }                 \
     default: return cudaErrorInvalidValue;              \
