@@ -51,6 +51,22 @@ def _peaks():
     return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
 
 
+def reduce_over_ranks(x: float, op: str, world_size: int, device: str = "cuda") -> float:
+    """max / sum of one number over the ranks of the job (replicas only: the only cross-rank traffic of the bench)."""
+    if world_size == 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX if op == "max" else dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def replica_seed(config: int, rank: int) -> int:
+    """Each rank steps an independent replica of the batch: same geometry, its own material draws."""
+    return 260706337 + 1000 * config + rank
+
+
 class ClockSampler(threading.Thread):
     """SM clock and throttle reasons during the timed region (NVML; the recipe's nvidia-smi clocks line)."""
 
@@ -136,7 +152,7 @@ def run_cuda(args, rank: int, world_size: int):
     W, S = len(specs), args.substeps
     n_links = sum(s.n_links for s in specs)
     n_apples = sum(s.n_apples for s in specs)
-    seed = 260706337 + 1000 * args.config + rank       # each rank is an independent replica of the batch
+    seed = replica_seed(args.config, rank)
     n_epochs = args.warmup + args.steps
     epochs = [_loads_arrays(specs, e, f_lo, f_hi) for e in range(n_epochs)]
 
@@ -198,18 +214,10 @@ def run_cuda(args, rank: int, world_size: int):
     e2e = run(e2e=True)
 
     def max_over_ranks(x: float) -> float:
-        if world_size == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return reduce_over_ranks(x, "max", world_size)
 
     def sum_over_ranks(x: float) -> float:
-        if world_size == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        return float(t.item())
+        return reduce_over_ranks(x, "sum", world_size)
 
     kern_total_ms = max_over_ranks(sum(dev["kern_ms"]))
     region_ms = max_over_ranks(dev["region_ms"])

@@ -92,6 +92,29 @@ def test_workspace_bytes_validates_on_the_host():
     assert L.ob_workspace_bytes(None, 0, C.byref(ob.params_struct(P)), C.byref(n)) == ob.OB_E_ARG
 
 
+def test_capacity_limits_are_reported_not_crashed():
+    """A link with more children than the packed topology word holds (15), or a world too large for one CTA's
+    shared memory, is refused with OB_E_CAPACITY by the host-side planner."""
+    P = config_params(1)
+    n = 18
+    star = ob_star_spec(n)
+    rc, _, msg = _ws_bytes([star], P)
+    assert rc == ob.OB_E_CAPACITY and "children" in msg
+    rc, _, _ = _ws_bytes([ob_star_spec(16)], P)          # 15 children: fine
+    assert rc == ob.OB_OK
+
+
+def ob_star_spec(n_links):
+    from workloads import WorldSpec
+    q = np.zeros((n_links, 4), np.float32)
+    q[:, 0] = 1.0
+    return WorldSpec(parent=np.array([-1] + [0] * (n_links - 1), np.int32), length=np.full(n_links, 0.3, np.float32),
+                     diameter=np.full(n_links, 0.02, np.float32), rest_quat=q, density=800.0, E=8e9, MOR=6e7,
+                     apple_link=np.zeros(0, np.int32), apple_offset=np.zeros((0, 3), np.float32),
+                     apple_mass=np.zeros(0, np.float32), apple_radius=np.zeros(0, np.float32),
+                     apple_k=np.zeros(0, np.float32), apple_c=None, apple_detach=np.zeros(0, np.float32))
+
+
 def test_null_context_calls_return_arg_errors():
     L = ob.load_library()
     assert L.ob_step(None, 1) == ob.OB_E_ARG
