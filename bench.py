@@ -120,6 +120,19 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.samples)}
 
 
+def _profiled_traffic(n_worlds: int, substeps: int):
+    """DRAM bytes of one k_step launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed ncu --set full
+    capture, profiles/r1_k_step_dram.txt; null unless that capture was of a launch of this size."""
+    tp = os.path.join(ROOT, "profiles", "r1_k_step_dram.txt")
+    try:
+        kv = dict(l.split("=", 1) for l in open(tp).read().split() if "=" in l)
+        if int(kv["worlds"]) == n_worlds and int(kv["substeps"]) == substeps:
+            return float(kv["dram_bytes_per_launch"])
+    except Exception:
+        pass
+    return None
+
+
 def _workload(config: int, n_worlds: int):
     from workloads import config_params, make_config
     base = make_config(config, min(n_worlds, 4096))
@@ -243,13 +256,7 @@ def run_cuda(args, rank: int, world_size: int):
         bytes_ws = links_per_world * BYTES_LINK_STEP + apples_per_world * BYTES_APPLE_STEP + BYTES_WRENCH
         hbm_stream = bytes_ws * ws_per_launch / (k_ms * 1e-3) / 1e9   # as if the state were streamed every step
         hbm_fused = hbm_stream / S                                    # what one launch really has to move
-        traffic = None
-        tp = os.path.join(ROOT, "profiles", "k_step_traffic.json")
-        if os.path.exists(tp):
-            try:
-                traffic = json.load(open(tp)).get("dram_bytes_per_launch")
-            except Exception:
-                traffic = None
+        traffic = _profiled_traffic(W, S)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world_size, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": region_ms / args.steps, "higher_is_better": True,
