@@ -626,6 +626,247 @@ __device__ OB_COLD_ATTR void sweep_inertia(const World *wd, const DevCtx &c, con
 }
 
 // ------------------------------------------------------------------------------------------------------
+// phase C as a function of its own (not inlined): its registers are allocated for the PCG loop alone, and what
+// it needs of the world comes out of shared memory (World).  Returns the number of iterations; *flags gets
+// OB_STATUS_CG_MAXITER, bit 30 = non-finite.
+// ------------------------------------------------------------------------------------------------------
+constexpr int kPcgBad = 1 << 30;
+
+template <int NT, int LPT>
+__device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *stage, int *flipp, const int otid,
+                                      const bool top_warp, const float bb, const float bz, int *flags) {
+  const Sm s = wd->s;
+  const Gm g = wd->g;
+  const ob_params &P = c.P;
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int Np = s.Np, N = wd->N, nlev = wd->nlev, ntop = wd->ntop;
+  float4 *const PL = s.P;
+  float4 *const XR = s.XR;
+  Reducer<NT> red;
+  red.stage = stage; red.flip = *flipp; red.tid = tid;
+  int status = 0;
+  // lanes of the top warp <-> links of the n_top leading levels: level of the lane's link, widest child list
+  // that stays inside the warp
+  const int ntopN = s.lev[ntop];
+  int top_lvl = -1, top_maxc = 0;
+  if (lane < ntopN) {
+    for (int l = 0; l < ntop; l++)
+      if (lane >= s.lev[l]) top_lvl = l;
+    if (top_lvl < ntop - 1) top_maxc = (int)((s.T[lane] >> kNcShift) & kNcMask);
+  }
+  top_maxc = __reduce_max_sync(0xffffffffu, top_maxc);
+  int it = 0;
+  bool bad = false;
+  if (bb == 0.f) {
+#pragma unroll
+    for (int k = 0; k < LPT; k++) {
+      const int i = otid + k * NT;
+      if (i < N) XR[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+  } else if (!(bb < INFINITY)) {
+    bad = true;
+  } else {
+#pragma unroll
+    for (int k = 0; k < LPT; k++) {                 // first product: A x, i.e. p = x
+      const int i = otid + k * NT;
+      if (i < N) *reinterpret_cast<float2 *>(PL + 7 * i + 2) = *reinterpret_cast<const float2 *>(XR + i);
+    }
+    bool first = true;
+    float rz = 0.f, rr = 0.f;
+    // stopping rule: |r| <= tol |b| in the 2-norm (cg_norm 0) or in the preconditioned norm (cg_norm 1)
+    const float tol2 = P.cg_tol * P.cg_tol * (P.cg_norm ? bz : bb);
+    for (;;) {
+      // ---- A p.  The n_top leading levels live in warp 0, lane = link: own record in registers, parents
+      //      and children by shuffle, no barrier.  The other levels are swept by the whole CTA, one block
+      //      barrier per level; the deepest level turns around at once ----
+      float pAp_part = 0.f;
+      if (top_warp) {
+        const int me = lane < ntopN ? lane : Np;             // idle lanes work on the zero record
+        const uint32_t tw = s.T[me];
+        float4 *rec = PL + 7 * me;
+        const float4 pd = rec[2];
+        const Jt j = load_jt(PL, me);
+        const int parl = (tw & kTrunk) ? lane : (int)(tw & kParMask);   // the trunk's "parent" is all zero at level 0
+        const float3 sp = f3(j.c2 * pd.x, pd.y, j.s2 * pd.x);
+        float3 al = f3(0, 0, 0), a = f3(0, 0, 0);
+#pragma unroll 1
+        for (int l = 0; l < ntop; l++) {                      // branch-free: every lane computes, level l commits
+          float3 alp, ap;
+          alp.x = __shfl_sync(0xffffffffu, al.x, parl); alp.y = __shfl_sync(0xffffffffu, al.y, parl);
+          alp.z = __shfl_sync(0xffffffffu, al.z, parl);
+          ap.x = __shfl_sync(0xffffffffu, a.x, parl); ap.y = __shfl_sync(0xffffffffu, a.y, parl);
+          ap.z = __shfl_sync(0xffffffffu, a.z, parl);
+          const float3 nal = mul(j.E, alp) + sp;
+          const float3 na = mul(j.E, f3(ap.x + alp.y * j.rz, ap.y - alp.x * j.rz, ap.z));
+          const bool mine = top_lvl == l;
+          al.x = mine ? nal.x : al.x; al.y = mine ? nal.y : al.y; al.z = mine ? nal.z : al.z;
+          a.x = mine ? na.x : a.x; a.y = mine ? na.y : a.y; a.z = mine ? na.z : a.z;
+        }
+        if (lane < ntopN) {
+          rec[0] = make_float4(al.x, al.y, al.z, a.x);
+          *reinterpret_cast<float2 *>(rec + 1) = make_float2(a.y, a.z);
+        }
+      }
+      __syncthreads();
+#pragma unroll 1
+      for (int l = ntop; l < nlev; l++) {
+        const int le = s.lev[l + 1];
+        const bool deepest = l == nlev - 1;
+#pragma unroll 1
+        for (int i = s.lev[l] + tid; i < le; i += NT) {
+          const uint32_t tw = s.T[i];
+          float4 *rec = PL + 7 * i;
+          const float4 pd = rec[2];
+          const Jt j = load_jt(PL, i);
+          float3 al, a;
+          mv_down(j, PL, tw, pd, al, a);
+          if (deepest) {
+            pAp_part += mv_up<false>(j, PL, PL + 7 * Np, i, tw, pd, al, a, s, g, c);
+          } else {
+            rec[0] = make_float4(al.x, al.y, al.z, a.x);
+            *reinterpret_cast<float2 *>(rec + 1) = make_float2(a.y, a.z);
+          }
+        }
+        __syncthreads();
+      }
+#pragma unroll 1
+      for (int l = nlev - 2; l >= ntop; l--) {
+        const int le = s.lev[l + 1];
+#pragma unroll 1
+        for (int i = s.lev[l] + tid; i < le; i += NT) {
+          const uint32_t tw = s.T[i];
+          const float4 *rec = PL + 7 * i;
+          const float4 pd = rec[2];
+          const Jt j = load_jt(PL, i);
+          const float4 u = rec[0], v = rec[1];
+          pAp_part += mv_up<true>(j, PL, PL + 7 * Np, i, tw, pd, f3(u.x, u.y, u.z), f3(u.w, v.x, v.y), s, g, c);
+        }
+        __syncthreads();
+      }
+      if (top_warp) {
+        const int me = lane < ntopN ? lane : Np;
+        const uint32_t tw = s.T[me];
+        float4 *rec = PL + 7 * me;
+        const float4 pd = rec[2], I = rec[6];
+        const Jt j = load_jt(PL, me);
+        const float4 u = rec[0], v = rec[1];
+        const float3 al = f3(u.x, u.y, u.z), a = f3(u.w, v.x, v.y);
+        const int fc = (int)((tw >> kChShift) & kParMask), nc = (int)((tw >> kNcShift) & kNcMask);
+        // own inertia force; the children of the last top level are in shared memory, all others are lanes
+        float3 n0 = f3(I.z * al.x - I.y * a.y, I.z * al.y + I.y * a.x, I.w * al.z);
+        float3 f0 = f3(I.x * a.x + I.y * al.y, I.x * a.y - I.y * al.x, I.x * a.z);
+        if (tw & kOffax) {
+          const Force6 t = offaxis_tethers(__ldg(g.topo2 + me), al, a, s.att, s.ao, s.ak, s.Ap, P.h * P.h);
+          n0 = n0 + t.n; f0 = f0 + t.f;
+        }
+        if (top_lvl == ntop - 1) gather_children(PL, PL + 7 * Np, fc, nc, n0, f0);
+        const int nct = (top_lvl >= 0 && top_lvl < ntop - 1) ? nc : 0;
+        float3 un = f3(0, 0, 0), uf = f3(0, 0, 0);           // (n, f) of this link in its parent's frame
+        float t1 = 0.f, t2 = 0.f;
+#pragma unroll 1
+        for (int l = ntop - 1; l >= 0; l--) {                // branch-free: every lane computes, level l commits
+          float3 n = n0, f = f0;
+#pragma unroll
+          for (int k = 0; k < 4; k++) {
+            const int src = min(fc + k, 31);
+            const float c0 = __shfl_sync(0xffffffffu, un.x, src), c1 = __shfl_sync(0xffffffffu, un.y, src),
+                        c2 = __shfl_sync(0xffffffffu, un.z, src), c3 = __shfl_sync(0xffffffffu, uf.x, src),
+                        c4 = __shfl_sync(0xffffffffu, uf.y, src), c5 = __shfl_sync(0xffffffffu, uf.z, src);
+            const bool on = k < nct;
+            n.x += on ? c0 : 0.f; n.y += on ? c1 : 0.f; n.z += on ? c2 : 0.f;
+            f.x += on ? c3 : 0.f; f.y += on ? c4 : 0.f; f.z += on ? c5 : 0.f;
+          }
+          if (top_maxc > 4) {                                // uniform over the warp; wide fans are rare
+#pragma unroll 1
+            for (int k = 4; k < top_maxc; k++) {
+              const int src = min(fc + k, 31);
+              const float c0 = __shfl_sync(0xffffffffu, un.x, src), c1 = __shfl_sync(0xffffffffu, un.y, src),
+                          c2 = __shfl_sync(0xffffffffu, un.z, src), c3 = __shfl_sync(0xffffffffu, uf.x, src),
+                          c4 = __shfl_sync(0xffffffffu, uf.y, src), c5 = __shfl_sync(0xffffffffu, uf.z, src);
+              const bool on = k < nct;
+              n.x += on ? c0 : 0.f; n.y += on ? c1 : 0.f; n.z += on ? c2 : 0.f;
+              f.x += on ? c3 : 0.f; f.y += on ? c4 : 0.f; f.z += on ? c5 : 0.f;
+            }
+          }
+          const float nt1 = j.c2 * n.x + j.s2 * n.z + pd.z * pd.x;
+          const float nt2 = n.y + pd.w * pd.y;
+          const float3 nuf = mulT(j.E, f);
+          float3 nun = mulT(j.E, n);
+          nun.x -= j.rz * nuf.y; nun.y += j.rz * nuf.x;
+          const bool mine = top_lvl == l;
+          t1 = mine ? nt1 : t1; t2 = mine ? nt2 : t2;
+          un.x = mine ? nun.x : un.x; un.y = mine ? nun.y : un.y; un.z = mine ? nun.z : un.z;
+          uf.x = mine ? nuf.x : uf.x; uf.y = mine ? nuf.y : uf.y; uf.z = mine ? nuf.z : uf.z;
+        }
+        if (lane < ntopN) {
+          reinterpret_cast<float2 *>(rec + 1)[1] = make_float2(t1, t2);
+          pAp_part += pd.x * t1 + pd.y * t2;
+        }
+      }
+      float rz_p = 0.f, rr_p = 0.f;
+      if (first) {                                 // r = b - A x, z = P^-1 r, p = z
+        first = false;
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < LPT; k++) {
+          const int i = otid + k * NT;
+          if (i < N) {
+            const float2 ap = reinterpret_cast<const float2 *>(PL + 7 * i + 1)[1];
+            const float2 idg = s.G[i];
+            float2 r = reinterpret_cast<const float2 *>(XR + i)[1];
+            r.x -= ap.x; r.y -= ap.y;
+            reinterpret_cast<float2 *>(XR + i)[1] = r;
+            const float za = r.x * idg.x, zb = r.y * idg.y;
+            *reinterpret_cast<float2 *>(PL + 7 * i + 2) = make_float2(za, zb);
+            rz_p += r.x * za + r.y * zb; rr_p += r.x * r.x + r.y * r.y;
+          }
+        }
+        const float2 t = red.sum(rz_p, rr_p);
+        rz = t.x; rr = P.cg_norm ? t.x : t.y;
+      } else {
+        const float pAp = red.sum(pAp_part, 0.f).x;
+        const float alpha = rz / pAp;
+        float2 z[LPT], pk[LPT];
+#pragma unroll
+        for (int k = 0; k < LPT; k++) {
+          const int i = otid + k * NT;
+          z[k] = make_float2(0.f, 0.f); pk[k] = make_float2(0.f, 0.f);
+          if (i < N) {
+            const float2 ap = reinterpret_cast<const float2 *>(PL + 7 * i + 1)[1];
+            const float2 idg = s.G[i];
+            pk[k] = *reinterpret_cast<const float2 *>(PL + 7 * i + 2);
+            float4 xr = XR[i];
+            xr.x += alpha * pk[k].x; xr.y += alpha * pk[k].y;
+            xr.z -= alpha * ap.x; xr.w -= alpha * ap.y;
+            XR[i] = xr;
+            z[k] = make_float2(xr.z * idg.x, xr.w * idg.y);
+            rz_p += xr.z * z[k].x + xr.w * z[k].y; rr_p += xr.z * xr.z + xr.w * xr.w;
+          }
+        }
+        const float2 t = red.sum(rz_p, rr_p);
+        const float beta = t.x / rz;
+        rz = t.x; rr = P.cg_norm ? t.x : t.y;
+#pragma unroll
+        for (int k = 0; k < LPT; k++) {
+          const int i = otid + k * NT;
+          if (i < N)
+            *reinterpret_cast<float2 *>(PL + 7 * i + 2) = make_float2(z[k].x + beta * pk[k].x, z[k].y + beta * pk[k].y);
+        }
+        it++;
+      }
+      if (!(rr > tol2 && it < P.cg_max_iter)) break;
+    }
+    if (!(rr <= tol2)) {
+      if (rr == rr && rr < INFINITY) status |= OB_STATUS_CG_MAXITER;
+      else bad = true;
+    }
+  }
+  *flipp = red.flip;
+  *flags = status | (bad ? kPcgBad : 0);
+  return it;
+}
+
+// ------------------------------------------------------------------------------------------------------
 // k_step<NT, LPT>
 // ------------------------------------------------------------------------------------------------------
 template <int NT, int LPT, int MINB>
@@ -716,16 +957,6 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       parity ^= 1;
     }
     __syncthreads();
-    // lanes of warp 0 <-> links of the n_top leading levels: level of the lane's link, widest child list that
-    // stays inside the warp
-    const int ntopN = s.lev[ntop];
-    int top_lvl = -1, top_maxc = 0;
-    if (lane < ntopN) {
-      for (int l = 0; l < ntop; l++)
-        if (lane >= s.lev[l]) top_lvl = l;
-      if (top_lvl < ntop - 1) top_maxc = (int)((s.T[lane] >> kNcShift) & kNcMask);
-    }
-    top_maxc = __reduce_max_sync(0xffffffffu, top_maxc);
     // user forces on apples are constant over the launch
     for (int a = tid; a < d.A; a += NT) {
       float3 fu = f3(0, 0, 0);
@@ -763,212 +994,10 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       const float2 bbz = red.sum(bb_part, bz_part);
       const float bb = bbz.x, bz = bbz.y;
       // ---- C: PCG, warm-started from the previous dqd (x) ----
-      int it = 0;
-      bool bad = false;
-      if (bb == 0.f) {
-#pragma unroll
-        for (int k = 0; k < LPT; k++) {
-          const int i = otid + k * NT;
-          if (i < N) XR[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-        }
-      } else if (!(bb < INFINITY)) {
-        bad = true;
-      } else {
-#pragma unroll
-        for (int k = 0; k < LPT; k++) {                 // first product: A x, i.e. p = x
-          const int i = otid + k * NT;
-          if (i < N) *reinterpret_cast<float2 *>(PL + 7 * i + 2) = *reinterpret_cast<const float2 *>(XR + i);
-        }
-        bool first = true;
-        float rz = 0.f, rr = 0.f;
-        // stopping rule: |r| <= tol |b| in the 2-norm (cg_norm 0) or in the preconditioned norm (cg_norm 1)
-        const float tol2 = P.cg_tol * P.cg_tol * (P.cg_norm ? bz : bb);
-        for (;;) {
-          // ---- A p.  The n_top leading levels live in warp 0, lane = link: own record in registers, parents
-          //      and children by shuffle, no barrier.  The other levels are swept by the whole CTA, one block
-          //      barrier per level; the deepest level turns around at once ----
-          float pAp_part = 0.f;
-          if (top_warp) {
-            const int me = lane < ntopN ? lane : Np;             // idle lanes work on the zero record
-            const uint32_t tw = s.T[me];
-            float4 *rec = PL + 7 * me;
-            const float4 pd = rec[2];
-            const Jt j = load_jt(PL, me);
-            const int parl = (tw & kTrunk) ? lane : (int)(tw & kParMask);   // the trunk's "parent" is all zero at level 0
-            const float3 sp = f3(j.c2 * pd.x, pd.y, j.s2 * pd.x);
-            float3 al = f3(0, 0, 0), a = f3(0, 0, 0);
-#pragma unroll 1
-            for (int l = 0; l < ntop; l++) {                      // branch-free: every lane computes, level l commits
-              float3 alp, ap;
-              alp.x = __shfl_sync(0xffffffffu, al.x, parl); alp.y = __shfl_sync(0xffffffffu, al.y, parl);
-              alp.z = __shfl_sync(0xffffffffu, al.z, parl);
-              ap.x = __shfl_sync(0xffffffffu, a.x, parl); ap.y = __shfl_sync(0xffffffffu, a.y, parl);
-              ap.z = __shfl_sync(0xffffffffu, a.z, parl);
-              const float3 nal = mul(j.E, alp) + sp;
-              const float3 na = mul(j.E, f3(ap.x + alp.y * j.rz, ap.y - alp.x * j.rz, ap.z));
-              const bool mine = top_lvl == l;
-              al.x = mine ? nal.x : al.x; al.y = mine ? nal.y : al.y; al.z = mine ? nal.z : al.z;
-              a.x = mine ? na.x : a.x; a.y = mine ? na.y : a.y; a.z = mine ? na.z : a.z;
-            }
-            if (lane < ntopN) {
-              rec[0] = make_float4(al.x, al.y, al.z, a.x);
-              *reinterpret_cast<float2 *>(rec + 1) = make_float2(a.y, a.z);
-            }
-          }
-          __syncthreads();
-#pragma unroll 1
-          for (int l = ntop; l < nlev; l++) {
-            const int le = s.lev[l + 1];
-            const bool deepest = l == nlev - 1;
-#pragma unroll 1
-            for (int i = s.lev[l] + tid; i < le; i += NT) {
-              const uint32_t tw = s.T[i];
-              float4 *rec = PL + 7 * i;
-              const float4 pd = rec[2];
-              const Jt j = load_jt(PL, i);
-              float3 al, a;
-              mv_down(j, PL, tw, pd, al, a);
-              if (deepest) {
-                pAp_part += mv_up<false>(j, PL, PL + 7 * Np, i, tw, pd, al, a, s, g, c);
-              } else {
-                rec[0] = make_float4(al.x, al.y, al.z, a.x);
-                *reinterpret_cast<float2 *>(rec + 1) = make_float2(a.y, a.z);
-              }
-            }
-            __syncthreads();
-          }
-#pragma unroll 1
-          for (int l = nlev - 2; l >= ntop; l--) {
-            const int le = s.lev[l + 1];
-#pragma unroll 1
-            for (int i = s.lev[l] + tid; i < le; i += NT) {
-              const uint32_t tw = s.T[i];
-              const float4 *rec = PL + 7 * i;
-              const float4 pd = rec[2];
-              const Jt j = load_jt(PL, i);
-              const float4 u = rec[0], v = rec[1];
-              pAp_part += mv_up<true>(j, PL, PL + 7 * Np, i, tw, pd, f3(u.x, u.y, u.z), f3(u.w, v.x, v.y), s, g, c);
-            }
-            __syncthreads();
-          }
-          if (top_warp) {
-            const int me = lane < ntopN ? lane : Np;
-            const uint32_t tw = s.T[me];
-            float4 *rec = PL + 7 * me;
-            const float4 pd = rec[2], I = rec[6];
-            const Jt j = load_jt(PL, me);
-            const float4 u = rec[0], v = rec[1];
-            const float3 al = f3(u.x, u.y, u.z), a = f3(u.w, v.x, v.y);
-            const int fc = (int)((tw >> kChShift) & kParMask), nc = (int)((tw >> kNcShift) & kNcMask);
-            // own inertia force; the children of the last top level are in shared memory, all others are lanes
-            float3 n0 = f3(I.z * al.x - I.y * a.y, I.z * al.y + I.y * a.x, I.w * al.z);
-            float3 f0 = f3(I.x * a.x + I.y * al.y, I.x * a.y - I.y * al.x, I.x * a.z);
-            if (tw & kOffax) {
-              const Force6 t = offaxis_tethers(__ldg(g.topo2 + me), al, a, s.att, s.ao, s.ak, s.Ap, P.h * P.h);
-              n0 = n0 + t.n; f0 = f0 + t.f;
-            }
-            if (top_lvl == ntop - 1) gather_children(PL, PL + 7 * Np, fc, nc, n0, f0);
-            const int nct = (top_lvl >= 0 && top_lvl < ntop - 1) ? nc : 0;
-            float3 un = f3(0, 0, 0), uf = f3(0, 0, 0);           // (n, f) of this link in its parent's frame
-            float t1 = 0.f, t2 = 0.f;
-#pragma unroll 1
-            for (int l = ntop - 1; l >= 0; l--) {                // branch-free: every lane computes, level l commits
-              float3 n = n0, f = f0;
-#pragma unroll
-              for (int k = 0; k < 4; k++) {
-                const int src = min(fc + k, 31);
-                const float c0 = __shfl_sync(0xffffffffu, un.x, src), c1 = __shfl_sync(0xffffffffu, un.y, src),
-                            c2 = __shfl_sync(0xffffffffu, un.z, src), c3 = __shfl_sync(0xffffffffu, uf.x, src),
-                            c4 = __shfl_sync(0xffffffffu, uf.y, src), c5 = __shfl_sync(0xffffffffu, uf.z, src);
-                const bool on = k < nct;
-                n.x += on ? c0 : 0.f; n.y += on ? c1 : 0.f; n.z += on ? c2 : 0.f;
-                f.x += on ? c3 : 0.f; f.y += on ? c4 : 0.f; f.z += on ? c5 : 0.f;
-              }
-              if (top_maxc > 4) {                                // uniform over the warp; wide fans are rare
-#pragma unroll 1
-                for (int k = 4; k < top_maxc; k++) {
-                  const int src = min(fc + k, 31);
-                  const float c0 = __shfl_sync(0xffffffffu, un.x, src), c1 = __shfl_sync(0xffffffffu, un.y, src),
-                              c2 = __shfl_sync(0xffffffffu, un.z, src), c3 = __shfl_sync(0xffffffffu, uf.x, src),
-                              c4 = __shfl_sync(0xffffffffu, uf.y, src), c5 = __shfl_sync(0xffffffffu, uf.z, src);
-                  const bool on = k < nct;
-                  n.x += on ? c0 : 0.f; n.y += on ? c1 : 0.f; n.z += on ? c2 : 0.f;
-                  f.x += on ? c3 : 0.f; f.y += on ? c4 : 0.f; f.z += on ? c5 : 0.f;
-                }
-              }
-              const float nt1 = j.c2 * n.x + j.s2 * n.z + pd.z * pd.x;
-              const float nt2 = n.y + pd.w * pd.y;
-              const float3 nuf = mulT(j.E, f);
-              float3 nun = mulT(j.E, n);
-              nun.x -= j.rz * nuf.y; nun.y += j.rz * nuf.x;
-              const bool mine = top_lvl == l;
-              t1 = mine ? nt1 : t1; t2 = mine ? nt2 : t2;
-              un.x = mine ? nun.x : un.x; un.y = mine ? nun.y : un.y; un.z = mine ? nun.z : un.z;
-              uf.x = mine ? nuf.x : uf.x; uf.y = mine ? nuf.y : uf.y; uf.z = mine ? nuf.z : uf.z;
-            }
-            if (lane < ntopN) {
-              reinterpret_cast<float2 *>(rec + 1)[1] = make_float2(t1, t2);
-              pAp_part += pd.x * t1 + pd.y * t2;
-            }
-          }
-          float rz_p = 0.f, rr_p = 0.f;
-          if (first) {                                 // r = b - A x, z = P^-1 r, p = z
-            first = false;
-            __syncthreads();
-#pragma unroll
-            for (int k = 0; k < LPT; k++) {
-              const int i = otid + k * NT;
-              if (i < N) {
-                const float2 ap = reinterpret_cast<const float2 *>(PL + 7 * i + 1)[1];
-                const float2 idg = s.G[i];
-                float2 r = reinterpret_cast<const float2 *>(XR + i)[1];
-                r.x -= ap.x; r.y -= ap.y;
-                reinterpret_cast<float2 *>(XR + i)[1] = r;
-                const float za = r.x * idg.x, zb = r.y * idg.y;
-                *reinterpret_cast<float2 *>(PL + 7 * i + 2) = make_float2(za, zb);
-                rz_p += r.x * za + r.y * zb; rr_p += r.x * r.x + r.y * r.y;
-              }
-            }
-            const float2 t = red.sum(rz_p, rr_p);
-            rz = t.x; rr = P.cg_norm ? t.x : t.y;
-          } else {
-            const float pAp = red.sum(pAp_part, 0.f).x;
-            const float alpha = rz / pAp;
-            float2 z[LPT], pk[LPT];
-#pragma unroll
-            for (int k = 0; k < LPT; k++) {
-              const int i = otid + k * NT;
-              z[k] = make_float2(0.f, 0.f); pk[k] = make_float2(0.f, 0.f);
-              if (i < N) {
-                const float2 ap = reinterpret_cast<const float2 *>(PL + 7 * i + 1)[1];
-                const float2 idg = s.G[i];
-                pk[k] = *reinterpret_cast<const float2 *>(PL + 7 * i + 2);
-                float4 xr = XR[i];
-                xr.x += alpha * pk[k].x; xr.y += alpha * pk[k].y;
-                xr.z -= alpha * ap.x; xr.w -= alpha * ap.y;
-                XR[i] = xr;
-                z[k] = make_float2(xr.z * idg.x, xr.w * idg.y);
-                rz_p += xr.z * z[k].x + xr.w * z[k].y; rr_p += xr.z * xr.z + xr.w * xr.w;
-              }
-            }
-            const float2 t = red.sum(rz_p, rr_p);
-            const float beta = t.x / rz;
-            rz = t.x; rr = P.cg_norm ? t.x : t.y;
-#pragma unroll
-            for (int k = 0; k < LPT; k++) {
-              const int i = otid + k * NT;
-              if (i < N)
-                *reinterpret_cast<float2 *>(PL + 7 * i + 2) = make_float2(z[k].x + beta * pk[k].x, z[k].y + beta * pk[k].y);
-            }
-            it++;
-          }
-          if (!(rr > tol2 && it < P.cg_max_iter)) break;
-        }
-        if (!(rr <= tol2)) {
-          if (rr == rr && rr < INFINITY) status |= OB_STATUS_CG_MAXITER;
-          else bad = true;
-        }
-      }
+      int pcg_flags = 0;
+      const int it = pcg_solve<NT, LPT>(&s_world, c, s_stage, &red.flip, otid, top_warp, bb, bz, &pcg_flags);
+      status |= pcg_flags & OB_STATUS_CG_MAXITER;
+      const bool bad = (pcg_flags & kPcgBad) != 0;
       // a non-finite solve freezes the world at its last finite state
       int nf = 0;
 #pragma unroll
