@@ -106,13 +106,17 @@ struct DevCtx {
 //      registers; everything the level sweeps touch lives in shared memory, so the sweep code exists once and
 //      runs over any number of links.
 struct StepClass { int nt, lpt, min_ctas; };
-constexpr int kNumClasses = 4;
+constexpr int kNumClasses = 5;
 #ifndef OB_CLS1_NT
-#define OB_CLS1_NT 192
-#define OB_CLS1_LPT 3
+#define OB_CLS1_NT 128
+#define OB_CLS1_LPT 4
 #endif
-constexpr StepClass kStepClasses[kNumClasses] = {{128, 2, 6}, {OB_CLS1_NT, OB_CLS1_LPT, 3}, {512, 2, 1}, {512, 3, 1}};
-constexpr int kMaxLinksOnChip = 512 * 3;
+// Few threads per world: measured on configs[3] (350-450 links, three worlds per SM) 128 threads x 4 links
+// give 3.75M world-steps/s, 192 x 3 3.26M, 256 x 2 2.90M, 64 x 8 3.27M: a PCG iteration is a chain of short
+// phases, and more warps per world only add barrier and loop overhead to each of them.
+constexpr StepClass kStepClasses[kNumClasses] = {
+    {64, 4, 6}, {OB_CLS1_NT, OB_CLS1_LPT, 3}, {192, 4, 2}, {256, 4, 1}, {256, 6, 1}};
+constexpr int kMaxLinksOnChip = 256 * 6;
 constexpr int kMaxChildren = 15;     // children per link (4 bits of the packed topology word)
 inline int step_class_of(int Np) {   // host only
   for (int k = 0; k < kNumClasses; k++)

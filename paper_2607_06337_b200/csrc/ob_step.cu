@@ -128,9 +128,15 @@ struct Reducer {
     if ((tid & 15) == 0) st[2 * (tid >> 5) + (hi ? 1 : 0)] = v;
     __syncthreads();
     float sa = 0.f, sb = 0.f;
-    const float4 *s4 = reinterpret_cast<const float4 *>(st);
+    if (NT % 64 == 0) {
+      const float4 *s4 = reinterpret_cast<const float4 *>(st);
 #pragma unroll
-    for (int k = 0; k < NT / 64; k++) { const float4 t = s4[k]; sa += t.x + t.z; sb += t.y + t.w; }
+      for (int k = 0; k < NT / 64; k++) { const float4 t = s4[k]; sa += t.x + t.z; sb += t.y + t.w; }
+    } else {
+      const float2 *s2 = reinterpret_cast<const float2 *>(st);
+#pragma unroll
+      for (int k = 0; k < NT / 32; k++) { const float2 t = s2[k]; sa += t.x; sb += t.y; }
+    }
     return make_float2(sa, sb);
   }
 };
@@ -1104,13 +1110,14 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
 // ------------------------------------------------------------------------------------------------------
 // launchers: one instantiation per size class (ob_internal.h: kStepClasses)
 // ------------------------------------------------------------------------------------------------------
-#define OB_FOR_CLASS(cls, CALL)                         \
-  switch (cls) {                                        \
-    case 0: { CALL(128, 2, 6); break; }                 \
-    case 1: { CALL(OB_CLS1_NT, OB_CLS1_LPT, 3); break; }                 \
-    case 2: { CALL(512, 2, 1); break; }                 \
-    case 3: { CALL(512, 3, 1); break; }                 \
-    default: return cudaErrorInvalidValue;              \
+#define OB_FOR_CLASS(cls, CALL)                                     \
+  switch (cls) {                                                    \
+    case 0: { CALL(64, 4, 6); break; }                              \
+    case 1: { CALL(OB_CLS1_NT, OB_CLS1_LPT, 3); break; }            \
+    case 2: { CALL(192, 4, 2); break; }                             \
+    case 3: { CALL(256, 4, 1); break; }                             \
+    case 4: { CALL(256, 6, 1); break; }                             \
+    default: return cudaErrorInvalidValue;                          \
   }
 
 cudaError_t step_kernel_setup(int cls, int smem_bytes, int *max_blocks_per_sm) {

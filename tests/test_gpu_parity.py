@@ -416,12 +416,14 @@ def test_edge_cases_single_link_no_apples_and_heterogeneous_batch():
              chain_spec(17, 1.7, 0.03, root_quat=quat_axis("y", 60.0),
                         apples=[(16, (0, 0, 0.1), 0.2, 2e3, 20.0), (16, (0.01, 0, 0.05), 0.15, 2e3, 15.0),
                                 (3, (0, 0.015, 0.02), 0.25, 2e3, 25.0)]),
-             binary_tree_config1(), big]
+             binary_tree_config1(), big,
+             stochastic_world(rng, 600, 640, 60, depth_choices=(6, 7)),      # one world per k_step size class
+             stochastic_world(rng, 900, 960, 90, depth_choices=(7, 8))]
     P = config_params(4)
     sim, refs = _make(specs, P, seed=31337)
     _apply(sim, refs, [(1, 9, (0.0, 0.015, 0.05), (3.0, -2.0, 1.0)), (3, BIG_N // 2, (0.0, 0.0, 0.01), (5.0, 5.0, -5.0))])
     sim.step(10)
-    errs = _single_step_errors(sim, refs, range(4))
+    errs = _single_step_errors(sim, refs, range(len(specs)))
     for w, e in errs.items():
         assert e["max"] <= TOL_STEP, (w, e)
     info = sim.launch_info()
