@@ -157,7 +157,7 @@ inline int pad8(int n) { return (n + 7) / 8 * 8; }
 
 struct Layout {
   size_t total = 0;
-  Pool desc, order, link_blk, apple_blk, topo, topo2, child_list, quat, quat_raw, R0, Mmax, Lown, diam, arm, link_ext, apple_ext, apple_nom,
+  Pool desc, order, link_blk, apple_blk, topo, topo2, child_list, quat, quat_raw, R0, Mmax, mdiag, Lown, diam, arm, link_ext, apple_ext, apple_nom,
       apple_c, anchor, level_off, info, wrench, events, ev_count, queue, pose7;
   size_t sumNp = 0, sumAp = 0, sumLev = 0, ev_cap = 0;
   int max_Np = 0, max_Ap = 0, max_smem = 0;
@@ -215,6 +215,7 @@ int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) 
   take(L, L.quat_raw, sizeof(float4) * L.sumNp);
   take(L, L.R0, sizeof(float) * 9 * L.sumNp);
   take(L, L.Mmax, sizeof(float) * L.sumNp);
+  take(L, L.mdiag, sizeof(float2) * L.sumNp);
   take(L, L.Lown, sizeof(float) * L.sumNp);
   take(L, L.diam, sizeof(float) * L.sumNp);
   take(L, L.arm, L.any_arm ? sizeof(float) * 2 * L.sumNp : 0);
@@ -463,6 +464,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   D.quat_raw = reinterpret_cast<float4 *>(base + L.quat_raw.off);
   D.R0 = reinterpret_cast<float *>(base + L.R0.off);
   D.Mmax = reinterpret_cast<float *>(base + L.Mmax.off);
+  D.mdiag = reinterpret_cast<float2 *>(base + L.mdiag.off);
   D.Lown = reinterpret_cast<float *>(base + L.Lown.off);
   D.diam = reinterpret_cast<float *>(base + L.diam.off);
   D.arm = L.any_arm ? reinterpret_cast<float *>(base + L.arm.off) : nullptr;
@@ -700,6 +702,7 @@ int ob_set_state(ob_ctx *ctx, int world, const float *q, const float *qd, const 
     if (attached) { af[a] = attached[e] ? 1 : 0; af[d.Ap + a] = 0; af[2 * d.Ap + a] = 0; }
   }
   wi.status = 0;
+  wi.diag_age = 0;          // the state was written from outside: recompute the preconditioner at the next step
   CU(cpy(ctx, ctx->dev.link_blk + d.link_blk_off, lb.data(), lb.size(), cudaMemcpyHostToDevice, ctx->stream));
   if (d.Ap)
     CU(cpy(ctx, ctx->dev.apple_blk + d.apple_blk_off, ab.data(), apple_state_bytes(d.Ap), cudaMemcpyHostToDevice,

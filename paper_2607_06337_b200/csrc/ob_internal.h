@@ -54,7 +54,7 @@ struct WorldInfo {       // mutable per-world scalars
   int32_t steps_taken;           // world-steps actually advanced (frozen worlds do not count)
   unsigned long long cg_iters;   // PCG iterations since ob_create
   float E, MOR, density;         // current material draws
-  int32_t pad_;
+  int32_t diag_age;              // steps since diag(M) of the Jacobi preconditioner was recomputed (0 = recompute)
 };
 
 struct WrenchSlots {     // device mirror of the persistent wrenches of one world (internal body indices)
@@ -82,6 +82,7 @@ struct DevCtx {
   const float4 *quat_raw;        // rest quaternion exactly as the caller gave it (create-time fp64 rest pose)
   float *R0;                     // [9 * link_base + k * Np + i] rest world rotation, row-major k
   float *Mmax;                   // rupture moment (after randomize)
+  float2 *mdiag;                 // [link_base + i] diag(M) of the two DoF as last computed by phase B2
   const float *Lown;             // link length
   const float *diam;             // link diameter
   const float *arm;              // [2 * link_base + k * Np + i] armature or nullptr
@@ -117,6 +118,7 @@ constexpr int kNumClasses = 5;
 constexpr StepClass kStepClasses[kNumClasses] = {
     {64, 4, 6}, {OB_CLS1_NT, OB_CLS1_LPT, 3}, {192, 4, 2}, {256, 4, 1}, {256, 6, 1}};
 constexpr int kMaxLinksOnChip = 256 * 6;
+constexpr int kDiagRefresh = 8;      // phase B2 (exact diag(M)) runs every kDiagRefresh-th step of a world
 constexpr int kMaxChildren = 15;     // children per link (4 bits of the packed topology word)
 inline int step_class_of(int Np) {   // host only
   for (int k = 0; k < kNumClasses; k++)

@@ -98,6 +98,7 @@ struct Gm {
   const float4 *quat;
   const float *R0;                  // [k * Np + i]
   const float *Mmax;
+  float2 *mdiag;                    // diag(M) as last computed by phase B2 (the Jacobi preconditioner may lag)
   const float *arm;                 // [k * Np + i] or nullptr
   const int4 *topo2;                // x = first apple | n_apples << 16, y = inner slot | parent's inner slot << 16
 };
@@ -266,6 +267,9 @@ __device__ __forceinline__ float mv_up(const Jt &j, float4 *P, const float4 *zer
 //   B1  bottom-up inner links: own (n, f) + children -> rhs b (-> G), (n, f) for the parent
 // ------------------------------------------------------------------------------------------------------
 
+// the views of the world every thread of the CTA shares (in shared memory, filled once per world)
+struct World { Sm s; Gm g; int N, nlev, ntop; };
+
 // a double carried as two floats (hi + lo): 48 bits, plenty for a displacement summed along <= 2000 links
 __device__ __forceinline__ float2 split2(const double v) {
   const float hi = (float)v;
@@ -350,8 +354,12 @@ __device__ __forceinline__ void link_fk(const int i, const Sm &s) {
 // tether reactions (Eq. 6 / Eq. 7) and user wrenches on one link, subtracted from its bias
 // force (n, f); also leaves the tether force and |f_s| of each apple for phase D.  Only links that carry apples or
 // a wrench come here.
+// (Not inlined.  It takes the World in shared memory, not references to the caller's copies: a reference would
+// force those copies into local memory, and every pointer fetched from there is an L2 round trip.)
 __device__ __noinline__ Force6 external_forces(const int i, const float3 om, const float3 vl, const uint32_t tw,
-                                               const Sm &s, const Gm &g, const DevCtx &c) {
+                                               const World *wd, const DevCtx &c) {
+  const Sm s = wd->s;
+  const Gm g = wd->g;
   const ob_params &P = c.P;
   const int Np = s.Np, Ap = s.Ap;
   Force6 out;
@@ -429,7 +437,7 @@ __device__ __forceinline__ void finish_bias(const Jt &j, const int i, const uint
 
 // ---- A2 ----  velocity, bias acceleration (gravity as base acceleration), own bias force
 //               f = I a + v x* I v - tether reactions - user wrenches  (RNEA with qdd = 0)
-__device__ __forceinline__ void link_bias(const int i, const Sm &s, const Gm &g, const DevCtx &c) {
+__device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm &s, const Gm &g, const DevCtx &c) {
   const ob_params &P = c.P;
   const int NIp = s.NIp;
   const uint32_t tw = s.T[i];
@@ -470,7 +478,7 @@ __device__ __forceinline__ void link_bias(const int i, const Sm &s, const Gm &g,
   bool ext = (tw & kHasApples) != 0u;
   for (int q = 0; q < s.wr->n; q++) ext |= s.wr->body[q] == i;
   if (ext) {
-    const Force6 e = external_forces(i, om, vl, tw, s, g, c);
+    const Force6 e = external_forces(i, om, vl, tw, wd, c);
     n = n + e.n; f = f + e.f;
   }
   if (inner) {                                                    // parked until B1 adds the children
@@ -533,10 +541,10 @@ __device__ __forceinline__ void up_inertia(const int i, const Sm &s, const Gm &g
   const Jt j = load_jt(s.P, i);
   const float c2 = j.c2, s2 = j.s2;
   const float2 dt = reinterpret_cast<const float2 *>(s.P + 7 * i + 2)[1];
-  const float d1 = c2 * c2 * Ixx + 2.f * c2 * s2 * Ixz + s2 * s2 * Izz + dt.x;
-  const float d2 = Iyy + dt.y;
+  const float m1 = c2 * c2 * Ixx + 2.f * c2 * s2 * Ixz + s2 * s2 * Izz, m2 = Iyy;
+  g.mdiag[i] = make_float2(m1, m2);
   float2 id = make_float2(1.f, 1.f);
-  if (P.precond == 1) id = make_float2(1.f / d1, 1.f / d2);
+  if (P.precond == 1) id = make_float2(1.f / (m1 + dt.x), 1.f / (m2 + dt.y));
   s.G[i] = id;
   if (!(tw & kTrunk)) {
     const M3 &E = j.E;
@@ -557,6 +565,36 @@ __device__ __forceinline__ void up_inertia(const int i, const Sm &s, const Gm &g
   }
 }
 
+// phase B2 on the steps between two recomputations of diag(M): the effective link inertia (it is part of A and must
+// be exact: it changes when an apple detaches, and phase A1 borrows its slot) and the Jacobi factors from the stored
+// diag(M) plus the CURRENT diagonal spring-damper terms.  A lagging preconditioner changes the number of PCG
+// iterations, never the system that is solved.
+__device__ __forceinline__ void link_inertia_lagged(const int i, const Sm &s, const Gm &g, const DevCtx &c) {
+  const ob_params &P = c.P;
+  const int Ap = s.Ap;
+  uint32_t tw = s.T[i];
+  float4 eff = __ldg(g.c4 + i);
+  const float2 md = g.mdiag[i];
+  if (P.tether_implicit && (tw & kHasApples)) {
+    tw &= ~kOffax;
+    const int4 t2 = __ldg(g.topo2 + i);
+    const int ast = t2.x & 0xffff, nap = t2.x >> 16;
+    for (int a = ast; a < ast + nap; a++) {
+      if (!s.att[a]) continue;
+      const float mv = P.h * P.h * s.ak[a];
+      const float3 o = f3(s.ao[a], s.ao[Ap + a], s.ao[2 * Ap + a]);
+      if (o.x == 0.f && o.y == 0.f) { eff.x += mv; eff.y += mv * o.z; eff.z += mv * o.z * o.z; }
+      else tw |= kOffax;
+    }
+    s.T[i] = tw;
+  }
+  s.P[7 * i + 6] = eff;
+  const float2 dt = reinterpret_cast<const float2 *>(s.P + 7 * i + 2)[1];
+  float2 id = make_float2(1.f, 1.f);
+  if (P.precond == 1) id = make_float2(1.f / (md.x + dt.x), 1.f / (md.y + dt.y));
+  s.G[i] = id;
+}
+
 // fence after level l of a top-down sweep / after level l of a bottom-up sweep (see "Order" above)
 #define OB_FENCE_DOWN(l) { if ((l) + 1 < ntop) __syncwarp(); else __syncthreads(); }
 #define OB_FENCE_UP(l) { if ((l) < ntop) __syncwarp(); else __syncthreads(); }
@@ -566,7 +604,6 @@ __device__ __forceinline__ void up_inertia(const int i, const Sm &s, const Gm &g
 // quantities per link in flight) stays out of the allocation of the PCG loop.  The views of the world live in
 // shared memory (World), the context is the kernel's __grid_constant__ parameter.
 // ------------------------------------------------------------------------------------------------------
-struct World { Sm s; Gm g; int N, nlev, ntop; };
 #ifndef OB_COLD_ATTR
 #define OB_COLD_ATTR __noinline__
 #endif
@@ -593,7 +630,7 @@ __device__ OB_COLD_ATTR void sweep_bias(const World *wd, const DevCtx &c, const 
   for (int l = l_first_down; l < nlev; l++) {
     const int le = s.lev[l + 1];
 #pragma unroll 1
-    for (int i = s.lev[l] + tid; i < le; i += nt) link_bias(i, s, g, c);
+    for (int i = s.lev[l] + tid; i < le; i += nt) link_bias(i, wd, s, g, c);
     OB_FENCE_DOWN(l)
   }
   // ---- B1: bias forces bottom-up over the inner links -> rhs b ----
@@ -610,10 +647,17 @@ __device__ OB_COLD_ATTR void sweep_bias(const World *wd, const DevCtx &c, const 
   __syncthreads();
 }
 
-__device__ OB_COLD_ATTR void sweep_inertia(const World *wd, const DevCtx &c, const int nt, const int otid) {
+__device__ OB_COLD_ATTR void sweep_inertia(const World *wd, const DevCtx &c, const int nt, const int otid,
+                                           const bool refresh) {
   const Sm s = wd->s;
   const Gm g = wd->g;
   const int nlev = wd->nlev, ntop = wd->ntop, N = wd->N, tid = threadIdx.x;
+  if (!refresh) {
+#pragma unroll 1
+    for (int i = otid; i < N; i += nt) link_inertia_lagged(i, s, g, c);
+    __syncthreads();
+    return;
+  }
   const int l_last_up = tid < 32 ? 0 : ntop;
   // ---- B2: composite inertia bottom-up -> Jacobi factors, effective inertia (all leaves first) ----
 #pragma unroll 1
@@ -927,6 +971,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       g.quat = c.quat + d.link_base;
       g.R0 = c.R0 + 9 * (size_t)d.link_base;
       g.Mmax = c.Mmax + d.link_base;
+      g.mdiag = c.mdiag + d.link_base;
       g.arm = c.arm ? c.arm + 2 * (size_t)d.link_base : nullptr;
       g.topo2 = c.topo2 + d.link_base;
     }
@@ -973,7 +1018,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
     }
     __syncthreads();
 
-    int step0 = info->step, steps_done = 0, last_iters = 0;
+    int step0 = info->step, steps_done = 0, last_iters = 0, diag_age = info->diag_age;
     unsigned long long iters_total = 0;
     for (int sidx = 0; sidx < n_steps; sidx++) {
       sweep_bias(&s_world, c, NT);                      // A, B1
@@ -985,7 +1030,8 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
           XR[i] = make_float4(x0.x, x0.y, b.x, b.y);
         }
       }
-      sweep_inertia(&s_world, c, NT, otid);                   // B2: G[i] is first rewritten by the thread that just read it
+      sweep_inertia(&s_world, c, NT, otid, diag_age == 0);
+      diag_age = diag_age + 1 >= kDiagRefresh ? 0 : diag_age + 1;   // (B2 first rewrites G[i] by the thread that just read it)
       float bb_part = 0.f, bz_part = 0.f;
 #pragma unroll
       for (int k = 0; k < LPT; k++) {
@@ -1100,6 +1146,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       info->step = step0 + steps_done;
       info->last_iters = last_iters;
       info->status = status;
+      info->diag_age = diag_age;
       info->steps_taken += steps_done;
       info->cg_iters += iters_total;
     }
