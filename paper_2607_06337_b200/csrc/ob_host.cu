@@ -157,7 +157,7 @@ inline int pad8(int n) { return (n + 7) / 8 * 8; }
 
 struct Layout {
   size_t total = 0;
-  Pool desc, order, link_blk, apple_blk, topo, topo2, child_list, quat, quat_raw, R0, Mmax, mdiag, Lown, diam, arm, link_ext, apple_ext, apple_nom,
+  Pool desc, order, link_blk, apple_blk, topo, topo2, child_list, quat, quat_raw, R0, Mmax, mdiag, xprev, Lown, diam, arm, link_ext, apple_ext, apple_nom,
       apple_c, anchor, level_off, info, wrench, events, ev_count, queue, pose7;
   size_t sumNp = 0, sumAp = 0, sumLev = 0, ev_cap = 0;
   int max_Np = 0, max_Ap = 0, max_smem = 0;
@@ -216,6 +216,7 @@ int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) 
   take(L, L.R0, sizeof(float) * 9 * L.sumNp);
   take(L, L.Mmax, sizeof(float) * L.sumNp);
   take(L, L.mdiag, sizeof(float2) * L.sumNp);
+  take(L, L.xprev, sizeof(float2) * 2 * L.sumNp);
   take(L, L.Lown, sizeof(float) * L.sumNp);
   take(L, L.diam, sizeof(float) * L.sumNp);
   take(L, L.arm, L.any_arm ? sizeof(float) * 2 * L.sumNp : 0);
@@ -465,6 +466,8 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   D.R0 = reinterpret_cast<float *>(base + L.R0.off);
   D.Mmax = reinterpret_cast<float *>(base + L.Mmax.off);
   D.mdiag = reinterpret_cast<float2 *>(base + L.mdiag.off);
+  D.xprev = reinterpret_cast<float2 *>(base + L.xprev.off);
+  D.sum_np = (int32_t)L.sumNp;
   D.Lown = reinterpret_cast<float *>(base + L.Lown.off);
   D.diam = reinterpret_cast<float *>(base + L.diam.off);
   D.arm = L.any_arm ? reinterpret_cast<float *>(base + L.arm.off) : nullptr;

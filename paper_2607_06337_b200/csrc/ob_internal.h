@@ -83,6 +83,8 @@ struct DevCtx {
   float *R0;                     // [9 * link_base + k * Np + i] rest world rotation, row-major k
   float *Mmax;                   // rupture moment (after randomize)
   float2 *mdiag;                 // [link_base + i] diag(M) of the two DoF as last computed by phase B2
+  float2 *xprev;                 // [2][sumNp]: dqd of the two steps before the last (PCG start: extrapolation)
+  int32_t sum_np;                // stride of xprev
   const float *Lown;             // link length
   const float *diam;             // link diameter
   const float *arm;              // [2 * link_base + k * Np + i] armature or nullptr
