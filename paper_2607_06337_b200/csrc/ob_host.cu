@@ -216,7 +216,7 @@ int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) 
   take(L, L.R0, sizeof(float) * 9 * L.sumNp);
   take(L, L.Mmax, sizeof(float) * L.sumNp);
   take(L, L.mdiag, sizeof(float2) * L.sumNp);
-  take(L, L.xprev, sizeof(float2) * 2 * L.sumNp);
+  take(L, L.xprev, sizeof(float2) * 3 * L.sumNp);
   take(L, L.Lown, sizeof(float) * L.sumNp);
   take(L, L.diam, sizeof(float) * L.sumNp);
   take(L, L.arm, L.any_arm ? sizeof(float) * 2 * L.sumNp : 0);

@@ -109,6 +109,7 @@ __global__ void k_randomize(DevCtx c, unsigned long long seed, int redraw) {
     fl[i] = 0; fl[d.Np + i] = 0;
     c.xprev[d.link_base + i] = make_float2(0.f, 0.f);              // PCG start-vector history
     c.xprev[c.sum_np + d.link_base + i] = make_float2(0.f, 0.f);
+    c.xprev[2 * c.sum_np + d.link_base + i] = make_float2(0.f, 0.f);
     if (i < d.N) {
       double dd = diam[i], L = Lown[i], r = 0.5 * dd;
       double K = (double)E * PI * dd * dd * dd * dd / (64.0 * L);   // Eq. 4

@@ -99,7 +99,7 @@ struct Gm {
   const float *R0;                  // [k * Np + i]
   const float *Mmax;
   float2 *mdiag;                    // diag(M) as last computed by phase B2 (the Jacobi preconditioner may lag)
-  float2 *xprev, *xprev2;           // dqd of the two steps before the last
+  float2 *xprev, *xprev2, *xprev3;  // dqd of the three steps before the last
   const float *arm;                 // [k * Np + i] or nullptr
   const int4 *topo2;                // x = first apple | n_apples << 16, y = inner slot | parent's inner slot << 16
 };
@@ -270,16 +270,18 @@ __device__ __forceinline__ float mv_up(const Jt &j, float4 *P, const float4 *zer
 
 // the views of the world every thread of the CTA shares (in shared memory, filled once per world)
 struct World { Sm s; Gm g; int N, nlev, ntop; };
-// PCG start vector from the last three solutions: 0 = the last one, 1 = linear, 2 = quadratic extrapolation
+// PCG start vector from the last solutions: 0 = the last one, 1 = linear, 2 = quadratic, 3 = cubic extrapolation
 #ifndef OB_X0_ORDER
-#define OB_X0_ORDER 2
+#define OB_X0_ORDER 3
 #endif
-#if OB_X0_ORDER == 2
-#define OB_X0(x1, x2, x3) (3.f * ((x1) - (x2)) + (x3))
+#if OB_X0_ORDER == 3
+#define OB_X0(x1, x2, x3, x4) (4.f * ((x1) + (x3)) - 6.f * (x2) - (x4))
+#elif OB_X0_ORDER == 2
+#define OB_X0(x1, x2, x3, x4) (3.f * ((x1) - (x2)) + (x3))
 #elif OB_X0_ORDER == 1
-#define OB_X0(x1, x2, x3) (2.f * (x1) - (x2))
+#define OB_X0(x1, x2, x3, x4) (2.f * (x1) - (x2))
 #else
-#define OB_X0(x1, x2, x3) (x1)
+#define OB_X0(x1, x2, x3, x4) (x1)
 #endif
 
 // a double carried as two floats (hi + lo): 48 bits, plenty for a displacement summed along <= 2000 links
@@ -986,6 +988,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       g.mdiag = c.mdiag + d.link_base;
       g.xprev = c.xprev + d.link_base;
       g.xprev2 = c.xprev + c.sum_np + d.link_base;
+      g.xprev3 = c.xprev + 2 * c.sum_np + d.link_base;
       g.arm = c.arm ? c.arm + 2 * (size_t)d.link_base : nullptr;
       g.topo2 = c.topo2 + d.link_base;
     }
@@ -1040,8 +1043,8 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       for (int k = 0; k < LPT; k++) {
         const int i = otid + k * NT;
         if (i < N) {                                    // r = b; x = previous dqd (warm start), kept in global memory
-          const float2 b = s.G[i], x1 = g.x2[i], x2 = g.xprev[i], x3 = g.xprev2[i];
-          XR[i] = make_float4(OB_X0(x1.x, x2.x, x3.x), OB_X0(x1.y, x2.y, x3.y), b.x, b.y);
+          const float2 b = s.G[i], x1 = g.x2[i], x2 = g.xprev[i], x3 = g.xprev2[i], x4 = g.xprev3[i];
+          XR[i] = make_float4(OB_X0(x1.x, x2.x, x3.x, x4.x), OB_X0(x1.y, x2.y, x3.y, x4.y), b.x, b.y);
         }
       }
       sweep_inertia(&s_world, c, NT, otid, diag_age == 0);
@@ -1084,6 +1087,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         if (i >= N) continue;
         const float2 w0 = g.w2[i], q0 = g.q2[i];
         const float2 x = *reinterpret_cast<const float2 *>(XR + i);
+        g.xprev3[i] = g.xprev2[i];
         g.xprev2[i] = g.xprev[i];
         g.xprev[i] = g.x2[i];
         g.x2[i] = x;
@@ -1149,7 +1153,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
 #pragma unroll
       for (int k = 0; k < LPT; k++) {
         const int i = otid + k * NT;
-        if (i < N) { g.x2[i] = make_float2(0.f, 0.f); g.xprev[i] = make_float2(0.f, 0.f); g.xprev2[i] = make_float2(0.f, 0.f); }
+        if (i < N) { g.x2[i] = make_float2(0.f, 0.f); g.xprev[i] = make_float2(0.f, 0.f); g.xprev2[i] = make_float2(0.f, 0.f); g.xprev3[i] = make_float2(0.f, 0.f); }
       }
     }
     fence_proxy_async();
