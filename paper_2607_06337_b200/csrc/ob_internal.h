@@ -11,10 +11,9 @@ namespace ob {
 constexpr int kPad = 16;  // links and apples per world are padded to a multiple of 16 (16-byte TMA granules)
 __host__ __device__ inline int pad16(int n) { return (n + kPad - 1) / kPad * kPad; }
 
-// ---- per-world "link block" in global memory: one contiguous chunk; its state part is staged to shared
-//      memory by one TMA bulk copy and written back by one bulk store, its constants are read from L2 once
-//      per step (they are consumed straight into registers).
-//   float2  q[Np] qd[Np] x[Np]          state, the two DoF of a joint interleaved (x = previous dqd, PCG warm start)
+// ---- per-world "link block" in global memory: one contiguous chunk.  k_step reads and writes it in place (L2):
+//      only the once-per-step phases touch it.
+//   float2  q[Np] qd[Np] x[Np]          state, the two DoF of a joint interleaved (x = previous dqd, PCG start)
 //   bytes   ruptured[Np] rc[Np]         state
 //   float4  c4[Np] = (m, m c, I about the joint, I_zz)   constants (after ob_randomize)
 //   floats  K[Np] rz[Np]                constants (joint stiffness Eq. 4, parent length)

@@ -1,35 +1,42 @@
 // ob_step.cu -- k_step, the product kernel (sm_100a): n physics steps of every world in one launch.
 //
-// One CTA per world in flight (persistent, work queue per size class), several CTAs per SM.  Everything the
-// level-synchronous tree sweeps touch lives in SHARED MEMORY as float4 planes indexed by link, so the sweep code
-// exists once, is a few hundred instructions long (it has to stay inside the instruction cache: the first
-// versions of this kernel were no_instruction-stalled) and runs over any number of links.  Registers hold what
-// only the owner of a link needs: the PCG vectors x, r and the Jacobi factors (link tid + k * NT <-> slot k).
-// The apple block is staged by one TMA bulk copy (UBLKCP) and written back the same way; q, qd stay in global
-// memory (L2) because only the once-per-step phases A and D touch them.
+// One CTA per world in flight (persistent, work queue per size class), three CTAs of 128 threads per SM at the
+// headline size.  Everything the level-synchronous tree sweeps touch lives in SHARED MEMORY as one 112-byte
+// record of seven float4 per link (stride 7 x 16 B: 128-bit accesses of consecutive links are conflict-free),
+// so the sweep code exists once, is about a thousand instructions long (it has to stay inside the instruction
+// cache: the first versions of this kernel were no_instruction-stalled) and runs over any number of links.
+// The apple block is staged by one TMA bulk copy (UBLKCP) and written back the same way; q, qd and the PCG start
+// vectors stay in global memory (L2): only the once-per-step phases touch them.
 //
-//   A   top-down:  joint transforms (Eq. 3), displacement-form FK, velocities, bias accelerations;
-//                  tether forces (Eq. 6 / Eq. 7) and user wrenches -> link bias forces
-//   B1  bottom-up: bias torques -> rhs b (Eq. 4 spring-damper terms)
-//   B2  bottom-up: composite inertia -> exact diagonal of M for the Jacobi preconditioner, effective link inertia
-//   C   matrix-free Jacobi-PCG on (M + M_teth + diag(arm + hD + h^2 K)) dqd = b  (north_star);
-//                  M v = acceleration-only inverse dynamics: top-down a_i, bottom-up f_i, project on S_i
+//   A0  flat:      joint transforms (Eq. 3), own part of the displacement-form FK, spring-damper
+//                  part of the rhs (Eq. 4)
+//   A1  top-down:  displacement-form FK (positions in fp64)
+//   A2  top-down:  velocities, bias accelerations, bias force of every link incl. tether reactions (Eq. 6 / Eq. 7,
+//                  PAPER.md:149-161) and user wrenches; leaves finish at once
+//   B1  bottom-up: bias torques of the inner links -> rhs b
+//   B2  bottom-up: composite inertia -> exact diagonal of M for the Jacobi preconditioner (every kDiagRefresh-th
+//                  step; in between the stored diagonal + the current spring-damper terms), effective link inertia
+//   C   matrix-free Jacobi-PCG on (M + M_teth + diag(arm + hD + h^2 K)) dqd = b  (north_star), started from the
+//                  cubic extrapolation of the last four solutions; M v = acceleration-only inverse dynamics:
+//                  top-down a_i, bottom-up f_i, project on S_i
 //   D   integrate joints and apples; rupture (Eq. 5) and detach predicates
 //
-// Order.  Links are in plain breadth-first order: levels contiguous, the children of a link contiguous.  The
-// leading levels that fit into links 0..31 (n_top of them) are swept by warp 0 with __syncwarp only; every other
-// level ends with one block barrier.  In the PCG sweeps only the deepest level turns around inside the top-down
-// pass (all of its links are leaves); in the once-per-step sweeps every leaf does.
+// Order.  Links are in plain breadth-first order: levels contiguous, the children of a link contiguous.  In the
+// PCG sweeps the leading levels that fit into 32 links (n_top of them) are swept by ONE warp, lane = link, own
+// record in registers, parents and children by shuffle, no barrier; every other level ends with one block
+// barrier; only the deepest level turns around inside the top-down pass (all of its links are leaves).  In the
+// once-per-step sweeps warp 0 takes the leading levels with __syncwarp and every leaf turns around.
 //
-// Planes (S = Np + 1 columns; column Np is never written and stays zero: it stands in for the trunk's parent).
-//   M0, M1   A: kinematics an inner link publishes for its children (with PD, C3 and the overflow: 24 floats);
-//            B1: (n, f) for the parent; B2: composite inertia for the parent; C: (alpha, a) on the way down,
-//            (n, f) on the way up, A p in M1.zw
-//   PD       (p, diagonal terms arm + (h c_d + h^2) K); B2 borrows .xy
-//   C0..C2   E (parent -> link rotation, row-major), c2, s2, parent length
-//   C3       effective link inertia (m, m c, I about the joint, I_zz) incl. on-axis virtual tether masses (A15)
-//   G        b after B1 (it moves into the owner's registers), then 1 / diag(A) after B2
-//   T        packed topology word: parent | first child << 11 | children << 22 | flags
+// Record of link i (P[7 i + j]); record Np is never written and stays zero: the trunk's parent, missing children.
+//   0, 1  M0, M1   A0: R0 (RxRy - I); A1: dR; A2: parked bias force / (n, f) for the parent; B2: composite inertia
+//                  for the parent; C: (alpha, a) on the way down, (n, f) on the way up, A p in M1.zw
+//   2     PD       (p, diagonal terms arm + (h c_d + h^2) K); A1: dR[8], dp.x; B2 borrows .xy
+//   3..5  C0..C2   E (parent -> link rotation, row-major), c2, s2, parent length
+//   6     C3       effective link inertia (m, m c, I about the joint, I_zz) incl. on-axis virtual tether masses
+//                  (A15); A1: dp.y, dp.z
+// Beside the records: G (float2: spring-damper rhs part, then b, then 1 / diag(A)), T (packed topology word:
+// parent | first child << 11 | children << 22 | flags), and one region shared by the A2 overflow (12 floats per
+// inner link: velocity and bias acceleration for the children) and the PCG's (x, r) (one float4 per link).
 //
 // Spatial vectors are [angular; linear at the link origin] in link coordinates.  Link frame: origin at the
 // proximal joint, +z along the link.  Joint i: R_rel = Q_i Rx(theta1) Ry(theta2); E_i = R_rel^T maps parent
@@ -64,16 +71,20 @@ struct Sm {
   WrenchSlots *wr;
 };
 
-__device__ __forceinline__ Sm carve(unsigned char *base, const WorldDesc &d) {
+// The functions that are not inlined carve the CTA's dynamic shared memory again from the sizes (World) instead of
+// taking pointers: pointers handed over through memory are generic, and the sweeps then run on LD.E / ST.E with
+// 64-bit address arithmetic instead of LDS / STS.
+extern __shared__ __align__(128) unsigned char ob_smem[];
+
+__device__ __forceinline__ Sm carve(unsigned char *base, const int Np, const int Ap, const int NIp, const int n_levels) {
   Sm s;
-  s.Np = d.Np; s.Ap = d.Ap; s.NIp = d.NIp; s.S = d.Np + 1;
-  const int Np = d.Np, Ap = d.Ap;
+  s.Np = Np; s.Ap = Ap; s.NIp = NIp; s.S = Np + 1;
   unsigned char *p = base;
   s.P = reinterpret_cast<float4 *>(p); p += step_planes_bytes(Np);
   s.G = reinterpret_cast<float2 *>(p); p += r16(8 * (Np + 1));
   s.T = reinterpret_cast<uint32_t *>(p); p += r16(4 * (Np + 1));
-  s.ovf = reinterpret_cast<float4 *>(p); s.XR = s.ovf; p += step_ovf_bytes(Np, d.NIp);
-  s.lev = reinterpret_cast<int *>(p); p += r16(4 * (d.n_levels + 1));
+  s.ovf = reinterpret_cast<float4 *>(p); s.XR = s.ovf; p += step_ovf_bytes(Np, NIp);
+  s.lev = reinterpret_cast<int *>(p); p += r16(4 * (n_levels + 1));
   float *f = reinterpret_cast<float *>(p);
   s.u = f; s.v = f + 3 * Ap;
   s.att = p + 24 * Ap; s.cA = s.att + Ap; s.cB = s.cA + Ap;
@@ -269,7 +280,8 @@ __device__ __forceinline__ float mv_up(const Jt &j, float4 *P, const float4 *zer
 // ------------------------------------------------------------------------------------------------------
 
 // the views of the world every thread of the CTA shares (in shared memory, filled once per world)
-struct World { Sm s; Gm g; int N, nlev, ntop; };
+struct World { Gm g; int N, Np, Ap, NIp, nlev, ntop; };
+__device__ __forceinline__ Sm carve(const World *wd) { return carve(ob_smem, wd->Np, wd->Ap, wd->NIp, wd->nlev); }
 // PCG start vector from the last solutions: 0 = the last one, 1 = linear, 2 = quadratic, 3 = cubic extrapolation
 #ifndef OB_X0_ORDER
 #define OB_X0_ORDER 3
@@ -372,7 +384,7 @@ __device__ __forceinline__ void link_fk(const int i, const Sm &s) {
 // force those copies into local memory, and every pointer fetched from there is an L2 round trip.)
 __device__ __noinline__ Force6 external_forces(const int i, const float3 om, const float3 vl, const uint32_t tw,
                                                const World *wd, const DevCtx &c) {
-  const Sm s = wd->s;
+  const Sm s = carve(wd);
   const Gm g = wd->g;
   const ob_params &P = c.P;
   const int Np = s.Np, Ap = s.Ap;
@@ -623,7 +635,7 @@ __device__ __forceinline__ void link_inertia_lagged(const int i, const Sm &s, co
 #endif
 
 __device__ OB_COLD_ATTR void sweep_bias(const World *wd, const DevCtx &c, const int nt) {
-  const Sm s = wd->s;
+  const Sm s = carve(wd);
   const Gm g = wd->g;
   const int nlev = wd->nlev, ntop = wd->ntop, tid = threadIdx.x;
   const int l_first_down = tid < 32 ? 0 : ntop - 1, l_last_up = tid < 32 ? 0 : ntop;
@@ -663,7 +675,7 @@ __device__ OB_COLD_ATTR void sweep_bias(const World *wd, const DevCtx &c, const 
 
 __device__ OB_COLD_ATTR void sweep_inertia(const World *wd, const DevCtx &c, const int nt, const int otid,
                                            const bool refresh) {
-  const Sm s = wd->s;
+  const Sm s = carve(wd);
   const Gm g = wd->g;
   const int nlev = wd->nlev, ntop = wd->ntop, N = wd->N, tid = threadIdx.x;
   if (!refresh) {
@@ -699,7 +711,7 @@ constexpr int kPcgBad = 1 << 30;
 template <int NT, int LPT>
 __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *stage, int *flipp, const int otid,
                                       const bool top_warp, const float bb, const float bz, int *flags) {
-  const Sm s = wd->s;
+  const Sm s = carve(wd);
   const Gm g = wd->g;
   const ob_params &P = c.P;
   const int tid = threadIdx.x, lane = tid & 31;
@@ -937,7 +949,7 @@ template <int NT, int LPT, int MINB>
 __global__ void __launch_bounds__(NT, MINB)
 k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *queue, int n_steps,
        int top_rot) {
-  extern __shared__ __align__(128) unsigned char smem[];
+  unsigned char *const smem = ob_smem;
   __shared__ __align__(8) uint64_t s_bar;
   __shared__ int s_next;
   __shared__ World s_world;
@@ -969,7 +981,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
     WorldInfo *info = c.info + w;
     int status = info->status;
     if (status & OB_STATUS_NONFINITE) continue;      // frozen world
-    const Sm s = carve(smem, d);
+    const Sm s = carve(smem, d.Np, d.Ap, d.NIp, d.n_levels);
     const int Np = d.Np, S = Np + 1, N = d.N;
     const int nlev = d.n_levels, ntop = d.n_top;
     float4 *const PL = s.P;
@@ -992,7 +1004,10 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       g.arm = c.arm ? c.arm + 2 * (size_t)d.link_base : nullptr;
       g.topo2 = c.topo2 + d.link_base;
     }
-    if (tid == 0) { s_world.s = s; s_world.g = g; s_world.N = N; s_world.nlev = nlev; s_world.ntop = ntop; }
+    if (tid == 0) {
+      s_world.g = g; s_world.N = N; s_world.Np = Np; s_world.Ap = d.Ap; s_world.NIp = d.NIp; s_world.nlev = nlev;
+      s_world.ntop = ntop;
+    }
 
     // ---- stage the world: the apple block by one TMA bulk copy; topology words, level offsets, wrench slots ----
     if (tid == 0 && d.Ap) {
