@@ -158,7 +158,7 @@ inline int pad8(int n) { return (n + 7) / 8 * 8; }
 struct Layout {
   size_t total = 0;
   Pool desc, order, link_blk, apple_blk, topo, topo2, child_list, quat, quat_raw, R0, Mmax, mdiag, xprev, Lown, diam, arm, link_ext, apple_ext, apple_nom,
-      apple_c, anchor, level_off, info, wrench, events, ev_count, queue, pose7;
+      apple_c, anchor, level_off, info, wrench, events, ev_count, queue, progress, pose7;
   size_t sumNp = 0, sumAp = 0, sumLev = 0, ev_cap = 0;
   int max_Np = 0, max_Ap = 0, max_smem = 0;
   bool any_arm = false;
@@ -216,7 +216,7 @@ int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) 
   take(L, L.R0, sizeof(float) * 9 * L.sumNp);
   take(L, L.Mmax, sizeof(float) * L.sumNp);
   take(L, L.mdiag, sizeof(float2) * L.sumNp);
-  take(L, L.xprev, sizeof(float2) * 3 * L.sumNp);
+  take(L, L.xprev, sizeof(float2) * 4 * L.sumNp);
   take(L, L.Lown, sizeof(float) * L.sumNp);
   take(L, L.diam, sizeof(float) * L.sumNp);
   take(L, L.arm, L.any_arm ? sizeof(float) * 2 * L.sumNp : 0);
@@ -231,6 +231,7 @@ int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) 
   take(L, L.events, sizeof(ob_event) * L.ev_cap);
   take(L, L.ev_count, sizeof(int32_t) * 4);
   take(L, L.queue, sizeof(int32_t) * 2 * kNumClasses);
+  take(L, L.progress, sizeof(int32_t) * n_worlds);
   take(L, L.pose7, sizeof(float) * 7 * L.max_Np);
   L.total = (L.total + kAlign - 1) / kAlign * kAlign;
   return OB_OK;
@@ -483,6 +484,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   D.ev_cap = (int32_t)std::min<size_t>(L.ev_cap, 0x7fffffff);
   D.ev_count = reinterpret_cast<int32_t *>(base + L.ev_count.off);
   D.queue = reinterpret_cast<int32_t *>(base + L.queue.off);
+  D.progress = reinterpret_cast<int32_t *>(base + L.progress.off);
   D.pose7 = reinterpret_cast<float *>(base + L.pose7.off);
   D.P = *params;
 
@@ -611,11 +613,15 @@ int ob_step(ob_ctx *ctx, int n) {
   int rc = flush_wrenches(ctx);
   if (rc != OB_OK) return rc;
   CU(cudaMemsetAsync(ctx->dev.queue, 0, sizeof(int32_t) * kNumClasses, ctx->stream));
+  CU(cudaMemsetAsync(ctx->dev.progress, 0, sizeof(int32_t) * ctx->n_worlds, ctx->stream));
+  // queue items of about ten steps: short enough that the tail of the launch (CTAs out of work) stays small, long
+  // enough that staging a world is amortised
+  const int n_chunks = std::max(1, std::min(8, (n + 9) / 10));
   ctx->launches = 0;
   for (int k = kNumClasses - 1; k >= 0; k--) {      // the class of the largest worlds first
     if (!ctx->cls_n[k]) continue;
     CU(launch_step(ctx->dev, k, ctx->dev.order + ctx->cls_off[k], ctx->cls_n[k], ctx->dev.queue + k, n,
-                   ctx->cls_grid[k], ctx->cls_smem[k], ctx->n_sm, ctx->stream));
+                   ctx->cls_grid[k], ctx->cls_smem[k], ctx->n_sm, n_chunks, ctx->dev.progress, ctx->stream));
     ctx->launches += 1;
     ctx->kernel_launches += 1;
   }

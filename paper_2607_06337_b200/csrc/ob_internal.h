@@ -82,7 +82,7 @@ struct DevCtx {
   float *R0;                     // [9 * link_base + k * Np + i] rest world rotation, row-major k
   float *Mmax;                   // rupture moment (after randomize)
   float2 *mdiag;                 // [link_base + i] diag(M) of the two DoF as last computed by phase B2
-  float2 *xprev;                 // [2][sumNp]: dqd of the two steps before the last (PCG start: extrapolation)
+  float2 *xprev;                 // [4][sumNp]: dqd of the last four steps, slot = step & 3 (PCG start: extrapolation)
   int32_t sum_np;                // stride of xprev
   const float *Lown;             // link length
   const float *diam;             // link diameter
@@ -99,6 +99,7 @@ struct DevCtx {
   int32_t ev_cap;
   int32_t *ev_count;             // [0] = appended, [1] = overflow flag
   int32_t *queue;                // work-queue counters, one per size class
+  int32_t *progress;             // [n_worlds] chunks of the current launch a world has finished
   float *pose7;                  // scratch for ob_get_state(link_pose7): 7 * max Np floats
   ob_params P;
 };
@@ -154,7 +155,7 @@ __host__ __device__ inline int step_smem_bytes(int Np, int Ap, int NIp, int nlev
 cudaError_t launch_rest_pose(const DevCtx &c, int total_links_padded, int total_apples_padded, cudaStream_t s);
 cudaError_t launch_randomize(const DevCtx &c, unsigned long long seed, int redraw, cudaStream_t s);
 cudaError_t launch_step(const DevCtx &c, int cls, const int32_t *order, int n_in_class, int32_t *queue, int n_steps,
-                        int grid, int smem, int n_sm, cudaStream_t s);
+                        int grid, int smem, int n_sm, int n_chunks, int32_t *progress, cudaStream_t s);
 cudaError_t launch_pose(const DevCtx &c, int world, cudaStream_t s);
 cudaError_t step_kernel_setup(int cls, int smem_bytes, int *max_blocks_per_sm);
 

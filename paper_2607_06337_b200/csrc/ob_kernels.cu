@@ -110,6 +110,7 @@ __global__ void k_randomize(DevCtx c, unsigned long long seed, int redraw) {
     c.xprev[d.link_base + i] = make_float2(0.f, 0.f);              // PCG start-vector history
     c.xprev[c.sum_np + d.link_base + i] = make_float2(0.f, 0.f);
     c.xprev[2 * c.sum_np + d.link_base + i] = make_float2(0.f, 0.f);
+    c.xprev[3 * c.sum_np + d.link_base + i] = make_float2(0.f, 0.f);
     if (i < d.N) {
       double dd = diam[i], L = Lown[i], r = 0.5 * dd;
       double K = (double)E * PI * dd * dd * dd * dd / (64.0 * L);   // Eq. 4

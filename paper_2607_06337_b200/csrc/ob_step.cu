@@ -110,7 +110,7 @@ struct Gm {
   const float *R0;                  // [k * Np + i]
   const float *Mmax;
   float2 *mdiag;                    // diag(M) as last computed by phase B2 (the Jacobi preconditioner may lag)
-  float2 *xprev, *xprev2, *xprev3;  // dqd of the three steps before the last
+  float2 *hist;                     // [4][sum_np]: dqd of the last four steps, slot = step & 3
   const float *arm;                 // [k * Np + i] or nullptr
   const int4 *topo2;                // x = first apple | n_apples << 16, y = inner slot | parent's inner slot << 16
 };
@@ -307,7 +307,7 @@ __device__ __forceinline__ double join2(const float hi, const float lo) { return
 __device__ __forceinline__ void link_prepare(const int i, const Sm &s, const Gm &g, const DevCtx &c) {
   const ob_params &P = c.P;
   const int Np = s.Np;
-  const float2 th = g.q2[i], w = g.w2[i];
+  const float2 th = __ldcg(g.q2 + i), w = __ldcg(g.w2 + i);
   const float4 qt = __ldg(g.quat + i);
   const float Ki = __ldg(g.K + i);
   const float rz = (s.T[i] & kTrunk) ? 0.f : __ldg(g.rz + i);
@@ -467,7 +467,7 @@ __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm
   const ob_params &P = c.P;
   const int NIp = s.NIp;
   const uint32_t tw = s.T[i];
-  const float2 w = g.w2[i];
+  const float2 w = __ldcg(g.w2 + i);
   const float4 c4 = __ldg(g.c4 + i);
   const int ty = __ldg(&g.topo2[i].y);                            // inner slot | parent's inner slot << 16
   const Jt j = load_jt(s.P, i);
@@ -600,7 +600,7 @@ __device__ __forceinline__ void link_inertia_lagged(const int i, const Sm &s, co
   const int Ap = s.Ap;
   uint32_t tw = s.T[i];
   float4 eff = __ldg(g.c4 + i);
-  const float2 md = g.mdiag[i];
+  const float2 md = __ldcg(g.mdiag + i);
   if (P.tether_implicit && (tw & kHasApples)) {
     tw &= ~kOffax;
     const int4 t2 = __ldg(g.topo2 + i);
@@ -948,7 +948,7 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
 template <int NT, int LPT, int MINB>
 __global__ void __launch_bounds__(NT, MINB)
 k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int n_in_class, int32_t *queue, int n_steps,
-       int top_rot) {
+       int top_rot, int n_chunks, int32_t *progress) {
   unsigned char *const smem = ob_smem;
   __shared__ __align__(8) uint64_t s_bar;
   __shared__ int s_next;
@@ -975,12 +975,28 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
     __syncthreads();
     const int qi = s_next;
     __syncthreads();
-    if (qi >= n_in_class) break;
-    const int w = order[qi];
+    if (qi >= n_in_class * n_chunks) break;
+    // The n steps of a launch are cut into n_chunks queue items per world (all first chunks, then all second ones,
+    // ...): the tail of the launch, where CTAs run out of work, is a fraction of a chunk instead of a fraction of
+    // the whole launch.  A later chunk of a world waits until the earlier one (taken by a resident CTA before,
+    // the queue is in order) has published its state; all state crosses in global memory (L2: __ldcg loads).
+    const int chunk = qi / n_in_class;
+    const int w = order[qi - chunk * n_in_class];
+    const int n_my = (int)(((long long)n_steps * (chunk + 1)) / n_chunks - ((long long)n_steps * chunk) / n_chunks);
+    if (chunk > 0) {
+      if (tid == 0) {
+        while (*reinterpret_cast<volatile int32_t *>(progress + w) < chunk) __nanosleep(200);
+        __threadfence();
+      }
+      __syncthreads();
+    }
     const WorldDesc d = c.desc[w];
     WorldInfo *info = c.info + w;
-    int status = info->status;
-    if (status & OB_STATUS_NONFINITE) continue;      // frozen world
+    int status = __ldcg(&info->status);
+    if ((status & OB_STATUS_NONFINITE) || n_my == 0) {      // frozen world (or nothing to do): pass the baton
+      if (tid == 0) { __threadfence(); atomicExch(progress + w, chunk + 1); }
+      continue;
+    }
     const Sm s = carve(smem, d.Np, d.Ap, d.NIp, d.n_levels);
     const int Np = d.Np, S = Np + 1, N = d.N;
     const int nlev = d.n_levels, ntop = d.n_top;
@@ -998,9 +1014,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       g.R0 = c.R0 + 9 * (size_t)d.link_base;
       g.Mmax = c.Mmax + d.link_base;
       g.mdiag = c.mdiag + d.link_base;
-      g.xprev = c.xprev + d.link_base;
-      g.xprev2 = c.xprev + c.sum_np + d.link_base;
-      g.xprev3 = c.xprev + 2 * c.sum_np + d.link_base;
+      g.hist = c.xprev + d.link_base;
       g.arm = c.arm ? c.arm + 2 * (size_t)d.link_base : nullptr;
       g.topo2 = c.topo2 + d.link_base;
     }
@@ -1029,7 +1043,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
           const int4 t2 = __ldg(g.topo2 + i);
           const uint32_t nc = (uint32_t)t2.w, fc = nc ? ((uint32_t)tp.y & 0xffffu) : 0u;
           tw = (tp.x >= 0 ? (uint32_t)tp.x : ((uint32_t)Np | kTrunk)) | (fc << kChShift) | (nc << kNcShift) |
-               ((t2.x >> 16) ? kHasApples : 0u) | (g.rupt[i] ? kRuptured : 0u);
+               ((t2.x >> 16) ? kHasApples : 0u) | (__ldcg(g.rupt + i) ? kRuptured : 0u);
         }
         s.T[i] = tw;
       }
@@ -1050,15 +1064,19 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
     }
     __syncthreads();
 
-    int step0 = info->step, steps_done = 0, last_iters = 0, diag_age = info->diag_age;
+    int step0 = __ldcg(&info->step), steps_done = 0, last_iters = 0, diag_age = __ldcg(&info->diag_age);
     unsigned long long iters_total = 0;
-    for (int sidx = 0; sidx < n_steps; sidx++) {
+    for (int sidx = 0; sidx < n_my; sidx++) {
       sweep_bias(&s_world, c, NT);                      // A, B1
 #pragma unroll
       for (int k = 0; k < LPT; k++) {
         const int i = otid + k * NT;
         if (i < N) {                                    // r = b; x = previous dqd (warm start), kept in global memory
-          const float2 b = s.G[i], x1 = g.x2[i], x2 = g.xprev[i], x3 = g.xprev2[i], x4 = g.xprev3[i];
+          const int t = step0 + sidx;                   // solutions of steps t-1 .. t-4 out of the ring of four
+          const float2 b = s.G[i], x1 = __ldcg(g.hist + ((t - 1) & 3) * (size_t)c.sum_np + i),
+                       x2 = __ldcg(g.hist + ((t - 2) & 3) * (size_t)c.sum_np + i),
+                       x3 = __ldcg(g.hist + ((t - 3) & 3) * (size_t)c.sum_np + i),
+                       x4 = __ldcg(g.hist + (t & 3) * (size_t)c.sum_np + i);
           XR[i] = make_float4(OB_X0(x1.x, x2.x, x3.x, x4.x), OB_X0(x1.y, x2.y, x3.y, x4.y), b.x, b.y);
         }
       }
@@ -1100,12 +1118,9 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       for (int k = 0; k < LPT; k++) {
         const int i = otid + k * NT;
         if (i >= N) continue;
-        const float2 w0 = g.w2[i], q0 = g.q2[i];
+        const float2 w0 = __ldcg(g.w2 + i), q0 = __ldcg(g.q2 + i);
         const float2 x = *reinterpret_cast<const float2 *>(XR + i);
-        g.xprev3[i] = g.xprev2[i];
-        g.xprev2[i] = g.xprev[i];
-        g.xprev[i] = g.x2[i];
-        g.x2[i] = x;
+        g.hist[(step_now & 3) * (size_t)c.sum_np + i] = x;
         float wa = w0.x + x.x, wb = w0.y + x.y;
         if (P.qd_max > 0.f) {
           wa = fminf(fmaxf(wa, -P.qd_max), P.qd_max);
@@ -1117,7 +1132,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         if (!(tw & kRuptured)) {
           const float Ki = __ldg(g.K + i), Mx = __ldg(g.Mmax + i);
           const float mu = Ki * sqrtf(qa * qa + qb * qb);                   // Eq. 5
-          const int rc0 = g.rc[i];
+          const int rc0 = __ldcg(g.rc + i);
           const int rcn = mu > Mx ? rc0 + 1 : 0;
           if (rcn >= P.rupture_frames) {
             g.rupt[i] = 1; g.rc[i] = 0;
@@ -1168,7 +1183,8 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
 #pragma unroll
       for (int k = 0; k < LPT; k++) {
         const int i = otid + k * NT;
-        if (i < N) { g.x2[i] = make_float2(0.f, 0.f); g.xprev[i] = make_float2(0.f, 0.f); g.xprev2[i] = make_float2(0.f, 0.f); g.xprev3[i] = make_float2(0.f, 0.f); }
+        if (i < N)
+          for (int q = 0; q < 4; q++) g.hist[q * (size_t)c.sum_np + i] = make_float2(0.f, 0.f);
       }
     }
     fence_proxy_async();
@@ -1182,10 +1198,11 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       info->last_iters = last_iters;
       info->status = status;
       info->diag_age = diag_age;
-      info->steps_taken += steps_done;
-      info->cg_iters += iters_total;
+      info->steps_taken = __ldcg(&info->steps_taken) + steps_done;
+      info->cg_iters = __ldcg(&info->cg_iters) + iters_total;
     }
-    __syncthreads();
+    __syncthreads();                                 // every thread's global writes of this chunk are done
+    if (tid == 0) { __threadfence(); atomicExch(progress + w, chunk + 1); }
   }
 }
 
@@ -1214,9 +1231,10 @@ cudaError_t step_kernel_setup(int cls, int smem_bytes, int *max_blocks_per_sm) {
 }
 
 cudaError_t launch_step(const DevCtx &c, int cls, const int32_t *order, int n_in_class, int32_t *queue, int n_steps,
-                        int grid, int smem, int n_sm, cudaStream_t s) {
-#define OB_LAUNCH(NT, LPT, MINB) \
-  k_step<NT, LPT, MINB><<<grid, NT, smem, s>>>(c, order, n_in_class, queue, n_steps, n_sm > 0 ? n_sm : 1);
+                        int grid, int smem, int n_sm, int n_chunks, int32_t *progress, cudaStream_t s) {
+#define OB_LAUNCH(NT, LPT, MINB)                                                                                   \
+  k_step<NT, LPT, MINB><<<grid, NT, smem, s>>>(c, order, n_in_class, queue, n_steps, n_sm > 0 ? n_sm : 1, n_chunks, \
+                                               progress);
   OB_FOR_CLASS(cls, OB_LAUNCH)
 #undef OB_LAUNCH
   return cudaGetLastError();
