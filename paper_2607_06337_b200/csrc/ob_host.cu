@@ -712,6 +712,8 @@ int ob_set_state(ob_ctx *ctx, int world, const float *q, const float *qd, const 
   }
   wi.status = 0;
   wi.diag_age = 0;          // the state was written from outside: recompute the preconditioner at the next step
+  for (int k = 0; k < 4; k++)   // ... and forget the solution history the PCG start vector is extrapolated from
+    CU(cudaMemsetAsync(ctx->dev.xprev + (size_t)k * ctx->dev.sum_np + d.link_base, 0, sizeof(float2) * d.Np, ctx->stream));
   CU(cpy(ctx, ctx->dev.link_blk + d.link_blk_off, lb.data(), lb.size(), cudaMemcpyHostToDevice, ctx->stream));
   if (d.Ap)
     CU(cpy(ctx, ctx->dev.apple_blk + d.apple_blk_off, ab.data(), apple_state_bytes(d.Ap), cudaMemcpyHostToDevice,
