@@ -262,7 +262,7 @@ def run_cuda(args, rank: int, world_size: int):
             "warmup": args.warmup, "ms_per_step": region_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {W} worlds x "
-                                   f"{links_per_world:.0f} links (350-450), {apples_per_world:.0f} apples, h = {P.h * 1e3:g} ms, "
+                                   f"{links_per_world:.0f} links ({min(x.n_links for x in specs)}-{max(x.n_links for x in specs)}), {apples_per_world:.0f} apples, h = {P.h * 1e3:g} ms, "
                                    f"wrench U({f_lo:g},{f_hi:g}) N per world resampled every {S} steps",
                        "worlds_per_gpu": W, "physics_steps_per_bench_step": S, "links_total": n_links,
                        "apples_total": n_apples, "cg_tol": P.cg_tol, "replicas": world_size,

@@ -271,12 +271,19 @@ class Orchard:
         self._check(self._L.ob_get_material(self._h, world, _ptr(emr), _ptr(det), _ptr(mass)))
         return dict(E=emr[0], MOR=emr[1], density=emr[2], detach=det, mass=mass)
 
+    _EV_DTYPE = np.dtype([("world", np.int32), ("step", np.int32), ("kind", np.int32), ("index", np.int32),
+                          ("value", np.float32), ("threshold", np.float32)])
+
     def events(self, cap: Optional[int] = None) -> List[tuple]:
+        """Drain the device event list: (world, step, kind, index, value, threshold), sorted by the library."""
         cap = cap if cap is not None else sum(self.n_links) + sum(self.n_apples) + 64
-        buf = (ob_event * max(cap, 1))()
+        cap = max(cap, 1)
+        buf = getattr(self, "_ev_buf", None)
+        if buf is None or len(buf) < cap:                  # one reusable host buffer (argument marshalling only)
+            buf = self._ev_buf = (ob_event * cap)()
         n = C.c_int(0)
         rc = self._L.ob_events(self._h, buf, cap, C.byref(n))
-        out = [(e.world, e.step, e.kind, e.index, e.value, e.threshold) for e in buf[:n.value]]
+        out = np.frombuffer(buf, dtype=self._EV_DTYPE, count=n.value).tolist()
         self._check(rc)
         return out
 

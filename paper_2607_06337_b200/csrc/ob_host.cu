@@ -16,7 +16,7 @@ using namespace ob;
 namespace {
 
 constexpr size_t kAlign = 256;
-constexpr int kMaxSmem = 227 * 1024 - 2048;   // per-CTA limit minus the kernel's static shared memory
+constexpr int kMaxSmem = 227 * 1024 - 1024;   // per-CTA limit minus the kernel's static shared memory (896 B)
 const char *kNullCtx = "null context";
 
 struct Pool {

@@ -67,7 +67,7 @@ struct Sm {
   float *u, *v;                       // [3][Ap]
   unsigned char *att, *cA, *cB;
   float *ao, *ak, *am, *ac, *afd;     // ao = [3][Ap]
-  float *ft, *fu, *fsn, *fun;         // tether force [3][Ap], user force [3][Ap], |f_s|, |f_user|
+  float *ft, *fsn;                    // tether force [3][Ap], |f_s| [Ap] (phase A2 -> phase D)
   WrenchSlots *wr;
 };
 
@@ -93,9 +93,7 @@ __device__ __forceinline__ Sm carve(unsigned char *base, const int Np, const int
   p += r16(apple_block_bytes(Ap));
   f = reinterpret_cast<float *>(p);
   s.ft = f; f += 3 * Ap;
-  s.fu = f; f += 3 * Ap;
   s.fsn = f; f += Ap;
-  s.fun = f; f += Ap;
   s.wr = reinterpret_cast<WrenchSlots *>(f);
   return s;
 }
@@ -1054,16 +1052,6 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       parity ^= 1;
     }
     __syncthreads();
-    // user forces on apples are constant over the launch
-    for (int a = tid; a < d.A; a += NT) {
-      float3 fu = f3(0, 0, 0);
-      for (int k = 0; k < s.wr->n; k++)
-        if (s.wr->body[k] == N + a) fu = fu + f3(s.wr->force[k][0], s.wr->force[k][1], s.wr->force[k][2]);
-      s.fu[a] = fu.x; s.fu[d.Ap + a] = fu.y; s.fu[2 * d.Ap + a] = fu.z;
-      s.fun[a] = sqrtf(dot(fu, fu));
-    }
-    __syncthreads();
-
     int step0 = __ldcg(&info->step), steps_done = 0, last_iters = 0, diag_age = __ldcg(&info->diag_age);
     unsigned long long iters_total = 0;
     for (int sidx = 0; sidx < n_my; sidx++) {
@@ -1149,7 +1137,9 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         const float ma = s.am[a], inv_m = 1.f / ma;
         const float fdet = s.afd[a];
         float3 ft = att ? f3(s.ft[a], s.ft[Ap + a], s.ft[2 * Ap + a]) : f3(0, 0, 0);
-        const float3 fu = f3(s.fu[a], s.fu[Ap + a], s.fu[2 * Ap + a]);
+        float3 fu = f3(0, 0, 0);                                            // user force on the apple (wrench slots)
+        for (int k = 0; k < s.wr->n; k++)
+          if (s.wr->body[k] == N + a) fu = fu + f3(s.wr->force[k][0], s.wr->force[k][1], s.wr->force[k][2]);
         float3 va = f3(s.v[a], s.v[Ap + a], s.v[2 * Ap + a]);
         va.x += P.h * (P.gravity[0] + (ft.x + fu.x) * inv_m);
         va.y += P.h * (P.gravity[1] + (ft.y + fu.y) * inv_m);
@@ -1158,7 +1148,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         s.u[a] = fmaf(P.h, va.x, s.u[a]); s.u[Ap + a] = fmaf(P.h, va.y, s.u[Ap + a]);
         s.u[2 * Ap + a] = fmaf(P.h, va.z, s.u[2 * Ap + a]);
         if (att) {
-          const float fun = s.fun[a], fsn = s.fsn[a], thrB = P.detach_kappa * fdet;
+          const float fun = sqrtf(dot(fu, fu)), fsn = s.fsn[a], thrB = P.detach_kappa * fdet;
           const int ca = fun > fdet ? s.cA[a] + 1 : 0;
           const int cb = fsn > thrB ? s.cB[a] + 1 : 0;
           if (ca >= P.detach_frames_pull) {
