@@ -96,6 +96,9 @@ typedef struct {
   float range_density[2];
   float range_detach[2];        /* per apple */
   float range_apple_mass[2];    /* per apple */
+  float mass_damping;           /* {0} 1/s >= 0: velocity-proportional damping F = -c_v m v, tau = -c_omega I omega on
+                                   every link and apple with c_v = c_omega = mass_damping; in joint
+                                   space -mass_damping M(q) qd, taken linearly implicit like the joint damper */
 } ob_params;
 
 typedef struct {

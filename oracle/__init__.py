@@ -34,7 +34,7 @@ class OboParams(C.Structure):
         ("cg_max_iter", C.c_int32), ("solver", C.c_int32), ("rupture_frames", C.c_int32),
         ("detach_frames_pull", C.c_int32), ("detach_kappa", C.c_double),
         ("detach_frames_tension", C.c_int32), ("tether_implicit", C.c_int32),
-        ("react_max", C.c_double), ("qd_max", C.c_double), ("zeta_s", C.c_double),
+        ("react_max", C.c_double), ("qd_max", C.c_double), ("zeta_s", C.c_double), ("alpha_m", C.c_double),
         ("forces_off_on_snapped", C.c_int32), ("pad_", C.c_int32),
         ("range_E", C.c_float * 2), ("range_MOR", C.c_float * 2), ("range_density", C.c_float * 2),
         ("range_detach", C.c_float * 2), ("range_apple_mass", C.c_float * 2),
@@ -114,6 +114,7 @@ def _params_struct(p, solver: int = 0) -> OboParams:
     s.react_max = float(np.float32(p.react_max))
     s.qd_max = float(np.float32(p.qd_max))
     s.zeta_s = float(np.float32(p.zeta_s))
+    s.alpha_m = float(np.float32(getattr(p, "mass_damping", 0.0)))
     s.forces_off_on_snapped = p.forces_off_on_snapped
     s.h = float(np.float32(p.h))
     for name in ("range_E", "range_MOR", "range_density", "range_detach", "range_apple_mass"):

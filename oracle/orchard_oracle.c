@@ -57,6 +57,7 @@ typedef struct {
   double react_max;
   double qd_max;
   double zeta_s;
+  double alpha_m;               /* mass- and inertia-proportional damping c_v = c_omega, 1/s (A32) */
   int32_t forces_off_on_snapped;
   int32_t pad_;
   float range_E[2], range_MOR[2], range_density[2], range_detach[2], range_apple_mass[2];
@@ -686,6 +687,19 @@ static void build_system(const obo_world *W, system_t *S) {
   }
   /* 5. A = M + eta M_teth + diag(arm + h D + h^2 K) */
   mass_matrix(W, W->q, S->A);
+  /* Velocity-proportional damping F = -c_v m v, tau = -c_omega I omega on every link, reading A32:
+     c_v = c_omega = alpha_m.  The generalized force of these body forces is -alpha sum_i J_i^T I_i J_i qd =
+     -alpha M(q) qd (M = sum J^T I J, the identity pin P2 checks).  Taken at the end-of-step velocity qd + dqd
+     (linearly implicit, like the joint damper):  M dqd = h [ ... - alpha M (qd + dqd) ]  ->
+     A gets (1 + h alpha) M, b gets - h alpha M qd. */
+  if (P->alpha_m != 0.0) {
+    for (int r_ = 0; r_ < n; r_++) {
+      double mq = 0.0;
+      for (int c_ = 0; c_ < n; c_++) mq += S->A[(size_t)r_ * n + c_] * W->qd[c_];
+      S->b[r_] -= h * P->alpha_m * mq;
+    }
+    for (size_t k = 0; k < (size_t)n * n; k++) S->A[k] *= 1.0 + h * P->alpha_m;
+  }
   for (int i = 0; i < N; i++) {
     double Kt = W->ruptured[i] ? 0.0 : W->K[i], Dt = P->c_d * Kt;
     for (int k = 0; k < 2; k++) {
@@ -760,7 +774,8 @@ static void step_once(obo_world *W) {
   for (int a = 0; a < A; a++) {
     double att = W->attached[a] ? 1.0 : 0.0;
     for (int k = 0; k < 3; k++) {
-      double acc = P->g[k] + (att * S.fteth[3 * a + k] + S.fuser[3 * a + k]) / W->am[a];
+      /* the apple is a body too: F = -c_v m v, explicit at the start-of-step velocity */
+      double acc = P->g[k] + (att * S.fteth[3 * a + k] + S.fuser[3 * a + k]) / W->am[a] - P->alpha_m * W->av[3 * a + k];
       W->av[3 * a + k] += h * acc;
       W->ax[3 * a + k] += h * W->av[3 * a + k];
     }

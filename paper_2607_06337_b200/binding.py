@@ -44,7 +44,7 @@ class ob_params(C.Structure):
         ("react_max", C.c_float), ("tether_implicit", C.c_int32), ("qd_max", C.c_float), ("zeta_s", C.c_float),
         ("forces_off_on_snapped", C.c_int32),
         ("range_E", C.c_float * 2), ("range_MOR", C.c_float * 2), ("range_density", C.c_float * 2),
-        ("range_detach", C.c_float * 2), ("range_apple_mass", C.c_float * 2),
+        ("range_detach", C.c_float * 2), ("range_apple_mass", C.c_float * 2), ("mass_damping", C.c_float),
     ]
 
 
@@ -120,7 +120,7 @@ def params_struct(p) -> ob_params:
     s.gravity = (C.c_float * 3)(*p.gravity)
     for name in ("c_d", "cg_tol", "cg_max_iter", "precond", "cg_norm", "rupture_frames", "detach_frames_pull", "detach_kappa",
                  "detach_frames_tension", "react_max", "tether_implicit", "qd_max", "zeta_s",
-                 "forces_off_on_snapped"):
+                 "forces_off_on_snapped", "mass_damping"):
         setattr(s, name, getattr(p, name))
     for name in ("range_E", "range_MOR", "range_density", "range_detach", "range_apple_mass"):
         setattr(s, name, (C.c_float * 2)(*getattr(p, name)))

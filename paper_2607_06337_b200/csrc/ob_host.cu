@@ -84,7 +84,7 @@ int validate(const ob_world_spec *specs, int n_worlds, const ob_params *P, std::
   if (!specs || !P || n_worlds < 1) { why = "null specs/params or n_worlds < 1"; return OB_E_ARG; }
   if (!(P->h > 0.f) || !(P->cg_tol > 0.f) || P->cg_max_iter < 1 || P->rupture_frames < 1 || P->rupture_frames > 255 ||
       P->detach_frames_pull < 1 || P->detach_frames_pull > 255 || P->detach_frames_tension < 1 ||
-      P->detach_frames_tension > 255 || !(P->react_max >= 0.f) || !(P->c_d >= 0.f) || P->precond < 0 || P->precond > 1 || P->cg_norm < 0 || P->cg_norm > 1) {
+      P->detach_frames_tension > 255 || !(P->react_max >= 0.f) || !(P->c_d >= 0.f) || !(P->mass_damping >= 0.f) || P->precond < 0 || P->precond > 1 || P->cg_norm < 0 || P->cg_norm > 1) {
     why = "ob_params out of range";
     return OB_E_ARG;
   }
@@ -303,6 +303,7 @@ int ob_default_params(ob_params *p) {
   p->qd_max = 50.f;
   p->zeta_s = 0.1f;
   p->forces_off_on_snapped = 1;
+  p->mass_damping = 0.f;
   return OB_OK;
 }
 

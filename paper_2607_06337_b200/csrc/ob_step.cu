@@ -482,7 +482,9 @@ __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm
   const float3 om = mul(j.E, wp) + vJ;
   const float3 vl = mul(j.E, f3(vp.x + wp.y * rz, vp.y - wp.x * rz, vp.z));
   const float ww = w.x * w.y;
-  const float3 al = mul(j.E, alp) + f3(-s2 * ww, 0.f, c2 * ww) + cross(om, vJ);
+  // mass-proportional damping (A32): its generalized force -alpha M qd enters the bias pass as the
+  // joint acceleration alpha qd, i.e. alpha S qd = alpha vJ on top of the velocity-product terms
+  const float3 al = mul(j.E, alp) + f3(-s2 * ww, 0.f, c2 * ww) + cross(om, vJ) + P.mass_damping * vJ;
   const float3 aln = mul(j.E, f3(ap.x + alp.y * rz, ap.y - alp.x * rz, ap.z)) + cross(vl, vJ);
   const bool inner = ((tw >> kNcShift) & kNcMask) != 0u;
   if (inner) {
@@ -531,7 +533,11 @@ __device__ __forceinline__ void up_inertia(const int i, const Sm &s, const Gm &g
   const int S = s.S, Ap = s.Ap;
   const ob_params &P = c.P;
   uint32_t tw = s.T[i];
-  const float4 c4 = __ldg(g.c4 + i);
+  float4 c4 = __ldg(g.c4 + i);
+  {                                  // mass-proportional damping, implicit: the operator carries (1 + h alpha) M
+    const float sc = 1.f + P.h * P.mass_damping;
+    c4.x *= sc; c4.y *= sc; c4.z *= sc; c4.w *= sc;
+  }
   float cm = c4.x;
   float3 ch3 = f3(0.f, 0.f, c4.y);
   float Ixx = c4.z, Iyy = c4.z, Izz = c4.w, Ixy = 0.f, Ixz = 0.f, Iyz = 0.f;
@@ -598,6 +604,10 @@ __device__ __forceinline__ void link_inertia_lagged(const int i, const Sm &s, co
   const int Ap = s.Ap;
   uint32_t tw = s.T[i];
   float4 eff = __ldg(g.c4 + i);
+  {
+    const float sc = 1.f + P.h * P.mass_damping;
+    eff.x *= sc; eff.y *= sc; eff.z *= sc; eff.w *= sc;
+  }
   const float2 md = __ldcg(g.mdiag + i);
   if (P.tether_implicit && (tw & kHasApples)) {
     tw &= ~kOffax;
@@ -1141,9 +1151,10 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         for (int k = 0; k < s.wr->n; k++)
           if (s.wr->body[k] == N + a) fu = fu + f3(s.wr->force[k][0], s.wr->force[k][1], s.wr->force[k][2]);
         float3 va = f3(s.v[a], s.v[Ap + a], s.v[2 * Ap + a]);
-        va.x += P.h * (P.gravity[0] + (ft.x + fu.x) * inv_m);
-        va.y += P.h * (P.gravity[1] + (ft.y + fu.y) * inv_m);
-        va.z += P.h * (P.gravity[2] + (ft.z + fu.z) * inv_m);
+        const float3 v0 = va;                                               // F = -c_v m v on the apple
+        va.x += P.h * (P.gravity[0] + (ft.x + fu.x) * inv_m - P.mass_damping * v0.x);
+        va.y += P.h * (P.gravity[1] + (ft.y + fu.y) * inv_m - P.mass_damping * v0.y);
+        va.z += P.h * (P.gravity[2] + (ft.z + fu.z) * inv_m - P.mass_damping * v0.z);
         s.v[a] = va.x; s.v[Ap + a] = va.y; s.v[2 * Ap + a] = va.z;
         s.u[a] = fmaf(P.h, va.x, s.u[a]); s.u[Ap + a] = fmaf(P.h, va.y, s.u[Ap + a]);
         s.u[2 * Ap + a] = fmaf(P.h, va.z, s.u[2 * Ap + a]);

@@ -36,7 +36,7 @@ def test_library_exports_every_declared_symbol():
 def test_struct_layouts_match_the_header():
     # ob_event: 4 x int32 + 2 x float; ob_params: counted from the header's field list
     assert C.sizeof(ob.ob_event) == 24
-    assert C.sizeof(ob.ob_params) == 4 * (1 + 3 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 10)
+    assert C.sizeof(ob.ob_params) == 4 * (1 + 3 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 10 + 1)
     assert C.sizeof(ob.ob_world_spec) == 8 * 15 if C.sizeof(C.c_void_p) == 8 else True
     L = ob.load_library()
     assert L.ob_sizeof_params() == C.sizeof(ob.ob_params)
@@ -50,7 +50,7 @@ def test_default_params_are_the_documented_readings():
     assert abs(p.c_d - 0.05) < 1e-8 and abs(p.cg_tol - 1e-6) < 1e-12 and p.cg_max_iter == 200 and p.precond == 1
     assert p.rupture_frames == 3 and p.detach_frames_pull == 3 and p.detach_frames_tension == 10
     assert abs(p.detach_kappa - 1.1) < 1e-6 and p.react_max == 40.0 and p.tether_implicit == 1
-    assert p.qd_max == 50.0 and abs(p.zeta_s - 0.1) < 1e-7 and p.forces_off_on_snapped == 1
+    assert p.qd_max == 50.0 and abs(p.zeta_s - 0.1) < 1e-7 and p.forces_off_on_snapped == 1 and p.mass_damping == 0.0
     assert ob.load_library().ob_default_params(None) == ob.OB_E_ARG
 
 

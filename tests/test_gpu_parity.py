@@ -191,6 +191,32 @@ def test_single_step_explicit_tether_and_no_preconditioner():
         sim.close()
 
 
+def test_single_step_and_free_run_with_mass_proportional_damping():
+    """SURVEY.md 8(f) item 2 / reading A32: F = -c_v m v, tau = -c_omega I omega with
+    c_v = c_omega = mass_damping, implicit in the joints ((1 + h a) M in the operator, a qd as joint acceleration of
+    the bias pass), explicit on the apples: single steps and a 200-step free run against the oracle."""
+    specs = list(_stochastic(131, 150, 250, 20, 3))
+    P = dataclasses.replace(config_params(2), mass_damping=1.5)
+    sim, refs = _make(specs, P, seed=MASTER_SEED + 77)
+    for epoch in range(2):
+        _apply(sim, refs, wrench_process(specs, epoch, 0.0, 60.0))
+        sim.step(20)
+        for w, e in _single_step_errors(sim, refs, range(len(specs))).items():
+            assert e["max"] <= TOL_STEP, (epoch, w, e)
+        sim.step(9)
+    sim.close()
+    spec = binary_tree_config1()
+    P1 = dataclasses.replace(config_params(1), mass_damping=1.5)
+    sim, refs = _make([spec], P1)
+    for s_ in range(200):
+        _apply(sim, refs, config1_loads(spec, s_, 500, 30.0, 400.0))
+        sim.step(1)
+        refs[0].step(1)
+    e, g, o = _err(sim, refs[0], 0)
+    assert e["max"] <= TOL_RUN, e
+    sim.close()
+
+
 # ----------------------------------------------------------------------------------------------------
 # 200-step trajectories without events: relative state error <= 1e-3 (north_star)
 # ----------------------------------------------------------------------------------------------------

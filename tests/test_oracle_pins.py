@@ -622,3 +622,67 @@ def test_state_round_trip_reproduces_the_run_after_a_rupture():
     c.apply_wrench(spec.n_links + 0, (0, 0, 0), config1_loads(spec, 460, 500, 30.0, 5000.0)[0][3])
     c.step(20)
     assert np.abs(c.get_state()["q"] - sb["q"]).max() < 1e-12
+
+
+# ---------------------------------------------------------------- A32: mass-proportional damping
+def test_mass_damping_single_dof_step_map_closed_form():
+    """(J (1 + h a) + h D + h^2 K) dv = h [-K q - (D + h K) v - a J v]: the 1-DoF step map with F = -c_v m v,
+    tau = -c_omega I omega (c_v = c_omega = a) taken implicitly, written out by hand."""
+    L, d, rho, E = 0.6, 0.02, 800.0, 1e8
+    spec = chain_spec(1, L, d, density=rho, E=E)
+    h, c_d, a = 2e-3, 0.05, 3.0
+    w = OracleWorld(spec, Params(h=h, gravity=(0, 0, 0), c_d=c_d, qd_max=0.0, mass_damping=a))
+    hh, cd = float(np.float32(h)), float(np.float32(c_d))
+    r, Lf = float(spec.diameter[0]) / 2, float(spec.length[0])
+    m = rho * math.pi * r * r * Lf
+    J = m * Lf * Lf / 3 + m * r * r / 4
+    K = E * math.pi * (2 * r) ** 4 / (64 * Lf)
+    D = cd * K
+    q, v = 0.01, -0.3
+    w.set_state(q=[0.0, q], qd=[0.0, v])
+    for _ in range(50):
+        v = v + hh * (-K * q - (D + hh * K) * v - a * J * v) / (J * (1 + hh * a) + hh * D + hh * hh * K)
+        q = q + hh * v
+        w.step(1)
+        s = w.get_state()
+        assert abs(s["q"][1] - q) < 1e-13 and abs(s["qd"][1] - v) < 1e-11
+
+
+def test_mass_damping_free_hinge_decays_geometrically_and_dissipates_2aT():
+    """A ruptured (free) hinge without gravity: v_n = v_0 / (1 + h a)^n exactly; on a tree the kinetic energy
+    falls at the rate -2 a T (power of F = -a m v, tau = -a I omega summed over the links), to first order in h."""
+    spec = chain_spec(1, 0.5, 0.02)
+    h, a = 1e-3, 2.0
+    w = OracleWorld(spec, Params(h=h, gravity=(0, 0, 0), qd_max=0.0, mass_damping=a))
+    w.set_state(qd=[0.0, 1.5], ruptured=[1])
+    hh = float(np.float32(h))
+    for n in range(1, 40):
+        w.step(1)
+        assert abs(w.get_state()["qd"][1] - 1.5 / (1 + hh * a) ** n) < 1e-13
+    # energy rate on a soft, undamped, gravity-free tree
+    rng = np.random.default_rng(5)
+    tree = strip_apples(stochastic_world(rng, 20, 30, 0, depth_choices=(3,)))
+    tree = dataclasses.replace(tree, E=1e-3)               # springs negligible: kinetic energy only
+    par = Params(h=1e-4, gravity=(0, 0, 0), c_d=0.0, qd_max=0.0, mass_damping=a)
+    w = OracleWorld(tree, par)
+    qd0 = 0.3 * rng.standard_normal(2 * tree.n_links)
+    w.set_state(qd=qd0)
+    T0, _ = w.energy()
+    w.step(100)
+    T1, _ = w.energy()
+    t = 100 * float(np.float32(1e-4))
+    assert abs(math.log(T1 / T0) / t + 2 * a) < 2e-2 * 2 * a
+
+
+def test_mass_damping_on_a_detached_apple():
+    """v <- v + h (g - a v): the detached apple is a point body with F = -c_v m v (explicit)."""
+    spec = chain_spec(1, 0.5, 0.02, apples=[(0, (0, 0, 0.5), 0.2, 2e3, 20.0)])
+    h, a = 2e-3, 1.5
+    w = OracleWorld(spec, Params(h=h, qd_max=0.0, mass_damping=a))
+    w.set_state(attached=[0], apple_v=[[0.4, 0.0, -0.2]])
+    hh = float(np.float32(h))
+    v = np.array([0.4, 0.0, -0.2])
+    for _ in range(20):
+        v = v + hh * (np.array([0.0, 0.0, -G]) - a * v)
+        w.step(1)
+        assert np.abs(w.get_state()["apple_v"][0] - v).max() < 1e-13

@@ -70,6 +70,7 @@ class Params:
     qd_max: float = 50.0
     zeta_s: float = 0.1
     forces_off_on_snapped: int = 1
+    mass_damping: float = 0.0      # c_v = c_omega of PAPER.md:128, 1/s (reading A32); 0 = off
     range_E: tuple = (0.0, 0.0)
     range_MOR: tuple = (0.0, 0.0)
     range_density: tuple = (0.0, 0.0)
