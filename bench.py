@@ -261,7 +261,8 @@ def run_cuda(args, rank: int, world_size: int):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world_size, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": region_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {W} worlds x "
+            "config": {"workload": (f"BASELINE.json configs[{args.config - 1}]" if args.config <= 5 else
+                                     "ternary L-system of PAPER.md Eq. 1, n = 4 (SURVEY.md 8(f) item 4)") + f": {W} worlds x "
                                    f"{links_per_world:.0f} links ({min(x.n_links for x in specs)}-{max(x.n_links for x in specs)}), {apples_per_world:.0f} apples, h = {P.h * 1e3:g} ms, "
                                    f"wrench U({f_lo:g},{f_hi:g}) N per world resampled every {S} steps",
                        "worlds_per_gpu": W, "physics_steps_per_bench_step": S, "links_total": n_links,
@@ -379,7 +380,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--config", type=int, default=4, help="1-based index into BASELINE.json configs (3, 4 or 5)")
+    ap.add_argument("--config", type=int, default=4, help="1-based index into BASELINE.json configs (3, 4 or 5); 6 = the homogeneous ternary L-system batch")
     ap.add_argument("--worlds", type=int, default=4096)
     ap.add_argument("--substeps", type=int, default=50, help="physics steps per bench step (one wrench epoch)")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -191,6 +191,22 @@ def test_single_step_explicit_tether_and_no_preconditioner():
         sim.close()
 
 
+def test_single_step_ternary_lsystem_homogeneous_batch():
+    """the ternary L-system of Eq. 1 (161 links at n = 4), one geometry for every world of
+    the batch (the paper's batching model), materials and apples randomized per world; under the A25 wrenches."""
+    from workloads import make_config
+    specs = make_config(6, 5)
+    P = config_params(6)
+    sim, refs = _make(specs, P, seed=MASTER_SEED + 6000)
+    for epoch in range(2):
+        _apply(sim, refs, wrench_process(specs, epoch, 0.0, 60.0))
+        sim.step(20)
+        for w, e in _single_step_errors(sim, refs, range(len(specs))).items():
+            assert e["max"] <= TOL_STEP, (epoch, w, e)
+        sim.step(9)
+    sim.close()
+
+
 def test_single_step_and_free_run_with_mass_proportional_damping():
     """SURVEY.md 8(f) item 2 / reading A32: F = -c_v m v, tau = -c_omega I omega with
     c_v = c_omega = mass_damping, implicit in the joints ((1 + h a) M in the operator, a qd as joint acceleration of

@@ -686,3 +686,21 @@ def test_mass_damping_on_a_detached_apple():
         v = v + hh * (np.array([0.0, 0.0, -G]) - a * v)
         w.step(1)
         assert np.abs(w.get_state()["apple_v"][0] - v).max() < 1e-13
+
+
+# ---------------------------------------------------------------- Eq. 1: ternary L-system workload (8(f) item 4)
+def test_ternary_lsystem_body_count_and_oracle_rest():
+    """after n derivations the body count is 1 + 2 (3^n - 1); every apex carries three branches and
+    one straight continuation; the tree is at rest in the oracle (apples hang m g / k_s below their tips)."""
+    from workloads import ternary_lsystem_world
+    for n in (1, 2, 3, 4):
+        w = ternary_lsystem_world(n, 30)
+        assert w.n_links == 1 + 2 * (3 ** n - 1)
+        kids = np.bincount(w.parent[1:], minlength=w.n_links)
+        assert sorted(set(kids.tolist())) == [0, 1, 3] and (kids == 0).sum() == 3 ** n
+        assert np.all(w.parent[1:] < np.arange(1, w.n_links))
+    w = ternary_lsystem_world(3, 9)
+    ow = OracleWorld(w, Params(h=1e-3, gravity=(0, 0, 0)))
+    ow.step(5)
+    s = ow.get_state()
+    assert np.abs(s["q"]).max() < 1e-12 and np.abs(s["qd"]).max() < 1e-10

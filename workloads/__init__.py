@@ -14,6 +14,7 @@ from .trees import (  # noqa: F401
     Params,
     binary_tree_config1,
     stochastic_world,
+    ternary_lsystem_world,
     make_config,
     config_params,
 )

@@ -165,6 +165,58 @@ def binary_tree_config1() -> WorldSpec:
 
 
 # --------------------------------------------------------------------------
+# ternary bracketed L-system of Eq. 1: SURVEY.md 8(f) item 4
+# --------------------------------------------------------------------------
+
+def ternary_lsystem_world(n_derivations: int = 4, n_apples: int = 30,
+                          rng: Optional[np.random.Generator] = None,
+                          branch_angle_deg: float = 18.95, length_ratio: float = 1.109,
+                          width_ratio: float = math.sqrt(3.0), f0: float = 0.22,
+                          tip_diameter: float = 0.006) -> WorldSpec:
+    """A -> !(v_r) F(F0) [&(a) F(F0) A] /(d1) [&(a) F(F0) A] /(d2) [&(a) F(F0) A]  from an axiom trunk,
+    d1 = d2 = 137.5 deg; internodes elongate by l_r and thicken by v_r at every later derivation.
+    After n derivations the body count is 1 + 2 (3^n - 1).  The paper gives no values for a, l_r, v_r, F0
+    (reading A33): a = 18.95 deg and l_r = 1.109 are the classic Honda-style values of this grammar,
+    v_r = sqrt(3) is the pipe rule with beta = 2 for three equal children (A20).  An internode made at
+    derivation k has length F0 l_r^(n-k) and diameter tip v_r^(n-k); the axiom trunk counts as k = 0.
+    Apples hang at the tips of distinct random terminal internodes."""
+    n = int(n_derivations)
+    rng = np.random.default_rng(0) if rng is None else rng
+    parent, born, quat = [-1], [0], [np.array([1.0, 0.0, 0.0, 0.0])]
+    apices = [0]                                   # internodes that carry an apex A at their tip
+    for k in range(1, n + 1):
+        nxt = []
+        for tip in apices:
+            main = len(parent)                     # F(F0): straight continuation
+            parent.append(tip); born.append(k); quat.append(np.array([1.0, 0.0, 0.0, 0.0]))
+            roll = 0.0
+            for c in range(3):                     # [&(a) F A] /(d1) [&(a) F A] /(d2) [&(a) F A]
+                parent.append(main); born.append(k); quat.append(_child_quat(roll, branch_angle_deg))
+                nxt.append(len(parent) - 1)
+                roll += 137.5
+        apices = nxt
+    N = len(parent)
+    assert N == 1 + 2 * (3 ** n - 1)
+    age = n - np.asarray(born)
+    length = (f0 * length_ratio ** age).astype(np.float32)
+    diam = (tip_diameter * width_ratio ** age).astype(np.float32)
+    leaves = np.asarray(apices, dtype=np.int32)
+    n_apples = min(int(n_apples), len(leaves))
+    apple_link = np.sort(rng.choice(leaves, size=n_apples, replace=False)).astype(np.int32)
+    off = np.zeros((n_apples, 3), dtype=np.float32)
+    off[:, 2] = length[apple_link]
+    return WorldSpec(
+        parent=np.asarray(parent, dtype=np.int32), length=length, diameter=diam,
+        rest_quat=_finish_quats(np.asarray(quat)), density=800.0, E=8e9, MOR=60e6,
+        apple_link=apple_link, apple_offset=off,
+        apple_mass=np.full(n_apples, 0.2, dtype=np.float32),
+        apple_radius=np.full(n_apples, 0.04, dtype=np.float32),
+        apple_k=np.full(n_apples, 2e3, dtype=np.float32),
+        apple_detach=np.full(n_apples, 20.0, dtype=np.float32),
+    )
+
+
+# --------------------------------------------------------------------------
 # stochastic generator (configs 2-5)
 # --------------------------------------------------------------------------
 
@@ -283,6 +335,8 @@ def config_params(config: int) -> Params:
     if config == 5:
         dr["range_MOR"] = (30e6, 60e6)
         return Params(h=1e-3, **dr)
+    if config == 6:      # not a BASELINE.json config: the homogeneous ternary L-system batch of SURVEY.md 8(f) item 4
+        return Params(h=1e-3, **dr)
     raise ValueError(config)
 
 
@@ -308,4 +362,8 @@ def make_config(config: int, n_worlds: Optional[int] = None) -> List[WorldSpec]:
             lo, hi = max(100, n - 10), min(1500, n + 10)
             out.append(stochastic_world(rng, lo, hi, a, depth_choices=depths))
         return out
+    if config == 6:      # one topology, one geometry for every world (the paper's batching model);
+        w = 4096 if n_worlds is None else n_worlds   # materials and apples still differ per world (ob_randomize)
+        base = ternary_lsystem_world(4, 30, rng)
+        return [base for _ in range(w)]
     raise ValueError(config)
