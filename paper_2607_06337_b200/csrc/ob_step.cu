@@ -302,16 +302,29 @@ __device__ __forceinline__ float2 split2(const double v) {
 __device__ __forceinline__ double join2(const float hi, const float lo) { return (double)hi + (double)lo; }
 
 // ---- A0 ----
-__device__ __forceinline__ void link_prepare(const int i, const Sm &s, const Gm &g, const DevCtx &c) {
-  const ob_params &P = c.P;
-  const int Np = s.Np;
-  const float2 th = __ldcg(g.q2 + i), w = __ldcg(g.w2 + i);
-  const float4 qt = __ldg(g.quat + i);
-  const float Ki = __ldg(g.K + i);
-  const float rz = (s.T[i] & kTrunk) ? 0.f : __ldg(g.rz + i);
+struct PrepIn {                     // what phase A0 reads of a link from global memory
+  float2 th, w;
+  float4 qt;
+  float Ki, rz;
   M3 R0;
+};
+__device__ __forceinline__ PrepIn link_prepare_load(const int i, const Sm &s, const Gm &g) {
+  PrepIn in;
+  in.th = __ldcg(g.q2 + i); in.w = __ldcg(g.w2 + i);
+  in.qt = __ldg(g.quat + i);
+  in.Ki = __ldg(g.K + i);
+  in.rz = __ldg(g.rz + i);
 #pragma unroll
-  for (int q = 0; q < 9; q++) R0.a[q] = __ldg(g.R0 + (size_t)q * Np + i);
+  for (int q = 0; q < 9; q++) in.R0.a[q] = __ldg(g.R0 + (size_t)q * s.Np + i);
+  return in;
+}
+__device__ __forceinline__ void link_prepare(const int i, const PrepIn &in, const Sm &s, const DevCtx &c) {
+  const ob_params &P = c.P;
+  const float2 th = in.th, w = in.w;
+  const float4 qt = in.qt;
+  const float Ki = in.Ki;
+  const float rz = (s.T[i] & kTrunk) ? 0.f : in.rz;
+  const M3 &R0 = in.R0;
   const float2 sc1 = sincos2(th.x), sc2 = sincos2(th.y);
   const float s1 = sc1.x, c1 = sc1.y, s2 = sc2.x, c2 = sc2.y;
   const float vc1 = cos_minus_one(s1, c1), vc2 = cos_minus_one(s2, c2);
@@ -599,16 +612,15 @@ __device__ __forceinline__ void up_inertia(const int i, const Sm &s, const Gm &g
 // be exact: it changes when an apple detaches, and phase A1 borrows its slot) and the Jacobi factors from the stored
 // diag(M) plus the CURRENT diagonal spring-damper terms.  A lagging preconditioner changes the number of PCG
 // iterations, never the system that is solved.
-__device__ __forceinline__ void link_inertia_lagged(const int i, const Sm &s, const Gm &g, const DevCtx &c) {
+__device__ __forceinline__ void link_inertia_lagged(const int i, float4 eff, const float2 md, const Sm &s, const Gm &g,
+                                                    const DevCtx &c) {
   const ob_params &P = c.P;
   const int Ap = s.Ap;
   uint32_t tw = s.T[i];
-  float4 eff = __ldg(g.c4 + i);
   {
     const float sc = 1.f + P.h * P.mass_damping;
     eff.x *= sc; eff.y *= sc; eff.z *= sc; eff.w *= sc;
   }
-  const float2 md = __ldcg(g.mdiag + i);
   if (P.tether_implicit && (tw & kHasApples)) {
     tw &= ~kOffax;
     const int4 t2 = __ldg(g.topo2 + i);
@@ -649,7 +661,12 @@ __device__ OB_COLD_ATTR void sweep_bias(const World *wd, const DevCtx &c, const 
   const int l_first_down = tid < 32 ? 0 : ntop - 1, l_last_up = tid < 32 ? 0 : ntop;
   // ---- A0: per link, flat ----
 #pragma unroll 1
-  for (int i = tid; i < wd->N; i += nt) link_prepare(i, s, g, c);
+  for (int i0 = tid; i0 < wd->N; i0 += 2 * nt) {      // two links per trip: all their global loads are in flight
+    const int i1 = i0 + nt < wd->N ? i0 + nt : i0;     // together (a store in between would serialise the trips)
+    const PrepIn in0 = link_prepare_load(i0, s, g), in1 = link_prepare_load(i1, s, g);
+    link_prepare(i0, in0, s, c);
+    if (i1 != i0) link_prepare(i1, in1, s, c);
+  }
   __syncthreads();
   // ---- A1: displacement-form FK, top-down ----
 #pragma unroll 1
@@ -688,7 +705,18 @@ __device__ OB_COLD_ATTR void sweep_inertia(const World *wd, const DevCtx &c, con
   const int nlev = wd->nlev, ntop = wd->ntop, N = wd->N, tid = threadIdx.x;
   if (!refresh) {
 #pragma unroll 1
-    for (int i = otid; i < N; i += nt) link_inertia_lagged(i, s, g, c);
+    for (int i0 = otid; i0 < N; i0 += 4 * nt) {          // four links per trip to L2
+      float4 c4v[4];
+      float2 mdv[4];
+#pragma unroll
+      for (int k = 0; k < 4; k++) {
+        const int i = min(i0 + k * nt, N - 1);
+        c4v[k] = __ldg(g.c4 + i); mdv[k] = __ldcg(g.mdiag + i);
+      }
+#pragma unroll
+      for (int k = 0; k < 4; k++)
+        if (i0 + k * nt < N) link_inertia_lagged(i0 + k * nt, c4v[k], mdv[k], s, g, c);
+    }
     __syncthreads();
     return;
   }
@@ -1066,16 +1094,24 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
     unsigned long long iters_total = 0;
     for (int sidx = 0; sidx < n_my; sidx++) {
       sweep_bias(&s_world, c, NT);                      // A, B1
+      {                                                 // r = b; x = cubic extrapolation of the last four solutions
+        const int t = step0 + sidx;                     // (ring of four in global memory, slot = step & 3)
+        float2 h1[LPT], h2[LPT], h3[LPT], h4[LPT];
 #pragma unroll
-      for (int k = 0; k < LPT; k++) {
-        const int i = otid + k * NT;
-        if (i < N) {                                    // r = b; x = previous dqd (warm start), kept in global memory
-          const int t = step0 + sidx;                   // solutions of steps t-1 .. t-4 out of the ring of four
-          const float2 b = s.G[i], x1 = __ldcg(g.hist + ((t - 1) & 3) * (size_t)c.sum_np + i),
-                       x2 = __ldcg(g.hist + ((t - 2) & 3) * (size_t)c.sum_np + i),
-                       x3 = __ldcg(g.hist + ((t - 3) & 3) * (size_t)c.sum_np + i),
-                       x4 = __ldcg(g.hist + (t & 3) * (size_t)c.sum_np + i);
-          XR[i] = make_float4(OB_X0(x1.x, x2.x, x3.x, x4.x), OB_X0(x1.y, x2.y, x3.y, x4.y), b.x, b.y);
+        for (int k = 0; k < LPT; k++) {
+          const int i = min(otid + k * NT, N - 1);
+          h1[k] = __ldcg(g.hist + ((t - 1) & 3) * (size_t)c.sum_np + i);
+          h2[k] = __ldcg(g.hist + ((t - 2) & 3) * (size_t)c.sum_np + i);
+          h3[k] = __ldcg(g.hist + ((t - 3) & 3) * (size_t)c.sum_np + i);
+          h4[k] = __ldcg(g.hist + (t & 3) * (size_t)c.sum_np + i);
+        }
+#pragma unroll
+        for (int k = 0; k < LPT; k++) {
+          const int i = otid + k * NT;
+          if (i < N) {
+            const float2 b = s.G[i];
+            XR[i] = make_float4(OB_X0(h1[k].x, h2[k].x, h3[k].x, h4[k].x), OB_X0(h1[k].y, h2[k].y, h3[k].y, h4[k].y), b.x, b.y);
+          }
         }
       }
       sweep_inertia(&s_world, c, NT, otid, diag_age == 0);
@@ -1112,11 +1148,22 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
 
       // ---- D: integrate, predicates ----
       const int step_now = step0 + sidx;
+      // (all global loads of the thread's links first: a store between two loads would serialise their L2 round trips)
+      float2 dw0[LPT], dq0[LPT];
+      float dK[LPT], dMx[LPT];
+      int drc[LPT];
+#pragma unroll
+      for (int k = 0; k < LPT; k++) {
+        const int i = min(otid + k * NT, N - 1);
+        dw0[k] = __ldcg(g.w2 + i); dq0[k] = __ldcg(g.q2 + i);
+        dK[k] = __ldg(g.K + i); dMx[k] = __ldg(g.Mmax + i);
+        drc[k] = __ldcg(g.rc + i);
+      }
 #pragma unroll
       for (int k = 0; k < LPT; k++) {
         const int i = otid + k * NT;
         if (i >= N) continue;
-        const float2 w0 = __ldcg(g.w2 + i), q0 = __ldcg(g.q2 + i);
+        const float2 w0 = dw0[k], q0 = dq0[k];
         const float2 x = *reinterpret_cast<const float2 *>(XR + i);
         g.hist[(step_now & 3) * (size_t)c.sum_np + i] = x;
         float wa = w0.x + x.x, wb = w0.y + x.y;
@@ -1128,9 +1175,9 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         g.w2[i] = make_float2(wa, wb); g.q2[i] = make_float2(qa, qb);
         const uint32_t tw = s.T[i];
         if (!(tw & kRuptured)) {
-          const float Ki = __ldg(g.K + i), Mx = __ldg(g.Mmax + i);
+          const float Ki = dK[k], Mx = dMx[k];
           const float mu = Ki * sqrtf(qa * qa + qb * qb);                   // Eq. 5
-          const int rc0 = __ldcg(g.rc + i);
+          const int rc0 = drc[k];
           const int rcn = mu > Mx ? rc0 + 1 : 0;
           if (rcn >= P.rupture_frames) {
             g.rupt[i] = 1; g.rc[i] = 0;
