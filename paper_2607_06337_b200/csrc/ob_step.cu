@@ -56,7 +56,7 @@ constexpr uint32_t kHasApples = 1u << 26, kOffax = 1u << 27, kSnapped = 1u << 28
 // shared-memory view of one world
 // ------------------------------------------------------------------------------------------------------
 struct Sm {
-  int Np, Ap, NIp, S;
+  int Np, Ap, NIp;
   float4 *P;                          // records: P[7 * i + j], j = 0 M0, 1 M1, 2 PD, 3..5 C0..C2, 6 C3
   float2 *G;
   uint32_t *T;
@@ -78,7 +78,7 @@ extern __shared__ __align__(128) unsigned char ob_smem[];
 
 __device__ __forceinline__ Sm carve(unsigned char *base, const int Np, const int Ap, const int NIp, const int n_levels) {
   Sm s;
-  s.Np = Np; s.Ap = Ap; s.NIp = NIp; s.S = Np + 1;
+  s.Np = Np; s.Ap = Ap; s.NIp = NIp;
   unsigned char *p = base;
   s.P = reinterpret_cast<float4 *>(p); p += step_planes_bytes(Np);
   s.G = reinterpret_cast<float2 *>(p); p += r16(8 * (Np + 1));
@@ -100,7 +100,7 @@ __device__ __forceinline__ Sm carve(unsigned char *base, const int Np, const int
 
 // per-link data of one world in global memory (L2-resident; only the once-per-step phases read it)
 struct Gm {
-  float2 *q2, *w2, *x2;             // state (link block)
+  float2 *q2, *w2;                  // state (link block)
   unsigned char *rupt, *rc;
   const float4 *c4;                 // (m, m c, I about the joint, I_zz)
   const float *K, *rz;              // joint stiffness (Eq. 4), parent length
@@ -543,7 +543,7 @@ __device__ __forceinline__ void link_bias_up(const int i, const uint32_t tw, con
 // composite inertia in the parent frame (M0[i], M1[i], PD[i].xy)
 // ------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void up_inertia(const int i, const Sm &s, const Gm &g, const DevCtx &c) {
-  const int S = s.S, Ap = s.Ap;
+  const int Ap = s.Ap;
   const ob_params &P = c.P;
   uint32_t tw = s.T[i];
   float4 c4 = __ldg(g.c4 + i);
@@ -990,7 +990,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
   __shared__ int s_next;
   __shared__ World s_world;
   __shared__ __align__(16) float2 s_stage[64];
-  const int tid = threadIdx.x, lane = tid & 31;
+  const int tid = threadIdx.x;
   // the warp that sweeps the top levels of the PCG products: rotated over the CTAs that share an SM, so that these
   // serial stretches do not all land on the same warp scheduler
   const int topw = (int)((blockIdx.x / (unsigned)top_rot) % (NT / 32));
@@ -1034,13 +1034,13 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       continue;
     }
     const Sm s = carve(smem, d.Np, d.Ap, d.NIp, d.n_levels);
-    const int Np = d.Np, S = Np + 1, N = d.N;
+    const int Np = d.Np, N = d.N;
     const int nlev = d.n_levels, ntop = d.n_top;
     float4 *const PL = s.P;
     Gm g;
     {
       unsigned char *lb = c.link_blk + d.link_blk_off;
-      g.q2 = reinterpret_cast<float2 *>(lb); g.w2 = g.q2 + Np; g.x2 = g.w2 + Np;
+      g.q2 = reinterpret_cast<float2 *>(lb); g.w2 = g.q2 + Np;
       g.rupt = lb + 24 * Np; g.rc = g.rupt + Np;
       const unsigned char *cst = lb + link_state_bytes(Np);
       g.c4 = reinterpret_cast<const float4 *>(cst);
@@ -1072,7 +1072,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       for (int k = tid; k < (int)(sizeof(WrenchSlots) / 4); k += NT) dst[k] = __ldg(src + k);
       if (tid < 7) PL[7 * Np + tid] = make_float4(0.f, 0.f, 0.f, 0.f);            // the zero column
       for (int k = tid; k <= nlev; k += NT) s.lev[k] = __ldg(c.level_off + d.level_base + k);
-      for (int i = tid; i < S; i += NT) {
+      for (int i = tid; i <= Np; i += NT) {
         uint32_t tw = (uint32_t)Np | kTrunk;
         if (i < N) {
           const int4 tp = __ldg(c.topo + d.link_base + i);
