@@ -79,7 +79,9 @@ __device__ __forceinline__ void tma_store(void *gdst, const void *smem_src, uint
 }
 __device__ __forceinline__ void tma_store_commit_wait() {
   asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-  asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+  // full completion, not .read: the next chunk of this world may be staged by another CTA as soon as the progress
+  // word is published, so the bulk store's global writes must have landed, not only its shared-memory reads
+  asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 

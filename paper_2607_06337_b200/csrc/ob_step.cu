@@ -125,7 +125,7 @@ __device__ __forceinline__ float cos_minus_one(float sn, float cs) { return cs >
 template <int NT>
 struct Reducer {
   float2 *stage;   // [2][32]
-  int flip, tid;
+  int flip, tid;   // tid = the thread's LOGICAL index (otid): the sum must not depend on which warp is the top warp
   __device__ __forceinline__ float2 sum(float a, float b) {
     // five shuffles for the pair: the two halves of the warp trade a for b first
     const bool hi = (tid & 16) != 0;
@@ -755,7 +755,7 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
   float4 *const PL = s.P;
   float4 *const XR = s.XR;
   Reducer<NT> red;
-  red.stage = stage; red.flip = *flipp; red.tid = tid;
+  red.stage = stage; red.flip = *flipp; red.tid = otid;
   int status = 0;
   // lanes of the top warp <-> links of the n_top leading levels: level of the lane's link, widest child list
   // that stays inside the warp
@@ -825,7 +825,7 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
         const int le = s.lev[l + 1];
         const bool deepest = l == nlev - 1;
 #pragma unroll 1
-        for (int i = s.lev[l] + tid; i < le; i += NT) {
+        for (int i = s.lev[l] + otid; i < le; i += NT) {
           const uint32_t tw = s.T[i];
           float4 *rec = PL + 7 * i;
           const float4 pd = rec[2];
@@ -845,7 +845,7 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
       for (int l = nlev - 2; l >= ntop; l--) {
         const int le = s.lev[l + 1];
 #pragma unroll 1
-        for (int i = s.lev[l] + tid; i < le; i += NT) {
+        for (int i = s.lev[l] + otid; i < le; i += NT) {
           const uint32_t tw = s.T[i];
           const float4 *rec = PL + 7 * i;
           const float4 pd = rec[2];
@@ -992,7 +992,9 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
   __shared__ __align__(16) float2 s_stage[64];
   const int tid = threadIdx.x;
   // the warp that sweeps the top levels of the PCG products: rotated over the CTAs that share an SM, so that these
-  // serial stretches do not all land on the same warp scheduler
+  // serial stretches do not all land on the same warp scheduler.  Everything arithmetic is indexed by the logical
+  // thread index otid (a rotation of tid by whole warps), so the results do not depend on the rotation: a world
+  // gives the same bits whichever CTA of the queue picks it up
   const int topw = (int)((blockIdx.x / (unsigned)top_rot) % (NT / 32));
   const bool top_warp = (tid >> 5) == topw;
   // flat ownership: thread otid + k * NT <-> link; the top warp owns links 0..31, i.e. exactly its lanes' links
@@ -1004,7 +1006,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
   Reducer<NT> red;
   red.stage = s_stage;
   red.flip = 0;
-  red.tid = tid;
+  red.tid = otid;
 
   for (;;) {
     if (tid == 0) s_next = atomicAdd(queue, 1);

@@ -417,6 +417,34 @@ def test_state_round_trip_and_multi_step_launch_are_bit_exact():
     a.close(); b.close()
 
 
+def test_chunked_launch_hand_off_is_bit_exact_at_scale():
+    """A launch of 50 steps is cut into five queue items per world that different CTAs may take (the state of a
+    world crosses in global memory behind a progress word).  2048 worlds over 444 resident CTAs: step(50) must equal
+    5 x step(10) (no hand-off inside a launch) bit for bit, twice in a row (a stale read would show as a difference)."""
+    specs = make_config(4, 2048)
+    P = config_params(4)
+    loads = wrench_process(specs, 0, 0.0, 150.0)
+    sims = [ob.Orchard(specs, P) for _ in range(3)]
+    for sim in sims:
+        sim.randomize(99)
+        sim.apply_wrench_batch([l[0] for l in loads], [l[1] for l in loads], [l[2] for l in loads], [l[3] for l in loads])
+    sims[0].step(50)
+    sims[1].step(50)
+    for _ in range(5):
+        sims[2].step(10)
+    st = [sim.stats() for sim in sims]
+    assert st[0] == st[1] == st[2], st
+    ev = [sorted(sim.events()) for sim in sims]
+    assert ev[0] == ev[1] == ev[2]
+    for w in list(range(0, len(specs), 16)) + [len(specs) - 1]:
+        g = [sim.get_state(w) for sim in sims]
+        for k in ("q", "qd", "apple_v", "ruptured", "attached"):
+            assert g[0][k].tobytes() == g[1][k].tobytes() == g[2][k].tobytes(), (w, k)
+        assert g[0]["apple_x64"].tobytes() == g[1]["apple_x64"].tobytes() == g[2]["apple_x64"].tobytes(), w
+    for sim in sims:
+        sim.close()
+
+
 def test_wrench_slots_and_event_drain():
     spec = binary_tree_config1()
     P = dataclasses.replace(config_params(1), detach_frames_pull=1)
