@@ -180,6 +180,13 @@ int ob_sizeof_params(void);
 int ob_sizeof_world_spec(void);
 int ob_sizeof_event(void);
 
+/* Self-test of the device Philox4x32-10 (reading A23) against NVIDIA's own implementation: for n (counter, key)
+   pairs computes the library's generator and cuRAND's curand_Philox4x32_10 on the device.  ctr: [4*n], key: [2*n],
+   out_lib / out_curand: [4*n] host arrays; dev_scratch: caller-provided device memory of >= 56*n bytes; the work is
+   enqueued on cuda_stream and the call synchronises it.  No context needed.  Returns OB_E_ARG / OB_E_CUDA. */
+int ob_selftest_philox(int n, const uint32_t *ctr, const uint32_t *key, uint32_t *out_lib, uint32_t *out_curand,
+                       void *dev_scratch, void *cuda_stream);
+
 const char *ob_last_error(const ob_ctx *ctx);
 void ob_destroy(ob_ctx *ctx);
 

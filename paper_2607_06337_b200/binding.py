@@ -22,6 +22,7 @@ EXPORTS = [
     "ob_apply_wrench_batch", "ob_step", "ob_get_state", "ob_set_state", "ob_get_apple_x64", "ob_get_counters", "ob_set_counters",
     "ob_get_material", "ob_events", "ob_stats", "ob_launch_info", "ob_last_error", "ob_destroy",
     "ob_sizeof_params", "ob_sizeof_world_spec", "ob_sizeof_event", "ob_counters", "ob_flush",
+    "ob_selftest_philox",
 ]
 
 

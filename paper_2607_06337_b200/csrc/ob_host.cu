@@ -879,6 +879,29 @@ int ob_sizeof_params(void) { return (int)sizeof(ob_params); }
 int ob_sizeof_world_spec(void) { return (int)sizeof(ob_world_spec); }
 int ob_sizeof_event(void) { return (int)sizeof(ob_event); }
 
+int ob_selftest_philox(int n, const uint32_t *ctr, const uint32_t *key, uint32_t *out_lib, uint32_t *out_curand,
+                       void *dev_scratch, void *cuda_stream) {
+  if (n < 1 || !ctr || !key || !out_lib || !out_curand || !dev_scratch) return fail0(OB_E_ARG, "ob_selftest_philox: null or empty");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  std::vector<uint32_t> in(6 * (size_t)n), out(8 * (size_t)n);
+  for (int i = 0; i < n; i++) {
+    for (int k = 0; k < 4; k++) in[6 * (size_t)i + k] = ctr[4 * (size_t)i + k];
+    for (int k = 0; k < 2; k++) in[6 * (size_t)i + 4 + k] = key[2 * (size_t)i + k];
+  }
+  uint32_t *d_in = reinterpret_cast<uint32_t *>(dev_scratch), *d_out = d_in + 6 * (size_t)n;
+  cudaError_t e = cudaMemcpyAsync(d_in, in.data(), in.size() * 4, cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) e = launch_philox_selftest(n, d_in, d_out, st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(out.data(), d_out, out.size() * 4, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return fail0(OB_E_CUDA, cudaGetErrorString(e));
+  for (int i = 0; i < n; i++)
+    for (int k = 0; k < 4; k++) {
+      out_lib[4 * (size_t)i + k] = out[8 * (size_t)i + k];
+      out_curand[4 * (size_t)i + k] = out[8 * (size_t)i + 4 + k];
+    }
+  return OB_OK;
+}
+
 const char *ob_last_error(const ob_ctx *ctx) { return ctx ? ctx->err.c_str() : (g_err.empty() ? kNullCtx : g_err.c_str()); }
 
 void ob_destroy(ob_ctx *ctx) {

@@ -157,6 +157,7 @@ cudaError_t launch_randomize(const DevCtx &c, unsigned long long seed, int redra
 cudaError_t launch_step(const DevCtx &c, int cls, const int32_t *order, int n_in_class, int32_t *queue, int n_steps,
                         int grid, int smem, int n_sm, int n_chunks, int32_t *progress, cudaStream_t s);
 cudaError_t launch_pose(const DevCtx &c, int world, cudaStream_t s);
+cudaError_t launch_philox_selftest(int n, const uint32_t *d_in, uint32_t *d_out, cudaStream_t s);
 cudaError_t step_kernel_setup(int cls, int smem_bytes, int *max_blocks_per_sm);
 
 }  // namespace ob

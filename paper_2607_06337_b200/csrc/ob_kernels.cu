@@ -13,6 +13,8 @@
 #include "ob_device.h"
 #include "ob_internal.h"
 
+#include <curand_philox4x32_x.h>
+
 namespace ob {
 
 // ------------------------------------------------------------------------------------------------------
@@ -225,6 +227,22 @@ cudaError_t launch_randomize(const DevCtx &c, unsigned long long seed, int redra
 }
 cudaError_t launch_pose(const DevCtx &c, int world, cudaStream_t s) {
   k_pose<<<4, 128, 0, s>>>(c, world);
+  return cudaGetLastError();
+}
+
+// self-test: the generator above and cuRAND's curand_Philox4x32_10 on the same (counter, key) pairs
+__global__ void k_philox_selftest(int n, const uint32_t *__restrict__ in, uint32_t *__restrict__ out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint4 ctr = make_uint4(in[6 * i], in[6 * i + 1], in[6 * i + 2], in[6 * i + 3]);
+  const uint2 key = make_uint2(in[6 * i + 4], in[6 * i + 5]);
+  const uint4 a = philox4x32_10(ctr, key);
+  const uint4 b = curand_Philox4x32_10(ctr, key);
+  out[8 * i] = a.x; out[8 * i + 1] = a.y; out[8 * i + 2] = a.z; out[8 * i + 3] = a.w;
+  out[8 * i + 4] = b.x; out[8 * i + 5] = b.y; out[8 * i + 6] = b.z; out[8 * i + 7] = b.w;
+}
+cudaError_t launch_philox_selftest(int n, const uint32_t *d_in, uint32_t *d_out, cudaStream_t s) {
+  k_philox_selftest<<<(n + 127) / 128, 128, 0, s>>>(n, d_in, d_out);
   return cudaGetLastError();
 }
 
