@@ -5,7 +5,7 @@
  * bench.py's cpu_baseline / --impl reference legs may load this file.  It shares
  * no code, header, table or helper with paper_2607_06337_b200/ (the CUDA path)
  * and is written from the paper (/root/reference/PAPER.md, cited as PAPER.md:<line>)
- * plus the readings listed in DESIGN.md ("Readings", A1..A31 of SURVEY.md 8(c)).
+ * plus the readings listed in DESIGN.md ("Readings": A1..A31 of SURVEY.md 8(c), A32, A33).
  *
  * What it computes, in the paper's order, all in double precision:
  *   - the articulation of PAPER.md:113-117 (Eq. 3): links are rigid cylinders
