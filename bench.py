@@ -179,6 +179,8 @@ def run_cuda(args, rank: int, world_size: int):
         sim.randomize(seed)
         stream = sim.stream
         for e in range(args.warmup):
+            if args.config == 5 and e > 0 and e % 5 == 0:
+                sim.randomize(seed + 5000 + e // 5)
             sim.apply_wrench_batch(*epochs[e])
             sim.step(S)
             if e2e:
@@ -194,6 +196,9 @@ def run_cuda(args, rank: int, world_size: int):
         t_begin.record(stream)
         wall0 = time.perf_counter()
         for k in range(args.steps):
+            if args.config == 5 and (args.warmup + k) % 5 == 0:
+                # configs[4]: on-device Philox re-randomization and reset of every world every 250 steps
+                sim.randomize(seed + 5000 + (args.warmup + k) // 5)
             if e2e:
                 sim.apply_wrench_batch(*epochs[args.warmup + k])      # host arrays -> pinned staging -> device
                 sim.step(S)
