@@ -157,7 +157,7 @@ inline int pad8(int n) { return (n + 7) / 8 * 8; }
 
 struct Layout {
   size_t total = 0;
-  Pool desc, order, link_blk, apple_blk, topo, topo2, child_list, quat, quat_raw, R0, Mmax, mdiag, xprev, Lown, diam, arm, link_ext, apple_ext, apple_nom,
+  Pool desc, order, link_blk, apple_blk, topo, topo2, child_list, quat, quat_raw, quatd, R0, Mmax, mdiag, xprev, Lown, diam, arm, link_ext, apple_ext, apple_nom,
       apple_c, anchor, level_off, info, wrench, events, ev_count, queue, progress, pose7;
   size_t sumNp = 0, sumAp = 0, sumLev = 0, ev_cap = 0;
   int max_Np = 0, max_Ap = 0, max_smem = 0;
@@ -213,6 +213,7 @@ int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) 
   take(L, L.child_list, sizeof(int32_t) * L.sumNp);
   take(L, L.quat, sizeof(float4) * L.sumNp);
   take(L, L.quat_raw, sizeof(float4) * L.sumNp);
+  take(L, L.quatd, sizeof(double) * 4 * L.sumNp);
   take(L, L.R0, sizeof(float) * 9 * L.sumNp);
   take(L, L.Mmax, sizeof(float) * L.sumNp);
   take(L, L.mdiag, sizeof(float2) * L.sumNp);
@@ -465,6 +466,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   D.child_list = reinterpret_cast<int32_t *>(base + L.child_list.off);
   D.quat = reinterpret_cast<float4 *>(base + L.quat.off);
   D.quat_raw = reinterpret_cast<float4 *>(base + L.quat_raw.off);
+  D.quatd = reinterpret_cast<double *>(base + L.quatd.off);
   D.R0 = reinterpret_cast<float *>(base + L.R0.off);
   D.Mmax = reinterpret_cast<float *>(base + L.Mmax.off);
   D.mdiag = reinterpret_cast<float2 *>(base + L.mdiag.off);

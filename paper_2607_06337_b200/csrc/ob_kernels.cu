@@ -64,6 +64,12 @@ __global__ void k_rest_pose(DevCtx c) {
       for (int k = 0; k < 9; k++) R[k] = T[k];
     }
     for (int k = 0; k < 9; k++) c.R0[9 * (size_t)d.link_base + (size_t)k * d.Np + i] = (float)R[k];
+    {                                           // the link's own rest quaternion, normalised in fp64, for the FK of k_step
+      const float4 q = quat[i];
+      const double w = q.x, x = q.y, y = q.z, z = q.w, n = sqrt(w * w + x * x + y * y + z * z);
+      double *qd = c.quatd + 4 * ((size_t)d.link_base + i);
+      qd[0] = w / n; qd[1] = x / n; qd[2] = y / n; qd[3] = z / n;
+    }
   }
   const unsigned char *ab = c.apple_blk + d.apple_blk_off;
   const float *ao = reinterpret_cast<const float *>(ab + apple_state_bytes(d.Ap));

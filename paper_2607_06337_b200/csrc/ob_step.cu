@@ -68,6 +68,7 @@ struct Sm {
   unsigned char *att, *cA, *cB;
   float *ao, *ak, *am, *ac, *afd;     // ao = [3][Ap]
   float *ft, *fsn;                    // tether force [3][Ap], |f_s| [Ap] (phase A2 -> phase D)
+  float *hd;                          // [6][Ap] anchor - x_hang of every apple, fp64 as (hi, lo) pairs (phase A1 -> A2)
   WrenchSlots *wr;
 };
 
@@ -94,6 +95,7 @@ __device__ __forceinline__ Sm carve(unsigned char *base, const int Np, const int
   f = reinterpret_cast<float *>(p);
   s.ft = f; f += 3 * Ap;
   s.fsn = f; f += Ap;
+  s.hd = f; f += 6 * Ap;
   s.wr = reinterpret_cast<WrenchSlots *>(f);
   return s;
 }
@@ -104,7 +106,8 @@ struct Gm {
   unsigned char *rupt, *rc;
   const float4 *c4;                 // (m, m c, I about the joint, I_zz)
   const float *K, *rz;              // joint stiffness (Eq. 4), parent length
-  const float4 *quat;
+  const double2 *quatd;             // rest quaternions, normalised, fp64: (w, x), (y, z) of link i at 2 i, 2 i + 1
+  const double *anchor;             // [k * Ap + a] rest hang points, world frame, fp64
   const float *R0;                  // [k * Np + i]
   const float *Mmax;
   float2 *mdiag;                    // diag(M) as last computed by phase B2 (the Jacobi preconditioner may lag)
@@ -301,91 +304,94 @@ __device__ __forceinline__ float2 split2(const double v) {
 }
 __device__ __forceinline__ double join2(const float hi, const float lo) { return (double)hi + (double)lo; }
 
-// ---- A0 ----
-struct PrepIn {                     // what phase A0 reads of a link from global memory
-  float2 th, w;
-  float4 qt;
-  float Ki, rz;
-  M3 R0;
-};
-__device__ __forceinline__ PrepIn link_prepare_load(const int i, const Sm &s, const Gm &g) {
-  PrepIn in;
-  in.th = __ldcg(g.q2 + i); in.w = __ldcg(g.w2 + i);
-  in.qt = __ldg(g.quat + i);
-  in.Ki = __ldg(g.K + i);
-  in.rz = __ldg(g.rz + i);
-#pragma unroll
-  for (int q = 0; q < 9; q++) in.R0.a[q] = __ldg(g.R0 + (size_t)q * s.Np + i);
-  return in;
-}
-__device__ __forceinline__ void link_prepare(const int i, const PrepIn &in, const Sm &s, const DevCtx &c) {
-  const ob_params &P = c.P;
-  const float2 th = in.th, w = in.w;
-  const float4 qt = in.qt;
-  const float Ki = in.Ki;
-  const float rz = (s.T[i] & kTrunk) ? 0.f : in.rz;
-  const M3 &R0 = in.R0;
-  const float2 sc1 = sincos2(th.x), sc2 = sincos2(th.y);
-  const float s1 = sc1.x, c1 = sc1.y, s2 = sc2.x, c2 = sc2.y;
-  const float vc1 = cos_minus_one(s1, c1), vc2 = cos_minus_one(s2, c2);
-  M3 XY;                                                           // Rx(th1) Ry(th2)
-  XY.a[0] = c2;       XY.a[1] = 0.f; XY.a[2] = s2;
-  XY.a[3] = s1 * s2;  XY.a[4] = c1;  XY.a[5] = -s1 * c2;
-  XY.a[6] = -c1 * s2; XY.a[7] = s1;  XY.a[8] = c1 * c2;
-  {
-    const M3 Rrel = mul(quat_to_mat(qt), XY);
-    Jt j;                                                          // E = Rrel^T
-#pragma unroll
-    for (int r = 0; r < 3; r++)
-#pragma unroll
-      for (int cc = 0; cc < 3; cc++) j.E.a[3 * r + cc] = Rrel.a[3 * cc + r];
-    j.c2 = c2; j.s2 = s2; j.rz = rz;
-    store_jt(s.P, i, j);
-  }
-  // displacement-form FK, own part: R0_i (RxRy - I)
-  XY.a[0] = vc2; XY.a[4] = vc1; XY.a[8] = fmaf(vc1, vc2, vc1 + vc2);
-  const M3 t2m = mul(R0, XY);
-  // spring-damper part of the rhs and of the diagonal (Eq. 4, PAPER.md:123); a ruptured joint has K = D = 0
-  const float Kt = (s.T[i] & kRuptured) ? 0.f : Ki, Dt = P.c_d * Kt;
-  s.G[i] = make_float2(Kt * th.x + (Dt + P.h * Kt) * w.x, Kt * th.y + (Dt + P.h * Kt) * w.y);
-  s.P[7 * i] = make_float4(t2m.a[0], t2m.a[1], t2m.a[2], t2m.a[3]);
-  s.P[7 * i + 1] = make_float4(t2m.a[4], t2m.a[5], t2m.a[6], t2m.a[7]);
-  s.P[7 * i + 2] = make_float4(t2m.a[8], 0.f, 0.f, (P.h * P.c_d + P.h * P.h) * Kt);
-}
-
-// ---- A1 ----  dR_i = dR_p Rrel + R0_i (RxRy - I),  dp_i = dp_p + dR_p (0,0,rz)
-__device__ __forceinline__ void link_fk(const int i, const Sm &s) {
+// ---- A1 ----  forward kinematics in fp64 (Eq. 3): R_i = R_p Q_i Rx(th1) Ry(th2),
+//               p_i = p_p + R_p (0,0,L_p).  The tether stretch x_a - x_hang is a millimetre-sized difference of
+//               metre-sized positions, k_s = 2e3 N/m turns 1e-8 m of it into the whole error budget of a 3 mm twig:
+//               rest rotations, sin / cos of the joint angles and the chain of products are therefore fp64, and the
+//               hang point of every apple is formed here, where the fp64 pose is at hand.  The dynamics get the
+//               fp32-rounded joint transform E = R_rel^T.
+// Publish of an inner link for its children (twelve doubles): R[0..7] in the record slots 0, 1, 2, 6, R[8] in G,
+// p in the overflow slot.  A leaf keeps its fp32 rotation in slots 0, 1, 2.x for phase A2.
+__device__ __forceinline__ void link_fk(const int i, const Sm &s, const Gm &g) {
   float4 *rec = s.P + 7 * i;
   uint32_t tw = s.T[i];
-  const float4 *par = s.P + 7 * (int)(tw & kParMask);             // the trunk reads the zero record
-  const float4 p0 = par[0], p1 = par[1], p2 = par[2], p3 = par[6];
-  const uint32_t snapped_p = (tw & kTrunk) ? 0u : (s.T[tw & kParMask] & kSnapped);
-  const float4 o0 = rec[0], o1 = rec[1];
-  const float o8 = rec[2].x;
-  const Jt j = load_jt(s.P, i);
-  M3 dRp, Rrel, dR;
-  dRp.a[0] = p0.x; dRp.a[1] = p0.y; dRp.a[2] = p0.z; dRp.a[3] = p0.w;
-  dRp.a[4] = p1.x; dRp.a[5] = p1.y; dRp.a[6] = p1.z; dRp.a[7] = p1.w; dRp.a[8] = p2.x;
+  const double2 qa = __ldg(g.quatd + 2 * i), qb = __ldg(g.quatd + 2 * i + 1);
+  const int4 t2 = __ldg(g.topo2 + i);
+  const bool trunk = (tw & kTrunk) != 0u;
+  const float rzf = trunk ? 0.f : __ldg(g.rz + i);
+  double Q[9], X[9], Rrel[9];
+  {
+    const double w = qa.x, x = qa.y, y = qb.x, z = qb.y;
+    Q[0] = 1 - 2 * (y * y + z * z); Q[1] = 2 * (x * y - w * z);     Q[2] = 2 * (x * z + w * y);
+    Q[3] = 2 * (x * y + w * z);     Q[4] = 1 - 2 * (x * x + z * z); Q[5] = 2 * (y * z - w * x);
+    Q[6] = 2 * (x * z - w * y);     Q[7] = 2 * (y * z + w * x);     Q[8] = 1 - 2 * (x * x + y * y);
+  }
+  // sin / cos of the two joint angles in fp64: phase A0 left them in the link's own record slots 0, 1
+  const double2 sc1 = reinterpret_cast<const double2 *>(rec)[0], sc2 = reinterpret_cast<const double2 *>(rec)[1];
+  const double s1 = sc1.x, c1 = sc1.y, s2 = sc2.x, c2 = sc2.y;
+  X[0] = c2;       X[1] = 0.0; X[2] = s2;                           // Rx(th1) Ry(th2)
+  X[3] = s1 * s2;  X[4] = c1;  X[5] = -s1 * c2;
+  X[6] = -c1 * s2; X[7] = s1;  X[8] = c1 * c2;
 #pragma unroll
   for (int r = 0; r < 3; r++)
 #pragma unroll
-    for (int cc = 0; cc < 3; cc++) Rrel.a[3 * r + cc] = j.E.a[3 * cc + r];
-  dR = mul(dRp, Rrel);
-  dR.a[0] += o0.x; dR.a[1] += o0.y; dR.a[2] += o0.z; dR.a[3] += o0.w;
-  dR.a[4] += o1.x; dR.a[5] += o1.y; dR.a[6] += o1.z; dR.a[7] += o1.w; dR.a[8] += o8;
-  // fp64: the tether stretch is the small difference of two sums along the chain, and k_s times its rounding
-  // error is what the thinnest twigs feel
-  const double rz = (double)j.rz;
-  const float2 dx = split2(join2(p2.y, p2.z) + rz * (double)dRp.a[2]);
-  const float2 dy = split2(join2(p3.x, p3.y) + rz * (double)dRp.a[5]);
-  const float2 dz = split2(join2(p3.z, p3.w) + rz * (double)dRp.a[8]);
-  const float dt0 = rec[2].w;
-  rec[0] = make_float4(dR.a[0], dR.a[1], dR.a[2], dR.a[3]);
-  rec[1] = make_float4(dR.a[4], dR.a[5], dR.a[6], dR.a[7]);
-  rec[2] = make_float4(dR.a[8], dx.x, dx.y, dt0);
-  rec[6] = make_float4(dy.x, dy.y, dz.x, dz.y);
+    for (int cc = 0; cc < 3; cc++) Rrel[3 * r + cc] = Q[3 * r] * X[cc] + Q[3 * r + 1] * X[3 + cc] + Q[3 * r + 2] * X[6 + cc];
+  {
+    Jt j;                                                            // E = Rrel^T, rounded once
+#pragma unroll
+    for (int r = 0; r < 3; r++)
+#pragma unroll
+      for (int cc = 0; cc < 3; cc++) j.E.a[3 * r + cc] = (float)Rrel[3 * cc + r];
+    j.c2 = (float)c2; j.s2 = (float)s2; j.rz = rzf;
+    store_jt(s.P, i, j);
+  }
+  double Rp[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1}, pp[3] = {0, 0, 0};
+  uint32_t snapped_p = 0u;
+  if (!trunk) {
+    const int par = (int)(tw & kParMask), ps = (int)((uint32_t)t2.y >> 16);
+    const double2 *pr = reinterpret_cast<const double2 *>(s.P + 7 * par);
+    const double2 a0 = pr[0], a1 = pr[1], a2 = pr[2], a3 = pr[6];
+    Rp[0] = a0.x; Rp[1] = a0.y; Rp[2] = a1.x; Rp[3] = a1.y; Rp[4] = a2.x; Rp[5] = a2.y; Rp[6] = a3.x; Rp[7] = a3.y;
+    Rp[8] = *reinterpret_cast<const double *>(s.G + par);
+    const double2 b0 = *reinterpret_cast<const double2 *>(s.ovf + ps);
+    pp[0] = b0.x; pp[1] = b0.y; pp[2] = *reinterpret_cast<const double *>(s.ovf + s.NIp + ps);
+    snapped_p = s.T[par] & kSnapped;
+  }
+  double R[9], pw[3];
+#pragma unroll
+  for (int r = 0; r < 3; r++)
+#pragma unroll
+    for (int cc = 0; cc < 3; cc++) R[3 * r + cc] = Rp[3 * r] * Rrel[cc] + Rp[3 * r + 1] * Rrel[3 + cc] + Rp[3 * r + 2] * Rrel[6 + cc];
+  const double rz = (double)rzf;
+  pw[0] = pp[0] + rz * Rp[2]; pw[1] = pp[1] + rz * Rp[5]; pw[2] = pp[2] + rz * Rp[8];
   tw = (tw & ~kSnapped) | (((tw & kRuptured) || snapped_p) ? kSnapped : 0u);
   s.T[i] = tw;
+  // hang points of the apples on this link: anchor - x_hang (the anchor is the rest hang point, fp64)
+  if (tw & kHasApples) {
+    const int Ap = s.Ap, ast = t2.x & 0xffff, nap = t2.x >> 16;
+    for (int a = ast; a < ast + nap; a++) {
+      const double ox = s.ao[a], oy = s.ao[Ap + a], oz = s.ao[2 * Ap + a];
+#pragma unroll
+      for (int k = 0; k < 3; k++) {
+        const double xh = pw[k] + R[3 * k] * ox + R[3 * k + 1] * oy + R[3 * k + 2] * oz;
+        const float2 dd = split2(__ldg(g.anchor + (size_t)k * Ap + a) - xh);
+        s.hd[(2 * k) * Ap + a] = dd.x; s.hd[(2 * k + 1) * Ap + a] = dd.y;
+      }
+    }
+  }
+  if ((tw >> kNcShift) & kNcMask) {
+    const int is = t2.y & 0xffff;
+    double2 *pr = reinterpret_cast<double2 *>(rec);
+    pr[0] = make_double2(R[0], R[1]); pr[1] = make_double2(R[2], R[3]); pr[2] = make_double2(R[4], R[5]);
+    pr[6] = make_double2(R[6], R[7]);
+    *reinterpret_cast<double *>(s.G + i) = R[8];
+    *reinterpret_cast<double2 *>(s.ovf + is) = make_double2(pw[0], pw[1]);
+    *reinterpret_cast<double *>(s.ovf + s.NIp + is) = pw[2];
+  } else {
+    rec[0] = make_float4((float)R[0], (float)R[1], (float)R[2], (float)R[3]);
+    rec[1] = make_float4((float)R[4], (float)R[5], (float)R[6], (float)R[7]);
+    rec[2] = make_float4((float)R[8], 0.f, 0.f, 0.f);
+  }
 }
 
 // tether reactions (Eq. 6 / Eq. 7) and user wrenches on one link, subtracted from its bias
@@ -398,31 +404,36 @@ __device__ __noinline__ Force6 external_forces(const int i, const float3 om, con
   const Sm s = carve(wd);
   const Gm g = wd->g;
   const ob_params &P = c.P;
-  const int Np = s.Np, Ap = s.Ap;
+  const int Ap = s.Ap;
   Force6 out;
   out.n = f3(0, 0, 0); out.f = f3(0, 0, 0);
-  const float4 *rec = s.P + 7 * i;
-  const float4 r0 = rec[0], r1 = rec[1], r2 = rec[2], r3 = rec[6];
-  M3 dR, R;                                                               // world rotation R0 + dR
-  dR.a[0] = r0.x; dR.a[1] = r0.y; dR.a[2] = r0.z; dR.a[3] = r0.w;
-  dR.a[4] = r1.x; dR.a[5] = r1.y; dR.a[6] = r1.z; dR.a[7] = r1.w; dR.a[8] = r2.x;
-  const double dpx = join2(r2.y, r2.z), dpy = join2(r3.x, r3.y), dpz = join2(r3.z, r3.w);
-#pragma unroll
-  for (int q = 0; q < 9; q++) R.a[q] = __ldg(g.R0 + (size_t)q * Np + i) + dR.a[q];
+  M3 R;                                   // world rotation of the link (phase A1): fp64 publish of an inner link, fp32 of a leaf
+  if ((tw >> kNcShift) & kNcMask) {
+    const double2 *pr = reinterpret_cast<const double2 *>(s.P + 7 * i);
+    const double2 a0 = pr[0], a1 = pr[1], a2 = pr[2], a3 = pr[6];
+    R.a[0] = (float)a0.x; R.a[1] = (float)a0.y; R.a[2] = (float)a1.x; R.a[3] = (float)a1.y; R.a[4] = (float)a2.x;
+    R.a[5] = (float)a2.y; R.a[6] = (float)a3.x; R.a[7] = (float)a3.y;
+    R.a[8] = (float)*reinterpret_cast<const double *>(s.G + i);
+  } else {
+    const float4 *rec = s.P + 7 * i;
+    const float4 r0 = rec[0], r1 = rec[1];
+    R.a[0] = r0.x; R.a[1] = r0.y; R.a[2] = r0.z; R.a[3] = r0.w;
+    R.a[4] = r1.x; R.a[5] = r1.y; R.a[6] = r1.z; R.a[7] = r1.w; R.a[8] = rec[2].x;
+  }
   const int4 t2 = __ldg(g.topo2 + i);
   const int ast = t2.x & 0xffff, nap = t2.x >> 16;
   const float eta_h = P.tether_implicit ? P.h : 0.f;
   for (int a = ast; a < ast + nap; a++) {
     if (!s.att[a]) continue;
     const float3 o = f3(s.ao[a], s.ao[Ap + a], s.ao[2 * Ap + a]);
-    const float3 dro = mul(dR, o);
-    const double dhx = dpx + (double)dro.x, dhy = dpy + (double)dro.y, dhz = dpz + (double)dro.z;   // x_hang - anchor
     const float ks = s.ak[a], cdamp = s.ac[a], ma = s.am[a];
-    // x_a - x_hang = u + sag - dh with the rest sag m g / k_s (u is stored relative to the rest position)
-    const float gk = ma / ks;
-    const float3 st = f3((float)((double)s.u[a] + ((double)(gk * P.gravity[0]) - dhx)),
-                         (float)((double)s.u[Ap + a] + ((double)(gk * P.gravity[1]) - dhy)),
-                         (float)((double)s.u[2 * Ap + a] + ((double)(gk * P.gravity[2]) - dhz)));
+    // x_a - x_hang = (anchor - x_hang) + sag + u: the apple is stored as u = x_a - (anchor + sag), sag = m g / k_s,
+    // and phase A1 left anchor - x_hang in fp64 (as two floats)
+    const double mk = (double)ma / (double)ks;
+    const float3 st = f3((float)(join2(s.hd[a], s.hd[Ap + a]) + (double)ma * (double)P.gravity[0] / (double)ks + (double)s.u[a]),
+                         (float)(join2(s.hd[2 * Ap + a], s.hd[3 * Ap + a]) + (double)ma * (double)P.gravity[1] / (double)ks + (double)s.u[Ap + a]),
+                         (float)(join2(s.hd[4 * Ap + a], s.hd[5 * Ap + a]) + (double)ma * (double)P.gravity[2] / (double)ks + (double)s.u[2 * Ap + a]));
+    (void)mk;
     const float3 vh = mul(R, vl + cross(om, o));                          // world velocity of the hang point
     const float3 fs = (-ks) * st;
     const float3 va = f3(s.v[a], s.v[Ap + a], s.v[2 * Ap + a]);
@@ -455,9 +466,12 @@ __device__ __forceinline__ void finish_bias(const Jt &j, const int i, const uint
                                             const Sm &s, const Gm &g, const DevCtx &c) {
   const ob_params &P = c.P;
   float4 *rec = s.P + 7 * i;
-  const float2 kq = s.G[i];
+  // spring-damper part of the rhs and of the diagonal (Eq. 4, PAPER.md:123); a ruptured joint has K = D = 0
+  const float2 th = __ldcg(g.q2 + i), w = __ldcg(g.w2 + i);
+  const float Kt = (tw & kRuptured) ? 0.f : __ldg(g.K + i), Dt = P.c_d * Kt;
+  const float2 kq = make_float2(Kt * th.x + (Dt + P.h * Kt) * w.x, Kt * th.y + (Dt + P.h * Kt) * w.y);
   s.G[i] = make_float2(P.h * (-(j.c2 * n.x + j.s2 * n.z) - kq.x), P.h * (-n.y - kq.y));
-  float dt0 = rec[2].w, dt1 = dt0;
+  float dt0 = (P.h * P.c_d + P.h * P.h) * Kt, dt1 = dt0;
   if (g.arm) {
     dt0 += __ldg(g.arm + i);
     dt1 += __ldg(g.arm + s.Np + i);
@@ -659,21 +673,24 @@ __device__ OB_COLD_ATTR void sweep_bias(const World *wd, const DevCtx &c, const 
   const Gm g = wd->g;
   const int nlev = wd->nlev, ntop = wd->ntop, tid = threadIdx.x;
   const int l_first_down = tid < 32 ? 0 : ntop - 1, l_last_up = tid < 32 ? 0 : ntop;
-  // ---- A0: per link, flat ----
+  // ---- A0: sin / cos of the joint angles in fp64, flat (the two double sincos are the expensive part of the FK and
+  //      depend on nothing but the link's own q: kept out of the level-by-level chain) ----
 #pragma unroll 1
-  for (int i0 = tid; i0 < wd->N; i0 += 2 * nt) {      // two links per trip: all their global loads are in flight
-    const int i1 = i0 + nt < wd->N ? i0 + nt : i0;     // together (a store in between would serialise the trips)
-    const PrepIn in0 = link_prepare_load(i0, s, g), in1 = link_prepare_load(i1, s, g);
-    link_prepare(i0, in0, s, c);
-    if (i1 != i0) link_prepare(i1, in1, s, c);
+  for (int i = tid; i < wd->N; i += nt) {
+    const float2 th = __ldcg(g.q2 + i);
+    double s1, c1, s2, c2;
+    sincos((double)th.x, &s1, &c1);
+    sincos((double)th.y, &s2, &c2);
+    double2 *pr = reinterpret_cast<double2 *>(s.P + 7 * i);
+    pr[0] = make_double2(s1, c1); pr[1] = make_double2(s2, c2);
   }
   __syncthreads();
-  // ---- A1: displacement-form FK, top-down ----
+  // ---- A1: forward kinematics in fp64, joint transforms, hang points, top-down ----
 #pragma unroll 1
   for (int l = l_first_down; l < nlev; l++) {
     const int le = s.lev[l + 1];
 #pragma unroll 1
-    for (int i = s.lev[l] + tid; i < le; i += nt) link_fk(i, s);
+    for (int i = s.lev[l] + tid; i < le; i += nt) link_fk(i, s, g);
     OB_FENCE_DOWN(l)
   }
   // ---- A2 (+ B1 for leaves): velocities, bias accelerations, bias forces, top-down ----
@@ -1048,7 +1065,8 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       g.c4 = reinterpret_cast<const float4 *>(cst);
       g.K = reinterpret_cast<const float *>(cst) + 4 * Np;
       g.rz = g.K + Np;
-      g.quat = c.quat + d.link_base;
+      g.quatd = reinterpret_cast<const double2 *>(c.quatd) + 2 * (size_t)d.link_base;
+      g.anchor = c.anchor + 3 * (size_t)d.apple_base;
       g.R0 = c.R0 + 9 * (size_t)d.link_base;
       g.Mmax = c.Mmax + d.link_base;
       g.mdiag = c.mdiag + d.link_base;
