@@ -304,6 +304,43 @@ __device__ __forceinline__ float2 split2(const double v) {
 }
 __device__ __forceinline__ double join2(const float hi, const float lo) { return (double)hi + (double)lo; }
 
+// ---- A0 ----  R_rel = Q Rx(th1) Ry(th2) of one link in fp64 -> the link's own record slots 0, 1, 2, 6 and G (they are
+//               free until the link's turn in A1); E = R_rel^T rounded to fp32, cos / sin th2 and the parent length
+//               -> C0..C2 for the dynamics
+__device__ __forceinline__ void link_joint(const int i, const Sm &s, const Gm &g) {
+  const float2 th = __ldcg(g.q2 + i);
+  const double2 qa = __ldg(g.quatd + 2 * i), qb = __ldg(g.quatd + 2 * i + 1);
+  const float rzf = (s.T[i] & kTrunk) ? 0.f : __ldg(g.rz + i);
+  double Q[9], X[9], Rrel[9];
+  {
+    const double w = qa.x, x = qa.y, y = qb.x, z = qb.y;
+    Q[0] = 1 - 2 * (y * y + z * z); Q[1] = 2 * (x * y - w * z);     Q[2] = 2 * (x * z + w * y);
+    Q[3] = 2 * (x * y + w * z);     Q[4] = 1 - 2 * (x * x + z * z); Q[5] = 2 * (y * z - w * x);
+    Q[6] = 2 * (x * z - w * y);     Q[7] = 2 * (y * z + w * x);     Q[8] = 1 - 2 * (x * x + y * y);
+  }
+  double s1, c1, s2, c2;
+  sincos((double)th.x, &s1, &c1);
+  sincos((double)th.y, &s2, &c2);
+  X[0] = c2;       X[1] = 0.0; X[2] = s2;                           // Rx(th1) Ry(th2)
+  X[3] = s1 * s2;  X[4] = c1;  X[5] = -s1 * c2;
+  X[6] = -c1 * s2; X[7] = s1;  X[8] = c1 * c2;
+#pragma unroll
+  for (int r = 0; r < 3; r++)
+#pragma unroll
+    for (int cc = 0; cc < 3; cc++) Rrel[3 * r + cc] = Q[3 * r] * X[cc] + Q[3 * r + 1] * X[3 + cc] + Q[3 * r + 2] * X[6 + cc];
+  Jt j;                                                              // E = Rrel^T, rounded once
+#pragma unroll
+  for (int r = 0; r < 3; r++)
+#pragma unroll
+    for (int cc = 0; cc < 3; cc++) j.E.a[3 * r + cc] = (float)Rrel[3 * cc + r];
+  j.c2 = (float)c2; j.s2 = (float)s2; j.rz = rzf;
+  store_jt(s.P, i, j);
+  double2 *pr = reinterpret_cast<double2 *>(s.P + 7 * i);
+  pr[0] = make_double2(Rrel[0], Rrel[1]); pr[1] = make_double2(Rrel[2], Rrel[3]); pr[2] = make_double2(Rrel[4], Rrel[5]);
+  pr[6] = make_double2(Rrel[6], Rrel[7]);
+  *reinterpret_cast<double *>(s.G + i) = Rrel[8];
+}
+
 // ---- A1 ----  forward kinematics in fp64 (Eq. 3): R_i = R_p Q_i Rx(th1) Ry(th2),
 //               p_i = p_p + R_p (0,0,L_p).  The tether stretch x_a - x_hang is a millimetre-sized difference of
 //               metre-sized positions, k_s = 2e3 N/m turns 1e-8 m of it into the whole error budget of a 3 mm twig:
@@ -315,36 +352,16 @@ __device__ __forceinline__ double join2(const float hi, const float lo) { return
 __device__ __forceinline__ void link_fk(const int i, const Sm &s, const Gm &g) {
   float4 *rec = s.P + 7 * i;
   uint32_t tw = s.T[i];
-  const double2 qa = __ldg(g.quatd + 2 * i), qb = __ldg(g.quatd + 2 * i + 1);
   const int4 t2 = __ldg(g.topo2 + i);
   const bool trunk = (tw & kTrunk) != 0u;
-  const float rzf = trunk ? 0.f : __ldg(g.rz + i);
-  double Q[9], X[9], Rrel[9];
+  double Rrel[9];                                   // Q Rx(th1) Ry(th2) in fp64: phase A0 left it in the link's own slots
   {
-    const double w = qa.x, x = qa.y, y = qb.x, z = qb.y;
-    Q[0] = 1 - 2 * (y * y + z * z); Q[1] = 2 * (x * y - w * z);     Q[2] = 2 * (x * z + w * y);
-    Q[3] = 2 * (x * y + w * z);     Q[4] = 1 - 2 * (x * x + z * z); Q[5] = 2 * (y * z - w * x);
-    Q[6] = 2 * (x * z - w * y);     Q[7] = 2 * (y * z + w * x);     Q[8] = 1 - 2 * (x * x + y * y);
+    const double2 *pr = reinterpret_cast<const double2 *>(rec);
+    const double2 a0 = pr[0], a1 = pr[1], a2 = pr[2], a3 = pr[6];
+    Rrel[0] = a0.x; Rrel[1] = a0.y; Rrel[2] = a1.x; Rrel[3] = a1.y; Rrel[4] = a2.x; Rrel[5] = a2.y; Rrel[6] = a3.x;
+    Rrel[7] = a3.y; Rrel[8] = *reinterpret_cast<const double *>(s.G + i);
   }
-  // sin / cos of the two joint angles in fp64: phase A0 left them in the link's own record slots 0, 1
-  const double2 sc1 = reinterpret_cast<const double2 *>(rec)[0], sc2 = reinterpret_cast<const double2 *>(rec)[1];
-  const double s1 = sc1.x, c1 = sc1.y, s2 = sc2.x, c2 = sc2.y;
-  X[0] = c2;       X[1] = 0.0; X[2] = s2;                           // Rx(th1) Ry(th2)
-  X[3] = s1 * s2;  X[4] = c1;  X[5] = -s1 * c2;
-  X[6] = -c1 * s2; X[7] = s1;  X[8] = c1 * c2;
-#pragma unroll
-  for (int r = 0; r < 3; r++)
-#pragma unroll
-    for (int cc = 0; cc < 3; cc++) Rrel[3 * r + cc] = Q[3 * r] * X[cc] + Q[3 * r + 1] * X[3 + cc] + Q[3 * r + 2] * X[6 + cc];
-  {
-    Jt j;                                                            // E = Rrel^T, rounded once
-#pragma unroll
-    for (int r = 0; r < 3; r++)
-#pragma unroll
-      for (int cc = 0; cc < 3; cc++) j.E.a[3 * r + cc] = (float)Rrel[3 * cc + r];
-    j.c2 = (float)c2; j.s2 = (float)s2; j.rz = rzf;
-    store_jt(s.P, i, j);
-  }
+  const float rzf = rec[5].w;                       // parent length (0 for the trunk), stored with E by phase A0
   double Rp[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1}, pp[3] = {0, 0, 0};
   uint32_t snapped_p = 0u;
   if (!trunk) {
@@ -673,17 +690,10 @@ __device__ OB_COLD_ATTR void sweep_bias(const World *wd, const DevCtx &c, const 
   const Gm g = wd->g;
   const int nlev = wd->nlev, ntop = wd->ntop, tid = threadIdx.x;
   const int l_first_down = tid < 32 ? 0 : ntop - 1, l_last_up = tid < 32 ? 0 : ntop;
-  // ---- A0: sin / cos of the joint angles in fp64, flat (the two double sincos are the expensive part of the FK and
+  // ---- A0: joint transforms in fp64, flat (the two double sincos and Q Rx Ry are the expensive part of the FK and
   //      depend on nothing but the link's own q: kept out of the level-by-level chain) ----
 #pragma unroll 1
-  for (int i = tid; i < wd->N; i += nt) {
-    const float2 th = __ldcg(g.q2 + i);
-    double s1, c1, s2, c2;
-    sincos((double)th.x, &s1, &c1);
-    sincos((double)th.y, &s2, &c2);
-    double2 *pr = reinterpret_cast<double2 *>(s.P + 7 * i);
-    pr[0] = make_double2(s1, c1); pr[1] = make_double2(s2, c2);
-  }
+  for (int i = tid; i < wd->N; i += nt) link_joint(i, s, g);
   __syncthreads();
   // ---- A1: forward kinematics in fp64, joint transforms, hang points, top-down ----
 #pragma unroll 1
