@@ -8,9 +8,8 @@
 // The apple block is staged by one TMA bulk copy (UBLKCP) and written back the same way; q, qd and the PCG start
 // vectors stay in global memory (L2): only the once-per-step phases touch them.
 //
-//   A0  flat:      joint transforms (Eq. 3), own part of the displacement-form FK, spring-damper
-//                  part of the rhs (Eq. 4)
-//   A1  top-down:  displacement-form FK (positions in fp64)
+//   A0  flat:      joint transforms R_rel = Q Rx Ry (Eq. 3) in fp64; E = R_rel^T rounded for the dynamics
+//   A1  top-down:  forward kinematics in fp64 (world rotations and positions), hang points of the apples
 //   A2  top-down:  velocities, bias accelerations, bias force of every link incl. tether reactions (Eq. 6 / Eq. 7,
 //                  PAPER.md:149-161) and user wrenches; leaves finish at once
 //   B1  bottom-up: bias torques of the inner links -> rhs b
@@ -28,13 +27,14 @@
 // once-per-step sweeps warp 0 takes the leading levels with __syncwarp and every leaf turns around.
 //
 // Record of link i (P[7 i + j]); record Np is never written and stays zero: the trunk's parent, missing children.
-//   0, 1  M0, M1   A0: R0 (RxRy - I); A1: dR; A2: parked bias force / (n, f) for the parent; B2: composite inertia
-//                  for the parent; C: (alpha, a) on the way down, (n, f) on the way up, A p in M1.zw
-//   2     PD       (p, diagonal terms arm + (h c_d + h^2) K); A1: dR[8], dp.x; B2 borrows .xy
+//   0, 1  M0, M1   A0: R_rel (fp64); A1: world rotation R (fp64 for an inner link, fp32 for a leaf); A2: parked bias
+//                  force / (n, f) for the parent; B2: composite inertia for the parent; C: (alpha, a) on the way
+//                  down, (n, f) on the way up, A p in M1.zw
+//   2     PD       (p, diagonal terms arm + (h c_d + h^2) K); A0, A1: more of R_rel, R; B2 borrows .xy
 //   3..5  C0..C2   E (parent -> link rotation, row-major), c2, s2, parent length
 //   6     C3       effective link inertia (m, m c, I about the joint, I_zz) incl. on-axis virtual tether masses
-//                  (A15); A1: dp.y, dp.z
-// Beside the records: G (float2: spring-damper rhs part, then b, then 1 / diag(A)), T (packed topology word:
+//                  (A15); A0, A1: the rest of R_rel, R
+// Beside the records: G (float2: the ninth entry of R_rel / R as a double, then b, then 1 / diag(A)), T (packed topology word:
 // parent | first child << 11 | children << 22 | flags), and one region shared by the A2 overflow (12 floats per
 // inner link: velocity and bias acceleration for the children) and the PCG's (x, r) (one float4 per link).
 //
@@ -271,9 +271,10 @@ __device__ __forceinline__ float mv_up(const Jt &j, float4 *P, const float4 *zer
 // ------------------------------------------------------------------------------------------------------
 // The once-per-step phases, cut into passes that each keep a small working set in registers (a spilled
 // register costs an L2 round trip here: the three CTAs of an SM leave the L1 only ~28 KB):
-//   A0  flat      per link, no dependence on other links: joint transform E (-> C0..C2), R0 (RxRy - I)
-//                 (-> M0, M1, PD.x), spring-damper part of the rhs (-> G), diagonal terms (-> PD.w)
-//   A1  top-down  displacement-form FK: dR, dp of every link (-> M0, M1, PD.xyz, C3), snapped flags
+//   A0  flat      per link, no dependence on other links: R_rel = Q Rx Ry in fp64 (-> slots 0, 1, 2, 6, G),
+//                 E = R_rel^T rounded (-> C0..C2)
+//   A1  top-down  FK in fp64: R, p of every link (an inner link publishes twelve doubles: slots 0, 1, 2, 6, G and the
+//                 overflow), hang points of the apples (-> hd), snapped flags
 //   A2  top-down  velocities and bias accelerations (inner links publish 12 floats in the overflow); own bias
 //                 force of every link incl. tethers and wrenches; a leaf finishes at once, an inner link
 //                 parks (n, f) in M0, M1.xy
