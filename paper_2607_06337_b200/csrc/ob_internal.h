@@ -134,7 +134,7 @@ inline int step_class_of(int Np) {   // host only
 //   seven float4 planes [S]: M0, M1 (parent <-> child mailboxes, A p), PD (p, diagonal terms), C0..C2 (joint
 //   transform E, c2, s2, parent length), C3 (effective link inertia) | G float2 [S] (b, then 1/diag) |
 //   T uint32 [S] (packed topology + flags) | overflow float4 [3][NIp] (phase A) | level offsets |
-//   apple block (TMA) | f_tether [3][Ap], |f_s| [Ap], anchor - x_hang [6][Ap] | wrench slots
+//   apple block (TMA) | six float planes [Ap]: anchor - x_hang (phase A1 -> A2), then f_tether, |f_s| (A2 -> D) | wrench slots
 __host__ __device__ inline int r16(int b) { return (b + 15) / 16 * 16; }
 __host__ __device__ inline int step_planes_bytes(int Np) { return 7 * 16 * (Np + 1); }
 // phase-A overflow (three float4 per inner link) and the PCG's (x, r) (one float4 per link) share one region
@@ -147,7 +147,7 @@ __host__ __device__ inline int step_smem_bytes(int Np, int Ap, int NIp, int nlev
   b += step_ovf_bytes(Np, NIp);
   b += r16(4 * (nlev + 1));
   b += r16(apple_block_bytes(Ap));
-  b += (3 + 1 + 6) * 4 * Ap;
+  b += 6 * 4 * Ap;
   b += (int)sizeof(WrenchSlots);
   return (b + 127) / 128 * 128;
 }

@@ -68,7 +68,8 @@ struct Sm {
   unsigned char *att, *cA, *cB;
   float *ao, *ak, *am, *ac, *afd;     // ao = [3][Ap]
   float *ft, *fsn;                    // tether force [3][Ap], |f_s| [Ap] (phase A2 -> phase D)
-  float *hd;                          // [6][Ap] anchor - x_hang of every apple, fp64 as (hi, lo) pairs (phase A1 -> A2)
+  float *hd;                          // [6][Ap] anchor - x_hang of every apple, fp64 as (hi, lo) pairs (phase A1 -> A2);
+                                      // aliases ft, fsn (see carve)
   WrenchSlots *wr;
 };
 
@@ -95,7 +96,7 @@ __device__ __forceinline__ Sm carve(unsigned char *base, const int Np, const int
   f = reinterpret_cast<float *>(p);
   s.ft = f; f += 3 * Ap;
   s.fsn = f; f += Ap;
-  s.hd = f; f += 6 * Ap;
+  s.hd = s.ft; f += 2 * Ap;             // hd[0..3] share the memory of ft[0..2], fsn: per apple, phase A2 reads hd, then writes them
   s.wr = reinterpret_cast<WrenchSlots *>(f);
   return s;
 }

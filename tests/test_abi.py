@@ -102,6 +102,10 @@ def test_capacity_limits_are_reported_not_crashed():
     assert rc == ob.OB_E_CAPACITY and "children" in msg
     rc, _, _ = _ws_bytes([ob_star_spec(16)], P)          # 15 children: fine
     assert rc == ob.OB_OK
+    # the largest worlds of BASELINE.json configs[4] (1500 links, 150 apples) must fit into one CTA's shared memory
+    from workloads import stochastic_world
+    big = stochastic_world(np.random.default_rng(3), 1497, 1500, 150, depth_choices=(7, 8))
+    assert big.n_links >= 1497 and _ws_bytes([big], config_params(5))[0] == ob.OB_OK
 
 
 def ob_star_spec(n_links):
