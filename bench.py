@@ -331,7 +331,7 @@ def cpu_baseline(specs, P, seed, f_lo, f_hi) -> dict:
     cores = _omp_threads()
     os.environ.setdefault("OMP_NUM_THREADS", str(cores))
     n_sample = int(min(max(cores, 8), 64, len(specs)))
-    n_steps = 4
+    n_steps = 8                                                  # ~1 s wall on 16 cores = 10-20 s of CPU work
     worlds = _oracle_sample(specs, P, seed, f_lo, f_hi, n_sample)
     oracle.step_many(worlds, 1)                                  # warm-up (page-in, first-touch)
     t0 = time.perf_counter()
