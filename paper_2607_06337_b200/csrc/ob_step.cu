@@ -419,9 +419,8 @@ __device__ __forceinline__ void link_fk(const int i, const Sm &s, const Gm &g) {
 // (Not inlined.  It takes the World in shared memory, not references to the caller's copies: a reference would
 // force those copies into local memory, and every pointer fetched from there is an L2 round trip.)
 __device__ __noinline__ Force6 external_forces(const int i, const float3 om, const float3 vl, const uint32_t tw,
-                                               const World *wd, const DevCtx &c) {
+                                               const int apples, const World *wd, const DevCtx &c) {
   const Sm s = carve(wd);
-  const Gm g = wd->g;
   const ob_params &P = c.P;
   const int Ap = s.Ap;
   Force6 out;
@@ -439,8 +438,7 @@ __device__ __noinline__ Force6 external_forces(const int i, const float3 om, con
     R.a[0] = r0.x; R.a[1] = r0.y; R.a[2] = r0.z; R.a[3] = r0.w;
     R.a[4] = r1.x; R.a[5] = r1.y; R.a[6] = r1.z; R.a[7] = r1.w; R.a[8] = rec[2].x;
   }
-  const int4 t2 = __ldg(g.topo2 + i);
-  const int ast = t2.x & 0xffff, nap = t2.x >> 16;
+  const int ast = apples & 0xffff, nap = apples >> 16;          // first apple | count << 16 (topo2.x, loaded by the caller)
   const float eta_h = P.tether_implicit ? P.h : 0.f;
   for (int a = ast; a < ast + nap; a++) {
     if (!s.att[a]) continue;
@@ -448,11 +446,10 @@ __device__ __noinline__ Force6 external_forces(const int i, const float3 om, con
     const float ks = s.ak[a], cdamp = s.ac[a], ma = s.am[a];
     // x_a - x_hang = (anchor - x_hang) + sag + u: the apple is stored as u = x_a - (anchor + sag), sag = m g / k_s,
     // and phase A1 left anchor - x_hang in fp64 (as two floats)
-    const double mk = (double)ma / (double)ks;
-    const float3 st = f3((float)(join2(s.hd[a], s.hd[Ap + a]) + (double)ma * (double)P.gravity[0] / (double)ks + (double)s.u[a]),
-                         (float)(join2(s.hd[2 * Ap + a], s.hd[3 * Ap + a]) + (double)ma * (double)P.gravity[1] / (double)ks + (double)s.u[Ap + a]),
-                         (float)(join2(s.hd[4 * Ap + a], s.hd[5 * Ap + a]) + (double)ma * (double)P.gravity[2] / (double)ks + (double)s.u[2 * Ap + a]));
-    (void)mk;
+    const double mk = (double)ma / (double)ks;               // one fp64 division; sag = (m / k_s) g to ~1e-19 m of m g / k_s
+    const float3 st = f3((float)(join2(s.hd[a], s.hd[Ap + a]) + mk * (double)P.gravity[0] + (double)s.u[a]),
+                         (float)(join2(s.hd[2 * Ap + a], s.hd[3 * Ap + a]) + mk * (double)P.gravity[1] + (double)s.u[Ap + a]),
+                         (float)(join2(s.hd[4 * Ap + a], s.hd[5 * Ap + a]) + mk * (double)P.gravity[2] + (double)s.u[2 * Ap + a]));
     const float3 vh = mul(R, vl + cross(om, o));                          // world velocity of the hang point
     const float3 fs = (-ks) * st;
     const float3 va = f3(s.v[a], s.v[Ap + a], s.v[2 * Ap + a]);
@@ -481,13 +478,14 @@ __device__ __noinline__ Force6 external_forces(const int i, const float3 om, con
 
 // project the accumulated bias force on the joint axes -> rhs b (G[i]), the diagonal terms of both DoF (PD[i].zw),
 // and publish (n, f) in the parent frame (M0[i], M1[i].xy)
-__device__ __forceinline__ void finish_bias(const Jt &j, const int i, const uint32_t tw, float3 n, float3 f,
-                                            const Sm &s, const Gm &g, const DevCtx &c) {
+// (th, w, Ki = q, qd, K of the joint: the caller loads them at the top of its turn, with its other global inputs)
+__device__ __forceinline__ void finish_bias(const Jt &j, const int i, const uint32_t tw, const float2 th, const float2 w,
+                                            const float Ki, float3 n, float3 f, const Sm &s, const Gm &g,
+                                            const DevCtx &c) {
   const ob_params &P = c.P;
   float4 *rec = s.P + 7 * i;
   // spring-damper part of the rhs and of the diagonal (Eq. 4); a ruptured joint has K = D = 0
-  const float2 th = __ldcg(g.q2 + i), w = __ldcg(g.w2 + i);
-  const float Kt = (tw & kRuptured) ? 0.f : __ldg(g.K + i), Dt = P.c_d * Kt;
+  const float Kt = (tw & kRuptured) ? 0.f : Ki, Dt = P.c_d * Kt;
   const float2 kq = make_float2(Kt * th.x + (Dt + P.h * Kt) * w.x, Kt * th.y + (Dt + P.h * Kt) * w.y);
   s.G[i] = make_float2(P.h * (-(j.c2 * n.x + j.s2 * n.z) - kq.x), P.h * (-n.y - kq.y));
   float dt0 = (P.h * P.c_d + P.h * P.h) * Kt, dt1 = dt0;
@@ -511,9 +509,11 @@ __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm
   const ob_params &P = c.P;
   const int NIp = s.NIp;
   const uint32_t tw = s.T[i];
-  const float2 w = __ldcg(g.w2 + i);
+  const float2 w = __ldcg(g.w2 + i), th = __ldcg(g.q2 + i);       // all global inputs of the link's turn at once
   const float4 c4 = __ldg(g.c4 + i);
-  const int ty = __ldg(&g.topo2[i].y);                            // inner slot | parent's inner slot << 16
+  const float Ki = __ldg(g.K + i);
+  const int4 t2g = __ldg(g.topo2 + i);
+  const int ty = t2g.y;                                           // inner slot | parent's inner slot << 16
   const Jt j = load_jt(s.P, i);
   float3 wp = f3(0, 0, 0), vp = f3(0, 0, 0), alp = f3(0, 0, 0);
   float3 ap = f3(-P.gravity[0], -P.gravity[1], -P.gravity[2]);   // world = parent of the trunk: at rest, (0; -g)
@@ -550,24 +550,26 @@ __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm
   bool ext = (tw & kHasApples) != 0u;
   for (int q = 0; q < s.wr->n; q++) ext |= s.wr->body[q] == i;
   if (ext) {
-    const Force6 e = external_forces(i, om, vl, tw, wd, c);
+    const Force6 e = external_forces(i, om, vl, tw, t2g.x, wd, c);
     n = n + e.n; f = f + e.f;
   }
   if (inner) {                                                    // parked until B1 adds the children
     s.P[7 * i] = make_float4(n.x, n.y, n.z, f.x);
     *reinterpret_cast<float2 *>(s.P + 7 * i + 1) = make_float2(f.y, f.z);
   } else {
-    finish_bias(j, i, tw, n, f, s, g, c);
+    finish_bias(j, i, tw, th, w, Ki, n, f, s, g, c);
   }
 }
 
 // ---- B1 ----  one inner link: its parked bias force plus what its children sent up
 __device__ __forceinline__ void link_bias_up(const int i, const uint32_t tw, const Sm &s, const Gm &g, const DevCtx &c) {
+  const float2 th = __ldcg(g.q2 + i), w = __ldcg(g.w2 + i);
+  const float Ki = __ldg(g.K + i);
   const float4 u0 = s.P[7 * i];
   const float2 v0 = *reinterpret_cast<const float2 *>(s.P + 7 * i + 1);
   float3 n = f3(u0.x, u0.y, u0.z), f = f3(u0.w, v0.x, v0.y);
   gather_children(s.P, s.P + 7 * s.Np, (int)((tw >> kChShift) & kParMask), (int)((tw >> kNcShift) & kNcMask), n, f);
-  finish_bias(load_jt(s.P, i), i, tw, n, f, s, g, c);
+  finish_bias(load_jt(s.P, i), i, tw, th, w, Ki, n, f, s, g, c);
 }
 
 // ------------------------------------------------------------------------------------------------------
