@@ -157,7 +157,7 @@ inline int pad8(int n) { return (n + 7) / 8 * 8; }
 
 struct Layout {
   size_t total = 0;
-  Pool desc, order, link_blk, apple_blk, topo, topo2, child_list, quat, quat_raw, quatd, R0, Mmax, mdiag, xprev, Lown, diam, arm, link_ext, apple_ext, apple_nom,
+  Pool desc, order, link_blk, apple_blk, topo, topo2, child_list, quat_raw, quatd, Mmax, mdiag, xprev, Lown, diam, arm, link_ext, apple_ext, apple_nom,
       apple_c, anchor, level_off, info, wrench, events, ev_count, queue, progress, pose7;
   size_t sumNp = 0, sumAp = 0, sumLev = 0, ev_cap = 0;
   int max_Np = 0, max_Ap = 0, max_smem = 0;
@@ -211,10 +211,8 @@ int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) 
   take(L, L.topo, sizeof(int4) * L.sumNp);
   take(L, L.topo2, sizeof(int4) * L.sumNp);
   take(L, L.child_list, sizeof(int32_t) * L.sumNp);
-  take(L, L.quat, sizeof(float4) * L.sumNp);
   take(L, L.quat_raw, sizeof(float4) * L.sumNp);
   take(L, L.quatd, sizeof(double) * 4 * L.sumNp);
-  take(L, L.R0, sizeof(float) * 9 * L.sumNp);
   take(L, L.Mmax, sizeof(float) * L.sumNp);
   take(L, L.mdiag, sizeof(float2) * L.sumNp);
   take(L, L.xprev, sizeof(float2) * 4 * L.sumNp);
@@ -350,7 +348,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   std::vector<unsigned char> h_link(L.link_blk.bytes, 0), h_apple(L.apple_blk.bytes, 0);
   std::vector<int4> h_topo(L.sumNp, make_int4(-1, -1, -1, 0xfff)), h_topo2(L.sumNp, make_int4(0, -1, 0, 0));
   std::vector<int32_t> h_child(L.sumNp, 0);
-  std::vector<float4> h_quat(L.sumNp, make_float4(1.f, 0.f, 0.f, 0.f)), h_quat_raw(L.sumNp, make_float4(1.f, 0.f, 0.f, 0.f));
+  std::vector<float4> h_quat_raw(L.sumNp, make_float4(1.f, 0.f, 0.f, 0.f));
   std::vector<float> h_Lown(L.sumNp, 1.f), h_diam(L.sumNp, 1.f), h_arm(L.any_arm ? 2 * L.sumNp : 0, 0.f);
   std::vector<int32_t> h_link_ext(L.sumNp, 0), h_apple_ext(std::max<size_t>(L.sumAp, 16), 0), h_lev(L.sumLev, 0);
   std::vector<float> h_nom(2 * std::max<size_t>(L.sumAp, 16), 0.f), h_c(std::max<size_t>(L.sumAp, 16), 0.f);
@@ -413,7 +411,6 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
                                          islot[i] | ((p >= 0 ? islot[p] : 0xffff) << 16), cl_off[i], n_child[i]);
       const float *q = s.rest_quat + 4 * e;
       const double n = std::sqrt((double)q[0] * q[0] + (double)q[1] * q[1] + (double)q[2] * q[2] + (double)q[3] * q[3]);
-      h_quat[link_base + i] = make_float4((float)(q[0] / n), (float)(q[1] / n), (float)(q[2] / n), (float)(q[3] / n));
       h_quat_raw[link_base + i] = make_float4(q[0], q[1], q[2], q[3]);
       h_Lown[link_base + i] = s.length[e];
       h_diam[link_base + i] = s.diameter[e];
@@ -464,10 +461,8 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   D.topo = reinterpret_cast<int4 *>(base + L.topo.off);
   D.topo2 = reinterpret_cast<int4 *>(base + L.topo2.off);
   D.child_list = reinterpret_cast<int32_t *>(base + L.child_list.off);
-  D.quat = reinterpret_cast<float4 *>(base + L.quat.off);
   D.quat_raw = reinterpret_cast<float4 *>(base + L.quat_raw.off);
   D.quatd = reinterpret_cast<double *>(base + L.quatd.off);
-  D.R0 = reinterpret_cast<float *>(base + L.R0.off);
   D.Mmax = reinterpret_cast<float *>(base + L.Mmax.off);
   D.mdiag = reinterpret_cast<float2 *>(base + L.mdiag.off);
   D.xprev = reinterpret_cast<float2 *>(base + L.xprev.off);
@@ -503,7 +498,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   cudaError_t e = cudaMemsetAsync(base, 0, L.total, ctx->stream);
   if (e != cudaSuccess) { g_err = cudaGetErrorString(e); delete ctx; return OB_E_CUDA; }
   UP(L.desc, ctx->desc); UP(L.order, h_order); UP(L.link_blk, h_link); UP(L.apple_blk, h_apple); UP(L.topo, h_topo); UP(L.topo2, h_topo2); UP(L.child_list, h_child);
-  UP(L.quat, h_quat); UP(L.quat_raw, h_quat_raw); UP(L.Lown, h_Lown); UP(L.diam, h_diam); UP(L.arm, h_arm); UP(L.link_ext, h_link_ext);
+  UP(L.quat_raw, h_quat_raw); UP(L.Lown, h_Lown); UP(L.diam, h_diam); UP(L.arm, h_arm); UP(L.link_ext, h_link_ext);
   UP(L.apple_ext, h_apple_ext); UP(L.apple_nom, h_nom); UP(L.apple_c, h_c); UP(L.level_off, h_lev);
 #undef UP
   e = cudaStreamSynchronize(ctx->stream);   // the host images die at the end of this call

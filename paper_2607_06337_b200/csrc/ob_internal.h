@@ -77,10 +77,8 @@ struct DevCtx {
   const int4 *topo2;             // x = first apple | n_apples << 16, y = inner slot | parent's inner slot << 16,
                                  // z = offset of this link's children in child_list, w = n_children
   const int32_t *child_list;     // [link_base + z + c] children of every link (internal indices), CSR
-  const float4 *quat;            // rest quaternion (w,x,y,z), normalised in fp64 then rounded (k_step)
   const float4 *quat_raw;        // rest quaternion exactly as the caller gave it (create-time fp64 rest pose)
   double *quatd;                 // [4 * (link_base + i)] the same, normalised, in fp64 (k_rest_pose; the FK of k_step)
-  float *R0;                     // [9 * link_base + k * Np + i] rest world rotation, row-major k
   float *Mmax;                   // rupture moment (after randomize)
   float2 *mdiag;                 // [link_base + i] diag(M) of the two DoF as last computed by phase B2
   float2 *xprev;                 // [4][sumNp]: dqd of the last four steps, slot = step & 3 (PCG start: extrapolation)

@@ -37,8 +37,9 @@ __device__ __forceinline__ float philox_uniform(uint32_t x, float lo, float hi) 
 }
 
 // ------------------------------------------------------------------------------------------------------
-// k_rest_pose: one CTA per world.  R0_i = Q_0 ... Q_i and anchor_a = p0_b + R0_b o by walking up the
-// ancestors in fp64 (create-time only; Eq. 3).
+// k_rest_pose: one CTA per world.  The rest quaternion of every link normalised in fp64 (the FK of k_step starts from
+// it) and anchor_a = p0_b + R0_b o of every apple by walking up the ancestors in fp64 (create-time only; Eq. 3,
+// PAPER.md:115).
 // ------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void quat_to_mat_d(float4 q, double *R) {   // normalises in fp64
   double w = q.x, x = q.y, y = q.z, z = q.w;
@@ -55,15 +56,6 @@ __global__ void k_rest_pose(DevCtx c) {
   const float4 *quat = c.quat_raw + d.link_base;   // the caller's quaternions, normalised in fp64 here
   const float *Lown = c.Lown + d.link_base;
   for (int i = threadIdx.x; i < d.N; i += blockDim.x) {
-    double R[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1};
-    for (int j = i; j >= 0; j = topo[j].x) {
-      double Q[9], T[9];
-      quat_to_mat_d(quat[j], Q);
-      for (int r = 0; r < 3; r++)
-        for (int cc = 0; cc < 3; cc++) T[3 * r + cc] = Q[3 * r] * R[cc] + Q[3 * r + 1] * R[3 + cc] + Q[3 * r + 2] * R[6 + cc];
-      for (int k = 0; k < 9; k++) R[k] = T[k];
-    }
-    for (int k = 0; k < 9; k++) c.R0[9 * (size_t)d.link_base + (size_t)k * d.Np + i] = (float)R[k];
     {                                           // the link's own rest quaternion, normalised in fp64, for the FK of k_step
       const float4 q = quat[i];
       const double w = q.x, x = q.y, y = q.z, z = q.w, n = sqrt(w * w + x * x + y * y + z * z);

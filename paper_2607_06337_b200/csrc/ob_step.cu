@@ -109,7 +109,6 @@ struct Gm {
   const float *K, *rz;              // joint stiffness (Eq. 4), parent length
   const double2 *quatd;             // rest quaternions, normalised, fp64: (w, x), (y, z) of link i at 2 i, 2 i + 1
   const double *anchor;             // [k * Ap + a] rest hang points, world frame, fp64
-  const float *R0;                  // [k * Np + i]
   const float *Mmax;
   float2 *mdiag;                    // diag(M) as last computed by phase B2 (the Jacobi preconditioner may lag)
   float2 *hist;                     // [4][sum_np]: dqd of the last four steps, slot = step & 3
@@ -1081,7 +1080,6 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       g.rz = g.K + Np;
       g.quatd = reinterpret_cast<const double2 *>(c.quatd) + 2 * (size_t)d.link_base;
       g.anchor = c.anchor + 3 * (size_t)d.apple_base;
-      g.R0 = c.R0 + 9 * (size_t)d.link_base;
       g.Mmax = c.Mmax + d.link_base;
       g.mdiag = c.mdiag + d.link_base;
       g.hist = c.xprev + d.link_base;
