@@ -12,6 +12,13 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
 
 
+def pytest_sessionstart(session):
+    """Build the C-ABI CUDA library in-tree if it is missing or older than its sources (nvcc cross-compiles without a
+    GPU); the oracle builds itself on first use.  A failing build fails the session loudly: there is no fallback."""
+    from paper_2607_06337_b200 import build as ob_build
+    ob_build.build()
+
+
 def pytest_collection_modifyitems(config, items):
     """GPU tests are skipped (not failed) on a machine without a device."""
     try:
