@@ -704,3 +704,135 @@ def test_ternary_lsystem_body_count_and_oracle_rest():
     ow.step(5)
     s = ow.get_state()
     assert np.abs(s["q"]).max() < 1e-12 and np.abs(s["qd"]).max() < 1e-10
+
+
+# ---------------------------------------------------------------- Eq. 7 clamp, implicit-tether term, speed clamp, wrench slots
+def _fd_jacobian(spec, q, link, offset, eps=1e-6):
+    """3 x n Jacobian of the world position of a link-fixed point, by central differences of the scipy FK."""
+    n = 2 * spec.n_links
+    J = np.zeros((3, n))
+    o = np.asarray(offset, dtype=np.float64)
+    for j in range(n):
+        dq = np.zeros(n)
+        dq[j] = eps
+        Rp, pp = _numpy_fk(spec, q + dq)
+        Rm, pm = _numpy_fk(spec, q - dq)
+        J[:, j] = ((pp[link] + Rp[link] @ o) - (pm[link] + Rm[link] @ o)) / (2 * eps)
+    return J
+
+
+def _tether_rhs(spec, P, q, qd, apple_x):
+    """b(tree with the apple) - b(the same tree without it): the generalized force of the tether reaction times h."""
+    w1 = OracleWorld(spec, P)
+    w1.set_state(q=q, qd=qd, apple_x=apple_x)
+    w0 = OracleWorld(strip_apples(spec), P)
+    w0.set_state(q=q, qd=qd)
+    return w1.system()[1] - w0.system()[1]
+
+
+def test_tether_reaction_norm_clamp_at_react_max():
+    """Eq. 7 + PAPER.md:161 (A13): f_react = k_s (x_a - x_hang) + m g zhat, clamped in NORM to react_max = 40 N.
+    b_with - b_without = h J^T f_react with J the finite-difference Jacobian of the hang point.
+    (Perturbations this fails on: no clamp; a component-wise clamp; clamping before adding m g.)"""
+    mA, ks, off = 0.2, 2e3, (0.01, -0.02, 0.13)
+    spec = chain_spec(3, 0.9, 0.03, root_quat=quat_axis("y", 70.0), apples=[(2, off, mA, ks, 20.0)])
+    P = Params(h=2e-3, react_max=40.0)
+    h = float(np.float32(P.h))
+    rng = np.random.default_rng(12)
+    q = rng.uniform(-0.15, 0.15, size=6)
+    R, p = _numpy_fk(spec, q)
+    xh = p[2] + R[2] @ np.array(off, dtype=np.float64)
+    J = _fd_jacobian(spec, q, 2, off)
+    d = np.array([0.6, -0.3, 0.74])
+    d /= np.linalg.norm(d)
+    for stretch, clamped in ((0.004, False), (0.0185, False), (0.0215, True), (0.05, True)):
+        x_a = xh + stretch * d
+        f = ks * (x_a - xh) + np.array([0.0, 0.0, mA * G])
+        assert (np.linalg.norm(f) > 40.0) == clamped
+        if clamped:
+            f = f * (40.0 / np.linalg.norm(f))
+        db = _tether_rhs(spec, P, q, np.zeros(6), [x_a])
+        assert np.abs(db - h * J.T @ f).max() < 2e-7 * np.abs(db).max(), (stretch, db, h * J.T @ f)
+
+
+def test_implicit_tether_term_eta_h_v_hang():
+    """A15: the reaction is taken at the hang point advanced by eta h v_hang, v_hang = J qd (point_velocity).
+    The tether part of b changes with qd by exactly -h^2 k_s J^T J qd in implicit mode and by 0 with
+    tether_implicit = 0.  (Perturbations this fails on: the sign of the term; v_hang of the link origin instead of
+    the hang point; a missing ancestor in the velocity sum.)"""
+    mA, ks, off = 0.2, 2e3, (0.015, 0.01, 0.11)
+    spec = chain_spec(3, 0.9, 0.03, root_quat=quat_axis("y", 70.0), apples=[(2, off, mA, ks, 20.0)])
+    rng = np.random.default_rng(13)
+    q = rng.uniform(-0.15, 0.15, size=6)
+    qd = rng.uniform(-0.8, 0.8, size=6)
+    R, p = _numpy_fk(spec, q)
+    xh = p[2] + R[2] @ np.array(off, dtype=np.float64)
+    x_a = xh + np.array([0.001, -0.002, -0.0015])            # 5 N of stretch: far below the clamp
+    J = _fd_jacobian(spec, q, 2, off)
+    for eta in (1, 0):
+        P = Params(h=2e-3, tether_implicit=eta)
+        h = float(np.float32(P.h))
+        diff = _tether_rhs(spec, P, q, qd, [x_a]) - _tether_rhs(spec, P, q, np.zeros(6), [x_a])
+        expect = -eta * h * h * ks * (J.T @ (J @ qd))
+        scale = h * h * ks * np.abs(J.T @ (J @ qd)).max()
+        assert np.abs(diff - expect).max() < 1e-6 * scale, (eta, diff, expect)
+
+
+def test_joint_speed_clamp_componentwise_and_q_uses_the_clamped_speed():
+    """A16: qd+ = clamp(qd + dqd, +-qd_max) component-wise, q+ = q + h qd+ with the clamped value.
+    The unclamped update comes from a twin world with the clamp disabled.  (Perturbations this fails on: no clamp;
+    a norm clamp over the two DoF of a joint; q advanced with the unclamped speed.)"""
+    spec = chain_spec(2, 0.6, 0.004, root_quat=quat_axis("x", -90.0), E=2e8)
+    q0 = np.array([0.02, -0.01, 0.03, 0.015])
+    qd0 = np.array([56.0, -12.0, -61.0, 49.0])
+    free = OracleWorld(spec, Params(h=2e-3, qd_max=0.0))
+    free.set_state(q=q0, qd=qd0)
+    free.step(1)
+    v = free.get_state()["qd"]
+    assert (np.abs(v) > 50.0).sum() >= 2 and (np.abs(v) < 50.0).sum() >= 1     # the case exercises both branches
+    w = OracleWorld(spec, Params(h=2e-3, qd_max=50.0))
+    w.set_state(q=q0, qd=qd0)
+    w.step(1)
+    s = w.get_state()
+    vc = np.clip(v, -50.0, 50.0)
+    assert np.abs(s["qd"] - vc).max() == 0.0
+    assert np.abs(s["q"] - (q0 + float(np.float32(2e-3)) * vc)).max() < 1e-15
+
+
+def test_wrench_slot_semantics():
+    """a wrench persists, a second one on the same body REPLACES it, a zero force frees the slot,
+    distinct bodies superpose, a ninth distinct body is refused (rc -2) until a slot is freed.  Checked on the
+    right-hand side b, which is affine in the applied forces."""
+    spec = binary_tree_config1()
+    P = config_params(1)
+    w = OracleWorld(spec, P)
+    rng = np.random.default_rng(14)
+    q = rng.uniform(-0.05, 0.05, size=2 * spec.n_links)
+
+    def rhs(loads):
+        x = OracleWorld(spec, P)
+        x.set_state(q=q)
+        for (body, pt, f) in loads:
+            x.apply_wrench(body, pt, f)
+        return x.system()[1]
+    b0 = rhs([])
+    F1, F2 = (5.0, -3.0, 2.0), (-1.0, 4.0, 6.0)
+    b1 = rhs([(4, (0, 0, 0.2), F1)])
+    b2 = rhs([(9, (0.01, 0, 0.1), F2)])
+    assert np.abs(b1 - b0).max() > 1e-6 and np.abs(b2 - b0).max() > 1e-6
+    assert np.abs(rhs([(4, (0, 0, 0.2), F2), (4, (0, 0, 0.2), F1)]) - b1).max() < 1e-15        # replace, not add
+    assert np.abs(rhs([(4, (0, 0, 0.2), F1), (4, (0, 0, 0), (0, 0, 0))]) - b0).max() == 0.0     # zero frees
+    both = rhs([(4, (0, 0, 0.2), F1), (9, (0.01, 0, 0.1), F2)])
+    assert np.abs((both - b0) - ((b1 - b0) + (b2 - b0))).max() < 1e-12 * np.abs(both).max()     # distinct bodies add
+    for body in range(8):
+        w.apply_wrench(body, (0, 0, 0.1), (1.0, 0, 0))
+    w.apply_wrench(3, (0, 0, 0.1), (2.0, 0, 0))                  # same body: no new slot
+    with pytest.raises(RuntimeError):
+        w.apply_wrench(20, (0, 0, 0.1), (1.0, 0, 0))             # ninth distinct body
+    w.apply_wrench(0, (0, 0, 0), (0, 0, 0))
+    w.apply_wrench(20, (0, 0, 0.1), (1.0, 0, 0))                 # fits after the free
+    with pytest.raises(RuntimeError):
+        w.apply_wrench(spec.n_links + spec.n_apples, (0, 0, 0), (1.0, 0, 0))   # body out of range
+    # a wrench on an apple is a force on the apple, not on the tree: b is unchanged, the apple accelerates
+    ba = rhs([(spec.n_links + 1, (0, 0, 0), (0.0, 3.0, 0.0))])
+    assert np.abs(ba - b0).max() == 0.0
