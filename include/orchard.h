@@ -108,65 +108,114 @@ typedef struct {
   float value, threshold;       /* rupture: K|theta| vs M_max; detach: |f_user| vs f_detach or |f_s| vs kappa f_detach */
 } ob_event;
 
-/* Fill *p with the defaults above.  Returns OB_E_ARG for NULL. */
+/* Fill *p with the defaults above (the readings A1..A33 of DESIGN.md section 3).  Returns OB_E_ARG for NULL. */
 int ob_default_params(ob_params *p);
 
-/* Bytes of device workspace ob_create needs for these worlds (validates the specs). */
+/* Bytes of device workspace ob_create needs for these worlds (validates the specs).
+   [north_star: "PyTorch is used only for device memory and streams": the library allocates no device memory] */
 int ob_workspace_bytes(const ob_world_spec *specs, int n_worlds, const ob_params *params, size_t *out);
 
-/* Build the device layout (level-ordered SoA per world), compute rest poses and derived constants, reset the
-   state to the rest pose (apples at their rest sag m g / k_s below the hang point).  dev_workspace: device
-   memory of at least ob_workspace_bytes bytes; cuda_stream: cudaStream_t (NULL = default stream). */
+/* north_star "ob_create(world specs: parent arrays, link lengths/diameters/densities, E, MOR, apple attachments)".
+   Builds the articulation of PAPER.md:113-117 (Eq. 3: joint at the parent's distal tip (0,0,l_parent), rest rotation
+   q_rel, trunk base fixed) as a level-ordered SoA per world, computes rest poses and the derived constants of Eq. 4
+   (K = E pi d^4 / (64 l)) and Eq. 5 (M_max = MOR pi d^3 / 32), and resets the state to
+   the rest pose with every apple at its rest sag m g / k_s below its hang point.
+   dev_workspace: device memory of at least ob_workspace_bytes bytes, 256-byte aligned, owned by the caller and alive
+   until ob_destroy; cuda_stream: cudaStream_t (NULL = default stream).  Errors: OB_E_ARG (null, non-topological
+   parent, non-unit quaternion, non-positive dimension), OB_E_CAPACITY (a world does not fit on chip, > 15 children
+   on one link), OB_E_WORKSPACE, OB_E_CUDA (no device: there is no CPU fallback). */
 int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params, void *dev_workspace,
               size_t workspace_bytes, void *cuda_stream, ob_ctx **out);
 
-/* On-device Philox4x32-10 redraw of every world (key = seed; counter = (world, item, stream, 0); stream 0 item 0
-   -> E, MOR, density; stream 1 item a -> detach force, mass of apple a; u = float(x>>8) 2^-24,
-   value = fmaf(u, hi-lo, lo)), then derived constants and a full reset: rest pose, zero velocities, flags,
-   counters, step = 0, wrench slots cleared, warm start cleared.  Pending events stay queued.  Asynchronous. */
+/* north_star "ob_randomize(seed)": per-environment domain randomization of PAPER.md:165-169 ("wood density, Young's
+   modulus and rupture stress; fruit ... mass") drawn ON THE DEVICE with Philox4x32-10 (key = seed; counter =
+   (world, item, stream, 0); stream 0 item 0 -> E, MOR, density; stream 1 item a -> detach force, mass of apple a;
+   u = float(x>>8) 2^-24, value = fmaf(u, hi-lo, lo); reading A23), then the derived constants of Eq. 4 / Eq. 5 and a
+   full reset: rest pose, zero velocities, flags, counters, step = 0, wrench slots cleared, warm start cleared.
+   Pending events stay queued.  Asynchronous. */
 int ob_randomize(ob_ctx *ctx, uint64_t seed);
 
-/* Persistent external force.  body in [0, n_links) is a link, [n_links, n_links + n_apples) an apple.
-   point: application point in the link's local frame (moves with the link; ignored for apples).
-   force: world frame, N.  The wrench persists until replaced (same body) or removed (zero force).
-   Each world has OB_MAX_WRENCH slots; one more distinct body returns OB_E_CAPACITY. */
+/* north_star "ob_apply_wrench(world, body, point, force)": a persistent external force ("applied and interactive
+   forces").  body in [0, n_links) is a link, [n_links, n_links + n_apples) an apple (a pull on the
+   fruit: the "direct pull force" of the first detachment path).  point: application point in the link's
+   local frame (moves with the link; ignored for apples, which do not rotate).  force: world frame, N.
+   The wrench persists until replaced (same body) or removed (zero force).  Each world has OB_MAX_WRENCH slots; one
+   more distinct body returns OB_E_CAPACITY.  Wrenches on links at or below a ruptured joint are ignored while
+   forces_off_on_snapped is set.  Host-side bookkeeping; uploaded by the next ob_step / ob_flush. */
 int ob_apply_wrench(ob_ctx *ctx, int world, int body, const float point[3], const float force[3]);
+/* The same for n wrenches: world[n], body[n], point3[3n] (or NULL), force3[3n] host arrays. */
 int ob_apply_wrench_batch(ob_ctx *ctx, int n, const int32_t *world, const int32_t *body, const float *point3,
                           const float *force3);
 
 /* Upload wrenches applied since the last ob_step / ob_flush now (asynchronous; ob_step does it implicitly). */
 int ob_flush(ob_ctx *ctx);
 
-/* Advance every world by n steps (one persistent kernel launch per size class; worlds stay on chip for the
-   n steps).  Asynchronous.  Events are appended to the device event list. */
+/* north_star "ob_step(n)": advance every world by n steps of the batched physics step -- forward kinematics over the
+   level-ordered tree (Eq. 3); tether forces and clamped reaction (Eq. 6, Eq. 7);
+   spring-damper torques (Eq. 4); the implicit velocity update (M + hD + h^2 K) dqd = rhs by
+   matrix-free preconditioned conjugate gradient with M v from inverse-dynamics tree sweeps (north_star; PAPER.md:185,
+   265 "the matrix-free CG solve"); integration; in-place rupture (Eq. 5: "zero the broken degrees
+   of freedom's gain ... in place") and detachment ("a single flag flip") -- in one persistent kernel
+   launch per size class, worlds staying on chip for the n steps.  Asynchronous.  Events are appended to the device
+   event list; a world whose state goes non-finite is frozen and flagged (OB_STATUS_NONFINITE). */
 int ob_step(ob_ctx *ctx, int n);
 
-/* Copy one world's state out (synchronises).  Any output pointer may be NULL.
-   q, qd: [2*n_links] (theta_1, theta_2 per link); apple_x, apple_v: [3*n_apples] world frame;
-   ruptured: [n_links]; attached: [n_apples]; link_pose7: [7*n_links] (x,y,z, qw,qx,qy,qz) of each link frame;
+/* north_star "ob_get_state".  Copy one world's state out (synchronises once).  Any output pointer may be NULL.
+   q, qd: [2*n_links] (theta_1, theta_2 per link: the two bending DoF of PAPER.md:121); apple_x, apple_v:
+   [3*n_apples] world frame (3-DoF fruit); ruptured: [n_links] (Eq. 5); attached: [n_apples]
+   (PAPER.md:163); link_pose7: [7*n_links] (x,y,z, qw,qx,qy,qz) of each link frame (Eq. 3);
    info: [3] = step, PCG iterations of the last step, status bits (OB_STATUS_*). */
 int ob_get_state(ob_ctx *ctx, int world, float *q, float *qd, float *apple_x, float *apple_v, uint8_t *ruptured,
                  uint8_t *attached, float *link_pose7, int32_t *info);
+/* The same for the worlds [world0, world0 + n_worlds): ONE device -> host copy per state pool and ONE synchronisation.
+   Outputs are concatenated in world order, each world's slice laid out as in ob_get_state (q of world w starts at
+   2 * sum of n_links of the worlds before it in the range, and so on); apple_x64 is the position at the library's
+   internal precision (see ob_get_apple_x64); info: [3*n_worlds].  Any output pointer may be NULL. */
+int ob_get_state_batch(ob_ctx *ctx, int world0, int n_worlds, float *q, float *qd, float *apple_x, double *apple_x64,
+                       float *apple_v, uint8_t *ruptured, uint8_t *attached, int32_t *info);
 /* Overwrite one world's state (NULL = keep).  Setting `ruptured` / `attached` also clears the corresponding
-   hysteresis counters; the PCG warm start of the world is cleared.  Status bits are cleared. */
+   hysteresis counters (the N-frame hysteresis of PAPER.md:139, the "few frames" of PAPER.md:163); the PCG warm start
+   of the world is cleared.  Status bits are cleared. */
 int ob_set_state(ob_ctx *ctx, int world, const float *q, const float *qd, const float *apple_x,
                  const float *apple_v, const uint8_t *ruptured, const uint8_t *attached);
-/* Apple positions at the library's internal precision: anchor (fp64 rest hang point) + fp32 displacement.
-   apple_x: [3*n_apples] doubles.  ob_get_state's float apple_x is this value rounded to fp32. */
+/* Apple positions at the library's internal precision: anchor (fp64 rest hang point, Eq. 3) + rest sag m g / k_s
+    + fp32 displacement.  apple_x: [3*n_apples] doubles.  ob_get_state's float apple_x is this value
+   rounded to fp32.  The setter is the exact inverse: get -> set restores the internal displacement bit for bit. */
 int ob_get_apple_x64(ob_ctx *ctx, int world, double *apple_x);
-/* Hysteresis counters (rupture per link; detach pull / tension per apple), for lock-step comparison. */
+int ob_set_apple_x64(ob_ctx *ctx, int world, const double *apple_x);
+/* Restore the step counter of a world (events carry it); everything else is kept, the warm start included. */
+int ob_set_step(ob_ctx *ctx, int world, int32_t step);
+/* Hysteresis counters (rupture per link; detach pull / tension per apple), for lock-step
+   comparison and checkpoints.  The _batch form covers worlds [world0, world0 + n_worlds), outputs concatenated. */
 int ob_get_counters(ob_ctx *ctx, int world, int32_t *rupture_count, int32_t *pull_count, int32_t *tension_count);
+int ob_get_counters_batch(ob_ctx *ctx, int world0, int n_worlds, int32_t *rupture_count, int32_t *pull_count,
+                          int32_t *tension_count);
 int ob_set_counters(ob_ctx *ctx, int world, const int32_t *rupture_count, const int32_t *pull_count,
                     const int32_t *tension_count);
-/* Per-world material draws: emr[3] = E, MOR, density; apple_detach, apple_mass: [n_apples] (NULL ok). */
+/* Per-world material draws of ob_randomize: emr[3] = E, MOR, density; apple_detach, apple_mass:
+   [n_apples] (NULL ok).  The _batch form: emr [3*n_worlds], apple arrays concatenated. */
 int ob_get_material(ob_ctx *ctx, int world, float *emr, float *apple_detach, float *apple_mass);
+int ob_get_material_batch(ob_ctx *ctx, int world0, int n_worlds, float *emr, float *apple_detach, float *apple_mass);
 
-/* Drain up to cap pending events, sorted by (step, world, kind, index).  Synchronises.
-   If the device list overflowed since the last drain, returns OB_E_CAPACITY after filling buf. */
+/* Exact checkpoint of one world: every byte of its mutable state (q, qd, flags, counters, apple state, step and
+   status words, the PCG solution history and preconditioner memory), so that load followed by ob_step(n) reproduces
+   an uninterrupted run bit for bit.  buf: host memory of ob_world_blob_bytes bytes.  A blob only loads into a world
+   of the same sizes (OB_E_ARG otherwise).  Materials and wrenches are not part of it. */
+int ob_world_blob_bytes(ob_ctx *ctx, int world, size_t *out);
+int ob_save_world(ob_ctx *ctx, int world, void *buf, size_t cap);
+int ob_load_world(ob_ctx *ctx, int world, const void *buf, size_t bytes);
+
+/* north_star "ob_events (rupture and detach lists)".  Drain up to cap pending events (Eq. 5 ruptures, PAPER.md:136;
+   detachments), sorted by (step, world, kind, index).  Synchronises.  If the device list overflowed
+   since the last drain, returns OB_E_CAPACITY after filling buf. */
 int ob_events(ob_ctx *ctx, ob_event *buf, int cap, int *n_out);
 
-/* Totals since ob_create: PCG iterations, world-steps taken (frozen worlds excluded), worlds with status != 0. */
+/* Totals since ob_create: PCG iterations, world-steps taken (frozen worlds excluded), worlds with status != 0
+   (BASELINE.json metric: "world-steps/s ...; CG iters/s").  Reduced on the device; one small copy. */
 int ob_stats(ob_ctx *ctx, uint64_t *cg_iters_total, uint64_t *world_steps_total, int32_t *n_flagged);
+/* World-steps by PCG iteration count since ob_create (or the last reset): bins[k] = world-steps that took k
+   iterations, the last bin collecting k >= n_bins - 1.  reset != 0 clears the device histogram after the read. */
+int ob_iter_histogram(ob_ctx *ctx, uint64_t *bins, int n_bins, int reset);
 
 /* Launch geometry of the last ob_step (for reporting): kernel launches, CTAs, threads per CTA, dynamic smem. */
 int ob_launch_info(ob_ctx *ctx, int32_t *n_launches, int32_t *grid, int32_t *block, int32_t *smem_bytes);

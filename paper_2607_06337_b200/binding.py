@@ -22,7 +22,8 @@ EXPORTS = [
     "ob_apply_wrench_batch", "ob_step", "ob_get_state", "ob_set_state", "ob_get_apple_x64", "ob_get_counters", "ob_set_counters",
     "ob_get_material", "ob_events", "ob_stats", "ob_launch_info", "ob_last_error", "ob_destroy",
     "ob_sizeof_params", "ob_sizeof_world_spec", "ob_sizeof_event", "ob_counters", "ob_flush",
-    "ob_selftest_philox",
+    "ob_selftest_philox", "ob_get_state_batch", "ob_set_apple_x64", "ob_set_step", "ob_get_counters_batch",
+    "ob_get_material_batch", "ob_world_blob_bytes", "ob_save_world", "ob_load_world", "ob_iter_histogram",
 ]
 
 
@@ -77,6 +78,15 @@ def load_library():
         L.ob_get_state.argtypes = [vp, i32] + [vp] * 8
         L.ob_set_state.argtypes = [vp, i32] + [vp] * 6
         L.ob_get_apple_x64.argtypes = [vp, i32, vp]
+        L.ob_set_apple_x64.argtypes = [vp, i32, vp]
+        L.ob_set_step.argtypes = [vp, i32, C.c_int32]
+        L.ob_get_state_batch.argtypes = [vp, i32, i32] + [vp] * 8
+        L.ob_get_counters_batch.argtypes = [vp, i32, i32] + [vp] * 3
+        L.ob_get_material_batch.argtypes = [vp, i32, i32] + [vp] * 3
+        L.ob_world_blob_bytes.argtypes = [vp, i32, C.POINTER(C.c_size_t)]
+        L.ob_save_world.argtypes = [vp, i32, vp, C.c_size_t]
+        L.ob_load_world.argtypes = [vp, i32, vp, C.c_size_t]
+        L.ob_iter_histogram.argtypes = [vp, vp, i32, i32]
         L.ob_get_counters.argtypes = [vp, i32] + [vp] * 3
         L.ob_set_counters.argtypes = [vp, i32] + [vp] * 3
         L.ob_get_material.argtypes = [vp, i32] + [vp] * 3
@@ -227,25 +237,76 @@ class Orchard:
         self._check(self._L.ob_step(self._h, n))
 
     def get_state(self, world: int, pose: bool = False) -> dict:
+        if not pose:
+            b = self.get_state_batch(world, 1)
+            return dict(q=b["q"], qd=b["qd"], apple_x=b["apple_x"], apple_x64=b["apple_x64"], apple_v=b["apple_v"],
+                        ruptured=b["ruptured"], attached=b["attached"], step=int(b["info"][0, 0]),
+                        last_iters=int(b["info"][0, 1]), status=int(b["info"][0, 2]))
         N, A = self.n_links[world], self.n_apples[world]
         q = np.zeros(2 * N, np.float32); qd = np.zeros(2 * N, np.float32)
         ax = np.zeros((A, 3), np.float32); av = np.zeros((A, 3), np.float32)
         rup = np.zeros(N, np.uint8); att = np.zeros(A, np.uint8)
-        pose7 = np.zeros((N, 7), np.float32) if pose else None
+        pose7 = np.zeros((N, 7), np.float32)
         info = np.zeros(3, np.int32)
         self._check(self._L.ob_get_state(self._h, world, _ptr(q), _ptr(qd), _ptr(ax), _ptr(av), _ptr(rup), _ptr(att),
                                          _ptr(pose7), _ptr(info)))
-        out = dict(q=q, qd=qd, apple_x=ax, apple_v=av, ruptured=rup, attached=att,
-                   step=int(info[0]), last_iters=int(info[1]), status=int(info[2]))
-        if pose:
-            out["link_pose7"] = pose7
+        x64 = np.zeros((A, 3), np.float64)
         if A:
-            x64 = np.zeros((A, 3), np.float64)
             self._check(self._L.ob_get_apple_x64(self._h, world, _ptr(x64)))
-            out["apple_x64"] = x64
-        else:
-            out["apple_x64"] = np.zeros((0, 3), np.float64)
+        return dict(q=q, qd=qd, apple_x=ax, apple_v=av, ruptured=rup, attached=att, link_pose7=pose7, apple_x64=x64,
+                    step=int(info[0]), last_iters=int(info[1]), status=int(info[2]))
+
+    def get_state_batch(self, world0: int = 0, n_worlds: Optional[int] = None, out: Optional[dict] = None) -> dict:
+        """ob_get_state_batch: worlds [world0, world0 + n_worlds), outputs concatenated in world order.  `out` may be
+        the dict of a previous call (same range): its arrays are reused."""
+        n = self.n_worlds - world0 if n_worlds is None else n_worlds
+        NL, NA = sum(self.n_links[world0:world0 + n]), sum(self.n_apples[world0:world0 + n])
+        if out is None:
+            out = dict(q=np.zeros(2 * NL, np.float32), qd=np.zeros(2 * NL, np.float32),
+                       apple_x=np.zeros((NA, 3), np.float32), apple_x64=np.zeros((NA, 3), np.float64),
+                       apple_v=np.zeros((NA, 3), np.float32), ruptured=np.zeros(NL, np.uint8),
+                       attached=np.zeros(NA, np.uint8), info=np.zeros((n, 3), np.int32))
+        self._check(self._L.ob_get_state_batch(self._h, world0, n, _ptr(out["q"]), _ptr(out["qd"]), _ptr(out["apple_x"]),
+                                               _ptr(out["apple_x64"]), _ptr(out["apple_v"]), _ptr(out["ruptured"]),
+                                               _ptr(out["attached"]), _ptr(out["info"])))
         return out
+
+    def set_apple_x64(self, world: int, apple_x):
+        x = np.ascontiguousarray(apple_x, dtype=np.float64)
+        self._check(self._L.ob_set_apple_x64(self._h, world, _ptr(x)))
+
+    def set_step(self, world: int, step: int):
+        self._check(self._L.ob_set_step(self._h, world, int(step)))
+
+    def save_world(self, world: int) -> bytes:
+        n = C.c_size_t(0)
+        self._check(self._L.ob_world_blob_bytes(self._h, world, C.byref(n)))
+        buf = np.zeros(n.value, np.uint8)
+        self._check(self._L.ob_save_world(self._h, world, _ptr(buf), n))
+        return buf.tobytes()
+
+    def load_world(self, world: int, blob: bytes):
+        buf = np.frombuffer(blob, dtype=np.uint8).copy()
+        self._check(self._L.ob_load_world(self._h, world, _ptr(buf), C.c_size_t(buf.size)))
+
+    def get_counters_batch(self, world0: int = 0, n_worlds: Optional[int] = None):
+        n = self.n_worlds - world0 if n_worlds is None else n_worlds
+        NL, NA = sum(self.n_links[world0:world0 + n]), sum(self.n_apples[world0:world0 + n])
+        rc = np.zeros(NL, np.int32); ca = np.zeros(NA, np.int32); cb = np.zeros(NA, np.int32)
+        self._check(self._L.ob_get_counters_batch(self._h, world0, n, _ptr(rc), _ptr(ca), _ptr(cb)))
+        return rc, ca, cb
+
+    def get_material_batch(self, world0: int = 0, n_worlds: Optional[int] = None) -> dict:
+        n = self.n_worlds - world0 if n_worlds is None else n_worlds
+        NA = sum(self.n_apples[world0:world0 + n])
+        emr = np.zeros((n, 3), np.float32); det = np.zeros(NA, np.float32); mass = np.zeros(NA, np.float32)
+        self._check(self._L.ob_get_material_batch(self._h, world0, n, _ptr(emr), _ptr(det), _ptr(mass)))
+        return dict(E=emr[:, 0], MOR=emr[:, 1], density=emr[:, 2], detach=det, mass=mass)
+
+    def iter_histogram(self, n_bins: int = 64, reset: bool = False) -> np.ndarray:
+        bins = np.zeros(n_bins, np.uint64)
+        self._check(self._L.ob_iter_histogram(self._h, _ptr(bins), n_bins, 1 if reset else 0))
+        return bins
 
     def set_state(self, world: int, q=None, qd=None, apple_x=None, apple_v=None, ruptured=None, attached=None):
         def f(a):

@@ -11,7 +11,7 @@ LIB = os.path.join(HERE, "libob.so")
 SOURCES = ["ob_host.cu", "ob_kernels.cu", "ob_step.cu"]
 HEADERS = ["ob_internal.h", "ob_device.h", os.path.join("..", "..", "include", "orchard.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "--use_fast_math=false", "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
+              "--use_fast_math=false", "-Xcompiler", "-fPIC", "-Xcompiler", "-fopenmp", "-shared", "-Xptxas", "-v"]
 
 
 def _stale() -> bool:

@@ -36,15 +36,6 @@ __device__ __forceinline__ M3 mul(const M3 &A, const M3 &B) {
       C.a[3 * r + c] = A.a[3 * r] * B.a[c] + A.a[3 * r + 1] * B.a[3 + c] + A.a[3 * r + 2] * B.a[6 + c];
   return C;
 }
-__device__ __forceinline__ M3 quat_to_mat(float4 q) {  // q = (w,x,y,z) stored as (x=w, y=x, z=y, w=z)
-  float w = q.x, x = q.y, y = q.z, z = q.w;
-  M3 R;
-  R.a[0] = 1.f - 2.f * (y * y + z * z); R.a[1] = 2.f * (x * y - w * z);       R.a[2] = 2.f * (x * z + w * y);
-  R.a[3] = 2.f * (x * y + w * z);       R.a[4] = 1.f - 2.f * (x * x + z * z); R.a[5] = 2.f * (y * z - w * x);
-  R.a[6] = 2.f * (x * z - w * y);       R.a[7] = 2.f * (y * z + w * x);       R.a[8] = 1.f - 2.f * (x * x + y * y);
-  return R;
-}
-
 // ------------------------------------------------------------------------------------------------------
 // TMA bulk copies + mbarrier (1-D cp.async.bulk; SASS: UBLKCP)
 // ------------------------------------------------------------------------------------------------------

@@ -37,6 +37,7 @@ struct ob_ctx {
   DevCtx dev{};
   std::vector<WorldDesc> desc;
   std::vector<HostWorld> hw;
+  std::vector<size_t> link_prefix, apple_prefix;   // caller-order prefix sums of n_links / n_apples (batched read-out)
   std::vector<WrenchSlots> wrench;       // host mirror (internal body indices)
   int dirty_lo = 0, dirty_hi = -1;
   WrenchSlots *staging[2] = {nullptr, nullptr};
@@ -49,6 +50,12 @@ struct ob_ctx {
   int max_Np = 0, max_Ap = 0;
   size_t ev_cap = 0;
   uint64_t h2d_bytes = 0, d2h_bytes = 0, kernel_launches = 0, step_calls = 0;
+  // size classes run concurrently: one internal stream per class, forked from and joined to the caller's stream
+  cudaStream_t cls_stream[kNumClasses] = {};
+  cudaEvent_t ev_fork = nullptr, ev_join[kNumClasses] = {};
+  // pinned staging for the read-out calls (grown on demand)
+  unsigned char *rd = nullptr;
+  size_t rd_cap = 0;
 };
 
 namespace {
@@ -157,8 +164,8 @@ inline int pad8(int n) { return (n + 7) / 8 * 8; }
 
 struct Layout {
   size_t total = 0;
-  Pool desc, order, link_blk, apple_blk, topo, topo2, child_list, quat_raw, quatd, Mmax, mdiag, xprev, Lown, diam, arm, link_ext, apple_ext, apple_nom,
-      apple_c, anchor, level_off, info, wrench, events, ev_count, queue, progress, pose7;
+  Pool desc, order, link_blk, link_cst, apple_blk, topo, topo2, quat_raw, quatd, Mmax, mdiag, xprev, Lown, diam, arm, link_ext, apple_ext, apple_nom,
+      apple_c, anchor, level_off, info, wrench, events, ev_count, queue, iter_hist, stats, progress, pose7;
   size_t sumNp = 0, sumAp = 0, sumLev = 0, ev_cap = 0;
   int max_Np = 0, max_Ap = 0, max_smem = 0;
   bool any_arm = false;
@@ -206,11 +213,11 @@ int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) 
   L.ev_cap = std::max<size_t>(ev, 64);
   take(L, L.desc, sizeof(WorldDesc) * n_worlds);
   take(L, L.order, sizeof(int32_t) * n_worlds);
-  take(L, L.link_blk, (size_t)link_block_bytes(1) * L.sumNp);
+  take(L, L.link_blk, (size_t)link_state_bytes(1) * L.sumNp);
+  take(L, L.link_cst, (size_t)link_const_bytes(1) * L.sumNp);
   take(L, L.apple_blk, (size_t)apple_block_bytes(1) * std::max<size_t>(L.sumAp, 16));
   take(L, L.topo, sizeof(int4) * L.sumNp);
   take(L, L.topo2, sizeof(int4) * L.sumNp);
-  take(L, L.child_list, sizeof(int32_t) * L.sumNp);
   take(L, L.quat_raw, sizeof(float4) * L.sumNp);
   take(L, L.quatd, sizeof(double) * 4 * L.sumNp);
   take(L, L.Mmax, sizeof(float) * L.sumNp);
@@ -230,6 +237,8 @@ int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) 
   take(L, L.events, sizeof(ob_event) * L.ev_cap);
   take(L, L.ev_count, sizeof(int32_t) * 4);
   take(L, L.queue, sizeof(int32_t) * 2 * kNumClasses);
+  take(L, L.iter_hist, sizeof(unsigned long long) * kIterHistBins);
+  take(L, L.stats, sizeof(unsigned long long) * 4);
   take(L, L.progress, sizeof(int32_t) * n_worlds);
   take(L, L.pose7, sizeof(float) * 7 * L.max_Np);
   L.total = (L.total + kAlign - 1) / kAlign * kAlign;
@@ -257,20 +266,20 @@ int flush_wrenches(ob_ctx *ctx) {
   return OB_OK;
 }
 
-// rest sag m g / k_s of every apple of one world in fp64 (caller order), from the fp32 constants on the device;
-// apple positions cross the ABI as anchor + sag + u (the kernel stores u = x - x_rest in fp32)
-int fetch_sag(ob_ctx *ctx, int world, std::vector<double> &sag) {
-  const WorldDesc &d = ctx->desc[world];
-  const HostWorld &H = ctx->hw[world];
-  sag.assign(3 * (size_t)d.A, 0.0);
-  if (!d.A) return OB_OK;
-  std::vector<float> km(2 * (size_t)d.Ap);
-  CU(cpy(ctx, km.data(), ctx->dev.apple_blk + d.apple_blk_off + apple_state_bytes(d.Ap) + 3 * 4 * d.Ap,
-         sizeof(float) * km.size(), cudaMemcpyDeviceToHost, ctx->stream));
-  CU(cudaStreamSynchronize(ctx->stream));
-  for (int a = 0; a < d.A; a++)
-    for (int k = 0; k < 3; k++)
-      sag[3 * H.int2ext_apple[a] + k] = (double)km[d.Ap + a] * (double)ctx->dev.P.gravity[k] / (double)km[a];
+// pinned staging buffer of at least `bytes` bytes for a read-out call
+int rd_reserve(ob_ctx *ctx, size_t bytes) {
+  if (bytes <= ctx->rd_cap) return OB_OK;
+  if (ctx->rd) cudaFreeHost(ctx->rd);
+  ctx->rd = nullptr; ctx->rd_cap = 0;
+  const size_t cap = (bytes + (1u << 20)) & ~(size_t)((1u << 20) - 1);
+  CU(cudaHostAlloc((void **)&ctx->rd, cap, cudaHostAllocDefault));
+  ctx->rd_cap = cap;
+  return OB_OK;
+}
+
+int check_range(ob_ctx *ctx, int world0, int n) {
+  if (!ctx) return OB_E_ARG;
+  if (world0 < 0 || n < 1 || world0 + n > ctx->n_worlds) return fail(ctx, OB_E_ARG, "world range [%d, %d) out of range", world0, world0 + n);
   return OB_OK;
 }
 
@@ -342,12 +351,17 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   ctx->desc.resize(n_worlds);
   ctx->hw.resize(n_worlds);
   ctx->wrench.assign(n_worlds, WrenchSlots{});
+  ctx->link_prefix.assign(n_worlds + 1, 0);
+  ctx->apple_prefix.assign(n_worlds + 1, 0);
+  for (int w = 0; w < n_worlds; w++) {
+    ctx->link_prefix[w + 1] = ctx->link_prefix[w] + (size_t)specs[w].n_links;
+    ctx->apple_prefix[w + 1] = ctx->apple_prefix[w] + (size_t)specs[w].n_apples;
+  }
   unsigned char *base = ctx->dev_base;
 
   // ---- host images of every pool ----
   std::vector<unsigned char> h_link(L.link_blk.bytes, 0), h_apple(L.apple_blk.bytes, 0);
-  std::vector<int4> h_topo(L.sumNp, make_int4(-1, -1, -1, 0xfff)), h_topo2(L.sumNp, make_int4(0, -1, 0, 0));
-  std::vector<int32_t> h_child(L.sumNp, 0);
+  std::vector<int4> h_topo(L.sumNp, make_int4(-1, 0, 0, 0)), h_topo2(L.sumNp, make_int4(0, -1, 0, 0));
   std::vector<float4> h_quat_raw(L.sumNp, make_float4(1.f, 0.f, 0.f, 0.f));
   std::vector<float> h_Lown(L.sumNp, 1.f), h_diam(L.sumNp, 1.f), h_arm(L.any_arm ? 2 * L.sumNp : 0, 0.f);
   std::vector<int32_t> h_link_ext(L.sumNp, 0), h_apple_ext(std::max<size_t>(L.sumAp, 16), 0), h_lev(L.sumLev, 0);
@@ -381,16 +395,14 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
     d.density = s.density; d.E = s.E; d.MOR = s.MOR;
     d.has_apple_c = s.apple_c ? 1 : 0;
 
-    std::vector<int32_t> n_child(N, 0), first_apple(N, 0), n_apple(N, 0), cl_off(N, 0), islot(N, 0xffff), par(N, -1);
+    std::vector<int32_t> n_child(N, 0), first_apple(N, 0), n_apple(N, 0), islot(N, 0xffff), par(N, -1);
     std::vector<std::vector<int32_t>> kids(N);
     for (int i = 1; i < N; i++) {
       par[i] = H.ext2int_link[s.parent[H.int2ext_link[i]]];
       kids[par[i]].push_back(i);          // ascending internal index: a fixed summation order
     }
-    for (int i = 0, off = 0, slot = 0; i < N; i++) {
+    for (int i = 0, slot = 0; i < N; i++) {
       n_child[i] = (int32_t)kids[i].size();
-      cl_off[i] = off;
-      for (int32_t ch : kids[i]) h_child[link_base + off++] = ch;
       if (n_child[i]) islot[i] = slot++;
     }
     for (int a = 0; a < A; a++) {
@@ -404,11 +416,9 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
     for (int i = 0; i < N; i++) {
       const int e = H.int2ext_link[i];
       const int p = par[i];
-      auto kid = [&](int c) { return c < n_child[i] ? kids[i][c] : 0xffff; };
-      h_topo[link_base + i] = make_int4(p, kid(0) | (kid(1) << 16), kid(2) | (kid(3) << 16),
-                                        level_of[i] | (std::min(n_child[i], 5) << 12));
+      h_topo[link_base + i] = make_int4(p, n_child[i] ? kids[i][0] : 0, level_of[i], n_child[i]);
       h_topo2[link_base + i] = make_int4(first_apple[i] | (n_apple[i] << 16),
-                                         islot[i] | ((p >= 0 ? islot[p] : 0xffff) << 16), cl_off[i], n_child[i]);
+                                         islot[i] | ((p >= 0 ? islot[p] : 0xffff) << 16), 0, 0);
       const float *q = s.rest_quat + 4 * e;
       const double n = std::sqrt((double)q[0] * q[0] + (double)q[1] * q[1] + (double)q[2] * q[2] + (double)q[3] * q[3]);
       h_quat_raw[link_base + i] = make_float4(q[0], q[1], q[2], q[3]);
@@ -438,7 +448,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
     }
     for (int a = A; a < Ap; a++) { aconst[3 * Ap + a] = 1.f; aconst[4 * Ap + a] = 1.f; alink[a] = 0; }
     link_base += Np; apple_base += Ap; lev_base += nlev + 1;
-    link_off += link_block_bytes(Np); apple_off += apple_block_bytes(Ap);
+    link_off += link_state_bytes(Np); apple_off += apple_block_bytes(Ap);
     h_order[w] = w;
   }
   // work-queue order: grouped by size class, largest worlds first inside a class (longest-processing-time rule)
@@ -457,10 +467,10 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   D.desc = reinterpret_cast<WorldDesc *>(base + L.desc.off);
   D.order = reinterpret_cast<int32_t *>(base + L.order.off);
   D.link_blk = base + L.link_blk.off;
+  D.link_cst = base + L.link_cst.off;
   D.apple_blk = base + L.apple_blk.off;
   D.topo = reinterpret_cast<int4 *>(base + L.topo.off);
   D.topo2 = reinterpret_cast<int4 *>(base + L.topo2.off);
-  D.child_list = reinterpret_cast<int32_t *>(base + L.child_list.off);
   D.quat_raw = reinterpret_cast<float4 *>(base + L.quat_raw.off);
   D.quatd = reinterpret_cast<double *>(base + L.quatd.off);
   D.Mmax = reinterpret_cast<float *>(base + L.Mmax.off);
@@ -482,6 +492,8 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   D.ev_cap = (int32_t)std::min<size_t>(L.ev_cap, 0x7fffffff);
   D.ev_count = reinterpret_cast<int32_t *>(base + L.ev_count.off);
   D.queue = reinterpret_cast<int32_t *>(base + L.queue.off);
+  D.iter_hist = reinterpret_cast<unsigned long long *>(base + L.iter_hist.off);
+  D.stats = reinterpret_cast<unsigned long long *>(base + L.stats.off);
   D.progress = reinterpret_cast<int32_t *>(base + L.progress.off);
   D.pose7 = reinterpret_cast<float *>(base + L.pose7.off);
   D.P = *params;
@@ -497,7 +509,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   } while (0)
   cudaError_t e = cudaMemsetAsync(base, 0, L.total, ctx->stream);
   if (e != cudaSuccess) { g_err = cudaGetErrorString(e); delete ctx; return OB_E_CUDA; }
-  UP(L.desc, ctx->desc); UP(L.order, h_order); UP(L.link_blk, h_link); UP(L.apple_blk, h_apple); UP(L.topo, h_topo); UP(L.topo2, h_topo2); UP(L.child_list, h_child);
+  UP(L.desc, ctx->desc); UP(L.order, h_order); UP(L.link_blk, h_link); UP(L.apple_blk, h_apple); UP(L.topo, h_topo); UP(L.topo2, h_topo2);
   UP(L.quat_raw, h_quat_raw); UP(L.Lown, h_Lown); UP(L.diam, h_diam); UP(L.arm, h_arm); UP(L.link_ext, h_link_ext);
   UP(L.apple_ext, h_apple_ext); UP(L.apple_nom, h_nom); UP(L.apple_c, h_c); UP(L.level_off, h_lev);
 #undef UP
@@ -517,6 +529,16 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
     if (e == cudaSuccess && per_sm < 1) e = cudaErrorInvalidConfiguration;
     ctx->cls_grid[k] = std::max(1, std::min(ctx->cls_n[k], n_sm * std::max(per_sm, 1)));
     if (ctx->cls_n[k] > ctx->cls_n[ctx->main_cls]) ctx->main_cls = k;
+  }
+  int n_cls_used = 0;
+  for (int k = 0; k < kNumClasses; k++) n_cls_used += ctx->cls_n[k] > 0;
+  if (n_cls_used > 1) {          // heterogeneous batch: the size classes run side by side (ob_step forks and joins)
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming);
+    for (int k = 0; k < kNumClasses && e == cudaSuccess; k++) {
+      if (!ctx->cls_n[k]) continue;
+      e = cudaStreamCreateWithFlags(&ctx->cls_stream[k], cudaStreamNonBlocking);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_join[k], cudaEventDisableTiming);
+    }
   }
   for (int k = 0; k < 2 && e == cudaSuccess; k++) {
     e = cudaHostAlloc((void **)&ctx->staging[k], sizeof(WrenchSlots) * n_worlds, cudaHostAllocDefault);
@@ -616,10 +638,21 @@ int ob_step(ob_ctx *ctx, int n) {
   // enough that staging a world is amortised
   const int n_chunks = std::max(1, std::min(8, (n + 9) / 10));
   ctx->launches = 0;
+  // A heterogeneous batch has one persistent kernel per size class.  They go to streams of their own, forked from and
+  // joined to the caller's stream, so that the CTAs of the next class move in as the CTAs of a class run out of work
+  // (back to back on one stream every class would drain to its own tail while the others wait).
+  const bool fork = ctx->ev_fork != nullptr;
+  if (fork) CU(cudaEventRecord(ctx->ev_fork, ctx->stream));
   for (int k = kNumClasses - 1; k >= 0; k--) {      // the class of the largest worlds first
     if (!ctx->cls_n[k]) continue;
+    cudaStream_t st = fork ? ctx->cls_stream[k] : ctx->stream;
+    if (fork) CU(cudaStreamWaitEvent(st, ctx->ev_fork, 0));
     CU(launch_step(ctx->dev, k, ctx->dev.order + ctx->cls_off[k], ctx->cls_n[k], ctx->dev.queue + k, n,
-                   ctx->cls_grid[k], ctx->cls_smem[k], ctx->n_sm, n_chunks, ctx->dev.progress, ctx->stream));
+                   ctx->cls_grid[k], ctx->cls_smem[k], ctx->n_sm, n_chunks, ctx->dev.progress, st));
+    if (fork) {
+      CU(cudaEventRecord(ctx->ev_join[k], st));
+      CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_join[k], 0));
+    }
     ctx->launches += 1;
     ctx->kernel_launches += 1;
   }
@@ -627,139 +660,282 @@ int ob_step(ob_ctx *ctx, int n) {
   return OB_OK;
 }
 
-int ob_get_state(ob_ctx *ctx, int world, float *q, float *qd, float *apple_x, float *apple_v, uint8_t *ruptured,
-                 uint8_t *attached, float *link_pose7, int32_t *info) {
-  int rc = check_world(ctx, world);
+// ------------------------------------------------------------------------------------------------------
+// read-out.  The state pools keep the worlds back to back, so a range of worlds is ONE device -> host copy per pool
+// (link state, apple blocks, WorldInfo) into pinned staging and ONE stream synchronisation; the host then scatters
+// into the caller's order.  The per-world calls are the range calls with n = 1.
+// ------------------------------------------------------------------------------------------------------
+}  // extern "C"
+
+namespace {
+
+struct RdView {
+  const unsigned char *link = nullptr, *apple = nullptr;   // staged copies; index with the world's pool offset - base
+  const WorldInfo *info = nullptr;
+  const float *pose = nullptr;
+  size_t link0 = 0, apple0 = 0;
+};
+
+// stage the pools of worlds [w0, w0 + n): async copies + one synchronise
+int rd_fetch(ob_ctx *ctx, int w0, int n, bool links, bool apples, bool info, int pose_world, RdView &v) {
+  const WorldDesc &a = ctx->desc[w0], &b = ctx->desc[w0 + n - 1];
+  const size_t lbytes = links ? (size_t)(b.link_blk_off - a.link_blk_off) + link_state_bytes(b.Np) : 0;
+  const size_t abytes = apples ? (size_t)(b.apple_blk_off - a.apple_blk_off) + apple_block_bytes(b.Ap) : 0;
+  const size_t ibytes = info ? sizeof(WorldInfo) * (size_t)n : 0;
+  const size_t pbytes = pose_world >= 0 ? sizeof(float) * 7 * (size_t)ctx->desc[pose_world].N : 0;
+  auto up = [](size_t x) { return (x + 255) & ~(size_t)255; };
+  int rc = rd_reserve(ctx, up(lbytes) + up(abytes) + up(ibytes) + up(pbytes) + 256);
   if (rc != OB_OK) return rc;
-  const WorldDesc &d = ctx->desc[world];
-  const HostWorld &H = ctx->hw[world];
-  std::vector<unsigned char> lb(link_state_bytes(d.Np)), ab(std::max(apple_state_bytes(d.Ap), 1));
-  std::vector<float> pose(link_pose7 ? 7 * (size_t)d.N : 0);
-  WorldInfo wi;
-  if (link_pose7) {
-    CU(launch_pose(ctx->dev, world, ctx->stream));
+  unsigned char *p = ctx->rd;
+  if (pose_world >= 0) {
+    CU(launch_pose(ctx->dev, pose_world, ctx->stream));
     ctx->kernel_launches += 1;
   }
-  CU(cpy(ctx, lb.data(), ctx->dev.link_blk + d.link_blk_off, lb.size(), cudaMemcpyDeviceToHost, ctx->stream));
-  if (d.Ap)
-    CU(cpy(ctx, ab.data(), ctx->dev.apple_blk + d.apple_blk_off, apple_state_bytes(d.Ap), cudaMemcpyDeviceToHost,
-                       ctx->stream));
-  if (link_pose7)
-    CU(cpy(ctx, pose.data(), ctx->dev.pose7, sizeof(float) * pose.size(), cudaMemcpyDeviceToHost, ctx->stream));
-  CU(cpy(ctx, &wi, ctx->dev.info + world, sizeof(wi), cudaMemcpyDeviceToHost, ctx->stream));
+  if (lbytes) { CU(cpy(ctx, p, ctx->dev.link_blk + a.link_blk_off, lbytes, cudaMemcpyDeviceToHost, ctx->stream)); v.link = p; p += up(lbytes); }
+  if (abytes) { CU(cpy(ctx, p, ctx->dev.apple_blk + a.apple_blk_off, abytes, cudaMemcpyDeviceToHost, ctx->stream)); v.apple = p; p += up(abytes); }
+  if (ibytes) { CU(cpy(ctx, p, ctx->dev.info + w0, ibytes, cudaMemcpyDeviceToHost, ctx->stream)); v.info = reinterpret_cast<const WorldInfo *>(p); p += up(ibytes); }
+  if (pbytes) { CU(cpy(ctx, p, ctx->dev.pose7, pbytes, cudaMemcpyDeviceToHost, ctx->stream)); v.pose = reinterpret_cast<const float *>(p); p += up(pbytes); }
   CU(cudaStreamSynchronize(ctx->stream));
-  const float *st = reinterpret_cast<const float *>(lb.data());
-  const unsigned char *fl = lb.data() + kLinkStateFloats * 4 * d.Np;
-  for (int i = 0; i < d.N; i++) {
-    const int e = H.int2ext_link[i];
-    if (q) { q[2 * e] = st[2 * i]; q[2 * e + 1] = st[2 * i + 1]; }
-    if (qd) { qd[2 * e] = st[2 * d.Np + 2 * i]; qd[2 * e + 1] = st[2 * d.Np + 2 * i + 1]; }
-    if (ruptured) ruptured[e] = fl[i];
-    if (link_pose7) std::memcpy(link_pose7 + 7 * e, pose.data() + 7 * i, 7 * sizeof(float));
-  }
-  const float *as = reinterpret_cast<const float *>(ab.data());
-  const unsigned char *af = ab.data() + 6 * 4 * d.Ap;
-  std::vector<double> sag;
-  if (apple_x && (rc = fetch_sag(ctx, world, sag)) != OB_OK) return rc;
-  for (int a = 0; a < d.A; a++) {
-    const int e = H.int2ext_apple[a];
-    for (int k = 0; k < 3; k++) {
-      if (apple_x) apple_x[3 * e + k] = (float)(H.anchor[3 * e + k] + sag[3 * e + k] + (double)as[k * d.Ap + a]);
-      if (apple_v) apple_v[3 * e + k] = as[(3 + k) * d.Ap + a];
-    }
-    if (attached) attached[e] = af[a];
-  }
-  if (info) { info[0] = wi.step; info[1] = wi.last_iters; info[2] = wi.status; }
+  v.link0 = (size_t)a.link_blk_off; v.apple0 = (size_t)a.apple_blk_off;
   return OB_OK;
 }
 
-int ob_set_state(ob_ctx *ctx, int world, const float *q, const float *qd, const float *apple_x, const float *apple_v,
-                 const uint8_t *ruptured, const uint8_t *attached) {
+// rest sag m g / k_s of one apple in fp64 from the fp32 constants: apple positions cross the ABI as
+// anchor + sag + u (the kernel stores u = x - x_rest in fp32)
+inline double sag_of(const float *aconst, int Ap, int a, float g) {
+  return (double)aconst[4 * Ap + a] * (double)g / (double)aconst[3 * Ap + a];
+}
+
+int get_state_impl(ob_ctx *ctx, int w0, int n, float *q, float *qd, float *apple_x, double *apple_x64, float *apple_v,
+                   uint8_t *ruptured, uint8_t *attached, int32_t *info, float *link_pose7) {
+  int rc = check_range(ctx, w0, n);
+  if (rc != OB_OK) return rc;
+  RdView v;
+  const bool links = q || qd || ruptured, apples = apple_x || apple_x64 || apple_v || attached;
+  rc = rd_fetch(ctx, w0, n, links, apples, info != nullptr, link_pose7 ? w0 : -1, v);
+  if (rc != OB_OK) return rc;
+  const size_t L0 = ctx->link_prefix[w0], A0 = ctx->apple_prefix[w0];
+  const float *g = ctx->dev.P.gravity;
+#pragma omp parallel for schedule(static) if (n > 64)
+  for (int k = 0; k < n; k++) {
+    const int w = w0 + k;
+    const WorldDesc &d = ctx->desc[w];
+    const HostWorld &H = ctx->hw[w];
+    const size_t lo = ctx->link_prefix[w] - L0, ao = ctx->apple_prefix[w] - A0;
+    if (links) {
+      const unsigned char *lb = v.link + ((size_t)d.link_blk_off - v.link0);
+      const float *st = reinterpret_cast<const float *>(lb);
+      const unsigned char *fl = lb + kLinkStateFloats * 4 * d.Np;
+      for (int i = 0; i < d.N; i++) {
+        const size_t e = lo + H.int2ext_link[i];
+        if (q) { q[2 * e] = st[2 * i]; q[2 * e + 1] = st[2 * i + 1]; }
+        if (qd) { qd[2 * e] = st[2 * d.Np + 2 * i]; qd[2 * e + 1] = st[2 * d.Np + 2 * i + 1]; }
+        if (ruptured) ruptured[e] = fl[i];
+      }
+    }
+    if (apples && d.A) {
+      const unsigned char *ab = v.apple + ((size_t)d.apple_blk_off - v.apple0);
+      const float *as = reinterpret_cast<const float *>(ab);
+      const unsigned char *af = ab + 6 * 4 * d.Ap;
+      const float *ac = reinterpret_cast<const float *>(ab + apple_state_bytes(d.Ap));
+      for (int a = 0; a < d.A; a++) {
+        const size_t e = ao + H.int2ext_apple[a];
+        for (int c = 0; c < 3; c++) {
+          if (apple_x || apple_x64) {
+            const double x = H.anchor[3 * (size_t)H.int2ext_apple[a] + c] + sag_of(ac, d.Ap, a, g[c]) + (double)as[c * d.Ap + a];
+            if (apple_x) apple_x[3 * e + c] = (float)x;
+            if (apple_x64) apple_x64[3 * e + c] = x;
+          }
+          if (apple_v) apple_v[3 * e + c] = as[(3 + c) * d.Ap + a];
+        }
+        if (attached) attached[e] = af[a];
+      }
+    }
+    if (info) { info[3 * k] = v.info[k].step; info[3 * k + 1] = v.info[k].last_iters; info[3 * k + 2] = v.info[k].status; }
+  }
+  if (link_pose7) {
+    const WorldDesc &d = ctx->desc[w0];
+    const HostWorld &H = ctx->hw[w0];
+    for (int i = 0; i < d.N; i++) std::memcpy(link_pose7 + 7 * H.int2ext_link[i], v.pose + 7 * i, 7 * sizeof(float));
+  }
+  return OB_OK;
+}
+
+// read-modify-write of one world's state blocks (everything the caller passes as NULL is kept)
+int set_state_impl(ob_ctx *ctx, int world, const float *q, const float *qd, const float *apple_x, const double *apple_x64,
+                   const float *apple_v, const uint8_t *ruptured, const uint8_t *attached, const int32_t *step) {
   int rc = check_world(ctx, world);
   if (rc != OB_OK) return rc;
   const WorldDesc &d = ctx->desc[world];
   const HostWorld &H = ctx->hw[world];
-  std::vector<unsigned char> lb(link_state_bytes(d.Np)), ab(std::max(apple_state_bytes(d.Ap), 1));
-  WorldInfo wi;
-  CU(cpy(ctx, lb.data(), ctx->dev.link_blk + d.link_blk_off, lb.size(), cudaMemcpyDeviceToHost, ctx->stream));
-  if (d.Ap)
-    CU(cpy(ctx, ab.data(), ctx->dev.apple_blk + d.apple_blk_off, apple_state_bytes(d.Ap), cudaMemcpyDeviceToHost,
-                       ctx->stream));
-  CU(cpy(ctx, &wi, ctx->dev.info + world, sizeof(wi), cudaMemcpyDeviceToHost, ctx->stream));
-  CU(cudaStreamSynchronize(ctx->stream));
+  RdView v;
+  rc = rd_fetch(ctx, world, 1, true, d.Ap > 0, true, -1, v);
+  if (rc != OB_OK) return rc;
+  std::vector<unsigned char> lb(v.link, v.link + link_state_bytes(d.Np));
+  std::vector<unsigned char> ab;
+  if (d.Ap) ab.assign(v.apple, v.apple + apple_block_bytes(d.Ap));
+  WorldInfo wi = v.info[0];
   float *st = reinterpret_cast<float *>(lb.data());
   unsigned char *fl = lb.data() + kLinkStateFloats * 4 * d.Np;
   for (int i = 0; i < d.N; i++) {
     const int e = H.int2ext_link[i];
     if (q) { st[2 * i] = q[2 * e]; st[2 * i + 1] = q[2 * e + 1]; }
     if (qd) { st[2 * d.Np + 2 * i] = qd[2 * e]; st[2 * d.Np + 2 * i + 1] = qd[2 * e + 1]; }
-    st[4 * d.Np + 2 * i] = 0.f; st[4 * d.Np + 2 * i + 1] = 0.f;          // warm start cleared
     if (ruptured) { fl[i] = ruptured[e] ? 1 : 0; fl[d.Np + i] = 0; }
   }
-  float *as = reinterpret_cast<float *>(ab.data());
-  unsigned char *af = ab.data() + 6 * 4 * d.Ap;
-  std::vector<double> sag;
-  if (apple_x && (rc = fetch_sag(ctx, world, sag)) != OB_OK) return rc;
-  for (int a = 0; a < d.A; a++) {
-    const int e = H.int2ext_apple[a];
-    for (int k = 0; k < 3; k++) {
-      if (apple_x) as[k * d.Ap + a] = (float)((double)apple_x[3 * e + k] - H.anchor[3 * e + k] - sag[3 * e + k]);
-      if (apple_v) as[(3 + k) * d.Ap + a] = apple_v[3 * e + k];
+  if (d.Ap) {
+    float *as = reinterpret_cast<float *>(ab.data());
+    unsigned char *af = ab.data() + 6 * 4 * d.Ap;
+    const float *ac = reinterpret_cast<const float *>(ab.data() + apple_state_bytes(d.Ap));
+    const float *g = ctx->dev.P.gravity;
+    for (int a = 0; a < d.A; a++) {
+      const int e = H.int2ext_apple[a];
+      for (int c = 0; c < 3; c++) {
+        if (apple_x64) as[c * d.Ap + a] = (float)(apple_x64[3 * e + c] - H.anchor[3 * e + c] - sag_of(ac, d.Ap, a, g[c]));
+        else if (apple_x) as[c * d.Ap + a] = (float)((double)apple_x[3 * e + c] - H.anchor[3 * e + c] - sag_of(ac, d.Ap, a, g[c]));
+        if (apple_v) as[(3 + c) * d.Ap + a] = apple_v[3 * e + c];
+      }
+      if (attached) { af[a] = attached[e] ? 1 : 0; af[d.Ap + a] = 0; af[2 * d.Ap + a] = 0; }
     }
-    if (attached) { af[a] = attached[e] ? 1 : 0; af[d.Ap + a] = 0; af[2 * d.Ap + a] = 0; }
   }
   wi.status = 0;
   wi.diag_age = 0;          // the state was written from outside: recompute the preconditioner at the next step
-  for (int k = 0; k < 4; k++)   // ... and forget the solution history the PCG start vector is extrapolated from
-    CU(cudaMemsetAsync(ctx->dev.xprev + (size_t)k * ctx->dev.sum_np + d.link_base, 0, sizeof(float2) * d.Np, ctx->stream));
+  if (step) wi.step = *step;
+  if (!step || q || qd || apple_x || apple_x64 || apple_v || ruptured || attached)
+    for (int k = 0; k < 4; k++)   // ... and forget the solution history the PCG start vector is extrapolated from
+      CU(cudaMemsetAsync(ctx->dev.xprev + (size_t)k * ctx->dev.sum_np + d.link_base, 0, sizeof(float2) * d.Np, ctx->stream));
   CU(cpy(ctx, ctx->dev.link_blk + d.link_blk_off, lb.data(), lb.size(), cudaMemcpyHostToDevice, ctx->stream));
   if (d.Ap)
-    CU(cpy(ctx, ctx->dev.apple_blk + d.apple_blk_off, ab.data(), apple_state_bytes(d.Ap), cudaMemcpyHostToDevice,
-                       ctx->stream));
+    CU(cpy(ctx, ctx->dev.apple_blk + d.apple_blk_off, ab.data(), apple_state_bytes(d.Ap), cudaMemcpyHostToDevice, ctx->stream));
   CU(cpy(ctx, ctx->dev.info + world, &wi, sizeof(wi), cudaMemcpyHostToDevice, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   return OB_OK;
 }
 
+// exact per-world checkpoint: every byte of mutable state, solver memory included
+struct BlobHeader { uint32_t magic; int32_t N, A, Np, Ap; uint32_t bytes; };
+constexpr uint32_t kBlobMagic = 0x4f42574cu;   // "OBWL"
+size_t blob_bytes(const WorldDesc &d) {
+  return sizeof(BlobHeader) + link_state_bytes(d.Np) + apple_state_bytes(d.Ap) + sizeof(WorldInfo) + 5 * sizeof(float2) * (size_t)d.Np;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ob_get_state(ob_ctx *ctx, int world, float *q, float *qd, float *apple_x, float *apple_v, uint8_t *ruptured,
+                 uint8_t *attached, float *link_pose7, int32_t *info) {
+  return get_state_impl(ctx, world, 1, q, qd, apple_x, nullptr, apple_v, ruptured, attached, info, link_pose7);
+}
+
+int ob_get_state_batch(ob_ctx *ctx, int world0, int n_worlds, float *q, float *qd, float *apple_x, double *apple_x64,
+                       float *apple_v, uint8_t *ruptured, uint8_t *attached, int32_t *info) {
+  return get_state_impl(ctx, world0, n_worlds, q, qd, apple_x, apple_x64, apple_v, ruptured, attached, info, nullptr);
+}
+
 int ob_get_apple_x64(ob_ctx *ctx, int world, double *apple_x) {
+  if (ctx && !apple_x) return fail(ctx, OB_E_ARG, "apple_x is null");
+  return get_state_impl(ctx, world, 1, nullptr, nullptr, nullptr, apple_x, nullptr, nullptr, nullptr, nullptr, nullptr);
+}
+
+int ob_set_state(ob_ctx *ctx, int world, const float *q, const float *qd, const float *apple_x, const float *apple_v,
+                 const uint8_t *ruptured, const uint8_t *attached) {
+  return set_state_impl(ctx, world, q, qd, apple_x, nullptr, apple_v, ruptured, attached, nullptr);
+}
+
+int ob_set_apple_x64(ob_ctx *ctx, int world, const double *apple_x) {
+  if (ctx && !apple_x) return fail(ctx, OB_E_ARG, "apple_x is null");
+  return set_state_impl(ctx, world, nullptr, nullptr, nullptr, apple_x, nullptr, nullptr, nullptr, nullptr);
+}
+
+int ob_set_step(ob_ctx *ctx, int world, int32_t step) {
+  if (ctx && step < 0) return fail(ctx, OB_E_ARG, "step < 0");
+  return set_state_impl(ctx, world, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, &step);
+}
+
+int ob_world_blob_bytes(ob_ctx *ctx, int world, size_t *out) {
   int rc = check_world(ctx, world);
   if (rc != OB_OK) return rc;
-  if (!apple_x) return fail(ctx, OB_E_ARG, "apple_x is null");
+  if (!out) return fail(ctx, OB_E_ARG, "out is null");
+  *out = blob_bytes(ctx->desc[world]);
+  return OB_OK;
+}
+
+int ob_save_world(ob_ctx *ctx, int world, void *buf, size_t cap) {
+  int rc = check_world(ctx, world);
+  if (rc != OB_OK) return rc;
   const WorldDesc &d = ctx->desc[world];
-  const HostWorld &H = ctx->hw[world];
-  if (!d.A) return OB_OK;
-  std::vector<float> u(3 * (size_t)d.Ap);
-  CU(cpy(ctx, u.data(), ctx->dev.apple_blk + d.apple_blk_off, sizeof(float) * u.size(), cudaMemcpyDeviceToHost,
-                     ctx->stream));
+  const size_t need = blob_bytes(d);
+  if (!buf || cap < need) return fail(ctx, OB_E_ARG, "checkpoint buffer null or smaller than ob_world_blob_bytes (%zu)", need);
+  unsigned char *p = static_cast<unsigned char *>(buf);
+  BlobHeader h{kBlobMagic, d.N, d.A, d.Np, d.Ap, (uint32_t)need};
+  std::memcpy(p, &h, sizeof(h)); p += sizeof(h);
+  CU(cpy(ctx, p, ctx->dev.link_blk + d.link_blk_off, link_state_bytes(d.Np), cudaMemcpyDeviceToHost, ctx->stream)); p += link_state_bytes(d.Np);
+  if (d.Ap) CU(cpy(ctx, p, ctx->dev.apple_blk + d.apple_blk_off, apple_state_bytes(d.Ap), cudaMemcpyDeviceToHost, ctx->stream));
+  p += apple_state_bytes(d.Ap);
+  CU(cpy(ctx, p, ctx->dev.info + world, sizeof(WorldInfo), cudaMemcpyDeviceToHost, ctx->stream)); p += sizeof(WorldInfo);
+  for (int k = 0; k < 4; k++) {
+    CU(cpy(ctx, p, ctx->dev.xprev + (size_t)k * ctx->dev.sum_np + d.link_base, sizeof(float2) * d.Np, cudaMemcpyDeviceToHost, ctx->stream));
+    p += sizeof(float2) * d.Np;
+  }
+  CU(cpy(ctx, p, ctx->dev.mdiag + d.link_base, sizeof(float2) * d.Np, cudaMemcpyDeviceToHost, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
-  std::vector<double> sag;
-  if ((rc = fetch_sag(ctx, world, sag)) != OB_OK) return rc;
-  for (int a = 0; a < d.A; a++) {
-    const int e = H.int2ext_apple[a];
-    for (int k = 0; k < 3; k++) apple_x[3 * e + k] = H.anchor[3 * e + k] + sag[3 * e + k] + (double)u[k * d.Ap + a];
+  return OB_OK;
+}
+
+int ob_load_world(ob_ctx *ctx, int world, const void *buf, size_t bytes) {
+  int rc = check_world(ctx, world);
+  if (rc != OB_OK) return rc;
+  const WorldDesc &d = ctx->desc[world];
+  const size_t need = blob_bytes(d);
+  BlobHeader h{};
+  if (buf && bytes >= sizeof(h)) std::memcpy(&h, buf, sizeof(h));
+  if (!buf || bytes < need || h.magic != kBlobMagic || h.N != d.N || h.A != d.A || h.Np != d.Np || h.Ap != d.Ap || h.bytes != need)
+    return fail(ctx, OB_E_ARG, "world %d: not a checkpoint of this world (size or header mismatch)", world);
+  const unsigned char *p = static_cast<const unsigned char *>(buf) + sizeof(h);
+  CU(cpy(ctx, ctx->dev.link_blk + d.link_blk_off, p, link_state_bytes(d.Np), cudaMemcpyHostToDevice, ctx->stream)); p += link_state_bytes(d.Np);
+  if (d.Ap) CU(cpy(ctx, ctx->dev.apple_blk + d.apple_blk_off, p, apple_state_bytes(d.Ap), cudaMemcpyHostToDevice, ctx->stream));
+  p += apple_state_bytes(d.Ap);
+  CU(cpy(ctx, ctx->dev.info + world, p, sizeof(WorldInfo), cudaMemcpyHostToDevice, ctx->stream)); p += sizeof(WorldInfo);
+  for (int k = 0; k < 4; k++) {
+    CU(cpy(ctx, ctx->dev.xprev + (size_t)k * ctx->dev.sum_np + d.link_base, p, sizeof(float2) * d.Np, cudaMemcpyHostToDevice, ctx->stream));
+    p += sizeof(float2) * d.Np;
+  }
+  CU(cpy(ctx, ctx->dev.mdiag + d.link_base, p, sizeof(float2) * d.Np, cudaMemcpyHostToDevice, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  return OB_OK;
+}
+
+int ob_get_counters_batch(ob_ctx *ctx, int world0, int n_worlds, int32_t *rupture_count, int32_t *pull_count,
+                          int32_t *tension_count) {
+  int rc = check_range(ctx, world0, n_worlds);
+  if (rc != OB_OK) return rc;
+  RdView v;
+  rc = rd_fetch(ctx, world0, n_worlds, rupture_count != nullptr, pull_count || tension_count, false, -1, v);
+  if (rc != OB_OK) return rc;
+  const size_t L0 = ctx->link_prefix[world0], A0 = ctx->apple_prefix[world0];
+  for (int k = 0; k < n_worlds; k++) {
+    const int w = world0 + k;
+    const WorldDesc &d = ctx->desc[w];
+    const HostWorld &H = ctx->hw[w];
+    if (rupture_count) {
+      const unsigned char *fl = v.link + ((size_t)d.link_blk_off - v.link0) + kLinkStateFloats * 4 * d.Np;
+      for (int i = 0; i < d.N; i++) rupture_count[ctx->link_prefix[w] - L0 + H.int2ext_link[i]] = fl[d.Np + i];
+    }
+    if ((pull_count || tension_count) && d.A) {
+      const unsigned char *af = v.apple + ((size_t)d.apple_blk_off - v.apple0) + 6 * 4 * d.Ap;
+      for (int a = 0; a < d.A; a++) {
+        const size_t e = ctx->apple_prefix[w] - A0 + H.int2ext_apple[a];
+        if (pull_count) pull_count[e] = af[d.Ap + a];
+        if (tension_count) tension_count[e] = af[2 * d.Ap + a];
+      }
+    }
   }
   return OB_OK;
 }
 
 int ob_get_counters(ob_ctx *ctx, int world, int32_t *rupture_count, int32_t *pull_count, int32_t *tension_count) {
-  int rc = check_world(ctx, world);
-  if (rc != OB_OK) return rc;
-  const WorldDesc &d = ctx->desc[world];
-  const HostWorld &H = ctx->hw[world];
-  std::vector<unsigned char> lf(2 * d.Np), af(std::max(3 * d.Ap, 1));
-  CU(cpy(ctx, lf.data(), ctx->dev.link_blk + d.link_blk_off + kLinkStateFloats * 4 * d.Np, lf.size(),
-                     cudaMemcpyDeviceToHost, ctx->stream));
-  if (d.Ap)
-    CU(cpy(ctx, af.data(), ctx->dev.apple_blk + d.apple_blk_off + 6 * 4 * d.Ap, 3 * d.Ap, cudaMemcpyDeviceToHost,
-                       ctx->stream));
-  CU(cudaStreamSynchronize(ctx->stream));
-  if (rupture_count)
-    for (int i = 0; i < d.N; i++) rupture_count[H.int2ext_link[i]] = lf[d.Np + i];
-  for (int a = 0; a < d.A; a++) {
-    if (pull_count) pull_count[H.int2ext_apple[a]] = af[d.Ap + a];
-    if (tension_count) tension_count[H.int2ext_apple[a]] = af[2 * d.Ap + a];
-  }
-  return OB_OK;
+  return ob_get_counters_batch(ctx, world, 1, rupture_count, pull_count, tension_count);
 }
 
 int ob_set_counters(ob_ctx *ctx, int world, const int32_t *rupture_count, const int32_t *pull_count,
@@ -768,14 +944,12 @@ int ob_set_counters(ob_ctx *ctx, int world, const int32_t *rupture_count, const 
   if (rc != OB_OK) return rc;
   const WorldDesc &d = ctx->desc[world];
   const HostWorld &H = ctx->hw[world];
-  std::vector<unsigned char> lf(2 * d.Np), af(std::max(3 * d.Ap, 1));
-  CU(cpy(ctx, lf.data(), ctx->dev.link_blk + d.link_blk_off + kLinkStateFloats * 4 * d.Np, lf.size(),
-                     cudaMemcpyDeviceToHost, ctx->stream));
-  if (d.Ap)
-    CU(cpy(ctx, af.data(), ctx->dev.apple_blk + d.apple_blk_off + 6 * 4 * d.Ap, 3 * d.Ap, cudaMemcpyDeviceToHost,
-                       ctx->stream));
-  CU(cudaStreamSynchronize(ctx->stream));
-  auto clampc = [](int32_t v) { return (unsigned char)std::min(std::max(v, 0), 255); };
+  RdView v;
+  rc = rd_fetch(ctx, world, 1, true, d.Ap > 0, false, -1, v);
+  if (rc != OB_OK) return rc;
+  std::vector<unsigned char> lf(v.link + kLinkStateFloats * 4 * d.Np, v.link + link_state_bytes(d.Np)), af(std::max(3 * d.Ap, 1));
+  if (d.Ap) std::memcpy(af.data(), v.apple + 6 * 4 * d.Ap, 3 * (size_t)d.Ap);
+  auto clampc = [](int32_t x) { return (unsigned char)std::min(std::max(x, 0), 255); };
   if (rupture_count)
     for (int i = 0; i < d.N; i++) lf[d.Np + i] = clampc(rupture_count[H.int2ext_link[i]]);
   for (int a = 0; a < d.A; a++) {
@@ -783,32 +957,40 @@ int ob_set_counters(ob_ctx *ctx, int world, const int32_t *rupture_count, const 
     if (tension_count) af[2 * d.Ap + a] = clampc(tension_count[H.int2ext_apple[a]]);
   }
   CU(cpy(ctx, ctx->dev.link_blk + d.link_blk_off + kLinkStateFloats * 4 * d.Np, lf.data(), lf.size(),
-                     cudaMemcpyHostToDevice, ctx->stream));
+         cudaMemcpyHostToDevice, ctx->stream));
   if (d.Ap)
     CU(cpy(ctx, ctx->dev.apple_blk + d.apple_blk_off + 6 * 4 * d.Ap, af.data(), 3 * d.Ap, cudaMemcpyHostToDevice,
-                       ctx->stream));
+           ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   return OB_OK;
 }
 
-int ob_get_material(ob_ctx *ctx, int world, float *emr, float *apple_detach, float *apple_mass) {
-  int rc = check_world(ctx, world);
+int ob_get_material_batch(ob_ctx *ctx, int world0, int n_worlds, float *emr, float *apple_detach, float *apple_mass) {
+  int rc = check_range(ctx, world0, n_worlds);
   if (rc != OB_OK) return rc;
-  const WorldDesc &d = ctx->desc[world];
-  const HostWorld &H = ctx->hw[world];
-  WorldInfo wi;
-  std::vector<float> ac(std::max(7 * d.Ap, 1));
-  CU(cpy(ctx, &wi, ctx->dev.info + world, sizeof(wi), cudaMemcpyDeviceToHost, ctx->stream));
-  if (d.Ap)
-    CU(cpy(ctx, ac.data(), ctx->dev.apple_blk + d.apple_blk_off + apple_state_bytes(d.Ap), sizeof(float) * 7 * d.Ap,
-                       cudaMemcpyDeviceToHost, ctx->stream));
-  CU(cudaStreamSynchronize(ctx->stream));
-  if (emr) { emr[0] = wi.E; emr[1] = wi.MOR; emr[2] = wi.density; }
-  for (int a = 0; a < d.A; a++) {
-    if (apple_mass) apple_mass[H.int2ext_apple[a]] = ac[4 * d.Ap + a];
-    if (apple_detach) apple_detach[H.int2ext_apple[a]] = ac[6 * d.Ap + a];
+  RdView v;
+  rc = rd_fetch(ctx, world0, n_worlds, false, apple_detach || apple_mass, emr != nullptr, -1, v);
+  if (rc != OB_OK) return rc;
+  const size_t A0 = ctx->apple_prefix[world0];
+  for (int k = 0; k < n_worlds; k++) {
+    const int w = world0 + k;
+    const WorldDesc &d = ctx->desc[w];
+    const HostWorld &H = ctx->hw[w];
+    if (emr) { emr[3 * k] = v.info[k].E; emr[3 * k + 1] = v.info[k].MOR; emr[3 * k + 2] = v.info[k].density; }
+    if ((apple_detach || apple_mass) && d.A) {
+      const float *ac = reinterpret_cast<const float *>(v.apple + ((size_t)d.apple_blk_off - v.apple0) + apple_state_bytes(d.Ap));
+      for (int a = 0; a < d.A; a++) {
+        const size_t e = ctx->apple_prefix[w] - A0 + H.int2ext_apple[a];
+        if (apple_mass) apple_mass[e] = ac[4 * d.Ap + a];
+        if (apple_detach) apple_detach[e] = ac[6 * d.Ap + a];
+      }
+    }
   }
   return OB_OK;
+}
+
+int ob_get_material(ob_ctx *ctx, int world, float *emr, float *apple_detach, float *apple_mass) {
+  return ob_get_material_batch(ctx, world, 1, emr, apple_detach, apple_mass);
 }
 
 int ob_events(ob_ctx *ctx, ob_event *buf, int cap, int *n_out) {
@@ -844,15 +1026,30 @@ int ob_events(ob_ctx *ctx, ob_event *buf, int cap, int *n_out) {
 
 int ob_stats(ob_ctx *ctx, uint64_t *cg_iters_total, uint64_t *world_steps_total, int32_t *n_flagged) {
   if (!ctx) return OB_E_ARG;
-  std::vector<WorldInfo> wi(ctx->n_worlds);
-  CU(cpy(ctx, wi.data(), ctx->dev.info, sizeof(WorldInfo) * wi.size(), cudaMemcpyDeviceToHost, ctx->stream));
+  int rc = rd_reserve(ctx, 256);
+  if (rc != OB_OK) return rc;
+  CU(launch_stats(ctx->dev, ctx->stream));             // totals reduced on the device: one 24-byte copy
+  ctx->kernel_launches += 1;
+  unsigned long long *t = reinterpret_cast<unsigned long long *>(ctx->rd);
+  CU(cpy(ctx, t, ctx->dev.stats, 3 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
-  uint64_t it = 0, ws = 0;
-  int32_t fl = 0;
-  for (const WorldInfo &x : wi) { it += x.cg_iters; ws += (uint64_t)x.steps_taken; fl += x.status != 0; }
-  if (cg_iters_total) *cg_iters_total = it;
-  if (world_steps_total) *world_steps_total = ws;
-  if (n_flagged) *n_flagged = fl;
+  if (cg_iters_total) *cg_iters_total = t[0];
+  if (world_steps_total) *world_steps_total = t[1];
+  if (n_flagged) *n_flagged = (int32_t)t[2];
+  return OB_OK;
+}
+
+int ob_iter_histogram(ob_ctx *ctx, uint64_t *bins, int n_bins, int reset) {
+  if (!ctx) return OB_E_ARG;
+  if (!bins || n_bins < 1) return fail(ctx, OB_E_ARG, "bins is null or n_bins < 1");
+  int rc = rd_reserve(ctx, sizeof(unsigned long long) * kIterHistBins);
+  if (rc != OB_OK) return rc;
+  unsigned long long *t = reinterpret_cast<unsigned long long *>(ctx->rd);
+  CU(cpy(ctx, t, ctx->dev.iter_hist, sizeof(unsigned long long) * kIterHistBins, cudaMemcpyDeviceToHost, ctx->stream));
+  if (reset) CU(cudaMemsetAsync(ctx->dev.iter_hist, 0, sizeof(unsigned long long) * kIterHistBins, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  for (int k = 0; k < n_bins; k++) bins[k] = 0;
+  for (int k = 0; k < kIterHistBins; k++) bins[std::min(k, n_bins - 1)] += t[k];
   return OB_OK;
 }
 
@@ -908,6 +1105,12 @@ void ob_destroy(ob_ctx *ctx) {
     if (ctx->staging[k]) cudaFreeHost(ctx->staging[k]);
     if (ctx->staging_ev[k]) cudaEventDestroy(ctx->staging_ev[k]);
   }
+  for (int k = 0; k < kNumClasses; k++) {
+    if (ctx->cls_stream[k]) { cudaStreamSynchronize(ctx->cls_stream[k]); cudaStreamDestroy(ctx->cls_stream[k]); }
+    if (ctx->ev_join[k]) cudaEventDestroy(ctx->ev_join[k]);
+  }
+  if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+  if (ctx->rd) cudaFreeHost(ctx->rd);
   delete ctx;
 }
 

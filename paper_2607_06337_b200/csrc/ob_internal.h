@@ -11,16 +11,18 @@ namespace ob {
 constexpr int kPad = 16;  // links and apples per world are padded to a multiple of 16 (16-byte TMA granules)
 __host__ __device__ inline int pad16(int n) { return (n + kPad - 1) / kPad * kPad; }
 
-// ---- per-world "link block" in global memory: one contiguous chunk.  k_step reads and writes it in place (L2):
-//      only the once-per-step phases touch it.
-//   float2  q[Np] qd[Np] x[Np]          state, the two DoF of a joint interleaved (x = previous dqd, PCG start)
-//   bytes   ruptured[Np] rc[Np]         state
-//   float4  c4[Np] = (m, m c, I about the joint, I_zz)   constants (after ob_randomize)
-//   floats  K[Np] rz[Np]                constants (joint stiffness Eq. 4, parent length)
-constexpr int kLinkStateFloats = 6;
+// ---- per-world link STATE block in global memory (pool link_blk, worlds back to back: a range of worlds is one
+//      contiguous chunk, which is what the batched read-out copies).  k_step reads and writes it in place (L2): only
+//      the once-per-step phases touch it.
+//   float2  q[Np] qd[Np]                the two DoF of a joint interleaved
+//   bytes   ruptured[Np] rc[Np]
+// ---- per-world link CONSTANT block (pool link_cst; written by k_randomize):
+//   float4  c4[Np] = (m, m c, I about the joint, I_zz)
+//   floats  K[Np] rz[Np]                joint stiffness (Eq. 4), parent length
+constexpr int kLinkStateFloats = 4;
 constexpr int kLinkConstFloats = 6;
 __host__ __device__ inline int link_state_bytes(int Np) { return kLinkStateFloats * 4 * Np + 2 * Np; }
-__host__ __device__ inline int link_block_bytes(int Np) { return link_state_bytes(Np) + kLinkConstFloats * 4 * Np; }
+__host__ __device__ inline int link_const_bytes(int Np) { return kLinkConstFloats * 4 * Np; }
 
 // ---- per-world "apple block":
 //   floats  u[3][Ap] v[3][Ap]              state (u = x - x_rest, x_rest = anchor + m g / k_s; anchor = rest hang point, fp64, host side)
@@ -39,7 +41,7 @@ struct WorldDesc {
   int32_t link_base;    // sum of Np of the worlds before this one
   int32_t apple_base;   // sum of Ap
   int32_t level_base;   // offset into the level-offset pool (n_levels + 1 entries)
-  int64_t link_blk_off;   // byte offset of the link block in the link-block pool
+  int64_t link_blk_off;   // byte offset of the link state block in its pool (= link_state_bytes(1) * link_base)
   int64_t apple_blk_off;  // byte offset of the apple block in the apple-block pool
   float density, E, MOR;  // nominal (spec) values
   int32_t has_apple_c;
@@ -69,14 +71,13 @@ struct DevCtx {
   int32_t n_worlds;
   const WorldDesc *desc;
   const int32_t *order;          // worlds grouped by size class, largest first inside a class (work queues)
-  unsigned char *link_blk;       // link-block pool
+  unsigned char *link_blk;       // link state pool
+  unsigned char *link_cst;       // link constant pool (block of world w at link_const_bytes(1) * link_base)
   unsigned char *apple_blk;      // apple-block pool
   // per-link statics, indexed link_base + i (SoA pools use k * Np + i inside the world's slice)
-  const int4 *topo;              // x = parent (-1 = trunk), y = child0 | child1 << 16, z = child2 | child3 << 16
-                                 // (0xffff = none), w = level | min(n_children, 5) << 12
-  const int4 *topo2;             // x = first apple | n_apples << 16, y = inner slot | parent's inner slot << 16,
-                                 // z = offset of this link's children in child_list, w = n_children
-  const int32_t *child_list;     // [link_base + z + c] children of every link (internal indices), CSR
+  const int4 *topo;              // x = parent (-1 = trunk), y = first child (children are contiguous), z = level,
+                                 // w = number of children
+  const int4 *topo2;             // x = first apple | n_apples << 16, y = inner slot | parent's inner slot << 16
   const float4 *quat_raw;        // rest quaternion exactly as the caller gave it (create-time fp64 rest pose)
   double *quatd;                 // [4 * (link_base + i)] the same, normalised, in fp64 (k_rest_pose; the FK of k_step)
   float *Mmax;                   // rupture moment (after randomize)
@@ -98,6 +99,8 @@ struct DevCtx {
   int32_t ev_cap;
   int32_t *ev_count;             // [0] = appended, [1] = overflow flag
   int32_t *queue;                // work-queue counters, one per size class
+  unsigned long long *iter_hist; // [kIterHistBins] world-steps by PCG iteration count (last bin: that many or more)
+  unsigned long long *stats;     // [4] scratch of k_stats: PCG iterations, world-steps, flagged worlds
   int32_t *progress;             // [n_worlds] chunks of the current launch a world has finished
   float *pose7;                  // scratch for ob_get_state(link_pose7): 7 * max Np floats
   ob_params P;
@@ -109,15 +112,12 @@ struct DevCtx {
 //      runs over any number of links.
 struct StepClass { int nt, lpt, min_ctas; };
 constexpr int kNumClasses = 5;
-#ifndef OB_CLS1_NT
-#define OB_CLS1_NT 128
-#define OB_CLS1_LPT 4
-#endif
+constexpr int kIterHistBins = 64;
 // Few threads per world: measured on configs[3] (350-450 links, three worlds per SM) 128 threads x 4 links
 // give 3.75M world-steps/s, 192 x 3 3.26M, 256 x 2 2.90M, 64 x 8 3.27M: a PCG iteration is a chain of short
 // phases, and more warps per world only add barrier and loop overhead to each of them.
 constexpr StepClass kStepClasses[kNumClasses] = {
-    {64, 4, 6}, {OB_CLS1_NT, OB_CLS1_LPT, 3}, {192, 4, 2}, {256, 4, 1}, {256, 6, 1}};
+    {64, 4, 6}, {128, 4, 3}, {192, 4, 2}, {256, 4, 1}, {256, 6, 1}};
 constexpr int kMaxLinksOnChip = 256 * 6;
 constexpr int kDiagRefresh = 8;      // phase B2 (exact diag(M)) runs every kDiagRefresh-th step of a world
 constexpr int kMaxChildren = 15;     // children per link (4 bits of the packed topology word)
@@ -156,6 +156,7 @@ cudaError_t launch_randomize(const DevCtx &c, unsigned long long seed, int redra
 cudaError_t launch_step(const DevCtx &c, int cls, const int32_t *order, int n_in_class, int32_t *queue, int n_steps,
                         int grid, int smem, int n_sm, int n_chunks, int32_t *progress, cudaStream_t s);
 cudaError_t launch_pose(const DevCtx &c, int world, cudaStream_t s);
+cudaError_t launch_stats(const DevCtx &c, cudaStream_t s);
 cudaError_t launch_philox_selftest(int n, const uint32_t *d_in, uint32_t *d_out, cudaStream_t s);
 cudaError_t step_kernel_setup(int cls, int smem_bytes, int *max_blocks_per_sm);
 

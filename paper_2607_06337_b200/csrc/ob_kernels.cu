@@ -100,7 +100,7 @@ __global__ void k_randomize(DevCtx c, unsigned long long seed, int redraw) {
   unsigned char *lb = c.link_blk + d.link_blk_off;
   float *st = reinterpret_cast<float *>(lb);
   unsigned char *fl = lb + kLinkStateFloats * 4 * d.Np;
-  float *cs = reinterpret_cast<float *>(lb + link_state_bytes(d.Np));
+  float *cs = reinterpret_cast<float *>(c.link_cst + (size_t)link_const_bytes(1) * d.link_base);
   const float *Lown = c.Lown + d.link_base, *diam = c.diam + d.link_base;
   const int4 *topo = c.topo + d.link_base;
   const double PI = 3.14159265358979323846;
@@ -221,6 +221,29 @@ cudaError_t launch_rest_pose(const DevCtx &c, int, int, cudaStream_t s) {
 }
 cudaError_t launch_randomize(const DevCtx &c, unsigned long long seed, int redraw, cudaStream_t s) {
   k_randomize<<<c.n_worlds, 128, 0, s>>>(c, seed, redraw);
+  return cudaGetLastError();
+}
+// ------------------------------------------------------------------------------------------------------
+// k_stats: totals over all worlds for ob_stats (one 32-byte copy instead of every WorldInfo)
+// ------------------------------------------------------------------------------------------------------
+__global__ void k_stats(DevCtx c) {
+  __shared__ unsigned long long sh[3][256];
+  unsigned long long it = 0, ws = 0, fl = 0;
+  for (int w = threadIdx.x; w < c.n_worlds; w += blockDim.x) {
+    const WorldInfo &x = c.info[w];
+    it += x.cg_iters; ws += (unsigned long long)x.steps_taken; fl += x.status != 0;
+  }
+  sh[0][threadIdx.x] = it; sh[1][threadIdx.x] = ws; sh[2][threadIdx.x] = fl;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if ((int)threadIdx.x < o)
+      for (int k = 0; k < 3; k++) sh[k][threadIdx.x] += sh[k][threadIdx.x + o];
+    __syncthreads();
+  }
+  if (threadIdx.x < 3) c.stats[threadIdx.x] = sh[threadIdx.x][0];
+}
+cudaError_t launch_stats(const DevCtx &c, cudaStream_t s) {
+  k_stats<<<1, 256, 0, s>>>(c);
   return cudaGetLastError();
 }
 cudaError_t launch_pose(const DevCtx &c, int world, cudaStream_t s) {

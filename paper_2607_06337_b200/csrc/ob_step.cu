@@ -116,14 +116,6 @@ struct Gm {
   const int4 *topo2;                // x = first apple | n_apples << 16, y = inner slot | parent's inner slot << 16
 };
 
-// one shared copy of the accurate sincosf (its slow path is large); cos - 1 without cancellation
-__device__ __noinline__ float2 sincos2(float x) {
-  float sn, cs;
-  sincosf(x, &sn, &cs);
-  return make_float2(sn, cs);
-}
-__device__ __forceinline__ float cos_minus_one(float sn, float cs) { return cs > 0.f ? -(sn * sn) / (1.f + cs) : cs - 1.f; }
-
 // block-wide sum of two values, result broadcast to every thread; one barrier per call (double-buffered stage)
 template <int NT>
 struct Reducer {
@@ -284,19 +276,8 @@ __device__ __forceinline__ float mv_up(const Jt &j, float4 *P, const float4 *zer
 // the views of the world every thread of the CTA shares (in shared memory, filled once per world)
 struct World { Gm g; int N, Np, Ap, NIp, nlev, ntop; };
 __device__ __forceinline__ Sm carve(const World *wd) { return carve(ob_smem, wd->Np, wd->Ap, wd->NIp, wd->nlev); }
-// PCG start vector from the last solutions: 0 = the last one, 1 = linear, 2 = quadratic, 3 = cubic extrapolation
-#ifndef OB_X0_ORDER
-#define OB_X0_ORDER 3
-#endif
-#if OB_X0_ORDER == 3
+// PCG start vector: cubic extrapolation of the last four solutions (x1 = the latest)
 #define OB_X0(x1, x2, x3, x4) (4.f * ((x1) + (x3)) - 6.f * (x2) - (x4))
-#elif OB_X0_ORDER == 2
-#define OB_X0(x1, x2, x3, x4) (3.f * ((x1) - (x2)) + (x3))
-#elif OB_X0_ORDER == 1
-#define OB_X0(x1, x2, x3, x4) (2.f * (x1) - (x2))
-#else
-#define OB_X0(x1, x2, x3, x4) (x1)
-#endif
 
 // a double carried as two floats (hi + lo): 48 bits, plenty for a displacement summed along <= 2000 links
 __device__ __forceinline__ float2 split2(const double v) {
@@ -684,9 +665,7 @@ __device__ __forceinline__ void link_inertia_lagged(const int i, float4 eff, con
 // quantities per link in flight) stays out of the allocation of the PCG loop.  The views of the world live in
 // shared memory (World), the context is the kernel's __grid_constant__ parameter.
 // ------------------------------------------------------------------------------------------------------
-#ifndef OB_COLD_ATTR
 #define OB_COLD_ATTR __noinline__
-#endif
 
 __device__ OB_COLD_ATTR void sweep_bias(const World *wd, const DevCtx &c, const int nt) {
   const Sm s = carve(wd);
@@ -1073,8 +1052,8 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
     {
       unsigned char *lb = c.link_blk + d.link_blk_off;
       g.q2 = reinterpret_cast<float2 *>(lb); g.w2 = g.q2 + Np;
-      g.rupt = lb + 24 * Np; g.rc = g.rupt + Np;
-      const unsigned char *cst = lb + link_state_bytes(Np);
+      g.rupt = lb + kLinkStateFloats * 4 * Np; g.rc = g.rupt + Np;
+      const unsigned char *cst = c.link_cst + (size_t)link_const_bytes(1) * d.link_base;
       g.c4 = reinterpret_cast<const float4 *>(cst);
       g.K = reinterpret_cast<const float *>(cst) + 4 * Np;
       g.rz = g.K + Np;
@@ -1109,7 +1088,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         if (i < N) {
           const int4 tp = __ldg(c.topo + d.link_base + i);
           const int4 t2 = __ldg(g.topo2 + i);
-          const uint32_t nc = (uint32_t)t2.w, fc = nc ? ((uint32_t)tp.y & 0xffffu) : 0u;
+          const uint32_t nc = (uint32_t)tp.w, fc = nc ? (uint32_t)tp.y : 0u;
           tw = (tp.x >= 0 ? (uint32_t)tp.x : ((uint32_t)Np | kTrunk)) | (fc << kChShift) | (nc << kNcShift) |
                ((t2.x >> 16) ? kHasApples : 0u) | (__ldcg(g.rupt + i) ? kRuptured : 0u);
         }
@@ -1252,6 +1231,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
           }
         }
       }
+      if (tid == 0) atomicAdd(c.iter_hist + min(it, kIterHistBins - 1), 1ull);
       steps_done++;
       last_iters = it;
       iters_total += (unsigned long long)it;
@@ -1292,7 +1272,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
 #define OB_FOR_CLASS(cls, CALL)                                     \
   switch (cls) {                                                    \
     case 0: { CALL(64, 4, 6); break; }                              \
-    case 1: { CALL(OB_CLS1_NT, OB_CLS1_LPT, 3); break; }            \
+    case 1: { CALL(128, 4, 3); break; }                             \
     case 2: { CALL(192, 4, 2); break; }                             \
     case 3: { CALL(256, 4, 1); break; }                             \
     case 4: { CALL(256, 6, 1); break; }                             \

@@ -26,7 +26,7 @@ pytestmark = pytest.mark.gpu
 
 TOL_STEP = 1e-5      # north_star: single step, fp32
 TOL_RUN = 1e-3       # north_star: 200-step trajectory without events
-BIG_N = 1000         # largest world of the heterogeneous edge-case batch (configs[4] asks for 1500: DESIGN.md)
+BIG_N = 1500         # largest world of the heterogeneous edge-case batch: the top of configs[4]'s [100, 1500] range
 NEAR = 1e-4          # north_star: relative margin of a threshold inside which a one-sided event is tolerated
 
 
@@ -326,15 +326,28 @@ def test_config1_event_sets_match_the_oracle_run(variant, branch_fmax):
 # ----------------------------------------------------------------------------------------------------
 # events over long violent runs: lock-step protocol (SURVEY.md 8(c) "Comparison protocol" (iii))
 # ----------------------------------------------------------------------------------------------------
-def _lockstep(sim, refs, specs, n_steps, loads_at):
+def _masked_qd_error(g, o, keep):
+    """A27 norm of the qd block over the DoFs in `keep` only."""
+    d = (g["qd"].astype(np.float64) - o["qd"])[keep]
+    den = max(np.linalg.norm(o["qd"][keep]), 1e-4 * np.sqrt(max(int(keep.sum()), 1)))
+    return float(np.linalg.norm(d) / den)
+
+
+def _lockstep(sim, refs, specs, n_steps, loads_at, on_step=None):
     """Every step: oracle <- GPU state and counters; both advance one step; flags, counters and events of
-    that step must agree.  A one-sided predicate decision is tolerated only within NEAR of its threshold."""
+    that step must agree.  A one-sided predicate decision is tolerated only within NEAR of its threshold, and only
+    for THAT (world, kind, index) in THAT step: every other event key of the step must match, with value within
+    2e-4 and threshold within 1e-6 relative (fp32 against fp64).  `on_step(s)` runs before step s (e.g. a mid-run
+    ob_randomize on both sides) and returns True when materials were redrawn."""
     near = 0
     n_events = 0
-    worst = 0.0
+    errs, errs_rest = [], []
     derived = [r.derived() for r in refs]
     mats = [r.material() for r in refs]
     for s in range(n_steps):
+        if on_step is not None and on_step(s):
+            derived = [r.derived() for r in refs]
+            mats = [r.material() for r in refs]
         loads = loads_at(s)
         if loads:
             _apply(sim, refs, loads)
@@ -344,14 +357,19 @@ def _lockstep(sim, refs, specs, n_steps, loads_at):
         pre_fk = [r.fk() for r in refs]
         sim.step(1)
         oracle.step_many(refs, 1)
-        gev = sorted(_key(e) for e in sim.events())
-        oev = sorted(_key(e) for r in refs for e in r.events())
+        gev = {_key(e): e for e in sim.events()}
+        oev = {_key(e): e for r in refs for e in r.events()}
         n_events += len(gev)
+        near_keys = set()                                        # (world, kind, index) decided within NEAR this step
         for w, r in enumerate(refs):
             e, g, o = _err(sim, r, w)
             if g["status"] & ob.OB_STATUS_NONFINITE:
                 raise AssertionError(f"world {w} went non-finite at step {s}")
-            worst = max(worst, e["max"])
+            errs.append(e["max"])
+            # the same error without the speeds of ruptured joints (free hinges of gram-scale twigs: joint inertia
+            # ~1e-7 kg m^2, the system is ill-conditioned in exactly that DoF)
+            keep = ~np.repeat(o["ruptured"].astype(bool), 2)
+            errs_rest.append(max(e["q"], e["apple_x"], e["apple_v"], _masked_qd_error(g, o, keep)) if not keep.all() else e["max"])
             grc, gca, gcb = sim.get_counters(w)
             orc, oca, ocb = r.get_counters()
             # rupture decisions (flag or counter differs): K |theta| of the NEW q within NEAR of M_max
@@ -360,6 +378,7 @@ def _lockstep(sim, refs, specs, n_steps, loads_at):
                 mu = derived[w]["K"][i] * np.hypot(o["q"][2 * i], o["q"][2 * i + 1])
                 assert abs(mu / derived[w]["Mmax"][i] - 1.0) <= NEAR, ("rupture", s, w, i, mu, derived[w]["Mmax"][i])
                 near += 1
+                near_keys.add((w, 0, int(i)))
             # detach decisions: |f_user| vs f_det (path A) or |f_s| vs kappa f_det (path B), start-of-step forces
             bad = np.nonzero((g["attached"] != o["attached"]) | (((gca != oca) | (gcb != ocb)) & (g["attached"] == 1)))[0]
             for a in bad:
@@ -370,9 +389,25 @@ def _lockstep(sim, refs, specs, n_steps, loads_at):
                 thr = float(np.float32(sim.params.detach_kappa)) * mats[w]["detach"][a]
                 assert abs(fs / thr - 1.0) <= NEAR, ("detach", s, w, a, fs, thr)
                 near += 1
-        if near == 0:
-            assert gev == oev, (s, gev, oev)
-    return dict(near=near, events=n_events, worst_single_step=worst)
+                near_keys.add((w, 1, int(a)))
+        gk = {k for k in gev if (k[0], k[2], k[3]) not in near_keys}
+        ok = {k for k in oev if (k[0], k[2], k[3]) not in near_keys}
+        assert gk == ok, (s, sorted(gk ^ ok))
+        for k in gk:
+            ge, oe = gev[k], oev[k]
+            assert abs(ge[4] - oe[4]) <= 2e-4 * abs(oe[4]) and abs(ge[5] - oe[5]) <= 1e-6 * abs(oe[5]), (s, ge, oe)
+    a = np.sort(np.array(errs))
+    dist = dict(median=float(np.median(a)), p90=float(a[int(0.9 * (len(a) - 1))]), p99=float(a[int(0.99 * (len(a) - 1))]), max=float(a[-1]))
+    return dict(near=near, events=n_events, worst_single_step=float(a[-1]), worst_rest=float(max(errs_rest)), dist=dist)
+
+
+def _assert_lockstep_bound(res):
+    """north_star: 1e-5 per step.  The factor 10 of round 1 survives only for the joint speeds of ruptured (free-hinge)
+    joints; everything else (every other DoF, q, apples) must meet the bound itself."""
+    print("lock-step single-step error distribution:", {k: f"{v:.1e}" for k, v in res["dist"].items()},
+          f"worst outside free hinges {res['worst_rest']:.1e}")
+    assert res["worst_rest"] <= TOL_STEP, res
+    assert res["worst_single_step"] <= 10 * TOL_STEP, res
 
 
 def test_lockstep_event_sets_cascading_ruptures():
@@ -386,7 +421,7 @@ def test_lockstep_event_sets_cascading_ruptures():
     print("lock-step:", res)
     assert res["events"] >= 4, res            # the stress does produce events
     assert res["near"] <= 2, res
-    assert res["worst_single_step"] <= 10 * TOL_STEP, res   # free hinges at the speed clamp included
+    _assert_lockstep_bound(res)
     sim.close()
 
 
@@ -500,15 +535,18 @@ def test_wrench_slots_and_event_drain():
 
 def test_edge_cases_single_link_no_apples_and_heterogeneous_batch():
     """Degenerate and extreme shapes in ONE batch: a 1-link world without apples, a 17-link chain (one more than
-    the 16-link padding granule), configs[0], and a BIG_N-link / 150-apple world (the largest of configs[4])."""
+    the 16-link padding granule), configs[0] (size class 0), a BIG_N-link / 150-apple world (the largest of
+    configs[4]: size class 4, k_step<256,6,1>), and a world of each of the classes 2 and 3 (601-768, 769-1024 links);
+    class 1 (257-512 links) is what every configs[2..3] test runs."""
     rng = np.random.default_rng(3)
     big = stochastic_world(rng, BIG_N - 10, BIG_N, 150, depth_choices=(7, 8))
+    assert big.n_links > 1024
     specs = [chain_spec(1, 0.4, 0.02, root_quat=quat_axis("y", 90.0)),
              chain_spec(17, 1.7, 0.03, root_quat=quat_axis("y", 60.0),
                         apples=[(16, (0, 0, 0.1), 0.2, 2e3, 20.0), (16, (0.01, 0, 0.05), 0.15, 2e3, 15.0),
                                 (3, (0, 0.015, 0.02), 0.25, 2e3, 25.0)]),
              binary_tree_config1(), big,
-             stochastic_world(rng, 600, 640, 60, depth_choices=(6, 7)),      # one world per k_step size class
+             stochastic_world(rng, 600, 640, 60, depth_choices=(6, 7)),
              stochastic_world(rng, 900, 960, 90, depth_choices=(7, 8))]
     P = config_params(4)
     sim, refs = _make(specs, P, seed=31337)
@@ -551,6 +589,45 @@ def test_nonfinite_world_is_frozen_and_flagged():
 # ----------------------------------------------------------------------------------------------------
 # full size, in the launch configuration bench.py times: configs[3] (4096 worlds x 350-450 links, 60 apples)
 # ----------------------------------------------------------------------------------------------------
+def _philox_u32(ctr_rows, key):
+    """Philox4x32-10 of many counters at once (numpy restatement of the published algorithm for the all-worlds
+    comparison; tests/test_gpu_philox.py and the known-answer pin tie the oracle's and the library's generators to
+    cuRAND and to the Random123 vectors, and this routine is checked against the oracle's on a sample below)."""
+    c = np.array(ctr_rows, dtype=np.uint64).reshape(-1, 4).T.copy()
+    k0, k1 = np.uint64(key[0]), np.uint64(key[1])
+    M0, M1, mask = np.uint64(0xD2511F53), np.uint64(0xCD9E8D57), np.uint64(0xFFFFFFFF)
+    for _ in range(10):
+        p0, p1 = M0 * c[0], M1 * c[2]
+        c = np.stack([(p1 >> np.uint64(32)) ^ c[1] ^ k0, p1 & mask, (p0 >> np.uint64(32)) ^ c[3] ^ k1, p0 & mask])
+        k0 = (k0 + np.uint64(0x9E3779B9)) & mask
+        k1 = (k1 + np.uint64(0xBB67AE85)) & mask
+    return c.T.astype(np.uint32)
+
+
+def _uniform32(x, lo, hi):
+    u = (x >> np.uint32(8)).astype(np.float32) * np.float32(2.0 ** -24)
+    lo, hi = np.float32(lo), np.float32(hi)
+    return (u.astype(np.float64) * np.float64(hi - lo) + np.float64(lo)).astype(np.float32)     # fmaf: one rounding
+
+
+def _check_all_philox_draws(sim, specs, P, seed):
+    """Reading A23 for EVERY world and apple of the batch: E, MOR, density, detach force, apple mass, bit-exact."""
+    key = [seed & 0xffffffff, seed >> 32]
+    W = len(specs)
+    m = sim.get_material_batch()
+    o = _philox_u32([[w, 0, 0, 0] for w in range(W)], key)
+    for w in (0, 1, W // 2, W - 1):
+        assert o[w].tolist() == oracle.philox4x32_10([w, 0, 0, 0], key).tolist()
+    assert m["E"].tobytes() == _uniform32(o[:, 0], *P.range_E).tobytes()
+    assert m["MOR"].tobytes() == _uniform32(o[:, 1], *P.range_MOR).tobytes()
+    assert m["density"].tobytes() == _uniform32(o[:, 2], *P.range_density).tobytes()
+    ctr = [[w, a, 1, 0] for w in range(W) for a in range(specs[w].n_apples)]
+    oa = _philox_u32(ctr, key)
+    assert oa[-1].tolist() == oracle.philox4x32_10(ctr[-1], key).tolist()
+    assert m["detach"].tobytes() == _uniform32(oa[:, 0], *P.range_detach).tobytes()
+    assert m["mass"].tobytes() == _uniform32(oa[:, 1], *P.range_apple_mass).tobytes()
+
+
 def test_full_size_config4_sampled_worlds_and_invariants():
     """All 4096 worlds run 20 steps in one launch under the wrench process; every Philox draw is compared;
     eight sampled worlds are compared with the oracle (free run from the randomized rest state); properties
@@ -566,17 +643,8 @@ def test_full_size_config4_sampled_worlds_and_invariants():
     st = sim.stats()
     assert st["world_steps_total"] == 20 * len(specs) and st["n_flagged"] == 0
     assert 2 * 20 * len(specs) <= st["cg_iters_total"] <= 60 * 20 * len(specs)
-    # Philox: every world, bit-exact (the draw is a pure function of (seed, world, apple): reading A23)
-    key = [seed & 0xffffffff, seed >> 32]
-    for w in range(0, len(specs), 1):
-        m = sim.get_material(w) if w % 16 == 0 else None
-        if m is None:
-            continue
-        o = oracle.philox4x32_10([w, 0, 0, 0], key)
-        u = np.float32(o[0] >> 8) * np.float32(2.0 ** -24)
-        lo, hi = np.float32(P.range_E[0]), np.float32(P.range_E[1])
-        expect = np.float32(np.float64(u) * np.float64(hi - lo) + np.float64(lo))   # fmaf: one rounding
-        assert np.float32(m["E"]).tobytes() == expect.tobytes(), w
+    # Philox: every world and every apple, bit-exact (the draw is a pure function of (seed, world, apple): A23)
+    _check_all_philox_draws(sim, specs, P, seed)
     sample = [0, 1, 517, 1023, 2048, 3000, 4000, 4095]
     refs = {w: oracle.OracleWorld(specs[w], P, world_index=w) for w in sample}
     for w, r in refs.items():
@@ -601,4 +669,222 @@ def test_full_size_config4_sampled_worlds_and_invariants():
             worst = max(worst, e["max"])
     print(f"config 4 full size: 20-step worst relative error on sampled worlds {worst:.2e}; "
           f"mean PCG iterations {st['cg_iters_total'] / st['world_steps_total']:.2f}; launch {sim.launch_info()}")
+    sim.close()
+
+
+# ----------------------------------------------------------------------------------------------------
+# configs[4] (heterogeneous, violent, re-randomized mid-run) at reduced length, all five k_step size classes
+# ----------------------------------------------------------------------------------------------------
+def _config5_worlds():
+    """Eight worlds spanning the five size classes of k_step (<= 256, 512, 768, 1024, 1536 links), apples = N / 10."""
+    rng = np.random.default_rng(505)
+    sizes = [(110, 130, (5, 6)), (200, 240, (5, 6, 7)), (300, 340, (6, 7)), (440, 500, (6, 7)), (560, 620, (6, 7)),
+             (700, 760, (7, 8)), (880, 960, (7, 8)), (1180, 1260, (7, 8))]
+    return [stochastic_world(rng, lo, hi, min(max(round(lo / 10), 10), 150), depth_choices=d) for lo, hi, d in sizes]
+
+
+def test_lockstep_config5_protocol_all_size_classes_with_mid_run_randomize():
+    """configs[4]'s protocol at reduced length: loads U(100,600) N, MOR ~ U(30,60) MPa, and an on-device Philox
+    re-randomization + reset of every world in the MIDDLE of the run (ob_randomize(seed + epoch) on both sides), in
+    lock-step against the oracle; event lists bit-exact outside the 1e-4 margin."""
+    specs = _config5_worlds()
+    P = config_params(5)
+    seed = MASTER_SEED + 5000
+    sim, refs = _make(specs, P, seed=seed)
+    classes = sorted({int(np.searchsorted([256, 512, 768, 1024, 1536], -(-s.n_links // 16) * 16)) for s in specs})
+    assert classes == [0, 1, 2, 3, 4], classes
+    n_half = 8
+
+    def on_step(s):
+        if s != n_half:
+            return False
+        sim.randomize(seed + 1)
+        for r in refs:
+            r.randomize(seed + 1)
+            r._x_rest = r.get_state()["apple_x"].copy()
+        mb = sim.get_material_batch()
+        om = [r.material() for r in refs]
+        assert mb["E"].tobytes() == np.array([m["E"] for m in om], np.float32).tobytes()
+        assert mb["MOR"].tobytes() == np.array([m["MOR"] for m in om], np.float32).tobytes()
+        assert mb["detach"].tobytes() == np.concatenate([m["detach"] for m in om]).astype(np.float32).tobytes()
+        return True
+
+    def loads_at(s):
+        if s % n_half == 0:
+            return wrench_process(specs, s // n_half, 100.0, 600.0, seed_offset=5000)
+        return []
+    res = _lockstep(sim, refs, specs, 2 * n_half, loads_at, on_step=on_step)
+    print("config-5 lock-step:", {k: v for k, v in res.items() if k != "dist"})
+    assert res["near"] <= 2, res
+    _assert_lockstep_bound(res)
+    st = sim.get_state_batch()
+    assert (st["info"][:, 0] == n_half).all() and (st["info"][:, 2] & ob.OB_STATUS_NONFINITE == 0).all()
+    sim.close()
+
+
+def test_size_class_4_world_single_step_and_lockstep_under_heavy_wrench():
+    """k_step<256,6,1> (1025-1536 links) against the oracle: a 1500-link / 150-apple world, single steps from a moving
+    state and a short lock-step under a 100-600 N wrench (the oracle needs ~10 s per step at this size)."""
+    rng = np.random.default_rng(1500)
+    big = stochastic_world(rng, BIG_N - 10, BIG_N, 150, depth_choices=(7, 8))
+    assert big.n_links > 1024 and big.n_apples == 150
+    specs = [big]
+    P = config_params(5)
+    sim, refs = _make(specs, P, seed=MASTER_SEED + 5000)
+    _apply(sim, refs, wrench_process(specs, 0, 400.0, 600.0, seed_offset=5000))
+    sim.step(30)
+    e = _single_step_errors(sim, refs, [0])[0]
+    assert e["max"] <= TOL_STEP, e
+    res = _lockstep(sim, refs, specs, 6, lambda s: [])
+    print("class-4 lock-step:", {k: v for k, v in res.items() if k != "dist"})
+    _assert_lockstep_bound(res)
+    sim.close()
+
+
+def test_mixed_class_chunked_launch_is_bit_exact():
+    """The chunked hand-off (several queue items per world and launch) on a batch whose five size-class kernels run
+    side by side on forked streams: step(40) equals 4 x step(10) bit for bit."""
+    specs = make_config(5, 96) + _config5_worlds()
+    P = config_params(5)
+    loads = wrench_process(specs, 0, 100.0, 600.0, seed_offset=5000)
+    sims = [ob.Orchard(specs, P) for _ in range(2)]
+    for sim in sims:
+        sim.randomize(7)
+        sim.apply_wrench_batch([l[0] for l in loads], [l[1] for l in loads], [l[2] for l in loads], [l[3] for l in loads])
+    sims[0].step(40)
+    for _ in range(4):
+        sims[1].step(10)
+    assert sims[0].launch_info()["n_launches"] == 5
+    assert sims[0].stats() == sims[1].stats()
+    assert sorted(sims[0].events()) == sorted(sims[1].events())
+    a, b = sims[0].get_state_batch(), sims[1].get_state_batch()
+    for k in a:
+        assert a[k].tobytes() == b[k].tobytes(), k
+    assert (a["info"][:, 0] == 40).all()
+    for sim in sims:
+        sim.close()
+
+
+# ----------------------------------------------------------------------------------------------------
+# batched read-out, exact checkpoints
+# ----------------------------------------------------------------------------------------------------
+def test_batched_read_out_equals_per_world_read_out():
+    specs = list(_stochastic(78, 150, 250, 20, 5)) + [binary_tree_config1(), chain_spec(1, 0.4, 0.02)]
+    P = config_params(2)
+    sim = ob.Orchard(specs, P)
+    sim.randomize(4243)
+    for (w, body, pt, f) in wrench_process(specs[:5], 0, 0.0, 200.0):
+        sim.apply_wrench(w, body, pt, f)
+    sim.step(60)
+    c0 = sim.counters()
+    full = sim.get_state_batch()
+    part = sim.get_state_batch(2, 4)
+    c1 = sim.counters()
+    cnt = sim.get_counters_batch()
+    mat = sim.get_material_batch()
+    lo = np.cumsum([0] + sim.n_links)
+    ao = np.cumsum([0] + sim.n_apples)
+    for w in range(len(specs)):
+        g = sim.get_state(w)
+        assert g["q"].tobytes() == full["q"][2 * lo[w]:2 * lo[w + 1]].tobytes()
+        assert g["qd"].tobytes() == full["qd"][2 * lo[w]:2 * lo[w + 1]].tobytes()
+        assert g["ruptured"].tobytes() == full["ruptured"][lo[w]:lo[w + 1]].tobytes()
+        assert g["apple_x"].tobytes() == full["apple_x"][ao[w]:ao[w + 1]].tobytes()
+        assert g["apple_x64"].tobytes() == full["apple_x64"][ao[w]:ao[w + 1]].tobytes()
+        assert g["apple_v"].tobytes() == full["apple_v"][ao[w]:ao[w + 1]].tobytes()
+        assert g["attached"].tobytes() == full["attached"][ao[w]:ao[w + 1]].tobytes()
+        assert (g["step"], g["last_iters"], g["status"]) == tuple(full["info"][w])
+        rc, ca, cb = sim.get_counters(w)
+        assert rc.tobytes() == cnt[0][lo[w]:lo[w + 1]].tobytes() and ca.tobytes() == cnt[1][ao[w]:ao[w + 1]].tobytes()
+        m = sim.get_material(w)
+        assert np.float32(m["E"]).tobytes() == mat["E"][w].tobytes() and m["mass"].tobytes() == mat["mass"][ao[w]:ao[w + 1]].tobytes()
+    assert part["q"].tobytes() == full["q"][2 * lo[2]:2 * lo[6]].tobytes()
+    assert part["apple_x64"].tobytes() == full["apple_x64"][ao[2]:ao[6]].tobytes()
+    assert full["ruptured"].sum() > 0 or full["attached"].sum() < full["attached"].size or True
+    # two range calls: a handful of copies in all, not a handful per world
+    assert c1["d2h_bytes"] - c0["d2h_bytes"] < 2.2 * (18 * 16 * sum(-(-n // 16) for n in sim.n_links) + 59 * 16 * sum(-(-n // 16) for n in sim.n_apples) + 48 * len(specs))
+    with pytest.raises(ob.OrchardError):
+        sim.get_state_batch(3, len(specs))
+    sim.close()
+
+
+def test_checkpoints_exact_blob_and_public_state_round_trip():
+    """ob_save_world / ob_load_world: load + step(10) equals the uninterrupted run bit for bit (warm start included).
+    The public route (get_state + apple_x64 + counters + step -> set_*) restores q, qd, the internal apple
+    displacement, flags, counters and the step counter bit for bit; only the PCG warm start is lost, so the
+    continuation agrees to solver tolerance instead."""
+    specs = list(_stochastic(79, 150, 250, 20, 3))
+    P = config_params(2)
+    loads = wrench_process(specs, 0, 0.0, 150.0)
+    a, b, c = (ob.Orchard(specs, P) for _ in range(3))
+    for sim in (a, b, c):
+        sim.randomize(4244)
+        for (w, body, pt, f) in loads:
+            sim.apply_wrench(w, body, pt, f)
+        sim.step(40)
+    blobs = [a.save_world(w) for w in range(len(specs))]
+    pub = [(a.get_state(w), a.get_counters(w)) for w in range(len(specs))]
+    a.step(10)
+    # b: scramble, then restore from the blobs
+    b.step(7)
+    for w in range(len(specs)):
+        b.load_world(w, blobs[w])
+    b.step(10)
+    # c: scramble, then restore through the public state calls
+    c.step(3)
+    for w, (g, cnt) in enumerate(pub):
+        c.set_state(w, q=g["q"], qd=g["qd"], apple_v=g["apple_v"], ruptured=g["ruptured"], attached=g["attached"])
+        c.set_apple_x64(w, g["apple_x64"])
+        c.set_counters(w, *cnt)
+        c.set_step(w, g["step"])
+        r = c.get_state(w)
+        for k in ("q", "qd", "apple_v", "ruptured", "attached", "apple_x64"):
+            assert r[k].tobytes() == g[k].tobytes(), (w, k)
+        assert r["step"] == g["step"] and all(x.tobytes() == y.tobytes() for x, y in zip(c.get_counters(w), cnt))
+    c.step(10)
+    sa, sb, sc = a.get_state_batch(), b.get_state_batch(), c.get_state_batch()
+    for k in sa:
+        assert sa[k].tobytes() == sb[k].tobytes(), k
+    assert (sc["info"][:, 0] == 50).all() and sc["ruptured"].tobytes() == sa["ruptured"].tobytes()
+    assert np.abs(sc["q"] - sa["q"]).max() <= 1e-6 * max(np.abs(sa["q"]).max(), 1e-3)
+    with pytest.raises(ob.OrchardError):
+        b.load_world(0, blobs[1])
+    for sim in (a, b, c):
+        sim.close()
+
+
+def test_saturation_batch_16384_worlds_invariants_and_sampled_parity():
+    """configs[3]'s saturation variant: 16384 worlds (the 4096 geometries four times over, materials by world).  All
+    worlds: finite state, step counter, nothing flagged, Philox draws of EVERY world and apple bit-exact (batched
+    read-out); sampled worlds against the oracle for 20 steps."""
+    base = make_config(4, 4096)
+    specs = [base[w % 4096] for w in range(16384)]
+    P = config_params(4)
+    seed = MASTER_SEED + 4000
+    sim = ob.Orchard(specs, P)
+    sim.randomize(seed)
+    loads = wrench_process(specs, 0, 0.0, 150.0)
+    sim.apply_wrench_batch([l[0] for l in loads], [l[1] for l in loads], [l[2] for l in loads], [l[3] for l in loads])
+    sim.step(20)
+    st = sim.stats()
+    assert st["world_steps_total"] == 20 * len(specs) and st["n_flagged"] == 0
+    full = sim.get_state_batch()
+    assert (full["info"][:, 0] == 20).all() and (full["info"][:, 2] == 0).all()
+    assert np.isfinite(full["q"]).all() and np.isfinite(full["qd"]).all() and np.isfinite(full["apple_x64"]).all()
+    _check_all_philox_draws(sim, specs, P, seed)
+    sample = [4096, 9000, 16383]
+    refs = {w: oracle.OracleWorld(specs[w], P, world_index=w) for w in sample}
+    for w, r in refs.items():
+        r.randomize(seed)
+        r._x_rest = r.get_state()["apple_x"].copy()
+        r.apply_wrench(loads[w][1], loads[w][2], loads[w][3])
+    oracle.step_many(list(refs.values()), 20)
+    gev = {}
+    for e in sim.events():
+        gev.setdefault(e[0], []).append(_key(e))
+    for w, r in refs.items():
+        e, g, o = _err(sim, r, w)
+        assert gev.get(w, []) == [_key(x) for x in r.events()]
+        if not gev.get(w):
+            assert e["max"] <= TOL_RUN, (w, e)
     sim.close()
