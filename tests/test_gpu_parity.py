@@ -735,6 +735,7 @@ def test_size_class_4_world_single_step_and_lockstep_under_heavy_wrench():
     sim.step(30)
     e = _single_step_errors(sim, refs, [0])[0]
     assert e["max"] <= TOL_STEP, e
+    sim.events(); refs[0].events()                      # the lock-step below compares the events of its own steps
     res = _lockstep(sim, refs, specs, 6, lambda s: [])
     print("class-4 lock-step:", {k: v for k, v in res.items() if k != "dist"})
     _assert_lockstep_bound(res)
