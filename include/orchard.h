@@ -79,7 +79,9 @@ typedef struct {
   float c_d;                    /* {0.05} s; D = c_d K (Eq. 4) */
   float cg_tol;                 /* {1e-6} PCG stops at |r| <= cg_tol |b| in the norm selected by cg_norm */
   int32_t cg_max_iter;          /* {200} */
-  int32_t precond;              /* {1} 0 = none, 1 = Jacobi (exact diagonal from a composite-inertia sweep) */
+  int32_t precond;              /* {2} 0 = none, 1 = Jacobi (exact diagonal from a composite-inertia sweep), 2 = the tree
+                                   itself: an articulated-body factorisation of A, exact in exact arithmetic, so PCG
+                                   converges in 1-2 iterations (cg_norm must be 0) */
   int32_t cg_norm;              /* {0} residual norm of the stopping rule: 0 = plain 2-norm; 1 = the preconditioned
                                    norm sqrt(r^T P^-1 r) that PCG carries anyway (one reduction fewer) */
   int32_t rupture_frames;       /* {3} consecutive steps above M_max before a joint ruptures (<= 255) */
@@ -198,8 +200,8 @@ int ob_get_material(ob_ctx *ctx, int world, float *emr, float *apple_detach, flo
 int ob_get_material_batch(ob_ctx *ctx, int world0, int n_worlds, float *emr, float *apple_detach, float *apple_mass);
 
 /* Exact checkpoint of one world: every byte of its mutable state (q, qd, flags, counters, apple state, step and
-   status words, the PCG solution history and preconditioner memory), so that load followed by ob_step(n) reproduces
-   an uninterrupted run bit for bit.  buf: host memory of ob_world_blob_bytes bytes.  A blob only loads into a world
+   status words, the PCG solution history), so that load followed by ob_step(n) reproduces
+   an uninterrupted run bit for bit (PCG solution history included).  buf: host memory of ob_world_blob_bytes bytes.  A blob only loads into a world
    of the same sizes (OB_E_ARG otherwise).  Materials and wrenches are not part of it. */
 int ob_world_blob_bytes(ob_ctx *ctx, int world, size_t *out);
 int ob_save_world(ob_ctx *ctx, int world, void *buf, size_t cap);

@@ -91,7 +91,7 @@ int validate(const ob_world_spec *specs, int n_worlds, const ob_params *P, std::
   if (!specs || !P || n_worlds < 1) { why = "null specs/params or n_worlds < 1"; return OB_E_ARG; }
   if (!(P->h > 0.f) || !(P->cg_tol > 0.f) || P->cg_max_iter < 1 || P->rupture_frames < 1 || P->rupture_frames > 255 ||
       P->detach_frames_pull < 1 || P->detach_frames_pull > 255 || P->detach_frames_tension < 1 ||
-      P->detach_frames_tension > 255 || !(P->react_max >= 0.f) || !(P->c_d >= 0.f) || !(P->mass_damping >= 0.f) || P->precond < 0 || P->precond > 1 || P->cg_norm < 0 || P->cg_norm > 1) {
+      P->detach_frames_tension > 255 || !(P->react_max >= 0.f) || !(P->c_d >= 0.f) || !(P->mass_damping >= 0.f) || P->precond < 0 || P->precond > 2 || P->cg_norm < 0 || P->cg_norm > 1 || (P->precond == 2 && P->cg_norm == 1)) {
     why = "ob_params out of range";
     return OB_E_ARG;
   }
@@ -161,10 +161,30 @@ int level_order(const ob_world_spec &s, std::vector<int32_t> &int2ext, std::vect
   return n_inner;
 }
 inline int pad8(int n) { return (n + 7) / 8 * 8; }
+int count_factor_slots_raw(const ob_world_spec &s);
+// padded number of factor slots a world is laid out with: 0 when it runs without the tree preconditioner, either by
+// ob_params.precond or because the factor planes would not fit into one CTA's shared memory (it then runs Jacobi)
+int world_factor_slots(const ob_world_spec &s, const ob_params &P, int Np, int Ap, int nlev) {
+  if (P.precond != 2) return 0;
+  const int NFp = pad8(count_factor_slots_raw(s));
+  return step_smem_bytes(Np, Ap, NFp, nlev) <= kMaxSmem ? NFp : 0;
+}
+
+// links that need a factor slot for the tree preconditioner: links with children, and leaves that carry an apple off
+// their axis (their articulated inertia is not a body of revolution)
+int count_factor_slots_raw(const ob_world_spec &s) {
+  std::vector<char> need(s.n_links, 0);
+  for (int i = 1; i < s.n_links; i++) need[s.parent[i]] = 1;
+  for (int a = 0; a < s.n_apples; a++)
+    if (s.apple_offset[3 * a] != 0.f || s.apple_offset[3 * a + 1] != 0.f) need[s.apple_link[a]] = 1;
+  int n = 0;
+  for (char c : need) n += c;
+  return n;
+}
 
 struct Layout {
   size_t total = 0;
-  Pool desc, order, link_blk, link_cst, apple_blk, topo, topo2, quat_raw, quatd, Mmax, mdiag, xprev, Lown, diam, arm, link_ext, apple_ext, apple_nom,
+  Pool desc, order, link_blk, link_cst, apple_blk, topo, topo2, quat_raw, quatd, Mmax, xprev, Lown, diam, arm, link_ext, apple_ext, apple_nom,
       apple_c, anchor, level_off, info, wrench, events, ev_count, queue, iter_hist, stats, progress, pose7;
   size_t sumNp = 0, sumAp = 0, sumLev = 0, ev_cap = 0;
   int max_Np = 0, max_Ap = 0, max_smem = 0;
@@ -178,16 +198,17 @@ void take(Layout &L, Pool &p, size_t bytes) {
   L.total += bytes;
 }
 
-int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) {
+int plan(const ob_world_spec *specs, int n_worlds, const ob_params *P, Layout &L, std::string &why) {
   size_t ev = 0;
   for (int w = 0; w < n_worlds; w++) {
     const ob_world_spec &s = specs[w];
     std::vector<int32_t> i2e, lev;
-    const int NIp = pad8(level_order(s, i2e, lev));
+    level_order(s, i2e, lev);
     const int Np = pad16(s.n_links), Ap = pad16(s.n_apples), nlev = (int)lev.size() - 1;
+    const int NFp = world_factor_slots(s, *P, Np, Ap, nlev);
     L.sumNp += Np; L.sumAp += Ap; L.sumLev += nlev + 1;
     L.max_Np = std::max(L.max_Np, Np); L.max_Ap = std::max(L.max_Ap, Ap);
-    const int sm = step_smem_bytes(Np, Ap, NIp, nlev);
+    const int sm = step_smem_bytes(Np, Ap, NFp, nlev);
     int max_kids = 0;
     {
       std::vector<int> nk(s.n_links, 0);
@@ -199,7 +220,7 @@ int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) 
       why = b;
       return OB_E_CAPACITY;
     }
-    if (sm > kMaxSmem || step_class_of(Np) < 0) {
+    if (sm > kMaxSmem || step_class_of(Np, sm) < 0) {
       char b[200];
       snprintf(b, sizeof(b), "world %d (%d links, %d apples) does not fit on chip: %d B of shared memory (limit %d), "
                "%d links (limit %d)", w, s.n_links, s.n_apples, sm, kMaxSmem, s.n_links, kMaxLinksOnChip);
@@ -221,7 +242,6 @@ int plan(const ob_world_spec *specs, int n_worlds, Layout &L, std::string &why) 
   take(L, L.quat_raw, sizeof(float4) * L.sumNp);
   take(L, L.quatd, sizeof(double) * 4 * L.sumNp);
   take(L, L.Mmax, sizeof(float) * L.sumNp);
-  take(L, L.mdiag, sizeof(float2) * L.sumNp);
   take(L, L.xprev, sizeof(float2) * 4 * L.sumNp);
   take(L, L.Lown, sizeof(float) * L.sumNp);
   take(L, L.diam, sizeof(float) * L.sumNp);
@@ -301,7 +321,7 @@ int ob_default_params(ob_params *p) {
   p->c_d = 0.05f;
   p->cg_tol = 1e-6f;
   p->cg_max_iter = 200;
-  p->precond = 1;
+  p->precond = 2;
   p->rupture_frames = 3;
   p->detach_frames_pull = 3;
   p->detach_kappa = 1.1f;
@@ -321,7 +341,7 @@ int ob_workspace_bytes(const ob_world_spec *specs, int n_worlds, const ob_params
   int rc = validate(specs, n_worlds, params, why);
   if (rc != OB_OK) return fail0(rc, why.c_str());
   Layout L;
-  rc = plan(specs, n_worlds, L, why);
+  rc = plan(specs, n_worlds, params, L, why);
   if (rc != OB_OK) return fail0(rc, why.c_str());
   *out = L.total;
   return OB_OK;
@@ -335,7 +355,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   int rc = validate(specs, n_worlds, params, why);
   if (rc != OB_OK) return fail0(rc, why.c_str());
   Layout L;
-  rc = plan(specs, n_worlds, L, why);
+  rc = plan(specs, n_worlds, params, L, why);
   if (rc != OB_OK) return fail0(rc, why.c_str());
   if (!dev_workspace || workspace_bytes < L.total || ((uintptr_t)dev_workspace % kAlign) != 0)
     return fail0(OB_E_WORKSPACE, "workspace null, misaligned (256 B) or smaller than ob_workspace_bytes");
@@ -372,7 +392,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
     const ob_world_spec &s = specs[w];
     HostWorld &H = ctx->hw[w];
     std::vector<int32_t> lev;
-    const int n_inner = level_order(s, H.int2ext_link, lev);
+    level_order(s, H.int2ext_link, lev);
     const int N = s.n_links, A = s.n_apples, Np = pad16(N), Ap = pad16(A), nlev = (int)lev.size() - 1;
     H.ext2int_link.assign(N, 0);
     for (int i = 0; i < N; i++) H.ext2int_link[H.int2ext_link[i]] = i;
@@ -386,10 +406,11 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
     for (int a = 0; a < A; a++) H.ext2int_apple[H.int2ext_apple[a]] = a;
 
     WorldDesc &d = ctx->desc[w];
-    d.N = N; d.A = A; d.Np = Np; d.Ap = Ap; d.NIp = pad8(n_inner); d.n_levels = nlev;
+    d.N = N; d.A = A; d.Np = Np; d.Ap = Ap; d.NFp = world_factor_slots(s, *params, Np, Ap, nlev); d.n_levels = nlev;
+    d.precond = params->precond == 2 && d.NFp == 0 && count_factor_slots_raw(s) > 0 ? 1 : params->precond;
     d.n_top = 0;
     while (d.n_top < nlev && lev[d.n_top + 1] <= 32) d.n_top++;
-    d.cls = step_class_of(Np);
+    d.cls = step_class_of(Np, step_smem_bytes(Np, Ap, d.NFp, nlev));
     d.link_base = (int32_t)link_base; d.apple_base = (int32_t)apple_base; d.level_base = (int32_t)lev_base;
     d.link_blk_off = (int64_t)link_off; d.apple_blk_off = (int64_t)apple_off;
     d.density = s.density; d.E = s.E; d.MOR = s.MOR;
@@ -401,9 +422,12 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
       par[i] = H.ext2int_link[s.parent[H.int2ext_link[i]]];
       kids[par[i]].push_back(i);          // ascending internal index: a fixed summation order
     }
+    std::vector<char> offax(N, 0);
+    for (int a = 0; a < A; a++)
+      if (s.apple_offset[3 * a] != 0.f || s.apple_offset[3 * a + 1] != 0.f) offax[H.ext2int_link[s.apple_link[a]]] = 1;
     for (int i = 0, slot = 0; i < N; i++) {
       n_child[i] = (int32_t)kids[i].size();
-      if (n_child[i]) islot[i] = slot++;
+      if (n_child[i] || offax[i]) islot[i] = slot++;
     }
     for (int a = 0; a < A; a++) {
       const int l = H.ext2int_link[s.apple_link[H.int2ext_apple[a]]];
@@ -418,7 +442,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
       const int p = par[i];
       h_topo[link_base + i] = make_int4(p, n_child[i] ? kids[i][0] : 0, level_of[i], n_child[i]);
       h_topo2[link_base + i] = make_int4(first_apple[i] | (n_apple[i] << 16),
-                                         islot[i] | ((p >= 0 ? islot[p] : 0xffff) << 16), 0, 0);
+                                         islot[i], 0, 0);
       const float *q = s.rest_quat + 4 * e;
       const double n = std::sqrt((double)q[0] * q[0] + (double)q[1] * q[1] + (double)q[2] * q[2] + (double)q[3] * q[3]);
       h_quat_raw[link_base + i] = make_float4(q[0], q[1], q[2], q[3]);
@@ -459,7 +483,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   for (int k = 0; k < n_worlds; k++) {
     const WorldDesc &d = ctx->desc[h_order[k]];
     if (ctx->cls_n[d.cls]++ == 0) ctx->cls_off[d.cls] = k;
-    ctx->cls_smem[d.cls] = std::max(ctx->cls_smem[d.cls], step_smem_bytes(d.Np, d.Ap, d.NIp, d.n_levels));
+    ctx->cls_smem[d.cls] = std::max(ctx->cls_smem[d.cls], step_smem_bytes(d.Np, d.Ap, d.NFp, d.n_levels));
   }
 
   DevCtx &D = ctx->dev;
@@ -474,7 +498,6 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   D.quat_raw = reinterpret_cast<float4 *>(base + L.quat_raw.off);
   D.quatd = reinterpret_cast<double *>(base + L.quatd.off);
   D.Mmax = reinterpret_cast<float *>(base + L.Mmax.off);
-  D.mdiag = reinterpret_cast<float2 *>(base + L.mdiag.off);
   D.xprev = reinterpret_cast<float2 *>(base + L.xprev.off);
   D.sum_np = (int32_t)L.sumNp;
   D.Lown = reinterpret_cast<float *>(base + L.Lown.off);
@@ -799,7 +822,6 @@ int set_state_impl(ob_ctx *ctx, int world, const float *q, const float *qd, cons
     }
   }
   wi.status = 0;
-  wi.diag_age = 0;          // the state was written from outside: recompute the preconditioner at the next step
   if (step) wi.step = *step;
   if (!step || q || qd || apple_x || apple_x64 || apple_v || ruptured || attached)
     for (int k = 0; k < 4; k++)   // ... and forget the solution history the PCG start vector is extrapolated from
@@ -816,7 +838,7 @@ int set_state_impl(ob_ctx *ctx, int world, const float *q, const float *qd, cons
 struct BlobHeader { uint32_t magic; int32_t N, A, Np, Ap; uint32_t bytes; };
 constexpr uint32_t kBlobMagic = 0x4f42574cu;   // "OBWL"
 size_t blob_bytes(const WorldDesc &d) {
-  return sizeof(BlobHeader) + link_state_bytes(d.Np) + apple_state_bytes(d.Ap) + sizeof(WorldInfo) + 5 * sizeof(float2) * (size_t)d.Np;
+  return sizeof(BlobHeader) + link_state_bytes(d.Np) + apple_state_bytes(d.Ap) + sizeof(WorldInfo) + 4 * sizeof(float2) * (size_t)d.Np;
 }
 
 }  // namespace
@@ -878,7 +900,6 @@ int ob_save_world(ob_ctx *ctx, int world, void *buf, size_t cap) {
     CU(cpy(ctx, p, ctx->dev.xprev + (size_t)k * ctx->dev.sum_np + d.link_base, sizeof(float2) * d.Np, cudaMemcpyDeviceToHost, ctx->stream));
     p += sizeof(float2) * d.Np;
   }
-  CU(cpy(ctx, p, ctx->dev.mdiag + d.link_base, sizeof(float2) * d.Np, cudaMemcpyDeviceToHost, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   return OB_OK;
 }
@@ -901,7 +922,6 @@ int ob_load_world(ob_ctx *ctx, int world, const void *buf, size_t bytes) {
     CU(cpy(ctx, ctx->dev.xprev + (size_t)k * ctx->dev.sum_np + d.link_base, p, sizeof(float2) * d.Np, cudaMemcpyHostToDevice, ctx->stream));
     p += sizeof(float2) * d.Np;
   }
-  CU(cpy(ctx, ctx->dev.mdiag + d.link_base, p, sizeof(float2) * d.Np, cudaMemcpyHostToDevice, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   return OB_OK;
 }

@@ -34,7 +34,7 @@ __host__ __device__ inline int apple_block_bytes(int Ap) { return apple_state_by
 
 struct WorldDesc {
   int32_t N, A, Np, Ap;
-  int32_t NIp;          // links with children, padded to a multiple of 8 (phase-A overflow mailbox)
+  int32_t NFp;          // factor slots (links with children, leaves with an off-axis apple), padded to a multiple of 8
   int32_t n_levels;
   int32_t n_top;        // leading levels whose links all lie in [0, 32): swept by warp 0 with __syncwarp only
   int32_t cls;          // size class (index into kStepClasses)
@@ -45,7 +45,9 @@ struct WorldDesc {
   int64_t apple_blk_off;  // byte offset of the apple block in the apple-block pool
   float density, E, MOR;  // nominal (spec) values
   int32_t has_apple_c;
-  int32_t pad_[3];
+  int32_t precond;      // the preconditioner this world runs with: ob_params.precond, or 1 (Jacobi) where the factor planes
+                        // of precond 2 do not fit into one CTA's shared memory beside the world
+  int32_t pad_[2];
 };
 
 struct WorldInfo {       // mutable per-world scalars
@@ -55,7 +57,7 @@ struct WorldInfo {       // mutable per-world scalars
   int32_t steps_taken;           // world-steps actually advanced (frozen worlds do not count)
   unsigned long long cg_iters;   // PCG iterations since ob_create
   float E, MOR, density;         // current material draws
-  int32_t diag_age;              // steps since diag(M) of the Jacobi preconditioner was recomputed (0 = recompute)
+  int32_t pad_;
 };
 
 struct WrenchSlots {     // device mirror of the persistent wrenches of one world (internal body indices)
@@ -81,7 +83,6 @@ struct DevCtx {
   const float4 *quat_raw;        // rest quaternion exactly as the caller gave it (create-time fp64 rest pose)
   double *quatd;                 // [4 * (link_base + i)] the same, normalised, in fp64 (k_rest_pose; the FK of k_step)
   float *Mmax;                   // rupture moment (after randomize)
-  float2 *mdiag;                 // [link_base + i] diag(M) of the two DoF as last computed by phase B2
   float2 *xprev;                 // [4][sumNp]: dqd of the last four steps, slot = step & 3 (PCG start: extrapolation)
   int32_t sum_np;                // stride of xprev
   const float *Lown;             // link length
@@ -119,36 +120,41 @@ constexpr int kIterHistBins = 64;
 constexpr StepClass kStepClasses[kNumClasses] = {
     {64, 4, 6}, {128, 4, 3}, {192, 4, 2}, {256, 4, 1}, {256, 6, 1}};
 constexpr int kMaxLinksOnChip = 256 * 6;
-constexpr int kDiagRefresh = 8;      // phase B2 (exact diag(M)) runs every kDiagRefresh-th step of a world
 constexpr int kMaxChildren = 15;     // children per link (4 bits of the packed topology word)
-inline int step_class_of(int Np) {   // host only
+// the smallest class whose threads cover the links and whose per-SM residency the world's shared memory allows
+inline int class_smem_cap(int min_ctas);
+inline int step_class_of(int Np, int smem_bytes) {   // host only
   for (int k = 0; k < kNumClasses; k++)
-    if (Np <= kStepClasses[k].nt * kStepClasses[k].lpt) return k;
+    if (Np <= kStepClasses[k].nt * kStepClasses[k].lpt && smem_bytes <= class_smem_cap(kStepClasses[k].min_ctas)) return k;
   return -1;
 }
 
-// shared-memory footprint of one world in k_step (bytes); the host uses it to size the launch.  S = Np + 1
-// columns per plane (column Np stays zero: the trunk's parent).
-//   seven float4 planes [S]: M0, M1 (parent <-> child mailboxes, A p), PD (p, diagonal terms), C0..C2 (joint
-//   transform E, c2, s2, parent length), C3 (effective link inertia) | G float2 [S] (b, then 1/diag) |
-//   T uint32 [S] (packed topology + flags) | overflow float4 [3][NIp] (phase A) | level offsets |
-//   apple block (TMA) | six float planes [Ap]: anchor - x_hang (phase A1 -> A2), then f_tether, |f_s| (A2 -> D) | wrench slots
+// shared-memory footprint of one world in k_step (bytes); the host uses it to size the launch and to pick the size
+// class.  Np + 1 records of seven float4 (record Np stays zero: the trunk's parent, missing children) | X21 float
+// [Np + 1] | factor-slot index uint16 [Np + 1] | factor planes: four float4 [NFp] (precond 2), or 1 / diag(A) float2
+// [Np + 1] (precond 0, 1) | level offsets | apple block (TMA) | ten float planes [Ap]: anchor - x_hang (A1 -> A2), then
+// f_tether, |f_s| (A2 -> D); the world quaternion of the apple's link | world quaternions of the wrench links |
+// wrench slots
 __host__ __device__ inline int r16(int b) { return (b + 15) / 16 * 16; }
 __host__ __device__ inline int step_planes_bytes(int Np) { return 7 * 16 * (Np + 1); }
-// phase-A overflow (three float4 per inner link) and the PCG's (x, r) (one float4 per link) share one region
-__host__ __device__ inline int step_ovf_bytes(int Np, int NIp) { return 48 * NIp > 16 * Np ? 48 * NIp : 16 * Np; }
-__host__ __device__ inline int step_smem_bytes(int Np, int Ap, int NIp, int nlev) {
+__host__ __device__ inline int step_fac_bytes(int Np, int NFp) { return 64 * NFp > r16(8 * (Np + 1)) ? 64 * NFp : r16(8 * (Np + 1)); }
+// (a world that runs with precond <= 1 passes NFp = 0)
+__host__ __device__ inline int step_smem_bytes(int Np, int Ap, int NFp, int nlev) {
   int b = 0;
   b += step_planes_bytes(Np);
-  b += r16(8 * (Np + 1));
   b += r16(4 * (Np + 1));
-  b += step_ovf_bytes(Np, NIp);
+  b += r16(2 * (Np + 1));
+  b += step_fac_bytes(Np, NFp);
   b += r16(4 * (nlev + 1));
   b += r16(apple_block_bytes(Ap));
-  b += 6 * 4 * Ap;
+  b += 10 * 4 * Ap;
+  b += 16 * OB_MAX_WRENCH;
   b += (int)sizeof(WrenchSlots);
   return (b + 127) / 128 * 128;
 }
+// the most dynamic shared memory a CTA of a class may use so that min_ctas of them stay resident on an SM (228 KB per
+// SM, 1 KB reserved per CTA, 1 KB for the kernel's static shared memory)
+inline int class_smem_cap(int min_ctas) { return (228 * 1024) / min_ctas - 1024 - 1024; }
 
 // kernel launchers (ob_kernels.cu)
 cudaError_t launch_rest_pose(const DevCtx &c, int total_links_padded, int total_apples_padded, cudaStream_t s);

@@ -160,7 +160,7 @@ __global__ void k_randomize(DevCtx c, unsigned long long seed, int redraw) {
     }
   }
   if (threadIdx.x == 0) {
-    info->step = 0; info->last_iters = 0; info->status = 0; info->diag_age = 0;
+    info->step = 0; info->last_iters = 0; info->status = 0;
     info->E = E; info->MOR = MOR; info->density = rho;
   }
 }

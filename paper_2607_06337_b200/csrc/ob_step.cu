@@ -3,44 +3,49 @@
 // One CTA per world in flight (persistent, work queue per size class), three CTAs of 128 threads per SM at the
 // headline size.  Everything the level-synchronous tree sweeps touch lives in SHARED MEMORY as one 112-byte
 // record of seven float4 per link (stride 7 x 16 B: 128-bit accesses of consecutive links are conflict-free),
-// so the sweep code exists once, is about a thousand instructions long (it has to stay inside the instruction
-// cache: the first versions of this kernel were no_instruction-stalled) and runs over any number of links.
-// The apple block is staged by one TMA bulk copy (UBLKCP) and written back the same way; q, qd and the PCG start
-// vectors stay in global memory (L2): only the once-per-step phases touch them.
+// so the sweep code exists once and runs over any number of links.  The apple block is staged by one TMA bulk copy
+// (UBLKCP) and written back the same way; q, qd and the PCG start vectors stay in global memory (L2): only the
+// once-per-step phases touch them.
 //
-//   A0  flat:      joint transforms R_rel = Q Rx Ry (Eq. 3) in fp64; E = R_rel^T rounded for the dynamics
-//   A1  top-down:  forward kinematics in fp64 (world rotations and positions), hang points of the apples
+//   A0  flat:      joint rotations q_rel = Q qx(theta1) qy(theta2) (Eq. 3) as fp64 quaternions; the fp32
+//                  copy is what the dynamics rotate with
+//   A1  top-down:  forward kinematics in fp64 (world quaternion and position of every link), hang points of the apples
+//   F   bottom-up: the preconditioner of the step.  precond = 2: articulated-body inertias of the tree whose joints
+//                  carry the "armature" arm + h D + h^2 K, i.e. an exact O(N) factorisation of the system matrix
+//                  A = M + M_teth + diag(arm + hD + h^2 K) (Featherstone's articulated-body recursion; A is the
+//                  joint-space inertia of that tree), kept as K_i = U_i D_i^-1 and D_i^-1 per inner link;
+//                  precond = 1: composite inertias -> exact diagonal of M (Jacobi)
 //   A2  top-down:  velocities, bias accelerations, bias force of every link incl. tether reactions (Eq. 6 / Eq. 7,
 //                  PAPER.md:149-161) and user wrenches; leaves finish at once
 //   B1  bottom-up: bias torques of the inner links -> rhs b
-//   B2  bottom-up: composite inertia -> exact diagonal of M for the Jacobi preconditioner (every kDiagRefresh-th
-//                  step; in between the stored diagonal + the current spring-damper terms), effective link inertia
-//   C   matrix-free Jacobi-PCG on (M + M_teth + diag(arm + hD + h^2 K)) dqd = b  (north_star), started from the
-//                  cubic extrapolation of the last four solutions; M v = acceleration-only inverse dynamics:
-//                  top-down a_i, bottom-up f_i, project on S_i
+//   C   matrix-free preconditioned CG on A dqd = b (north_star), started from the cubic extrapolation of the last
+//                  four solutions; A v = acceleration-only inverse dynamics (top-down a_i, bottom-up f_i, project on
+//                  S_i); with precond = 2, z = P^-1 r is one bottom-up and one top-down sweep of the same shape
 //   D   integrate joints and apples; rupture (Eq. 5) and detach predicates
 //
 // Order.  Links are in plain breadth-first order: levels contiguous, the children of a link contiguous.  In the
-// PCG sweeps the leading levels that fit into 32 links (n_top of them) are swept by ONE warp, lane = link, own
+// A v sweeps the leading levels that fit into 32 links (n_top of them) are swept by ONE warp, lane = link, own
 // record in registers, parents and children by shuffle, no barrier; every other level ends with one block
 // barrier; only the deepest level turns around inside the top-down pass (all of its links are leaves).  In the
-// once-per-step sweeps warp 0 takes the leading levels with __syncwarp and every leaf turns around.
+// other sweeps that warp takes the leading levels with __syncwarp.
 //
 // Record of link i (P[7 i + j]); record Np is never written and stays zero: the trunk's parent, missing children.
-//   0, 1  M0, M1   A0: R_rel (fp64); A1: world rotation R (fp64 for an inner link, fp32 for a leaf); A2: parked bias
-//                  force / (n, f) for the parent; B2: composite inertia for the parent; C: (alpha, a) on the way
-//                  down, (n, f) on the way up, A p in M1.zw
-//   2     PD       (p, diagonal terms arm + (h c_d + h^2) K); A0, A1: more of R_rel, R; B2 borrows .xy
-//   3..5  C0..C2   E (parent -> link rotation, row-major), c2, s2, parent length
-//   6     C3       effective link inertia (m, m c, I about the joint, I_zz) incl. on-axis virtual tether masses
-//                  (A15); A0, A1: the rest of R_rel, R
-// Beside the records: G (float2: the ninth entry of R_rel / R as a double, then b, then 1 / diag(A)), T (packed topology word:
-// parent | first child << 11 | children << 22 | flags), and one region shared by the A2 overflow (12 floats per
-// inner link: velocity and bias acceleration for the children) and the PCG's (x, r) (one float4 per link).
+//   0  QR   fp32 quaternion (w,x,y,z) of R_rel; E = R_rel^T maps parent coordinates to link coordinates
+//   1  CS   cos theta2, sin theta2, parent length, packed topology word (parent | first child << 11 | children << 22 |
+//           flags)
+//   2  IN   effective link inertia (m, m c, I about the joint, I_zz) incl. on-axis virtual tether masses (A15)
+//   3  PD   (p, diagonal terms arm + (h c_d + h^2) K)
+//   4, 5  M0, M1   parent <-> child mailbox (six floats); M1.zw = A p, then the solve's D^-1 u, then z
+//   6  XR   (x, r) of the PCG
+// Before the PCG the slots double as mailboxes of the once-per-step sweeps: A0 -> A1 q_rel in fp64 (M0, M1); A1 the
+// fp64 world pose of an inner link for its children (M0, M1, PD, XR.xy); F 21 floats of articulated inertia for the
+// parent (IN, PD, M0, M1, XR + the X21 plane); A2 velocity and bias acceleration of an inner link for its children
+// (XR, IN, PD.xy, M1.zw) beside its parked bias force (M0, M1.xy).  A2 / B1 then leave IN, PD.zw, XR.zw (= b) as the
+// PCG wants them.
 //
 // Spatial vectors are [angular; linear at the link origin] in link coordinates.  Link frame: origin at the
-// proximal joint, +z along the link.  Joint i: R_rel = Q_i Rx(theta1) Ry(theta2); E_i = R_rel^T maps parent
-// coordinates to link coordinates; the joint sits at r = (0,0,L_parent) in the parent frame.
+// proximal joint, +z along the link.  Joint i: R_rel = Q_i Rx(theta1) Ry(theta2); the joint sits at
+// r = (0,0,L_parent) in the parent frame; joint axes in link coordinates S = [(c2, 0, s2), (0, 1, 0)].
 #include <math.h>
 
 #include "ob_device.h"
@@ -51,17 +56,19 @@ namespace ob {
 // packed topology word
 constexpr uint32_t kParMask = 0x7ffu, kChShift = 11, kNcShift = 22, kNcMask = 0xfu;
 constexpr uint32_t kHasApples = 1u << 26, kOffax = 1u << 27, kSnapped = 1u << 28, kRuptured = 1u << 29, kTrunk = 1u << 30;
+constexpr int kQR = 0, kCS = 1, kIN = 2, kPD = 3, kM0 = 4, kM1 = 5, kXR = 6;
+constexpr uint32_t kNoSlot = 0xffffu;
 
 // ------------------------------------------------------------------------------------------------------
 // shared-memory view of one world
 // ------------------------------------------------------------------------------------------------------
 struct Sm {
-  int Np, Ap, NIp;
-  float4 *P;                          // records: P[7 * i + j], j = 0 M0, 1 M1, 2 PD, 3..5 C0..C2, 6 C3
-  float2 *G;
-  uint32_t *T;
-  float4 *ovf;                        // ovf[j * NIp + inner slot], j = 0..2
-  float4 *XR;                         // [Np] (x, r) of the PCG; same memory as ovf (phase A2 / B1 only)
+  int Np, Ap, NFp;
+  float4 *P;                          // records
+  float *X21;                         // [Np + 1] the 21st float of the F mailbox
+  uint16_t *SL;                       // [Np + 1] factor slot of the link (inner links, off-axis tether links) or kNoSlot
+  float4 *FAC;                        // precond 2: four planes [NFp]: K (6 x 2) and D^-1 per slot
+  float2 *IDG;                        // precond 0 / 1: 1 / diag(A) per link (same memory as FAC)
   int *lev;                           // level offsets [n_levels + 1]
   // apple block (TMA)
   float *u, *v;                       // [3][Ap]
@@ -70,6 +77,8 @@ struct Sm {
   float *ft, *fsn;                    // tether force [3][Ap], |f_s| [Ap] (phase A2 -> phase D)
   float *hd;                          // [6][Ap] anchor - x_hang of every apple, fp64 as (hi, lo) pairs (phase A1 -> A2);
                                       // aliases ft, fsn (see carve)
+  float *aq;                          // [4][Ap] world quaternion (fp32) of the apple's link (phase A1 -> A2)
+  float4 *wq;                         // [OB_MAX_WRENCH] world quaternion of the link of each wrench slot
   WrenchSlots *wr;
 };
 
@@ -78,14 +87,14 @@ struct Sm {
 // 64-bit address arithmetic instead of LDS / STS.
 extern __shared__ __align__(128) unsigned char ob_smem[];
 
-__device__ __forceinline__ Sm carve(unsigned char *base, const int Np, const int Ap, const int NIp, const int n_levels) {
+__device__ __forceinline__ Sm carve(unsigned char *base, const int Np, const int Ap, const int NFp, const int n_levels) {
   Sm s;
-  s.Np = Np; s.Ap = Ap; s.NIp = NIp;
+  s.Np = Np; s.Ap = Ap; s.NFp = NFp;
   unsigned char *p = base;
   s.P = reinterpret_cast<float4 *>(p); p += step_planes_bytes(Np);
-  s.G = reinterpret_cast<float2 *>(p); p += r16(8 * (Np + 1));
-  s.T = reinterpret_cast<uint32_t *>(p); p += r16(4 * (Np + 1));
-  s.ovf = reinterpret_cast<float4 *>(p); s.XR = s.ovf; p += step_ovf_bytes(Np, NIp);
+  s.X21 = reinterpret_cast<float *>(p); p += r16(4 * (Np + 1));
+  s.SL = reinterpret_cast<uint16_t *>(p); p += r16(2 * (Np + 1));
+  s.FAC = reinterpret_cast<float4 *>(p); s.IDG = reinterpret_cast<float2 *>(p); p += step_fac_bytes(Np, NFp);
   s.lev = reinterpret_cast<int *>(p); p += r16(4 * (n_levels + 1));
   float *f = reinterpret_cast<float *>(p);
   s.u = f; s.v = f + 3 * Ap;
@@ -94,9 +103,9 @@ __device__ __forceinline__ Sm carve(unsigned char *base, const int Np, const int
   s.ao = f; s.ak = f + 3 * Ap; s.am = f + 4 * Ap; s.ac = f + 5 * Ap; s.afd = f + 6 * Ap;
   p += r16(apple_block_bytes(Ap));
   f = reinterpret_cast<float *>(p);
-  s.ft = f; f += 3 * Ap;
-  s.fsn = f; f += Ap;
-  s.hd = s.ft; f += 2 * Ap;             // hd[0..3] share the memory of ft[0..2], fsn: per apple, phase A2 reads hd, then writes them
+  s.ft = f; s.fsn = f + 3 * Ap; s.hd = f; f += 6 * Ap;   // hd[0..3] share the memory of ft[0..2], fsn: per apple, phase A2
+  s.aq = f; f += 4 * Ap;                                 // reads hd, then writes them
+  s.wq = reinterpret_cast<float4 *>(f); f += 4 * OB_MAX_WRENCH;
   s.wr = reinterpret_cast<WrenchSlots *>(f);
   return s;
 }
@@ -110,11 +119,14 @@ struct Gm {
   const double2 *quatd;             // rest quaternions, normalised, fp64: (w, x), (y, z) of link i at 2 i, 2 i + 1
   const double *anchor;             // [k * Ap + a] rest hang points, world frame, fp64
   const float *Mmax;
-  float2 *mdiag;                    // diag(M) as last computed by phase B2 (the Jacobi preconditioner may lag)
   float2 *hist;                     // [4][sum_np]: dqd of the last four steps, slot = step & 3
   const float *arm;                 // [k * Np + i] or nullptr
-  const int4 *topo2;                // x = first apple | n_apples << 16, y = inner slot | parent's inner slot << 16
+  const int4 *topo2;                // x = first apple | n_apples << 16, y = factor slot (or 0xffff)
 };
+
+// the views of the world every thread of the CTA shares (in shared memory, filled once per world)
+struct World { Gm g; int N, Np, Ap, NFp, nlev, ntop, precond; };
+__device__ __forceinline__ Sm carve(const World *wd) { return carve(ob_smem, wd->Np, wd->Ap, wd->NFp, wd->nlev); }
 
 // block-wide sum of two values, result broadcast to every thread; one barrier per call (double-buffered stage)
 template <int NT>
@@ -159,23 +171,55 @@ __device__ __forceinline__ void push_event(const DevCtx &c, int world, int step,
   }
 }
 
-// joint transform of one link as the sweeps use it
+// ------------------------------------------------------------------------------------------------------
+// joint transform of one link as the sweeps use it: the unit quaternion of R_rel (link -> parent), cos / sin theta2,
+// the parent length, the topology word
+// ------------------------------------------------------------------------------------------------------
 struct Jt {
-  M3 E;                // parent -> link rotation
+  float4 q;            // (w, x, y, z) in (.x, .y, .z, .w)
   float c2, s2, rz;
+  uint32_t tw;
 };
 __device__ __forceinline__ Jt load_jt(const float4 *P, const int i) {
-  const float4 e0 = P[7 * i + 3], e1 = P[7 * i + 4], e2 = P[7 * i + 5];
+  const float4 q = P[7 * i + kQR], c = P[7 * i + kCS];
   Jt j;
-  j.E.a[0] = e0.x; j.E.a[1] = e0.y; j.E.a[2] = e0.z; j.E.a[3] = e0.w;
-  j.E.a[4] = e1.x; j.E.a[5] = e1.y; j.E.a[6] = e1.z; j.E.a[7] = e1.w;
-  j.E.a[8] = e2.x; j.c2 = e2.y; j.s2 = e2.z; j.rz = e2.w;
+  j.q = q; j.c2 = c.x; j.s2 = c.y; j.rz = c.z; j.tw = __float_as_uint(c.w);
   return j;
 }
-__device__ __forceinline__ void store_jt(float4 *P, const int i, const Jt &j) {
-  P[7 * i + 3] = make_float4(j.E.a[0], j.E.a[1], j.E.a[2], j.E.a[3]);
-  P[7 * i + 4] = make_float4(j.E.a[4], j.E.a[5], j.E.a[6], j.E.a[7]);
-  P[7 * i + 5] = make_float4(j.E.a[8], j.c2, j.s2, j.rz);
+// R(q) x  (link -> parent) and R(q)^T x = E x  (parent -> link)
+__device__ __forceinline__ float3 rot_up(const float4 q, const float3 x) {
+  const float3 v = f3(q.y, q.z, q.w);
+  const float3 t = cross(v, x);
+  const float3 t2 = f3(t.x + t.x, t.y + t.y, t.z + t.z);
+  return x + q.x * t2 + cross(v, t2);
+}
+__device__ __forceinline__ float3 rot_down(const float4 q, const float3 x) {
+  const float3 v = f3(q.y, q.z, q.w);
+  const float3 t = cross(v, x);
+  const float3 t2 = f3(t.x + t.x, t.y + t.y, t.z + t.z);
+  return x - q.x * t2 + cross(v, t2);
+}
+__device__ __forceinline__ M3 quat_mat(const float4 q) {   // R(q), row-major
+  const float w = q.x, x = q.y, y = q.z, z = q.w;
+  M3 R;
+  R.a[0] = 1.f - 2.f * (y * y + z * z); R.a[1] = 2.f * (x * y - w * z);       R.a[2] = 2.f * (x * z + w * y);
+  R.a[3] = 2.f * (x * y + w * z);       R.a[4] = 1.f - 2.f * (x * x + z * z); R.a[5] = 2.f * (y * z - w * x);
+  R.a[6] = 2.f * (x * z - w * y);       R.a[7] = 2.f * (y * z + w * x);       R.a[8] = 1.f - 2.f * (x * x + y * y);
+  return R;
+}
+
+struct Force6 { float3 n, f; };
+
+// a spatial vector of the parent (motion) into the link frame: al = E alp, a = E (ap + alp x r), r = (0,0,rz)
+__device__ __forceinline__ void motion_down(const Jt &j, const float3 alp, const float3 ap, float3 &al, float3 &a) {
+  al = rot_down(j.q, alp);
+  a = rot_down(j.q, f3(ap.x + alp.y * j.rz, ap.y - alp.x * j.rz, ap.z));
+}
+// a spatial force of the link into the parent frame: fp = E^T f, np = E^T n + r x fp
+__device__ __forceinline__ void force_up(const Jt &j, const float3 n, const float3 f, float3 &np, float3 &fp) {
+  fp = rot_up(j.q, f);
+  np = rot_up(j.q, n);
+  np.x -= j.rz * fp.y; np.y += j.rz * fp.x;
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -186,7 +230,6 @@ __device__ __forceinline__ void store_jt(float4 *P, const int i, const Jt &j) {
 // ------------------------------------------------------------------------------------------------------
 // virtual tether masses off the link axis (rare: the workloads hang apples on the axis), one by one.  Everything
 // goes in and out by value so that nothing of the caller is forced into local memory.
-struct Force6 { float3 n, f; };
 __device__ __noinline__ Force6 offaxis_tethers(const int4 t2, const float3 al, const float3 a, const unsigned char *att,
                                                const float *ao, const float *ak, const int Ap, const float hh) {
   Force6 r;
@@ -204,13 +247,11 @@ __device__ __noinline__ Force6 offaxis_tethers(const int4 t2, const float3 al, c
   return r;
 }
 
-__device__ __forceinline__ void mv_down(const Jt &j, const float4 *P, const uint32_t tw, const float4 pd, float3 &al,
-                                        float3 &a) {
-  const float4 *par = P + 7 * (int)(tw & kParMask);
-  const float4 u = par[0], v = par[1];
-  const float3 alp = f3(u.x, u.y, u.z), ap = f3(u.w, v.x, v.y);
-  al = mul(j.E, alp) + f3(j.c2 * pd.x, pd.y, j.s2 * pd.x);
-  a = mul(j.E, f3(ap.x + alp.y * j.rz, ap.y - alp.x * j.rz, ap.z));
+__device__ __forceinline__ void mv_down(const Jt &j, const float4 *P, const float4 pd, float3 &al, float3 &a) {
+  const float4 *par = P + 7 * (int)(j.tw & kParMask);
+  const float4 u = par[kM0], v = par[kM1];
+  motion_down(j, f3(u.x, u.y, u.z), f3(u.w, v.x, v.y), al, a);
+  al = al + f3(j.c2 * pd.x, pd.y, j.s2 * pd.x);
 }
 
 // children of a link out of shared memory, added in ascending order: the first four with all loads in flight
@@ -222,7 +263,7 @@ __device__ __forceinline__ void gather_children(const float4 *P, const float4 *z
 #pragma unroll
   for (int k = 0; k < 4; k++) {
     const float4 *q = k < nc ? ch + 7 * k : zero_rec;
-    cu[k] = q[0]; cv[k] = q[1];
+    cu[k] = q[kM0]; cv[k] = q[kM1];
   }
 #pragma unroll
   for (int k = 0; k < 4; k++) {
@@ -231,51 +272,105 @@ __device__ __forceinline__ void gather_children(const float4 *P, const float4 *z
   }
 #pragma unroll 1
   for (int k = 4; k < nc; k++) {
-    const float4 u = ch[7 * k], v = ch[7 * k + 1];
+    const float4 u = ch[7 * k + kM0], v = ch[7 * k + kM1];
     n = n + f3(u.x, u.y, u.z);
     f = f + f3(u.w, v.x, v.y);
   }
 }
 
+// inertia force of the link's own effective inertia (a body of revolution about +z through the joint)
+__device__ __forceinline__ void own_inertia_force(const float4 I, const float3 al, const float3 a, float3 &n, float3 &f) {
+  n = f3(I.z * al.x - I.y * a.y, I.z * al.y + I.y * a.x, I.w * al.z);
+  f = f3(I.x * a.x + I.y * al.y, I.x * a.y - I.y * al.x, I.x * a.z);
+}
+
 template <bool GATHER>
-__device__ __forceinline__ float mv_up(const Jt &j, float4 *P, const float4 *zero_rec, const int i, const uint32_t tw,
-                                       const float4 pd, const float3 al, const float3 a, const Sm &s, const Gm &g,
-                                       const DevCtx &c) {
+__device__ __forceinline__ float mv_up(const Jt &j, float4 *P, const float4 *zero_rec, const int i, const float4 pd,
+                                       const float3 al, const float3 a, const Sm &s, const Gm &g, const DevCtx &c) {
   float4 *rec = P + 7 * i;
-  const float4 I = rec[6];                                    // (m, m c, I about the joint, I_zz)
-  float3 n = f3(I.z * al.x - I.y * a.y, I.z * al.y + I.y * a.x, I.w * al.z);
-  float3 f = f3(I.x * a.x + I.y * al.y, I.x * a.y - I.y * al.x, I.x * a.z);
-  if (tw & kOffax) {
+  float3 n, f;
+  own_inertia_force(rec[kIN], al, a, n, f);
+  if (j.tw & kOffax) {
     const Force6 t = offaxis_tethers(__ldg(g.topo2 + i), al, a, s.att, s.ao, s.ak, s.Ap, c.P.h * c.P.h);
     n = n + t.n; f = f + t.f;
   }
-  if (GATHER) gather_children(P, zero_rec, (int)((tw >> kChShift) & kParMask), (int)((tw >> kNcShift) & kNcMask), n, f);
+  if (GATHER) gather_children(P, zero_rec, (int)((j.tw >> kChShift) & kParMask), (int)((j.tw >> kNcShift) & kNcMask), n, f);
   const float t1 = j.c2 * n.x + j.s2 * n.z + pd.z * pd.x;     // pd = (p0, p1, dt0, dt1)
   const float t2 = n.y + pd.w * pd.y;
-  const float3 fp = mulT(j.E, f);                             // the trunk publishes into its own column, which nobody reads
-  float3 np = mulT(j.E, n);
-  np.x -= j.rz * fp.y; np.y += j.rz * fp.x;
-  rec[0] = make_float4(np.x, np.y, np.z, fp.x);
-  rec[1] = make_float4(fp.y, fp.z, t1, t2);
+  float3 np, fp;                                              // the trunk publishes into its own record, which nobody reads
+  force_up(j, n, f, np, fp);
+  rec[kM0] = make_float4(np.x, np.y, np.z, fp.x);
+  rec[kM1] = make_float4(fp.y, fp.z, t1, t2);
   return pd.x * t1 + pd.y * t2;
 }
 
 // ------------------------------------------------------------------------------------------------------
-// The once-per-step phases, cut into passes that each keep a small working set in registers (a spilled
-// register costs an L2 round trip here: the three CTAs of an SM leave the L1 only ~28 KB):
-//   A0  flat      per link, no dependence on other links: R_rel = Q Rx Ry in fp64 (-> slots 0, 1, 2, 6, G),
-//                 E = R_rel^T rounded (-> C0..C2)
-//   A1  top-down  FK in fp64: R, p of every link (an inner link publishes twelve doubles: slots 0, 1, 2, 6, G and the
-//                 overflow), hang points of the apples (-> hd), snapped flags
-//   A2  top-down  velocities and bias accelerations (inner links publish 12 floats in the overflow); own bias
-//                 force of every link incl. tethers and wrenches; a leaf finishes at once, an inner link
-//                 parks (n, f) in M0, M1.xy
-//   B1  bottom-up inner links: own (n, f) + children -> rhs b (-> G), (n, f) for the parent
+// precond = 2: z = P^-1 r with the factors of phase F.  K = U D^-1 (6 x 2: columns k1, k2 as (angular, linear)) and
+// D^-1 (symmetric 2 x 2) of one link: out of the factor planes for a link with a slot; for a plain leaf (its
+// articulated inertia is its own effective inertia) from the closed form
+//   U1 = (I c2, 0, Izz s2; 0, -mc c2, 0), U2 = (0, I, 0; mc, 0, 0), D = diag(I c2^2 + Izz s2^2 + dt0, I + dt1)
 // ------------------------------------------------------------------------------------------------------
+struct Kf { float3 k1n, k1f, k2n, k2f; float d11, d12, d22; };
+__device__ __forceinline__ Kf load_kf(const Sm &s, const int i, const Jt &j, const float4 I, const float dt0, const float dt1) {
+  Kf k;
+  const uint32_t slot = s.SL[i];
+  if (slot != kNoSlot) {
+    const float4 a = s.FAC[slot], b = s.FAC[s.NFp + slot], cc = s.FAC[2 * s.NFp + slot], d = s.FAC[3 * s.NFp + slot];
+    k.k1n = f3(a.x, a.y, a.z); k.k1f = f3(a.w, b.x, b.y);
+    k.k2n = f3(b.z, b.w, cc.x); k.k2f = f3(cc.y, cc.z, cc.w);
+    k.d11 = d.x; k.d12 = d.y; k.d22 = d.z;
+  } else {
+    const float i11 = __fdividef(1.f, j.c2 * j.c2 * I.z + j.s2 * j.s2 * I.w + dt0), i22 = __fdividef(1.f, I.z + dt1);
+    k.k1n = f3(I.z * j.c2 * i11, 0.f, I.w * j.s2 * i11); k.k1f = f3(0.f, -I.y * j.c2 * i11, 0.f);
+    k.k2n = f3(0.f, I.z * i22, 0.f); k.k2f = f3(I.y * i22, 0.f, 0.f);
+    k.d11 = i11; k.d12 = 0.f; k.d22 = i22;
+  }
+  return k;
+}
 
-// the views of the world every thread of the CTA shares (in shared memory, filled once per world)
-struct World { Gm g; int N, Np, Ap, NIp, nlev, ntop; };
-__device__ __forceinline__ Sm carve(const World *wd) { return carve(ob_smem, wd->Np, wd->Ap, wd->NIp, wd->nlev); }
+// bottom-up turn of one link: u = r - S^T p (p = what the children sent up), publish p + K u in the parent frame,
+// keep y = D^-1 u (M1.zw)
+template <bool GATHER>
+__device__ __forceinline__ void solve_up(const int i, float4 *P, const Sm &s) {
+  float4 *rec = P + 7 * i;
+  const Jt j = load_jt(P, i);
+  const float4 I = rec[kIN], pd = rec[kPD], xr = rec[kXR];
+  const Kf k = load_kf(s, i, j, I, pd.z, pd.w);
+  float3 n = f3(0, 0, 0), f = f3(0, 0, 0);
+  if (GATHER) gather_children(P, P + 7 * s.Np, (int)((j.tw >> kChShift) & kParMask), (int)((j.tw >> kNcShift) & kNcMask), n, f);
+  const float u0 = xr.z - (j.c2 * n.x + j.s2 * n.z), u1 = xr.w - n.y;
+  n = n + u0 * k.k1n + u1 * k.k2n;
+  f = f + u0 * k.k1f + u1 * k.k2f;
+  float3 np, fp;
+  force_up(j, n, f, np, fp);
+  rec[kM0] = make_float4(np.x, np.y, np.z, fp.x);
+  rec[kM1] = make_float4(fp.y, fp.z, k.d11 * u0 + k.d12 * u1, k.d12 * u0 + k.d22 * u1);
+}
+
+// top-down turn: a' = X a_parent, z = y - K^T a', a = a' + S z for the children; z -> M1.zw
+__device__ __forceinline__ void solve_down(const int i, float4 *P, const Sm &s) {
+  float4 *rec = P + 7 * i;
+  const Jt j = load_jt(P, i);
+  const float4 I = rec[kIN], pd = rec[kPD];
+  const float2 y = reinterpret_cast<const float2 *>(rec + kM1)[1];
+  const Kf k = load_kf(s, i, j, I, pd.z, pd.w);
+  const float4 *par = P + 7 * (int)(j.tw & kParMask);
+  const float4 u = par[kM0], v = par[kM1];
+  float3 al, a;
+  motion_down(j, f3(u.x, u.y, u.z), f3(u.w, v.x, v.y), al, a);
+  const float z0 = y.x - (dot(k.k1n, al) + dot(k.k1f, a)), z1 = y.y - (dot(k.k2n, al) + dot(k.k2f, a));
+  if ((j.tw >> kNcShift) & kNcMask) {
+    rec[kM0] = make_float4(al.x + j.c2 * z0, al.y + z1, al.z + j.s2 * z0, a.x);
+    rec[kM1] = make_float4(a.y, a.z, z0, z1);
+  } else {
+    reinterpret_cast<float2 *>(rec + kM1)[1] = make_float2(z0, z1);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------
+// The once-per-step phases, cut into passes that each keep a small working set in registers (a spilled
+// register costs an L2 round trip here: the three CTAs of an SM leave the L1 only ~28 KB).
+// ------------------------------------------------------------------------------------------------------
 // PCG start vector: cubic extrapolation of the last four solutions (x1 = the latest)
 #define OB_X0(x1, x2, x3, x4) (4.f * ((x1) + (x3)) - 6.f * (x2) - (x4))
 
@@ -286,88 +381,86 @@ __device__ __forceinline__ float2 split2(const double v) {
 }
 __device__ __forceinline__ double join2(const float hi, const float lo) { return (double)hi + (double)lo; }
 
-// ---- A0 ----  R_rel = Q Rx(th1) Ry(th2) of one link in fp64 -> the link's own record slots 0, 1, 2, 6 and G (they are
-//               free until the link's turn in A1); E = R_rel^T rounded to fp32, cos / sin th2 and the parent length
-//               -> C0..C2 for the dynamics
-__device__ __forceinline__ void link_joint(const int i, const Sm &s, const Gm &g) {
-  const float2 th = __ldcg(g.q2 + i);
-  const double2 qa = __ldg(g.quatd + 2 * i), qb = __ldg(g.quatd + 2 * i + 1);
-  const float rzf = (s.T[i] & kTrunk) ? 0.f : __ldg(g.rz + i);
-  double Q[9], X[9], Rrel[9];
-  {
-    const double w = qa.x, x = qa.y, y = qb.x, z = qb.y;
-    Q[0] = 1 - 2 * (y * y + z * z); Q[1] = 2 * (x * y - w * z);     Q[2] = 2 * (x * z + w * y);
-    Q[3] = 2 * (x * y + w * z);     Q[4] = 1 - 2 * (x * x + z * z); Q[5] = 2 * (y * z - w * x);
-    Q[6] = 2 * (x * z - w * y);     Q[7] = 2 * (y * z + w * x);     Q[8] = 1 - 2 * (x * x + y * y);
-  }
-  double s1, c1, s2, c2;
-  sincos((double)th.x, &s1, &c1);
-  sincos((double)th.y, &s2, &c2);
-  X[0] = c2;       X[1] = 0.0; X[2] = s2;                           // Rx(th1) Ry(th2)
-  X[3] = s1 * s2;  X[4] = c1;  X[5] = -s1 * c2;
-  X[6] = -c1 * s2; X[7] = s1;  X[8] = c1 * c2;
-#pragma unroll
-  for (int r = 0; r < 3; r++)
-#pragma unroll
-    for (int cc = 0; cc < 3; cc++) Rrel[3 * r + cc] = Q[3 * r] * X[cc] + Q[3 * r + 1] * X[3 + cc] + Q[3 * r + 2] * X[6 + cc];
-  Jt j;                                                              // E = Rrel^T, rounded once
-#pragma unroll
-  for (int r = 0; r < 3; r++)
-#pragma unroll
-    for (int cc = 0; cc < 3; cc++) j.E.a[3 * r + cc] = (float)Rrel[3 * cc + r];
-  j.c2 = (float)c2; j.s2 = (float)s2; j.rz = rzf;
-  store_jt(s.P, i, j);
-  double2 *pr = reinterpret_cast<double2 *>(s.P + 7 * i);
-  pr[0] = make_double2(Rrel[0], Rrel[1]); pr[1] = make_double2(Rrel[2], Rrel[3]); pr[2] = make_double2(Rrel[4], Rrel[5]);
-  pr[6] = make_double2(Rrel[6], Rrel[7]);
-  *reinterpret_cast<double *>(s.G + i) = Rrel[8];
+struct Qd { double w, x, y, z; };
+__device__ __forceinline__ Qd qmul(const Qd a, const Qd b) {
+  Qd r;
+  r.w = a.w * b.w - a.x * b.x - a.y * b.y - a.z * b.z;
+  r.x = a.w * b.x + a.x * b.w + a.y * b.z - a.z * b.y;
+  r.y = a.w * b.y - a.x * b.z + a.y * b.w + a.z * b.x;
+  r.z = a.w * b.z + a.x * b.y - a.y * b.x + a.z * b.w;
+  return r;
+}
+__device__ __forceinline__ void store_qd(float4 *rec, const Qd q) {
+  double2 *pr = reinterpret_cast<double2 *>(rec + kM0);
+  pr[0] = make_double2(q.w, q.x); pr[1] = make_double2(q.y, q.z);
+}
+__device__ __forceinline__ Qd load_qd(const float4 *rec) {
+  const double2 *pr = reinterpret_cast<const double2 *>(rec + kM0);
+  const double2 a = pr[0], b = pr[1];
+  Qd q;
+  q.w = a.x; q.x = a.y; q.y = b.x; q.z = b.y;
+  return q;
 }
 
-// ---- A1 ----  forward kinematics in fp64 (Eq. 3): R_i = R_p Q_i Rx(th1) Ry(th2),
-//               p_i = p_p + R_p (0,0,L_p).  The tether stretch x_a - x_hang is a millimetre-sized difference of
-//               metre-sized positions, k_s = 2e3 N/m turns 1e-8 m of it into the whole error budget of a 3 mm twig:
-//               rest rotations, sin / cos of the joint angles and the chain of products are therefore fp64, and the
-//               hang point of every apple is formed here, where the fp64 pose is at hand.  The dynamics get the
-//               fp32-rounded joint transform E = R_rel^T.
-// Publish of an inner link for its children (twelve doubles): R[0..7] in the record slots 0, 1, 2, 6, R[8] in G,
-// p in the overflow slot.  A leaf keeps its fp32 rotation in slots 0, 1, 2.x for phase A2.
+// ---- A0 ----  q_rel = Q qx(th1) qy(th2) of one link in fp64 (Eq. 3: R_rel = Q Rx(th1) Ry(th2)) -> M0, M1 of the link's
+//               own record for A1; its fp32 copy, cos / sin th2 and the parent length -> QR, CS for the dynamics
+__device__ __forceinline__ void link_joint(const int i, const Sm &s, const Gm &g) {
+  float4 *rec = s.P + 7 * i;
+  const float2 th = __ldcg(g.q2 + i);
+  const double2 qa = __ldg(g.quatd + 2 * i), qb = __ldg(g.quatd + 2 * i + 1);
+  const uint32_t tw = __float_as_uint(rec[kCS].w);
+  const float rzf = (tw & kTrunk) ? 0.f : __ldg(g.rz + i);
+  double s1, c1, s2, c2;
+  sincos(0.5 * (double)th.x, &s1, &c1);
+  sincos(0.5 * (double)th.y, &s2, &c2);
+  Qd Q, b;
+  Q.w = qa.x; Q.x = qa.y; Q.y = qb.x; Q.z = qb.y;
+  b.w = c1 * c2; b.x = s1 * c2; b.y = c1 * s2; b.z = s1 * s2;          // qx(th1) qy(th2)
+  const Qd q = qmul(Q, b);
+  rec[kQR] = make_float4((float)q.w, (float)q.x, (float)q.y, (float)q.z);
+  rec[kCS] = make_float4((float)(c2 * c2 - s2 * s2), (float)(2.0 * s2 * c2), rzf, __uint_as_float(tw));
+  store_qd(rec, q);
+}
+
+// ---- A1 ----  forward kinematics in fp64 (Eq. 3): q_i = q_p q_rel, p_i = p_p + R(q_p) (0,0,L_p).
+//               The tether stretch x_a - x_hang is a millimetre-sized difference of metre-sized positions, k_s = 2e3
+//               N/m turns 1e-8 m of it into the whole error budget of a 3 mm twig: rest rotations, sin / cos of the
+//               joint angles and the chain of products are therefore fp64, and the hang point of every apple is
+//               formed here, where the fp64 pose is at hand.
+// Publish of an inner link for its children (seven doubles): q in M0, M1, p in PD and XR.xy.
 __device__ __forceinline__ void link_fk(const int i, const Sm &s, const Gm &g) {
   float4 *rec = s.P + 7 * i;
-  uint32_t tw = s.T[i];
-  const int4 t2 = __ldg(g.topo2 + i);
-  const bool trunk = (tw & kTrunk) != 0u;
-  double Rrel[9];                                   // Q Rx(th1) Ry(th2) in fp64: phase A0 left it in the link's own slots
-  {
-    const double2 *pr = reinterpret_cast<const double2 *>(rec);
-    const double2 a0 = pr[0], a1 = pr[1], a2 = pr[2], a3 = pr[6];
-    Rrel[0] = a0.x; Rrel[1] = a0.y; Rrel[2] = a1.x; Rrel[3] = a1.y; Rrel[4] = a2.x; Rrel[5] = a2.y; Rrel[6] = a3.x;
-    Rrel[7] = a3.y; Rrel[8] = *reinterpret_cast<const double *>(s.G + i);
-  }
-  const float rzf = rec[5].w;                       // parent length (0 for the trunk), stored with E by phase A0
-  double Rp[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1}, pp[3] = {0, 0, 0};
+  const float4 cs = rec[kCS];
+  uint32_t tw = __float_as_uint(cs.w);
+  const Qd qrel = load_qd(rec);
+  Qd qp;
+  qp.w = 1.0; qp.x = 0.0; qp.y = 0.0; qp.z = 0.0;
+  double pp[3] = {0, 0, 0};
   uint32_t snapped_p = 0u;
-  if (!trunk) {
-    const int par = (int)(tw & kParMask), ps = (int)((uint32_t)t2.y >> 16);
-    const double2 *pr = reinterpret_cast<const double2 *>(s.P + 7 * par);
-    const double2 a0 = pr[0], a1 = pr[1], a2 = pr[2], a3 = pr[6];
-    Rp[0] = a0.x; Rp[1] = a0.y; Rp[2] = a1.x; Rp[3] = a1.y; Rp[4] = a2.x; Rp[5] = a2.y; Rp[6] = a3.x; Rp[7] = a3.y;
-    Rp[8] = *reinterpret_cast<const double *>(s.G + par);
-    const double2 b0 = *reinterpret_cast<const double2 *>(s.ovf + ps);
-    pp[0] = b0.x; pp[1] = b0.y; pp[2] = *reinterpret_cast<const double *>(s.ovf + s.NIp + ps);
-    snapped_p = s.T[par] & kSnapped;
+  if (!(tw & kTrunk)) {
+    const float4 *par = s.P + 7 * (int)(tw & kParMask);
+    qp = load_qd(par);
+    const double2 b0 = *reinterpret_cast<const double2 *>(par + kPD);
+    pp[0] = b0.x; pp[1] = b0.y; pp[2] = *reinterpret_cast<const double *>(par + kXR);
+    snapped_p = __float_as_uint(par[kCS].w) & kSnapped;
   }
-  double R[9], pw[3];
-#pragma unroll
-  for (int r = 0; r < 3; r++)
-#pragma unroll
-    for (int cc = 0; cc < 3; cc++) R[3 * r + cc] = Rp[3 * r] * Rrel[cc] + Rp[3 * r + 1] * Rrel[3 + cc] + Rp[3 * r + 2] * Rrel[6 + cc];
-  const double rz = (double)rzf;
-  pw[0] = pp[0] + rz * Rp[2]; pw[1] = pp[1] + rz * Rp[5]; pw[2] = pp[2] + rz * Rp[8];
+  const Qd q = qmul(qp, qrel);
+  const double rz = (double)cs.z;
+  double pw[3];
+  pw[0] = pp[0] + rz * (2.0 * (qp.x * qp.z + qp.w * qp.y));
+  pw[1] = pp[1] + rz * (2.0 * (qp.y * qp.z - qp.w * qp.x));
+  pw[2] = pp[2] + rz * (1.0 - 2.0 * (qp.x * qp.x + qp.y * qp.y));
   tw = (tw & ~kSnapped) | (((tw & kRuptured) || snapped_p) ? kSnapped : 0u);
-  s.T[i] = tw;
+  rec[kCS].w = __uint_as_float(tw);
+  const float4 qf = make_float4((float)q.w, (float)q.x, (float)q.y, (float)q.z);
   // hang points of the apples on this link: anchor - x_hang (the anchor is the rest hang point, fp64)
   if (tw & kHasApples) {
+    const int4 t2 = __ldg(g.topo2 + i);
     const int Ap = s.Ap, ast = t2.x & 0xffff, nap = t2.x >> 16;
+    double R[9];
+    R[0] = 1 - 2 * (q.y * q.y + q.z * q.z); R[1] = 2 * (q.x * q.y - q.w * q.z);     R[2] = 2 * (q.x * q.z + q.w * q.y);
+    R[3] = 2 * (q.x * q.y + q.w * q.z);     R[4] = 1 - 2 * (q.x * q.x + q.z * q.z); R[5] = 2 * (q.y * q.z - q.w * q.x);
+    R[6] = 2 * (q.x * q.z - q.w * q.y);     R[7] = 2 * (q.y * q.z + q.w * q.x);     R[8] = 1 - 2 * (q.x * q.x + q.y * q.y);
     for (int a = ast; a < ast + nap; a++) {
       const double ox = s.ao[a], oy = s.ao[Ap + a], oz = s.ao[2 * Ap + a];
 #pragma unroll
@@ -376,21 +469,51 @@ __device__ __forceinline__ void link_fk(const int i, const Sm &s, const Gm &g) {
         const float2 dd = split2(__ldg(g.anchor + (size_t)k * Ap + a) - xh);
         s.hd[(2 * k) * Ap + a] = dd.x; s.hd[(2 * k + 1) * Ap + a] = dd.y;
       }
+      s.aq[a] = qf.x; s.aq[Ap + a] = qf.y; s.aq[2 * Ap + a] = qf.z; s.aq[3 * Ap + a] = qf.w;
     }
   }
+  for (int k = 0; k < s.wr->n; k++)
+    if (s.wr->body[k] == i) s.wq[k] = qf;
   if ((tw >> kNcShift) & kNcMask) {
-    const int is = t2.y & 0xffff;
-    double2 *pr = reinterpret_cast<double2 *>(rec);
-    pr[0] = make_double2(R[0], R[1]); pr[1] = make_double2(R[2], R[3]); pr[2] = make_double2(R[4], R[5]);
-    pr[6] = make_double2(R[6], R[7]);
-    *reinterpret_cast<double *>(s.G + i) = R[8];
-    *reinterpret_cast<double2 *>(s.ovf + is) = make_double2(pw[0], pw[1]);
-    *reinterpret_cast<double *>(s.ovf + s.NIp + is) = pw[2];
-  } else {
-    rec[0] = make_float4((float)R[0], (float)R[1], (float)R[2], (float)R[3]);
-    rec[1] = make_float4((float)R[4], (float)R[5], (float)R[6], (float)R[7]);
-    rec[2] = make_float4((float)R[8], 0.f, 0.f, 0.f);
+    store_qd(rec, q);
+    *reinterpret_cast<double2 *>(rec + kPD) = make_double2(pw[0], pw[1]);
+    *reinterpret_cast<double *>(rec + kXR) = pw[2];
   }
+}
+
+// diagonal terms of the two DoF of a joint: arm + (h c_d + h^2) K (Eq. 4; a ruptured joint has K = D = 0)
+__device__ __forceinline__ float2 diag_terms(const int i, const uint32_t tw, const float Ki, const Sm &s, const Gm &g,
+                                             const ob_params &P) {
+  const float Kt = (tw & kRuptured) ? 0.f : Ki;
+  float dt0 = (P.h * P.c_d + P.h * P.h) * Kt, dt1 = dt0;
+  if (g.arm) {
+    dt0 += __ldg(g.arm + i);
+    dt1 += __ldg(g.arm + s.Np + i);
+  }
+  return make_float2(dt0, dt1);
+}
+
+// effective link inertia (m, m c, I about the joint, I_zz): the link's own, times (1 + h alpha) for the implicit
+// mass-proportional damping (A32), plus the virtual tether masses h^2 k_s of the attached apples that hang on the
+// link axis (A15).  Apples off the axis set kOffax in the returned topology word and are added one by one.
+__device__ __forceinline__ float4 eff_inertia(const int i, uint32_t &tw, float4 c4, const Sm &s, const Gm &g,
+                                              const ob_params &P) {
+  const float sc = 1.f + P.h * P.mass_damping;
+  c4.x *= sc; c4.y *= sc; c4.z *= sc; c4.w *= sc;
+  if (P.tether_implicit && (tw & kHasApples)) {
+    tw &= ~kOffax;
+    const int Ap = s.Ap;
+    const int4 t2 = __ldg(g.topo2 + i);
+    const int ast = t2.x & 0xffff, nap = t2.x >> 16;
+    for (int a = ast; a < ast + nap; a++) {
+      if (!s.att[a]) continue;
+      const float mv = P.h * P.h * s.ak[a];                     // virtual point mass h^2 k_s at the hang point
+      const float3 o = f3(s.ao[a], s.ao[Ap + a], s.ao[2 * Ap + a]);
+      if (o.x == 0.f && o.y == 0.f) { c4.x += mv; c4.y += mv * o.z; c4.z += mv * o.z * o.z; }   // stays a body of revolution
+      else tw |= kOffax;
+    }
+  }
+  return c4;
 }
 
 // tether reactions (Eq. 6 / Eq. 7) and user wrenches on one link, subtracted from its bias
@@ -405,23 +528,11 @@ __device__ __noinline__ Force6 external_forces(const int i, const float3 om, con
   const int Ap = s.Ap;
   Force6 out;
   out.n = f3(0, 0, 0); out.f = f3(0, 0, 0);
-  M3 R;                                   // world rotation of the link (phase A1): fp64 publish of an inner link, fp32 of a leaf
-  if ((tw >> kNcShift) & kNcMask) {
-    const double2 *pr = reinterpret_cast<const double2 *>(s.P + 7 * i);
-    const double2 a0 = pr[0], a1 = pr[1], a2 = pr[2], a3 = pr[6];
-    R.a[0] = (float)a0.x; R.a[1] = (float)a0.y; R.a[2] = (float)a1.x; R.a[3] = (float)a1.y; R.a[4] = (float)a2.x;
-    R.a[5] = (float)a2.y; R.a[6] = (float)a3.x; R.a[7] = (float)a3.y;
-    R.a[8] = (float)*reinterpret_cast<const double *>(s.G + i);
-  } else {
-    const float4 *rec = s.P + 7 * i;
-    const float4 r0 = rec[0], r1 = rec[1];
-    R.a[0] = r0.x; R.a[1] = r0.y; R.a[2] = r0.z; R.a[3] = r0.w;
-    R.a[4] = r1.x; R.a[5] = r1.y; R.a[6] = r1.z; R.a[7] = r1.w; R.a[8] = rec[2].x;
-  }
   const int ast = apples & 0xffff, nap = apples >> 16;          // first apple | count << 16 (topo2.x, loaded by the caller)
   const float eta_h = P.tether_implicit ? P.h : 0.f;
   for (int a = ast; a < ast + nap; a++) {
     if (!s.att[a]) continue;
+    const float4 qw = make_float4(s.aq[a], s.aq[Ap + a], s.aq[2 * Ap + a], s.aq[3 * Ap + a]);   // world rotation of the link
     const float3 o = f3(s.ao[a], s.ao[Ap + a], s.ao[2 * Ap + a]);
     const float ks = s.ak[a], cdamp = s.ac[a], ma = s.am[a];
     // x_a - x_hang = (anchor - x_hang) + sag + u: the apple is stored as u = x_a - (anchor + sag), sag = m g / k_s,
@@ -430,7 +541,7 @@ __device__ __noinline__ Force6 external_forces(const int i, const float3 om, con
     const float3 st = f3((float)(join2(s.hd[a], s.hd[Ap + a]) + mk * (double)P.gravity[0] + (double)s.u[a]),
                          (float)(join2(s.hd[2 * Ap + a], s.hd[3 * Ap + a]) + mk * (double)P.gravity[1] + (double)s.u[Ap + a]),
                          (float)(join2(s.hd[4 * Ap + a], s.hd[5 * Ap + a]) + mk * (double)P.gravity[2] + (double)s.u[2 * Ap + a]));
-    const float3 vh = mul(R, vl + cross(om, o));                          // world velocity of the hang point
+    const float3 vh = rot_up(qw, vl + cross(om, o));                      // world velocity of the hang point
     const float3 fs = (-ks) * st;
     const float3 va = f3(s.v[a], s.v[Ap + a], s.v[2 * Ap + a]);
     s.ft[a] = fs.x - cdamp * va.x; s.ft[Ap + a] = fs.y - cdamp * va.y; s.ft[2 * Ap + a] = fs.z - cdamp * va.z;
@@ -439,7 +550,7 @@ __device__ __noinline__ Force6 external_forces(const int i, const float3 om, con
                    ks * (st.z - eta_h * vh.z) - ma * P.gravity[2]);
     const float nr = sqrtf(dot(fr, fr));
     if (nr > P.react_max) fr = (P.react_max / nr) * fr;                   // clamp
-    const float3 fl = mulT(R, fr);
+    const float3 fl = rot_down(qw, fr);
     out.f = out.f - fl;
     out.n = out.n - cross(o, fl);
   }
@@ -448,7 +559,7 @@ __device__ __noinline__ Force6 external_forces(const int i, const float3 om, con
   for (int q = 0; q < nwr; q++) {
     if (s.wr->body[q] != i) continue;
     if ((tw & kSnapped) && P.forces_off_on_snapped) continue;
-    const float3 fl = mulT(R, f3(s.wr->force[q][0], s.wr->force[q][1], s.wr->force[q][2]));
+    const float3 fl = rot_down(s.wq[q], f3(s.wr->force[q][0], s.wr->force[q][1], s.wr->force[q][2]));
     const float3 pt = f3(s.wr->point[q][0], s.wr->point[q][1], s.wr->point[q][2]);
     out.f = out.f - fl;
     out.n = out.n - cross(pt, fl);
@@ -456,69 +567,63 @@ __device__ __noinline__ Force6 external_forces(const int i, const float3 om, con
   return out;
 }
 
-// project the accumulated bias force on the joint axes -> rhs b (G[i]), the diagonal terms of both DoF (PD[i].zw),
-// and publish (n, f) in the parent frame (M0[i], M1[i].xy)
-// (th, w, Ki = q, qd, K of the joint: the caller loads them at the top of its turn, with its other global inputs)
-__device__ __forceinline__ void finish_bias(const Jt &j, const int i, const uint32_t tw, const float2 th, const float2 w,
-                                            const float Ki, float3 n, float3 f, const Sm &s, const Gm &g,
+// project the accumulated bias force on the joint axes -> rhs b (XR[i].zw), the diagonal terms of both DoF (PD[i].zw),
+// the effective inertia (IN[i]), and publish (n, f) in the parent frame (M0[i], M1[i].xy)
+// (th, w, Ki, c4 = q, qd, K, inertia of the link: the caller loads them at the top of its turn, with its other global
+// inputs)
+__device__ __forceinline__ void finish_bias(const Jt &j, const int i, const float2 th, const float2 w, const float Ki,
+                                            const float4 c4, float3 n, float3 f, const Sm &s, const Gm &g,
                                             const DevCtx &c) {
   const ob_params &P = c.P;
   float4 *rec = s.P + 7 * i;
+  uint32_t tw = j.tw;
   // spring-damper part of the rhs and of the diagonal (Eq. 4); a ruptured joint has K = D = 0
   const float Kt = (tw & kRuptured) ? 0.f : Ki, Dt = P.c_d * Kt;
   const float2 kq = make_float2(Kt * th.x + (Dt + P.h * Kt) * w.x, Kt * th.y + (Dt + P.h * Kt) * w.y);
-  s.G[i] = make_float2(P.h * (-(j.c2 * n.x + j.s2 * n.z) - kq.x), P.h * (-n.y - kq.y));
-  float dt0 = (P.h * P.c_d + P.h * P.h) * Kt, dt1 = dt0;
-  if (g.arm) {
-    dt0 += __ldg(g.arm + i);
-    dt1 += __ldg(g.arm + s.Np + i);
-  }
-  reinterpret_cast<float2 *>(rec + 2)[1] = make_float2(dt0, dt1);            // arm + (h c_d + h^2) K per DoF
+  reinterpret_cast<float2 *>(rec + kXR)[1] = make_float2(P.h * (-(j.c2 * n.x + j.s2 * n.z) - kq.x), P.h * (-n.y - kq.y));
+  reinterpret_cast<float2 *>(rec + kPD)[1] = diag_terms(i, tw, Ki, s, g, P);
+  rec[kIN] = eff_inertia(i, tw, c4, s, g, P);
+  if (tw != j.tw) rec[kCS].w = __uint_as_float(tw);
   if (!(tw & kTrunk)) {
-    const float3 fp = mulT(j.E, f);
-    float3 np = mulT(j.E, n);
-    np.x -= j.rz * fp.y; np.y += j.rz * fp.x;
-    rec[0] = make_float4(np.x, np.y, np.z, fp.x);
-    *reinterpret_cast<float2 *>(rec + 1) = make_float2(fp.y, fp.z);
+    float3 np, fp;
+    force_up(j, n, f, np, fp);
+    rec[kM0] = make_float4(np.x, np.y, np.z, fp.x);
+    *reinterpret_cast<float2 *>(rec + kM1) = make_float2(fp.y, fp.z);
   }
 }
 
 // ---- A2 ----  velocity, bias acceleration (gravity as base acceleration), own bias force
 //               f = I a + v x* I v - tether reactions - user wrenches  (RNEA with qdd = 0)
+// An inner link leaves (om, vl, al, aln) for its children in XR, IN, PD.xy, M1.zw and parks its force in M0, M1.xy.
 __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm &s, const Gm &g, const DevCtx &c) {
   const ob_params &P = c.P;
-  const int NIp = s.NIp;
-  const uint32_t tw = s.T[i];
+  float4 *rec = s.P + 7 * i;
   const float2 w = __ldcg(g.w2 + i), th = __ldcg(g.q2 + i);       // all global inputs of the link's turn at once
   const float4 c4 = __ldg(g.c4 + i);
   const float Ki = __ldg(g.K + i);
-  const int4 t2g = __ldg(g.topo2 + i);
-  const int ty = t2g.y;                                           // inner slot | parent's inner slot << 16
   const Jt j = load_jt(s.P, i);
+  const uint32_t tw = j.tw;
   float3 wp = f3(0, 0, 0), vp = f3(0, 0, 0), alp = f3(0, 0, 0);
   float3 ap = f3(-P.gravity[0], -P.gravity[1], -P.gravity[2]);   // world = parent of the trunk: at rest, (0; -g)
   if (!(tw & kTrunk)) {
-    const int ps = (int)((uint32_t)ty >> 16);
-    const float4 t0 = s.ovf[ps], t1 = s.ovf[NIp + ps], t2 = s.ovf[2 * NIp + ps];
+    const float4 *par = s.P + 7 * (int)(tw & kParMask);
+    const float4 t0 = par[kXR], t1 = par[kIN];
+    const float2 t2 = *reinterpret_cast<const float2 *>(par + kPD), t3 = reinterpret_cast<const float2 *>(par + kM1)[1];
     wp = f3(t0.x, t0.y, t0.z); vp = f3(t0.w, t1.x, t1.y);
-    alp = f3(t1.z, t1.w, t2.x); ap = f3(t2.y, t2.z, t2.w);
+    alp = f3(t1.z, t1.w, t2.x); ap = f3(t2.y, t3.x, t3.y);
   }
-  const float rz = j.rz, c2 = j.c2, s2 = j.s2;
+  const float c2 = j.c2, s2 = j.s2;
   const float3 vJ = f3(c2 * w.x, w.y, s2 * w.x);
-  const float3 om = mul(j.E, wp) + vJ;
-  const float3 vl = mul(j.E, f3(vp.x + wp.y * rz, vp.y - wp.x * rz, vp.z));
+  float3 om, vl, al, aln;
+  motion_down(j, wp, vp, om, vl);
+  om = om + vJ;
+  motion_down(j, alp, ap, al, aln);
   const float ww = w.x * w.y;
   // mass-proportional damping (A32): its generalized force -alpha M qd enters the bias pass as the
   // joint acceleration alpha qd, i.e. alpha S qd = alpha vJ on top of the velocity-product terms
-  const float3 al = mul(j.E, alp) + f3(-s2 * ww, 0.f, c2 * ww) + cross(om, vJ) + P.mass_damping * vJ;
-  const float3 aln = mul(j.E, f3(ap.x + alp.y * rz, ap.y - alp.x * rz, ap.z)) + cross(vl, vJ);
+  al = al + f3(-s2 * ww, 0.f, c2 * ww) + cross(om, vJ) + P.mass_damping * vJ;
+  aln = aln + cross(vl, vJ);
   const bool inner = ((tw >> kNcShift) & kNcMask) != 0u;
-  if (inner) {
-    const int is = ty & 0xffff;
-    s.ovf[is] = make_float4(om.x, om.y, om.z, vl.x);
-    s.ovf[NIp + is] = make_float4(vl.y, vl.z, al.x, al.y);
-    s.ovf[2 * NIp + is] = make_float4(al.z, aln.x, aln.y, aln.z);
-  }
   // f = I a + v x* I v  (cylinder: com on +z)
   const float m = c4.x, mc = c4.y, Io = c4.z, Iz = c4.w;
   float3 n = f3(Io * al.x - mc * aln.y, Io * al.y + mc * aln.x, Iz * al.z);
@@ -530,130 +635,205 @@ __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm
   bool ext = (tw & kHasApples) != 0u;
   for (int q = 0; q < s.wr->n; q++) ext |= s.wr->body[q] == i;
   if (ext) {
+    const int4 t2g = __ldg(g.topo2 + i);
     const Force6 e = external_forces(i, om, vl, tw, t2g.x, wd, c);
     n = n + e.n; f = f + e.f;
   }
   if (inner) {                                                    // parked until B1 adds the children
-    s.P[7 * i] = make_float4(n.x, n.y, n.z, f.x);
-    *reinterpret_cast<float2 *>(s.P + 7 * i + 1) = make_float2(f.y, f.z);
+    const float2 dt = diag_terms(i, tw, Ki, s, g, P);
+    rec[kXR] = make_float4(om.x, om.y, om.z, vl.x);
+    rec[kIN] = make_float4(vl.y, vl.z, al.x, al.y);
+    rec[kPD] = make_float4(al.z, aln.x, dt.x, dt.y);
+    rec[kM0] = make_float4(n.x, n.y, n.z, f.x);
+    rec[kM1] = make_float4(f.y, f.z, aln.y, aln.z);
   } else {
-    finish_bias(j, i, tw, th, w, Ki, n, f, s, g, c);
+    finish_bias(j, i, th, w, Ki, c4, n, f, s, g, c);
   }
 }
 
 // ---- B1 ----  one inner link: its parked bias force plus what its children sent up
-__device__ __forceinline__ void link_bias_up(const int i, const uint32_t tw, const Sm &s, const Gm &g, const DevCtx &c) {
+__device__ __forceinline__ void link_bias_up(const int i, const Jt &j, const Sm &s, const Gm &g, const DevCtx &c) {
   const float2 th = __ldcg(g.q2 + i), w = __ldcg(g.w2 + i);
   const float Ki = __ldg(g.K + i);
-  const float4 u0 = s.P[7 * i];
-  const float2 v0 = *reinterpret_cast<const float2 *>(s.P + 7 * i + 1);
+  const float4 c4 = __ldg(g.c4 + i);
+  const float4 u0 = s.P[7 * i + kM0];
+  const float2 v0 = *reinterpret_cast<const float2 *>(s.P + 7 * i + kM1);
   float3 n = f3(u0.x, u0.y, u0.z), f = f3(u0.w, v0.x, v0.y);
-  gather_children(s.P, s.P + 7 * s.Np, (int)((tw >> kChShift) & kParMask), (int)((tw >> kNcShift) & kNcMask), n, f);
-  finish_bias(load_jt(s.P, i), i, tw, th, w, Ki, n, f, s, g, c);
+  gather_children(s.P, s.P + 7 * s.Np, (int)((j.tw >> kChShift) & kParMask), (int)((j.tw >> kNcShift) & kNcMask), n, f);
+  finish_bias(j, i, th, w, Ki, c4, n, f, s, g, c);
 }
 
 // ------------------------------------------------------------------------------------------------------
-// phase B2 for one link: composite rigid-body inertia about the link origin (mass, first moment h, symmetric
-// I) -> exact diagonal of M -> Jacobi factors (G[i]); effective link inertia for A v (C3[i]); publish the
-// composite inertia in the parent frame (M0[i], M1[i], PD[i].xy)
+// phase F, precond = 2: articulated-body inertia of one link (Featherstone).  The system matrix
+// A = M + M_teth + diag(arm + hD + h^2 K) is the joint-space inertia of the tree whose joints carry the armature
+// d = arm + hD + h^2 K, so the articulated-body recursion factorises it exactly in O(N):
+//   I^A_i = I_i + sum_children X^T I^a_c X,   U = I^A S,   D = S^T U + diag(d),   K = U D^-1,   I^a = I^A - K U^T.
+// A spatial inertia is kept as three 3 x 3 blocks, n = A alpha + B a, f = B^T alpha + C a (A, C symmetric); the
+// 21 floats of I^a go to the parent through the link's own record (IN, PD, M0, M1, XR) and the X21 plane, already
+// rotated into the parent's frame and moved to the parent's origin.  K and D^-1 stay in the factor planes.
 // ------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void up_inertia(const int i, const Sm &s, const Gm &g, const DevCtx &c) {
+__device__ __forceinline__ void rot_block(const M3 &R, const float *M, float *out) {   // out = R M R^T (3 x 3, row-major)
+  float T[9];
+#pragma unroll
+  for (int r = 0; r < 3; r++)
+#pragma unroll
+    for (int cc = 0; cc < 3; cc++) T[3 * r + cc] = R.a[3 * r] * M[cc] + R.a[3 * r + 1] * M[3 + cc] + R.a[3 * r + 2] * M[6 + cc];
+#pragma unroll
+  for (int r = 0; r < 3; r++)
+#pragma unroll
+    for (int cc = 0; cc < 3; cc++) out[3 * r + cc] = T[3 * r] * R.a[3 * cc] + T[3 * r + 1] * R.a[3 * cc + 1] + T[3 * r + 2] * R.a[3 * cc + 2];
+}
+
+__device__ __forceinline__ void factor_link(const int i, const Sm &s, const Gm &g, const DevCtx &c) {
+  const ob_params &P = c.P;
+  float4 *rec = s.P + 7 * i;
+  const Jt j = load_jt(s.P, i);
+  uint32_t tw = j.tw;
+  const float Ki = __ldg(g.K + i);
+  const float4 eff = eff_inertia(i, tw, __ldg(g.c4 + i), s, g, P);
+  const float2 dt = diag_terms(i, tw, Ki, s, g, P);
+  if (tw != j.tw) rec[kCS].w = __uint_as_float(tw);
+  // own inertia: body of revolution about +z through the joint
+  float A[9] = {eff.z, 0, 0, 0, eff.z, 0, 0, 0, eff.w};
+  float B[9] = {0, -eff.y, 0, eff.y, 0, 0, 0, 0, 0};
+  float C[9] = {eff.x, 0, 0, 0, eff.x, 0, 0, 0, eff.x};
+  if (tw & kOffax) {                                       // virtual tether masses off the axis: point masses
+    const int Ap = s.Ap;
+    const int4 t2 = __ldg(g.topo2 + i);
+    const int ast = t2.x & 0xffff, nap = t2.x >> 16;
+    for (int a = ast; a < ast + nap; a++) {
+      if (!s.att[a]) continue;
+      const float3 o = f3(s.ao[a], s.ao[Ap + a], s.ao[2 * Ap + a]);
+      if (o.x == 0.f && o.y == 0.f) continue;
+      const float mv = P.h * P.h * s.ak[a];
+      const float oo = dot(o, o);
+      A[0] += mv * (oo - o.x * o.x); A[4] += mv * (oo - o.y * o.y); A[8] += mv * (oo - o.z * o.z);
+      A[1] -= mv * o.x * o.y; A[3] -= mv * o.x * o.y; A[2] -= mv * o.x * o.z; A[6] -= mv * o.x * o.z;
+      A[5] -= mv * o.y * o.z; A[7] -= mv * o.y * o.z;
+      B[1] -= mv * o.z; B[2] += mv * o.y; B[3] += mv * o.z; B[5] -= mv * o.x; B[6] -= mv * o.y; B[7] += mv * o.x;
+      C[0] += mv; C[4] += mv; C[8] += mv;
+    }
+  }
+  const int fc = (int)((tw >> kChShift) & kParMask), nc = (int)((tw >> kNcShift) & kNcMask);
+#pragma unroll 1
+  for (int k = 0; k < nc; k++) {                           // ascending order: a fixed summation order
+    const float4 *ch = s.P + 7 * (fc + k);
+    const float4 a0 = ch[kIN], a1 = ch[kPD], a2 = ch[kM0], a3 = ch[kM1], a4 = ch[kXR];
+    const float a5 = s.X21[fc + k];
+    A[0] += a0.x; A[4] += a0.y; A[8] += a0.z; A[1] += a0.w; A[3] += a0.w;
+    A[2] += a1.x; A[6] += a1.x; A[5] += a1.y; A[7] += a1.y;
+    C[0] += a1.z; C[4] += a1.w; C[8] += a2.x; C[1] += a2.y; C[3] += a2.y; C[2] += a2.z; C[6] += a2.z; C[5] += a2.w; C[7] += a2.w;
+    B[0] += a3.x; B[1] += a3.y; B[2] += a3.z; B[3] += a3.w; B[4] += a4.x; B[5] += a4.y; B[6] += a4.z; B[7] += a4.w; B[8] += a5;
+  }
+  // U = I^A S, S = [(c2, 0, s2; 0), (0, 1, 0; 0)]
+  const float c2 = j.c2, s2 = j.s2;
+  const float3 u1n = f3(c2 * A[0] + s2 * A[2], c2 * A[3] + s2 * A[5], c2 * A[6] + s2 * A[8]);
+  const float3 u1f = f3(c2 * B[0] + s2 * B[6], c2 * B[1] + s2 * B[7], c2 * B[2] + s2 * B[8]);      // B^T s1
+  const float3 u2n = f3(A[1], A[4], A[7]);
+  const float3 u2f = f3(B[3], B[4], B[5]);
+  const float d11 = c2 * u1n.x + s2 * u1n.z + dt.x, d12 = u1n.y, d22 = u2n.y + dt.y;
+  const float idet = 1.f / (d11 * d22 - d12 * d12);
+  const float i11 = d22 * idet, i12 = -d12 * idet, i22 = d11 * idet;
+  const float3 k1n = i11 * u1n + i12 * u2n, k1f = i11 * u1f + i12 * u2f;
+  const float3 k2n = i12 * u1n + i22 * u2n, k2f = i12 * u1f + i22 * u2f;
+  const uint32_t slot = s.SL[i];
+  if (slot != kNoSlot) {
+    s.FAC[slot] = make_float4(k1n.x, k1n.y, k1n.z, k1f.x);
+    s.FAC[s.NFp + slot] = make_float4(k1f.y, k1f.z, k2n.x, k2n.y);
+    s.FAC[2 * s.NFp + slot] = make_float4(k2n.z, k2f.x, k2f.y, k2f.z);
+    s.FAC[3 * s.NFp + slot] = make_float4(i11, i12, i22, 0.f);
+  }
+  if (tw & kTrunk) return;
+  // I^a = I^A - K U^T (upper triangles of A, C; mirrored below)
+  const float k1na[3] = {k1n.x, k1n.y, k1n.z}, k2na[3] = {k2n.x, k2n.y, k2n.z}, k1fa[3] = {k1f.x, k1f.y, k1f.z}, k2fa[3] = {k2f.x, k2f.y, k2f.z};
+  const float u1na[3] = {u1n.x, u1n.y, u1n.z}, u2na[3] = {u2n.x, u2n.y, u2n.z}, u1fa[3] = {u1f.x, u1f.y, u1f.z}, u2fa[3] = {u2f.x, u2f.y, u2f.z};
+#pragma unroll
+  for (int r = 0; r < 3; r++)
+#pragma unroll
+    for (int cc = 0; cc < 3; cc++) {
+      B[3 * r + cc] -= k1na[r] * u1fa[cc] + k2na[r] * u2fa[cc];
+      if (cc >= r) {
+        A[3 * r + cc] -= k1na[r] * u1na[cc] + k2na[r] * u2na[cc];
+        C[3 * r + cc] -= k1fa[r] * u1fa[cc] + k2fa[r] * u2fa[cc];
+      }
+    }
+  A[3] = A[1]; A[6] = A[2]; A[7] = A[5]; C[3] = C[1]; C[6] = C[2]; C[7] = C[5];
+  // into the parent's orientation, then from the joint (at r = (0,0,rz) of the parent) to the parent's origin:
+  //   C' = C,  B' = B + r x C,  A' = A - B r x + r x B^T - r x C r x     (r x = rz [[0,-1,0],[1,0,0],[0,0,0]])
+  const M3 R = quat_mat(j.q);
+  float Ar[9], Br[9], Cr[9];
+  rot_block(R, A, Ar); rot_block(R, B, Br); rot_block(R, C, Cr);
+  const float z = j.rz, zz = z * z;
+  // G = B r x: column 0 = z B[:,1], column 1 = -z B[:,0], column 2 = 0;  A' = A - G - G^T + z^2 [[C11, -C01, 0], [-C01, C00, 0], 0]
+  const float g00 = z * Br[1], g10 = z * Br[4], g20 = z * Br[7], g01 = -z * Br[0], g11 = -z * Br[3], g21 = -z * Br[6];
+  const float Axx = Ar[0] - 2.f * g00 + zz * Cr[4], Ayy = Ar[4] - 2.f * g11 + zz * Cr[0], Azz = Ar[8];
+  const float Axy = Ar[1] - g01 - g10 - zz * Cr[1], Axz = Ar[2] - g20, Ayz = Ar[5] - g21;
+  // B' = B + r x C: row 0 -= z C[1,:], row 1 += z C[0,:]
+  const float B00 = Br[0] - z * Cr[3], B01 = Br[1] - z * Cr[4], B02 = Br[2] - z * Cr[5];
+  const float B10 = Br[3] + z * Cr[0], B11 = Br[4] + z * Cr[1], B12 = Br[5] + z * Cr[2];
+  rec[kIN] = make_float4(Axx, Ayy, Azz, Axy);
+  rec[kPD] = make_float4(Axz, Ayz, Cr[0], Cr[4]);
+  rec[kM0] = make_float4(Cr[8], Cr[1], Cr[2], Cr[5]);
+  rec[kM1] = make_float4(B00, B01, B02, B10);
+  rec[kXR] = make_float4(B11, B12, Br[6], Br[7]);
+  s.X21[i] = Br[8];
+}
+
+// ------------------------------------------------------------------------------------------------------
+// phase F, precond <= 1: composite rigid-body inertia about the link origin (mass, first moment h, symmetric I) ->
+// exact diagonal of M -> Jacobi factors 1 / diag(A) (IDG[i]); composite inertia to the parent through M0, M1, PD.xy
+// ------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void composite_link(const int i, const Sm &s, const Gm &g, const DevCtx &c) {
   const int Ap = s.Ap;
   const ob_params &P = c.P;
-  uint32_t tw = s.T[i];
+  float4 *rec = s.P + 7 * i;
+  const Jt j = load_jt(s.P, i);
+  uint32_t tw = j.tw;
   float4 c4 = __ldg(g.c4 + i);
-  {                                  // mass-proportional damping, implicit: the operator carries (1 + h alpha) M
+  const float2 dt = diag_terms(i, tw, __ldg(g.K + i), s, g, P);
+  {
     const float sc = 1.f + P.h * P.mass_damping;
     c4.x *= sc; c4.y *= sc; c4.z *= sc; c4.w *= sc;
   }
   float cm = c4.x;
   float3 ch3 = f3(0.f, 0.f, c4.y);
   float Ixx = c4.z, Iyy = c4.z, Izz = c4.w, Ixy = 0.f, Ixz = 0.f, Iyz = 0.f;
-  float4 eff = c4;
   if (P.tether_implicit && (tw & kHasApples)) {
-    tw &= ~kOffax;
-    const int4 t2 = __ldg(g.topo2 + i);
-    const int ast = t2.x & 0xffff, nap = t2.x >> 16;
-    for (int a = ast; a < ast + nap; a++) {
-      if (!s.att[a]) continue;
-      const float mv = P.h * P.h * s.ak[a];                     // virtual point mass h^2 k_s at the hang point
-      const float3 o = f3(s.ao[a], s.ao[Ap + a], s.ao[2 * Ap + a]);
-      cm += mv; ch3 = ch3 + mv * o;
-      Ixx += mv * (o.y * o.y + o.z * o.z); Iyy += mv * (o.x * o.x + o.z * o.z); Izz += mv * (o.x * o.x + o.y * o.y);
-      Ixy -= mv * o.x * o.y; Ixz -= mv * o.x * o.z; Iyz -= mv * o.y * o.z;
-      if (o.x == 0.f && o.y == 0.f) { eff.x += mv; eff.y += mv * o.z; eff.z += mv * o.z * o.z; }   // stays a body of revolution
-      else tw |= kOffax;
-    }
-    s.T[i] = tw;
-  }
-  s.P[7 * i + 6] = eff;
-  const int fc = (int)((tw >> kChShift) & kParMask), nc = (int)((tw >> kNcShift) & kNcMask);
-  for (int ch = fc; ch < fc + nc; ch++) {
-    const float4 u0 = s.P[7 * ch];
-    const float4 u1 = s.P[7 * ch + 1];
-    const float2 u2 = *reinterpret_cast<const float2 *>(s.P + 7 * ch + 2);
-    cm += u0.x;
-    ch3 = ch3 + f3(u0.y, u0.z, u0.w);
-    Ixx += u1.x; Iyy += u1.y; Izz += u1.z; Ixy += u1.w; Ixz += u2.x; Iyz += u2.y;
-  }
-  const Jt j = load_jt(s.P, i);
-  const float c2 = j.c2, s2 = j.s2;
-  const float2 dt = reinterpret_cast<const float2 *>(s.P + 7 * i + 2)[1];
-  const float m1 = c2 * c2 * Ixx + 2.f * c2 * s2 * Ixz + s2 * s2 * Izz, m2 = Iyy;
-  g.mdiag[i] = make_float2(m1, m2);
-  float2 id = make_float2(1.f, 1.f);
-  if (P.precond == 1) id = make_float2(1.f / (m1 + dt.x), 1.f / (m2 + dt.y));
-  s.G[i] = id;
-  if (!(tw & kTrunk)) {
-    const M3 &E = j.E;
-    const float rz = j.rz;
-    // composite inertia into the parent frame: rotate by Rrel = E^T, then move the origin by r = (0,0,rz)
-    const float3 hp = mulT(E, ch3);
-    M3 I, T, Ip;
-    I.a[0] = Ixx; I.a[1] = Ixy; I.a[2] = Ixz; I.a[3] = Ixy; I.a[4] = Iyy; I.a[5] = Iyz; I.a[6] = Ixz; I.a[7] = Iyz; I.a[8] = Izz;
-#pragma unroll
-    for (int r = 0; r < 3; r++)
-#pragma unroll
-      for (int cc = 0; cc < 3; cc++) T.a[3 * r + cc] = E.a[r] * I.a[cc] + E.a[3 + r] * I.a[3 + cc] + E.a[6 + r] * I.a[6 + cc];
-    Ip = mul(T, E);
-    const float sh = 2.f * rz * hp.z + cm * rz * rz;
-    s.P[7 * i] = make_float4(cm, hp.x, hp.y, hp.z + cm * rz);
-    s.P[7 * i + 1] = make_float4(Ip.a[0] + sh, Ip.a[4] + sh, Ip.a[8], Ip.a[1]);
-    *reinterpret_cast<float2 *>(s.P + 7 * i + 2) = make_float2(Ip.a[2] - rz * hp.x, Ip.a[5] - rz * hp.y);
-  }
-}
-
-// phase B2 on the steps between two recomputations of diag(M): the effective link inertia (it is part of A and must
-// be exact: it changes when an apple detaches, and phase A1 borrows its slot) and the Jacobi factors from the stored
-// diag(M) plus the CURRENT diagonal spring-damper terms.  A lagging preconditioner changes the number of PCG
-// iterations, never the system that is solved.
-__device__ __forceinline__ void link_inertia_lagged(const int i, float4 eff, const float2 md, const Sm &s, const Gm &g,
-                                                    const DevCtx &c) {
-  const ob_params &P = c.P;
-  const int Ap = s.Ap;
-  uint32_t tw = s.T[i];
-  {
-    const float sc = 1.f + P.h * P.mass_damping;
-    eff.x *= sc; eff.y *= sc; eff.z *= sc; eff.w *= sc;
-  }
-  if (P.tether_implicit && (tw & kHasApples)) {
-    tw &= ~kOffax;
     const int4 t2 = __ldg(g.topo2 + i);
     const int ast = t2.x & 0xffff, nap = t2.x >> 16;
     for (int a = ast; a < ast + nap; a++) {
       if (!s.att[a]) continue;
       const float mv = P.h * P.h * s.ak[a];
       const float3 o = f3(s.ao[a], s.ao[Ap + a], s.ao[2 * Ap + a]);
-      if (o.x == 0.f && o.y == 0.f) { eff.x += mv; eff.y += mv * o.z; eff.z += mv * o.z * o.z; }
-      else tw |= kOffax;
+      cm += mv; ch3 = ch3 + mv * o;
+      Ixx += mv * (o.y * o.y + o.z * o.z); Iyy += mv * (o.x * o.x + o.z * o.z); Izz += mv * (o.x * o.x + o.y * o.y);
+      Ixy -= mv * o.x * o.y; Ixz -= mv * o.x * o.z; Iyz -= mv * o.y * o.z;
     }
-    s.T[i] = tw;
   }
-  s.P[7 * i + 6] = eff;
-  const float2 dt = reinterpret_cast<const float2 *>(s.P + 7 * i + 2)[1];
-  float2 id = make_float2(1.f, 1.f);
-  if (P.precond == 1) id = make_float2(1.f / (md.x + dt.x), 1.f / (md.y + dt.y));
-  s.G[i] = id;
+  const int fc = (int)((tw >> kChShift) & kParMask), nc = (int)((tw >> kNcShift) & kNcMask);
+  for (int ch = fc; ch < fc + nc; ch++) {
+    const float4 u0 = s.P[7 * ch + kM0], u1 = s.P[7 * ch + kM1];
+    const float2 u2 = *reinterpret_cast<const float2 *>(s.P + 7 * ch + kPD);
+    cm += u0.x;
+    ch3 = ch3 + f3(u0.y, u0.z, u0.w);
+    Ixx += u1.x; Iyy += u1.y; Izz += u1.z; Ixy += u1.w; Ixz += u2.x; Iyz += u2.y;
+  }
+  const float c2 = j.c2, s2 = j.s2;
+  const float m1 = c2 * c2 * Ixx + 2.f * c2 * s2 * Ixz + s2 * s2 * Izz, m2 = Iyy;
+  s.IDG[i] = make_float2(1.f / (m1 + dt.x), 1.f / (m2 + dt.y));
+  if (!(tw & kTrunk)) {
+    // composite inertia into the parent frame: rotate by R_rel, then move the origin by r = (0,0,rz)
+    const M3 R = quat_mat(j.q);
+    const float rz = j.rz;
+    const float3 hp = mul(R, ch3);
+    const float I[9] = {Ixx, Ixy, Ixz, Ixy, Iyy, Iyz, Ixz, Iyz, Izz};
+    float Ip[9];
+    rot_block(R, I, Ip);
+    const float sh = 2.f * rz * hp.z + cm * rz * rz;
+    rec[kM0] = make_float4(cm, hp.x, hp.y, hp.z + cm * rz);
+    rec[kM1] = make_float4(Ip[0] + sh, Ip[4] + sh, Ip[8], Ip[1]);
+    *reinterpret_cast<float2 *>(rec + kPD) = make_float2(Ip[2] - rz * hp.x, Ip[5] - rz * hp.y);
+  }
 }
 
 // fence after level l of a top-down sweep / after level l of a bottom-up sweep (see "Order" above)
@@ -661,23 +841,21 @@ __device__ __forceinline__ void link_inertia_lagged(const int i, float4 eff, con
 #define OB_FENCE_UP(l) { if ((l) < ntop) __syncwarp(); else __syncthreads(); }
 
 // ------------------------------------------------------------------------------------------------------
-// the once-per-step sweeps as functions of their own (not inlined): their register pressure (24 kinematic
-// quantities per link in flight) stays out of the allocation of the PCG loop.  The views of the world live in
-// shared memory (World), the context is the kernel's __grid_constant__ parameter.
+// the once-per-step sweeps as functions of their own (not inlined): their register pressure stays out of the
+// allocation of the PCG loop.  The views of the world live in shared memory (World), the context is the kernel's
+// __grid_constant__ parameter.
 // ------------------------------------------------------------------------------------------------------
-#define OB_COLD_ATTR __noinline__
-
-__device__ OB_COLD_ATTR void sweep_bias(const World *wd, const DevCtx &c, const int nt) {
+__device__ __noinline__ void sweep_kinematics(const World *wd, const DevCtx &c, const int nt) {
   const Sm s = carve(wd);
   const Gm g = wd->g;
   const int nlev = wd->nlev, ntop = wd->ntop, tid = threadIdx.x;
-  const int l_first_down = tid < 32 ? 0 : ntop - 1, l_last_up = tid < 32 ? 0 : ntop;
-  // ---- A0: joint transforms in fp64, flat (the two double sincos and Q Rx Ry are the expensive part of the FK and
-  //      depend on nothing but the link's own q: kept out of the level-by-level chain) ----
+  const int l_first_down = tid < 32 ? 0 : ntop - 1;
+  // ---- A0: joint rotations in fp64, flat (the two double sincos depend on nothing but the link's own q: kept out
+  //      of the level-by-level chain) ----
 #pragma unroll 1
   for (int i = tid; i < wd->N; i += nt) link_joint(i, s, g);
   __syncthreads();
-  // ---- A1: forward kinematics in fp64, joint transforms, hang points, top-down ----
+  // ---- A1: forward kinematics in fp64, hang points, top-down ----
 #pragma unroll 1
   for (int l = l_first_down; l < nlev; l++) {
     const int le = s.lev[l + 1];
@@ -685,6 +863,39 @@ __device__ OB_COLD_ATTR void sweep_bias(const World *wd, const DevCtx &c, const 
     for (int i = s.lev[l] + tid; i < le; i += nt) link_fk(i, s, g);
     OB_FENCE_DOWN(l)
   }
+}
+
+__device__ __noinline__ void sweep_factor(const World *wd, const DevCtx &c, const int nt) {
+  const Sm s = carve(wd);
+  const Gm g = wd->g;
+  const int nlev = wd->nlev, ntop = wd->ntop, N = wd->N, tid = threadIdx.x;
+  const int l_last_up = tid < 32 ? 0 : ntop;
+  const bool tree = wd->precond == 2;
+  // ---- F: all leaves first (flat, evenly spread), then the inner links bottom-up ----
+#pragma unroll 1
+  for (int i = tid; i < N; i += nt)
+    if (((__float_as_uint(s.P[7 * i + kCS].w) >> kNcShift) & kNcMask) == 0u) {
+      if (tree) factor_link(i, s, g, c); else composite_link(i, s, g, c);
+    }
+  __syncthreads();
+#pragma unroll 1
+  for (int l = nlev - 2; l >= l_last_up; l--) {
+    const int le = s.lev[l + 1];
+#pragma unroll 1
+    for (int i = s.lev[l] + tid; i < le; i += nt)
+      if ((__float_as_uint(s.P[7 * i + kCS].w) >> kNcShift) & kNcMask) {
+        if (tree) factor_link(i, s, g, c); else composite_link(i, s, g, c);
+      }
+    OB_FENCE_UP(l)
+  }
+  __syncthreads();
+}
+
+__device__ __noinline__ void sweep_bias(const World *wd, const DevCtx &c, const int nt) {
+  const Sm s = carve(wd);
+  const Gm g = wd->g;
+  const int nlev = wd->nlev, ntop = wd->ntop, tid = threadIdx.x;
+  const int l_first_down = tid < 32 ? 0 : ntop - 1, l_last_up = tid < 32 ? 0 : ntop;
   // ---- A2 (+ B1 for leaves): velocities, bias accelerations, bias forces, top-down ----
 #pragma unroll 1
   for (int l = l_first_down; l < nlev; l++) {
@@ -699,48 +910,9 @@ __device__ OB_COLD_ATTR void sweep_bias(const World *wd, const DevCtx &c, const 
     const int le = s.lev[l + 1];
 #pragma unroll 1
     for (int i = s.lev[l] + tid; i < le; i += nt) {
-      const uint32_t tw = s.T[i];
-      if ((tw >> kNcShift) & kNcMask) link_bias_up(i, tw, s, g, c);
+      const Jt j = load_jt(s.P, i);
+      if ((j.tw >> kNcShift) & kNcMask) link_bias_up(i, j, s, g, c);
     }
-    OB_FENCE_UP(l)
-  }
-  __syncthreads();
-}
-
-__device__ OB_COLD_ATTR void sweep_inertia(const World *wd, const DevCtx &c, const int nt, const int otid,
-                                           const bool refresh) {
-  const Sm s = carve(wd);
-  const Gm g = wd->g;
-  const int nlev = wd->nlev, ntop = wd->ntop, N = wd->N, tid = threadIdx.x;
-  if (!refresh) {
-#pragma unroll 1
-    for (int i0 = otid; i0 < N; i0 += 4 * nt) {          // four links per trip to L2
-      float4 c4v[4];
-      float2 mdv[4];
-#pragma unroll
-      for (int k = 0; k < 4; k++) {
-        const int i = min(i0 + k * nt, N - 1);
-        c4v[k] = __ldg(g.c4 + i); mdv[k] = __ldcg(g.mdiag + i);
-      }
-#pragma unroll
-      for (int k = 0; k < 4; k++)
-        if (i0 + k * nt < N) link_inertia_lagged(i0 + k * nt, c4v[k], mdv[k], s, g, c);
-    }
-    __syncthreads();
-    return;
-  }
-  const int l_last_up = tid < 32 ? 0 : ntop;
-  // ---- B2: composite inertia bottom-up -> Jacobi factors, effective inertia (all leaves first) ----
-#pragma unroll 1
-  for (int i = otid; i < N; i += nt)                       // flat ownership: G[i] was just read by this thread
-    if (((s.T[i] >> kNcShift) & kNcMask) == 0u) up_inertia(i, s, g, c);
-  __syncthreads();
-#pragma unroll 1
-  for (int l = nlev - 2; l >= l_last_up; l--) {
-    const int le = s.lev[l + 1];
-#pragma unroll 1
-    for (int i = s.lev[l] + tid; i < le; i += nt)
-      if ((s.T[i] >> kNcShift) & kNcMask) up_inertia(i, s, g, c);
     OB_FENCE_UP(l)
   }
   __syncthreads();
@@ -753,6 +925,34 @@ __device__ OB_COLD_ATTR void sweep_inertia(const World *wd, const DevCtx &c, con
 // ------------------------------------------------------------------------------------------------------
 constexpr int kPcgBad = 1 << 30;
 
+// z = P^-1 r for precond = 2 (r in XR.zw, z -> M1.zw): one bottom-up and one top-down sweep with the factors of phase F
+template <int NT>
+__device__ __forceinline__ void tree_solve(const Sm &s, const int otid, const int nlev, const int ntop) {
+  float4 *const PL = s.P;
+  const bool topw = otid < 32;
+  const int l_last_up = topw ? 0 : ntop, l_first_down = topw ? 0 : ntop - 1;
+#pragma unroll 1
+  for (int l = nlev - 1; l >= l_last_up; l--) {
+    const int le = s.lev[l + 1];
+    if (l == nlev - 1) {
+#pragma unroll 1
+      for (int i = s.lev[l] + otid; i < le; i += NT) solve_up<false>(i, PL, s);
+    } else {
+#pragma unroll 1
+      for (int i = s.lev[l] + otid; i < le; i += NT) solve_up<true>(i, PL, s);
+    }
+    OB_FENCE_UP(l)
+  }
+  __syncthreads();
+#pragma unroll 1
+  for (int l = l_first_down; l < nlev; l++) {
+    const int le = s.lev[l + 1];
+#pragma unroll 1
+    for (int i = s.lev[l] + otid; i < le; i += NT) solve_down(i, PL, s);
+    OB_FENCE_DOWN(l)
+  }
+}
+
 template <int NT, int LPT>
 __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *stage, int *flipp, const int otid,
                                       const bool top_warp, const float bb, const float bz, int *flags) {
@@ -761,8 +961,8 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
   const ob_params &P = c.P;
   const int tid = threadIdx.x, lane = tid & 31;
   const int Np = s.Np, N = wd->N, nlev = wd->nlev, ntop = wd->ntop;
+  const bool tree = wd->precond == 2;
   float4 *const PL = s.P;
-  float4 *const XR = s.XR;
   Reducer<NT> red;
   red.stage = stage; red.flip = *flipp; red.tid = otid;
   int status = 0;
@@ -773,7 +973,7 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
   if (lane < ntopN) {
     for (int l = 0; l < ntop; l++)
       if (lane >= s.lev[l]) top_lvl = l;
-    if (top_lvl < ntop - 1) top_maxc = (int)((s.T[lane] >> kNcShift) & kNcMask);
+    if (top_lvl < ntop - 1) top_maxc = (int)((__float_as_uint(PL[7 * lane + kCS].w) >> kNcShift) & kNcMask);
   }
   top_maxc = __reduce_max_sync(0xffffffffu, top_maxc);
   int it = 0;
@@ -782,7 +982,7 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
 #pragma unroll
     for (int k = 0; k < LPT; k++) {
       const int i = otid + k * NT;
-      if (i < N) XR[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (i < N) PL[7 * i + kXR] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
   } else if (!(bb < INFINITY)) {
     bad = true;
@@ -790,24 +990,23 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
 #pragma unroll
     for (int k = 0; k < LPT; k++) {                 // first product: A x, i.e. p = x
       const int i = otid + k * NT;
-      if (i < N) *reinterpret_cast<float2 *>(PL + 7 * i + 2) = *reinterpret_cast<const float2 *>(XR + i);
+      if (i < N) *reinterpret_cast<float2 *>(PL + 7 * i + kPD) = *reinterpret_cast<const float2 *>(PL + 7 * i + kXR);
     }
     bool first = true;
     float rz = 0.f, rr = 0.f;
-    // stopping rule: |r| <= tol |b| in the 2-norm (cg_norm 0) or in the preconditioned norm (cg_norm 1)
+    // stopping rule: |r| <= tol |b| in the 2-norm (cg_norm 0) or in the preconditioned norm (cg_norm 1, precond <= 1)
     const float tol2 = P.cg_tol * P.cg_tol * (P.cg_norm ? bz : bb);
     for (;;) {
-      // ---- A p.  The n_top leading levels live in warp 0, lane = link: own record in registers, parents
+      // ---- A p.  The n_top leading levels live in the top warp, lane = link: own record in registers, parents
       //      and children by shuffle, no barrier.  The other levels are swept by the whole CTA, one block
       //      barrier per level; the deepest level turns around at once ----
       float pAp_part = 0.f;
       if (top_warp) {
         const int me = lane < ntopN ? lane : Np;             // idle lanes work on the zero record
-        const uint32_t tw = s.T[me];
         float4 *rec = PL + 7 * me;
-        const float4 pd = rec[2];
+        const float4 pd = rec[kPD];
         const Jt j = load_jt(PL, me);
-        const int parl = (tw & kTrunk) ? lane : (int)(tw & kParMask);   // the trunk's "parent" is all zero at level 0
+        const int parl = (j.tw & kTrunk) ? lane : (int)(j.tw & kParMask);   // the trunk's "parent" is all zero at level 0
         const float3 sp = f3(j.c2 * pd.x, pd.y, j.s2 * pd.x);
         float3 al = f3(0, 0, 0), a = f3(0, 0, 0);
 #pragma unroll 1
@@ -817,15 +1016,16 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
           alp.z = __shfl_sync(0xffffffffu, al.z, parl);
           ap.x = __shfl_sync(0xffffffffu, a.x, parl); ap.y = __shfl_sync(0xffffffffu, a.y, parl);
           ap.z = __shfl_sync(0xffffffffu, a.z, parl);
-          const float3 nal = mul(j.E, alp) + sp;
-          const float3 na = mul(j.E, f3(ap.x + alp.y * j.rz, ap.y - alp.x * j.rz, ap.z));
+          float3 nal, na;
+          motion_down(j, alp, ap, nal, na);
+          nal = nal + sp;
           const bool mine = top_lvl == l;
           al.x = mine ? nal.x : al.x; al.y = mine ? nal.y : al.y; al.z = mine ? nal.z : al.z;
           a.x = mine ? na.x : a.x; a.y = mine ? na.y : a.y; a.z = mine ? na.z : a.z;
         }
         if (lane < ntopN) {
-          rec[0] = make_float4(al.x, al.y, al.z, a.x);
-          *reinterpret_cast<float2 *>(rec + 1) = make_float2(a.y, a.z);
+          rec[kM0] = make_float4(al.x, al.y, al.z, a.x);
+          *reinterpret_cast<float2 *>(rec + kM1) = make_float2(a.y, a.z);
         }
       }
       __syncthreads();
@@ -835,17 +1035,16 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
         const bool deepest = l == nlev - 1;
 #pragma unroll 1
         for (int i = s.lev[l] + otid; i < le; i += NT) {
-          const uint32_t tw = s.T[i];
           float4 *rec = PL + 7 * i;
-          const float4 pd = rec[2];
+          const float4 pd = rec[kPD];
           const Jt j = load_jt(PL, i);
           float3 al, a;
-          mv_down(j, PL, tw, pd, al, a);
+          mv_down(j, PL, pd, al, a);
           if (deepest) {
-            pAp_part += mv_up<false>(j, PL, PL + 7 * Np, i, tw, pd, al, a, s, g, c);
+            pAp_part += mv_up<false>(j, PL, PL + 7 * Np, i, pd, al, a, s, g, c);
           } else {
-            rec[0] = make_float4(al.x, al.y, al.z, a.x);
-            *reinterpret_cast<float2 *>(rec + 1) = make_float2(a.y, a.z);
+            rec[kM0] = make_float4(al.x, al.y, al.z, a.x);
+            *reinterpret_cast<float2 *>(rec + kM1) = make_float2(a.y, a.z);
           }
         }
         __syncthreads();
@@ -855,28 +1054,26 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
         const int le = s.lev[l + 1];
 #pragma unroll 1
         for (int i = s.lev[l] + otid; i < le; i += NT) {
-          const uint32_t tw = s.T[i];
           const float4 *rec = PL + 7 * i;
-          const float4 pd = rec[2];
+          const float4 pd = rec[kPD];
           const Jt j = load_jt(PL, i);
-          const float4 u = rec[0], v = rec[1];
-          pAp_part += mv_up<true>(j, PL, PL + 7 * Np, i, tw, pd, f3(u.x, u.y, u.z), f3(u.w, v.x, v.y), s, g, c);
+          const float4 u = rec[kM0], v = rec[kM1];
+          pAp_part += mv_up<true>(j, PL, PL + 7 * Np, i, pd, f3(u.x, u.y, u.z), f3(u.w, v.x, v.y), s, g, c);
         }
         __syncthreads();
       }
       if (top_warp) {
         const int me = lane < ntopN ? lane : Np;
-        const uint32_t tw = s.T[me];
         float4 *rec = PL + 7 * me;
-        const float4 pd = rec[2], I = rec[6];
+        const float4 pd = rec[kPD];
         const Jt j = load_jt(PL, me);
-        const float4 u = rec[0], v = rec[1];
+        const float4 u = rec[kM0], v = rec[kM1];
         const float3 al = f3(u.x, u.y, u.z), a = f3(u.w, v.x, v.y);
-        const int fc = (int)((tw >> kChShift) & kParMask), nc = (int)((tw >> kNcShift) & kNcMask);
+        const int fc = (int)((j.tw >> kChShift) & kParMask), nc = (int)((j.tw >> kNcShift) & kNcMask);
         // own inertia force; the children of the last top level are in shared memory, all others are lanes
-        float3 n0 = f3(I.z * al.x - I.y * a.y, I.z * al.y + I.y * a.x, I.w * al.z);
-        float3 f0 = f3(I.x * a.x + I.y * al.y, I.x * a.y - I.y * al.x, I.x * a.z);
-        if (tw & kOffax) {
+        float3 n0, f0;
+        own_inertia_force(rec[kIN], al, a, n0, f0);
+        if (j.tw & kOffax) {
           const Force6 t = offaxis_tethers(__ldg(g.topo2 + me), al, a, s.att, s.ao, s.ak, s.Ap, P.h * P.h);
           n0 = n0 + t.n; f0 = f0 + t.f;
         }
@@ -911,70 +1108,83 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
           }
           const float nt1 = j.c2 * n.x + j.s2 * n.z + pd.z * pd.x;
           const float nt2 = n.y + pd.w * pd.y;
-          const float3 nuf = mulT(j.E, f);
-          float3 nun = mulT(j.E, n);
-          nun.x -= j.rz * nuf.y; nun.y += j.rz * nuf.x;
+          float3 nun, nuf;
+          force_up(j, n, f, nun, nuf);
           const bool mine = top_lvl == l;
           t1 = mine ? nt1 : t1; t2 = mine ? nt2 : t2;
           un.x = mine ? nun.x : un.x; un.y = mine ? nun.y : un.y; un.z = mine ? nun.z : un.z;
           uf.x = mine ? nuf.x : uf.x; uf.y = mine ? nuf.y : uf.y; uf.z = mine ? nuf.z : uf.z;
         }
         if (lane < ntopN) {
-          reinterpret_cast<float2 *>(rec + 1)[1] = make_float2(t1, t2);
+          reinterpret_cast<float2 *>(rec + kM1)[1] = make_float2(t1, t2);
           pAp_part += pd.x * t1 + pd.y * t2;
         }
       }
+      // ---- x, r; z = P^-1 r; p ----
       float rz_p = 0.f, rr_p = 0.f;
-      if (first) {                                 // r = b - A x, z = P^-1 r, p = z
-        first = false;
-        __syncthreads();
-#pragma unroll
-        for (int k = 0; k < LPT; k++) {
-          const int i = otid + k * NT;
-          if (i < N) {
-            const float2 ap = reinterpret_cast<const float2 *>(PL + 7 * i + 1)[1];
-            const float2 idg = s.G[i];
-            float2 r = reinterpret_cast<const float2 *>(XR + i)[1];
-            r.x -= ap.x; r.y -= ap.y;
-            reinterpret_cast<float2 *>(XR + i)[1] = r;
-            const float za = r.x * idg.x, zb = r.y * idg.y;
-            *reinterpret_cast<float2 *>(PL + 7 * i + 2) = make_float2(za, zb);
-            rz_p += r.x * za + r.y * zb; rr_p += r.x * r.x + r.y * r.y;
-          }
-        }
-        const float2 t = red.sum(rz_p, rr_p);
-        rz = t.x; rr = P.cg_norm ? t.x : t.y;
+      float alpha = 0.f;
+      if (first) {
+        __syncthreads();                           // A x of the top levels (written by the top warp) is read below
       } else {
         const float pAp = red.sum(pAp_part, 0.f).x;
-        const float alpha = rz / pAp;
-        float2 z[LPT], pk[LPT];
+        alpha = rz / pAp;
+      }
+      float2 z[LPT], pk[LPT];
 #pragma unroll
-        for (int k = 0; k < LPT; k++) {
-          const int i = otid + k * NT;
-          z[k] = make_float2(0.f, 0.f); pk[k] = make_float2(0.f, 0.f);
-          if (i < N) {
-            const float2 ap = reinterpret_cast<const float2 *>(PL + 7 * i + 1)[1];
-            const float2 idg = s.G[i];
-            pk[k] = *reinterpret_cast<const float2 *>(PL + 7 * i + 2);
-            float4 xr = XR[i];
+      for (int k = 0; k < LPT; k++) {
+        const int i = otid + k * NT;
+        z[k] = make_float2(0.f, 0.f); pk[k] = make_float2(0.f, 0.f);
+        if (i < N) {
+          const float2 ap = reinterpret_cast<const float2 *>(PL + 7 * i + kM1)[1];
+          float4 xr = PL[7 * i + kXR];
+          if (first) {                               // r = b - A x
+            xr.z -= ap.x; xr.w -= ap.y;
+          } else {
+            pk[k] = *reinterpret_cast<const float2 *>(PL + 7 * i + kPD);
             xr.x += alpha * pk[k].x; xr.y += alpha * pk[k].y;
             xr.z -= alpha * ap.x; xr.w -= alpha * ap.y;
-            XR[i] = xr;
+          }
+          PL[7 * i + kXR] = xr;
+          rr_p += xr.z * xr.z + xr.w * xr.w;
+          if (!tree) {
+            const float2 idg = s.IDG[i];
             z[k] = make_float2(xr.z * idg.x, xr.w * idg.y);
-            rz_p += xr.z * z[k].x + xr.w * z[k].y; rr_p += xr.z * xr.z + xr.w * xr.w;
+            rz_p += xr.z * z[k].x + xr.w * z[k].y;
           }
         }
+      }
+      float rz_new;
+      if (!tree) {
         const float2 t = red.sum(rz_p, rr_p);
-        const float beta = t.x / rz;
-        rz = t.x; rr = P.cg_norm ? t.x : t.y;
+        rz_new = t.x; rr = P.cg_norm ? t.x : t.y;
+      } else {
+        rr = red.sum(rr_p, 0.f).x;
+        if (!(rr > tol2)) {                          // converged (or non-finite): no solve
+          if (!first) it++;
+          break;
+        }
+        tree_solve<NT>(s, otid, nlev, ntop);
 #pragma unroll
         for (int k = 0; k < LPT; k++) {
           const int i = otid + k * NT;
-          if (i < N)
-            *reinterpret_cast<float2 *>(PL + 7 * i + 2) = make_float2(z[k].x + beta * pk[k].x, z[k].y + beta * pk[k].y);
+          if (i < N) {
+            z[k] = reinterpret_cast<const float2 *>(PL + 7 * i + kM1)[1];
+            const float2 r = reinterpret_cast<const float2 *>(PL + 7 * i + kXR)[1];
+            rz_p += r.x * z[k].x + r.y * z[k].y;
+          }
         }
-        it++;
+        rz_new = red.sum(rz_p, 0.f).x;
       }
+      const float beta = first ? 0.f : rz_new / rz;
+      rz = rz_new;
+#pragma unroll
+      for (int k = 0; k < LPT; k++) {
+        const int i = otid + k * NT;
+        if (i < N)
+          *reinterpret_cast<float2 *>(PL + 7 * i + kPD) = make_float2(z[k].x + beta * pk[k].x, z[k].y + beta * pk[k].y);
+      }
+      if (!first) it++;
+      first = false;
       if (!(rr > tol2 && it < P.cg_max_iter)) break;
     }
     if (!(rr <= tol2)) {
@@ -1044,7 +1254,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       if (tid == 0) { __threadfence(); atomicExch(progress + w, chunk + 1); }
       continue;
     }
-    const Sm s = carve(smem, d.Np, d.Ap, d.NIp, d.n_levels);
+    const Sm s = carve(smem, d.Np, d.Ap, d.NFp, d.n_levels);
     const int Np = d.Np, N = d.N;
     const int nlev = d.n_levels, ntop = d.n_top;
     float4 *const PL = s.P;
@@ -1060,17 +1270,17 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       g.quatd = reinterpret_cast<const double2 *>(c.quatd) + 2 * (size_t)d.link_base;
       g.anchor = c.anchor + 3 * (size_t)d.apple_base;
       g.Mmax = c.Mmax + d.link_base;
-      g.mdiag = c.mdiag + d.link_base;
       g.hist = c.xprev + d.link_base;
       g.arm = c.arm ? c.arm + 2 * (size_t)d.link_base : nullptr;
       g.topo2 = c.topo2 + d.link_base;
     }
     if (tid == 0) {
-      s_world.g = g; s_world.N = N; s_world.Np = Np; s_world.Ap = d.Ap; s_world.NIp = d.NIp; s_world.nlev = nlev;
-      s_world.ntop = ntop;
+      s_world.g = g; s_world.N = N; s_world.Np = Np; s_world.Ap = d.Ap; s_world.NFp = d.NFp; s_world.nlev = nlev;
+      s_world.ntop = ntop; s_world.precond = d.precond;
     }
 
-    // ---- stage the world: the apple block by one TMA bulk copy; topology words, level offsets, wrench slots ----
+    // ---- stage the world: the apple block by one TMA bulk copy; topology words, factor slots, level offsets,
+    //      wrench slots ----
     if (tid == 0 && d.Ap) {
       fence_proxy_async();
       const uint32_t ab = (uint32_t)apple_block_bytes(d.Ap);
@@ -1081,31 +1291,31 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       const int32_t *src = reinterpret_cast<const int32_t *>(c.wrench + w);
       int32_t *dst = reinterpret_cast<int32_t *>(s.wr);
       for (int k = tid; k < (int)(sizeof(WrenchSlots) / 4); k += NT) dst[k] = __ldg(src + k);
-      if (tid < 7) PL[7 * Np + tid] = make_float4(0.f, 0.f, 0.f, 0.f);            // the zero column
+      if (tid < 7) PL[7 * Np + tid] = make_float4(0.f, 0.f, 0.f, 0.f);            // the zero record
       for (int k = tid; k <= nlev; k += NT) s.lev[k] = __ldg(c.level_off + d.level_base + k);
-      for (int i = tid; i <= Np; i += NT) {
-        uint32_t tw = (uint32_t)Np | kTrunk;
-        if (i < N) {
-          const int4 tp = __ldg(c.topo + d.link_base + i);
-          const int4 t2 = __ldg(g.topo2 + i);
-          const uint32_t nc = (uint32_t)tp.w, fc = nc ? (uint32_t)tp.y : 0u;
-          tw = (tp.x >= 0 ? (uint32_t)tp.x : ((uint32_t)Np | kTrunk)) | (fc << kChShift) | (nc << kNcShift) |
-               ((t2.x >> 16) ? kHasApples : 0u) | (__ldcg(g.rupt + i) ? kRuptured : 0u);
-        }
-        s.T[i] = tw;
+      for (int i = tid; i < N; i += NT) {
+        const int4 tp = __ldg(c.topo + d.link_base + i);
+        const int4 t2 = __ldg(g.topo2 + i);
+        const uint32_t nc = (uint32_t)tp.w, fc = nc ? (uint32_t)tp.y : 0u;
+        const uint32_t tw = (tp.x >= 0 ? (uint32_t)tp.x : ((uint32_t)Np | kTrunk)) | (fc << kChShift) | (nc << kNcShift) |
+                            ((t2.x >> 16) ? kHasApples : 0u) | (__ldcg(g.rupt + i) ? kRuptured : 0u);
+        PL[7 * i + kCS] = make_float4(0.f, 0.f, 0.f, __uint_as_float(tw));
+        s.SL[i] = (uint16_t)(t2.y & 0xffff);
       }
     }
-    float4 *const XR = s.XR;                           // (x, r) of the PCG per link; aliases the phase-A overflow
     if (d.Ap) {
       mbar_wait(&s_bar, parity);
       parity ^= 1;
     }
     __syncthreads();
-    int step0 = __ldcg(&info->step), steps_done = 0, last_iters = 0, diag_age = __ldcg(&info->diag_age);
+    int step0 = __ldcg(&info->step), steps_done = 0, last_iters = 0;
     unsigned long long iters_total = 0;
     for (int sidx = 0; sidx < n_my; sidx++) {
-      sweep_bias(&s_world, c, NT);                      // A, B1
-      {                                                 // r = b; x = cubic extrapolation of the last four solutions
+      sweep_kinematics(&s_world, c, NT);                // A0, A1
+      if (d.precond) sweep_factor(&s_world, c, NT);     // F
+      sweep_bias(&s_world, c, NT);                      // A2, B1: r = b
+      float bb_part = 0.f, bz_part = 0.f;
+      {                                                 // x = cubic extrapolation of the last four solutions
         const int t = step0 + sidx;                     // (ring of four in global memory, slot = step & 3)
         float2 h1[LPT], h2[LPT], h3[LPT], h4[LPT];
 #pragma unroll
@@ -1120,27 +1330,23 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         for (int k = 0; k < LPT; k++) {
           const int i = otid + k * NT;
           if (i < N) {
-            const float2 b = s.G[i];
-            XR[i] = make_float4(OB_X0(h1[k].x, h2[k].x, h3[k].x, h4[k].x), OB_X0(h1[k].y, h2[k].y, h3[k].y, h4[k].y), b.x, b.y);
+            const float2 b = reinterpret_cast<const float2 *>(PL + 7 * i + kXR)[1];
+            *reinterpret_cast<float2 *>(PL + 7 * i + kXR) =
+                make_float2(OB_X0(h1[k].x, h2[k].x, h3[k].x, h4[k].x), OB_X0(h1[k].y, h2[k].y, h3[k].y, h4[k].y));
+            bb_part += b.x * b.x + b.y * b.y;
+            if (d.precond == 1) {
+              const float2 idg = s.IDG[i];
+              bz_part += b.x * b.x * idg.x + b.y * b.y * idg.y;
+            } else {
+              if (!d.precond) s.IDG[i] = make_float2(1.f, 1.f);
+              bz_part += b.x * b.x + b.y * b.y;
+            }
           }
-        }
-      }
-      sweep_inertia(&s_world, c, NT, otid, diag_age == 0);
-      diag_age = diag_age + 1 >= kDiagRefresh ? 0 : diag_age + 1;   // (B2 first rewrites G[i] by the thread that just read it)
-      float bb_part = 0.f, bz_part = 0.f;
-#pragma unroll
-      for (int k = 0; k < LPT; k++) {
-        const int i = otid + k * NT;
-        if (i < N) {
-          const float2 idg = s.G[i];
-          const float4 xr = XR[i];
-          bb_part += xr.z * xr.z + xr.w * xr.w;
-          bz_part += xr.z * xr.z * idg.x + xr.w * xr.w * idg.y;
         }
       }
       const float2 bbz = red.sum(bb_part, bz_part);
       const float bb = bbz.x, bz = bbz.y;
-      // ---- C: PCG, warm-started from the previous dqd (x) ----
+      // ---- C: PCG, warm-started ----
       int pcg_flags = 0;
       const int it = pcg_solve<NT, LPT>(&s_world, c, s_stage, &red.flip, otid, top_warp, bb, bz, &pcg_flags);
       status |= pcg_flags & OB_STATUS_CG_MAXITER;
@@ -1151,7 +1357,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       for (int k = 0; k < LPT; k++) {
         const int i = otid + k * NT;
         if (i < N) {
-          const float2 x = *reinterpret_cast<const float2 *>(XR + i);
+          const float2 x = *reinterpret_cast<const float2 *>(PL + 7 * i + kXR);
           nf |= !(fabsf(x.x) < INFINITY) || !(fabsf(x.y) < INFINITY);
         }
       }
@@ -1175,7 +1381,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         const int i = otid + k * NT;
         if (i >= N) continue;
         const float2 w0 = dw0[k], q0 = dq0[k];
-        const float2 x = *reinterpret_cast<const float2 *>(XR + i);
+        const float2 x = *reinterpret_cast<const float2 *>(PL + 7 * i + kXR);
         g.hist[(step_now & 3) * (size_t)c.sum_np + i] = x;
         float wa = w0.x + x.x, wb = w0.y + x.y;
         if (P.qd_max > 0.f) {
@@ -1184,7 +1390,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         }
         const float qa = fmaf(P.h, wa, q0.x), qb = fmaf(P.h, wb, q0.y);
         g.w2[i] = make_float2(wa, wb); g.q2[i] = make_float2(qa, qb);
-        const uint32_t tw = s.T[i];
+        const uint32_t tw = __float_as_uint(PL[7 * i + kCS].w);
         if (!(tw & kRuptured)) {
           const float Ki = dK[k], Mx = dMx[k];
           const float mu = Ki * sqrtf(qa * qa + qb * qb);                   // Eq. 5
@@ -1192,7 +1398,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
           const int rcn = mu > Mx ? rc0 + 1 : 0;
           if (rcn >= P.rupture_frames) {
             g.rupt[i] = 1; g.rc[i] = 0;
-            s.T[i] = tw | kRuptured;
+            PL[7 * i + kCS].w = __uint_as_float(tw | kRuptured);
             push_event(c, w, step_now, 0, __ldg(c.link_ext + d.link_base + i), mu, Mx);
           } else if (rcn != rc0) {
             g.rc[i] = (unsigned char)rcn;
@@ -1257,7 +1463,6 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       info->step = step0 + steps_done;
       info->last_iters = last_iters;
       info->status = status;
-      info->diag_age = diag_age;
       info->steps_taken = __ldcg(&info->steps_taken) + steps_done;
       info->cg_iters = __ldcg(&info->cg_iters) + iters_total;
     }

@@ -47,7 +47,7 @@ def test_struct_layouts_match_the_header():
 def test_default_params_are_the_documented_readings():
     p = ob.default_params()
     assert abs(p.h - 2e-3) < 1e-9 and tuple(p.gravity) == (0.0, 0.0, np.float32(-9.81))
-    assert abs(p.c_d - 0.05) < 1e-8 and abs(p.cg_tol - 1e-6) < 1e-12 and p.cg_max_iter == 200 and p.precond == 1
+    assert abs(p.c_d - 0.05) < 1e-8 and abs(p.cg_tol - 1e-6) < 1e-12 and p.cg_max_iter == 200 and p.precond == 2
     assert p.rupture_frames == 3 and p.detach_frames_pull == 3 and p.detach_frames_tension == 10
     assert abs(p.detach_kappa - 1.1) < 1e-6 and p.react_max == 40.0 and p.tether_implicit == 1
     assert p.qd_max == 50.0 and abs(p.zeta_s - 0.1) < 1e-7 and p.forces_off_on_snapped == 1 and p.mass_damping == 0.0

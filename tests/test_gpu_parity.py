@@ -199,9 +199,10 @@ def test_single_step_margin_on_a_wider_sample():
 
 
 def test_single_step_explicit_tether_and_no_preconditioner():
-    """The paper-literal explicit Eq. 7 (tether_implicit = 0) and plain CG (precond = 0) reach the same step."""
+    """The paper-literal explicit Eq. 7 (tether_implicit = 0), plain CG (precond = 0) and Jacobi-PCG (precond = 1, in
+    both stopping norms) reach the same step as the default tree-preconditioned PCG."""
     spec = binary_tree_config1()
-    for kw in (dict(tether_implicit=0), dict(precond=0, cg_max_iter=2000), dict(cg_norm=1)):
+    for kw in (dict(tether_implicit=0), dict(precond=0, cg_max_iter=2000), dict(precond=1), dict(precond=1, cg_norm=1)):
         P = dataclasses.replace(config_params(1), **kw)
         sim, refs = _make([spec], P)
         for s in range(30):

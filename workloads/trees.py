@@ -59,7 +59,7 @@ class Params:
     c_d: float = 0.05
     cg_tol: float = 1e-6
     cg_max_iter: int = 200
-    precond: int = 1
+    precond: int = 2
     cg_norm: int = 0
     rupture_frames: int = 3
     detach_frames_pull: int = 3
