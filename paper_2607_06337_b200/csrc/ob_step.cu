@@ -422,6 +422,22 @@ __device__ __forceinline__ void link_joint(const int i, const Sm &s, const Gm &g
   store_qd(rec, q);
 }
 
+// The global inputs of a level sweep are staged by a FLAT pass before it (one L2 round trip for the whole world
+// instead of one per level of the sweep): the link's own inertia constants -> IN, (q, qd) -> XR, K -> PD.x (before
+// phase F: -> X21, because A1 publishes through PD).  Each sweep reads them at the link's own turn, before it
+// overwrites the slots with what it publishes.
+__device__ __forceinline__ void stage_link_inputs(const int i, const Sm &s, const Gm &g, const bool state) {
+  float4 *rec = s.P + 7 * i;
+  const float4 c4 = __ldg(g.c4 + i);
+  const float Ki = __ldg(g.K + i);
+  if (state) {
+    const float2 th = __ldcg(g.q2 + i), w = __ldcg(g.w2 + i);
+    rec[kXR] = make_float4(th.x, th.y, w.x, w.y);
+  }
+  rec[kIN] = c4;
+  if (state) rec[kPD].x = Ki; else s.X21[i] = Ki;
+}
+
 // ---- A1 ----  forward kinematics in fp64 (Eq. 3): q_i = q_p q_rel, p_i = p_p + R(q_p) (0,0,L_p).
 //               The tether stretch x_a - x_hang is a millimetre-sized difference of metre-sized positions, k_s = 2e3
 //               N/m turns 1e-8 m of it into the whole error budget of a 3 mm twig: rest rotations, sin / cos of the
@@ -598,9 +614,9 @@ __device__ __forceinline__ void finish_bias(const Jt &j, const int i, const floa
 __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm &s, const Gm &g, const DevCtx &c) {
   const ob_params &P = c.P;
   float4 *rec = s.P + 7 * i;
-  const float2 w = __ldcg(g.w2 + i), th = __ldcg(g.q2 + i);       // all global inputs of the link's turn at once
-  const float4 c4 = __ldg(g.c4 + i);
-  const float Ki = __ldg(g.K + i);
+  const float4 sq = rec[kXR], c4 = rec[kIN];                      // (q, qd), inertia, K: staged by the flat pass
+  const float2 th = make_float2(sq.x, sq.y), w = make_float2(sq.z, sq.w);
+  const float Ki = rec[kPD].x;
   const Jt j = load_jt(s.P, i);
   const uint32_t tw = j.tw;
   float3 wp = f3(0, 0, 0), vp = f3(0, 0, 0), alp = f3(0, 0, 0);
@@ -653,9 +669,9 @@ __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm
 
 // ---- B1 ----  one inner link: its parked bias force plus what its children sent up
 __device__ __forceinline__ void link_bias_up(const int i, const Jt &j, const Sm &s, const Gm &g, const DevCtx &c) {
-  const float2 th = __ldcg(g.q2 + i), w = __ldcg(g.w2 + i);
-  const float Ki = __ldg(g.K + i);
-  const float4 c4 = __ldg(g.c4 + i);
+  const float4 sq = s.P[7 * i + kXR], c4 = s.P[7 * i + kIN];     // staged by the flat pass between A2 and B1
+  const float2 th = make_float2(sq.x, sq.y), w = make_float2(sq.z, sq.w);
+  const float Ki = s.P[7 * i + kPD].x;
   const float4 u0 = s.P[7 * i + kM0];
   const float2 v0 = *reinterpret_cast<const float2 *>(s.P + 7 * i + kM1);
   float3 n = f3(u0.x, u0.y, u0.z), f = f3(u0.w, v0.x, v0.y);
@@ -689,8 +705,8 @@ __device__ __forceinline__ void factor_link(const int i, const Sm &s, const Gm &
   float4 *rec = s.P + 7 * i;
   const Jt j = load_jt(s.P, i);
   uint32_t tw = j.tw;
-  const float Ki = __ldg(g.K + i);
-  const float4 eff = eff_inertia(i, tw, __ldg(g.c4 + i), s, g, P);
+  const float Ki = s.X21[i];                                   // staged by the flat pass before the sweep
+  const float4 eff = eff_inertia(i, tw, rec[kIN], s, g, P);
   const float2 dt = diag_terms(i, tw, Ki, s, g, P);
   if (tw != j.tw) rec[kCS].w = __uint_as_float(tw);
   // own inertia: body of revolution about +z through the joint
@@ -789,8 +805,8 @@ __device__ __forceinline__ void composite_link(const int i, const Sm &s, const G
   float4 *rec = s.P + 7 * i;
   const Jt j = load_jt(s.P, i);
   uint32_t tw = j.tw;
-  float4 c4 = __ldg(g.c4 + i);
-  const float2 dt = diag_terms(i, tw, __ldg(g.K + i), s, g, P);
+  float4 c4 = rec[kIN];                                        // staged by the flat pass before the sweep
+  const float2 dt = diag_terms(i, tw, s.X21[i], s, g, P);
   {
     const float sc = 1.f + P.h * P.mass_damping;
     c4.x *= sc; c4.y *= sc; c4.z *= sc; c4.w *= sc;
@@ -853,7 +869,10 @@ __device__ __noinline__ void sweep_kinematics(const World *wd, const DevCtx &c, 
   // ---- A0: joint rotations in fp64, flat (the two double sincos depend on nothing but the link's own q: kept out
   //      of the level-by-level chain) ----
 #pragma unroll 1
-  for (int i = tid; i < wd->N; i += nt) link_joint(i, s, g);
+  for (int i = tid; i < wd->N; i += nt) {
+    link_joint(i, s, g);
+    stage_link_inputs(i, s, g, false);                  // for phase F (A1 leaves IN and PD.x of every link alone)
+  }
   __syncthreads();
   // ---- A1: forward kinematics in fp64, hang points, top-down ----
 #pragma unroll 1
@@ -896,6 +915,9 @@ __device__ __noinline__ void sweep_bias(const World *wd, const DevCtx &c, const 
   const Gm g = wd->g;
   const int nlev = wd->nlev, ntop = wd->ntop, tid = threadIdx.x;
   const int l_first_down = tid < 32 ? 0 : ntop - 1, l_last_up = tid < 32 ? 0 : ntop;
+#pragma unroll 1
+  for (int i = tid; i < wd->N; i += nt) stage_link_inputs(i, s, g, true);
+  __syncthreads();
   // ---- A2 (+ B1 for leaves): velocities, bias accelerations, bias forces, top-down ----
 #pragma unroll 1
   for (int l = l_first_down; l < nlev; l++) {
@@ -905,6 +927,10 @@ __device__ __noinline__ void sweep_bias(const World *wd, const DevCtx &c, const 
     OB_FENCE_DOWN(l)
   }
   // ---- B1: bias forces bottom-up over the inner links -> rhs b ----
+#pragma unroll 1
+  for (int i = tid; i < wd->N; i += nt)                 // what A2 left for the children of an inner link is dead now
+    if ((__float_as_uint(s.P[7 * i + kCS].w) >> kNcShift) & kNcMask) stage_link_inputs(i, s, g, true);
+  __syncthreads();
 #pragma unroll 1
   for (int l = nlev - 2; l >= l_last_up; l--) {
     const int le = s.lev[l + 1];

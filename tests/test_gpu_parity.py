@@ -643,7 +643,7 @@ def test_full_size_config4_sampled_worlds_and_invariants():
     sim.step(20)
     st = sim.stats()
     assert st["world_steps_total"] == 20 * len(specs) and st["n_flagged"] == 0
-    assert 2 * 20 * len(specs) <= st["cg_iters_total"] <= 60 * 20 * len(specs)
+    assert 10 * len(specs) <= st["cg_iters_total"] <= 60 * 20 * len(specs)     # the tree preconditioner needs ~1 per step
     # Philox: every world and every apple, bit-exact (the draw is a pure function of (seed, world, apple): A23)
     _check_all_philox_draws(sim, specs, P, seed)
     sample = [0, 1, 517, 1023, 2048, 3000, 4000, 4095]
