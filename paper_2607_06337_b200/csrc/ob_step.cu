@@ -347,8 +347,13 @@ __device__ __forceinline__ void solve_up(const int i, float4 *P, const Sm &s) {
   rec[kM1] = make_float4(fp.y, fp.z, k.d11 * u0 + k.d12 * u1, k.d12 * u0 + k.d22 * u1);
 }
 
-// top-down turn: a' = X a_parent, z = y - K^T a', a = a' + S z for the children; z -> M1.zw
-__device__ __forceinline__ void solve_down(const int i, float4 *P, const Sm &s) {
+// top-down turn: a' = X a_parent, z = y - K^T a', a = a' + S z for the children; z -> M1.zw.
+// FUSE (first PCG iteration: p = z): the accelerations this pass hands down ARE the top-down pass of the product A p
+// for p = z, so the pass doubles as that: p -> PD.xy, every link keeps (al, a) for its turn in the product's bottom-up
+// pass, and a link of the deepest level turns around at once (returns its p . A p).
+template <bool FUSE>
+__device__ __forceinline__ float solve_down(const int i, float4 *P, const Sm &s, const Gm &g, const DevCtx &c,
+                                            const bool turn) {
   float4 *rec = P + 7 * i;
   const Jt j = load_jt(P, i);
   const float4 I = rec[kIN], pd = rec[kPD];
@@ -359,12 +364,19 @@ __device__ __forceinline__ void solve_down(const int i, float4 *P, const Sm &s) 
   float3 al, a;
   motion_down(j, f3(u.x, u.y, u.z), f3(u.w, v.x, v.y), al, a);
   const float z0 = y.x - (dot(k.k1n, al) + dot(k.k1f, a)), z1 = y.y - (dot(k.k2n, al) + dot(k.k2f, a));
-  if ((j.tw >> kNcShift) & kNcMask) {
-    rec[kM0] = make_float4(al.x + j.c2 * z0, al.y + z1, al.z + j.s2 * z0, a.x);
+  al = al + f3(j.c2 * z0, z1, j.s2 * z0);
+  if (FUSE) {
+    *reinterpret_cast<float2 *>(rec + kPD) = make_float2(z0, z1);
+    if (turn) return mv_up<false>(j, P, P + 7 * s.Np, i, make_float4(z0, z1, pd.z, pd.w), al, a, s, g, c);
+    rec[kM0] = make_float4(al.x, al.y, al.z, a.x);
+    *reinterpret_cast<float2 *>(rec + kM1) = make_float2(a.y, a.z);
+  } else if ((j.tw >> kNcShift) & kNcMask) {
+    rec[kM0] = make_float4(al.x, al.y, al.z, a.x);
     rec[kM1] = make_float4(a.y, a.z, z0, z1);
   } else {
     reinterpret_cast<float2 *>(rec + kM1)[1] = make_float2(z0, z1);
   }
+  return 0.f;
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -553,7 +565,7 @@ __device__ __noinline__ Force6 external_forces(const int i, const float3 om, con
     const float ks = s.ak[a], cdamp = s.ac[a], ma = s.am[a];
     // x_a - x_hang = (anchor - x_hang) + sag + u: the apple is stored as u = x_a - (anchor + sag), sag = m g / k_s,
     // and phase A1 left anchor - x_hang in fp64 (as two floats)
-    const double mk = (double)ma / (double)ks;               // one fp64 division; sag = (m / k_s) g to ~1e-19 m of m g / k_s
+    const double mk = (double)(ma / ks);                     // sag = (m / k_s) g: ~1e-3 m, so fp32's 6e-8 is 1e-10 m
     const float3 st = f3((float)(join2(s.hd[a], s.hd[Ap + a]) + mk * (double)P.gravity[0] + (double)s.u[a]),
                          (float)(join2(s.hd[2 * Ap + a], s.hd[3 * Ap + a]) + mk * (double)P.gravity[1] + (double)s.u[Ap + a]),
                          (float)(join2(s.hd[4 * Ap + a], s.hd[5 * Ap + a]) + mk * (double)P.gravity[2] + (double)s.u[2 * Ap + a]));
@@ -700,7 +712,9 @@ __device__ __forceinline__ void rot_block(const M3 &R, const float *M, float *ou
     for (int cc = 0; cc < 3; cc++) out[3 * r + cc] = T[3 * r] * R.a[3 * cc] + T[3 * r + 1] * R.a[3 * cc + 1] + T[3 * r + 2] * R.a[3 * cc + 2];
 }
 
-__device__ __forceinline__ void factor_link(const int i, const Sm &s, const Gm &g, const DevCtx &c) {
+__device__ __noinline__ void factor_link(const int i, const World *wd, const DevCtx &c) {
+  const Sm s = carve(wd);
+  const Gm g = wd->g;
   const ob_params &P = c.P;
   float4 *rec = s.P + 7 * i;
   const Jt j = load_jt(s.P, i);
@@ -748,7 +762,7 @@ __device__ __forceinline__ void factor_link(const int i, const Sm &s, const Gm &
   const float3 u2n = f3(A[1], A[4], A[7]);
   const float3 u2f = f3(B[3], B[4], B[5]);
   const float d11 = c2 * u1n.x + s2 * u1n.z + dt.x, d12 = u1n.y, d22 = u2n.y + dt.y;
-  const float idet = 1.f / (d11 * d22 - d12 * d12);
+  const float idet = __fdividef(1.f, d11 * d22 - d12 * d12);     // (a preconditioner: an approximate reciprocal will do)
   const float i11 = d22 * idet, i12 = -d12 * idet, i22 = d11 * idet;
   const float3 k1n = i11 * u1n + i12 * u2n, k1f = i11 * u1f + i12 * u2f;
   const float3 k2n = i12 * u1n + i22 * u2n, k2f = i12 * u1f + i22 * u2f;
@@ -799,7 +813,9 @@ __device__ __forceinline__ void factor_link(const int i, const Sm &s, const Gm &
 // phase F, precond <= 1: composite rigid-body inertia about the link origin (mass, first moment h, symmetric I) ->
 // exact diagonal of M -> Jacobi factors 1 / diag(A) (IDG[i]); composite inertia to the parent through M0, M1, PD.xy
 // ------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void composite_link(const int i, const Sm &s, const Gm &g, const DevCtx &c) {
+__device__ __noinline__ void composite_link(const int i, const World *wd, const DevCtx &c) {
+  const Sm s = carve(wd);
+  const Gm g = wd->g;
   const int Ap = s.Ap;
   const ob_params &P = c.P;
   float4 *rec = s.P + 7 * i;
@@ -886,7 +902,6 @@ __device__ __noinline__ void sweep_kinematics(const World *wd, const DevCtx &c, 
 
 __device__ __noinline__ void sweep_factor(const World *wd, const DevCtx &c, const int nt) {
   const Sm s = carve(wd);
-  const Gm g = wd->g;
   const int nlev = wd->nlev, ntop = wd->ntop, N = wd->N, tid = threadIdx.x;
   const int l_last_up = tid < 32 ? 0 : ntop;
   const bool tree = wd->precond == 2;
@@ -894,7 +909,7 @@ __device__ __noinline__ void sweep_factor(const World *wd, const DevCtx &c, cons
 #pragma unroll 1
   for (int i = tid; i < N; i += nt)
     if (((__float_as_uint(s.P[7 * i + kCS].w) >> kNcShift) & kNcMask) == 0u) {
-      if (tree) factor_link(i, s, g, c); else composite_link(i, s, g, c);
+      if (tree) factor_link(i, wd, c); else composite_link(i, wd, c);
     }
   __syncthreads();
 #pragma unroll 1
@@ -903,7 +918,7 @@ __device__ __noinline__ void sweep_factor(const World *wd, const DevCtx &c, cons
 #pragma unroll 1
     for (int i = s.lev[l] + tid; i < le; i += nt)
       if ((__float_as_uint(s.P[7 * i + kCS].w) >> kNcShift) & kNcMask) {
-        if (tree) factor_link(i, s, g, c); else composite_link(i, s, g, c);
+        if (tree) factor_link(i, wd, c); else composite_link(i, wd, c);
       }
     OB_FENCE_UP(l)
   }
@@ -951,9 +966,12 @@ __device__ __noinline__ void sweep_bias(const World *wd, const DevCtx &c, const 
 // ------------------------------------------------------------------------------------------------------
 constexpr int kPcgBad = 1 << 30;
 
-// z = P^-1 r for precond = 2 (r in XR.zw, z -> M1.zw): one bottom-up and one top-down sweep with the factors of phase F
-template <int NT>
-__device__ __forceinline__ void tree_solve(const Sm &s, const int otid, const int nlev, const int ntop) {
+// z = P^-1 r for precond = 2 (r in XR.zw, z -> M1.zw): one bottom-up and one top-down sweep with the factors of phase F.
+// FUSE: z -> PD.xy (= p) and the top-down pass of A p is done with it (see solve_down); returns this thread's share of
+// p . A p from the links that turned around.
+template <int NT, bool FUSE>
+__device__ __forceinline__ float tree_solve(const Sm &s, const Gm &g, const DevCtx &c, const int otid, const int nlev,
+                                            const int ntop) {
   float4 *const PL = s.P;
   const bool topw = otid < 32;
   const int l_last_up = topw ? 0 : ntop, l_first_down = topw ? 0 : ntop - 1;
@@ -970,13 +988,16 @@ __device__ __forceinline__ void tree_solve(const Sm &s, const int otid, const in
     OB_FENCE_UP(l)
   }
   __syncthreads();
+  float part = 0.f;
 #pragma unroll 1
   for (int l = l_first_down; l < nlev; l++) {
     const int le = s.lev[l + 1];
+    const bool turn = FUSE && l == nlev - 1 && l >= ntop;   // (a tree that ends inside the top warp turns around there)
 #pragma unroll 1
-    for (int i = s.lev[l] + otid; i < le; i += NT) solve_down(i, PL, s);
+    for (int i = s.lev[l] + otid; i < le; i += NT) part += solve_down<FUSE>(i, PL, s, g, c, turn);
     OB_FENCE_DOWN(l)
   }
+  return part;
 }
 
 template <int NT, int LPT>
@@ -1018,15 +1039,16 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
       const int i = otid + k * NT;
       if (i < N) *reinterpret_cast<float2 *>(PL + 7 * i + kPD) = *reinterpret_cast<const float2 *>(PL + 7 * i + kXR);
     }
-    bool first = true;
-    float rz = 0.f, rr = 0.f;
+    bool first = true, have_down = false;
+    float rz = 0.f, rr = 0.f, pAp_carry = 0.f;
     // stopping rule: |r| <= tol |b| in the 2-norm (cg_norm 0) or in the preconditioned norm (cg_norm 1, precond <= 1)
     const float tol2 = P.cg_tol * P.cg_tol * (P.cg_norm ? bz : bb);
     for (;;) {
       // ---- A p.  The n_top leading levels live in the top warp, lane = link: own record in registers, parents
       //      and children by shuffle, no barrier.  The other levels are swept by the whole CTA, one block
       //      barrier per level; the deepest level turns around at once ----
-      float pAp_part = 0.f;
+      float pAp_part = pAp_carry;
+      if (!have_down) {
       if (top_warp) {
         const int me = lane < ntopN ? lane : Np;             // idle lanes work on the zero record
         float4 *rec = PL + 7 * me;
@@ -1075,6 +1097,8 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
         }
         __syncthreads();
       }
+      }                                              // (after a fused solve the top-down pass is done already)
+      have_down = false; pAp_carry = 0.f;
 #pragma unroll 1
       for (int l = nlev - 2; l >= ntop; l--) {
         const int le = s.lev[l + 1];
@@ -1189,12 +1213,17 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
           if (!first) it++;
           break;
         }
-        tree_solve<NT>(s, otid, nlev, ntop);
+        if (first) {                                 // p = z: the solve's top-down pass is the product's as well
+          pAp_carry = tree_solve<NT, true>(s, g, c, otid, nlev, ntop);
+          have_down = true;
+        } else {
+          tree_solve<NT, false>(s, g, c, otid, nlev, ntop);
+        }
 #pragma unroll
         for (int k = 0; k < LPT; k++) {
           const int i = otid + k * NT;
           if (i < N) {
-            z[k] = reinterpret_cast<const float2 *>(PL + 7 * i + kM1)[1];
+            z[k] = have_down ? *reinterpret_cast<const float2 *>(PL + 7 * i + kPD) : reinterpret_cast<const float2 *>(PL + 7 * i + kM1)[1];
             const float2 r = reinterpret_cast<const float2 *>(PL + 7 * i + kXR)[1];
             rz_p += r.x * z[k].x + r.y * z[k].y;
           }
@@ -1203,11 +1232,13 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
       }
       const float beta = first ? 0.f : rz_new / rz;
       rz = rz_new;
+      if (!have_down) {
 #pragma unroll
-      for (int k = 0; k < LPT; k++) {
-        const int i = otid + k * NT;
-        if (i < N)
-          *reinterpret_cast<float2 *>(PL + 7 * i + kPD) = make_float2(z[k].x + beta * pk[k].x, z[k].y + beta * pk[k].y);
+        for (int k = 0; k < LPT; k++) {
+          const int i = otid + k * NT;
+          if (i < N)
+            *reinterpret_cast<float2 *>(PL + 7 * i + kPD) = make_float2(z[k].x + beta * pk[k].x, z[k].y + beta * pk[k].y);
+        }
       }
       if (!first) it++;
       first = false;
