@@ -74,10 +74,12 @@ struct Sm {
   float *u, *v;                       // [3][Ap]
   unsigned char *att, *cA, *cB;
   float *ao, *ak, *am, *ac, *afd;     // ao = [3][Ap]
+  const int *alnk;                    // [Ap] internal index of the link that carries the apple
   float *ft, *fsn;                    // tether force [3][Ap], |f_s| [Ap] (phase A2 -> phase D)
-  float *hd;                          // [6][Ap] anchor - x_hang of every apple, fp64 as (hi, lo) pairs (phase A1 -> A2);
-                                      // aliases ft, fsn (see carve)
-  float *aq;                          // [4][Ap] world quaternion (fp32) of the apple's link (phase A1 -> A2)
+  float *hd;                          // [6][Ap] anchor - x_hang of every apple, fp64 as (hi, lo) pairs (phase A1 -> apple
+                                      // pass); aliases ft, fsn (see carve)
+  float *aq;                          // [4][Ap] world quaternion (fp32) of the apple's link (phase A1 -> apple pass); then,
+                                      // with hd[4], hd[5], the reaction of the apple on its link (apple pass -> B1)
   float4 *wq;                         // [OB_MAX_WRENCH] world quaternion of the link of each wrench slot
   WrenchSlots *wr;
 };
@@ -101,6 +103,7 @@ __device__ __forceinline__ Sm carve(unsigned char *base, const int Np, const int
   s.att = p + 24 * Ap; s.cA = s.att + Ap; s.cB = s.cA + Ap;
   f = reinterpret_cast<float *>(p + apple_state_bytes(Ap));
   s.ao = f; s.ak = f + 3 * Ap; s.am = f + 4 * Ap; s.ac = f + 5 * Ap; s.afd = f + 6 * Ap;
+  s.alnk = reinterpret_cast<const int *>(f + 7 * Ap);
   p += r16(apple_block_bytes(Ap));
   f = reinterpret_cast<float *>(p);
   s.ft = f; s.fsn = f + 3 * Ap; s.hd = f; f += 6 * Ap;   // hd[0..3] share the memory of ft[0..2], fsn: per apple, phase A2
@@ -125,7 +128,7 @@ struct Gm {
 };
 
 // the views of the world every thread of the CTA shares (in shared memory, filled once per world)
-struct World { Gm g; int N, Np, Ap, NFp, nlev, ntop, precond; };
+struct World { Gm g; int N, A, Np, Ap, NFp, nlev, ntop, precond; };
 __device__ __forceinline__ Sm carve(const World *wd) { return carve(ob_smem, wd->Np, wd->Ap, wd->NFp, wd->nlev); }
 
 // block-wide sum of two values, result broadcast to every thread; one barrier per call (double-buffered stage)
@@ -447,7 +450,12 @@ __device__ __forceinline__ void stage_link_inputs(const int i, const Sm &s, cons
     rec[kXR] = make_float4(th.x, th.y, w.x, w.y);
   }
   rec[kIN] = c4;
-  if (state) rec[kPD].x = Ki; else s.X21[i] = Ki;
+  if (state) {
+    rec[kPD].x = Ki;
+    if (__float_as_uint(rec[kCS].w) & kHasApples) s.X21[i] = __int_as_float(__ldg(g.topo2 + i).x);   // first apple | count << 16
+  } else {
+    s.X21[i] = Ki;
+  }
 }
 
 // ---- A1 ----  forward kinematics in fp64 (Eq. 3): q_i = q_p q_rel, p_i = p_p + R(q_p) (0,0,L_p).
@@ -544,55 +552,58 @@ __device__ __forceinline__ float4 eff_inertia(const int i, uint32_t &tw, float4 
   return c4;
 }
 
-// tether reactions (Eq. 6 / Eq. 7) and user wrenches on one link, subtracted from its bias
-// force (n, f); also leaves the tether force and |f_s| of each apple for phase D.  Only links that carry apples or
-// a wrench come here.
-// (Not inlined.  It takes the World in shared memory, not references to the caller's copies: a reference would
-// force those copies into local memory, and every pointer fetched from there is an L2 round trip.)
-__device__ __noinline__ Force6 external_forces(const int i, const float3 om, const float3 vl, const uint32_t tw,
-                                               const int apples, const World *wd, const DevCtx &c) {
-  const Sm s = carve(wd);
-  const ob_params &P = c.P;
+// Tether of one apple (Eq. 6 / Eq. 7): the tether force and |f_s| for phase D, and the clamped
+// reaction on the link as a spatial force (n, f) in link coordinates, which B1 subtracts from the link's bias force.
+// A flat pass over the apples between A2 (which left the velocity of every apple-carrying link in its record) and B1:
+// every lane has an apple, nothing of it sits in the level-by-level chain.
+__device__ __forceinline__ void apple_forces(const int a, const Sm &s, const ob_params &P) {
   const int Ap = s.Ap;
-  Force6 out;
-  out.n = f3(0, 0, 0); out.f = f3(0, 0, 0);
-  const int ast = apples & 0xffff, nap = apples >> 16;          // first apple | count << 16 (topo2.x, loaded by the caller)
-  const float eta_h = P.tether_implicit ? P.h : 0.f;
-  for (int a = ast; a < ast + nap; a++) {
-    if (!s.att[a]) continue;
-    const float4 qw = make_float4(s.aq[a], s.aq[Ap + a], s.aq[2 * Ap + a], s.aq[3 * Ap + a]);   // world rotation of the link
-    const float3 o = f3(s.ao[a], s.ao[Ap + a], s.ao[2 * Ap + a]);
-    const float ks = s.ak[a], cdamp = s.ac[a], ma = s.am[a];
-    // x_a - x_hang = (anchor - x_hang) + sag + u: the apple is stored as u = x_a - (anchor + sag), sag = m g / k_s,
-    // and phase A1 left anchor - x_hang in fp64 (as two floats)
-    const double mk = (double)(ma / ks);                     // sag = (m / k_s) g: ~1e-3 m, so fp32's 6e-8 is 1e-10 m
-    const float3 st = f3((float)(join2(s.hd[a], s.hd[Ap + a]) + mk * (double)P.gravity[0] + (double)s.u[a]),
-                         (float)(join2(s.hd[2 * Ap + a], s.hd[3 * Ap + a]) + mk * (double)P.gravity[1] + (double)s.u[Ap + a]),
-                         (float)(join2(s.hd[4 * Ap + a], s.hd[5 * Ap + a]) + mk * (double)P.gravity[2] + (double)s.u[2 * Ap + a]));
-    const float3 vh = rot_up(qw, vl + cross(om, o));                      // world velocity of the hang point
-    const float3 fs = (-ks) * st;
-    const float3 va = f3(s.v[a], s.v[Ap + a], s.v[2 * Ap + a]);
-    s.ft[a] = fs.x - cdamp * va.x; s.ft[Ap + a] = fs.y - cdamp * va.y; s.ft[2 * Ap + a] = fs.z - cdamp * va.z;
-    s.fsn[a] = sqrtf(dot(fs, fs));
-    float3 fr = f3(ks * (st.x - eta_h * vh.x) - ma * P.gravity[0], ks * (st.y - eta_h * vh.y) - ma * P.gravity[1],
-                   ks * (st.z - eta_h * vh.z) - ma * P.gravity[2]);
-    const float nr = sqrtf(dot(fr, fr));
-    if (nr > P.react_max) fr = (P.react_max / nr) * fr;                   // clamp
-    const float3 fl = rot_down(qw, fr);
-    out.f = out.f - fl;
-    out.n = out.n - cross(o, fl);
+  if (!s.att[a]) {
+    s.aq[a] = 0.f; s.aq[Ap + a] = 0.f; s.aq[2 * Ap + a] = 0.f; s.aq[3 * Ap + a] = 0.f;
+    s.hd[4 * Ap + a] = 0.f; s.hd[5 * Ap + a] = 0.f;
+    return;
   }
-  // user wrenches on this link (disabled on snapped sub-trees)
+  const float4 *rec = s.P + 7 * s.alnk[a];
+  const float4 t0 = rec[kXR];
+  const float2 t1 = *reinterpret_cast<const float2 *>(rec + kIN);
+  const float3 om = f3(t0.x, t0.y, t0.z), vl = f3(t0.w, t1.x, t1.y);
+  const float4 qw = make_float4(s.aq[a], s.aq[Ap + a], s.aq[2 * Ap + a], s.aq[3 * Ap + a]);   // world rotation of the link
+  const float3 o = f3(s.ao[a], s.ao[Ap + a], s.ao[2 * Ap + a]);
+  const float ks = s.ak[a], cdamp = s.ac[a], ma = s.am[a];
+  const float eta_h = P.tether_implicit ? P.h : 0.f;
+  // x_a - x_hang = (anchor - x_hang) + sag + u: the apple is stored as u = x_a - (anchor + sag), sag = m g / k_s,
+  // and phase A1 left anchor - x_hang in fp64 (as two floats)
+  const double mk = (double)(ma / ks);                     // sag = (m / k_s) g: ~1e-3 m, so fp32's 6e-8 is 1e-10 m
+  const float3 st = f3((float)(join2(s.hd[a], s.hd[Ap + a]) + mk * (double)P.gravity[0] + (double)s.u[a]),
+                       (float)(join2(s.hd[2 * Ap + a], s.hd[3 * Ap + a]) + mk * (double)P.gravity[1] + (double)s.u[Ap + a]),
+                       (float)(join2(s.hd[4 * Ap + a], s.hd[5 * Ap + a]) + mk * (double)P.gravity[2] + (double)s.u[2 * Ap + a]));
+  const float3 vh = rot_up(qw, vl + cross(om, o));                      // world velocity of the hang point
+  const float3 fs = (-ks) * st;
+  const float3 va = f3(s.v[a], s.v[Ap + a], s.v[2 * Ap + a]);
+  s.ft[a] = fs.x - cdamp * va.x; s.ft[Ap + a] = fs.y - cdamp * va.y; s.ft[2 * Ap + a] = fs.z - cdamp * va.z;
+  s.fsn[a] = sqrtf(dot(fs, fs));
+  float3 fr = f3(ks * (st.x - eta_h * vh.x) - ma * P.gravity[0], ks * (st.y - eta_h * vh.y) - ma * P.gravity[1],
+                 ks * (st.z - eta_h * vh.z) - ma * P.gravity[2]);
+  const float nr = sqrtf(dot(fr, fr));
+  if (nr > P.react_max) fr = (P.react_max / nr) * fr;                   // clamp
+  const float3 fl = rot_down(qw, fr);
+  const float3 nl = cross(o, fl);
+  s.aq[a] = nl.x; s.aq[Ap + a] = nl.y; s.aq[2 * Ap + a] = nl.z; s.aq[3 * Ap + a] = fl.x;
+  s.hd[4 * Ap + a] = fl.y; s.hd[5 * Ap + a] = fl.z;
+}
+
+// user wrenches on one link (disabled on snapped sub-trees), subtracted from its bias force
+__device__ __forceinline__ void wrench_forces(const int i, const uint32_t tw, const Sm &s, const ob_params &P, float3 &n,
+                                              float3 &f) {
   const int nwr = s.wr->n;
   for (int q = 0; q < nwr; q++) {
     if (s.wr->body[q] != i) continue;
     if ((tw & kSnapped) && P.forces_off_on_snapped) continue;
     const float3 fl = rot_down(s.wq[q], f3(s.wr->force[q][0], s.wr->force[q][1], s.wr->force[q][2]));
     const float3 pt = f3(s.wr->point[q][0], s.wr->point[q][1], s.wr->point[q][2]);
-    out.f = out.f - fl;
-    out.n = out.n - cross(pt, fl);
+    f = f - fl;
+    n = n - cross(pt, fl);
   }
-  return out;
 }
 
 // project the accumulated bias force on the joint axes -> rhs b (XR[i].zw), the diagonal terms of both DoF (PD[i].zw),
@@ -622,7 +633,8 @@ __device__ __forceinline__ void finish_bias(const Jt &j, const int i, const floa
 
 // ---- A2 ----  velocity, bias acceleration (gravity as base acceleration), own bias force
 //               f = I a + v x* I v - tether reactions - user wrenches  (RNEA with qdd = 0)
-// An inner link leaves (om, vl, al, aln) for its children in XR, IN, PD.xy, M1.zw and parks its force in M0, M1.xy.
+// An inner link leaves (om, vl, al, aln) for its children in XR, IN, PD.xy, M1.zw and parks its force in M0, M1.xy;
+// so does a link that carries apples (the apple pass reads its velocity).
 __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm &s, const Gm &g, const DevCtx &c) {
   const ob_params &P = c.P;
   float4 *rec = s.P + 7 * i;
@@ -651,7 +663,8 @@ __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm
   // joint acceleration alpha qd, i.e. alpha S qd = alpha vJ on top of the velocity-product terms
   al = al + f3(-s2 * ww, 0.f, c2 * ww) + cross(om, vJ) + P.mass_damping * vJ;
   aln = aln + cross(vl, vJ);
-  const bool inner = ((tw >> kNcShift) & kNcMask) != 0u;
+  // a link with children waits for them, a link with apples for the apple pass: both park
+  const bool inner = (((tw >> kNcShift) & kNcMask) | (tw & kHasApples)) != 0u;
   // f = I a + v x* I v  (cylinder: com on +z)
   const float m = c4.x, mc = c4.y, Io = c4.z, Iz = c4.w;
   float3 n = f3(Io * al.x - mc * aln.y, Io * al.y + mc * aln.x, Iz * al.z);
@@ -660,14 +673,8 @@ __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm
   const float3 hf = f3(m * vl.x + mc * om.y, m * vl.y - mc * om.x, m * vl.z);
   n = n + cross(om, hn) + cross(vl, hf);
   f = f + cross(om, hf);
-  bool ext = (tw & kHasApples) != 0u;
-  for (int q = 0; q < s.wr->n; q++) ext |= s.wr->body[q] == i;
-  if (ext) {
-    const int4 t2g = __ldg(g.topo2 + i);
-    const Force6 e = external_forces(i, om, vl, tw, t2g.x, wd, c);
-    n = n + e.n; f = f + e.f;
-  }
-  if (inner) {                                                    // parked until B1 adds the children
+  wrench_forces(i, tw, s, P, n, f);
+  if (inner) {                                                    // parked until B1 adds the children / the apples
     const float2 dt = diag_terms(i, tw, Ki, s, g, P);
     rec[kXR] = make_float4(om.x, om.y, om.z, vl.x);
     rec[kIN] = make_float4(vl.y, vl.z, al.x, al.y);
@@ -688,6 +695,13 @@ __device__ __forceinline__ void link_bias_up(const int i, const Jt &j, const Sm 
   const float2 v0 = *reinterpret_cast<const float2 *>(s.P + 7 * i + kM1);
   float3 n = f3(u0.x, u0.y, u0.z), f = f3(u0.w, v0.x, v0.y);
   gather_children(s.P, s.P + 7 * s.Np, (int)((j.tw >> kChShift) & kParMask), (int)((j.tw >> kNcShift) & kNcMask), n, f);
+  if (j.tw & kHasApples) {                                  // the reactions of its apples, in apple order
+    const int Ap = s.Ap, ap = __float_as_int(s.X21[i]), ast = ap & 0xffff, nap = ap >> 16;
+    for (int a = ast; a < ast + nap; a++) {
+      n = n - f3(s.aq[a], s.aq[Ap + a], s.aq[2 * Ap + a]);
+      f = f - f3(s.aq[3 * Ap + a], s.hd[4 * Ap + a], s.hd[5 * Ap + a]);
+    }
+  }
   finish_bias(j, i, th, w, Ki, c4, n, f, s, g, c);
 }
 
@@ -941,18 +955,24 @@ __device__ __noinline__ void sweep_bias(const World *wd, const DevCtx &c, const 
     for (int i = s.lev[l] + tid; i < le; i += nt) link_bias(i, wd, s, g, c);
     OB_FENCE_DOWN(l)
   }
-  // ---- B1: bias forces bottom-up over the inner links -> rhs b ----
+  // ---- the apples: tether forces, reactions on their links ----
 #pragma unroll 1
-  for (int i = tid; i < wd->N; i += nt)                 // what A2 left for the children of an inner link is dead now
-    if ((__float_as_uint(s.P[7 * i + kCS].w) >> kNcShift) & kNcMask) stage_link_inputs(i, s, g, true);
+  for (int a = tid; a < wd->A; a += nt) apple_forces(a, s, c.P);
+  __syncthreads();
+  // ---- B1: bias forces bottom-up over the parked links -> rhs b ----
+#pragma unroll 1
+  for (int i = tid; i < wd->N; i += nt) {               // what A2 left in the record of a parked link is dead now
+    const uint32_t tw = __float_as_uint(s.P[7 * i + kCS].w);
+    if (((tw >> kNcShift) & kNcMask) | (tw & kHasApples)) stage_link_inputs(i, s, g, true);
+  }
   __syncthreads();
 #pragma unroll 1
-  for (int l = nlev - 2; l >= l_last_up; l--) {
+  for (int l = nlev - 1; l >= l_last_up; l--) {
     const int le = s.lev[l + 1];
 #pragma unroll 1
     for (int i = s.lev[l] + tid; i < le; i += nt) {
       const Jt j = load_jt(s.P, i);
-      if ((j.tw >> kNcShift) & kNcMask) link_bias_up(i, j, s, g, c);
+      if (((j.tw >> kNcShift) & kNcMask) | (j.tw & kHasApples)) link_bias_up(i, j, s, g, c);
     }
     OB_FENCE_UP(l)
   }
@@ -1332,7 +1352,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       g.topo2 = c.topo2 + d.link_base;
     }
     if (tid == 0) {
-      s_world.g = g; s_world.N = N; s_world.Np = Np; s_world.Ap = d.Ap; s_world.NFp = d.NFp; s_world.nlev = nlev;
+      s_world.g = g; s_world.N = N; s_world.A = d.A; s_world.Np = Np; s_world.Ap = d.Ap; s_world.NFp = d.NFp; s_world.nlev = nlev;
       s_world.ntop = ntop; s_world.precond = d.precond;
     }
 
