@@ -32,10 +32,13 @@ import numpy as np  # noqa: E402
 METRIC = "world-steps/s at 4096 trees x ~400 links"
 UNIT = "world-steps/s"
 
-# Algorithmic work per link: flops of the formulas, not instructions executed.
-FLOP_LINK_STEP = 700.0        # FK + joint transforms + bias RNEA + composite-inertia diagonal + integration + predicates
-FLOP_LINK_ITER = 150.0        # one PCG iteration: M*v (two sweeps) + 5 vector updates + 2 dot products
-FLOP_APPLE_STEP = 120.0       # tether force, reaction, clamp, integration, detach predicates
+# Algorithmic work per link: flops of the formulas of the path as it runs with the tree
+# preconditioner (precond = 2), checked against the fp32 + fp64 instruction counts of the ncu capture in profiles/
+# (0.60 Mflop fp32 + 0.07 Mflop fp64 per world-step at 397 links, 60 apples, 1.03 iterations: within 3 % of this model).
+FLOP_LINK_STEP = 1180.0       # joint quaternions + FK (fp64) 150, articulated-inertia factorisation 500, bias RNEA
+                              # 350, first product A x0 150, integration + predicates 30
+FLOP_LINK_ITER = 320.0        # one PCG iteration: A p (two sweeps) 150, z = P^-1 r (two sweeps) 150, vector updates, dots
+FLOP_APPLE_STEP = 150.0       # tether force, reaction, clamp, integration, detach predicates
 # Algorithmic HBM bytes per world-step if the state were streamed every step: 84 B per link,
 # 72 B per apple, 32 B of wrench.  With n steps fused per launch the traffic falls to 1/n of this.
 BYTES_LINK_STEP = 84.0
@@ -120,13 +123,24 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.samples)}
 
 
+def kernel_source_hash() -> str:
+    """sha256 (16 hex digits) over the CUDA sources of the library: ties a committed profile to the kernel it was of."""
+    import hashlib
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_2607_06337_b200", "csrc")
+    for f in sorted(os.listdir(csrc)):
+        h.update(open(os.path.join(csrc, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
 def _profiled_traffic(n_worlds: int, substeps: int):
     """DRAM bytes of one k_step launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed ncu --set full
-    capture, profiles/r1_k_step_dram.txt; null unless that capture was of a launch of this size."""
-    tp = os.path.join(ROOT, "profiles", "r1_k_step_dram.txt")
+    capture, profiles/r2_k_step_dram.txt.  PROFILED, not measured in this run: null unless that capture was of a launch
+    of this size AND of the kernel sources as they are now (the file carries their hash)."""
+    tp = os.path.join(ROOT, "profiles", "r2_k_step_dram.txt")
     try:
         kv = dict(l.split("=", 1) for l in open(tp).read().split() if "=" in l)
-        if int(kv["worlds"]) == n_worlds and int(kv["substeps"]) == substeps:
+        if int(kv["worlds"]) == n_worlds and int(kv["substeps"]) == substeps and kv["kernel_source_hash"] == kernel_source_hash():
             return float(kv["dram_bytes_per_launch"])
     except Exception:
         pass
@@ -174,10 +188,11 @@ def run_cuda(args, rank: int, world_size: int):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def run(e2e: bool):
+    def run(e2e: bool, with_state: bool = False):
         sim = ob.Orchard(specs, P)
         sim.randomize(seed)
         stream = sim.stream
+        state = None
         for e in range(args.warmup):
             if args.config == 5 and e > 0 and e % 5 == 0:
                 sim.randomize(seed + 5000 + e // 5)
@@ -203,7 +218,9 @@ def run_cuda(args, rank: int, world_size: int):
                 sim.apply_wrench_batch(*epochs[args.warmup + k])      # host arrays -> pinned staging -> device
                 sim.step(S)
                 n_events += len(sim.events())                          # device -> host: event list
-                sim.stats()                                            # device -> host: per-world counters
+                sim.stats()                                            # device -> host: totals
+                if with_state:                                         # device -> host: the state of EVERY world
+                    state = sim.get_state_batch(out=state)             # (q, qd, apples, flags, step / status words)
             else:
                 # kernel-resident leg: the epoch's wrenches are uploaded outside the per-launch events but
                 # inside the region (they are part of the workload); the launches are timed one by one
@@ -219,7 +236,8 @@ def run_cuda(args, rank: int, world_size: int):
         region_ms = t_begin.elapsed_time(t_end)
         kern_ms = None if e2e else [a.elapsed_time(b) for a, b in zip(ev0, ev1)]
         c1, s1 = sim.counters(), sim.stats()
-        out = dict(region_ms=region_ms, wall_s=wall, kern_ms=kern_ms, clocks=clocks, n_events=n_events,
+        hist = sim.iter_histogram()
+        out = dict(iter_hist=hist, region_ms=region_ms, wall_s=wall, kern_ms=kern_ms, clocks=clocks, n_events=n_events,
                    world_steps=s1["world_steps_total"] - s0["world_steps_total"],
                    cg_iters=s1["cg_iters_total"] - s0["cg_iters_total"], flagged=s1["n_flagged"],
                    h2d=c1["h2d_bytes"] - c0["h2d_bytes"], d2h=c1["d2h_bytes"] - c0["d2h_bytes"],
@@ -230,6 +248,7 @@ def run_cuda(args, rank: int, world_size: int):
 
     dev = run(e2e=False)
     e2e = run(e2e=True)
+    e2s = run(e2e=True, with_state=True)
 
     def max_over_ranks(x: float) -> float:
         return reduce_over_ranks(x, "max", world_size)
@@ -240,6 +259,8 @@ def run_cuda(args, rank: int, world_size: int):
     kern_total_ms = max_over_ranks(sum(dev["kern_ms"]))
     region_ms = max_over_ranks(dev["region_ms"])
     e2e_ms = max_over_ranks(e2e["region_ms"])
+    e2s_ms = max_over_ranks(e2s["region_ms"])
+    ws_e2s = sum_over_ranks(e2s["world_steps"])
     ws_dev = sum_over_ranks(dev["world_steps"])
     ws_e2e = sum_over_ranks(e2e["world_steps"])
     iters_dev = sum_over_ranks(dev["cg_iters"])
@@ -279,13 +300,25 @@ def run_cuda(args, rank: int, world_size: int):
             "cg_iters_per_s": iters_dev / (region_ms * 1e-3),
             "cg_iters_per_world_step": iters_per_ws,
             "worlds_flagged": dev["flagged"],
+            "cg_iters_histogram": _hist_summary(dev["iter_hist"]),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"] / args.steps,
                     "d2h_bytes_per_step": e2e["d2h"] / args.steps, "ms_per_step": e2e_ms / args.steps,
-                    "events_read": e2e["n_events"]},
+                    "events_read": e2e["n_events"], "returns": "event list + totals every bench step",
+                    "with_state": {"value": ws_e2s / (e2s_ms * 1e-3), "unit": UNIT,
+                                   "h2d_bytes_per_step": e2s["h2d"] / args.steps,
+                                   "d2h_bytes_per_step": e2s["d2h"] / args.steps, "ms_per_step": e2s_ms / args.steps,
+                                   "returns": "event list + totals + q, qd, apple x / v, flags, step and status "
+                                              "words of EVERY world (ob_get_state_batch) every bench step"}},
             "gpu_launches": dev["launches"],
             "clocks": dev["clocks"],
             "roofline": {"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "TFLOP/s",
-                         "frac": alu_ach / alu_peak, "traffic": traffic, "kernel": "k_step",
+                         "frac": alu_ach / alu_peak, "traffic": traffic,
+                         "traffic_source": "profiled (profiles/r2_k_step_dram.txt, same kernel sources and launch size), "
+                                           "not measured in this run" if traffic is not None else None,
+                         "limiter": "latency, not throughput: a step is a chain of ~70 dependent level turns; ncu "
+                                    "(profiles/r2_k_step_ncu_full.md): issue slots 31 % busy, stall_barrier 3.6 / "
+                                    "no_instruction 1.3 / wait 1.4 per issued instruction",
+                         "kernel": "k_step",
                          "kernel_ms": k_ms, "flop_per_world_step": flop_ws,
                          "peak_source": f"148 SM x 128 fp32 lanes x 2 x {sm_mhz:.0f} MHz (clock sampled in the run)",
                          "hbm": {"achieved_streamed": hbm_stream, "achieved_fused": hbm_fused,
@@ -302,6 +335,19 @@ def run_cuda(args, rank: int, world_size: int):
         print(json.dumps(line), flush=True)
 
 
+def _hist_summary(hist) -> dict:
+    """p50 / p95 / max of PCG iterations per world-step from the device histogram (ob_iter_histogram)."""
+    h = np.asarray(hist, dtype=np.float64)
+    n = h.sum()
+    if n == 0:
+        return {"world_steps": 0}
+    cdf = np.cumsum(h) / n
+    nz = np.nonzero(h)[0]
+    return {"world_steps": int(n), "p50": int(np.searchsorted(cdf, 0.5)), "p95": int(np.searchsorted(cdf, 0.95)),
+            "p99": int(np.searchsorted(cdf, 0.99)), "max": int(nz[-1]), "last_bin_is_open": bool(nz[-1] == len(h) - 1),
+            "mean": float((np.arange(len(h)) * h).sum() / n)}
+
+
 def _omp_threads() -> int:
     try:
         n = len(os.sched_getaffinity(0))
@@ -310,14 +356,14 @@ def _omp_threads() -> int:
     return max(1, n)
 
 
-def _oracle_sample(specs, P, seed, f_lo, f_hi, n_sample):
+def _oracle_sample(specs, P, seed, f_lo, f_hi, n_sample, solver=0):
     """Oracle worlds for the first n_sample worlds of the batch, randomized and loaded like the GPU run."""
     import oracle
     from workloads import wrench_process
     loads = wrench_process(specs, 0, f_lo, f_hi)
     worlds = []
     for w in range(n_sample):
-        r = oracle.OracleWorld(specs[w], P, world_index=w)
+        r = oracle.OracleWorld(specs[w], P, world_index=w, solver=solver)
         r.randomize(seed)
         r.apply_wrench(loads[w][1], loads[w][2], loads[w][3])
         worlds.append(r)
@@ -337,9 +383,49 @@ def cpu_baseline(specs, P, seed, f_lo, f_hi) -> dict:
     t0 = time.perf_counter()
     oracle.step_many(worlds, n_steps)
     dt = time.perf_counter() - t0
-    return {"value": n_sample * n_steps / dt, "unit": UNIT, "cores": min(cores, n_sample), "kind": "oracle",
-            "sample": f"first {n_sample} worlds of the batch x {n_steps} steps after 1 warm-up step "
-                      f"(fp64, mass matrix by unit-acceleration RNEA columns, dense Cholesky), {dt:.2f} s wall"}
+    out = {"value": n_sample * n_steps / dt, "unit": UNIT, "cores": min(cores, n_sample), "kind": "oracle",
+           "sample": f"first {n_sample} worlds of the batch x {n_steps} steps after 1 warm-up step "
+                     f"(fp64, mass matrix by unit-acceleration RNEA columns, dense Cholesky), {dt:.2f} s wall"}
+    # the oracle's own fp64 Jacobi-PCG mode (same algorithm class as the GPU path; the matrix is still formed by
+    # brute force) as the fairer CPU figure SURVEY.md 8(d) asks for
+    pw = _oracle_sample(specs, P, seed, f_lo, f_hi, n_sample, solver=1)
+    oracle.step_many(pw, 1)
+    t0 = time.perf_counter()
+    oracle.step_many(pw, n_steps)
+    dtp = time.perf_counter() - t0
+    out["pcg_mode"] = {"value": n_sample * n_steps / dtp, "unit": UNIT,
+                       "sample": f"same sample, oracle solver = fp64 Jacobi-PCG on the assembled matrix, {dtp:.2f} s wall"}
+    out["parity_sample"] = _parity_sample(specs, P, seed, f_lo, f_hi, worlds, 1 + n_steps)
+    return out
+
+
+def _parity_sample(specs, P, seed, f_lo, f_hi, refs, n_steps) -> dict:
+    """The sampled worlds once more on the GPU, free-running the same steps as the (Cholesky) oracle worlds `refs`:
+    events on one side only, and the worst relative state error among the worlds without events."""
+    import paper_2607_06337_b200 as ob
+    from workloads import wrench_process
+    n = len(refs)
+    sim = ob.Orchard(specs[:n], P)
+    sim.randomize(seed)
+    loads = wrench_process(specs, 0, f_lo, f_hi)[:n]
+    sim.apply_wrench_batch([l[0] for l in loads], [l[1] for l in loads], [l[2] for l in loads], [l[3] for l in loads])
+    sim.step(n_steps)
+    gev = {(e[0], e[1], e[2], e[3]) for e in sim.events()}
+    oev = {(e[0], e[1], e[2], e[3]) for r in refs for e in r.events()}
+    worlds_with_events = {k[0] for k in gev | oev}
+    worst = 0.0
+    for w, r in enumerate(refs):
+        if w in worlds_with_events:
+            continue
+        g, o = sim.get_state(w), r.get_state()
+        for k, floor in (("q", 1e-6), ("qd", 1e-4)):
+            den = max(np.linalg.norm(o[k]), floor * math.sqrt(o[k].size))
+            worst = max(worst, float(np.linalg.norm(g[k].astype(np.float64) - o[k]) / den))
+    sim.close()
+    return {"worlds": n, "steps": n_steps, "events_gpu": len(gev), "events_oracle": len(oev),
+            "events_on_one_side_only": len(gev ^ oev), "max_rel_state_error_worlds_without_events": worst,
+            "protocol": "free run from the randomized rest state (the lock-step protocol with its near-threshold count "
+                        "is tests/test_gpu_parity.py)"}
 
 
 def run_reference(args, rank: int, world_size: int):
