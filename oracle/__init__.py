@@ -41,6 +41,16 @@ class OboParams(C.Structure):
     ]
 
 
+class OboGeometryRanges(C.Structure):
+    _fields_ = [(n, C.c_float * 2) for n in ("droop", "lean", "spread", "twist", "scale_length", "scale_diameter",
+                                             "jitter_length", "jitter_diameter")]
+
+
+GEOMETRY_IDENTITY = dict(droop=(0.0, 0.0), lean=(0.0, 0.0), spread=(0.0, 0.0), twist=(0.0, 0.0),
+                         scale_length=(1.0, 1.0), scale_diameter=(1.0, 1.0), jitter_length=(1.0, 1.0),
+                         jitter_diameter=(1.0, 1.0))
+
+
 class OboEvent(C.Structure):
     _fields_ = [("world", C.c_int32), ("step", C.c_int32), ("kind", C.c_int32), ("index", C.c_int32),
                 ("value", C.c_double), ("threshold", C.c_double)]
@@ -60,6 +70,8 @@ def lib():
                                     C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(OboParams)]
         L.obo_world_free.argtypes = [C.c_void_p]
         L.obo_randomize.argtypes = [C.c_void_p, C.c_uint64]
+        L.obo_randomize_geometry.argtypes = [C.c_void_p, C.c_uint64, C.POINTER(OboGeometryRanges)]
+        L.obo_diag_geometry.argtypes = [C.c_void_p] + [C.c_void_p] * 4
         L.obo_apply_wrench.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         L.obo_apply_wrench.restype = C.c_int
         L.obo_step.argtypes = [C.c_void_p, C.c_int]
@@ -159,6 +171,18 @@ class OracleWorld:
 
     def randomize(self, seed: int):
         lib().obo_randomize(self.h, C.c_uint64(seed))
+
+    def randomize_geometry(self, seed: int, **ranges):
+        """ranges: any of GEOMETRY_IDENTITY's keys as (lo, hi); the others keep their identity value."""
+        g = OboGeometryRanges()
+        for k, v in {**GEOMETRY_IDENTITY, **ranges}.items():
+            setattr(g, k, (C.c_float * 2)(*v))
+        lib().obo_randomize_geometry(self.h, C.c_uint64(seed), C.byref(g))
+
+    def geometry(self):
+        L = np.zeros(self.N); d = np.zeros(self.N); Q = np.zeros((self.N, 3, 3)); ao = np.zeros((self.A, 3))
+        lib().obo_diag_geometry(self.h, L.ctypes.data, d.ctypes.data, Q.ctypes.data, ao.ctypes.data)
+        return dict(length=L, diameter=d, Q=Q, apple_offset=ao)
 
     def apply_wrench(self, body: int, point, force):
         p = np.asarray(point, dtype=np.float32).astype(np.float64)

@@ -74,6 +74,8 @@ typedef struct {
   /* topology and rest geometry (from the fp32 inputs, promoted) */
   int *parent;
   double *L, *d, *Q /*[9N] rest rotation, row-major*/, *arm /*[2N]*/;
+  float *L0, *d0;           /* base geometry as given at construction (fp32 inputs) */
+  double *Q0, *aoff0;       /* base rest rotations and apple offsets */
   float rho_nom, E_nom, MOR_nom;
   float rho, E, MOR; /* current (fp32 draws, A23) */
   /* derived per link */
@@ -473,6 +475,9 @@ obo_world *obo_world_new(int world_index, int n_links, const int32_t *parent, co
   W->d = (double *)malloc(sizeof(double) * N);
   W->Q = (double *)malloc(sizeof(double) * 9 * N);
   W->arm = (double *)calloc(2 * (size_t)N, sizeof(double));
+  W->L0 = (float *)malloc(sizeof(float) * N);
+  W->d0 = (float *)malloc(sizeof(float) * N);
+  W->Q0 = (double *)malloc(sizeof(double) * 9 * N);
   W->K = (double *)malloc(sizeof(double) * N);
   W->Mmax = (double *)malloc(sizeof(double) * N);
   W->m = (double *)malloc(sizeof(double) * N);
@@ -484,11 +489,14 @@ obo_world *obo_world_new(int world_index, int n_links, const int32_t *parent, co
     W->d[i] = (double)diameter[i];
     double qn[4] = {rest_quat[4 * i], rest_quat[4 * i + 1], rest_quat[4 * i + 2], rest_quat[4 * i + 3]};
     quat_to_mat(qn, W->Q + 9 * i);
+    W->L0[i] = length[i]; W->d0[i] = diameter[i];
+    memcpy(W->Q0 + 9 * i, W->Q + 9 * i, sizeof(double) * 9);
     if (armature) { W->arm[2 * i] = armature[2 * i]; W->arm[2 * i + 1] = armature[2 * i + 1]; }
   }
   W->rho_nom = W->rho = density; W->E_nom = W->E = E; W->MOR_nom = W->MOR = MOR;
   W->alink = (int *)malloc(sizeof(int) * (A + 1));
   W->aoff = (double *)malloc(sizeof(double) * 3 * (A + 1));
+  W->aoff0 = (double *)malloc(sizeof(double) * 3 * (A + 1));
   W->am_nom = (float *)malloc(sizeof(float) * (A + 1));
   W->adet_nom = (float *)malloc(sizeof(float) * (A + 1));
   W->ac_in = (float *)calloc((size_t)A + 1, sizeof(float));
@@ -499,7 +507,7 @@ obo_world *obo_world_new(int world_index, int n_links, const int32_t *parent, co
   W->adet = (double *)malloc(sizeof(double) * (A + 1));
   for (int a = 0; a < A; a++) {
     W->alink[a] = apple_link[a];
-    for (int k = 0; k < 3; k++) W->aoff[3 * a + k] = (double)apple_offset[3 * a + k];
+    for (int k = 0; k < 3; k++) W->aoff0[3 * a + k] = W->aoff[3 * a + k] = (double)apple_offset[3 * a + k];
     W->am_nom[a] = apple_mass[a]; W->am[a] = (double)apple_mass[a];
     W->adet_nom[a] = apple_detach[a]; W->adet[a] = (double)apple_detach[a];
     W->ak[a] = (double)apple_k[a];
@@ -524,6 +532,7 @@ obo_world *obo_world_new(int world_index, int n_links, const int32_t *parent, co
 void obo_world_free(obo_world *W) {
   if (!W) return;
   free(W->parent); free(W->L); free(W->d); free(W->Q); free(W->arm);
+  free(W->L0); free(W->d0); free(W->Q0); free(W->aoff0);
   free(W->K); free(W->Mmax); free(W->m); free(W->Ixx); free(W->Izz);
   free(W->alink); free(W->aoff); free(W->am_nom); free(W->adet_nom); free(W->ac_in);
   free(W->am); free(W->ak); free(W->ac); free(W->adet);
@@ -555,6 +564,126 @@ void obo_randomize(obo_world *W, uint64_t seed) {
     W->adet[a] = (double)fd;
     W->am[a] = (double)fm;
   }
+  derive_constants(W);
+  reset_state(W);
+}
+
+/* ----------------------------------------------------------------------- */
+/* per-world geometry randomization (reading A37)     */
+/* ----------------------------------------------------------------------- */
+typedef struct {
+  float droop[2], lean[2], spread[2], twist[2];
+  float scale_length[2], scale_diameter[2], jitter_length[2], jitter_diameter[2];
+} obo_geometry_ranges;
+
+/* rotation by angle t about the unit axis a (Rodrigues) */
+static void rot_axis(const double a[3], double t, double *R) {
+  double c = cos(t), s = sin(t), v = 1.0 - c;
+  R[0] = c + a[0] * a[0] * v;        R[1] = a[0] * a[1] * v - a[2] * s; R[2] = a[0] * a[2] * v + a[1] * s;
+  R[3] = a[1] * a[0] * v + a[2] * s; R[4] = c + a[1] * a[1] * v;        R[5] = a[1] * a[2] * v - a[0] * s;
+  R[6] = a[2] * a[0] * v - a[1] * s; R[7] = a[2] * a[1] * v + a[0] * s; R[8] = c + a[2] * a[2] * v;
+}
+
+/* "we generate one base skeleton and perturb only continuous quantities per world ... per-segment bend and whole-tree
+   growth habit (a gravimorphic droop multiplier applied inside a forward-kinematic re-walk so droop compounds per
+   internode ..., plus whole-tree lean, fork spread and an env-wide phyllotactic twist)" and the per-branch
+   dimensions "(global scale and stockiness, and per-segment length and thickness)".  Always
+   starts from the BASE geometry, so zero strength reproduces the base model exactly.  Reading A37:
+     draws (A23 layout): stream 3 item 0 -> droop, lean, spread, twist; stream 3 item 1 -> lean azimuth (u * 2 pi),
+       length scale, diameter scale; stream 4 item i -> length jitter, diameter jitter of link i; a degenerate range
+       gives its lo value;
+     dimensions: L_i = (L0_i * scale_length) * jitter_i, d_i likewise, in fp32; apple offsets scale with their link
+       (x, y by the diameter factor, z by the length factor);
+     twist: every non-trunk rest rotation becomes Rz(twist) Q_i (turned about the parent's axis);
+     spread: the swing of Q_i away from the parent's axis (swing-twist decomposition about z) is scaled by 1 + spread;
+     lean: the trunk's rest rotation becomes Rot((cos phi, sin phi, 0), lean) Q_0;
+     droop: a top-down re-walk in the world frame; with d = R_i z the link direction, s = |d x z_w| the sine of its
+       angle to the vertical, the link frame is turned by droop * s about (d x -z_w) / s, i.e. towards the ground;
+       children inherit the turned frame (the droop compounds per internode).
+   Materials are kept; derived constants are recomputed and the state is reset. */
+void obo_randomize_geometry(obo_world *W, uint64_t seed, const obo_geometry_ranges *G) {
+  const double PI = 3.14159265358979323846;
+  uint32_t key[2] = {(uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32)};
+  uint32_t ctr[4] = {(uint32_t)W->world_index, 0u, 3u, 0u}, o[4];
+  obo_philox4x32_10(ctr, key, o);
+  float droop = philox_uniform(o[0], G->droop[0], G->droop[1]);
+  float lean = philox_uniform(o[1], G->lean[0], G->lean[1]);
+  float spread = philox_uniform(o[2], G->spread[0], G->spread[1]);
+  float twist = philox_uniform(o[3], G->twist[0], G->twist[1]);
+  ctr[1] = 1u;
+  obo_philox4x32_10(ctr, key, o);
+  float phi = philox_uniform(o[0], 0.0f, 6.2831855f);
+  float sL = philox_uniform(o[1], G->scale_length[0], G->scale_length[1]);
+  float sD = philox_uniform(o[2], G->scale_diameter[0], G->scale_diameter[1]);
+  int N = W->N;
+  float *fl = (float *)malloc(sizeof(float) * N), *fd = (float *)malloc(sizeof(float) * N);
+  for (int i = 0; i < N; i++) {
+    ctr[1] = (uint32_t)i; ctr[2] = 4u;
+    obo_philox4x32_10(ctr, key, o);
+    float jl = philox_uniform(o[0], G->jitter_length[0], G->jitter_length[1]);
+    float jd = philox_uniform(o[1], G->jitter_diameter[0], G->jitter_diameter[1]);
+    float t = W->L0[i] * sL; float Ln = t * jl;
+    float u = W->d0[i] * sD; float dn = u * jd;
+    W->L[i] = (double)Ln; W->d[i] = (double)dn;
+    fl[i] = Ln / W->L0[i]; fd[i] = dn / W->d0[i];
+  }
+  for (int a = 0; a < W->A; a++) {
+    int b = W->alink[a];
+    W->aoff[3 * a] = (double)((float)W->aoff0[3 * a] * fd[b]);
+    W->aoff[3 * a + 1] = (double)((float)W->aoff0[3 * a + 1] * fd[b]);
+    W->aoff[3 * a + 2] = (double)((float)W->aoff0[3 * a + 2] * fl[b]);
+  }
+  free(fl); free(fd);
+  /* rest rotations: twist, spread, lean, then the droop re-walk */
+  double *RW = (double *)malloc(sizeof(double) * 9 * N);   /* world rest rotation of every link, after droop */
+  for (int i = 0; i < N; i++) {
+    double Qn[9];
+    memcpy(Qn, W->Q0 + 9 * i, sizeof(Qn));
+    int pa = W->parent[i];
+    if (pa >= 0) {
+      /* swing-twist decomposition about z: the direction of the child axis in the parent frame is column 2 of Q */
+      double dz[3] = {Qn[2], Qn[5], Qn[8]};
+      double sw = atan2(sqrt(dz[0] * dz[0] + dz[1] * dz[1]), dz[2]);       /* swing angle away from the parent's axis */
+      double hn = sqrt(dz[0] * dz[0] + dz[1] * dz[1]);
+      if (hn > 1e-12 && spread != 0.0f) {
+        double ax[3] = {-dz[1] / hn, dz[0] / hn, 0.0};                     /* z x dz, the swing axis */
+        double Rs[9];
+        rot_axis(ax, sw * (double)spread, Rs);                             /* extra swing: sw (1 + spread) in all */
+        mat3mul(Rs, Qn, Qn);
+      }
+      if (twist != 0.0f) {
+        double z[3] = {0, 0, 1}, Rt[9];
+        rot_axis(z, (double)twist, Rt);
+        mat3mul(Rt, Qn, Qn);
+      }
+    } else if (lean != 0.0f) {
+      double ax[3] = {cos((double)phi), sin((double)phi), 0.0}, Rl[9];
+      rot_axis(ax, (double)lean, Rl);
+      mat3mul(Rl, Qn, Qn);
+    }
+    if (droop == 0.0f) {                       /* no re-walk: the modified rest rotation is the result, exactly */
+      memcpy(W->Q + 9 * i, Qn, sizeof(Qn));
+      continue;
+    }
+    static const double I3[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1};
+    const double *Rp = pa < 0 ? I3 : RW + 9 * pa;
+    double Ri[9];
+    mat3mul(Rp, Qn, Ri);
+    double d[3] = {Ri[2], Ri[5], Ri[8]};
+    double s = sqrt(d[0] * d[0] + d[1] * d[1]);                            /* |d x z_w| */
+    if (s > 1e-12 && droop != 0.0f) {
+      double ax[3] = {-d[1] / s, d[0] / s, 0.0}, Rd[9];                    /* (d x -z_w) / s */
+      rot_axis(ax, (double)droop * s, Rd);
+      mat3mul(Rd, Ri, Ri);
+    }
+    memcpy(RW + 9 * i, Ri, sizeof(Ri));
+    /* new rest rotation in the parent frame: Rp^T Ri */
+    double Rpt[9];
+    for (int r_ = 0; r_ < 3; r_++)
+      for (int c_ = 0; c_ < 3; c_++) Rpt[3 * r_ + c_] = Rp[3 * c_ + r_];
+    mat3mul(Rpt, Ri, W->Q + 9 * i);
+  }
+  free(RW);
   derive_constants(W);
   reset_state(W);
 }
@@ -866,6 +995,12 @@ int obo_n_events(const obo_world *W) { return W->n_ev; }
 /* ----------------------------------------------------------------------- */
 /* diagnostics for the pins                                                  */
 /* ----------------------------------------------------------------------- */
+void obo_diag_geometry(const obo_world *W, double *L, double *d, double *Q, double *aoff) {
+  if (L) memcpy(L, W->L, sizeof(double) * W->N);
+  if (d) memcpy(d, W->d, sizeof(double) * W->N);
+  if (Q) memcpy(Q, W->Q, sizeof(double) * 9 * W->N);
+  if (aoff) memcpy(aoff, W->aoff, sizeof(double) * 3 * W->A);
+}
 void obo_diag_material(const obo_world *W, float *E_MOR_rho /*3*/, double *adet, double *am, double *ac) {
   E_MOR_rho[0] = W->E; E_MOR_rho[1] = W->MOR; E_MOR_rho[2] = W->rho;
   for (int a = 0; a < W->A; a++) { if (adet) adet[a] = W->adet[a]; if (am) am[a] = W->am[a]; if (ac) ac[a] = W->ac[a]; }

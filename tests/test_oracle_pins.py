@@ -836,3 +836,116 @@ def test_wrench_slot_semantics():
     # a wrench on an apple is a force on the apple, not on the tree: b is unchanged, the apple accelerates
     ba = rhs([(spec.n_links + 1, (0, 0, 0), (0.0, 3.0, 0.0))])
     assert np.abs(ba - b0).max() == 0.0
+
+
+# ---------------------------------------------------------------- per-world geometry randomization (8(f) item 3, A37)
+def _u32_uniform(x, lo, hi):
+    u = np.float32(int(x) >> 8) * np.float32(2.0 ** -24)
+    return np.float32(np.float64(u) * np.float64(np.float32(hi) - np.float32(lo)) + np.float64(np.float32(lo)))
+
+
+def test_geometry_randomization_zero_strength_reproduces_the_base_model():
+    """the on-device build "reproduces the replicated base model exactly at zero strength"."""
+    rng = np.random.default_rng(21)
+    spec = stochastic_world(rng, 60, 90, 8, depth_choices=(4, 5))
+    P = config_params(2)
+    w = OracleWorld(spec, P, world_index=3)
+    g0, A0, b0, s0 = w.geometry(), *w.system(), w.get_state()
+    w.randomize_geometry(12345)
+    g1, (A1, b1), s1 = w.geometry(), w.system(), w.get_state()
+    for k in g0:
+        assert np.array_equal(g0[k], g1[k]) if k != "Q" else np.abs(g0[k] - g1[k]).max() < 1e-15, k
+    assert np.abs(A1 - A0).max() <= 1e-12 * np.abs(A0).max() and np.abs(s1["apple_x"] - s0["apple_x"]).max() < 1e-13
+
+
+def test_geometry_randomization_dimensions_follow_the_draws():
+    """Reading A37: L_i = (L0_i * scale) * jitter_i in fp32 (stream 3 item 1, stream 4 item i), diameters likewise;
+    K, M_max, m follow Eq. 4 / Eq. 5; apple offsets scale with their link; apples hang at rest under the new tips."""
+    rng = np.random.default_rng(22)
+    spec = stochastic_world(rng, 40, 60, 6, depth_choices=(4,))
+    w = OracleWorld(spec, config_params(2), world_index=5)
+    seed = (9 << 32) | 77
+    rg = dict(scale_length=(0.8, 1.25), scale_diameter=(0.7, 1.3), jitter_length=(0.9, 1.1), jitter_diameter=(0.85, 1.15))
+    w.randomize_geometry(seed, **rg)
+    key = [seed & 0xffffffff, seed >> 32]
+    o = philox4x32_10([5, 1, 3, 0], key)
+    sL, sD = _u32_uniform(o[1], *rg["scale_length"]), _u32_uniform(o[2], *rg["scale_diameter"])
+    g = w.geometry()
+    for i in range(spec.n_links):
+        oi = philox4x32_10([5, i, 4, 0], key)
+        Ln = np.float32(np.float32(spec.length[i] * sL) * _u32_uniform(oi[0], *rg["jitter_length"]))
+        dn = np.float32(np.float32(spec.diameter[i] * sD) * _u32_uniform(oi[1], *rg["jitter_diameter"]))
+        assert g["length"][i] == float(Ln) and g["diameter"][i] == float(dn), i
+    d = w.derived()
+    E, rho = float(np.float32(spec.E)), float(np.float32(spec.density))
+    assert np.allclose(d["K"], E * math.pi * g["diameter"] ** 4 / (64 * g["length"]), rtol=1e-12)
+    assert np.allclose(d["m"], rho * math.pi * (g["diameter"] / 2) ** 2 * g["length"], rtol=1e-12)
+    assert 0.55 < (g["length"] / spec.length).min() and (g["length"] / spec.length).max() < 1.45
+    for a in range(spec.n_apples):                       # apples sit at the tip (0, 0, L): they stay at the new tip
+        b = spec.apple_link[a]
+        assert abs(g["apple_offset"][a][2] - g["length"][b]) < 1e-6 * g["length"][b]
+    R, p, _, _ = w.fk()
+    s = w.get_state()
+    for a in range(spec.n_apples):
+        b = spec.apple_link[a]
+        xh = p[b] + R[b] @ g["apple_offset"][a]
+        assert np.allclose(xh - s["apple_x"][a], [0, 0, float(spec.apple_mass[a]) * G / float(spec.apple_k[a])], atol=1e-9)
+
+
+def test_geometry_randomization_lean_twist_spread_against_scipy():
+    """Lean tilts the trunk by the drawn angle about a horizontal axis of drawn azimuth; twist turns every child about
+    its parent's axis; spread scales the angle between a child and its parent's axis and keeps its azimuth."""
+    spec = binary_tree_config1()
+    seed = 4242
+    key = [seed, 0]
+    Q0 = np.stack([Rotation.from_quat([q[1], q[2], q[3], q[0]]).as_matrix() for q in spec.rest_quat.astype(np.float64)])
+    w = OracleWorld(spec, config_params(1), world_index=2)
+    o0, o1 = philox4x32_10([2, 0, 3, 0], key), philox4x32_10([2, 1, 3, 0], key)
+    # lean only
+    w.randomize_geometry(seed, lean=(0.05, 0.30))
+    lean = float(_u32_uniform(o0[1], 0.05, 0.30)); phi = float(_u32_uniform(o1[0], 0.0, 6.2831855))
+    Q = w.geometry()["Q"]
+    Rl = Rotation.from_rotvec(lean * np.array([math.cos(phi), math.sin(phi), 0.0])).as_matrix()
+    assert np.abs(Q[0] - Rl @ Q0[0]).max() < 1e-12 and np.abs(Q[1:] - Q0[1:]).max() < 1e-12
+    assert abs(math.acos(np.clip((Q[0] @ [0, 0, 1]) @ (Q0[0] @ [0, 0, 1]), -1, 1)) - lean) < 1e-9
+    # twist only
+    w.randomize_geometry(seed, twist=(-0.6, 0.6))
+    tw = float(_u32_uniform(o0[3], -0.6, 0.6))
+    Q = w.geometry()["Q"]
+    Rz = Rotation.from_euler("z", tw).as_matrix()
+    assert abs(tw) > 1e-3 and np.abs(Q[0] - Q0[0]).max() < 1e-15
+    for i in range(1, spec.n_links):
+        assert np.abs(Q[i] - Rz @ Q0[i]).max() < 1e-12
+    # spread only
+    w.randomize_geometry(seed, spread=(0.1, 0.4))
+    sp = float(_u32_uniform(o0[2], 0.1, 0.4))
+    Q = w.geometry()["Q"]
+    for i in range(1, spec.n_links):
+        d0, d1 = Q0[i] @ [0, 0, 1], Q[i] @ [0, 0, 1]
+        a0, a1 = math.atan2(math.hypot(d0[0], d0[1]), d0[2]), math.atan2(math.hypot(d1[0], d1[1]), d1[2])
+        assert abs(a1 - (1 + sp) * a0) < 1e-9 and abs(math.atan2(d1[1], d1[0]) - math.atan2(d0[1], d0[0])) < 1e-9
+        assert abs(np.linalg.det(Q[i]) - 1) < 1e-12 and np.abs(Q[i] @ Q[i].T - np.eye(3)).max() < 1e-12
+
+
+def test_geometry_randomization_droop_compounds_per_internode():
+    """"a gravimorphic droop multiplier applied inside a forward-kinematic re-walk so droop compounds per
+    internode".  A straight chain inclined by theta_0: internode k ends up at theta_k = t + droop sin t with
+    t = theta_(k-1) (its parent's final inclination), in the plane of the chain."""
+    n, th0, droop = 6, math.radians(40.0), 0.15
+    spec = chain_spec(n, 1.2, 0.03, root_quat=quat_axis("x", -math.degrees(th0)))     # tilted in the y-z plane
+    w = OracleWorld(spec, Params(), world_index=0)
+    R, p, _, _ = w.fk()
+    th0 = math.acos(R[0][2, 2])                        # the inputs are fp32: the inclination and the multiplier as
+    droop = float(np.float32(droop))                   # the oracle receives them
+    w.randomize_geometry(1, droop=(droop, droop))
+    R, p, _, _ = w.fk()
+    t = 0.0
+    prev = th0
+    for k in range(n):
+        base = prev if k > 0 else th0
+        t = base + droop * math.sin(base)
+        d = R[k] @ [0, 0, 1]
+        assert abs(d[0]) < 1e-12 and d[1] > 0                          # stays in the plane it was tilted in
+        assert abs(math.acos(np.clip(d[2], -1, 1)) - t) < 1e-9, (k, t)
+        prev = t
+    assert prev > th0 + n * droop * math.sin(th0) * 0.99              # compounding: more than n equal increments
