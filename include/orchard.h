@@ -110,6 +110,19 @@ typedef struct {
   float value, threshold;       /* rupture: K|theta| vs M_max; detach: |f_user| vs f_detach or |f_s| vs kappa f_detach */
 } ob_event;
 
+/* Ranges of ob_randomize_geometry (uniform per world unless noted; lo == hi gives that value for every world). */
+typedef struct {
+  float droop[2];               /* rad: every link is turned towards the ground by droop * sin(its angle to the vertical)
+                                   inside a top-down re-walk, so the droop compounds per internode */
+  float lean[2];                /* rad: whole-tree lean of the trunk about a horizontal axis of uniform azimuth */
+  float spread[2];              /* relative: the angle between a child and its parent's axis is scaled by 1 + spread */
+  float twist[2];               /* rad: every child's rest frame is turned about its parent's axis */
+  float scale_length[2];        /* per-world factor on every link length ("global scale") */
+  float scale_diameter[2];      /* per-world factor on every link diameter ("stockiness") */
+  float jitter_length[2];       /* per-LINK factor on its length ("per-segment length") */
+  float jitter_diameter[2];     /* per-LINK factor on its diameter ("per-segment thickness") */
+} ob_geometry_ranges;
+
 /* Fill *p with the defaults above (the readings A1..A33 of DESIGN.md section 3).  Returns OB_E_ARG for NULL. */
 int ob_default_params(ob_params *p);
 
@@ -136,6 +149,22 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
    full reset: rest pose, zero velocities, flags, counters, step = 0, wrench slots cleared, warm start cleared.
    Pending events stay queued.  Asynchronous. */
 int ob_randomize(ob_ctx *ctx, uint64_t seed);
+
+/* Per-world GEOMETRY randomization on the device ("per-segment bend and whole-tree growth habit (a
+   gravimorphic droop multiplier applied inside a forward-kinematic re-walk ..., plus whole-tree lean, fork spread and
+   an env-wide phyllotactic twist)" and the per-branch dimensions "(global scale and stockiness, and per-segment length
+   and thickness)"; "an on-device build that perturbs every world's branch geometry in a single ... kernel
+   (one thread per world)").  Every world gets its own draws (Philox4x32-10, key = seed; stream 3 item 0 -> droop, lean,
+   spread, twist; stream 3 item 1 -> lean azimuth, length scale, diameter scale; stream 4 item i -> length and
+   diameter jitter of link i), applied to the BASE geometry given to ob_create, so identity ranges (angles 0, factors
+   1) reproduce the base model exactly and calls do not compound.  Apple attach points move with their link (x, y by
+   its diameter factor, z by its length factor).  Then: rest hang points, the derived constants of Eq. 4 / Eq. 5 with
+   the materials as they are, and a full state reset as in ob_randomize.  Distinct geometry per world costs nothing
+   at step time here (every world carries its own dimensions anyway).  Synchronises (rest hang points come back). */
+int ob_randomize_geometry(ob_ctx *ctx, uint64_t seed, const ob_geometry_ranges *ranges);
+/* Current geometry of one world (after ob_randomize_geometry): length, diameter [n_links]; rest_quat [4*n_links] doubles
+   (w,x,y,z); apple_offset [3*n_apples].  Any pointer may be NULL.  Synchronises. */
+int ob_get_geometry(ob_ctx *ctx, int world, float *length, float *diameter, double *rest_quat, float *apple_offset);
 
 /* north_star "ob_apply_wrench(world, body, point, force)": a persistent external force ("applied and interactive
    forces").  body in [0, n_links) is a link, [n_links, n_links + n_apples) an apple (a pull on the
@@ -230,6 +259,7 @@ int ob_counters(ob_ctx *ctx, uint64_t out[4]);
 int ob_sizeof_params(void);
 int ob_sizeof_world_spec(void);
 int ob_sizeof_event(void);
+int ob_sizeof_geometry_ranges(void);
 
 /* Self-test of the device Philox4x32-10 (reading A23) against NVIDIA's own implementation: for n (counter, key)
    pairs computes the library's generator and cuRAND's curand_Philox4x32_10 on the device.  ctr: [4*n], key: [2*n],

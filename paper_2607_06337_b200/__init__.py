@@ -19,7 +19,9 @@ from .binding import (  # noqa: F401
     default_params,
     load_library,
     marshal_specs,
+    GEOMETRY_IDENTITY,
     ob_event,
+    ob_geometry_ranges,
     ob_params,
     ob_world_spec,
     params_struct,

@@ -24,6 +24,7 @@ EXPORTS = [
     "ob_sizeof_params", "ob_sizeof_world_spec", "ob_sizeof_event", "ob_counters", "ob_flush",
     "ob_selftest_philox", "ob_get_state_batch", "ob_set_apple_x64", "ob_set_step", "ob_get_counters_batch",
     "ob_get_material_batch", "ob_world_blob_bytes", "ob_save_world", "ob_load_world", "ob_iter_histogram",
+    "ob_randomize_geometry", "ob_get_geometry", "ob_sizeof_geometry_ranges",
 ]
 
 
@@ -48,6 +49,16 @@ class ob_params(C.Structure):
         ("range_E", C.c_float * 2), ("range_MOR", C.c_float * 2), ("range_density", C.c_float * 2),
         ("range_detach", C.c_float * 2), ("range_apple_mass", C.c_float * 2), ("mass_damping", C.c_float),
     ]
+
+
+class ob_geometry_ranges(C.Structure):
+    _fields_ = [(n, C.c_float * 2) for n in ("droop", "lean", "spread", "twist", "scale_length", "scale_diameter",
+                                             "jitter_length", "jitter_diameter")]
+
+
+GEOMETRY_IDENTITY = dict(droop=(0.0, 0.0), lean=(0.0, 0.0), spread=(0.0, 0.0), twist=(0.0, 0.0),
+                         scale_length=(1.0, 1.0), scale_diameter=(1.0, 1.0), jitter_length=(1.0, 1.0),
+                         jitter_diameter=(1.0, 1.0))
 
 
 class ob_event(C.Structure):
@@ -87,6 +98,8 @@ def load_library():
         L.ob_save_world.argtypes = [vp, i32, vp, C.c_size_t]
         L.ob_load_world.argtypes = [vp, i32, vp, C.c_size_t]
         L.ob_iter_histogram.argtypes = [vp, vp, i32, i32]
+        L.ob_randomize_geometry.argtypes = [vp, u64, C.POINTER(ob_geometry_ranges)]
+        L.ob_get_geometry.argtypes = [vp, i32] + [vp] * 4
         L.ob_get_counters.argtypes = [vp, i32] + [vp] * 3
         L.ob_set_counters.argtypes = [vp, i32] + [vp] * 3
         L.ob_get_material.argtypes = [vp, i32] + [vp] * 3
@@ -98,13 +111,14 @@ def load_library():
         L.ob_last_error.restype = C.c_char_p
         L.ob_destroy.argtypes = [vp]
         L.ob_destroy.restype = None
-        for name in ("ob_sizeof_params", "ob_sizeof_world_spec", "ob_sizeof_event"):
+        for name in ("ob_sizeof_params", "ob_sizeof_world_spec", "ob_sizeof_event", "ob_sizeof_geometry_ranges"):
             getattr(L, name).argtypes = []
         for name in EXPORTS:
             if name not in ("ob_last_error", "ob_destroy"):
                 getattr(L, name).restype = C.c_int
         if (L.ob_sizeof_params(), L.ob_sizeof_world_spec(), L.ob_sizeof_event()) != (
-                C.sizeof(ob_params), C.sizeof(ob_world_spec), C.sizeof(ob_event)):
+                C.sizeof(ob_params), C.sizeof(ob_world_spec), C.sizeof(ob_event)) or \
+                L.ob_sizeof_geometry_ranges() != C.sizeof(ob_geometry_ranges):
             raise RuntimeError("libob.so was built from a different include/orchard.h than this binding")
         _lib = L
     return _lib
@@ -221,6 +235,20 @@ class Orchard:
     # -- the C calls --
     def randomize(self, seed: int):
         self._check(self._L.ob_randomize(self._h, C.c_uint64(seed)))
+
+    def randomize_geometry(self, seed: int, **ranges):
+        """ranges: any of GEOMETRY_IDENTITY's keys as (lo, hi); the others keep their identity value."""
+        g = ob_geometry_ranges()
+        for k, v in {**GEOMETRY_IDENTITY, **ranges}.items():
+            setattr(g, k, (C.c_float * 2)(*v))
+        self._check(self._L.ob_randomize_geometry(self._h, C.c_uint64(seed), C.byref(g)))
+
+    def get_geometry(self, world: int) -> dict:
+        N, A = self.n_links[world], self.n_apples[world]
+        Ln = np.zeros(N, np.float32); dm = np.zeros(N, np.float32); q = np.zeros((N, 4), np.float64)
+        ao = np.zeros((A, 3), np.float32)
+        self._check(self._L.ob_get_geometry(self._h, world, _ptr(Ln), _ptr(dm), _ptr(q), _ptr(ao)))
+        return dict(length=Ln, diameter=dm, rest_quat=q, apple_offset=ao)
 
     def apply_wrench(self, world: int, body: int, point, force):
         p, f = _f32(point), _f32(force)

@@ -48,7 +48,7 @@ struct ob_ctx {
   int cls_off[kNumClasses] = {}, cls_n[kNumClasses] = {}, cls_grid[kNumClasses] = {}, cls_smem[kNumClasses] = {};
   int main_cls = 0, launches = 0, n_sm = 0;
   int max_Np = 0, max_Ap = 0;
-  size_t ev_cap = 0;
+  size_t ev_cap = 0, sum_ap = 0;
   uint64_t h2d_bytes = 0, d2h_bytes = 0, kernel_launches = 0, step_calls = 0;
   // size classes run concurrently: one internal stream per class, forked from and joined to the caller's stream
   cudaStream_t cls_stream[kNumClasses] = {};
@@ -184,7 +184,7 @@ int count_factor_slots_raw(const ob_world_spec &s) {
 
 struct Layout {
   size_t total = 0;
-  Pool desc, order, link_blk, link_cst, apple_blk, topo, topo2, quat_raw, quatd, Mmax, xprev, Lown, diam, arm, link_ext, apple_ext, apple_nom,
+  Pool desc, order, link_blk, link_cst, apple_blk, topo, topo2, quat_raw, quatd, Mmax, xprev, Lown, diam, Lown0, diam0, apple_off0, arm, link_ext, apple_ext, apple_nom,
       apple_c, anchor, level_off, info, wrench, events, ev_count, queue, iter_hist, stats, progress, pose7;
   size_t sumNp = 0, sumAp = 0, sumLev = 0, ev_cap = 0;
   int max_Np = 0, max_Ap = 0, max_smem = 0;
@@ -245,6 +245,9 @@ int plan(const ob_world_spec *specs, int n_worlds, const ob_params *P, Layout &L
   take(L, L.xprev, sizeof(float2) * 4 * L.sumNp);
   take(L, L.Lown, sizeof(float) * L.sumNp);
   take(L, L.diam, sizeof(float) * L.sumNp);
+  take(L, L.Lown0, sizeof(float) * L.sumNp);
+  take(L, L.diam0, sizeof(float) * L.sumNp);
+  take(L, L.apple_off0, sizeof(float) * 3 * std::max<size_t>(L.sumAp, 16));
   take(L, L.arm, L.any_arm ? sizeof(float) * 2 * L.sumNp : 0);
   take(L, L.link_ext, sizeof(int32_t) * L.sumNp);
   take(L, L.apple_ext, sizeof(int32_t) * std::max<size_t>(L.sumAp, 16));
@@ -300,6 +303,22 @@ int rd_reserve(ob_ctx *ctx, size_t bytes) {
 int check_range(ob_ctx *ctx, int world0, int n) {
   if (!ctx) return OB_E_ARG;
   if (world0 < 0 || n < 1 || world0 + n > ctx->n_worlds) return fail(ctx, OB_E_ARG, "world range [%d, %d) out of range", world0, world0 + n);
+  return OB_OK;
+}
+
+// rest hang points of every apple, device -> host mirror (caller order); synchronises
+int fetch_anchors(ob_ctx *ctx) {
+  std::vector<double> h_anchor(3 * ctx->sum_ap);
+  CU(cpy(ctx, h_anchor.data(), ctx->dev.anchor, sizeof(double) * h_anchor.size(), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  for (int w = 0; w < ctx->n_worlds; w++) {
+    const WorldDesc &d = ctx->desc[w];
+    HostWorld &H = ctx->hw[w];
+    H.anchor.resize(3 * (size_t)d.A);
+    for (int a = 0; a < d.A; a++)
+      for (int k = 0; k < 3; k++)
+        H.anchor[3 * H.int2ext_apple[a] + k] = h_anchor[3 * (size_t)d.apple_base + (size_t)k * d.Ap + a];
+  }
   return OB_OK;
 }
 
@@ -386,6 +405,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   std::vector<float> h_Lown(L.sumNp, 1.f), h_diam(L.sumNp, 1.f), h_arm(L.any_arm ? 2 * L.sumNp : 0, 0.f);
   std::vector<int32_t> h_link_ext(L.sumNp, 0), h_apple_ext(std::max<size_t>(L.sumAp, 16), 0), h_lev(L.sumLev, 0);
   std::vector<float> h_nom(2 * std::max<size_t>(L.sumAp, 16), 0.f), h_c(std::max<size_t>(L.sumAp, 16), 0.f);
+  std::vector<float> h_off0(3 * std::max<size_t>(L.sumAp, 16), 0.f);
   std::vector<int32_t> h_order(n_worlds);
   size_t link_base = 0, apple_base = 0, lev_base = 0, link_off = 0, apple_off = 0;
   for (int w = 0; w < n_worlds; w++) {
@@ -460,7 +480,7 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
     int32_t *alink = reinterpret_cast<int32_t *>(ab + apple_state_bytes(Ap) + 7 * 4 * Ap);
     for (int a = 0; a < A; a++) {
       const int e = H.int2ext_apple[a];
-      for (int k = 0; k < 3; k++) aconst[k * Ap + a] = s.apple_offset[3 * e + k];
+      for (int k = 0; k < 3; k++) h_off0[3 * apple_base + k * Ap + a] = aconst[k * Ap + a] = s.apple_offset[3 * e + k];
       aconst[3 * Ap + a] = s.apple_k[e];
       aconst[4 * Ap + a] = s.apple_mass[e];
       aconst[6 * Ap + a] = s.apple_detach[e];
@@ -502,6 +522,9 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   D.sum_np = (int32_t)L.sumNp;
   D.Lown = reinterpret_cast<float *>(base + L.Lown.off);
   D.diam = reinterpret_cast<float *>(base + L.diam.off);
+  D.Lown0 = reinterpret_cast<float *>(base + L.Lown0.off);
+  D.diam0 = reinterpret_cast<float *>(base + L.diam0.off);
+  D.apple_off0 = reinterpret_cast<float *>(base + L.apple_off0.off);
   D.arm = L.any_arm ? reinterpret_cast<float *>(base + L.arm.off) : nullptr;
   D.link_ext = reinterpret_cast<int32_t *>(base + L.link_ext.off);
   D.apple_ext = reinterpret_cast<int32_t *>(base + L.apple_ext.off);
@@ -533,13 +556,15 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
   cudaError_t e = cudaMemsetAsync(base, 0, L.total, ctx->stream);
   if (e != cudaSuccess) { g_err = cudaGetErrorString(e); delete ctx; return OB_E_CUDA; }
   UP(L.desc, ctx->desc); UP(L.order, h_order); UP(L.link_blk, h_link); UP(L.apple_blk, h_apple); UP(L.topo, h_topo); UP(L.topo2, h_topo2);
-  UP(L.quat_raw, h_quat_raw); UP(L.Lown, h_Lown); UP(L.diam, h_diam); UP(L.arm, h_arm); UP(L.link_ext, h_link_ext);
+  UP(L.quat_raw, h_quat_raw); UP(L.Lown, h_Lown); UP(L.diam, h_diam); UP(L.Lown0, h_Lown); UP(L.diam0, h_diam); UP(L.apple_off0, h_off0); UP(L.arm, h_arm); UP(L.link_ext, h_link_ext);
   UP(L.apple_ext, h_apple_ext); UP(L.apple_nom, h_nom); UP(L.apple_c, h_c); UP(L.level_off, h_lev);
 #undef UP
   e = cudaStreamSynchronize(ctx->stream);   // the host images die at the end of this call
   if (e == cudaSuccess) e = launch_rest_pose(D, 0, 0, ctx->stream);
+  if (e == cudaSuccess) e = launch_anchors(D, ctx->stream);
   if (e == cudaSuccess) e = launch_randomize(D, 0ull, 0, ctx->stream);
-  ctx->kernel_launches += 2;
+  ctx->kernel_launches += 3;
+  ctx->sum_ap = std::max<size_t>(L.sumAp, 16);
   // launch geometry of k_step
   int n_sm = 0, dev = 0;
   if (e == cudaSuccess) e = cudaGetDevice(&dev);
@@ -567,23 +592,12 @@ int ob_create(const ob_world_spec *specs, int n_worlds, const ob_params *params,
     e = cudaHostAlloc((void **)&ctx->staging[k], sizeof(WrenchSlots) * n_worlds, cudaHostAllocDefault);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->staging_ev[k], cudaEventDisableTiming);
   }
-  // anchors come back once (rest geometry never changes)
-  std::vector<double> h_anchor(3 * std::max<size_t>(L.sumAp, 16));
-  if (e == cudaSuccess)
-    e = cpy(ctx, h_anchor.data(), D.anchor, sizeof(double) * h_anchor.size(), cudaMemcpyDeviceToHost, ctx->stream);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+  // the rest hang points come back (they change only with ob_randomize_geometry)
+  if (e == cudaSuccess && fetch_anchors(ctx) != OB_OK) e = cudaErrorUnknown;
   if (e != cudaSuccess) {
     g_err = std::string("ob_create: ") + cudaGetErrorString(e);
     ob_destroy(ctx);
     return OB_E_CUDA;
-  }
-  for (int w = 0; w < n_worlds; w++) {
-    const WorldDesc &d = ctx->desc[w];
-    HostWorld &H = ctx->hw[w];
-    H.anchor.resize(3 * (size_t)d.A);
-    for (int a = 0; a < d.A; a++)
-      for (int k = 0; k < 3; k++)
-        H.anchor[3 * H.int2ext_apple[a] + k] = h_anchor[3 * (size_t)d.apple_base + (size_t)k * d.Ap + a];
   }
   *out = ctx;
   return OB_OK;
@@ -598,6 +612,52 @@ int ob_randomize(ob_ctx *ctx, uint64_t seed) {
   if (rc != OB_OK) return rc;
   CU(launch_randomize(ctx->dev, (unsigned long long)seed, 1, ctx->stream));
   ctx->kernel_launches += 1;
+  return OB_OK;
+}
+
+int ob_randomize_geometry(ob_ctx *ctx, uint64_t seed, const ob_geometry_ranges *ranges) {
+  if (!ctx) return OB_E_ARG;
+  if (!ranges) return fail(ctx, OB_E_ARG, "ranges is null");
+  const float *f = reinterpret_cast<const float *>(ranges);
+  for (int k = 0; k < 16; k++)
+    if (!std::isfinite(f[k])) return fail(ctx, OB_E_ARG, "non-finite geometry range");
+  for (int k = 8; k < 16; k++)
+    if (!(f[k] > 0.f)) return fail(ctx, OB_E_ARG, "dimension factors must be positive");
+  for (auto &wv : ctx->wrench) wv = WrenchSlots{};
+  ctx->dirty_lo = 0;
+  ctx->dirty_hi = ctx->n_worlds - 1;
+  int rc = flush_wrenches(ctx);
+  if (rc != OB_OK) return rc;
+  CU(launch_geometry(ctx->dev, (unsigned long long)seed, *ranges, ctx->stream));
+  CU(launch_anchors(ctx->dev, ctx->stream));
+  CU(launch_randomize(ctx->dev, 0ull, 2, ctx->stream));       // derived constants, reset; materials kept
+  ctx->kernel_launches += 3;
+  return fetch_anchors(ctx);
+}
+
+int ob_get_geometry(ob_ctx *ctx, int world, float *length, float *diameter, double *rest_quat, float *apple_offset) {
+  int rc = check_world(ctx, world);
+  if (rc != OB_OK) return rc;
+  const WorldDesc &d = ctx->desc[world];
+  const HostWorld &H = ctx->hw[world];
+  std::vector<float> L(d.Np), dm(d.Np), ao(3 * (size_t)std::max(d.Ap, 1));
+  std::vector<double> q(4 * (size_t)d.Np);
+  CU(cpy(ctx, L.data(), ctx->dev.Lown + d.link_base, sizeof(float) * d.Np, cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cpy(ctx, dm.data(), ctx->dev.diam + d.link_base, sizeof(float) * d.Np, cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cpy(ctx, q.data(), ctx->dev.quatd + 4 * (size_t)d.link_base, sizeof(double) * 4 * d.Np, cudaMemcpyDeviceToHost, ctx->stream));
+  if (d.Ap)
+    CU(cpy(ctx, ao.data(), ctx->dev.apple_blk + d.apple_blk_off + apple_state_bytes(d.Ap), sizeof(float) * 3 * d.Ap,
+           cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  for (int i = 0; i < d.N; i++) {
+    const int e = H.int2ext_link[i];
+    if (length) length[e] = L[i];
+    if (diameter) diameter[e] = dm[i];
+    if (rest_quat) for (int k = 0; k < 4; k++) rest_quat[4 * e + k] = q[4 * (size_t)i + k];
+  }
+  if (apple_offset)
+    for (int a = 0; a < d.A; a++)
+      for (int k = 0; k < 3; k++) apple_offset[3 * H.int2ext_apple[a] + k] = ao[(size_t)k * d.Ap + a];
   return OB_OK;
 }
 
@@ -1092,6 +1152,7 @@ int ob_counters(ob_ctx *ctx, uint64_t out[4]) {
 int ob_sizeof_params(void) { return (int)sizeof(ob_params); }
 int ob_sizeof_world_spec(void) { return (int)sizeof(ob_world_spec); }
 int ob_sizeof_event(void) { return (int)sizeof(ob_event); }
+int ob_sizeof_geometry_ranges(void) { return (int)sizeof(ob_geometry_ranges); }
 
 int ob_selftest_philox(int n, const uint32_t *ctr, const uint32_t *key, uint32_t *out_lib, uint32_t *out_curand,
                        void *dev_scratch, void *cuda_stream) {

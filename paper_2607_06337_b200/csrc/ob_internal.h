@@ -85,8 +85,10 @@ struct DevCtx {
   float *Mmax;                   // rupture moment (after randomize)
   float2 *xprev;                 // [4][sumNp]: dqd of the last four steps, slot = step & 3 (PCG start: extrapolation)
   int32_t sum_np;                // stride of xprev
-  const float *Lown;             // link length
-  const float *diam;             // link diameter
+  float *Lown;                   // link length (current: ob_randomize_geometry rewrites it from Lown0)
+  float *diam;                   // link diameter
+  const float *Lown0, *diam0;    // base geometry as given to ob_create
+  const float *apple_off0;       // [3 * apple_base + k * Ap + a] base attach points
   const float *arm;              // [2 * link_base + k * Np + i] armature or nullptr
   const int32_t *link_ext;       // internal -> caller's link index
   const int32_t *apple_ext;      // internal -> caller's apple index
@@ -163,6 +165,8 @@ cudaError_t launch_step(const DevCtx &c, int cls, const int32_t *order, int n_in
                         int grid, int smem, int n_sm, int n_chunks, int32_t *progress, cudaStream_t s);
 cudaError_t launch_pose(const DevCtx &c, int world, cudaStream_t s);
 cudaError_t launch_stats(const DevCtx &c, cudaStream_t s);
+cudaError_t launch_geometry(const DevCtx &c, unsigned long long seed, const ob_geometry_ranges &r, cudaStream_t s);
+cudaError_t launch_anchors(const DevCtx &c, cudaStream_t s);
 cudaError_t launch_philox_selftest(int n, const uint32_t *d_in, uint32_t *d_out, cudaStream_t s);
 cudaError_t step_kernel_setup(int cls, int smem_bytes, int *max_blocks_per_sm);
 

@@ -38,51 +38,160 @@ __device__ __forceinline__ float philox_uniform(uint32_t x, float lo, float hi) 
 
 // ------------------------------------------------------------------------------------------------------
 // k_rest_pose: one CTA per world.  The rest quaternion of every link normalised in fp64 (the FK of k_step starts from
-// it) and anchor_a = p0_b + R0_b o of every apple by walking up the ancestors in fp64 (create-time only; Eq. 3,
-// PAPER.md:115).
+// it); once per ob_create.  k_anchors: anchor_a = p0_b + R0_b o of every apple by walking up the ancestors in fp64 with
+// the CURRENT rest quaternions, lengths and attach points (Eq. 3); after ob_create and after
+// ob_randomize_geometry.
 // ------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void quat_to_mat_d(float4 q, double *R) {   // normalises in fp64
-  double w = q.x, x = q.y, y = q.z, z = q.w;
-  const double n = sqrt(w * w + x * x + y * y + z * z);
-  w /= n; x /= n; y /= n; z /= n;
-  R[0] = 1 - 2 * (y * y + z * z); R[1] = 2 * (x * y - w * z);     R[2] = 2 * (x * z + w * y);
-  R[3] = 2 * (x * y + w * z);     R[4] = 1 - 2 * (x * x + z * z); R[5] = 2 * (y * z - w * x);
-  R[6] = 2 * (x * z - w * y);     R[7] = 2 * (y * z + w * x);     R[8] = 1 - 2 * (x * x + y * y);
+struct Qd4 { double w, x, y, z; };
+__device__ __forceinline__ Qd4 qmul4(const Qd4 a, const Qd4 b) {
+  Qd4 r;
+  r.w = a.w * b.w - a.x * b.x - a.y * b.y - a.z * b.z;
+  r.x = a.w * b.x + a.x * b.w + a.y * b.z - a.z * b.y;
+  r.y = a.w * b.y - a.x * b.z + a.y * b.w + a.z * b.x;
+  r.z = a.w * b.z + a.x * b.y - a.y * b.x + a.z * b.w;
+  return r;
+}
+__device__ __forceinline__ void qrot4(const Qd4 q, const double v[3], double out[3]) {   // R(q) v
+  const double tx = 2 * (q.y * v[2] - q.z * v[1]), ty = 2 * (q.z * v[0] - q.x * v[2]), tz = 2 * (q.x * v[1] - q.y * v[0]);
+  out[0] = v[0] + q.w * tx + (q.y * tz - q.z * ty);
+  out[1] = v[1] + q.w * ty + (q.z * tx - q.x * tz);
+  out[2] = v[2] + q.w * tz + (q.x * ty - q.y * tx);
+}
+__device__ __forceinline__ Qd4 load_q4(const double *quatd, size_t i) {
+  Qd4 q;
+  q.w = quatd[4 * i]; q.x = quatd[4 * i + 1]; q.y = quatd[4 * i + 2]; q.z = quatd[4 * i + 3];
+  return q;
 }
 
 __global__ void k_rest_pose(DevCtx c) {
   const WorldDesc d = c.desc[blockIdx.x];
-  const int4 *topo = c.topo + d.link_base;
   const float4 *quat = c.quat_raw + d.link_base;   // the caller's quaternions, normalised in fp64 here
-  const float *Lown = c.Lown + d.link_base;
   for (int i = threadIdx.x; i < d.N; i += blockDim.x) {
-    {                                           // the link's own rest quaternion, normalised in fp64, for the FK of k_step
-      const float4 q = quat[i];
-      const double w = q.x, x = q.y, y = q.z, z = q.w, n = sqrt(w * w + x * x + y * y + z * z);
-      double *qd = c.quatd + 4 * ((size_t)d.link_base + i);
-      qd[0] = w / n; qd[1] = x / n; qd[2] = y / n; qd[3] = z / n;
-    }
+    const float4 q = quat[i];
+    const double w = q.x, x = q.y, y = q.z, z = q.w, n = sqrt(w * w + x * x + y * y + z * z);
+    double *qd = c.quatd + 4 * ((size_t)d.link_base + i);
+    qd[0] = w / n; qd[1] = x / n; qd[2] = y / n; qd[3] = z / n;
   }
+}
+
+__global__ void k_anchors(DevCtx c) {
+  const WorldDesc d = c.desc[blockIdx.x];
+  const int4 *topo = c.topo + d.link_base;
+  const float *Lown = c.Lown + d.link_base;
   const unsigned char *ab = c.apple_blk + d.apple_blk_off;
   const float *ao = reinterpret_cast<const float *>(ab + apple_state_bytes(d.Ap));
   const int32_t *alink = reinterpret_cast<const int32_t *>(ab + apple_state_bytes(d.Ap) + 7 * 4 * d.Ap);
   for (int a = threadIdx.x; a < d.A; a += blockDim.x) {
     double x[3] = {ao[a], ao[d.Ap + a], ao[2 * d.Ap + a]};
     for (int j = alink[a]; j >= 0; j = topo[j].x) {
-      double Q[9];
-      quat_to_mat_d(quat[j], Q);
-      double y0 = Q[0] * x[0] + Q[1] * x[1] + Q[2] * x[2];
-      double y1 = Q[3] * x[0] + Q[4] * x[1] + Q[5] * x[2];
-      double y2 = Q[6] * x[0] + Q[7] * x[1] + Q[8] * x[2];
-      int pa = topo[j].x;
-      x[0] = y0; x[1] = y1; x[2] = y2 + (pa >= 0 ? (double)Lown[pa] : 0.0);
+      double y[3];
+      qrot4(load_q4(c.quatd, (size_t)d.link_base + j), x, y);
+      const int pa = topo[j].x;
+      x[0] = y[0]; x[1] = y[1]; x[2] = y[2] + (pa >= 0 ? (double)Lown[pa] : 0.0);
     }
     for (int k = 0; k < 3; k++) c.anchor[3 * (size_t)d.apple_base + (size_t)k * d.Ap + a] = x[k];
   }
 }
 
 // ------------------------------------------------------------------------------------------------------
-// k_randomize: one CTA per world.  redraw = 0 keeps the current material (used by ob_create).
+// k_randomize_geometry: ONE THREAD PER WORLD ("an on-device build that perturbs every world's branch
+// geometry in a single ... kernel (one thread per world)"): per-world growth habit and dimensions drawn with
+// Philox4x32-10 and applied to the base geometry in a top-down re-walk (reading A37 in DESIGN.md;
+// the readings are spelled out at ob_randomize_geometry in include/orchard.h).  Quaternion algebra in fp64; the world
+// rest quaternion of every link (needed by its children while the droop compounds) is parked in the world's slice of the
+// PCG history pool, which the reset that follows clears anyway.
+// ------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ Qd4 axis_angle_xy(const double ax, const double ay, const double angle) {   // axis (ax, ay, 0)
+  double sn, cs;
+  sincos(0.5 * angle, &sn, &cs);
+  Qd4 q;
+  q.w = cs; q.x = ax * sn; q.y = ay * sn; q.z = 0.0;
+  return q;
+}
+
+__global__ void k_randomize_geometry(DevCtx c, unsigned long long seed, ob_geometry_ranges G) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= c.n_worlds) return;
+  const WorldDesc d = c.desc[w];
+  const uint2 key = make_uint2((uint32_t)(seed & 0xffffffffull), (uint32_t)(seed >> 32));
+  const uint4 o0 = philox4x32_10(make_uint4((uint32_t)w, 0u, 3u, 0u), key);
+  const uint4 o1 = philox4x32_10(make_uint4((uint32_t)w, 1u, 3u, 0u), key);
+  const float droop = philox_uniform(o0.x, G.droop[0], G.droop[1]);
+  const float lean = philox_uniform(o0.y, G.lean[0], G.lean[1]);
+  const float spread = philox_uniform(o0.z, G.spread[0], G.spread[1]);
+  const float twist = philox_uniform(o0.w, G.twist[0], G.twist[1]);
+  const float phi = philox_uniform(o1.x, 0.0f, 6.2831855f);
+  const float sL = philox_uniform(o1.y, G.scale_length[0], G.scale_length[1]);
+  const float sD = philox_uniform(o1.z, G.scale_diameter[0], G.scale_diameter[1]);
+  const int4 *topo = c.topo + d.link_base;
+  const float4 *quat0 = c.quat_raw + d.link_base;
+  double *park[4];                                     // world rest quaternion of link i: component k at park[k][i]
+  for (int k = 0; k < 4; k++) park[k] = reinterpret_cast<double *>(c.xprev + (size_t)k * c.sum_np + d.link_base);
+  for (int i = 0; i < d.N; i++) {
+    // dimensions: L = (L0 * scale) * jitter in fp32, the jitter drawn by the CALLER's link index
+    const uint4 oi = philox4x32_10(make_uint4((uint32_t)w, (uint32_t)c.link_ext[d.link_base + i], 4u, 0u), key);
+    const float jl = philox_uniform(oi.x, G.jitter_length[0], G.jitter_length[1]);
+    const float jd = philox_uniform(oi.y, G.jitter_diameter[0], G.jitter_diameter[1]);
+    c.Lown[d.link_base + i] = __fmul_rn(__fmul_rn(c.Lown0[d.link_base + i], sL), jl);
+    c.diam[d.link_base + i] = __fmul_rn(__fmul_rn(c.diam0[d.link_base + i], sD), jd);
+    // rest rotation: spread and twist of a child about its parent's axis, lean of the trunk
+    const float4 qf = quat0[i];
+    Qd4 q;
+    {
+      const double nn = sqrt((double)qf.x * qf.x + (double)qf.y * qf.y + (double)qf.z * qf.z + (double)qf.w * qf.w);
+      q.w = qf.x / nn; q.x = qf.y / nn; q.y = qf.z / nn; q.z = qf.w / nn;
+    }
+    const int pa = topo[i].x;
+    if (pa >= 0) {
+      // direction of the child's axis in the parent frame: R(q) z
+      const double dx = 2 * (q.x * q.z + q.w * q.y), dy = 2 * (q.y * q.z - q.w * q.x), dz = 1 - 2 * (q.x * q.x + q.y * q.y);
+      const double hn = sqrt(dx * dx + dy * dy);
+      if (hn > 1e-12 && spread != 0.f) q = qmul4(axis_angle_xy(-dy / hn, dx / hn, atan2(hn, dz) * (double)spread), q);
+      if (twist != 0.f) {
+        double sn, cs;
+        sincos(0.5 * (double)twist, &sn, &cs);
+        Qd4 t;
+        t.w = cs; t.x = 0.0; t.y = 0.0; t.z = sn;
+        q = qmul4(t, q);
+      }
+    } else if (lean != 0.f) {
+      q = qmul4(axis_angle_xy(cos((double)phi), sin((double)phi), (double)lean), q);
+    }
+    double *out = c.quatd + 4 * ((size_t)d.link_base + i);
+    if (droop == 0.f) {                               // no re-walk: the modified rest rotation is the result, exactly
+      out[0] = q.w; out[1] = q.x; out[2] = q.y; out[3] = q.z;
+      continue;
+    }
+    Qd4 qp;
+    qp.w = 1.0; qp.x = 0.0; qp.y = 0.0; qp.z = 0.0;
+    if (pa >= 0) { qp.w = park[0][pa]; qp.x = park[1][pa]; qp.y = park[2][pa]; qp.z = park[3][pa]; }
+    Qd4 qi = qmul4(qp, q);
+    {
+      const double dx = 2 * (qi.x * qi.z + qi.w * qi.y), dy = 2 * (qi.y * qi.z - qi.w * qi.x);
+      const double sn = sqrt(dx * dx + dy * dy);      // sine of the angle to the vertical
+      if (sn > 1e-12) qi = qmul4(axis_angle_xy(-dy / sn, dx / sn, (double)droop * sn), qi);   // towards the ground
+    }
+    park[0][i] = qi.w; park[1][i] = qi.x; park[2][i] = qi.y; park[3][i] = qi.z;
+    Qd4 qc;
+    qc.w = qp.w; qc.x = -qp.x; qc.y = -qp.y; qc.z = -qp.z;
+    const Qd4 qn = qmul4(qc, qi);                      // the new rest rotation in the (turned) parent frame
+    out[0] = qn.w; out[1] = qn.x; out[2] = qn.y; out[3] = qn.z;
+  }
+  // attach points move with their link: x, y by its diameter factor, z by its length factor
+  unsigned char *ab = c.apple_blk + d.apple_blk_off;
+  float *ao = reinterpret_cast<float *>(ab + apple_state_bytes(d.Ap));
+  const int32_t *alink = reinterpret_cast<const int32_t *>(ab + apple_state_bytes(d.Ap) + 7 * 4 * d.Ap);
+  const float *ao0 = c.apple_off0 + 3 * (size_t)d.apple_base;
+  for (int a = 0; a < d.A; a++) {
+    const int b = d.link_base + alink[a];
+    const float fl = __fdiv_rn(c.Lown[b], c.Lown0[b]), fd = __fdiv_rn(c.diam[b], c.diam0[b]);
+    ao[a] = __fmul_rn(ao0[a], fd); ao[d.Ap + a] = __fmul_rn(ao0[d.Ap + a], fd); ao[2 * d.Ap + a] = __fmul_rn(ao0[2 * d.Ap + a], fl);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------
+// k_randomize: one CTA per world.  redraw = 0: nominal materials of the specs (ob_create); 1: Philox draws; 2: keep the
+// current materials (after ob_randomize_geometry).  Always: derived constants from the current dimensions, full reset.
 // ------------------------------------------------------------------------------------------------------
 __global__ void k_randomize(DevCtx c, unsigned long long seed, int redraw) {
   const int w = blockIdx.x;
@@ -91,7 +200,9 @@ __global__ void k_randomize(DevCtx c, unsigned long long seed, int redraw) {
   WorldInfo *info = c.info + w;
   const uint2 key = make_uint2((uint32_t)(seed & 0xffffffffull), (uint32_t)(seed >> 32));
   float E = d.E, MOR = d.MOR, rho = d.density;
-  if (redraw) {
+  if (redraw == 2) {                                   // keep the materials as they are (after ob_randomize_geometry)
+    E = info->E; MOR = info->MOR; rho = info->density;
+  } else if (redraw) {
     uint4 o = philox4x32_10(make_uint4((uint32_t)w, 0u, 0u, 0u), key);
     if (P.range_E[0] != P.range_E[1]) E = philox_uniform(o.x, P.range_E[0], P.range_E[1]);
     if (P.range_MOR[0] != P.range_MOR[1]) MOR = philox_uniform(o.y, P.range_MOR[0], P.range_MOR[1]);
@@ -141,7 +252,7 @@ __global__ void k_randomize(DevCtx c, unsigned long long seed, int redraw) {
     af[a] = a < d.A ? 1 : 0; af[d.Ap + a] = 0; af[2 * d.Ap + a] = 0;
     if (a < d.A) {
       float m, fd;
-      if (redraw) {
+      if (redraw == 1) {
         // the counter item is the CALLER's apple index (the internal order is a private matter)
         uint4 o = philox4x32_10(make_uint4((uint32_t)w, (uint32_t)aext[a], 1u, 0u), key);
         fd = P.range_detach[0] != P.range_detach[1] ? philox_uniform(o.x, P.range_detach[0], P.range_detach[1])
@@ -171,14 +282,19 @@ __global__ void k_randomize(DevCtx c, unsigned long long seed, int redraw) {
 __global__ void k_pose(DevCtx c, int w) {
   const WorldDesc d = c.desc[w];
   const int4 *topo = c.topo + d.link_base;
-  const float4 *quat = c.quat_raw + d.link_base;
   const float *Lown = c.Lown + d.link_base;
   const float *st = reinterpret_cast<const float *>(c.link_blk + d.link_blk_off);
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < d.N; i += gridDim.x * blockDim.x) {
     double R[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1}, x[3] = {0, 0, 0};
     for (int j = i; j >= 0; j = topo[j].x) {
       double Q[9], T[9], A[9];
-      quat_to_mat_d(quat[j], Q);
+      {
+        const Qd4 q = load_q4(c.quatd, (size_t)d.link_base + j);
+        const double w = q.w, x = q.x, y = q.y, z = q.z;
+        Q[0] = 1 - 2 * (y * y + z * z); Q[1] = 2 * (x * y - w * z);     Q[2] = 2 * (x * z + w * y);
+        Q[3] = 2 * (x * y + w * z);     Q[4] = 1 - 2 * (x * x + z * z); Q[5] = 2 * (y * z - w * x);
+        Q[6] = 2 * (x * z - w * y);     Q[7] = 2 * (y * z + w * x);     Q[8] = 1 - 2 * (x * x + y * y);
+      }
       double s1, c1, s2, c2;
       sincos((double)st[2 * j], &s1, &c1);
       sincos((double)st[2 * j + 1], &s2, &c2);
@@ -217,6 +333,14 @@ __global__ void k_pose(DevCtx c, int w) {
 // ------------------------------------------------------------------------------------------------------
 cudaError_t launch_rest_pose(const DevCtx &c, int, int, cudaStream_t s) {
   k_rest_pose<<<c.n_worlds, 128, 0, s>>>(c);
+  return cudaGetLastError();
+}
+cudaError_t launch_anchors(const DevCtx &c, cudaStream_t s) {
+  k_anchors<<<c.n_worlds, 128, 0, s>>>(c);
+  return cudaGetLastError();
+}
+cudaError_t launch_geometry(const DevCtx &c, unsigned long long seed, const ob_geometry_ranges &r, cudaStream_t s) {
+  k_randomize_geometry<<<(c.n_worlds + 63) / 64, 64, 0, s>>>(c, seed, r);
   return cudaGetLastError();
 }
 cudaError_t launch_randomize(const DevCtx &c, unsigned long long seed, int redraw, cudaStream_t s) {

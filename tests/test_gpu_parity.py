@@ -890,3 +890,74 @@ def test_saturation_batch_16384_worlds_invariants_and_sampled_parity():
         if not gev.get(w):
             assert e["max"] <= TOL_RUN, (w, e)
     sim.close()
+
+
+# ----------------------------------------------------------------------------------------------------
+# per-world geometry randomization on the device (reading A37)
+# ----------------------------------------------------------------------------------------------------
+GEO = dict(droop=(0.0, 0.12), lean=(0.0, 0.15), spread=(-0.2, 0.3), twist=(-0.5, 0.5), scale_length=(0.85, 1.2),
+           scale_diameter=(0.8, 1.25), jitter_length=(0.9, 1.1), jitter_diameter=(0.9, 1.1))
+
+
+def test_geometry_randomization_identity_reproduces_the_base_model_exactly():
+    """the on-device build "reproduces the replicated base model exactly at zero strength"."""
+    specs = list(_stochastic(301, 150, 250, 20, 3))
+    P = config_params(2)
+    a, b = ob.Orchard(specs, P), ob.Orchard(specs, P)
+    for sim in (a, b):
+        sim.randomize(11)
+    b.randomize_geometry(999)                                  # identity ranges
+    for w in range(len(specs)):
+        ga, gb = a.get_geometry(w), b.get_geometry(w)
+        for k in ga:
+            assert ga[k].tobytes() == gb[k].tobytes(), (w, k)
+        assert a.get_material(w)["mass"].tobytes() == b.get_material(w)["mass"].tobytes()
+    loads = wrench_process(specs, 0, 0.0, 100.0)
+    for sim in (a, b):
+        for (w, body, pt, f) in loads:
+            sim.apply_wrench(w, body, pt, f)
+        sim.step(30)
+    sa, sb = a.get_state_batch(), b.get_state_batch()
+    for k in sa:
+        assert sa[k].tobytes() == sb[k].tobytes(), k
+    a.close(); b.close()
+
+
+def test_geometry_randomization_matches_the_oracle():
+    """Every world of the batch gets its own growth habit and dimensions: geometry, rest pose and derived constants
+    against the oracle (dimensions and attach points bit-exact, rest rotations to fp64 rounding), then single steps
+    from a moving state and the event sets of a short run."""
+    specs = list(_stochastic(302, 150, 250, 20, 4)) + [binary_tree_config1()]
+    P = config_params(2)
+    sim, refs = _make(specs, P, seed=MASTER_SEED + 7)
+    gseed = (5 << 32) | 12345
+    sim.randomize_geometry(gseed, **GEO)
+    for r in refs:
+        r.randomize_geometry(gseed, **GEO)
+        r._x_rest = r.get_state()["apple_x"].copy()
+    from scipy.spatial.transform import Rotation
+    for w, r in enumerate(refs):
+        g, o = sim.get_geometry(w), r.geometry()
+        assert g["length"].tobytes() == o["length"].astype(np.float32).tobytes()
+        assert g["diameter"].tobytes() == o["diameter"].astype(np.float32).tobytes()
+        assert g["apple_offset"].tobytes() == o["apple_offset"].astype(np.float32).tobytes()
+        q = g["rest_quat"]
+        Rg = Rotation.from_quat(np.stack([q[:, 1], q[:, 2], q[:, 3], q[:, 0]], axis=1)).as_matrix()
+        assert np.abs(Rg - o["Q"]).max() < 1e-12, w
+        assert np.abs(g["length"] / specs[w].length - 1).max() > 0.05       # the geometry did change
+        m, om = sim.get_material(w), r.material()                            # ... and the materials did not
+        assert np.float32(m["E"]).tobytes() == np.float32(om["E"]).tobytes() and m["mass"].tobytes() == om["mass"].astype(np.float32).tobytes()
+        st, so = sim.get_state(w, pose=True), r.get_state()
+        assert np.abs(st["apple_x64"] - so["apple_x"]).max() < 1e-9
+        R, p, _, _ = r.fk()
+        assert np.abs(st["link_pose7"][:, :3] - p).max() < 1e-6 and st["step"] == 0 and not st["q"].any()
+    worst = 0.0
+    for epoch in range(2):
+        _apply(sim, refs, wrench_process(specs, epoch, 0.0, 80.0))
+        sim.step(20)
+        for w, e in _single_step_errors(sim, refs, range(len(specs))).items():
+            assert e["max"] <= TOL_STEP, (epoch, w, e)
+            worst = max(worst, e["max"])
+        sim.step(9)
+    print(f"geometry DR: single-step worst relative error {worst:.2e}")
+    sim.close()
