@@ -29,6 +29,10 @@ if ROOT not in sys.path:
 
 import numpy as np  # noqa: E402
 
+# ranges of --geometry-dr (growth habit and per-branch dimensions, distinct in every world)
+GEOMETRY_DR_RANGES = dict(droop=(0.0, 0.10), lean=(0.0, 0.12), spread=(-0.15, 0.25), twist=(-0.4, 0.4),
+                          scale_length=(0.85, 1.15), scale_diameter=(0.85, 1.2), jitter_length=(0.9, 1.1),
+                          jitter_diameter=(0.9, 1.1))
 METRIC = "world-steps/s at 4096 trees x ~400 links"
 UNIT = "world-steps/s"
 
@@ -191,6 +195,8 @@ def run_cuda(args, rank: int, world_size: int):
     def run(e2e: bool, with_state: bool = False):
         sim = ob.Orchard(specs, P)
         sim.randomize(seed)
+        if args.geometry_dr:                               # distinct growth habit and dimensions in every world
+            sim.randomize_geometry(seed + 9, **GEOMETRY_DR_RANGES)
         stream = sim.stream
         state = None
         for e in range(args.warmup):
@@ -293,6 +299,8 @@ def run_cuda(args, rank: int, world_size: int):
                                    f"wrench U({f_lo:g},{f_hi:g}) N per world resampled every {S} steps",
                        "worlds_per_gpu": W, "physics_steps_per_bench_step": S, "links_total": n_links,
                        "apples_total": n_apples, "cg_tol": P.cg_tol, "replicas": world_size,
+                       "geometry": "ob_randomize_geometry: distinct growth habit and dimensions per world"
+                                   if args.geometry_dr else "as generated (every world its own tree)",
                        "l2": f"inputs exceed L2: workspace {dev['workspace'] / 2**20:.0f} MiB vs 126 MB L2",
                        "launch": dev["launch"]},
             "kernel_only": {"value": ws_dev / (kern_total_ms * 1e-3), "unit": UNIT,
@@ -475,6 +483,8 @@ def main():
     ap.add_argument("--worlds", type=int, default=4096)
     ap.add_argument("--substeps", type=int, default=50, help="physics steps per bench step (one wrench epoch)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--geometry-dr", action="store_true",
+                    help="per-world geometry randomization on the device before the run (SURVEY.md 8(f) item 3)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3                                    # timing rule: at least 3 warm-up steps
