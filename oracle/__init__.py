@@ -36,6 +36,8 @@ class OboParams(C.Structure):
         ("detach_frames_tension", C.c_int32), ("tether_implicit", C.c_int32),
         ("react_max", C.c_double), ("qd_max", C.c_double), ("zeta_s", C.c_double), ("alpha_m", C.c_double),
         ("forces_off_on_snapped", C.c_int32), ("pad_", C.c_int32),
+        ("fric_frac", C.c_double), ("fric_ramp", C.c_double), ("fric_time", C.c_double), ("fric_veps", C.c_double),
+        ("snap_drag_scale", C.c_double), ("rail_speed", C.c_double), ("rail_fade", C.c_double), ("rail_brake", C.c_double),
         ("range_E", C.c_float * 2), ("range_MOR", C.c_float * 2), ("range_density", C.c_float * 2),
         ("range_detach", C.c_float * 2), ("range_apple_mass", C.c_float * 2),
     ]
@@ -81,6 +83,8 @@ def lib():
         L.obo_get_counters.argtypes = [C.c_void_p] + [C.c_void_p] * 3
         L.obo_set_counters.argtypes = [C.c_void_p] + [C.c_void_p] * 3
         L.obo_set_step.argtypes = [C.c_void_p, C.c_int]
+        L.obo_get_rupture_steps.argtypes = [C.c_void_p, C.c_void_p]
+        L.obo_set_rupture_steps.argtypes = [C.c_void_p, C.c_void_p]
         L.obo_set_solver.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_int]
         L.obo_events.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.obo_events.restype = C.c_int
@@ -128,6 +132,8 @@ def _params_struct(p, solver: int = 0) -> OboParams:
     s.zeta_s = float(np.float32(p.zeta_s))
     s.alpha_m = float(np.float32(getattr(p, "mass_damping", 0.0)))
     s.forces_off_on_snapped = p.forces_off_on_snapped
+    for name in ("fric_frac", "fric_ramp", "fric_time", "fric_veps", "snap_drag_scale", "rail_speed", "rail_fade", "rail_brake"):
+        setattr(s, name, float(np.float32(getattr(p, name))))
     s.h = float(np.float32(p.h))
     for name in ("range_E", "range_MOR", "range_density", "range_detach", "range_apple_mass"):
         setattr(s, name, (C.c_float * 2)(*getattr(p, name)))
@@ -225,6 +231,15 @@ class OracleWorld:
 
     def set_step(self, step: int):
         lib().obo_set_step(self.h, step)
+
+    def get_rupture_steps(self):
+        r = np.zeros(self.N, dtype=np.int32)
+        lib().obo_get_rupture_steps(self.h, r.ctypes.data)
+        return r
+
+    def set_rupture_steps(self, rstep):
+        r = np.ascontiguousarray(rstep, dtype=np.int32)
+        lib().obo_set_rupture_steps(self.h, r.ctypes.data)
 
     def set_solver(self, solver: int, tol: float = 1e-12, max_iter: int = 10000):
         lib().obo_set_solver(self.h, solver, tol, max_iter)

@@ -60,6 +60,10 @@ typedef struct {
   double alpha_m;               /* mass- and inertia-proportional damping c_v = c_omega, 1/s (A32) */
   int32_t forces_off_on_snapped;
   int32_t pad_;
+  /* post-rupture dissipation (readings A34, A35) and the three force rails (A36) */
+  double fric_frac, fric_ramp, fric_time, fric_veps;   /* friction torque fric_frac * M_max, ramped x fric_ramp over fric_time */
+  double snap_drag_scale;                             /* factor on alpha_m for links of snapped sub-trees */
+  double rail_speed, rail_fade, rail_brake;           /* speed limit (0 = rails off), fade onset fraction, brake rate 1/s */
   float range_E[2], range_MOR[2], range_density[2], range_detach[2], range_apple_mass[2];
 } obo_params;
 
@@ -90,6 +94,7 @@ typedef struct {
   double *q, *qd, *dqd_prev, *ax, *av;
   uint8_t *ruptured, *attached;
   int *rc, *cA, *cB;
+  int *rstep;                   /* step during which the joint ruptured (valid where ruptured) */
   int step, status, last_iters;
   long long cg_iters_total;
   /* wrenches (persistent) */
@@ -439,6 +444,7 @@ static void reset_state(obo_world *W) {
   memset(W->dqd_prev, 0, sizeof(double) * 2 * N);
   memset(W->ruptured, 0, (size_t)N);
   memset(W->rc, 0, sizeof(int) * N);
+  memset(W->rstep, 0, sizeof(int) * N);
   memset(W->cA, 0, sizeof(int) * A);
   memset(W->cB, 0, sizeof(int) * A);
   for (int s = 0; s < OBO_MAX_WRENCH; s++) W->wr_body[s] = -1;
@@ -521,6 +527,7 @@ obo_world *obo_world_new(int world_index, int n_links, const int32_t *parent, co
   W->ruptured = (uint8_t *)calloc((size_t)N, 1);
   W->attached = (uint8_t *)calloc((size_t)A + 1, 1);
   W->rc = (int *)calloc((size_t)N, sizeof(int));
+  W->rstep = (int *)calloc((size_t)N, sizeof(int));
   W->cA = (int *)calloc((size_t)A + 1, sizeof(int));
   W->cB = (int *)calloc((size_t)A + 1, sizeof(int));
   W->ev = NULL; W->n_ev = 0; W->cap_ev = 0;
@@ -537,7 +544,7 @@ void obo_world_free(obo_world *W) {
   free(W->alink); free(W->aoff); free(W->am_nom); free(W->adet_nom); free(W->ac_in);
   free(W->am); free(W->ak); free(W->ac); free(W->adet);
   free(W->q); free(W->qd); free(W->dqd_prev); free(W->ax); free(W->av);
-  free(W->ruptured); free(W->attached); free(W->rc); free(W->cA); free(W->cB);
+  free(W->ruptured); free(W->attached); free(W->rc); free(W->cA); free(W->cB); free(W->rstep);
   free(W->ev);
   free(W);
 }
@@ -722,12 +729,13 @@ static void push_event(obo_world *W, int kind, int index, double value, double t
 typedef struct {
   double *A, *b;        /* n x n, n */
   double *fteth;        /* [3A] tether force on each apple (Eq. 6)       */
-  double *fuser;        /* [3A] user wrench on each apple                */
+  double *fuser;        /* [3A] user wrench on each apple, after the rails */
+  double *fuser_raw;    /* [3A] ... as applied                           */
   double *fs_norm;      /* [A]  |f_s|                                    */
   double *fu_norm;      /* [A]  |f_user|                                 */
 } system_t;
 
-static void system_free(system_t *S) { free(S->A); free(S->b); free(S->fteth); free(S->fuser); free(S->fs_norm); free(S->fu_norm); }
+static void system_free(system_t *S) { free(S->A); free(S->b); free(S->fteth); free(S->fuser); free(S->fuser_raw); free(S->fs_norm); free(S->fu_norm); }
 
 /* link velocity of a world point x attached to link b:  v = v_joint(b) + om_b x (x - p_b).
    Computed from the joint-rate Jacobian: v = sum_{j in path(b)} (ax_j qd_j) x (x - p_j). */
@@ -744,6 +752,51 @@ static void point_velocity(const obo_world *W, const fk_t *f, const double *qd, 
   }
 }
 
+/* Coulomb friction at a ruptured joint ("Coulomb friction is introduced at the break and ramped up ~5x
+   over ~1.5 s as the torn fibres seize"), reading A34: torque of magnitude
+     T_f(t) = fric_frac * M_max,i * (1 + (fric_ramp - 1) min(t / fric_time, 1)),   t = h (step - step of rupture),
+   against the joint velocity (both DoF together, like |theta| in Eq. 5); for the linearly implicit step it is taken as
+   the damper D_f = T_f / max(|qd_i|, fric_veps) at the start-of-step speed, which joins D = c_d K in the matrix and
+   in the right-hand side.  Returns D_f (0 for an intact joint or fric_frac = 0). */
+static double friction_damper(const obo_world *W, int i) {
+  const obo_params *P = &W->P;
+  if (!W->ruptured[i] || P->fric_frac <= 0.0) return 0.0;
+  double t = P->h * (double)(W->step - W->rstep[i]);
+  double ramp = P->fric_time > 0.0 ? (t < P->fric_time ? t / P->fric_time : 1.0) : 1.0;
+  double Tf = P->fric_frac * W->Mmax[i] * (1.0 + (P->fric_ramp - 1.0) * ramp);
+  double w = sqrt(W->qd[2 * i] * W->qd[2 * i] + W->qd[2 * i + 1] * W->qd[2 * i + 1]);
+  return Tf / (w > P->fric_veps ? w : P->fric_veps);
+}
+
+/* The three rails of PAPER.md:398 (App. B) on an applied force F acting on a FREE body of mass m that moves with
+   velocity v at the application point (reading A36; connected links are static loading, which the rails never touch):
+     (2) power fade: the part of F along v (if it pushes along v) is scaled by clamp((v_lim - |v|) / (v_lim - v_f), 0, 1),
+         v_f = rail_fade v_lim;
+     (1) impulse cap: |F| <= m max(v_lim - v . F^, 0) / h -- the force may not take the body past v_lim in one step;
+     (3) speed brake: above v_lim an extra force - rail_brake m (|v| - v_lim) v^.
+   rail_speed = 0 switches all three off. */
+static void apply_rails(const obo_params *P, double m, const double v[3], double F[3]) {
+  double vl = P->rail_speed;
+  if (!(vl > 0.0)) return;
+  double vn = norm3(v);
+  if (vn > 0.0) {
+    double vh[3] = {v[0] / vn, v[1] / vn, v[2] / vn};
+    double Fp = dot3(F, vh);
+    if (Fp > 0.0) {
+      double vf = P->rail_fade * vl;
+      double fade = vn <= vf ? 1.0 : (vn >= vl ? 0.0 : (vl - vn) / (vl - vf));
+      for (int k = 0; k < 3; k++) F[k] -= (1.0 - fade) * Fp * vh[k];
+    }
+  }
+  double Fn = norm3(F);
+  if (Fn > 0.0) {
+    double vF = dot3(v, F) / Fn;
+    double cap = m * (vl - vF > 0.0 ? vl - vF : 0.0) / P->h;
+    if (Fn > cap) for (int k = 0; k < 3; k++) F[k] *= cap / Fn;
+  }
+  if (vn > vl) for (int k = 0; k < 3; k++) F[k] -= P->rail_brake * m * (vn - vl) * v[k] / vn;
+}
+
 static void build_system(const obo_world *W, system_t *S) {
   int N = W->N, A = W->A, n = 2 * N;
   const obo_params *P = &W->P;
@@ -752,6 +805,7 @@ static void build_system(const obo_world *W, system_t *S) {
   S->b = (double *)calloc((size_t)n, sizeof(double));
   S->fteth = (double *)calloc(3 * (size_t)A + 3, sizeof(double));
   S->fuser = (double *)calloc(3 * (size_t)A + 3, sizeof(double));
+  S->fuser_raw = (double *)calloc(3 * (size_t)A + 3, sizeof(double));
   S->fs_norm = (double *)calloc((size_t)A + 1, sizeof(double));
   S->fu_norm = (double *)calloc((size_t)A + 1, sizeof(double));
 
@@ -768,20 +822,29 @@ static void build_system(const obo_world *W, system_t *S) {
     if (body < 0) continue;
     if (body >= N) {
       int a = body - N;
-      for (int k = 0; k < 3; k++) S->fuser[3 * a + k] += W->wr_force[s][k];
+      double F[3] = {W->wr_force[s][0], W->wr_force[s][1], W->wr_force[s][2]};
+      for (int k = 0; k < 3; k++) S->fuser_raw[3 * a + k] += F[k];            /* the detach predicate sees the pull itself */
+      apply_rails(P, W->am[a], W->av + 3 * a, F);                           /* an apple is a free body (A36) */
+      for (int k = 0; k < 3; k++) S->fuser[3 * a + k] += F[k];
     } else {
       if (P->forces_off_on_snapped && snapped[body]) continue;   /* reading A10 */
       int e = ext->n++;
-      double o[3];
+      double o[3], F[3] = {W->wr_force[s][0], W->wr_force[s][1], W->wr_force[s][2]};
       mat3vec(f.R + 9 * body, W->wr_point[s], o);
       ext->link[e] = body;
-      for (int k = 0; k < 3; k++) { ext->x[e][k] = f.p[3 * body + k] + o[k]; ext->F[e][k] = W->wr_force[s][k]; }
+      for (int k = 0; k < 3; k++) ext->x[e][k] = f.p[3 * body + k] + o[k];
+      if (snapped[body]) {                                       /* a link of a snapped sub-tree is a free body (A36) */
+        double vpt[3];
+        point_velocity(W, &f, W->qd, body, ext->x[e], vpt);
+        apply_rails(P, W->m[body], vpt, F);
+      }
+      for (int k = 0; k < 3; k++) ext->F[e][k] = F[k];
     }
   }
   /* 2. tethers (Eq. 6, Eq. 7; readings A11-A13, A15) */
   double *xh = (double *)calloc(3 * (size_t)A + 3, sizeof(double));
   for (int a = 0; a < A; a++) {
-    S->fu_norm[a] = norm3(S->fuser + 3 * a);
+    S->fu_norm[a] = norm3(S->fuser_raw + 3 * a);
     if (!W->attached[a]) continue;
     int b = W->alink[a];
     double o[3], vh[3], fs[3], fr[3];
@@ -808,7 +871,7 @@ static void build_system(const obo_world *W, system_t *S) {
   double *bias = (double *)calloc((size_t)n, sizeof(double));
   rnea(W, W->q, W->qd, zero, P->g, ext, bias);
   for (int i = 0; i < N; i++) {
-    double Kt = W->ruptured[i] ? 0.0 : W->K[i], Dt = P->c_d * Kt;
+    double Kt = W->ruptured[i] ? 0.0 : W->K[i], Dt = P->c_d * Kt + friction_damper(W, i);
     for (int k = 0; k < 2; k++) {
       int j = 2 * i + k;
       S->b[j] = h * (-bias[j] - Kt * W->q[j] - (Dt + h * Kt) * W->qd[j]);
@@ -822,15 +885,28 @@ static void build_system(const obo_world *W, system_t *S) {
      (linearly implicit, like the joint damper):  M dqd = h [ ... - alpha M (qd + dqd) ]  ->
      A gets (1 + h alpha) M, b gets - h alpha M qd. */
   if (P->alpha_m != 0.0) {
+    /* per link alpha_i = alpha_m, times snap_drag_scale on snapped sub-trees ("a snapped sub-tree's
+       linear drag is also reduced"; reading A35).  M is linear in the link inertias, so sum_i alpha_i J_i^T I_i J_i is
+       the mass matrix of the same tree with every inertia scaled by alpha_i. */
+    obo_world Ws = *W;
+    double *ms = (double *)malloc(sizeof(double) * N), *ix = (double *)malloc(sizeof(double) * N), *iz = (double *)malloc(sizeof(double) * N);
+    for (int i = 0; i < N; i++) {
+      double al = P->alpha_m * (snapped[i] ? P->snap_drag_scale : 1.0);
+      ms[i] = al * W->m[i]; ix[i] = al * W->Ixx[i]; iz[i] = al * W->Izz[i];
+    }
+    Ws.m = ms; Ws.Ixx = ix; Ws.Izz = iz;
+    double *Ma = (double *)calloc((size_t)n * n, sizeof(double));
+    mass_matrix(&Ws, W->q, Ma);
     for (int r_ = 0; r_ < n; r_++) {
       double mq = 0.0;
-      for (int c_ = 0; c_ < n; c_++) mq += S->A[(size_t)r_ * n + c_] * W->qd[c_];
-      S->b[r_] -= h * P->alpha_m * mq;
+      for (int c_ = 0; c_ < n; c_++) mq += Ma[(size_t)r_ * n + c_] * W->qd[c_];
+      S->b[r_] -= h * mq;
     }
-    for (size_t k = 0; k < (size_t)n * n; k++) S->A[k] *= 1.0 + h * P->alpha_m;
+    for (size_t k = 0; k < (size_t)n * n; k++) S->A[k] += h * Ma[k];
+    free(Ma); free(ms); free(ix); free(iz);
   }
   for (int i = 0; i < N; i++) {
-    double Kt = W->ruptured[i] ? 0.0 : W->K[i], Dt = P->c_d * Kt;
+    double Kt = W->ruptured[i] ? 0.0 : W->K[i], Dt = P->c_d * Kt + friction_damper(W, i);
     for (int k = 0; k < 2; k++) {
       int j = 2 * i + k;
       S->A[(size_t)j * n + j] += W->arm[j] + h * Dt + h * h * Kt;
@@ -916,6 +992,7 @@ static void step_once(obo_world *W) {
     W->rc[i] = mu > W->Mmax[i] ? W->rc[i] + 1 : 0;
     if (W->rc[i] >= P->rupture_frames) {
       W->ruptured[i] = 1;
+      W->rstep[i] = W->step;
       push_event(W, 0, i, mu, W->Mmax[i]);
     }
   }
@@ -963,7 +1040,11 @@ void obo_set_state(obo_world *W, const double *q, const double *qd, const double
   if (qd) memcpy(W->qd, qd, sizeof(double) * 2 * W->N);
   if (ax) memcpy(W->ax, ax, sizeof(double) * 3 * W->A);
   if (av) memcpy(W->av, av, sizeof(double) * 3 * W->A);
-  if (ruptured) { memcpy(W->ruptured, ruptured, (size_t)W->N); memset(W->rc, 0, sizeof(int) * W->N); }
+  if (ruptured) {
+    memcpy(W->ruptured, ruptured, (size_t)W->N);
+    memset(W->rc, 0, sizeof(int) * W->N);
+    for (int i = 0; i < W->N; i++) W->rstep[i] = W->step;      /* friction ramps from the moment the flag was set */
+  }
   if (attached) {
     memcpy(W->attached, attached, (size_t)W->A);
     memset(W->cA, 0, sizeof(int) * W->A);
@@ -980,6 +1061,8 @@ void obo_set_counters(obo_world *W, const int32_t *rc, const int32_t *cA, const 
   for (int a = 0; a < W->A; a++) { W->cA[a] = cA[a]; W->cB[a] = cB[a]; }
 }
 void obo_set_step(obo_world *W, int step) { W->step = step; }
+void obo_get_rupture_steps(const obo_world *W, int32_t *rstep) { for (int i = 0; i < W->N; i++) rstep[i] = W->rstep[i]; }
+void obo_set_rupture_steps(obo_world *W, const int32_t *rstep) { for (int i = 0; i < W->N; i++) W->rstep[i] = rstep[i]; }
 void obo_set_solver(obo_world *W, int solver, double tol, int max_iter) {
   W->P.solver = solver; W->P.cg_tol = tol; W->P.cg_max_iter = max_iter;
 }

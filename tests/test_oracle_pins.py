@@ -949,3 +949,118 @@ def test_geometry_randomization_droop_compounds_per_internode():
         assert abs(math.acos(np.clip(d[2], -1, 1)) - t) < 1e-9, (k, t)
         prev = t
     assert prev > th0 + n * droop * math.sin(th0) * 0.99              # compounding: more than n equal increments
+
+
+# ---------------------------------------------------------------- post-rupture dissipation and the force rails (8(f) item 1)
+def test_post_rupture_coulomb_friction_stops_a_free_hinge_in_the_closed_form_time():
+    """A34: a ruptured joint carries a friction torque T_f = fric_frac M_max against its velocity, taken
+    as the damper T_f / |qd| at the start-of-step speed.  One free hinge, no gravity: (J + h T / |w|) w+ = J w, i.e.
+    w+ = w - h T / J to first order: it stops after J w0 / T.  With the ramp T grows linearly to fric_ramp T_0 over
+    fric_time, counted from the step of the rupture."""
+    L, d, rho, MOR = 0.5, 0.02, 800.0, 60e6
+    spec = chain_spec(1, L, d)
+    Lf, df = float(spec.length[0]), float(spec.diameter[0])
+    m = rho * math.pi * (df / 2) ** 2 * Lf
+    J = m * Lf * Lf / 3 + m * (df / 2) ** 2 / 4
+    Mmax = MOR * math.pi * df ** 3 / 32
+    h = float(np.float32(1e-3))
+    for ramp, t_r in ((1.0, 1.5), (5.0, 0.05)):
+        frac = float(np.float32(2e-4))
+        P = Params(h=1e-3, gravity=(0, 0, 0), qd_max=0.0, fric_frac=frac, fric_ramp=ramp, fric_time=t_r, fric_veps=1e-3)
+        w = OracleWorld(spec, P)
+        w0 = 3.0
+        w.set_state(qd=[w0, 0.0], ruptured=[1])
+        v, steps, hist = w0, 0, []
+        T0 = frac * Mmax
+        t_rf = float(np.float32(t_r))
+        while v > 2e-3 and steps < 4000:
+            T = T0 * (1.0 + (ramp - 1.0) * min(h * steps / t_rf, 1.0))
+            v = J * v / (J + h * T / max(v, float(np.float32(1e-3))))
+            w.step(1)
+            steps += 1
+            assert abs(w.get_state()["qd"][0] - v) < 1e-9 * w0, (ramp, steps)
+            hist.append(v)
+        assert abs(w.get_state()["qd"][1]) < 1e-14
+        if ramp == 1.0:                                    # constant torque: linear deceleration, stop at J w0 / T
+            assert abs(steps * h - J * w0 / T0) < 0.02 * J * w0 / T0 + 3 * h, (steps * h, J * w0 / T0)
+        else:                                              # the ramp shortens it
+            assert steps * h < 0.75 * J * w0 / T0
+    # an intact joint feels none of it
+    wa, wb = OracleWorld(chain_spec(3, 0.9, 0.02), Params(fric_frac=0.1)), OracleWorld(chain_spec(3, 0.9, 0.02), Params())
+    for x in (wa, wb):
+        x.set_state(q=[0.01, 0.02, -0.01, 0.0, 0.02, 0.01], qd=[0.3, -0.2, 0.1, 0.5, -0.4, 0.2])
+    assert np.array_equal(wa.system()[0], wb.system()[0]) and np.array_equal(wa.system()[1], wb.system()[1])
+
+
+def test_snapped_subtree_drag_is_reduced():
+    """A35 ("a snapped sub-tree's linear drag is also reduced"): alpha_i = mass_damping snap_drag_scale on
+    the links at or below a ruptured joint.  A free hinge decays as v0 / (1 + h alpha scale)^n; the intact part of the
+    tree keeps the full alpha: the system of a 2-link chain with the outer joint ruptured equals
+    M + h alpha (M - M_outer) + h alpha scale M_outer, with M_outer the mass matrix of the outer link alone."""
+    alpha, scale, h = 2.0, 0.2, float(np.float32(2e-3))
+    spec = chain_spec(1, 0.5, 0.02)
+    w = OracleWorld(spec, Params(gravity=(0, 0, 0), qd_max=0.0, mass_damping=alpha, snap_drag_scale=scale))
+    w.set_state(qd=[0.7, 0.0], ruptured=[1])             # about the first axis only: theta_2 stays 0, M_11 constant
+    sc = float(np.float32(scale))
+    for n in range(1, 30):
+        w.step(1)
+        assert np.abs(w.get_state()["qd"] - np.array([0.7, 0.0]) / (1 + h * alpha * sc) ** n).max() < 1e-12
+    spec2 = chain_spec(2, 0.8, 0.02)
+    q = [0.05, -0.02, 0.03, 0.04]
+    full = OracleWorld(spec2, Params(gravity=(0, 0, 0)))
+    full.set_state(q=q, ruptured=[0, 1])
+    M = full.mass_matrix()
+    A0 = full.system()[0]
+    # M_outer: the same chain with the inner link's inertia removed = M - M(inner only); M(inner only) touches DoF 0, 1
+    inner = OracleWorld(chain_spec(1, 0.4, 0.02), Params(gravity=(0, 0, 0)))
+    inner.set_state(q=q[:2])
+    M_inner = np.zeros((4, 4)); M_inner[:2, :2] = inner.mass_matrix()
+    M_outer = M - M_inner
+    damped = OracleWorld(spec2, Params(gravity=(0, 0, 0), mass_damping=alpha, snap_drag_scale=scale))
+    damped.set_state(q=q, ruptured=[0, 1])
+    A1 = damped.system()[0]
+    expect = A0 + h * alpha * M_inner + h * alpha * sc * M_outer
+    assert np.abs(A1 - expect).max() < 1e-12 * np.abs(A1).max()
+
+
+def test_force_rails_on_a_free_apple_and_never_on_static_loading():
+    """A36 (App. B): (1) impulse cap: an applied force may not take a free body past rail_speed in one
+    step; (2) power fade: the part of the force along the body's velocity fades out between rail_fade rail_speed and
+    rail_speed; (3) speed brake above rail_speed.  A detached apple is the free body; gravity off."""
+    mA, vl, brake = 0.2, 4.0, 50.0
+    spec = chain_spec(1, 0.5, 0.02, apples=[(0, (0, 0, 0.5), mA, 2e3, 20.0)])
+    h = float(np.float32(1e-3))
+    mAf = float(np.float32(mA))
+    P = Params(h=1e-3, gravity=(0, 0, 0), rail_speed=vl, rail_fade=0.5, rail_brake=brake)
+
+    def run(v0, F, P=P):
+        w = OracleWorld(spec, P)
+        w.set_state(attached=[0], apple_v=[v0])
+        w.apply_wrench(1, (0, 0, 0), F)
+        w.step(1)
+        return w.get_state()["apple_v"][0]
+    # (1) cap: 5000 N on 0.2 kg would give 25 m/s in a step; the rail stops it at the limit, along the force
+    assert np.allclose(run([0, 0, 0], (5000.0, 0, 0)), [vl, 0, 0], atol=1e-12)
+    assert np.allclose(run([1.0, 0, 0], (0, 5000.0, 0)), [1.0, vl, 0], atol=1e-12)          # v . F^ = 0: full headroom
+    # no effect below the cap and below the fade onset
+    assert np.allclose(run([1.0, 0, 0], (30.0, 10.0, 0)), [1.0 + h * 30 / mAf, h * 10 / mAf, 0], atol=1e-12)
+    # (2) fade: at 3 m/s (half way between onset 2 and limit 4) the parallel part is halved, the rest untouched
+    assert np.allclose(run([3.0, 0, 0], (30.0, 10.0, 0)), [3.0 + h * 15 / mAf, h * 10 / mAf, 0], atol=1e-12)
+    assert np.allclose(run([3.0, 0, 0], (-30.0, 10.0, 0)), [3.0 - h * 30 / mAf, h * 10 / mAf, 0], atol=1e-12)   # braking force: no fade
+    # (3) brake above the limit: the pushing part is gone, and - brake m (|v| - v_lim) v^ acts
+    assert np.allclose(run([6.0, 0, 0], (30.0, 0.0, 0)), [6.0 - h * brake * 2.0, 0, 0], atol=1e-12)
+    # rails off: the raw force
+    assert np.allclose(run([0, 0, 0], (5000.0, 0, 0), dataclasses.replace(P, rail_speed=0.0)), [h * 5000 / mAf, 0, 0], atol=1e-9)
+    # the detach predicate sees the pull itself, not the railed force: config 1 with rails on has the same events, and
+    # static loading of the connected tree is untouched (same state after the run)
+    spec1 = binary_tree_config1()
+    res = []
+    for rs in (0.0, 3.0):
+        w = OracleWorld(spec1, dataclasses.replace(config_params(1), rail_speed=rs))
+        for s in range(400):
+            for (_, body, pt, f) in config1_loads(spec1, s, 500, 30.0, 400.0):
+                w.apply_wrench(body, pt, f)
+            w.step(1)
+        res.append((w.events(), w.get_state()["q"]))
+    assert [e[:4] for e in res[0][0]] == [e[:4] for e in res[1][0]] and len(res[0][0]) == 1
+    assert np.abs(res[0][1] - res[1][1]).max() < 1e-6

@@ -71,6 +71,14 @@ class Params:
     zeta_s: float = 0.1
     forces_off_on_snapped: int = 1
     mass_damping: float = 0.0      # c_v = c_omega of PAPER.md:128, 1/s (reading A32); 0 = off
+    fric_frac: float = 0.0         # post-rupture Coulomb friction torque as a fraction of M_max (A34); 0 = off
+    fric_ramp: float = 5.0         # ... ramped up by this factor ("~5x")
+    fric_time: float = 1.5         # ... over this time, s ("~1.5 s")
+    fric_veps: float = 1e-2        # ... regularised below this joint speed, rad/s
+    snap_drag_scale: float = 1.0   # factor on mass_damping for snapped sub-trees (A35); 1 = no reduction
+    rail_speed: float = 0.0        # speed limit of the three force rails, m/s (A36); 0 = rails off
+    rail_fade: float = 0.5         # power fade starts at this fraction of rail_speed
+    rail_brake: float = 50.0       # speed-brake rate above rail_speed, 1/s
     range_E: tuple = (0.0, 0.0)
     range_MOR: tuple = (0.0, 0.0)
     range_density: tuple = (0.0, 0.0)
