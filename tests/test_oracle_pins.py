@@ -1064,3 +1064,9 @@ def test_force_rails_on_a_free_apple_and_never_on_static_loading():
         res.append((w.events(), w.get_state()["q"]))
     assert [e[:4] for e in res[0][0]] == [e[:4] for e in res[1][0]] and len(res[0][0]) == 1
     assert np.abs(res[0][1] - res[1][1]).max() < 1e-6
+    # a rail so tight that it caps a 25 N pull to 1 N: path A still counts the pull itself (25 N > 20 N for 3 steps)
+    w = OracleWorld(spec1, dataclasses.replace(config_params(1), rail_speed=0.01))
+    w.apply_wrench(spec1.n_links + 2, (0, 0, 0), (0.0, 25.0, 0.0))
+    w.step(4)
+    ev = w.events()
+    assert len(ev) == 1 and ev[0][1:4] == (2, 1, 2) and ev[0][4] == 25.0
