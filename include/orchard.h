@@ -101,6 +101,20 @@ typedef struct {
   float mass_damping;           /* {0} 1/s >= 0: velocity-proportional damping F = -c_v m v, tau = -c_omega I omega on
                                    every link and apple with c_v = c_omega = mass_damping; in joint
                                    space -mass_damping M(q) qd, taken linearly implicit like the joint damper */
+  /* post-rupture dissipation */
+  float fric_frac;              /* {0 = off} Coulomb friction torque at a ruptured joint, as a fraction of its M_max,
+                                   against the joint velocity (regularised below fric_veps) */
+  float fric_ramp;              /* {5} ... ramped up by this factor ("~5x") */
+  float fric_time;              /* {1.5} ... over this time after the rupture, s ("~1.5 s") */
+  float fric_veps;              /* {1e-2} rad/s */
+  float snap_drag_scale;        /* {1 = no reduction} factor on mass_damping for the links of snapped sub-trees */
+  /* the three rails on applied forces (App. B): act on wrenches on FREE bodies -- apples, and links of
+     snapped sub-trees when forces_off_on_snapped = 0; connected links are static loading, which they never touch */
+  float rail_speed;             /* {0 = rails off} m/s: impulse cap (no force takes the body past it in one step) and
+                                   speed brake above it */
+  float rail_fade;              /* {0.5} the part of a force along the body's velocity fades out between
+                                   rail_fade * rail_speed and rail_speed */
+  float rail_brake;             /* {50} 1/s: brake force - rail_brake m (|v| - rail_speed) v^ above rail_speed */
 } ob_params;
 
 typedef struct {
@@ -216,6 +230,10 @@ int ob_get_apple_x64(ob_ctx *ctx, int world, double *apple_x);
 int ob_set_apple_x64(ob_ctx *ctx, int world, const double *apple_x);
 /* Restore the step counter of a world (events carry it); everything else is kept, the warm start included. */
 int ob_set_step(ob_ctx *ctx, int world, int32_t step);
+/* Step during which each joint ruptured ([n_links]; meaningful where ruptured): the post-rupture friction ramp
+    counts from it.  ob_set_state(ruptured) sets it to the world's current step. */
+int ob_get_rupture_steps(ob_ctx *ctx, int world, int32_t *rupture_step);
+int ob_set_rupture_steps(ob_ctx *ctx, int world, const int32_t *rupture_step);
 /* Hysteresis counters (rupture per link; detach pull / tension per apple), for lock-step
    comparison and checkpoints.  The _batch form covers worlds [world0, world0 + n_worlds), outputs concatenated. */
 int ob_get_counters(ob_ctx *ctx, int world, int32_t *rupture_count, int32_t *pull_count, int32_t *tension_count);

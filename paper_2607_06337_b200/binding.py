@@ -24,7 +24,8 @@ EXPORTS = [
     "ob_sizeof_params", "ob_sizeof_world_spec", "ob_sizeof_event", "ob_counters", "ob_flush",
     "ob_selftest_philox", "ob_get_state_batch", "ob_set_apple_x64", "ob_set_step", "ob_get_counters_batch",
     "ob_get_material_batch", "ob_world_blob_bytes", "ob_save_world", "ob_load_world", "ob_iter_histogram",
-    "ob_randomize_geometry", "ob_get_geometry", "ob_sizeof_geometry_ranges",
+    "ob_randomize_geometry", "ob_get_geometry", "ob_sizeof_geometry_ranges", "ob_get_rupture_steps",
+    "ob_set_rupture_steps",
 ]
 
 
@@ -48,6 +49,8 @@ class ob_params(C.Structure):
         ("forces_off_on_snapped", C.c_int32),
         ("range_E", C.c_float * 2), ("range_MOR", C.c_float * 2), ("range_density", C.c_float * 2),
         ("range_detach", C.c_float * 2), ("range_apple_mass", C.c_float * 2), ("mass_damping", C.c_float),
+        ("fric_frac", C.c_float), ("fric_ramp", C.c_float), ("fric_time", C.c_float), ("fric_veps", C.c_float),
+        ("snap_drag_scale", C.c_float), ("rail_speed", C.c_float), ("rail_fade", C.c_float), ("rail_brake", C.c_float),
     ]
 
 
@@ -91,6 +94,8 @@ def load_library():
         L.ob_get_apple_x64.argtypes = [vp, i32, vp]
         L.ob_set_apple_x64.argtypes = [vp, i32, vp]
         L.ob_set_step.argtypes = [vp, i32, C.c_int32]
+        L.ob_get_rupture_steps.argtypes = [vp, i32, vp]
+        L.ob_set_rupture_steps.argtypes = [vp, i32, vp]
         L.ob_get_state_batch.argtypes = [vp, i32, i32] + [vp] * 8
         L.ob_get_counters_batch.argtypes = [vp, i32, i32] + [vp] * 3
         L.ob_get_material_batch.argtypes = [vp, i32, i32] + [vp] * 3
@@ -145,7 +150,8 @@ def params_struct(p) -> ob_params:
     s.gravity = (C.c_float * 3)(*p.gravity)
     for name in ("c_d", "cg_tol", "cg_max_iter", "precond", "cg_norm", "rupture_frames", "detach_frames_pull", "detach_kappa",
                  "detach_frames_tension", "react_max", "tether_implicit", "qd_max", "zeta_s",
-                 "forces_off_on_snapped", "mass_damping"):
+                 "forces_off_on_snapped", "mass_damping", "fric_frac", "fric_ramp", "fric_time", "fric_veps",
+                 "snap_drag_scale", "rail_speed", "rail_fade", "rail_brake"):
         setattr(s, name, getattr(p, name))
     for name in ("range_E", "range_MOR", "range_density", "range_detach", "range_apple_mass"):
         setattr(s, name, (C.c_float * 2)(*getattr(p, name)))
@@ -305,6 +311,15 @@ class Orchard:
 
     def set_step(self, world: int, step: int):
         self._check(self._L.ob_set_step(self._h, world, int(step)))
+
+    def get_rupture_steps(self, world: int) -> np.ndarray:
+        r = np.zeros(self.n_links[world], np.int32)
+        self._check(self._L.ob_get_rupture_steps(self._h, world, _ptr(r)))
+        return r
+
+    def set_rupture_steps(self, world: int, rupture_step):
+        r = _i32(rupture_step)
+        self._check(self._L.ob_set_rupture_steps(self._h, world, _ptr(r)))
 
     def save_world(self, world: int) -> bytes:
         n = C.c_size_t(0)

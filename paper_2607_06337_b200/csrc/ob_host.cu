@@ -91,7 +91,10 @@ int validate(const ob_world_spec *specs, int n_worlds, const ob_params *P, std::
   if (!specs || !P || n_worlds < 1) { why = "null specs/params or n_worlds < 1"; return OB_E_ARG; }
   if (!(P->h > 0.f) || !(P->cg_tol > 0.f) || P->cg_max_iter < 1 || P->rupture_frames < 1 || P->rupture_frames > 255 ||
       P->detach_frames_pull < 1 || P->detach_frames_pull > 255 || P->detach_frames_tension < 1 ||
-      P->detach_frames_tension > 255 || !(P->react_max >= 0.f) || !(P->c_d >= 0.f) || !(P->mass_damping >= 0.f) || P->precond < 0 || P->precond > 2 || P->cg_norm < 0 || P->cg_norm > 1 || (P->precond == 2 && P->cg_norm == 1)) {
+      P->detach_frames_tension > 255 || !(P->react_max >= 0.f) || !(P->c_d >= 0.f) || !(P->mass_damping >= 0.f) || P->precond < 0 || P->precond > 2 || P->cg_norm < 0 || P->cg_norm > 1 || (P->precond == 2 && P->cg_norm == 1) ||
+      !(P->fric_frac >= 0.f) || !(P->fric_ramp >= 0.f) || !(P->fric_time >= 0.f) || !(P->fric_veps > 0.f) ||
+      !(P->snap_drag_scale >= 0.f) || !(P->rail_speed >= 0.f) || !(P->rail_fade >= 0.f) || !(P->rail_fade < 1.f) ||
+      !(P->rail_brake >= 0.f)) {
     why = "ob_params out of range";
     return OB_E_ARG;
   }
@@ -351,6 +354,9 @@ int ob_default_params(ob_params *p) {
   p->zeta_s = 0.1f;
   p->forces_off_on_snapped = 1;
   p->mass_damping = 0.f;
+  p->fric_frac = 0.f; p->fric_ramp = 5.f; p->fric_time = 1.5f; p->fric_veps = 1e-2f;
+  p->snap_drag_scale = 1.f;
+  p->rail_speed = 0.f; p->rail_fade = 0.5f; p->rail_brake = 50.f;
   return OB_OK;
 }
 
@@ -846,7 +852,8 @@ int get_state_impl(ob_ctx *ctx, int w0, int n, float *q, float *qd, float *apple
 
 // read-modify-write of one world's state blocks (everything the caller passes as NULL is kept)
 int set_state_impl(ob_ctx *ctx, int world, const float *q, const float *qd, const float *apple_x, const double *apple_x64,
-                   const float *apple_v, const uint8_t *ruptured, const uint8_t *attached, const int32_t *step) {
+                   const float *apple_v, const uint8_t *ruptured, const uint8_t *attached, const int32_t *step,
+                   const int32_t *rupture_step = nullptr) {
   int rc = check_world(ctx, world);
   if (rc != OB_OK) return rc;
   const WorldDesc &d = ctx->desc[world];
@@ -859,12 +866,14 @@ int set_state_impl(ob_ctx *ctx, int world, const float *q, const float *qd, cons
   if (d.Ap) ab.assign(v.apple, v.apple + apple_block_bytes(d.Ap));
   WorldInfo wi = v.info[0];
   float *st = reinterpret_cast<float *>(lb.data());
+  int32_t *rs = reinterpret_cast<int32_t *>(st + 4 * d.Np);          // step of the rupture per link
   unsigned char *fl = lb.data() + kLinkStateFloats * 4 * d.Np;
   for (int i = 0; i < d.N; i++) {
     const int e = H.int2ext_link[i];
     if (q) { st[2 * i] = q[2 * e]; st[2 * i + 1] = q[2 * e + 1]; }
     if (qd) { st[2 * d.Np + 2 * i] = qd[2 * e]; st[2 * d.Np + 2 * i + 1] = qd[2 * e + 1]; }
-    if (ruptured) { fl[i] = ruptured[e] ? 1 : 0; fl[d.Np + i] = 0; }
+    if (ruptured) { fl[i] = ruptured[e] ? 1 : 0; fl[d.Np + i] = 0; rs[i] = step ? *step : wi.step; }
+    if (rupture_step) rs[i] = rupture_step[e];
   }
   if (d.Ap) {
     float *as = reinterpret_cast<float *>(ab.data());
@@ -883,7 +892,7 @@ int set_state_impl(ob_ctx *ctx, int world, const float *q, const float *qd, cons
   }
   wi.status = 0;
   if (step) wi.step = *step;
-  if (!step || q || qd || apple_x || apple_x64 || apple_v || ruptured || attached)
+  if ((!step && !rupture_step) || q || qd || apple_x || apple_x64 || apple_v || ruptured || attached)
     for (int k = 0; k < 4; k++)   // ... and forget the solution history the PCG start vector is extrapolated from
       CU(cudaMemsetAsync(ctx->dev.xprev + (size_t)k * ctx->dev.sum_np + d.link_base, 0, sizeof(float2) * d.Np, ctx->stream));
   CU(cpy(ctx, ctx->dev.link_blk + d.link_blk_off, lb.data(), lb.size(), cudaMemcpyHostToDevice, ctx->stream));
@@ -933,6 +942,24 @@ int ob_set_apple_x64(ob_ctx *ctx, int world, const double *apple_x) {
 int ob_set_step(ob_ctx *ctx, int world, int32_t step) {
   if (ctx && step < 0) return fail(ctx, OB_E_ARG, "step < 0");
   return set_state_impl(ctx, world, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, &step);
+}
+
+int ob_get_rupture_steps(ob_ctx *ctx, int world, int32_t *rupture_step) {
+  int rc = check_world(ctx, world);
+  if (rc != OB_OK) return rc;
+  if (!rupture_step) return fail(ctx, OB_E_ARG, "rupture_step is null");
+  const WorldDesc &d = ctx->desc[world];
+  RdView v;
+  rc = rd_fetch(ctx, world, 1, true, false, false, -1, v);
+  if (rc != OB_OK) return rc;
+  const int32_t *rs = reinterpret_cast<const int32_t *>(v.link) + 4 * d.Np;
+  for (int i = 0; i < d.N; i++) rupture_step[ctx->hw[world].int2ext_link[i]] = rs[i];
+  return OB_OK;
+}
+
+int ob_set_rupture_steps(ob_ctx *ctx, int world, const int32_t *rupture_step) {
+  if (ctx && !rupture_step) return fail(ctx, OB_E_ARG, "rupture_step is null");
+  return set_state_impl(ctx, world, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, rupture_step);
 }
 
 int ob_world_blob_bytes(ob_ctx *ctx, int world, size_t *out) {

@@ -15,11 +15,12 @@ __host__ __device__ inline int pad16(int n) { return (n + kPad - 1) / kPad * kPa
 //      contiguous chunk, which is what the batched read-out copies).  k_step reads and writes it in place (L2): only
 //      the once-per-step phases touch it.
 //   float2  q[Np] qd[Np]                the two DoF of a joint interleaved
+//   int32   rstep[Np]                   step during which the joint ruptured (the friction ramp counts from it)
 //   bytes   ruptured[Np] rc[Np]
 // ---- per-world link CONSTANT block (pool link_cst; written by k_randomize):
 //   float4  c4[Np] = (m, m c, I about the joint, I_zz)
 //   floats  K[Np] rz[Np]                joint stiffness (Eq. 4), parent length
-constexpr int kLinkStateFloats = 4;
+constexpr int kLinkStateFloats = 5;
 constexpr int kLinkConstFloats = 6;
 __host__ __device__ inline int link_state_bytes(int Np) { return kLinkStateFloats * 4 * Np + 2 * Np; }
 __host__ __device__ inline int link_const_bytes(int Np) { return kLinkConstFloats * 4 * Np; }

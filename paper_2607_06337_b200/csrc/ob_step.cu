@@ -116,6 +116,7 @@ __device__ __forceinline__ Sm carve(unsigned char *base, const int Np, const int
 // per-link data of one world in global memory (L2-resident; only the once-per-step phases read it)
 struct Gm {
   float2 *q2, *w2;                  // state (link block)
+  int32_t *rstep;                   // step during which the joint ruptured
   unsigned char *rupt, *rc;
   const float4 *c4;                 // (m, m c, I about the joint, I_zz)
   const float *K, *rz;              // joint stiffness (Eq. 4), parent length
@@ -437,25 +438,41 @@ __device__ __forceinline__ void link_joint(const int i, const Sm &s, const Gm &g
   store_qd(rec, q);
 }
 
+// Coulomb friction at a ruptured joint ("introduced at the break and ramped up ~5x over ~1.5 s as the
+// torn fibres seize"; reading A34) as the damper D_f = T_f(t) / max(|qd|, v_eps) at the start-of-step joint speed,
+// T_f(t) = fric_frac M_max (1 + (fric_ramp - 1) min(t / fric_time, 1)), t = h (step - step of the rupture)
+__device__ __forceinline__ float friction_damper(const int i, const float2 w, const int step, const Gm &g, const ob_params &P) {
+  const float t = P.h * (float)(step - __ldcg(g.rstep + i));
+  const float ramp = P.fric_time > 0.f ? fminf(t / P.fric_time, 1.f) : 1.f;
+  const float Tf = P.fric_frac * __ldg(g.Mmax + i) * (1.f + (P.fric_ramp - 1.f) * ramp);
+  return Tf / fmaxf(sqrtf(w.x * w.x + w.y * w.y), P.fric_veps);
+}
+
 // The global inputs of a level sweep are staged by a FLAT pass before it (one L2 round trip for the whole world
 // instead of one per level of the sweep): the link's own inertia constants -> IN, (q, qd) -> XR, K -> PD.x (before
-// phase F: -> X21, because A1 publishes through PD).  Each sweep reads them at the link's own turn, before it
+// phase F: -> X21, because A1 publishes through PD and XR.xy).  Each sweep reads them at the link's own turn, before it
 // overwrites the slots with what it publishes.
-__device__ __forceinline__ void stage_link_inputs(const int i, const Sm &s, const Gm &g, const bool state) {
+// The friction damper D_f of a ruptured joint goes with them (PD.y; before phase F: XR.z).
+__device__ __forceinline__ void stage_link_inputs(const int i, const Sm &s, const Gm &g, const bool state, const int step,
+                                                  const ob_params &P) {
   float4 *rec = s.P + 7 * i;
   const float4 c4 = __ldg(g.c4 + i);
   const float Ki = __ldg(g.K + i);
+  const uint32_t tw = __float_as_uint(rec[kCS].w);
+  const bool fric = (tw & kRuptured) && P.fric_frac > 0.f;
+  float2 w = make_float2(0.f, 0.f);
+  if (state || fric) w = __ldcg(g.w2 + i);
+  const float Df = fric ? friction_damper(i, w, step, g, P) : 0.f;
   if (state) {
-    const float2 th = __ldcg(g.q2 + i), w = __ldcg(g.w2 + i);
+    const float2 th = __ldcg(g.q2 + i);
     rec[kXR] = make_float4(th.x, th.y, w.x, w.y);
-  }
-  rec[kIN] = c4;
-  if (state) {
-    rec[kPD].x = Ki;
-    if (__float_as_uint(rec[kCS].w) & kHasApples) s.X21[i] = __int_as_float(__ldg(g.topo2 + i).x);   // first apple | count << 16
+    *reinterpret_cast<float2 *>(rec + kPD) = make_float2(Ki, Df);
+    if (tw & kHasApples) s.X21[i] = __int_as_float(__ldg(g.topo2 + i).x);   // first apple | count << 16
   } else {
     s.X21[i] = Ki;
+    rec[kXR].z = Df;
   }
+  rec[kIN] = c4;
 }
 
 // ---- A1 ----  forward kinematics in fp64 (Eq. 3): q_i = q_p q_rel, p_i = p_p + R(q_p) (0,0,L_p).
@@ -517,11 +534,12 @@ __device__ __forceinline__ void link_fk(const int i, const Sm &s, const Gm &g) {
   }
 }
 
-// diagonal terms of the two DoF of a joint: arm + (h c_d + h^2) K (Eq. 4; a ruptured joint has K = D = 0)
-__device__ __forceinline__ float2 diag_terms(const int i, const uint32_t tw, const float Ki, const Sm &s, const Gm &g,
-                                             const ob_params &P) {
+// diagonal terms of the two DoF of a joint: arm + h (c_d K + D_f) + h^2 K (Eq. 4; a ruptured joint has K = 0 and only the
+// post-rupture friction damper D_f, if any)
+__device__ __forceinline__ float2 diag_terms(const int i, const uint32_t tw, const float Ki, const float Df, const Sm &s,
+                                             const Gm &g, const ob_params &P) {
   const float Kt = (tw & kRuptured) ? 0.f : Ki;
-  float dt0 = (P.h * P.c_d + P.h * P.h) * Kt, dt1 = dt0;
+  float dt0 = P.h * (P.c_d * Kt + Df) + P.h * P.h * Kt, dt1 = dt0;
   if (g.arm) {
     dt0 += __ldg(g.arm + i);
     dt1 += __ldg(g.arm + s.Np + i);
@@ -529,12 +547,18 @@ __device__ __forceinline__ float2 diag_terms(const int i, const uint32_t tw, con
   return make_float2(dt0, dt1);
 }
 
+// velocity-proportional damping coefficient of a link (A32), reduced on snapped sub-trees (PAPER.md:141
+// "a snapped sub-tree's linear drag is also reduced"; A35)
+__device__ __forceinline__ float link_alpha(const uint32_t tw, const ob_params &P) {
+  return (tw & kSnapped) ? P.mass_damping * P.snap_drag_scale : P.mass_damping;
+}
+
 // effective link inertia (m, m c, I about the joint, I_zz): the link's own, times (1 + h alpha) for the implicit
 // mass-proportional damping (A32), plus the virtual tether masses h^2 k_s of the attached apples that hang on the
 // link axis (A15).  Apples off the axis set kOffax in the returned topology word and are added one by one.
 __device__ __forceinline__ float4 eff_inertia(const int i, uint32_t &tw, float4 c4, const Sm &s, const Gm &g,
                                               const ob_params &P) {
-  const float sc = 1.f + P.h * P.mass_damping;
+  const float sc = 1.f + P.h * link_alpha(tw, P);
   c4.x *= sc; c4.y *= sc; c4.z *= sc; c4.w *= sc;
   if (P.tether_implicit && (tw & kHasApples)) {
     tw &= ~kOffax;
@@ -592,15 +616,44 @@ __device__ __forceinline__ void apple_forces(const int a, const Sm &s, const ob_
   s.hd[4 * Ap + a] = fl.y; s.hd[5 * Ap + a] = fl.z;
 }
 
-// user wrenches on one link (disabled on snapped sub-trees), subtracted from its bias force
-__device__ __forceinline__ void wrench_forces(const int i, const uint32_t tw, const Sm &s, const ob_params &P, float3 &n,
-                                              float3 &f) {
+// The three rails of PAPER.md:398 (App. B) on an applied force F on a FREE body of mass m moving with velocity v at the
+// application point (reading A36): power fade of the part of F along v between rail_fade v_lim and v_lim; impulse cap
+// |F| <= m max(v_lim - v . F^, 0) / h; speed brake - rail_brake m (|v| - v_lim) v^ above v_lim.
+__device__ __forceinline__ float3 apply_rails(const ob_params &P, const float m, const float3 v, float3 F) {
+  const float vl = P.rail_speed;
+  if (!(vl > 0.f)) return F;
+  const float vn = sqrtf(dot(v, v));
+  float3 vh = f3(0, 0, 0);
+  if (vn > 0.f) {
+    vh = (1.f / vn) * v;
+    const float Fp = dot(F, vh);
+    if (Fp > 0.f) {
+      const float vf = P.rail_fade * vl;
+      const float fade = vn <= vf ? 1.f : (vn >= vl ? 0.f : (vl - vn) / (vl - vf));
+      F = F - ((1.f - fade) * Fp) * vh;
+    }
+  }
+  const float Fn = sqrtf(dot(F, F));
+  if (Fn > 0.f) {
+    const float vF = dot(v, F) / Fn;
+    const float cap = m * fmaxf(vl - vF, 0.f) / P.h;
+    if (Fn > cap) F = (cap / Fn) * F;
+  }
+  if (vn > vl) F = F - (P.rail_brake * m * (vn - vl)) * vh;
+  return F;
+}
+
+// user wrenches on one link (disabled on snapped sub-trees; where they are not, a link of a snapped
+// sub-tree is a free body and its wrench goes through the rails), subtracted from its bias force
+__device__ __forceinline__ void wrench_forces(const int i, const uint32_t tw, const float m, const float3 om, const float3 vl,
+                                              const Sm &s, const ob_params &P, float3 &n, float3 &f) {
   const int nwr = s.wr->n;
   for (int q = 0; q < nwr; q++) {
     if (s.wr->body[q] != i) continue;
     if ((tw & kSnapped) && P.forces_off_on_snapped) continue;
-    const float3 fl = rot_down(s.wq[q], f3(s.wr->force[q][0], s.wr->force[q][1], s.wr->force[q][2]));
+    float3 fl = rot_down(s.wq[q], f3(s.wr->force[q][0], s.wr->force[q][1], s.wr->force[q][2]));
     const float3 pt = f3(s.wr->point[q][0], s.wr->point[q][1], s.wr->point[q][2]);
+    if (tw & kSnapped) fl = apply_rails(P, m, vl + cross(om, pt), fl);   // all in link coordinates
     f = f - fl;
     n = n - cross(pt, fl);
   }
@@ -611,16 +664,16 @@ __device__ __forceinline__ void wrench_forces(const int i, const uint32_t tw, co
 // (th, w, Ki, c4 = q, qd, K, inertia of the link: the caller loads them at the top of its turn, with its other global
 // inputs)
 __device__ __forceinline__ void finish_bias(const Jt &j, const int i, const float2 th, const float2 w, const float Ki,
-                                            const float4 c4, float3 n, float3 f, const Sm &s, const Gm &g,
-                                            const DevCtx &c) {
+                                            const float Df, const float4 c4, float3 n, float3 f, const Sm &s,
+                                            const Gm &g, const DevCtx &c) {
   const ob_params &P = c.P;
   float4 *rec = s.P + 7 * i;
   uint32_t tw = j.tw;
   // spring-damper part of the rhs and of the diagonal (Eq. 4); a ruptured joint has K = D = 0
-  const float Kt = (tw & kRuptured) ? 0.f : Ki, Dt = P.c_d * Kt;
+  const float Kt = (tw & kRuptured) ? 0.f : Ki, Dt = P.c_d * Kt + Df;
   const float2 kq = make_float2(Kt * th.x + (Dt + P.h * Kt) * w.x, Kt * th.y + (Dt + P.h * Kt) * w.y);
   reinterpret_cast<float2 *>(rec + kXR)[1] = make_float2(P.h * (-(j.c2 * n.x + j.s2 * n.z) - kq.x), P.h * (-n.y - kq.y));
-  reinterpret_cast<float2 *>(rec + kPD)[1] = diag_terms(i, tw, Ki, s, g, P);
+  reinterpret_cast<float2 *>(rec + kPD)[1] = diag_terms(i, tw, Ki, Df, s, g, P);
   rec[kIN] = eff_inertia(i, tw, c4, s, g, P);
   if (tw != j.tw) rec[kCS].w = __uint_as_float(tw);
   if (!(tw & kTrunk)) {
@@ -640,7 +693,8 @@ __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm
   float4 *rec = s.P + 7 * i;
   const float4 sq = rec[kXR], c4 = rec[kIN];                      // (q, qd), inertia, K: staged by the flat pass
   const float2 th = make_float2(sq.x, sq.y), w = make_float2(sq.z, sq.w);
-  const float Ki = rec[kPD].x;
+  const float2 kd = *reinterpret_cast<const float2 *>(rec + kPD);
+  const float Ki = kd.x, Df = kd.y;
   const Jt j = load_jt(s.P, i);
   const uint32_t tw = j.tw;
   float3 wp = f3(0, 0, 0), vp = f3(0, 0, 0), alp = f3(0, 0, 0);
@@ -659,9 +713,7 @@ __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm
   om = om + vJ;
   motion_down(j, alp, ap, al, aln);
   const float ww = w.x * w.y;
-  // mass-proportional damping (A32): its generalized force -alpha M qd enters the bias pass as the
-  // joint acceleration alpha qd, i.e. alpha S qd = alpha vJ on top of the velocity-product terms
-  al = al + f3(-s2 * ww, 0.f, c2 * ww) + cross(om, vJ) + P.mass_damping * vJ;
+  al = al + f3(-s2 * ww, 0.f, c2 * ww) + cross(om, vJ);
   aln = aln + cross(vl, vJ);
   // a link with children waits for them, a link with apples for the apple pass: both park
   const bool inner = (((tw >> kNcShift) & kNcMask) | (tw & kHasApples)) != 0u;
@@ -673,16 +725,20 @@ __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm
   const float3 hf = f3(m * vl.x + mc * om.y, m * vl.y - mc * om.x, m * vl.z);
   n = n + cross(om, hn) + cross(vl, hf);
   f = f + cross(om, hf);
-  wrench_forces(i, tw, s, P, n, f);
+  {                                       // velocity-proportional damping F = -c_v m v, tau = -c_omega I omega (
+    const float al_i = link_alpha(tw, P);   // A32, A35): minus alpha times the link's spatial momentum
+    n = n + al_i * hn; f = f + al_i * hf;
+  }
+  wrench_forces(i, tw, c4.x, om, vl, s, P, n, f);
   if (inner) {                                                    // parked until B1 adds the children / the apples
-    const float2 dt = diag_terms(i, tw, Ki, s, g, P);
+    const float2 dt = diag_terms(i, tw, Ki, Df, s, g, P);
     rec[kXR] = make_float4(om.x, om.y, om.z, vl.x);
     rec[kIN] = make_float4(vl.y, vl.z, al.x, al.y);
     rec[kPD] = make_float4(al.z, aln.x, dt.x, dt.y);
     rec[kM0] = make_float4(n.x, n.y, n.z, f.x);
     rec[kM1] = make_float4(f.y, f.z, aln.y, aln.z);
   } else {
-    finish_bias(j, i, th, w, Ki, c4, n, f, s, g, c);
+    finish_bias(j, i, th, w, Ki, Df, c4, n, f, s, g, c);
   }
 }
 
@@ -690,7 +746,8 @@ __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm
 __device__ __forceinline__ void link_bias_up(const int i, const Jt &j, const Sm &s, const Gm &g, const DevCtx &c) {
   const float4 sq = s.P[7 * i + kXR], c4 = s.P[7 * i + kIN];     // staged by the flat pass between A2 and B1
   const float2 th = make_float2(sq.x, sq.y), w = make_float2(sq.z, sq.w);
-  const float Ki = s.P[7 * i + kPD].x;
+  const float2 kd = *reinterpret_cast<const float2 *>(s.P + 7 * i + kPD);
+  const float Ki = kd.x, Df = kd.y;
   const float4 u0 = s.P[7 * i + kM0];
   const float2 v0 = *reinterpret_cast<const float2 *>(s.P + 7 * i + kM1);
   float3 n = f3(u0.x, u0.y, u0.z), f = f3(u0.w, v0.x, v0.y);
@@ -702,7 +759,7 @@ __device__ __forceinline__ void link_bias_up(const int i, const Jt &j, const Sm 
       f = f - f3(s.aq[3 * Ap + a], s.hd[4 * Ap + a], s.hd[5 * Ap + a]);
     }
   }
-  finish_bias(j, i, th, w, Ki, c4, n, f, s, g, c);
+  finish_bias(j, i, th, w, Ki, Df, c4, n, f, s, g, c);
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -735,7 +792,7 @@ __device__ __noinline__ void factor_link(const int i, const World *wd, const Dev
   uint32_t tw = j.tw;
   const float Ki = s.X21[i];                                   // staged by the flat pass before the sweep
   const float4 eff = eff_inertia(i, tw, rec[kIN], s, g, P);
-  const float2 dt = diag_terms(i, tw, Ki, s, g, P);
+  const float2 dt = diag_terms(i, tw, Ki, rec[kXR].z, s, g, P);
   if (tw != j.tw) rec[kCS].w = __uint_as_float(tw);
   // own inertia: body of revolution about +z through the joint
   float A[9] = {eff.z, 0, 0, 0, eff.z, 0, 0, 0, eff.w};
@@ -836,9 +893,9 @@ __device__ __noinline__ void composite_link(const int i, const World *wd, const 
   const Jt j = load_jt(s.P, i);
   uint32_t tw = j.tw;
   float4 c4 = rec[kIN];                                        // staged by the flat pass before the sweep
-  const float2 dt = diag_terms(i, tw, s.X21[i], s, g, P);
+  const float2 dt = diag_terms(i, tw, s.X21[i], rec[kXR].z, s, g, P);
   {
-    const float sc = 1.f + P.h * P.mass_damping;
+    const float sc = 1.f + P.h * link_alpha(tw, P);
     c4.x *= sc; c4.y *= sc; c4.z *= sc; c4.w *= sc;
   }
   float cm = c4.x;
@@ -891,7 +948,7 @@ __device__ __noinline__ void composite_link(const int i, const World *wd, const 
 // allocation of the PCG loop.  The views of the world live in shared memory (World), the context is the kernel's
 // __grid_constant__ parameter.
 // ------------------------------------------------------------------------------------------------------
-__device__ __noinline__ void sweep_kinematics(const World *wd, const DevCtx &c, const int nt) {
+__device__ __noinline__ void sweep_kinematics(const World *wd, const DevCtx &c, const int nt, const int step) {
   const Sm s = carve(wd);
   const Gm g = wd->g;
   const int nlev = wd->nlev, ntop = wd->ntop, tid = threadIdx.x;
@@ -901,7 +958,7 @@ __device__ __noinline__ void sweep_kinematics(const World *wd, const DevCtx &c, 
 #pragma unroll 1
   for (int i = tid; i < wd->N; i += nt) {
     link_joint(i, s, g);
-    stage_link_inputs(i, s, g, false);                  // for phase F (A1 leaves IN and PD.x of every link alone)
+    stage_link_inputs(i, s, g, false, step, c.P);       // for phase F (A1 leaves IN and PD.x of every link alone)
   }
   __syncthreads();
   // ---- A1: forward kinematics in fp64, hang points, top-down ----
@@ -939,13 +996,13 @@ __device__ __noinline__ void sweep_factor(const World *wd, const DevCtx &c, cons
   __syncthreads();
 }
 
-__device__ __noinline__ void sweep_bias(const World *wd, const DevCtx &c, const int nt) {
+__device__ __noinline__ void sweep_bias(const World *wd, const DevCtx &c, const int nt, const int step) {
   const Sm s = carve(wd);
   const Gm g = wd->g;
   const int nlev = wd->nlev, ntop = wd->ntop, tid = threadIdx.x;
   const int l_first_down = tid < 32 ? 0 : ntop - 1, l_last_up = tid < 32 ? 0 : ntop;
 #pragma unroll 1
-  for (int i = tid; i < wd->N; i += nt) stage_link_inputs(i, s, g, true);
+  for (int i = tid; i < wd->N; i += nt) stage_link_inputs(i, s, g, true, step, c.P);
   __syncthreads();
   // ---- A2 (+ B1 for leaves): velocities, bias accelerations, bias forces, top-down ----
 #pragma unroll 1
@@ -963,7 +1020,7 @@ __device__ __noinline__ void sweep_bias(const World *wd, const DevCtx &c, const 
 #pragma unroll 1
   for (int i = tid; i < wd->N; i += nt) {               // what A2 left in the record of a parked link is dead now
     const uint32_t tw = __float_as_uint(s.P[7 * i + kCS].w);
-    if (((tw >> kNcShift) & kNcMask) | (tw & kHasApples)) stage_link_inputs(i, s, g, true);
+    if (((tw >> kNcShift) & kNcMask) | (tw & kHasApples)) stage_link_inputs(i, s, g, true, step, c.P);
   }
   __syncthreads();
 #pragma unroll 1
@@ -1339,6 +1396,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
     {
       unsigned char *lb = c.link_blk + d.link_blk_off;
       g.q2 = reinterpret_cast<float2 *>(lb); g.w2 = g.q2 + Np;
+      g.rstep = reinterpret_cast<int32_t *>(g.w2 + Np);
       g.rupt = lb + kLinkStateFloats * 4 * Np; g.rc = g.rupt + Np;
       const unsigned char *cst = c.link_cst + (size_t)link_const_bytes(1) * d.link_base;
       g.c4 = reinterpret_cast<const float4 *>(cst);
@@ -1388,9 +1446,9 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
     int step0 = __ldcg(&info->step), steps_done = 0, last_iters = 0;
     unsigned long long iters_total = 0;
     for (int sidx = 0; sidx < n_my; sidx++) {
-      sweep_kinematics(&s_world, c, NT);                // A0, A1
+      sweep_kinematics(&s_world, c, NT, step0 + sidx);  // A0, A1
       if (d.precond) sweep_factor(&s_world, c, NT);     // F
-      sweep_bias(&s_world, c, NT);                      // A2, B1: r = b
+      sweep_bias(&s_world, c, NT, step0 + sidx);        // A2, B1: r = b
       float bb_part = 0.f, bz_part = 0.f;
       {                                                 // x = cubic extrapolation of the last four solutions
         const int t = step0 + sidx;                     // (ring of four in global memory, slot = step & 3)
@@ -1474,7 +1532,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
           const int rc0 = drc[k];
           const int rcn = mu > Mx ? rc0 + 1 : 0;
           if (rcn >= P.rupture_frames) {
-            g.rupt[i] = 1; g.rc[i] = 0;
+            g.rupt[i] = 1; g.rc[i] = 0; g.rstep[i] = step_now;
             PL[7 * i + kCS].w = __uint_as_float(tw | kRuptured);
             push_event(c, w, step_now, 0, __ldg(c.link_ext + d.link_base + i), mu, Mx);
           } else if (rcn != rc0) {
@@ -1493,6 +1551,8 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
           if (s.wr->body[k] == N + a) fu = fu + f3(s.wr->force[k][0], s.wr->force[k][1], s.wr->force[k][2]);
         float3 va = f3(s.v[a], s.v[Ap + a], s.v[2 * Ap + a]);
         const float3 v0 = va;                                               // F = -c_v m v on the apple
+        const float3 fraw = fu;                                             // the detach predicate counts the pull itself
+        fu = apply_rails(P, ma, v0, fu);                                    // an apple is a free body (A36)
         va.x += P.h * (P.gravity[0] + (ft.x + fu.x) * inv_m - P.mass_damping * v0.x);
         va.y += P.h * (P.gravity[1] + (ft.y + fu.y) * inv_m - P.mass_damping * v0.y);
         va.z += P.h * (P.gravity[2] + (ft.z + fu.z) * inv_m - P.mass_damping * v0.z);
@@ -1500,7 +1560,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         s.u[a] = fmaf(P.h, va.x, s.u[a]); s.u[Ap + a] = fmaf(P.h, va.y, s.u[Ap + a]);
         s.u[2 * Ap + a] = fmaf(P.h, va.z, s.u[2 * Ap + a]);
         if (att) {
-          const float fun = sqrtf(dot(fu, fu)), fsn = s.fsn[a], thrB = P.detach_kappa * fdet;
+          const float fun = sqrtf(dot(fraw, fraw)), fsn = s.fsn[a], thrB = P.detach_kappa * fdet;
           const int ca = fun > fdet ? s.cA[a] + 1 : 0;
           const int cb = fsn > thrB ? s.cB[a] + 1 : 0;
           if (ca >= P.detach_frames_pull) {

@@ -36,7 +36,8 @@ def test_library_exports_every_declared_symbol():
 def test_struct_layouts_match_the_header():
     # ob_event: 4 x int32 + 2 x float; ob_params: counted from the header's field list
     assert C.sizeof(ob.ob_event) == 24
-    assert C.sizeof(ob.ob_params) == 4 * (1 + 3 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 10 + 1)
+    assert C.sizeof(ob.ob_params) == 4 * (1 + 3 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 1 + 10 + 1 + 8)
+    assert C.sizeof(ob.ob_geometry_ranges) == 64
     assert C.sizeof(ob.ob_world_spec) == 8 * 15 if C.sizeof(C.c_void_p) == 8 else True
     L = ob.load_library()
     assert L.ob_sizeof_params() == C.sizeof(ob.ob_params)
@@ -51,6 +52,8 @@ def test_default_params_are_the_documented_readings():
     assert p.rupture_frames == 3 and p.detach_frames_pull == 3 and p.detach_frames_tension == 10
     assert abs(p.detach_kappa - 1.1) < 1e-6 and p.react_max == 40.0 and p.tether_implicit == 1
     assert p.qd_max == 50.0 and abs(p.zeta_s - 0.1) < 1e-7 and p.forces_off_on_snapped == 1 and p.mass_damping == 0.0
+    assert p.fric_frac == 0.0 and p.fric_ramp == 5.0 and p.fric_time == 1.5 and p.snap_drag_scale == 1.0
+    assert p.rail_speed == 0.0 and p.rail_fade == 0.5 and p.rail_brake == 50.0
     assert ob.load_library().ob_default_params(None) == ob.OB_E_ARG
 
 

@@ -64,6 +64,7 @@ def _sync_oracle_to_gpu(sim, ref, w):
                   ruptured=g["ruptured"], attached=g["attached"])
     ref.set_counters(*sim.get_counters(w))
     ref.set_step(g["step"])
+    ref.set_rupture_steps(sim.get_rupture_steps(w))
     return g
 
 
@@ -961,3 +962,58 @@ def test_geometry_randomization_matches_the_oracle():
         sim.step(9)
     print(f"geometry DR: single-step worst relative error {worst:.2e}")
     sim.close()
+
+
+# ----------------------------------------------------------------------------------------------------
+# post-rupture dissipation and the three force rails (readings A34-A36)
+# ----------------------------------------------------------------------------------------------------
+def test_lockstep_with_post_rupture_friction_reduced_drag_and_rails():
+    """Cascading ruptures with everything of 8(f) item 1 switched on: friction at the break ramped over 0.1 s, drag
+    reduced on snapped sub-trees, wrenches kept on snapped sub-trees (so that the rails act on their links), rails at
+    3 m/s, and pulls on apples strong enough to detach them and then hit the impulse cap on the free apple."""
+    specs = list(_stochastic(57, 100, 180, 12, 4, (5, 6)))
+    P = dataclasses.replace(config_params(5), mass_damping=1.0, snap_drag_scale=0.2, fric_frac=0.02, fric_time=0.1,
+                            rail_speed=3.0, forces_off_on_snapped=0)
+    sim, refs = _make(specs, P, seed=MASTER_SEED + 5001)
+    pulls = [(w, specs[w].n_links + a, (0.0, 0.0, 0.0), (35.0 * (1 + a), -20.0, 10.0)) for w in range(len(specs)) for a in (0, 1)]
+
+    def loads_at(s):
+        out = []
+        if s % 50 == 0:
+            out += wrench_process(specs, s // 50, 100.0, 600.0, seed_offset=5001)
+        if s == 20:
+            out += pulls
+        return out
+    res = _lockstep(sim, refs, specs, 150, loads_at)
+    print("lock-step with friction / reduced drag / rails:", {k: v for k, v in res.items() if k != "dist"})
+    assert res["events"] >= 8 and res["near"] <= 2, res
+    _assert_lockstep_bound(res)
+    st = sim.get_state_batch()
+    assert st["ruptured"].sum() >= 2 and st["attached"].sum() <= st["attached"].size - 4
+    # the detached, still pulled apples ride the rail: no faster than the limit (plus one step of gravity)
+    free = st["attached"] == 0
+    assert np.linalg.norm(st["apple_v"][free], axis=1).max() <= 3.0 + 0.05
+    rs = np.concatenate([sim.get_rupture_steps(w)[sim.get_state(w)["ruptured"] == 1] for w in range(len(specs))])
+    assert rs.size and (rs >= 0).all() and (rs < 150).all()
+    sim.close()
+
+
+def test_friction_and_rails_take_free_hinges_off_the_speed_clamp():
+    """What 8(f) item 1 is for ("some free twigs remain at the clamp"): the same violent run with
+    and without post-rupture friction; DoFs sitting on the qd_max clamp at the end are counted and reported."""
+    specs = make_config(5, 48)
+    counts = {}
+    for name, kw in (("off", {}), ("on", dict(fric_frac=0.02, mass_damping=0.5, snap_drag_scale=0.2, rail_speed=5.0))):
+        P = dataclasses.replace(config_params(5), **kw)
+        sim = ob.Orchard(specs, P)
+        sim.randomize(MASTER_SEED + 5002)
+        for epoch in range(8):
+            loads = wrench_process(specs, epoch, 100.0, 600.0, seed_offset=5002)
+            sim.apply_wrench_batch([l[0] for l in loads], [l[1] for l in loads], [l[2] for l in loads], [l[3] for l in loads])
+            sim.step(50)
+        st = sim.get_state_batch()
+        assert sim.stats()["n_flagged"] == 0 and np.isfinite(st["qd"]).all()
+        counts[name] = (int((np.abs(st["qd"]) >= 49.99).sum()), int(st["ruptured"].sum()))
+        sim.close()
+    print(f"DoFs on the 50 rad/s clamp after 400 steps (clamped, ruptured joints): without 8(f)1 {counts['off']}, with {counts['on']}")
+    assert counts["on"][0] <= counts["off"][0]
