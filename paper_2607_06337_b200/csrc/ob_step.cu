@@ -1547,12 +1547,13 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         const float fdet = s.afd[a];
         float3 ft = att ? f3(s.ft[a], s.ft[Ap + a], s.ft[2 * Ap + a]) : f3(0, 0, 0);
         float3 fu = f3(0, 0, 0);                                            // user force on the apple (wrench slots)
+        bool pulled = false;
         for (int k = 0; k < s.wr->n; k++)
-          if (s.wr->body[k] == N + a) fu = fu + f3(s.wr->force[k][0], s.wr->force[k][1], s.wr->force[k][2]);
+          if (s.wr->body[k] == N + a) { fu = fu + f3(s.wr->force[k][0], s.wr->force[k][1], s.wr->force[k][2]); pulled = true; }
         float3 va = f3(s.v[a], s.v[Ap + a], s.v[2 * Ap + a]);
         const float3 v0 = va;                                               // F = -c_v m v on the apple
         const float3 fraw = fu;                                             // the detach predicate counts the pull itself
-        fu = apply_rails(P, ma, v0, fu);                                    // an apple is a free body (A36)
+        if (pulled) fu = apply_rails(P, ma, v0, fu);                        // an apple is a free body (A36)
         va.x += P.h * (P.gravity[0] + (ft.x + fu.x) * inv_m - P.mass_damping * v0.x);
         va.y += P.h * (P.gravity[1] + (ft.y + fu.y) * inv_m - P.mass_damping * v0.y);
         va.z += P.h * (P.gravity[2] + (ft.z + fu.z) * inv_m - P.mass_damping * v0.z);
