@@ -441,7 +441,8 @@ __device__ __forceinline__ void link_joint(const int i, const Sm &s, const Gm &g
 // Coulomb friction at a ruptured joint ("introduced at the break and ramped up ~5x over ~1.5 s as the
 // torn fibres seize"; reading A34) as the damper D_f = T_f(t) / max(|qd|, v_eps) at the start-of-step joint speed,
 // T_f(t) = fric_frac M_max (1 + (fric_ramp - 1) min(t / fric_time, 1)), t = h (step - step of the rupture)
-__device__ __forceinline__ float friction_damper(const int i, const float2 w, const int step, const Gm &g, const ob_params &P) {
+// (out of line: cold unless fric_frac > 0 and the joint is ruptured)
+__device__ __noinline__ float friction_damper(const int i, const float2 w, const int step, const Gm &g, const ob_params &P) {
   const float t = P.h * (float)(step - __ldcg(g.rstep + i));
   const float ramp = P.fric_time > 0.f ? fminf(t / P.fric_time, 1.f) : 1.f;
   const float Tf = P.fric_frac * __ldg(g.Mmax + i) * (1.f + (P.fric_ramp - 1.f) * ramp);
@@ -452,7 +453,7 @@ __device__ __forceinline__ float friction_damper(const int i, const float2 w, co
 // instead of one per level of the sweep): the link's own inertia constants -> IN, (q, qd) -> XR, K -> PD.x (before
 // phase F: -> X21, because A1 publishes through PD and XR.xy).  Each sweep reads them at the link's own turn, before it
 // overwrites the slots with what it publishes.
-// The friction damper D_f of a ruptured joint goes with them (PD.y; before phase F: XR.z).
+// A ruptured joint has no K: its slot carries the friction damper D_f instead (split_kd sorts them out).
 __device__ __forceinline__ void stage_link_inputs(const int i, const Sm &s, const Gm &g, const bool state, const int step,
                                                   const ob_params &P) {
   float4 *rec = s.P + 7 * i;
@@ -462,15 +463,14 @@ __device__ __forceinline__ void stage_link_inputs(const int i, const Sm &s, cons
   const bool fric = (tw & kRuptured) && P.fric_frac > 0.f;
   float2 w = make_float2(0.f, 0.f);
   if (state || fric) w = __ldcg(g.w2 + i);
-  const float Df = fric ? friction_damper(i, w, step, g, P) : 0.f;
+  const float kd = (tw & kRuptured) ? (fric ? friction_damper(i, w, step, g, P) : 0.f) : Ki;
   if (state) {
     const float2 th = __ldcg(g.q2 + i);
     rec[kXR] = make_float4(th.x, th.y, w.x, w.y);
-    *reinterpret_cast<float2 *>(rec + kPD) = make_float2(Ki, Df);
+    rec[kPD].x = kd;
     if (tw & kHasApples) s.X21[i] = __int_as_float(__ldg(g.topo2 + i).x);   // first apple | count << 16
   } else {
-    s.X21[i] = Ki;
-    rec[kXR].z = Df;
+    s.X21[i] = kd;
   }
   rec[kIN] = c4;
 }
@@ -536,9 +536,9 @@ __device__ __forceinline__ void link_fk(const int i, const Sm &s, const Gm &g) {
 
 // diagonal terms of the two DoF of a joint: arm + h (c_d K + D_f) + h^2 K (Eq. 4; a ruptured joint has K = 0 and only the
 // post-rupture friction damper D_f, if any)
-__device__ __forceinline__ float2 diag_terms(const int i, const uint32_t tw, const float Ki, const float Df, const Sm &s,
-                                             const Gm &g, const ob_params &P) {
-  const float Kt = (tw & kRuptured) ? 0.f : Ki;
+__device__ __forceinline__ float2 diag_terms(const int i, const uint32_t tw, const float kd, const Sm &s, const Gm &g,
+                                             const ob_params &P) {
+  const float Kt = (tw & kRuptured) ? 0.f : kd, Df = (tw & kRuptured) ? kd : 0.f;   // staged: K, or D_f of a ruptured joint
   float dt0 = P.h * (P.c_d * Kt + Df) + P.h * P.h * Kt, dt1 = dt0;
   if (g.arm) {
     dt0 += __ldg(g.arm + i);
@@ -619,9 +619,9 @@ __device__ __forceinline__ void apple_forces(const int a, const Sm &s, const ob_
 // The three rails of PAPER.md:398 (App. B) on an applied force F on a FREE body of mass m moving with velocity v at the
 // application point (reading A36): power fade of the part of F along v between rail_fade v_lim and v_lim; impulse cap
 // |F| <= m max(v_lim - v . F^, 0) / h; speed brake - rail_brake m (|v| - v_lim) v^ above v_lim.
-__device__ __forceinline__ float3 apply_rails(const ob_params &P, const float m, const float3 v, float3 F) {
+// (out of line: the callers come here only with rail_speed > 0)
+__device__ __noinline__ float3 apply_rails(const ob_params &P, const float m, const float3 v, float3 F) {
   const float vl = P.rail_speed;
-  if (!(vl > 0.f)) return F;
   const float vn = sqrtf(dot(v, v));
   float3 vh = f3(0, 0, 0);
   if (vn > 0.f) {
@@ -653,7 +653,7 @@ __device__ __forceinline__ void wrench_forces(const int i, const uint32_t tw, co
     if ((tw & kSnapped) && P.forces_off_on_snapped) continue;
     float3 fl = rot_down(s.wq[q], f3(s.wr->force[q][0], s.wr->force[q][1], s.wr->force[q][2]));
     const float3 pt = f3(s.wr->point[q][0], s.wr->point[q][1], s.wr->point[q][2]);
-    if (tw & kSnapped) fl = apply_rails(P, m, vl + cross(om, pt), fl);   // all in link coordinates
+    if ((tw & kSnapped) && P.rail_speed > 0.f) fl = apply_rails(P, m, vl + cross(om, pt), fl);   // all in link coordinates
     f = f - fl;
     n = n - cross(pt, fl);
   }
@@ -664,16 +664,16 @@ __device__ __forceinline__ void wrench_forces(const int i, const uint32_t tw, co
 // (th, w, Ki, c4 = q, qd, K, inertia of the link: the caller loads them at the top of its turn, with its other global
 // inputs)
 __device__ __forceinline__ void finish_bias(const Jt &j, const int i, const float2 th, const float2 w, const float Ki,
-                                            const float Df, const float4 c4, float3 n, float3 f, const Sm &s,
-                                            const Gm &g, const DevCtx &c) {
+                                            const float4 c4, float3 n, float3 f, const Sm &s, const Gm &g,
+                                            const DevCtx &c) {
   const ob_params &P = c.P;
   float4 *rec = s.P + 7 * i;
   uint32_t tw = j.tw;
   // spring-damper part of the rhs and of the diagonal (Eq. 4); a ruptured joint has K = D = 0
-  const float Kt = (tw & kRuptured) ? 0.f : Ki, Dt = P.c_d * Kt + Df;
+  const float Kt = (tw & kRuptured) ? 0.f : Ki, Dt = P.c_d * Kt + ((tw & kRuptured) ? Ki : 0.f);   // Ki: K, or D_f (staged)
   const float2 kq = make_float2(Kt * th.x + (Dt + P.h * Kt) * w.x, Kt * th.y + (Dt + P.h * Kt) * w.y);
   reinterpret_cast<float2 *>(rec + kXR)[1] = make_float2(P.h * (-(j.c2 * n.x + j.s2 * n.z) - kq.x), P.h * (-n.y - kq.y));
-  reinterpret_cast<float2 *>(rec + kPD)[1] = diag_terms(i, tw, Ki, Df, s, g, P);
+  reinterpret_cast<float2 *>(rec + kPD)[1] = diag_terms(i, tw, Ki, s, g, P);
   rec[kIN] = eff_inertia(i, tw, c4, s, g, P);
   if (tw != j.tw) rec[kCS].w = __uint_as_float(tw);
   if (!(tw & kTrunk)) {
@@ -693,8 +693,7 @@ __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm
   float4 *rec = s.P + 7 * i;
   const float4 sq = rec[kXR], c4 = rec[kIN];                      // (q, qd), inertia, K: staged by the flat pass
   const float2 th = make_float2(sq.x, sq.y), w = make_float2(sq.z, sq.w);
-  const float2 kd = *reinterpret_cast<const float2 *>(rec + kPD);
-  const float Ki = kd.x, Df = kd.y;
+  const float Ki = rec[kPD].x;
   const Jt j = load_jt(s.P, i);
   const uint32_t tw = j.tw;
   float3 wp = f3(0, 0, 0), vp = f3(0, 0, 0), alp = f3(0, 0, 0);
@@ -725,20 +724,20 @@ __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm
   const float3 hf = f3(m * vl.x + mc * om.y, m * vl.y - mc * om.x, m * vl.z);
   n = n + cross(om, hn) + cross(vl, hf);
   f = f + cross(om, hf);
-  {                                       // velocity-proportional damping F = -c_v m v, tau = -c_omega I omega (
+  if (P.mass_damping != 0.f) {            // velocity-proportional damping F = -c_v m v, tau = -c_omega I omega (
     const float al_i = link_alpha(tw, P);   // A32, A35): minus alpha times the link's spatial momentum
     n = n + al_i * hn; f = f + al_i * hf;
   }
   wrench_forces(i, tw, c4.x, om, vl, s, P, n, f);
   if (inner) {                                                    // parked until B1 adds the children / the apples
-    const float2 dt = diag_terms(i, tw, Ki, Df, s, g, P);
+    const float2 dt = diag_terms(i, tw, Ki, s, g, P);
     rec[kXR] = make_float4(om.x, om.y, om.z, vl.x);
     rec[kIN] = make_float4(vl.y, vl.z, al.x, al.y);
     rec[kPD] = make_float4(al.z, aln.x, dt.x, dt.y);
     rec[kM0] = make_float4(n.x, n.y, n.z, f.x);
     rec[kM1] = make_float4(f.y, f.z, aln.y, aln.z);
   } else {
-    finish_bias(j, i, th, w, Ki, Df, c4, n, f, s, g, c);
+    finish_bias(j, i, th, w, Ki, c4, n, f, s, g, c);
   }
 }
 
@@ -746,8 +745,7 @@ __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm
 __device__ __forceinline__ void link_bias_up(const int i, const Jt &j, const Sm &s, const Gm &g, const DevCtx &c) {
   const float4 sq = s.P[7 * i + kXR], c4 = s.P[7 * i + kIN];     // staged by the flat pass between A2 and B1
   const float2 th = make_float2(sq.x, sq.y), w = make_float2(sq.z, sq.w);
-  const float2 kd = *reinterpret_cast<const float2 *>(s.P + 7 * i + kPD);
-  const float Ki = kd.x, Df = kd.y;
+  const float Ki = s.P[7 * i + kPD].x;
   const float4 u0 = s.P[7 * i + kM0];
   const float2 v0 = *reinterpret_cast<const float2 *>(s.P + 7 * i + kM1);
   float3 n = f3(u0.x, u0.y, u0.z), f = f3(u0.w, v0.x, v0.y);
@@ -759,7 +757,7 @@ __device__ __forceinline__ void link_bias_up(const int i, const Jt &j, const Sm 
       f = f - f3(s.aq[3 * Ap + a], s.hd[4 * Ap + a], s.hd[5 * Ap + a]);
     }
   }
-  finish_bias(j, i, th, w, Ki, Df, c4, n, f, s, g, c);
+  finish_bias(j, i, th, w, Ki, c4, n, f, s, g, c);
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -792,7 +790,7 @@ __device__ __noinline__ void factor_link(const int i, const World *wd, const Dev
   uint32_t tw = j.tw;
   const float Ki = s.X21[i];                                   // staged by the flat pass before the sweep
   const float4 eff = eff_inertia(i, tw, rec[kIN], s, g, P);
-  const float2 dt = diag_terms(i, tw, Ki, rec[kXR].z, s, g, P);
+  const float2 dt = diag_terms(i, tw, Ki, s, g, P);
   if (tw != j.tw) rec[kCS].w = __uint_as_float(tw);
   // own inertia: body of revolution about +z through the joint
   float A[9] = {eff.z, 0, 0, 0, eff.z, 0, 0, 0, eff.w};
@@ -893,7 +891,7 @@ __device__ __noinline__ void composite_link(const int i, const World *wd, const 
   const Jt j = load_jt(s.P, i);
   uint32_t tw = j.tw;
   float4 c4 = rec[kIN];                                        // staged by the flat pass before the sweep
-  const float2 dt = diag_terms(i, tw, s.X21[i], rec[kXR].z, s, g, P);
+  const float2 dt = diag_terms(i, tw, s.X21[i], s, g, P);
   {
     const float sc = 1.f + P.h * link_alpha(tw, P);
     c4.x *= sc; c4.y *= sc; c4.z *= sc; c4.w *= sc;
@@ -1553,7 +1551,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         float3 va = f3(s.v[a], s.v[Ap + a], s.v[2 * Ap + a]);
         const float3 v0 = va;                                               // F = -c_v m v on the apple
         const float3 fraw = fu;                                             // the detach predicate counts the pull itself
-        if (pulled) fu = apply_rails(P, ma, v0, fu);                        // an apple is a free body (A36)
+        if (pulled && P.rail_speed > 0.f) fu = apply_rails(P, ma, v0, fu);                        // an apple is a free body (A36)
         va.x += P.h * (P.gravity[0] + (ft.x + fu.x) * inv_m - P.mass_damping * v0.x);
         va.y += P.h * (P.gravity[1] + (ft.y + fu.y) * inv_m - P.mass_damping * v0.y);
         va.z += P.h * (P.gravity[2] + (ft.z + fu.z) * inv_m - P.mass_damping * v0.z);
