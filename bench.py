@@ -436,6 +436,53 @@ def _parity_sample(specs, P, seed, f_lo, f_hi, refs, n_steps) -> dict:
                         "is tests/test_gpu_parity.py)"}
 
 
+def run_cholesky_comparison(args):
+    """SURVEY.md 8(f) item 4, second half: a blocked-Cholesky GPU solve as a comparison point for the paper's "the
+    matrix-free CG solve is what makes laptop-scale batches practical" / "CG ~7x".  The LIBRARY's
+    batched blocked Cholesky (torch.linalg.cholesky + cholesky_solve: cuSOLVER / cuBLAS underneath) factors and solves
+    one SPD system of the size of every world of the batch (n = 2 x links, fp32, worlds grouped by n padded to 32),
+    which is what an assembled-matrix solver would do every step.  Only the factor + solve are timed: assembling the
+    matrix (n inverse-dynamics sweeps or a composite-rigid-body pass) is NOT counted, so the figure is an upper bound
+    on such a solver's step rate.  The matrices are random SPD of the right sizes: the time of a dense factorisation
+    does not depend on the entries."""
+    import torch
+    specs, P = _workload(args.config, args.worlds)
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    groups = {}
+    for sp in specs:
+        n = (2 * sp.n_links + 31) // 32 * 32
+        groups[n] = groups.get(n, 0) + 1
+    g = torch.Generator(device=dev).manual_seed(1)
+    mats = []
+    for n, cnt in sorted(groups.items()):
+        for b0 in range(0, cnt, 512):                                   # batches of <= 512 matrices: bounded memory
+            b = min(512, cnt - b0)
+            R = torch.randn(b, n, n, device=dev, generator=g) * (1.0 / math.sqrt(n))
+            A = R @ R.transpose(1, 2) + torch.eye(n, device=dev)
+            mats.append((A, torch.randn(b, n, 1, device=dev, generator=g)))
+    def once():
+        for A, rhs in mats:
+            L = torch.linalg.cholesky(A)
+            torch.cholesky_solve(rhs, L)
+    for _ in range(max(args.warmup, 1)):
+        once()
+    torch.cuda.synchronize()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    for _ in range(args.steps):
+        once()
+    t1.record()
+    torch.cuda.synchronize()
+    ms = t0.elapsed_time(t1) / args.steps
+    flop = sum(c * (n ** 3 / 3.0 + 2.0 * n * n) for n, c in groups.items())
+    line = {"comparison": "library batched blocked Cholesky (torch.linalg.cholesky + cholesky_solve), factor + solve only",
+            "workload": f"BASELINE.json configs[{args.config - 1}]: {len(specs)} systems, n = 2 x links "
+                        f"({min(groups)}-{max(groups)} after padding to 32), fp32, one factor + solve per world-step",
+            "value": len(specs) / (ms * 1e-3), "unit": UNIT + " (upper bound: assembly not counted)",
+            "ms_per_step_of_all_worlds": ms, "tflops": flop / (ms * 1e-3) / 1e12, "steps": args.steps}
+    print(json.dumps(line), flush=True)
+
+
 def run_reference(args, rank: int, world_size: int):
     """--impl reference: for this tier the reference arm is the oracle, timed as it stands on the host cores.
     Each bench step is a bounded sample of the workload (n_sample worlds x 1 physics step)."""
@@ -483,6 +530,8 @@ def main():
     ap.add_argument("--worlds", type=int, default=4096)
     ap.add_argument("--substeps", type=int, default=50, help="physics steps per bench step (one wrench epoch)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cholesky-comparison", action="store_true",
+                    help="time the library's batched blocked Cholesky on systems of the batch's sizes (SURVEY.md 8(f) item 4)")
     ap.add_argument("--geometry-dr", action="store_true",
                     help="per-world geometry randomization on the device before the run (SURVEY.md 8(f) item 3)")
     args = ap.parse_args()
@@ -490,7 +539,10 @@ def main():
         args.warmup = 3                                    # timing rule: at least 3 warm-up steps
     rank = int(os.environ.get("RANK", "0"))
     world_size = int(os.environ.get("WORLD_SIZE", "1"))
-    if args.impl == "reference":
+    if args.cholesky_comparison:
+        if rank == 0:
+            run_cholesky_comparison(args)
+    elif args.impl == "reference":
         run_reference(args, rank, world_size)
     else:
         run_cuda(args, rank, world_size)
