@@ -361,7 +361,8 @@ __device__ __forceinline__ float solve_down(const int i, float4 *P, const Sm &s,
   float4 *rec = P + 7 * i;
   const Jt j = load_jt(P, i);
   const float4 I = rec[kIN], pd = rec[kPD];
-  const float2 y = reinterpret_cast<const float2 *>(rec + kM1)[1];
+  const float4 m1 = rec[kM1];                                  // (128-bit accesses only: the 64-bit ones into the
+  const float2 y = make_float2(m1.z, m1.w);                    // 112-byte records are 2-way bank conflicted)
   const Kf k = load_kf(s, i, j, I, pd.z, pd.w);
   const float4 *par = P + 7 * (int)(j.tw & kParMask);
   const float4 u = par[kM0], v = par[kM1];
@@ -370,15 +371,15 @@ __device__ __forceinline__ float solve_down(const int i, float4 *P, const Sm &s,
   const float z0 = y.x - (dot(k.k1n, al) + dot(k.k1f, a)), z1 = y.y - (dot(k.k2n, al) + dot(k.k2f, a));
   al = al + f3(j.c2 * z0, z1, j.s2 * z0);
   if (FUSE) {
-    *reinterpret_cast<float2 *>(rec + kPD) = make_float2(z0, z1);
+    rec[kPD] = make_float4(z0, z1, pd.z, pd.w);
     if (turn) return mv_up<false>(j, P, P + 7 * s.Np, i, make_float4(z0, z1, pd.z, pd.w), al, a, s, g, c);
     rec[kM0] = make_float4(al.x, al.y, al.z, a.x);
-    *reinterpret_cast<float2 *>(rec + kM1) = make_float2(a.y, a.z);
+    rec[kM1] = make_float4(a.y, a.z, 0.f, 0.f);
   } else if ((j.tw >> kNcShift) & kNcMask) {
     rec[kM0] = make_float4(al.x, al.y, al.z, a.x);
     rec[kM1] = make_float4(a.y, a.z, z0, z1);
   } else {
-    reinterpret_cast<float2 *>(rec + kM1)[1] = make_float2(z0, z1);
+    rec[kM1] = make_float4(0.f, 0.f, z0, z1);
   }
   return 0.f;
 }
@@ -589,7 +590,7 @@ __device__ __forceinline__ void apple_forces(const int a, const Sm &s, const ob_
   }
   const float4 *rec = s.P + 7 * s.alnk[a];
   const float4 t0 = rec[kXR];
-  const float2 t1 = *reinterpret_cast<const float2 *>(rec + kIN);
+  const float4 t1 = rec[kIN];
   const float3 om = f3(t0.x, t0.y, t0.z), vl = f3(t0.w, t1.x, t1.y);
   const float4 qw = make_float4(s.aq[a], s.aq[Ap + a], s.aq[2 * Ap + a], s.aq[3 * Ap + a]);   // world rotation of the link
   const float3 o = f3(s.ao[a], s.ao[Ap + a], s.ao[2 * Ap + a]);
@@ -672,15 +673,18 @@ __device__ __forceinline__ void finish_bias(const Jt &j, const int i, const floa
   // spring-damper part of the rhs and of the diagonal (Eq. 4); a ruptured joint has K = D = 0
   const float Kt = (tw & kRuptured) ? 0.f : Ki, Dt = P.c_d * Kt + ((tw & kRuptured) ? Ki : 0.f);   // Ki: K, or D_f (staged)
   const float2 kq = make_float2(Kt * th.x + (Dt + P.h * Kt) * w.x, Kt * th.y + (Dt + P.h * Kt) * w.y);
-  reinterpret_cast<float2 *>(rec + kXR)[1] = make_float2(P.h * (-(j.c2 * n.x + j.s2 * n.z) - kq.x), P.h * (-n.y - kq.y));
-  reinterpret_cast<float2 *>(rec + kPD)[1] = diag_terms(i, tw, Ki, s, g, P);
+  rec[kXR] = make_float4(0.f, 0.f, P.h * (-(j.c2 * n.x + j.s2 * n.z) - kq.x), P.h * (-n.y - kq.y));
+  {
+    const float2 dt = diag_terms(i, tw, Ki, s, g, P);
+    rec[kPD] = make_float4(0.f, 0.f, dt.x, dt.y);
+  }
   rec[kIN] = eff_inertia(i, tw, c4, s, g, P);
   if (tw != j.tw) rec[kCS].w = __uint_as_float(tw);
   if (!(tw & kTrunk)) {
     float3 np, fp;
     force_up(j, n, f, np, fp);
     rec[kM0] = make_float4(np.x, np.y, np.z, fp.x);
-    *reinterpret_cast<float2 *>(rec + kM1) = make_float2(fp.y, fp.z);
+    rec[kM1] = make_float4(fp.y, fp.z, 0.f, 0.f);
   }
 }
 
@@ -701,9 +705,9 @@ __device__ __forceinline__ void link_bias(const int i, const World *wd, const Sm
   if (!(tw & kTrunk)) {
     const float4 *par = s.P + 7 * (int)(tw & kParMask);
     const float4 t0 = par[kXR], t1 = par[kIN];
-    const float2 t2 = *reinterpret_cast<const float2 *>(par + kPD), t3 = reinterpret_cast<const float2 *>(par + kM1)[1];
+    const float4 t2 = par[kPD], t3 = par[kM1];
     wp = f3(t0.x, t0.y, t0.z); vp = f3(t0.w, t1.x, t1.y);
-    alp = f3(t1.z, t1.w, t2.x); ap = f3(t2.y, t3.x, t3.y);
+    alp = f3(t1.z, t1.w, t2.x); ap = f3(t2.y, t3.z, t3.w);
   }
   const float c2 = j.c2, s2 = j.s2;
   const float3 vJ = f3(c2 * w.x, w.y, s2 * w.x);
@@ -747,7 +751,7 @@ __device__ __forceinline__ void link_bias_up(const int i, const Jt &j, const Sm 
   const float2 th = make_float2(sq.x, sq.y), w = make_float2(sq.z, sq.w);
   const float Ki = s.P[7 * i + kPD].x;
   const float4 u0 = s.P[7 * i + kM0];
-  const float2 v0 = *reinterpret_cast<const float2 *>(s.P + 7 * i + kM1);
+  const float4 v0 = s.P[7 * i + kM1];
   float3 n = f3(u0.x, u0.y, u0.z), f = f3(u0.w, v0.x, v0.y);
   gather_children(s.P, s.P + 7 * s.Np, (int)((j.tw >> kChShift) & kParMask), (int)((j.tw >> kNcShift) & kNcMask), n, f);
   if (j.tw & kHasApples) {                                  // the reactions of its apples, in apple order
@@ -1112,7 +1116,10 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
 #pragma unroll
     for (int k = 0; k < LPT; k++) {                 // first product: A x, i.e. p = x
       const int i = otid + k * NT;
-      if (i < N) *reinterpret_cast<float2 *>(PL + 7 * i + kPD) = *reinterpret_cast<const float2 *>(PL + 7 * i + kXR);
+      if (i < N) {
+        const float4 xr = PL[7 * i + kXR], pd = PL[7 * i + kPD];
+        PL[7 * i + kPD] = make_float4(xr.x, xr.y, pd.z, pd.w);
+      }
     }
     bool first = true, have_down = false;
     float rz = 0.f, rr = 0.f, pAp_carry = 0.f;
@@ -1148,7 +1155,7 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
         }
         if (lane < ntopN) {
           rec[kM0] = make_float4(al.x, al.y, al.z, a.x);
-          *reinterpret_cast<float2 *>(rec + kM1) = make_float2(a.y, a.z);
+          rec[kM1] = make_float4(a.y, a.z, 0.f, 0.f);
         }
       }
       __syncthreads();
@@ -1167,7 +1174,7 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
             pAp_part += mv_up<false>(j, PL, PL + 7 * Np, i, pd, al, a, s, g, c);
           } else {
             rec[kM0] = make_float4(al.x, al.y, al.z, a.x);
-            *reinterpret_cast<float2 *>(rec + kM1) = make_float2(a.y, a.z);
+            rec[kM1] = make_float4(a.y, a.z, 0.f, 0.f);
           }
         }
         __syncthreads();
@@ -1241,7 +1248,7 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
           uf.x = mine ? nuf.x : uf.x; uf.y = mine ? nuf.y : uf.y; uf.z = mine ? nuf.z : uf.z;
         }
         if (lane < ntopN) {
-          reinterpret_cast<float2 *>(rec + kM1)[1] = make_float2(t1, t2);
+          rec[kM1] = make_float4(v.x, v.y, t1, t2);
           pAp_part += pd.x * t1 + pd.y * t2;
         }
       }
@@ -1254,18 +1261,20 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
         const float pAp = red.sum(pAp_part, 0.f).x;
         alpha = rz / pAp;
       }
-      float2 z[LPT], pk[LPT];
+      float2 z[LPT], pk[LPT], dtk[LPT];
 #pragma unroll
       for (int k = 0; k < LPT; k++) {
         const int i = otid + k * NT;
-        z[k] = make_float2(0.f, 0.f); pk[k] = make_float2(0.f, 0.f);
+        z[k] = make_float2(0.f, 0.f); pk[k] = make_float2(0.f, 0.f); dtk[k] = make_float2(0.f, 0.f);
         if (i < N) {
-          const float2 ap = reinterpret_cast<const float2 *>(PL + 7 * i + kM1)[1];
+          const float4 m1 = PL[7 * i + kM1], pd = PL[7 * i + kPD];
+          const float2 ap = make_float2(m1.z, m1.w);
+          dtk[k] = make_float2(pd.z, pd.w);
           float4 xr = PL[7 * i + kXR];
           if (first) {                               // r = b - A x
             xr.z -= ap.x; xr.w -= ap.y;
           } else {
-            pk[k] = *reinterpret_cast<const float2 *>(PL + 7 * i + kPD);
+            pk[k] = make_float2(pd.x, pd.y);
             xr.x += alpha * pk[k].x; xr.y += alpha * pk[k].y;
             xr.z -= alpha * ap.x; xr.w -= alpha * ap.y;
           }
@@ -1298,9 +1307,9 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
         for (int k = 0; k < LPT; k++) {
           const int i = otid + k * NT;
           if (i < N) {
-            z[k] = have_down ? *reinterpret_cast<const float2 *>(PL + 7 * i + kPD) : reinterpret_cast<const float2 *>(PL + 7 * i + kM1)[1];
-            const float2 r = reinterpret_cast<const float2 *>(PL + 7 * i + kXR)[1];
-            rz_p += r.x * z[k].x + r.y * z[k].y;
+            const float4 zs = have_down ? PL[7 * i + kPD] : PL[7 * i + kM1], xr = PL[7 * i + kXR];
+            z[k] = have_down ? make_float2(zs.x, zs.y) : make_float2(zs.z, zs.w);
+            rz_p += xr.z * z[k].x + xr.w * z[k].y;
           }
         }
         rz_new = red.sum(rz_p, 0.f).x;
@@ -1312,7 +1321,7 @@ __device__ __noinline__ int pcg_solve(const World *wd, const DevCtx &c, float2 *
         for (int k = 0; k < LPT; k++) {
           const int i = otid + k * NT;
           if (i < N)
-            *reinterpret_cast<float2 *>(PL + 7 * i + kPD) = make_float2(z[k].x + beta * pk[k].x, z[k].y + beta * pk[k].y);
+            PL[7 * i + kPD] = make_float4(z[k].x + beta * pk[k].x, z[k].y + beta * pk[k].y, dtk[k].x, dtk[k].y);
         }
       }
       if (!first) it++;
@@ -1463,9 +1472,9 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         for (int k = 0; k < LPT; k++) {
           const int i = otid + k * NT;
           if (i < N) {
-            const float2 b = reinterpret_cast<const float2 *>(PL + 7 * i + kXR)[1];
-            *reinterpret_cast<float2 *>(PL + 7 * i + kXR) =
-                make_float2(OB_X0(h1[k].x, h2[k].x, h3[k].x, h4[k].x), OB_X0(h1[k].y, h2[k].y, h3[k].y, h4[k].y));
+            const float4 xb = PL[7 * i + kXR];
+            const float2 b = make_float2(xb.z, xb.w);
+            PL[7 * i + kXR] = make_float4(OB_X0(h1[k].x, h2[k].x, h3[k].x, h4[k].x), OB_X0(h1[k].y, h2[k].y, h3[k].y, h4[k].y), b.x, b.y);
             bb_part += b.x * b.x + b.y * b.y;
             if (d.precond == 1) {
               const float2 idg = s.IDG[i];
@@ -1490,7 +1499,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       for (int k = 0; k < LPT; k++) {
         const int i = otid + k * NT;
         if (i < N) {
-          const float2 x = *reinterpret_cast<const float2 *>(PL + 7 * i + kXR);
+          const float4 x = PL[7 * i + kXR];
           nf |= !(fabsf(x.x) < INFINITY) || !(fabsf(x.y) < INFINITY);
         }
       }
@@ -1514,7 +1523,8 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         const int i = otid + k * NT;
         if (i >= N) continue;
         const float2 w0 = dw0[k], q0 = dq0[k];
-        const float2 x = *reinterpret_cast<const float2 *>(PL + 7 * i + kXR);
+        const float4 x4 = PL[7 * i + kXR];
+        const float2 x = make_float2(x4.x, x4.y);
         g.hist[(step_now & 3) * (size_t)c.sum_np + i] = x;
         float wa = w0.x + x.x, wb = w0.y + x.y;
         if (P.qd_max > 0.f) {
