@@ -335,7 +335,7 @@ def run_cuda(args, rank: int, world_size: int):
                                  "peak_source": peaks["source"]}},
         }
         if world_size == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(specs, P, seed, f_lo, f_hi)
+            line["cpu_baseline"] = cpu_baseline(specs, P, seed, f_lo, f_hi, args.geometry_dr)
     if world_size > 1:
         dist.barrier()
         dist.destroy_process_group()
@@ -364,7 +364,7 @@ def _omp_threads() -> int:
     return max(1, n)
 
 
-def _oracle_sample(specs, P, seed, f_lo, f_hi, n_sample, solver=0):
+def _oracle_sample(specs, P, seed, f_lo, f_hi, n_sample, solver=0, geometry_dr=False):
     """Oracle worlds for the first n_sample worlds of the batch, randomized and loaded like the GPU run."""
     import oracle
     from workloads import wrench_process
@@ -373,12 +373,14 @@ def _oracle_sample(specs, P, seed, f_lo, f_hi, n_sample, solver=0):
     for w in range(n_sample):
         r = oracle.OracleWorld(specs[w], P, world_index=w, solver=solver)
         r.randomize(seed)
+        if geometry_dr:
+            r.randomize_geometry(seed + 9, **GEOMETRY_DR_RANGES)
         r.apply_wrench(loads[w][1], loads[w][2], loads[w][3])
         worlds.append(r)
     return worlds
 
 
-def cpu_baseline(specs, P, seed, f_lo, f_hi) -> dict:
+def cpu_baseline(specs, P, seed, f_lo, f_hi, geometry_dr=False) -> dict:
     """The fp64 oracle as it stands (brute-force mass matrix + dense Cholesky, OpenMP over worlds), timed on this
     box's host cores on a bounded sample of the same workload.  A reported baseline, not the target."""
     import oracle
@@ -386,7 +388,7 @@ def cpu_baseline(specs, P, seed, f_lo, f_hi) -> dict:
     os.environ.setdefault("OMP_NUM_THREADS", str(cores))
     n_sample = int(min(max(cores, 8), 64, len(specs)))
     n_steps = 8                                                  # ~1 s wall on 16 cores = 10-20 s of CPU work
-    worlds = _oracle_sample(specs, P, seed, f_lo, f_hi, n_sample)
+    worlds = _oracle_sample(specs, P, seed, f_lo, f_hi, n_sample, geometry_dr=geometry_dr)
     oracle.step_many(worlds, 1)                                  # warm-up (page-in, first-touch)
     t0 = time.perf_counter()
     oracle.step_many(worlds, n_steps)
@@ -396,18 +398,18 @@ def cpu_baseline(specs, P, seed, f_lo, f_hi) -> dict:
                      f"(fp64, mass matrix by unit-acceleration RNEA columns, dense Cholesky), {dt:.2f} s wall"}
     # the oracle's own fp64 Jacobi-PCG mode (same algorithm class as the GPU path; the matrix is still formed by
     # brute force) as the fairer CPU figure SURVEY.md 8(d) asks for
-    pw = _oracle_sample(specs, P, seed, f_lo, f_hi, n_sample, solver=1)
+    pw = _oracle_sample(specs, P, seed, f_lo, f_hi, n_sample, solver=1, geometry_dr=geometry_dr)
     oracle.step_many(pw, 1)
     t0 = time.perf_counter()
     oracle.step_many(pw, n_steps)
     dtp = time.perf_counter() - t0
     out["pcg_mode"] = {"value": n_sample * n_steps / dtp, "unit": UNIT,
                        "sample": f"same sample, oracle solver = fp64 Jacobi-PCG on the assembled matrix, {dtp:.2f} s wall"}
-    out["parity_sample"] = _parity_sample(specs, P, seed, f_lo, f_hi, worlds, 1 + n_steps)
+    out["parity_sample"] = _parity_sample(specs, P, seed, f_lo, f_hi, worlds, 1 + n_steps, geometry_dr)
     return out
 
 
-def _parity_sample(specs, P, seed, f_lo, f_hi, refs, n_steps) -> dict:
+def _parity_sample(specs, P, seed, f_lo, f_hi, refs, n_steps, geometry_dr=False) -> dict:
     """The sampled worlds once more on the GPU, free-running the same steps as the (Cholesky) oracle worlds `refs`:
     events on one side only, and the worst relative state error among the worlds without events."""
     import paper_2607_06337_b200 as ob
@@ -415,6 +417,8 @@ def _parity_sample(specs, P, seed, f_lo, f_hi, refs, n_steps) -> dict:
     n = len(refs)
     sim = ob.Orchard(specs[:n], P)
     sim.randomize(seed)
+    if geometry_dr:
+        sim.randomize_geometry(seed + 9, **GEOMETRY_DR_RANGES)
     loads = wrench_process(specs, 0, f_lo, f_hi)[:n]
     sim.apply_wrench_batch([l[0] for l in loads], [l[1] for l in loads], [l[2] for l in loads], [l[3] for l in loads])
     sim.step(n_steps)

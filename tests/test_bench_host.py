@@ -56,3 +56,12 @@ def test_reference_arm_two_ranks_prints_one_line():
     assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0
     assert d["cpu_baseline"]["kind"] == "oracle" and d["gpu_launches"] == 0
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["d2h_bytes_per_step"] == 0
+
+
+def test_committed_dram_profile_is_of_the_kernel_sources_as_they_are():
+    """bench.py reports roofline.traffic from profiles/r2_k_step_dram.txt only while that capture is of the CUDA
+    sources at HEAD (the file carries their hash): a stale profile would silently turn the field into null."""
+    import bench
+    assert bench._profiled_traffic(4096, 50) is not None, (
+        "profiles/r2_k_step_dram.txt is not of the kernel sources as they are (hash %s): re-capture it" % bench.kernel_source_hash())
+    assert bench._profiled_traffic(4096, 49) is None
