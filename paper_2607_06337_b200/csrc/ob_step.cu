@@ -609,19 +609,22 @@ __device__ __forceinline__ void apple_forces(const int a, const Sm &s, const ob_
   const float3 o = f3(s.ao[a], s.ao[Ap + a], s.ao[2 * Ap + a]);
   const float ks = s.ak[a], cdamp = s.ac[a], ma = s.am[a];
   const float eta_h = P.tether_implicit ? P.h : 0.f;
-  // x_a - x_hang = (anchor - x_hang) + sag + u: the apple is stored as u = x_a - (anchor + sag), sag = m g / k_s,
-  // and phase A1 left anchor - x_hang in fp64 (as two floats)
-  const double mk = (double)(ma / ks);                     // sag = (m / k_s) g: ~1e-3 m, so fp32's 6e-8 is 1e-10 m
-  const float3 st = f3((float)(join2(s.hd[a], s.hd[Ap + a]) + mk * (double)P.gravity[0] + (double)s.u[a]),
-                       (float)(join2(s.hd[2 * Ap + a], s.hd[3 * Ap + a]) + mk * (double)P.gravity[1] + (double)s.u[Ap + a]),
-                       (float)(join2(s.hd[4 * Ap + a], s.hd[5 * Ap + a]) + mk * (double)P.gravity[2] + (double)s.u[2 * Ap + a]));
+  // x_a - x_hang = (anchor - x_hang) + sag + u: the apple is stored as u = x_a - (anchor + sag), sag = m g / k_s, and
+  // phase A1 left anchor - x_hang in fp64 (as two floats).  At rest the spring force k_s sag and the weight m g cancel:
+  // they are never formed.  With du = (anchor - x_hang) + u (millimetres), exactly:
+  //   f_s = -k_s du - m g,   f_react = k_s (du - eta h v_hang)   (Eq. 7: the weight drops out),
+  //   apple: g + (f_s - c_s v) / m = (-k_s du - c_s v) / m        (phase D adds the user force and integrates)
+  // so a settled tree sees rounding of the small deviations only, not of two 2 N forces that cancel.
+  const float3 du = f3((float)(join2(s.hd[a], s.hd[Ap + a]) + (double)s.u[a]),
+                       (float)(join2(s.hd[2 * Ap + a], s.hd[3 * Ap + a]) + (double)s.u[Ap + a]),
+                       (float)(join2(s.hd[4 * Ap + a], s.hd[5 * Ap + a]) + (double)s.u[2 * Ap + a]));
   const float3 vh = rot_up(qw, vl + cross(om, o));                      // world velocity of the hang point
-  const float3 fs = (-ks) * st;
+  const float3 fe = (-ks) * du;                                          // elastic force beyond the rest sag
+  const float3 fs = f3(fe.x - ma * P.gravity[0], fe.y - ma * P.gravity[1], fe.z - ma * P.gravity[2]);
   const float3 va = f3(s.v[a], s.v[Ap + a], s.v[2 * Ap + a]);
-  s.ft[a] = fs.x - cdamp * va.x; s.ft[Ap + a] = fs.y - cdamp * va.y; s.ft[2 * Ap + a] = fs.z - cdamp * va.z;
+  s.ft[a] = fe.x - cdamp * va.x; s.ft[Ap + a] = fe.y - cdamp * va.y; s.ft[2 * Ap + a] = fe.z - cdamp * va.z;
   s.fsn[a] = sqrtf(dot(fs, fs));
-  float3 fr = f3(ks * (st.x - eta_h * vh.x) - ma * P.gravity[0], ks * (st.y - eta_h * vh.y) - ma * P.gravity[1],
-                 ks * (st.z - eta_h * vh.z) - ma * P.gravity[2]);
+  float3 fr = f3(ks * (du.x - eta_h * vh.x), ks * (du.y - eta_h * vh.y), ks * (du.z - eta_h * vh.z));
   const float nr = sqrtf(dot(fr, fr));
   if (nr > P.react_max) fr = (P.react_max / nr) * fr;                   // clamp
   const float3 fl = rot_down(qw, fr);
@@ -1567,7 +1570,9 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         const bool att = s.att[a] != 0;
         const float ma = s.am[a], inv_m = 1.f / ma;
         const float fdet = s.afd[a];
-        float3 ft = att ? f3(s.ft[a], s.ft[Ap + a], s.ft[2 * Ap + a]) : f3(0, 0, 0);
+        // attached: tether force beyond the rest sag (the sag carries the weight: no gravity term); detached: gravity
+        const float3 ft = att ? f3(s.ft[a], s.ft[Ap + a], s.ft[2 * Ap + a]) : f3(0, 0, 0);
+        const float3 ga = att ? f3(0, 0, 0) : f3(P.gravity[0], P.gravity[1], P.gravity[2]);
         float3 fu = f3(0, 0, 0);                                            // user force on the apple (wrench slots)
         bool pulled = false;
         for (int k = 0; k < s.wr->n; k++)
@@ -1576,9 +1581,9 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
         const float3 v0 = va;                                               // F = -c_v m v on the apple
         const float3 fraw = fu;                                             // the detach predicate counts the pull itself
         if (pulled && P.rail_speed > 0.f) fu = apply_rails(P, ma, v0, fu);                        // an apple is a free body (A36)
-        va.x += P.h * (P.gravity[0] + (ft.x + fu.x) * inv_m - P.mass_damping * v0.x);
-        va.y += P.h * (P.gravity[1] + (ft.y + fu.y) * inv_m - P.mass_damping * v0.y);
-        va.z += P.h * (P.gravity[2] + (ft.z + fu.z) * inv_m - P.mass_damping * v0.z);
+        va.x += P.h * (ga.x + (ft.x + fu.x) * inv_m - P.mass_damping * v0.x);
+        va.y += P.h * (ga.y + (ft.y + fu.y) * inv_m - P.mass_damping * v0.y);
+        va.z += P.h * (ga.z + (ft.z + fu.z) * inv_m - P.mass_damping * v0.z);
         s.v[a] = va.x; s.v[Ap + a] = va.y; s.v[2 * Ap + a] = va.z;
         s.u[a] = fmaf(P.h, va.x, s.u[a]); s.u[Ap + a] = fmaf(P.h, va.y, s.u[Ap + a]);
         s.u[2 * Ap + a] = fmaf(P.h, va.z, s.u[2 * Ap + a]);

@@ -335,7 +335,7 @@ def _masked_qd_error(g, o, keep):
     return float(np.linalg.norm(d) / den)
 
 
-def _lockstep(sim, refs, specs, n_steps, loads_at, on_step=None):
+def _lockstep(sim, refs, specs, n_steps, loads_at, on_step=None, check=None):
     """Every step: oracle <- GPU state and counters; both advance one step; flags, counters and events of
     that step must agree.  A one-sided predicate decision is tolerated only within NEAR of its threshold, and only
     for THAT (world, kind, index) in THAT step: every other event key of the step must match, with value within
@@ -368,6 +368,8 @@ def _lockstep(sim, refs, specs, n_steps, loads_at, on_step=None):
             if g["status"] & ob.OB_STATUS_NONFINITE:
                 raise AssertionError(f"world {w} went non-finite at step {s}")
             errs.append(e["max"])
+            if check is not None:
+                check(s, w, e, g, o)
             # the same error without the speeds of ruptured joints (free hinges of gram-scale twigs: joint inertia
             # ~1e-7 kg m^2, the system is ill-conditioned in exactly that DoF)
             keep = ~np.repeat(o["ruptured"].astype(bool), 2)
@@ -1020,3 +1022,88 @@ def test_friction_and_rails_take_free_hinges_off_the_speed_clamp():
         sim.close()
     print(f"DoFs on the 50 rad/s clamp after 400 steps (clamped, ruptured joints): without 8(f)1 {counts['off']}, with {counts['on']}")
     assert counts["on"][0] <= counts["off"][0]
+
+
+# ----------------------------------------------------------------------------------------------------
+# configs[1] on its own schedule, configs[2] at its own size
+# ----------------------------------------------------------------------------------------------------
+def test_config2_schedule_settle_then_pulls():
+    """configs[1]'s schedule (h = 2 ms; gravity only, then constant pulls U(0,40) N on five apples per world from step
+    500 on) on eight worlds of its generator: both sides settle freely for 480 steps (compared after 200 and after
+    480: no event may fire under gravity alone), then lock-step through the onset of the pulls (every pull above
+    f_detach must detach its apple after exactly three steps)."""
+    specs = make_config(2, 8)
+    P = config_params(2)
+    sim, refs = _make(specs, P, seed=MASTER_SEED + 2000)
+    sim.step(200)
+    oracle.step_many(refs, 200)
+    for w, r in enumerate(refs):
+        e, g, o = _err(sim, r, w)
+        assert e["max"] <= TOL_RUN, (w, e)
+    sim.step(280)
+    oracle.step_many(refs, 280)
+    assert not sim.events() and not any(r.events() for r in refs)
+    worst = max(_err(sim, r, w)[0]["max"] for w, r in enumerate(refs))
+    print(f"config 2: relative state error after 480 free steps {worst:.2e}")
+    assert worst <= 5 * TOL_RUN
+    pulls = config2_pulls(specs)
+    # A settled tree is the one regime where the velocity block cannot meet 1e-5 RELATIVE in fp32: the right-hand side
+    # is the difference of the gravity and the spring torque, each rounded at eps K |theta|, and the step divides by
+    # (h c_d + h^2) K, so every joint speed carries eps |theta| / (c_d + h) ~ 2e-7 rad/s of noise whatever the motion
+    # (DESIGN.md section 5).  Here |qd| ~ 2e-3 rad/s, so the check is: q, x, v within 1e-5, and qd within
+    # 1e-5 |qd| + 8 eps |theta|_2 / (c_d + h)  (a handful of roundings of K |theta|-sized quantities per joint).
+    eps32, cdh = 2.0 ** -24, float(np.float32(P.c_d)) + float(np.float32(P.h))
+    ratios = []
+
+    def check(s_, w, e, g, o):
+        assert max(e["q"], e["apple_x"], e["apple_v"]) <= TOL_STEP, (s_, w, e)
+        dq = np.linalg.norm(g["qd"].astype(np.float64) - o["qd"])
+        bound = TOL_STEP * max(np.linalg.norm(o["qd"]), 1e-4 * np.sqrt(o["qd"].size)) + 8.0 * eps32 * np.linalg.norm(o["q"]) / cdh
+        ratios.append(dq / bound)
+        assert dq <= bound, (s_, w, dq, bound, e)
+    res = _lockstep(sim, refs, specs, 60, lambda s: pulls if s == 20 else [], check=check)   # steps 480..539, pulls at 500
+    print(f"config 2 lock-step: velocity error / (1e-5 |qd| + fp32 floor): median {np.median(ratios):.2f}, max {max(ratios):.2f}")
+    mats = [r.material() for r in refs]
+    expect = {(w, 502, 1, body - specs[w].n_links) for (w, body, _p, f) in pulls
+              if np.linalg.norm(np.float32(f)) > np.float32(mats[w]["detach"][body - specs[w].n_links])}
+    assert res["near"] == 0 and res["events"] >= len(expect) >= 1, (res, expect)
+    st = sim.get_state_batch()
+    ao = np.cumsum([0] + sim.n_apples)
+    for (w, _s, _k, a) in expect:
+        assert st["attached"][ao[w] + a] == 0
+    assert (st["info"][:, 0] == 540).all()
+    sim.close()
+
+
+def test_full_size_config3_sampled_worlds_and_invariants():
+    """configs[2] at its own size (1024 worlds, h = 2 ms): every Philox draw, invariants on all worlds, sampled worlds
+    against the oracle over the first 20 steps of the wrench process."""
+    specs = make_config(3, 1024)
+    P = config_params(3)
+    seed = MASTER_SEED + 3000
+    sim = ob.Orchard(specs, P)
+    sim.randomize(seed)
+    loads = wrench_process(specs, 0, 0.0, 150.0)
+    sim.apply_wrench_batch([l[0] for l in loads], [l[1] for l in loads], [l[2] for l in loads], [l[3] for l in loads])
+    sim.step(20)
+    st = sim.stats()
+    assert st["world_steps_total"] == 20 * len(specs) and st["n_flagged"] == 0
+    _check_all_philox_draws(sim, specs, P, seed)
+    full = sim.get_state_batch()
+    assert (full["info"][:, 0] == 20).all() and np.isfinite(full["q"]).all() and np.isfinite(full["apple_x64"]).all()
+    sample = [0, 255, 640, 1023]
+    refs = {w: oracle.OracleWorld(specs[w], P, world_index=w) for w in sample}
+    for w, r in refs.items():
+        r.randomize(seed)
+        r._x_rest = r.get_state()["apple_x"].copy()
+        r.apply_wrench(loads[w][1], loads[w][2], loads[w][3])
+    oracle.step_many(list(refs.values()), 20)
+    gev = {}
+    for e in sim.events():
+        gev.setdefault(e[0], []).append(_key(e))
+    for w, r in refs.items():
+        e, g, o = _err(sim, r, w)
+        assert gev.get(w, []) == [_key(x) for x in r.events()]
+        if not gev.get(w):
+            assert e["max"] <= TOL_RUN, (w, e)
+    sim.close()
