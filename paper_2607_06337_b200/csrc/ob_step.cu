@@ -75,7 +75,8 @@ struct Sm {
   unsigned char *att, *cA, *cB;
   float *ao, *ak, *am, *ac, *afd;     // ao = [3][Ap]
   const int *alnk;                    // [Ap] internal index of the link that carries the apple
-  float *ft, *fsn;                    // tether force [3][Ap], |f_s| [Ap] (phase A2 -> phase D)
+  float *ft, *fsn;                    // tether force on the apple beyond its rest sag [3][Ap] (-k_s du - c_s v: the sag carries
+                                      // the weight), |f_s| [Ap] (apple pass -> phase D)
   float *hd;                          // [6][Ap] anchor - x_hang of every apple, fp64 as (hi, lo) pairs (phase A1 -> apple
                                       // pass); aliases ft, fsn (see carve)
   float *aq;                          // [4][Ap] world quaternion (fp32) of the apple's link (phase A1 -> apple pass); then,
