@@ -286,6 +286,29 @@ int ob_sizeof_geometry_ranges(void);
 int ob_selftest_philox(int n, const uint32_t *ctr, const uint32_t *key, uint32_t *out_lib, uint32_t *out_curand,
                        void *dev_scratch, void *cuda_stream);
 
+/* The same self-test for a caller that cannot supply dev_scratch.  Some code that wants to run this check has no way
+   to obtain device memory: a plug-in inside a host application whose pool allocator has already claimed the whole GPU
+   and forbids driver allocations behind its back, a start-up health probe that runs before any allocator exists, or a
+   thread for which cudaMalloc / cudaFree are off limits because they synchronise the device or would break a stream
+   capture under way elsewhere in the process.  For them the staging area is a fixed array inside libob.so itself.
+   Cost: OB_SELFTEST_STATIC_MAX * 56 bytes = 224 KB of device memory on every GPU that loads the library, held until
+   the process exits.  Limit: n <= OB_SELFTEST_STATIC_MAX; a larger n returns OB_E_CAPACITY (ob_last_error(NULL) says
+   so) before anything touches the GPU -- split the pairs over several calls, or use ob_selftest_philox.
+   Arguments and results as ob_selftest_philox (host arrays ctr [4n], key [2n] in, out_lib / out_curand [4n] out,
+   all owned by the caller; the results are bit-identical to ob_selftest_philox's).  cuda_stream must belong to the
+   device that is current on the calling thread; the work is enqueued on it and the call synchronises it.
+   The call allocates nothing on the device or through the CUDA runtime: no cudaMalloc, cudaFree, cudaMallocHost or
+   library routine that allocates; it copies directly between the caller's host arrays and the static array.
+   First call on each device: it looks up the device address of the static array (one cudaGetSymbolAddress, checked,
+   with that device current) and remembers it; make that first call before starting any stream capture.
+   Sharing: every call on a device uses the same array, and the array keeps the previous call's contents.  Nothing in
+   it has to start at zero (each call copies its inputs in and the kernel overwrites all 8n result words before they
+   are read back), so no clearing is done; but two calls that overlap on the same GPU (two host threads, two streams)
+   race on it and return garbage: serialise them.  Returns OB_E_ARG (null, n < 1), OB_E_CAPACITY, OB_E_CUDA. */
+#define OB_SELFTEST_STATIC_MAX 4096
+int ob_selftest_philox_static(int n, const uint32_t *ctr, const uint32_t *key, uint32_t *out_lib,
+                              uint32_t *out_curand, void *cuda_stream);
+
 const char *ob_last_error(const ob_ctx *ctx);
 void ob_destroy(ob_ctx *ctx);
 

@@ -25,7 +25,7 @@ EXPORTS = [
     "ob_selftest_philox", "ob_get_state_batch", "ob_set_apple_x64", "ob_set_step", "ob_get_counters_batch",
     "ob_get_material_batch", "ob_world_blob_bytes", "ob_save_world", "ob_load_world", "ob_iter_histogram",
     "ob_randomize_geometry", "ob_get_geometry", "ob_sizeof_geometry_ranges", "ob_get_rupture_steps",
-    "ob_set_rupture_steps",
+    "ob_set_rupture_steps", "ob_selftest_philox_static",
 ]
 
 
@@ -112,6 +112,8 @@ def load_library():
         L.ob_stats.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_int32)]
         L.ob_launch_info.argtypes = [vp] + [C.POINTER(C.c_int32)] * 4
         L.ob_counters.argtypes = [vp, C.POINTER(C.c_uint64 * 4)]
+        L.ob_selftest_philox.argtypes = [i32] + [vp] * 6
+        L.ob_selftest_philox_static.argtypes = [i32] + [vp] * 5
         L.ob_last_error.argtypes = [vp]
         L.ob_last_error.restype = C.c_char_p
         L.ob_destroy.argtypes = [vp]

@@ -1206,6 +1206,23 @@ int ob_selftest_philox(int n, const uint32_t *ctr, const uint32_t *key, uint32_t
   return OB_OK;
 }
 
+// ob_selftest_philox without any allocation: the staging area is the static device array of ob_kernels.cu, which is
+// also where the set-up (cudaGetSymbolAddress, once per device) and the launch live.  Sizes are checked here, before
+// the GPU is touched.
+int ob_selftest_philox_static(int n, const uint32_t *ctr, const uint32_t *key, uint32_t *out_lib, uint32_t *out_curand,
+                              void *cuda_stream) {
+  if (n < 1 || !ctr || !key || !out_lib || !out_curand) return fail0(OB_E_ARG, "ob_selftest_philox_static: null or empty");
+  if (n > OB_SELFTEST_STATIC_MAX) {
+    char b[160];
+    snprintf(b, sizeof(b), "ob_selftest_philox_static: n = %d exceeds the static scratch (OB_SELFTEST_STATIC_MAX = %d pairs); "
+             "split the call or use ob_selftest_philox", n, OB_SELFTEST_STATIC_MAX);
+    return fail0(OB_E_CAPACITY, b);
+  }
+  cudaError_t e = philox_selftest_static(n, ctr, key, out_lib, out_curand, (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return fail0(OB_E_CUDA, cudaGetErrorString(e));
+  return OB_OK;
+}
+
 const char *ob_last_error(const ob_ctx *ctx) { return ctx ? ctx->err.c_str() : (g_err.empty() ? kNullCtx : g_err.c_str()); }
 
 void ob_destroy(ob_ctx *ctx) {

@@ -169,6 +169,9 @@ cudaError_t launch_stats(const DevCtx &c, cudaStream_t s);
 cudaError_t launch_geometry(const DevCtx &c, unsigned long long seed, const ob_geometry_ranges &r, cudaStream_t s);
 cudaError_t launch_anchors(const DevCtx &c, cudaStream_t s);
 cudaError_t launch_philox_selftest(int n, const uint32_t *d_in, uint32_t *d_out, cudaStream_t s);
+// the self-test on the library's own static scratch (no allocation anywhere); n <= OB_SELFTEST_STATIC_MAX, synchronises s
+cudaError_t philox_selftest_static(int n, const uint32_t *ctr, const uint32_t *key, uint32_t *out_lib,
+                                   uint32_t *out_curand, cudaStream_t s);
 cudaError_t step_kernel_setup(int cls, int smem_bytes, int *max_blocks_per_sm);
 
 }  // namespace ob

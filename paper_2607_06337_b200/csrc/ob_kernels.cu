@@ -10,6 +10,8 @@
 // coordinates to link coordinates; the joint sits at r = (0,0,L_parent) in the parent frame.
 #include <math.h>
 
+#include <mutex>
+
 #include "ob_device.h"
 #include "ob_internal.h"
 
@@ -389,6 +391,75 @@ __global__ void k_philox_selftest(int n, const uint32_t *__restrict__ in, uint32
 cudaError_t launch_philox_selftest(int n, const uint32_t *d_in, uint32_t *d_out, cudaStream_t s) {
   k_philox_selftest<<<(n + 127) / 128, 128, 0, s>>>(n, d_in, d_out);
   return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------
+// The same self-test for callers that have no device memory to lend and may not ask the driver for any
+// (ob_selftest_philox_static in include/orchard.h).  Its staging area is the file-scope array below: 224 KB that
+// every GPU which loads libob.so holds from module load until the process exits.  All calls on one device share
+// it and it keeps whatever the previous call left there; the kernel overwrites all 8n output words of a call and
+// the inputs are copied in first, so nothing has to start at zero -- but two calls that overlap on the GPU race.
+//
+// g_selftest_scratch is a device symbol.  In host code that name is only the host-side stand-in of the symbol, not
+// an address a kernel can use, so the host asks the runtime for the device address (once per device, with that
+// device current) and hands the kernel that pointer.
+// ------------------------------------------------------------------------------------------------------
+static __device__ __align__(256) uint32_t g_selftest_scratch[14 * OB_SELFTEST_STATIC_MAX];
+
+// layout of the scratch for n pairs: ctr [4n] | key [2n] | library output [4n] | cuRAND output [4n]
+__global__ void k_philox_selftest_static(int n, uint32_t *__restrict__ scratch) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t *ctr_in = scratch, *key_in = scratch + 4 * (size_t)n;
+  uint32_t *out_lib = scratch + 6 * (size_t)n, *out_cur = scratch + 10 * (size_t)n;
+  const uint4 ctr = make_uint4(ctr_in[4 * i], ctr_in[4 * i + 1], ctr_in[4 * i + 2], ctr_in[4 * i + 3]);
+  const uint2 key = make_uint2(key_in[2 * i], key_in[2 * i + 1]);
+  const uint4 a = philox4x32_10(ctr, key);
+  const uint4 b = curand_Philox4x32_10(ctr, key);
+  out_lib[4 * i] = a.x; out_lib[4 * i + 1] = a.y; out_lib[4 * i + 2] = a.z; out_lib[4 * i + 3] = a.w;
+  out_cur[4 * i] = b.x; out_cur[4 * i + 1] = b.y; out_cur[4 * i + 2] = b.z; out_cur[4 * i + 3] = b.w;
+}
+
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_scratch_mutex;
+uint32_t *g_scratch_addr[kMaxDevices];   // device address of g_selftest_scratch on device d, 0 = not looked up yet
+}  // namespace
+
+// Device address of the static scratch on the CURRENT device; the first call on a device does the look-up.
+static cudaError_t selftest_scratch_address(uint32_t **out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_scratch_mutex);
+  if (!g_scratch_addr[dev]) {
+    void *p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_selftest_scratch);
+    if (e != cudaSuccess) return e;
+    if (!p) return cudaErrorInvalidSymbol;
+    g_scratch_addr[dev] = static_cast<uint32_t *>(p);
+  }
+  *out = g_scratch_addr[dev];
+  return cudaSuccess;
+}
+
+// Copies straight from / to the caller's host arrays (no host staging buffer either); synchronises s.
+cudaError_t philox_selftest_static(int n, const uint32_t *ctr, const uint32_t *key, uint32_t *out_lib,
+                                   uint32_t *out_curand, cudaStream_t s) {
+  uint32_t *d = nullptr;
+  cudaError_t e = selftest_scratch_address(&d);
+  if (e != cudaSuccess) return e;
+  const size_t N = (size_t)n;
+  e = cudaMemcpyAsync(d, ctr, 16 * N, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d + 4 * N, key, 8 * N, cudaMemcpyHostToDevice, s);
+  if (e != cudaSuccess) return e;
+  k_philox_selftest_static<<<(n + 127) / 128, 128, 0, s>>>(n, d);
+  e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaMemcpyAsync(out_lib, d + 6 * N, 16 * N, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(out_curand, d + 10 * N, 16 * N, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  return e;
 }
 
 }  // namespace ob
