@@ -1070,3 +1070,194 @@ def test_force_rails_on_a_free_apple_and_never_on_static_loading():
     w.step(4)
     ev = w.events()
     assert len(ev) == 1 and ev[0][1:4] == (2, 1, 2) and ev[0][4] == 25.0
+
+
+# ---------------------------------------------------------------- round 3: the hysteresis resets, snapped sub-trees, the order of the
+# updates inside a step, the absolute-velocity damper (the seven one-line mutants of round 2's review that survived)
+def _pinned_link(nr, **kw):
+    """One link whose joint an armature of 1e9 kg m^2 holds in place: q is whatever set_state puts there."""
+    spec = chain_spec(1, 0.5, 0.02, armature=np.full((1, 2), 1e9, dtype=np.float32))
+    d, L = float(spec.diameter[0]), float(spec.length[0])
+    Mmax, K = 60e6 * math.pi * d ** 3 / 32, 8e9 * math.pi * d ** 4 / (64 * L)
+    return spec, OracleWorld(spec, Params(gravity=(0, 0, 0), rupture_frames=nr, **kw)), Mmax / K
+
+
+def test_rupture_counter_resets_on_a_miss():
+    """PAPER.md:139 "N-frame hysteresis", reading A7: the N_r steps above M_max must be CONSECUTIVE.  Above for
+    N_r - 1 steps, one step below, above again: the joint ruptures N_r steps after the SECOND crossing.
+    (Perturbation this fails on: the counter kept, or merely not incremented, on a miss -- fires at step 3.)"""
+    nr = 3
+    spec, w, th = _pinned_link(nr)
+    hi, lo = [0.6 * 1.01 * th, 0.8 * 1.01 * th], [0.6 * 0.99 * th, 0.8 * 0.99 * th]
+    w.set_state(q=hi); w.step(nr - 1)                       # steps 0, 1: above
+    assert w.get_counters()[0][0] == nr - 1
+    w.set_state(q=lo); w.step(1)                            # step 2: below
+    assert w.get_counters()[0][0] == 0 and w.events() == []
+    w.set_state(q=hi); w.step(nr - 1)                       # steps 3, 4: above, not yet N_r in a row
+    assert w.events() == [] and w.get_state()["ruptured"][0] == 0
+    w.step(1)                                               # step 5
+    ev = w.events()
+    assert len(ev) == 1 and ev[0][1:4] == (nr - 1 + 1 + nr - 1, 0, 0)
+    assert w.get_state()["ruptured"][0] == 1
+
+
+def _apple_on_a_pinned_link(**kw):
+    mA, ks, fdet = 0.2, 2e3, 20.0
+    spec = chain_spec(1, 0.5, 0.08, apples=[(0, (0, 0, 0.5), mA, ks, fdet)], armature=np.full((1, 2), 1e9, dtype=np.float32))
+    return spec, OracleWorld(spec, Params(**kw)), mA, ks, fdet, np.array([0.0, 0.0, 0.5])
+
+
+def test_pull_counter_resets_on_a_miss():
+    """PAPER.md:163 "sustained for a few frames", reading A14, path A: pull above f_detach for 2 steps, 1 step below,
+    then above: the apple detaches N_A = 3 steps after the SECOND onset, with value |f_user| and threshold f_detach.
+    (Perturbation this fails on: c_A not reset on a miss -- detaches at step 3.)"""
+    spec, w, mA, ks, fdet, _ = _apple_on_a_pinned_link(detach_frames_pull=3, detach_frames_tension=10 ** 6)
+    pattern = [1.5, 1.5, 0.5, 1.5, 1.5, 1.5, 1.5]
+    fired = []
+    for s, f in enumerate(pattern):
+        w.apply_wrench(1, (0, 0, 0), (0.6 * f * fdet, 0.0, -0.8 * f * fdet))
+        w.step(1)
+        fired += w.events()
+        if s == 2:
+            assert w.get_counters()[1][0] == 0
+    assert len(fired) == 1 and fired[0][1:4] == (5, 1, 0)
+    assert abs(fired[0][4] - 1.5 * fdet) < 1e-5 and abs(fired[0][5] - fdet) < 1e-9
+
+
+def test_tension_counter_resets_on_a_miss():
+    """Reading A14, path B: |f_s| = k_s |x - x_hang| above kappa f_detach for 9 steps, 1 step below, then above:
+    detach N_B = 10 steps after the second onset (step 19), value k_s |x - x_hang|, threshold kappa f_detach.  The
+    stretch is imposed through set_state before every step (which leaves the counters alone).
+    (Perturbation this fails on: c_B not reset on a miss -- detaches at step 10.)"""
+    spec, w, mA, ks, fdet, xh = _apple_on_a_pinned_link(detach_frames_pull=10 ** 6, detach_frames_tension=10)
+    kap = float(np.float32(1.1))
+    s_hi, s_lo = 1.2 * kap * fdet / ks, 0.5 * kap * fdet / ks
+    fired = []
+    for s in range(24):
+        st = s_lo if s == 9 else s_hi
+        w.set_state(apple_x=[xh + st * np.array([0.0, 0.6, -0.8])], apple_v=[[0, 0, 0]])
+        w.step(1)
+        fired += [(s,) + e for e in w.events()]
+        if fired:
+            break
+        if s == 9:
+            assert w.get_counters()[2][0] == 0
+    assert len(fired) == 1 and fired[0][0] == 19 and fired[0][2:5] == (19, 1, 0)
+    assert abs(fired[0][5] - ks * s_hi) < 1e-7 and abs(fired[0][6] - kap * fdet) < 1e-9   # 1e-9 armature drift
+
+
+def test_detach_path_A_takes_precedence_when_both_paths_complete_in_one_step():
+    """Reading A14: one flag flip, one event; when the pull path and the tension path complete in the same step the
+    event carries path A's pair (|f_user|, f_detach).  (Perturbation: path B tested first.)"""
+    spec, w, mA, ks, fdet, xh = _apple_on_a_pinned_link(detach_frames_pull=3, detach_frames_tension=3)
+    kap = float(np.float32(1.1))
+    st = 1.3 * kap * fdet / ks
+    w.apply_wrench(1, (0, 0, 0), (0.0, 0.0, -1.5 * fdet))
+    for s in range(3):
+        w.set_state(apple_x=[xh + st * np.array([0.0, 0.0, -1.0])], apple_v=[[0, 0, 0]])
+        assert w.events() == []
+        w.step(1)
+    rc, cA, cB = w.get_counters()
+    assert cA[0] >= 3 and cB[0] >= 3                       # both paths complete in step 2
+    ev = w.events()
+    assert len(ev) == 1 and ev[0][1:4] == (2, 1, 0)
+    assert abs(ev[0][4] - 1.5 * fdet) < 1e-5 and abs(ev[0][5] - fdet) < 1e-9
+    assert w.get_state()["attached"][0] == 0
+
+
+def test_snapped_flag_covers_the_whole_subtree_below_a_ruptured_joint():
+    """PAPER.md:398 "forces off on snapped sub-trees", reading A10: with joint 1 of a 3-link chain ruptured, a wrench
+    on link 2 (BELOW the break, itself intact) leaves b untouched when forces_off_on_snapped = 1 and adds exactly
+    h J^T F when it is 0; a wrench on link 0 (above the break) always acts.
+    (Perturbation this fails on: snapped_i = ruptured_i without the parent's flag.)"""
+    spec = chain_spec(3, 0.9, 0.03, root_quat=quat_axis("y", 70.0))
+    rng = np.random.default_rng(3)
+    q = rng.uniform(-0.1, 0.1, size=6)
+    pt, F = (0.01, -0.02, 0.2), np.array([1.5, -2.0, 0.7])
+    h = float(np.float32(2e-3))
+
+    def rhs(flag, body):
+        w = OracleWorld(spec, Params(forces_off_on_snapped=flag))
+        w.set_state(q=q, ruptured=[0, 1, 0])
+        b0 = w.system()[1]
+        if body is not None:
+            w.apply_wrench(body, pt, F)
+        return w.system()[1] - b0
+
+    assert np.abs(rhs(1, 2)).max() == 0.0
+    ptf = np.asarray(pt, dtype=np.float32).astype(np.float64)
+    for flag, body in ((0, 2), (1, 0), (0, 0)):
+        J = _fd_jacobian(spec, q, body, ptf)
+        db = rhs(flag, body)
+        assert np.abs(db - h * J.T @ F).max() < 1e-7 * np.abs(db).max(), (flag, body)
+
+
+def test_rupture_predicate_reads_the_end_of_step_angle():
+    """SURVEY.md 8(c) steps 6 and 8, reading A8 (Eq. 5 on the configuration the step produced): a single DoF driven
+    so that K |theta| crosses M_max between q and q + h qd+ with N_r = 1.  The event belongs to step 0 and its value is
+    K |q + h qd+| with qd+ from the closed-form 1-DoF step map of the pin above.
+    (Perturbation this fails on: the predicate on the start-of-step q -- event one step late, other value.)"""
+    L, d, rho, E, MOR = 0.6, 0.02, 800.0, 8e9, 60e6
+    spec = chain_spec(1, L, d, density=rho, E=E, MOR=MOR)
+    w = OracleWorld(spec, Params(h=2e-3, gravity=(0, 0, 0), rupture_frames=1, qd_max=0.0))
+    hh, cd = float(np.float32(2e-3)), float(np.float32(0.05))
+    r, Lf = float(spec.diameter[0]) / 2, float(spec.length[0])
+    m = rho * math.pi * r * r * Lf
+    J = m * Lf * Lf / 3 + m * r * r / 4
+    K = E * math.pi * (2 * r) ** 4 / (64 * Lf)
+    Mmax = MOR * math.pi * (2 * r) ** 3 / 32
+    q0, v0 = 0.999 * Mmax / K, 20.0
+    v1 = (J * v0 - hh * K * q0) / (J + hh * cd * K + hh * hh * K)
+    q1 = q0 + hh * v1
+    assert K * q0 < Mmax < K * q1                           # the crossing happens inside step 0
+    w.set_state(q=[0.0, q0], qd=[0.0, v0])
+    w.step(1)
+    ev = w.events()
+    assert len(ev) == 1 and ev[0][1:4] == (0, 0, 0)
+    assert abs(ev[0][4] - K * q1) < 1e-9 * K * q1 and abs(ev[0][5] - Mmax) < 1e-9 * Mmax
+    assert abs(w.get_state()["q"][1] - q1) < 1e-13
+
+
+def test_apple_position_advances_with_the_end_of_step_velocity():
+    """PAPER.md:151 (3-DoF fruit): semi-implicit Euler, v += h a, then x += h v with the NEW v.
+    A detached apple under gravity and a constant pull: x_n = x_0 + h^2 a n (n + 1) / 2 exactly.
+    (Perturbation this fails on: x += h v_old, which gives n (n - 1) / 2 and misses by h^2 a n.)"""
+    mA = 0.25
+    spec = chain_spec(1, 0.5, 0.08, apples=[(0, (0, 0, 0.5), mA, 2e3, 20.0)])
+    w = OracleWorld(spec, Params(h=2e-3))
+    hh = float(np.float32(2e-3))
+    w.set_state(attached=[0])
+    x0 = w.get_state()["apple_x"][0].copy()
+    F = np.asarray(np.float32([0.3, -0.2, 0.9]), dtype=np.float64)
+    w.apply_wrench(1, (0, 0, 0), F)
+    a = np.array([0.0, 0.0, -G]) + F / float(np.float32(mA))
+    n = 25
+    w.step(n)
+    s = w.get_state()
+    assert np.abs(s["apple_v"][0] - hh * a * n).max() < 1e-12
+    assert np.abs(s["apple_x"][0] - (x0 + hh * hh * a * n * (n + 1) / 2)).max() < 1e-12
+    assert np.linalg.norm(hh * hh * a * n) > 1e-4           # the size of the miss of the start-of-step variant
+
+
+def test_tether_damper_acts_on_the_absolute_apple_velocity():
+    """Eq. 6, reading A11: f = -k_s (x - x_hang) - c_s v with v the apple's own (world) velocity.
+    (a) the branch swings (armature keeps qd), the apple is at rest in the world: after one step its velocity is
+    h (g - k_s (x - x_hang) / m), no damper term although the hang point moves at |v_hang| = 0.5 m/s;
+    (b) the branch is at rest, the apple moves: the damper term is -c_s v / m.
+    (Perturbation this fails on: the damper on the velocity relative to the hang point.)"""
+    mA, ks, zeta = 0.2, 2e3, 0.1
+    spec = chain_spec(1, 0.5, 0.08, apples=[(0, (0, 0, 0.5), mA, ks, 1e6)], armature=np.full((1, 2), 1e9, dtype=np.float32))
+    hh = float(np.float32(2e-3))
+    m32, k32 = float(np.float32(mA)), float(np.float32(ks))
+    cs = OracleWorld(spec, Params(zeta_s=zeta)).material()["c"][0]
+    assert abs(cs - 2 * float(np.float32(zeta)) * math.sqrt(k32 * m32)) < 1e-9
+    xh = np.array([0.0, 0.0, 0.5])
+    dx = np.array([0.004, -0.003, -0.006])
+    g = np.array([0.0, 0.0, -G])
+    for qd, v in (([1.0, 0.0], np.zeros(3)), ([0.0, 0.0], np.array([0.3, -0.2, 0.1]))):
+        w = OracleWorld(spec, Params(zeta_s=zeta))
+        w.set_state(qd=qd, apple_x=[xh + dx], apple_v=[v])
+        w.step(1)
+        v1 = w.get_state()["apple_v"][0]
+        assert np.abs(v1 - (v + hh * (g - k32 * dx / m32 - cs * v / m32))).max() < 1e-12, (qd, v1)
+    assert hh * cs * 0.5 / m32 > 1e-3                        # what the relative-velocity variant would add in (a)
