@@ -16,14 +16,19 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "orchard_oracle.c")
-_LIB = os.path.join(_HERE, "liborchard_oracle.so")
+# ORCHARD_ORACLE_SANITIZE=1 (tests/test_sanitizers.py): the same source built with ASan + UBSan into a library of its
+# own; the process must then run under LD_PRELOAD=libasan.so.
+_SANITIZE = os.environ.get("ORCHARD_ORACLE_SANITIZE", "") == "1"
+_LIB = os.path.join(_HERE, "liborchard_oracle_san.so" if _SANITIZE else "liborchard_oracle.so")
 
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (plain C, OpenMP over worlds)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-ffp-contract=off",
-               "-o", _LIB, _SRC, "-lm"]
+        opt = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined",
+               "-fno-omit-frame-pointer"] if _SANITIZE else ["-O2"]
+        cmd = ["gcc"] + opt + ["-std=c11", "-fopenmp", "-fPIC", "-shared", "-ffp-contract=off",
+                               "-o", _LIB, _SRC, "-lm"]
         subprocess.check_call(cmd)
     return _LIB
 

@@ -5,7 +5,7 @@
  * bench.py's cpu_baseline / --impl reference legs may load this file.  It shares
  * no code, header, table or helper with paper_2607_06337_b200/ (the CUDA path)
  * and is written from the paper (/root/reference/PAPER.md, cited as PAPER.md:<line>)
- * plus the readings listed in DESIGN.md ("Readings": A1..A31 of SURVEY.md 8(c), A32, A33).
+ * plus the readings listed in DESIGN.md section 3 (A1..A31 of SURVEY.md 8(c), A32..A37).
  *
  * What it computes, in the paper's order, all in double precision:
  *   - the articulation of PAPER.md:113-117 (Eq. 3): links are rigid cylinders
@@ -221,11 +221,12 @@ static void fk_run(const obo_world *W, const double *q, fk_t *f) {
 /* inverse dynamics: Newton-Euler recursion in world coordinates             */
 /*   tau = M(q) qdd + c(q,qd) - (gravity) - J^T f_ext                        */
 /* ----------------------------------------------------------------------- */
+#define OBO_MAX_APPLES 1024              /* obo_world_new refuses more: ext_t below holds one entry per apple */
 typedef struct {
   int n;
-  int link[OBO_MAX_WRENCH + 1024];
-  double x[OBO_MAX_WRENCH + 1024][3]; /* world application point */
-  double F[OBO_MAX_WRENCH + 1024][3]; /* world force             */
+  int link[OBO_MAX_WRENCH + OBO_MAX_APPLES];
+  double x[OBO_MAX_WRENCH + OBO_MAX_APPLES][3]; /* world application point */
+  double F[OBO_MAX_WRENCH + OBO_MAX_APPLES][3]; /* world force             */
 } ext_t;
 
 static void rnea(const obo_world *W, const double *q, const double *qd, const double *qdd, const double g[3],
@@ -470,7 +471,7 @@ obo_world *obo_world_new(int world_index, int n_links, const int32_t *parent, co
                          float E, float MOR, int n_apples, const int32_t *apple_link, const float *apple_offset,
                          const float *apple_mass, const float *apple_k, const float *apple_c,
                          const float *apple_detach, const obo_params *params) {
-  if (n_links < 1 || n_apples < 0 || n_apples > 1024) return NULL;
+  if (n_links < 1 || n_apples < 0 || n_apples > OBO_MAX_APPLES) return NULL;
   for (int i = 0; i < n_links; i++)
     if ((i == 0 && parent[i] != -1) || (i > 0 && (parent[i] < 0 || parent[i] >= i))) return NULL;
   obo_world *W = (obo_world *)calloc(1, sizeof(obo_world));
@@ -1068,6 +1069,7 @@ void obo_set_solver(obo_world *W, int solver, double tol, int max_iter) {
 }
 int obo_events(obo_world *W, obo_event *buf, int cap) {
   int n = W->n_ev < cap ? W->n_ev : cap;
+  if (n <= 0) return 0;                        /* an empty list has ev == NULL: nothing to copy */
   memcpy(buf, W->ev, sizeof(obo_event) * n);
   memmove(W->ev, W->ev + n, sizeof(obo_event) * (W->n_ev - n));
   W->n_ev -= n;
