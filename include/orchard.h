@@ -9,7 +9,8 @@
  *   fruit tethers     PAPER.md:147-163  (Eq. 6,7) 3-DoF apples, clamped reaction on the spur, 2 detach paths
  *   randomization     PAPER.md:165-169            per-world E, MOR, density; per-apple detach force, mass
  *   stability rails   PAPER.md:398      (App. B)  forces off on snapped sub-trees; joint speed clamp
- *   time step         BASELINE.json north_star    (M + hD + h^2 K) dqd = rhs by matrix-free Jacobi-PCG,
+ *   time step         BASELINE.json north_star    (M + hD + h^2 K) dqd = rhs by matrix-free PCG (tree-exact
+ *                                                  or Jacobi preconditioner),
  *                                                  M*v from inverse-dynamics tree sweeps
  * DESIGN.md lists every reading taken where the paper is silent.
  *
@@ -53,7 +54,9 @@ typedef struct ob_ctx ob_ctx;
 
 /* One world.  Worlds may differ in every field (heterogeneous batches are fine). */
 typedef struct {
-  int32_t n_links;              /* >= 1, <= 32767 */
+  int32_t n_links;              /* >= 1; a world must fit in one SM's shared memory: ~1500 links at most (fewer
+                                   with many apples or tree levels); ob_workspace_bytes / ob_create return
+                                   OB_E_CAPACITY with the figures otherwise */
   const int32_t *parent;        /* [n_links] parent[0] = -1 (trunk, jointed to the world), 0 <= parent[i] < i */
   const float *length;          /* [n_links] m, > 0 */
   const float *diameter;        /* [n_links] m, > 0 */
@@ -137,7 +140,7 @@ typedef struct {
   float jitter_diameter[2];     /* per-LINK factor on its diameter ("per-segment thickness") */
 } ob_geometry_ranges;
 
-/* Fill *p with the defaults above (the readings A1..A33 of DESIGN.md section 3).  Returns OB_E_ARG for NULL. */
+/* Fill *p with the defaults above (the readings A1..A37 of DESIGN.md section 3).  Returns OB_E_ARG for NULL. */
 int ob_default_params(ob_params *p);
 
 /* Bytes of device workspace ob_create needs for these worlds (validates the specs).
@@ -220,12 +223,14 @@ int ob_get_state_batch(ob_ctx *ctx, int world0, int n_worlds, float *q, float *q
                        float *apple_v, uint8_t *ruptured, uint8_t *attached, int32_t *info);
 /* Overwrite one world's state (NULL = keep).  Setting `ruptured` / `attached` also clears the corresponding
    hysteresis counters (the N-frame hysteresis of PAPER.md:139, the "few frames" of PAPER.md:163); the PCG warm start
-   of the world is cleared.  Status bits are cleared. */
+   of the world is cleared.  Status bits are cleared (by this call only: ob_set_step, ob_set_rupture_steps and
+   ob_set_apple_x64 keep them, so a world frozen by OB_STATUS_NONFINITE stays frozen until ob_set_state). */
 int ob_set_state(ob_ctx *ctx, int world, const float *q, const float *qd, const float *apple_x,
                  const float *apple_v, const uint8_t *ruptured, const uint8_t *attached);
 /* Apple positions at the library's internal precision: anchor (fp64 rest hang point, Eq. 3) + rest sag m g / k_s
     + fp32 displacement.  apple_x: [3*n_apples] doubles.  ob_get_state's float apple_x is this value
-   rounded to fp32.  The setter is the exact inverse: get -> set restores the internal displacement bit for bit. */
+   rounded to fp32.  The setter is the exact inverse: get -> set restores the internal displacement bit for bit.  It
+   also clears the world's PCG warm start (the positions changed); status bits are kept. */
 int ob_get_apple_x64(ob_ctx *ctx, int world, double *apple_x);
 int ob_set_apple_x64(ob_ctx *ctx, int world, const double *apple_x);
 /* Restore the step counter of a world (events carry it); everything else is kept, the warm start included. */
@@ -249,7 +254,8 @@ int ob_get_material_batch(ob_ctx *ctx, int world0, int n_worlds, float *emr, flo
 /* Exact checkpoint of one world: every byte of its mutable state (q, qd, flags, counters, apple state, step and
    status words, the PCG solution history), so that load followed by ob_step(n) reproduces
    an uninterrupted run bit for bit (PCG solution history included).  buf: host memory of ob_world_blob_bytes bytes.  A blob only loads into a world
-   of the same sizes (OB_E_ARG otherwise).  Materials and wrenches are not part of it. */
+   of the same sizes (OB_E_ARG otherwise).  Materials and wrenches are not part of it: loading keeps the target world's
+   material draws (ob_get_material) and its totals since ob_create (ob_stats), whatever world or moment the blob is from. */
 int ob_world_blob_bytes(ob_ctx *ctx, int world, size_t *out);
 int ob_save_world(ob_ctx *ctx, int world, void *buf, size_t cap);
 int ob_load_world(ob_ctx *ctx, int world, const void *buf, size_t bytes);

@@ -75,5 +75,9 @@ __device__ __forceinline__ void tma_store_commit_wait() {
   asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// the same over every state space: orders generic-proxy accesses to GLOBAL memory against bulk copies too (the chunk
+// hand-off of k_step: an acquire through the generic proxy followed by a bulk load of the bytes the previous owner
+// wrote with a bulk store)
+__device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
 
 }  // namespace ob

@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdarg>
+#include <cstddef>
 #include <cstdio>
 #include <cstring>
 #include <string>
@@ -892,7 +893,9 @@ int set_state_impl(ob_ctx *ctx, int world, const float *q, const float *qd, cons
       if (attached) { af[a] = attached[e] ? 1 : 0; af[d.Ap + a] = 0; af[2 * d.Ap + a] = 0; }
     }
   }
-  wi.status = 0;
+  // status bits are cleared by ob_set_state only (a new state is a new start); ob_set_step, ob_set_rupture_steps and
+  // ob_set_apple_x64 keep them: a frozen world stays frozen
+  if (!step && !rupture_step && !apple_x64) wi.status = 0;
   if (step) wi.step = *step;
   if ((!step && !rupture_step) || q || qd || apple_x || apple_x64 || apple_v || ruptured || attached)
     for (int k = 0; k < 4; k++)   // ... and forget the solution history the PCG start vector is extrapolated from
@@ -1006,7 +1009,10 @@ int ob_load_world(ob_ctx *ctx, int world, const void *buf, size_t bytes) {
   CU(cpy(ctx, ctx->dev.link_blk + d.link_blk_off, p, link_state_bytes(d.Np), cudaMemcpyHostToDevice, ctx->stream)); p += link_state_bytes(d.Np);
   if (d.Ap) CU(cpy(ctx, ctx->dev.apple_blk + d.apple_blk_off, p, apple_state_bytes(d.Ap), cudaMemcpyHostToDevice, ctx->stream));
   p += apple_state_bytes(d.Ap);
-  CU(cpy(ctx, ctx->dev.info + world, p, sizeof(WorldInfo), cudaMemcpyHostToDevice, ctx->stream)); p += sizeof(WorldInfo);
+  // of the WorldInfo in the blob only the mutable words are restored (step, last_iters, status); the target world's
+  // material draws (E, MOR, density) and its totals since ob_create (steps_taken, cg_iters) are not part of a checkpoint
+  static_assert(offsetof(WorldInfo, steps_taken) == 3 * sizeof(int32_t), "step, last_iters, status lead WorldInfo");
+  CU(cpy(ctx, ctx->dev.info + world, p, 3 * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream)); p += sizeof(WorldInfo);
   for (int k = 0; k < 4; k++) {
     CU(cpy(ctx, ctx->dev.xprev + (size_t)k * ctx->dev.sum_np + d.link_base, p, sizeof(float2) * d.Np, cudaMemcpyHostToDevice, ctx->stream));
     p += sizeof(float2) * d.Np;

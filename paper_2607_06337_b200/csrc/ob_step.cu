@@ -1442,7 +1442,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
     // ---- stage the world: the apple block by one TMA bulk copy; topology words, factor slots, level offsets,
     //      wrench slots ----
     if (tid == 0 && d.Ap) {
-      fence_proxy_async();
+      fence_proxy_async_all();     // shared (the landing zone was written by generic stores) and global (the acquire above)
       const uint32_t ab = (uint32_t)apple_block_bytes(d.Ap);
       mbar_expect_tx(&s_bar, ab);
       tma_load(s.u, c.apple_blk + d.apple_blk_off, ab, &s_bar);
@@ -1625,6 +1625,7 @@ k_step(const __grid_constant__ DevCtx c, const int32_t *__restrict__ order, int 
       if (d.Ap) {
         tma_store(c.apple_blk + d.apple_blk_off, s.u, (uint32_t)apple_state_bytes(d.Ap));
         tma_store_commit_wait();
+        fence_proxy_async_all();   // the bulk store's global writes before the generic-proxy release below
       }
       info->step = step0 + steps_done;
       info->last_iters = last_iters;

@@ -28,6 +28,17 @@ TOL_STEP = 1e-5      # north_star: single step, fp32
 TOL_RUN = 1e-3       # north_star: 200-step trajectory without events
 BIG_N = 1500         # largest world of the heterogeneous edge-case batch: the top of configs[4]'s [100, 1500] range
 NEAR = 1e-4          # north_star: relative margin of a threshold inside which a one-sided event is tolerated
+# Per-element bounds ("Per-element bound"; tests/helpers.py: rel_state_error): the worst ELEMENT of
+# a block against the block's largest meets the same number as the block norm; against its own magnitude (with 1 % of
+# the block's largest as the zero scale) 20x that for a single step and 2x for a run.
+OWN_STEP, OWN_RUN = 20.0, 2.0
+TOL_STEP_SETTLED = 1.5e-5   # reading A38: the speed block of a settled tree, plain A27 norm (measured 1.31e-5)
+
+
+def _within(e, tol):
+    """The A27 block norm AND the two per-element errors of rel_state_error are inside the bound."""
+    own = OWN_STEP if tol <= TOL_STEP else OWN_RUN
+    return e["max"] <= tol and e["max_inf"] <= tol and e["max_own"] <= own * tol
 
 
 # ----------------------------------------------------------------------------------------------------
@@ -154,7 +165,7 @@ def test_single_step_config1_along_the_run():
         _apply(sim, refs, config1_loads(spec, done, 500, 30.0, 5000.0))
         e = _single_step_errors(sim, refs, [0])[0]
         done += 1
-        assert e["max"] <= TOL_STEP, (target, e)
+        assert _within(e, TOL_STEP), (target, e)
     sim.close()
 
 
@@ -171,7 +182,7 @@ def test_single_step_stochastic_worlds_under_wrenches(n_lo, n_hi, apples, h_cfg)
         sim.step(25)
         errs = _single_step_errors(sim, refs, range(len(specs)))
         for w, e in errs.items():
-            assert e["max"] <= TOL_STEP, (epoch, w, specs[w].n_links, e)
+            assert _within(e, TOL_STEP), (epoch, w, specs[w].n_links, e)
             worst = max(worst, e["max"])
         sim.step(24)
     print(f"single-step worst relative error {worst:.2e}")
@@ -210,7 +221,7 @@ def test_single_step_explicit_tether_and_no_preconditioner():
             _apply(sim, refs, config1_loads(spec, 10 * s, 500, 30.0, 400.0))
             sim.step(1)
         e = _single_step_errors(sim, refs, [0])[0]
-        assert e["max"] <= TOL_STEP, (kw, e)
+        assert _within(e, TOL_STEP), (kw, e)
         sim.close()
 
 
@@ -225,7 +236,7 @@ def test_single_step_ternary_lsystem_homogeneous_batch():
         _apply(sim, refs, wrench_process(specs, epoch, 0.0, 60.0))
         sim.step(20)
         for w, e in _single_step_errors(sim, refs, range(len(specs))).items():
-            assert e["max"] <= TOL_STEP, (epoch, w, e)
+            assert _within(e, TOL_STEP), (epoch, w, e)
         sim.step(9)
     sim.close()
 
@@ -241,7 +252,7 @@ def test_single_step_and_free_run_with_mass_proportional_damping():
         _apply(sim, refs, wrench_process(specs, epoch, 0.0, 60.0))
         sim.step(20)
         for w, e in _single_step_errors(sim, refs, range(len(specs))).items():
-            assert e["max"] <= TOL_STEP, (epoch, w, e)
+            assert _within(e, TOL_STEP), (epoch, w, e)
         sim.step(9)
     sim.close()
     spec = binary_tree_config1()
@@ -252,7 +263,7 @@ def test_single_step_and_free_run_with_mass_proportional_damping():
         sim.step(1)
         refs[0].step(1)
     e, g, o = _err(sim, refs[0], 0)
-    assert e["max"] <= TOL_RUN, e
+    assert _within(e, TOL_RUN), e
     sim.close()
 
 
@@ -268,7 +279,7 @@ def test_free_run_200_steps_config1():
         refs[0].step(1)
     e, g, o = _err(sim, refs[0], 0)
     assert not sim.events() and not refs[0].events()
-    assert e["max"] <= TOL_RUN, e
+    assert _within(e, TOL_RUN), e
     sim.close()
 
 
@@ -286,7 +297,7 @@ def test_free_run_200_steps_stochastic(n_lo, n_hi, apples, cfg, count):
         assert not r.events()
         e, g, o = _err(sim, r, w)
         assert g["step"] == 200 and g["status"] == 0
-        assert e["max"] <= TOL_RUN, (w, specs[w].n_links, e)
+        assert _within(e, TOL_RUN), (w, specs[w].n_links, e)
     sim.close()
 
 
@@ -306,7 +317,7 @@ def test_config1_event_sets_match_the_oracle_run(variant, branch_fmax):
         refs[0].step(1)
         if s == 199:
             e, _, _ = _err(sim, refs[0], 0)
-            assert e["max"] <= TOL_RUN, e
+            assert _within(e, TOL_RUN), e
     gev, oev = sim.events(), refs[0].events()
     assert [_key(e) for e in gev] == [_key(e) for e in oev]
     for g, o in zip(gev, oev):
@@ -344,6 +355,7 @@ def _lockstep(sim, refs, specs, n_steps, loads_at, on_step=None, check=None):
     near = 0
     n_events = 0
     errs, errs_rest = [], []
+    worst_elem = [0.0, 0.0]
     derived = [r.derived() for r in refs]
     mats = [r.material() for r in refs]
     for s in range(n_steps):
@@ -368,6 +380,7 @@ def _lockstep(sim, refs, specs, n_steps, loads_at, on_step=None, check=None):
             if g["status"] & ob.OB_STATUS_NONFINITE:
                 raise AssertionError(f"world {w} went non-finite at step {s}")
             errs.append(e["max"])
+            worst_elem[0] = max(worst_elem[0], e["max_inf"]); worst_elem[1] = max(worst_elem[1], e["max_own"])
             if check is not None:
                 check(s, w, e, g, o)
             # the same error without the speeds of ruptured joints (free hinges of gram-scale twigs: joint inertia
@@ -402,16 +415,18 @@ def _lockstep(sim, refs, specs, n_steps, loads_at, on_step=None, check=None):
             assert abs(ge[4] - oe[4]) <= 2e-4 * abs(oe[4]) and abs(ge[5] - oe[5]) <= 1e-6 * abs(oe[5]), (s, ge, oe)
     a = np.sort(np.array(errs))
     dist = dict(median=float(np.median(a)), p90=float(a[int(0.9 * (len(a) - 1))]), p99=float(a[int(0.99 * (len(a) - 1))]), max=float(a[-1]))
-    return dict(near=near, events=n_events, worst_single_step=float(a[-1]), worst_rest=float(max(errs_rest)), dist=dist)
+    return dict(near=near, events=n_events, worst_single_step=float(a[-1]), worst_rest=float(max(errs_rest)), dist=dist,
+                worst_element_vs_block_max=worst_elem[0], worst_element_vs_own_size=worst_elem[1])
 
 
 def _assert_lockstep_bound(res):
-    """north_star: 1e-5 per step.  The factor 10 of round 1 survives only for the joint speeds of ruptured (free-hinge)
-    joints; everything else (every other DoF, q, apples) must meet the bound itself."""
+    """north_star: 1e-5 per step, on every block of every world in every step, the joint speeds of ruptured (free-hinge)
+    joints included (rounds 1-2 allowed those a factor 10)."""
     print("lock-step single-step error distribution:", {k: f"{v:.1e}" for k, v in res["dist"].items()},
           f"worst outside free hinges {res['worst_rest']:.1e}")
     assert res["worst_rest"] <= TOL_STEP, res
-    assert res["worst_single_step"] <= 10 * TOL_STEP, res
+    assert res["worst_single_step"] <= TOL_STEP, res
+    assert res["worst_element_vs_block_max"] <= TOL_STEP and res["worst_element_vs_own_size"] <= OWN_STEP * TOL_STEP, res
 
 
 def test_lockstep_event_sets_cascading_ruptures():
@@ -558,7 +573,7 @@ def test_edge_cases_single_link_no_apples_and_heterogeneous_batch():
     sim.step(10)
     errs = _single_step_errors(sim, refs, range(len(specs)))
     for w, e in errs.items():
-        assert e["max"] <= TOL_STEP, (w, e)
+        assert _within(e, TOL_STEP), (w, e)
     info = sim.launch_info()
     assert info["smem_bytes"] <= 227 * 1024
     sim.close()
@@ -587,6 +602,18 @@ def test_nonfinite_world_is_frozen_and_flagged():
     s = sim.stats()
     assert s["world_steps_total"] == 10 and s["n_flagged"] == 1
     assert sim.get_state(0)["q"].tobytes() == sim.get_state(2)["q"].tobytes()
+    # only ob_set_state unfreezes: the step counter, the rupture steps and the fp64 apple positions leave the status alone
+    sim.set_step(1, 3)
+    sim.set_rupture_steps(1, np.zeros(spec.n_links, np.int32))
+    sim.set_apple_x64(1, sim.get_state(1)["apple_x64"])
+    st = sim.get_state(1)
+    assert st["status"] & ob.OB_STATUS_NONFINITE and st["step"] == 3
+    sim.step(2)
+    assert sim.get_state(1)["step"] == 3                      # still frozen
+    sim.set_state(1, q=g["q"], qd=g["qd"])
+    assert sim.get_state(1)["status"] == 0
+    sim.step(2)
+    assert sim.get_state(1)["step"] == 5 and sim.get_state(1)["status"] == 0
     sim.close()
 
 
@@ -669,7 +696,7 @@ def test_full_size_config4_sampled_worlds_and_invariants():
         assert g["step"] == 20 and g["status"] == 0
         assert gev.get(w, []) == [_key(x) for x in r.events()]
         if not gev.get(w):
-            assert e["max"] <= TOL_RUN, (w, e)
+            assert _within(e, TOL_RUN), (w, e)
             worst = max(worst, e["max"])
     print(f"config 4 full size: 20-step worst relative error on sampled worlds {worst:.2e}; "
           f"mean PCG iterations {st['cg_iters_total'] / st['world_steps_total']:.2f}; launch {sim.launch_info()}")
@@ -738,7 +765,7 @@ def test_size_class_4_world_single_step_and_lockstep_under_heavy_wrench():
     _apply(sim, refs, wrench_process(specs, 0, 400.0, 600.0, seed_offset=5000))
     sim.step(30)
     e = _single_step_errors(sim, refs, [0])[0]
-    assert e["max"] <= TOL_STEP, e
+    assert _within(e, TOL_STEP), e
     sim.events(); refs[0].events()                      # the lock-step below compares the events of its own steps
     res = _lockstep(sim, refs, specs, 6, lambda s: [])
     print("class-4 lock-step:", {k: v for k, v in res.items() if k != "dist"})
@@ -858,6 +885,33 @@ def test_checkpoints_exact_blob_and_public_state_round_trip():
         sim.close()
 
 
+def test_checkpoint_keeps_the_target_worlds_materials_and_totals():
+    """A blob holds the mutable state only (include/orchard.h: "Materials and wrenches are not part of it").  Loading a
+    blob taken BEFORE an ob_randomize must leave the world's current material draws (ob_get_material) and the totals
+    since ob_create (ob_stats) as they are, and restore step / state."""
+    specs = list(_stochastic(83, 90, 150, 10, 3))
+    sim = ob.Orchard(specs, config_params(2))
+    sim.randomize(501)
+    sim.step(20)
+    blob = sim.save_world(1)
+    before = sim.get_state(1)
+    mat_old = sim.get_material(1)
+    sim.randomize(502)                                         # new materials, state reset
+    sim.step(6)
+    mat, tot = sim.get_material(1), sim.stats()
+    assert mat["E"] != mat_old["E"] and mat["density"] != mat_old["density"]
+    sim.load_world(1, blob)
+    mat2, tot2 = sim.get_material(1), sim.stats()
+    for k in mat:
+        assert np.asarray(mat[k]).tobytes() == np.asarray(mat2[k]).tobytes(), k
+    assert tot2 == tot and tot["world_steps_total"] == 3 * 26
+    after = sim.get_state(1)
+    assert after["step"] == 20 and after["q"].tobytes() == before["q"].tobytes() and after["status"] == before["status"]
+    sim.step(1)
+    assert sim.stats()["world_steps_total"] == 3 * 27
+    sim.close()
+
+
 def test_saturation_batch_16384_worlds_invariants_and_sampled_parity():
     """configs[3]'s saturation variant: 16384 worlds (the 4096 geometries four times over, materials by world).  All
     worlds: finite state, step counter, nothing flagged, Philox draws of EVERY world and apple bit-exact (batched
@@ -891,7 +945,7 @@ def test_saturation_batch_16384_worlds_invariants_and_sampled_parity():
         e, g, o = _err(sim, r, w)
         assert gev.get(w, []) == [_key(x) for x in r.events()]
         if not gev.get(w):
-            assert e["max"] <= TOL_RUN, (w, e)
+            assert _within(e, TOL_RUN), (w, e)
     sim.close()
 
 
@@ -959,7 +1013,7 @@ def test_geometry_randomization_matches_the_oracle():
         _apply(sim, refs, wrench_process(specs, epoch, 0.0, 80.0))
         sim.step(20)
         for w, e in _single_step_errors(sim, refs, range(len(specs))).items():
-            assert e["max"] <= TOL_STEP, (epoch, w, e)
+            assert _within(e, TOL_STEP), (epoch, w, e)
             worst = max(worst, e["max"])
         sim.step(9)
     print(f"geometry DR: single-step worst relative error {worst:.2e}")
@@ -1039,13 +1093,13 @@ def test_config2_schedule_settle_then_pulls():
     oracle.step_many(refs, 200)
     for w, r in enumerate(refs):
         e, g, o = _err(sim, r, w)
-        assert e["max"] <= TOL_RUN, (w, e)
+        assert _within(e, TOL_RUN), (w, e)
     sim.step(280)
     oracle.step_many(refs, 280)
     assert not sim.events() and not any(r.events() for r in refs)
     worst = max(_err(sim, r, w)[0]["max"] for w, r in enumerate(refs))
     print(f"config 2: relative state error after 480 free steps {worst:.2e}")
-    assert worst <= 5 * TOL_RUN
+    assert worst <= TOL_RUN                      # the 200-step bound holds over the 480 steps too (measured 1.8e-4)
     pulls = config2_pulls(specs)
     # A settled tree is the one regime where the velocity block cannot meet 1e-5 RELATIVE in fp32: the right-hand side
     # is the difference of the gravity and the spring torque, each rounded at eps K |theta|, and the step divides by
@@ -1053,16 +1107,19 @@ def test_config2_schedule_settle_then_pulls():
     # (DESIGN.md section 5).  Here |qd| ~ 2e-3 rad/s, so the check is: q, x, v within 1e-5, and qd within
     # 1e-5 |qd| + 8 eps |theta|_2 / (c_d + h)  (a handful of roundings of K |theta|-sized quantities per joint).
     eps32, cdh = 2.0 ** -24, float(np.float32(P.c_d)) + float(np.float32(P.h))
-    ratios = []
+    ratios, plain = [], []
 
     def check(s_, w, e, g, o):
         assert max(e["q"], e["apple_x"], e["apple_v"]) <= TOL_STEP, (s_, w, e)
         dq = np.linalg.norm(g["qd"].astype(np.float64) - o["qd"])
         bound = TOL_STEP * max(np.linalg.norm(o["qd"]), 1e-4 * np.sqrt(o["qd"].size)) + 8.0 * eps32 * np.linalg.norm(o["q"]) / cdh
         ratios.append(dq / bound)
+        plain.append(e["qd"])
         assert dq <= bound, (s_, w, dq, bound, e)
+        assert e["qd"] <= TOL_STEP_SETTLED, (s_, w, e)    # reading A38: the plain A27 norm, so that a regression shows
     res = _lockstep(sim, refs, specs, 60, lambda s: pulls if s == 20 else [], check=check)   # steps 480..539, pulls at 500
-    print(f"config 2 lock-step: velocity error / (1e-5 |qd| + fp32 floor): median {np.median(ratios):.2f}, max {max(ratios):.2f}")
+    print(f"config 2 lock-step: velocity error / (1e-5 |qd| + fp32 floor): median {np.median(ratios):.2f}, max {max(ratios):.2f}; "
+          f"plain A27 norm of the speed block: max {max(plain):.2e}")
     mats = [r.material() for r in refs]
     expect = {(w, 502, 1, body - specs[w].n_links) for (w, body, _p, f) in pulls
               if np.linalg.norm(np.float32(f)) > np.float32(mats[w]["detach"][body - specs[w].n_links])}
@@ -1105,5 +1162,5 @@ def test_full_size_config3_sampled_worlds_and_invariants():
         e, g, o = _err(sim, r, w)
         assert gev.get(w, []) == [_key(x) for x in r.events()]
         if not gev.get(w):
-            assert e["max"] <= TOL_RUN, (w, e)
+            assert _within(e, TOL_RUN), (w, e)
     sim.close()
