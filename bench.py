@@ -8,7 +8,7 @@
 
 One bench "step" = one wrench epoch of the whole hot path for every world of the batch: the epoch's wrenches
 (ob_apply_wrench_batch) followed by `substeps` physics steps in one ob_step launch (FK, tether forces, bias,
-Jacobi diagonal, PCG, integration, rupture / detach predicates, event append).  `value` = world-steps/s with
+tree factorisation (the preconditioner), PCG, integration, rupture / detach predicates, event append).  `value` = world-steps/s with
 the inputs resident in HBM (wrench slots already uploaded, timed with CUDA events around the ob_step launches);
 `e2e` = the same through the C ABI with HOST buffers: wrench arrays in, events + per-world counters out, copies
 inside the timed region.  Prints ONE JSON line (rank 0).  DESIGN.md section "Measurement" explains every field.
@@ -139,9 +139,9 @@ def kernel_source_hash() -> str:
 
 def _profiled_traffic(n_worlds: int, substeps: int):
     """DRAM bytes of one k_step launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed ncu --set full
-    capture, profiles/r2_k_step_dram.txt.  PROFILED, not measured in this run: null unless that capture was of a launch
+    capture, profiles/r3_k_step_dram.txt.  PROFILED, not measured in this run: null unless that capture was of a launch
     of this size AND of the kernel sources as they are now (the file carries their hash)."""
-    tp = os.path.join(ROOT, "profiles", "r2_k_step_dram.txt")
+    tp = os.path.join(ROOT, "profiles", "r3_k_step_dram.txt")
     try:
         kv = dict(l.split("=", 1) for l in open(tp).read().split() if "=" in l)
         if int(kv["worlds"]) == n_worlds and int(kv["substeps"]) == substeps and kv["kernel_source_hash"] == kernel_source_hash():
@@ -151,11 +151,20 @@ def _profiled_traffic(n_worlds: int, substeps: int):
     return None
 
 
-def _workload(config: int, n_worlds: int):
+# --post-rupture: the post-rupture model of PAPER.md:141 / 398 switched ON (readings A34-A36; the paper gives "~5x over
+# ~1.5 s" and no magnitudes, these are the values DESIGN.md section 1 row 8(f)1 was measured with)
+POST_RUPTURE = dict(fric_frac=0.02, fric_ramp=5.0, fric_time=1.5, mass_damping=0.5, snap_drag_scale=0.2,
+                    rail_speed=5.0, rail_fade=0.5, rail_brake=50.0, forces_off_on_snapped=0)
+
+
+def _workload(config: int, n_worlds: int, post_rupture: bool = False):
+    import dataclasses
+
     from workloads import config_params, make_config
     base = make_config(config, min(n_worlds, 4096))
     specs = [base[w % len(base)] for w in range(n_worlds)]     # 16384 = the 4096 geometries four times over;
-    return specs, config_params(config)                       # materials still differ per world (Philox by world)
+    P = config_params(config)                                 # materials still differ per world (Philox by world)
+    return specs, (dataclasses.replace(P, **POST_RUPTURE) if post_rupture else P)
 
 
 def _loads_arrays(specs, epoch, f_lo, f_hi):
@@ -178,7 +187,7 @@ def run_cuda(args, rank: int, world_size: int):
     if world_size > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     peaks = _peaks()
-    specs, P = _workload(args.config, args.worlds)
+    specs, P = _workload(args.config, args.worlds, args.post_rupture)
     f_lo, f_hi = (100.0, 600.0) if args.config == 5 else (0.0, 150.0)
     W, S = len(specs), args.substeps
     n_links = sum(s.n_links for s in specs)
@@ -301,6 +310,7 @@ def run_cuda(args, rank: int, world_size: int):
                        "apples_total": n_apples, "cg_tol": P.cg_tol, "replicas": world_size,
                        "geometry": "ob_randomize_geometry: distinct growth habit and dimensions per world"
                                    if args.geometry_dr else "as generated (every world its own tree)",
+                       "post_rupture": POST_RUPTURE if args.post_rupture else "off (BASELINE.json configs do not name it)",
                        "l2": f"inputs exceed L2: workspace {dev['workspace'] / 2**20:.0f} MiB vs 126 MB L2",
                        "launch": dev["launch"]},
             "kernel_only": {"value": ws_dev / (kern_total_ms * 1e-3), "unit": UNIT,
@@ -321,11 +331,11 @@ def run_cuda(args, rank: int, world_size: int):
             "clocks": dev["clocks"],
             "roofline": {"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "TFLOP/s",
                          "frac": alu_ach / alu_peak, "traffic": traffic,
-                         "traffic_source": "profiled (profiles/r2_k_step_dram.txt, same kernel sources and launch size), "
+                         "traffic_source": "profiled (profiles/r3_k_step_dram.txt, same kernel sources and launch size), "
                                            "not measured in this run" if traffic is not None else None,
                          "limiter": "latency, not throughput: a step is a chain of ~70 dependent level turns; ncu "
-                                    "(profiles/r2_k_step_ncu_full.md): issue slots 31 % busy, stall_barrier 3.6 / "
-                                    "no_instruction 1.3 / wait 1.4 per issued instruction",
+                                    "(profiles/r3_k_step_ncu_full.md): issue slots 31 % busy, stall_barrier 3.4 / "
+                                    "wait 1.4 / long_scoreboard 1.0 / no_instruction 0.9 per issued instruction",
                          "kernel": "k_step",
                          "kernel_ms": k_ms, "flop_per_world_step": flop_ws,
                          "peak_source": f"148 SM x 128 fp32 lanes x 2 x {sm_mhz:.0f} MHz (clock sampled in the run)",
@@ -450,7 +460,7 @@ def run_cholesky_comparison(args):
     on such a solver's step rate.  The matrices are random SPD of the right sizes: the time of a dense factorisation
     does not depend on the entries."""
     import torch
-    specs, P = _workload(args.config, args.worlds)
+    specs, P = _workload(args.config, args.worlds, args.post_rupture)
     dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
     groups = {}
     for sp in specs:
@@ -536,6 +546,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cholesky-comparison", action="store_true",
                     help="time the library's batched blocked Cholesky on systems of the batch's sizes (SURVEY.md 8(f) item 4)")
+    ap.add_argument("--post-rupture", action="store_true",
+                    help="post-rupture friction ramp, reduced drag on snapped sub-trees and the three force rails ON "
+                         "(PAPER.md:141, 398; SURVEY.md 8(f) item 1), wrenches kept on snapped links so the rails act")
     ap.add_argument("--geometry-dr", action="store_true",
                     help="per-world geometry randomization on the device before the run (SURVEY.md 8(f) item 3)")
     args = ap.parse_args()

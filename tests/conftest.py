@@ -32,3 +32,15 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+def pytest_terminal_summary(terminalreporter):
+    """Worst per-element errors of the parity comparisons, per test (tests/helpers.py: rel_state_error)."""
+    try:
+        from helpers import WORST_PER_ELEMENT
+    except Exception:  # pragma: no cover
+        return
+    if WORST_PER_ELEMENT:
+        terminalreporter.write_line("per-element parity errors (A27 block norm | worst element vs block max | vs its own size):")
+        for k, v in sorted(WORST_PER_ELEMENT.items()):
+            terminalreporter.write_line(f"  {v['max']:.1e} | {v['max_inf']:.1e} | {v['max_own']:.1e}  {k}")

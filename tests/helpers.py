@@ -68,4 +68,30 @@ def rel_state_error(gpu: dict, ref: dict, x_rest: np.ndarray) -> dict:
             den = max(np.linalg.norm(r), floor * math.sqrt(r.size))
         out[name] = float(np.linalg.norm(g - r) / den)
     out["max"] = max(out.values())
+    # Per-element view of the same comparison (not part of "max", which stays reading A27): a block 2-norm can hide one
+    # badly wrong twig among 800 DoFs.  "<block>_inf" = max_j |d_j| / max(max_j |ref_j|, floor): the worst element
+    # against the block's largest; "<block>_own" = max_j |d_j| / (|ref_j| + 0.01 max_j |ref_j| + floor): the worst
+    # element against ITS OWN magnitude, with 1 % of the block's largest as the scale below which an element counts as
+    # zero.  DESIGN.md section 5 ("Per-element bound") derives the bounds the parity tests put on them.
+    for name, floor in (("q", 1e-6), ("qd", 1e-4), ("apple_x", 1e-6), ("apple_v", 1e-4)):
+        g = np.asarray(gpu[name], dtype=np.float64).ravel()
+        r = np.asarray(ref[name], dtype=np.float64).ravel()
+        if g.size == 0:
+            out[name + "_inf"] = out[name + "_own"] = 0.0
+            continue
+        if name == "apple_x":
+            xr = np.asarray(x_rest, dtype=np.float64).ravel()
+            g, r = g - xr, r - xr
+        top = np.abs(r).max()
+        d = np.abs(g - r)
+        out[name + "_inf"] = float(d.max() / max(top, floor))
+        out[name + "_own"] = float((d / (np.abs(r) + 0.01 * top + floor)).max())
+    out["max_inf"] = max(out[k + "_inf"] for k in ("q", "qd", "apple_x", "apple_v"))
+    out["max_own"] = max(out[k + "_own"] for k in ("q", "qd", "apple_x", "apple_v"))
+    track = WORST_PER_ELEMENT.setdefault(os.environ.get("PYTEST_CURRENT_TEST", "?").split(" ")[0], {"max_inf": 0.0, "max_own": 0.0, "max": 0.0})
+    for k in track:
+        track[k] = max(track[k], out[k])
     return out
+
+
+WORST_PER_ELEMENT: dict = {}     # test id -> worst per-element errors seen (printed by conftest at the end of the session)

@@ -59,9 +59,9 @@ def test_reference_arm_two_ranks_prints_one_line():
 
 
 def test_committed_dram_profile_is_of_the_kernel_sources_as_they_are():
-    """bench.py reports roofline.traffic from profiles/r2_k_step_dram.txt only while that capture is of the CUDA
+    """bench.py reports roofline.traffic from profiles/r3_k_step_dram.txt only while that capture is of the CUDA
     sources at HEAD (the file carries their hash): a stale profile would silently turn the field into null."""
     import bench
     assert bench._profiled_traffic(4096, 50) is not None, (
-        "profiles/r2_k_step_dram.txt is not of the kernel sources as they are (hash %s): re-capture it" % bench.kernel_source_hash())
+        "profiles/r3_k_step_dram.txt is not of the kernel sources as they are (hash %s): re-capture it" % bench.kernel_source_hash())
     assert bench._profiled_traffic(4096, 49) is None
